@@ -1,0 +1,154 @@
+/* moto.h -- C ABI of libmoto.so: the B200-native (sm_100a, fp64) hot path of the bilayer
+ * minimum-mode kernel of arxiv 2509.26269 ("MOTO").  Citations are PAPER.md:<line> of the paper
+ * text and BASELINE.json:north_star; readings A1..A23 are listed in DESIGN.md.
+ *
+ * Conventions (all entry points)
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers; sizes are element counts.
+ *   - Layouts: configuration  m or x : [N][3]   fp64, site/atom-major (Eq. 3)
+ *              block of directions V : [k][N][3] fp64 (V_min = [v_1..v_k])
+ *   - Ownership: the caller owns every array including the workspace; the library allocates no
+ *     device memory (it keeps one small pinned host status buffer per context).
+ *   - All work is enqueued on the CUDA stream given to moto_create.  Calls return after
+ *     enqueueing, except moto_lowest_modes and the *_host variants, which synchronise the stream.
+ *   - Errors: every call returns a moto_status; nothing aborts or throws.  moto_last_error gives
+ *     a message.  MOTO_ENOTCONV still leaves the best iterate and its residuals in the outputs.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns MOTO_ECUDA.
+ */
+#ifndef MOTO_H
+#define MOTO_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MOTO_KMAX 8            /* largest block size k accepted by moto_hvp / moto_lowest_modes */
+#define MOTO_NSMAX (3 * MOTO_KMAX) /* largest Rayleigh-Ritz basis [X,W,P] */
+
+typedef struct moto_ctx moto_ctx; /* opaque */
+
+typedef enum {
+    MOTO_OK = 0,
+    MOTO_EINVAL = 1,   /* bad argument (k out of range, NULL pointer, bad lattice, workspace too small) */
+    MOTO_ENOMEM = 2,   /* host allocation failed / neighbour capacity exceeded */
+    MOTO_ECUDA = 3,    /* a CUDA runtime call failed (message in moto_last_error) */
+    MOTO_ENOTCONV = 4, /* eigen-solver hit max_iter; outputs hold the best iterate */
+    MOTO_ESTATE = 5    /* call not valid for this context kind */
+} moto_status;
+
+enum { MOTO_KIND_TRI2D = 0, MOTO_KIND_CARTESIAN = 1 };
+
+/* Lattice / atom container.
+ * kind 0: 2-D triangular spin lattice, site i = iy*Lx + ix at r_i = ix*a1 + iy*a2, a1=(1,0),
+ *         a2=(1/2,sqrt3/2); six neighbours at offsets (+-1,0),(0,+-1),(-1,+1),(+1,-1); pbc_x/pbc_y
+ *         select periodic (1) or open (0) boundaries (open: the missing neighbour contributes 0).
+ * kind 1: n_atoms Cartesian atoms, periodic in the in-plane cell spanned by the rows of cell
+ *         (Angstrom), open in z.  d_fixed: optional device mask [N], 1 = frozen (the paper's mask
+ *         Omega); NULL = all free.  Ignored for kind 0. */
+typedef struct {
+    int32_t kind;
+    int32_t Lx, Ly;
+    int32_t pbc_x, pbc_y;
+    int32_t n_atoms;
+    double cell[2][2];
+    const uint8_t* d_fixed;
+} moto_lattice;
+
+/* Eq. 4, nearest neighbours only: exchange J, interfacial DMI
+ * D_ij = D (z x rhat_ij) with rhat_ij = r_j - r_i, easy axis z with strength K, field B, moment mu.
+ * The pair sums run over ORDERED pairs i != j exactly as printed (reading A1). */
+typedef struct { double J, D, K, B[3], mu; } moto_spin_params;
+
+/* Morse pair potential phi(r) = De[exp(-2 alpha (r-r0)) - 2 exp(-alpha (r-r0))], r < rc
+ * (BASELINE.json configs[4]); energy shifted by -phi(rc) per pair (reading A21). */
+typedef struct { double De, alpha, r0, rc; } moto_morse_params;
+
+/* Eigen-solver knobs (PAPER.md:120 names Krylov depth / reorthogonalisation as the sensitive ones).
+ * Zero-initialise and pass to moto_set_solver to change the defaults given in brackets. */
+typedef struct {
+    int32_t guard;          /* extra block columns iterated but not returned            [0]  */
+    int32_t check_every;    /* iterations enqueued between host looks at the status     [8]  */
+    int32_t precond_degree; /* degree of the Chebyshev polynomial preconditioner, 0=off [0]  */
+    int32_t reserved;
+    double precond_lo;      /* preconditioner interval [lo, hi] in units of the shift   [auto] */
+    double precond_hi;
+    uint64_t seed;          /* seed of the counter-based start block when warm_start=0  [0x9E3779B97F4A7C15] */
+} moto_solver_opts;
+
+typedef struct {
+    int32_t iters;              /* LOBPCG iterations executed */
+    int32_t converged;          /* 1 if every returned column met tol */
+    double resid[MOTO_KMAX];    /* ||Hess v_j - lambda_j v_j||_2 of the returned columns */
+    int64_t hvp_count;          /* single-vector HVP applications (k per block HVP) */
+} moto_solve_info;
+
+/* Bytes of device workspace moto_create needs for block sizes up to kmax (<= MOTO_KMAX, guard included). */
+size_t moto_workspace_bytes(const moto_lattice* lat, int kmax);
+
+/* Build a context.  params: moto_spin_params* (kind 0) or moto_morse_params* (kind 1), copied.
+ * d_workspace: device buffer of >= moto_workspace_bytes bytes, 256-byte aligned, owned by the
+ * caller and alive until moto_destroy.  cuda_stream: a cudaStream_t (NULL = default stream). */
+moto_status moto_create(const moto_lattice* lat, const void* params, void* d_workspace, size_t ws_bytes,
+                        void* cuda_stream, int kmax, moto_ctx** out);
+void moto_destroy(moto_ctx* ctx);
+moto_status moto_set_solver(moto_ctx* ctx, const moto_solver_opts* opts);
+const char* moto_last_error(const moto_ctx* ctx);
+
+/* E(m) and its gradient.  d_E: [1] device.  d_g: [N][3] device, may be NULL.
+ * kind 0: d_g = tangent-projected gradient P g = g - (m.g) m ("forces ... understood as
+ *         tangent-projected").   kind 1: Euclidean gradient, rows of fixed atoms zero. */
+moto_status moto_energy_grad(moto_ctx* ctx, const double* d_spins, double* d_E, double* d_g);
+
+/* Block Hessian-vector product (north_star): for each column a,
+ * kind 0: HV_a = P (L Pv_a) - (m.g) Pv_a   (input projected, output tangent, reading A5)
+ * kind 1: HV_a = M H M v_a, M = mask of free atoms.   d_V, d_HV: [k][N][3]; must not alias. */
+moto_status moto_hvp(moto_ctx* ctx, const double* d_spins, const double* d_V, int k, double* d_HV);
+
+/* Smallest-k eigenpairs of the (masked) tangent Hessian by device-resident block LOBPCG
+ * (ref [27]).  Stops when every ||Hess v_j - lambda_j v_j||_2 <= tol
+ * (absolute, ||v_j|| = 1; reading A9) or after max_iter iterations (paper's cap: 200).
+ * warm_start = 1: d_V holds a start block (any full-rank block; it is projected and orthonormalised).
+ * Outputs: d_lambda [k] ascending; d_V [k][N][3] tangent, orthonormal, sign-normalised so the
+ * largest-|component| entry of each column is positive; info (host) may be NULL. */
+moto_status moto_lowest_modes(moto_ctx* ctx, const double* d_spins, int k, double tol, int max_iter,
+                              int warm_start, double* d_lambda, double* d_V, moto_solve_info* info);
+
+/* One reflected-force step (Eq. 2; Alg. 1 l.11-12):
+ * F = -grad (tangent-projected / masked), F_mmf = F - 2 sum_a (F.v_a) v_a over the kr columns given,
+ * kind 0: m' = normalize(m + dt F_mmf) per site (retraction);  kind 1: x' = x + dt F_mmf.
+ * d_spins_out may alias d_spins.  d_fnorm: optional [1] device, receives ||F_mmf||_2. */
+moto_status moto_mmf_step(moto_ctx* ctx, const double* d_spins, const double* d_v, int kr, double dt,
+                          double* d_spins_out, double* d_fnorm);
+
+/* Vector transport for warm starts after m -> m' (reading A17): V <- orthonormalise(P_{m'} V), in place. */
+moto_status moto_transport(moto_ctx* ctx, const double* d_spins_new, double* d_V, int k);
+
+/* Building blocks of the LOBPCG iteration, exported so they can be tested alone.
+ * moto_gram: G[i][j] = S_i . T_j for block vectors S [ns][N][3], T [nt][N][3]; d_G [ns][nt] row-major.
+ * moto_rayleigh_ritz: lowest nev pairs of G_A c = theta G_B c (n <= MOTO_NSMAX, row-major symmetric,
+ *   G_B positive semi-definite: near-null directions are dropped); d_theta [nev], d_C [n][nev] with
+ *   C^T G_B C = I.  Single CTA, Jacobi; nothing leaves the GPU. */
+moto_status moto_gram(moto_ctx* ctx, const double* d_S, int ns, const double* d_T, int nt, double* d_G);
+moto_status moto_rayleigh_ritz(moto_ctx* ctx, const double* d_GA, const double* d_GB, int n, int nev,
+                               double* d_theta, double* d_C);
+
+/* Host-buffer variants (end-to-end path): same semantics, all array arguments are HOST pointers
+ * (pinned or pageable); the library stages them through its workspace (host->device, compute,
+ * device->host) and synchronises the stream before returning. */
+moto_status moto_energy_grad_host(moto_ctx* ctx, const double* h_spins, double* h_E, double* h_g);
+moto_status moto_hvp_host(moto_ctx* ctx, const double* h_spins, const double* h_V, int k, double* h_HV);
+moto_status moto_lowest_modes_host(moto_ctx* ctx, const double* h_spins, int k, double tol, int max_iter,
+                                   int warm_start, double* h_lambda, double* h_V, moto_solve_info* info);
+moto_status moto_mmf_step_host(moto_ctx* ctx, const double* h_spins, const double* h_v, int kr, double dt,
+                               double* h_spins_out, double* h_fnorm);
+
+/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+int64_t moto_launch_count(const moto_ctx* ctx);
+const char* moto_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MOTO_H */

@@ -1,0 +1,282 @@
+"""Thin ctypes binding over libmoto.so (include/moto.h): argument marshalling only.
+
+torch is used for device memory and the CUDA stream handle; every step of the path runs inside the
+library's kernels.  There is no CPU fallback: if the library is missing or no CUDA device is
+present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+KMAX = 8
+NSMAX = 24
+OK, EINVAL, ENOMEM, ECUDA, ENOTCONV, ESTATE = range(6)
+KIND_TRI2D, KIND_CARTESIAN = 0, 1
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmoto.so")
+_lib = None
+
+
+class MotoError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"moto status {status}: {msg}")
+        self.status = status
+
+
+class Lattice(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("Lx", C.c_int32), ("Ly", C.c_int32), ("pbc_x", C.c_int32), ("pbc_y", C.c_int32),
+                ("n_atoms", C.c_int32), ("cell", (C.c_double * 2) * 2), ("d_fixed", C.c_void_p)]
+
+
+class SpinParams(C.Structure):
+    _fields_ = [("J", C.c_double), ("D", C.c_double), ("K", C.c_double), ("B", C.c_double * 3), ("mu", C.c_double)]
+
+
+class MorseParams(C.Structure):
+    _fields_ = [("De", C.c_double), ("alpha", C.c_double), ("r0", C.c_double), ("rc", C.c_double)]
+
+
+class SolverOpts(C.Structure):
+    _fields_ = [("guard", C.c_int32), ("check_every", C.c_int32), ("precond_degree", C.c_int32), ("reserved", C.c_int32),
+                ("precond_lo", C.c_double), ("precond_hi", C.c_double), ("seed", C.c_uint64)]
+
+
+class SolveInfo(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("converged", C.c_int32), ("resid", C.c_double * KMAX), ("hvp_count", C.c_int64)]
+
+
+_SIGS = {
+    "moto_version": (C.c_char_p, []),
+    "moto_workspace_bytes": (C.c_size_t, [C.POINTER(Lattice), C.c_int]),
+    "moto_create": (C.c_int, [C.POINTER(Lattice), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p, C.c_int,
+                              C.POINTER(C.c_void_p)]),
+    "moto_destroy": (None, [C.c_void_p]),
+    "moto_set_solver": (C.c_int, [C.c_void_p, C.POINTER(SolverOpts)]),
+    "moto_last_error": (C.c_char_p, [C.c_void_p]),
+    "moto_energy_grad": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "moto_hvp": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
+    "moto_lowest_modes": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
+                                    C.POINTER(SolveInfo)]),
+    "moto_mmf_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p, C.c_void_p]),
+    "moto_transport": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
+    "moto_gram": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
+    "moto_rayleigh_ritz": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
+    "moto_energy_grad_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "moto_hvp_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
+    "moto_lowest_modes_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_int, C.c_void_p,
+                                         C.c_void_p, C.POINTER(SolveInfo)]),
+    "moto_mmf_step_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p, C.c_void_p]),
+    "moto_launch_count": (C.c_int64, [C.c_void_p]),
+}
+EXPORTS = tuple(_SIGS)
+
+
+def load_library(path: str | None = None):
+    """dlopen libmoto.so and set the prototypes.  Raises (never falls back) if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} not found: build it with `python -m paper_2509_26269_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(path)
+    for name, (res, args) in _SIGS.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+def _ptr(t):
+    """Device/host address of a torch tensor or numpy array (None -> NULL)."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        assert t.dtype == np.float64 and t.flags.c_contiguous
+        return t.ctypes.data
+    assert t.is_contiguous()
+    return t.data_ptr()
+
+
+def _dev_f64(t, shape=None):
+    import torch
+    assert isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous(), \
+        "expected a contiguous CUDA float64 tensor"
+    if shape is not None:
+        assert tuple(t.shape) == tuple(shape), f"shape {tuple(t.shape)} != {tuple(shape)}"
+    return t
+
+
+class Context:
+    """A moto_ctx plus the torch-owned workspace it points into."""
+
+    def __init__(self, lattice: Lattice, params, kmax: int = 2, device="cuda:0", stream=None, fixed=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("moto: no CUDA device (there is no CPU fallback)")
+        self.lib = load_library()
+        self.device = torch.device(device)
+        self.kmax = int(kmax)
+        self._fixed = None
+        if fixed is not None:
+            self._fixed = torch.as_tensor(np.asarray(fixed, dtype=np.uint8)).to(self.device).contiguous()
+            lattice.d_fixed = self._fixed.data_ptr()
+        self.lattice = lattice
+        self.params = params
+        self.N = lattice.Lx * lattice.Ly if lattice.kind == KIND_TRI2D else lattice.n_atoms
+        nbytes = self.lib.moto_workspace_bytes(C.byref(lattice), self.kmax)
+        if nbytes == 0:
+            raise MotoError(EINVAL, "bad lattice or kmax")
+        self.workspace_bytes = int(nbytes)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            self._ws_ptr = (base + 255) & ~255
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = C.c_void_p()
+            st = self.lib.moto_create(C.byref(lattice), C.addressof(params), self._ws_ptr, nbytes,
+                                      self.stream.cuda_stream, self.kmax, C.byref(h))
+        if st != OK:
+            raise MotoError(st, "moto_create failed")
+        self._h = h
+
+    # -- helpers
+    def _check(self, st, allow=()):
+        if st != OK and st not in allow:
+            raise MotoError(st, self.lib.moto_last_error(self._h).decode())
+        return st
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.moto_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_solver(self, guard=0, check_every=8, precond_degree=0, precond_lo=0.0, precond_hi=0.0, seed=0):
+        o = SolverOpts(guard, check_every, precond_degree, 0, precond_lo, precond_hi, seed)
+        self._check(self.lib.moto_set_solver(self._h, C.byref(o)))
+
+    @property
+    def launch_count(self) -> int:
+        return int(self.lib.moto_launch_count(self._h))
+
+    def _empty(self, *shape):
+        import torch
+        return torch.empty(*shape, dtype=torch.float64, device=self.device)
+
+    # -- device-pointer API (names follow include/moto.h)
+    def energy_grad(self, spins, want_grad=True):
+        """moto_energy_grad -> (E [1] device tensor, g [N][3] device tensor or None)."""
+        _dev_f64(spins, (self.N, 3))
+        E = self._empty(1)
+        g = self._empty(self.N, 3) if want_grad else None
+        self._check(self.lib.moto_energy_grad(self._h, _ptr(spins), _ptr(E), _ptr(g)))
+        return E, g
+
+    def hvp(self, spins, V, out=None):
+        """moto_hvp: V [k][N][3] -> HV [k][N][3]."""
+        _dev_f64(spins, (self.N, 3))
+        k = V.shape[0]
+        _dev_f64(V, (k, self.N, 3))
+        HV = out if out is not None else self._empty(k, self.N, 3)
+        self._check(self.lib.moto_hvp(self._h, _ptr(spins), _ptr(V), k, _ptr(HV)))
+        return HV
+
+    def lowest_modes(self, spins, k, tol, max_iter=200, V0=None, allow_notconv=False):
+        """moto_lowest_modes -> (lam [k], V [k][N][3], info dict)."""
+        _dev_f64(spins, (self.N, 3))
+        lam = self._empty(k)
+        if V0 is not None:
+            V = _dev_f64(V0, (k, self.N, 3)).clone()
+            warm = 1
+        else:
+            V = self._empty(k, self.N, 3)
+            warm = 0
+        info = SolveInfo()
+        st = self._check(self.lib.moto_lowest_modes(self._h, _ptr(spins), k, float(tol), int(max_iter), warm, _ptr(lam),
+                                                    _ptr(V), C.byref(info)), allow=(ENOTCONV,) if allow_notconv else ())
+        return lam, V, dict(iters=info.iters, converged=bool(info.converged), resid=list(info.resid)[:k],
+                            hvp_count=info.hvp_count, status=st)
+
+    def mmf_step(self, spins, v, dt, out=None, want_fnorm=True):
+        """moto_mmf_step -> (spins', |F_mmf| [1] device tensor or None)."""
+        _dev_f64(spins, (self.N, 3))
+        kr = v.shape[0]
+        _dev_f64(v, (kr, self.N, 3))
+        out = out if out is not None else self._empty(self.N, 3)
+        fn = self._empty(1) if want_fnorm else None
+        self._check(self.lib.moto_mmf_step(self._h, _ptr(spins), _ptr(v), kr, float(dt), _ptr(out), _ptr(fn)))
+        return out, fn
+
+    def transport(self, spins_new, V):
+        k = V.shape[0]
+        _dev_f64(V, (k, self.N, 3))
+        self._check(self.lib.moto_transport(self._h, _ptr(spins_new), _ptr(V), k))
+        return V
+
+    def gram(self, S, T):
+        ns, nt = S.shape[0], T.shape[0]
+        _dev_f64(S, (ns, self.N, 3)); _dev_f64(T, (nt, self.N, 3))
+        G = self._empty(ns, nt)
+        self._check(self.lib.moto_gram(self._h, _ptr(S), ns, _ptr(T), nt, _ptr(G)))
+        return G
+
+    def rayleigh_ritz(self, GA, GB, nev):
+        n = GA.shape[0]
+        _dev_f64(GA, (n, n)); _dev_f64(GB, (n, n))
+        theta = self._empty(nev)
+        Cm = self._empty(n, nev)
+        self._check(self.lib.moto_rayleigh_ritz(self._h, _ptr(GA), _ptr(GB), n, nev, _ptr(theta), _ptr(Cm)))
+        return theta, Cm
+
+    # -- host-buffer API (numpy arrays, pinned or pageable)
+    def energy_grad_host(self, h_spins, h_g=None):
+        E = np.zeros(1)
+        self._check(self.lib.moto_energy_grad_host(self._h, _ptr(h_spins), _ptr(E), _ptr(h_g)))
+        return float(E[0]), h_g
+
+    def hvp_host(self, h_spins, h_V, h_HV):
+        self._check(self.lib.moto_hvp_host(self._h, _ptr(h_spins), _ptr(h_V), h_V.shape[0], _ptr(h_HV)))
+        return h_HV
+
+    def lowest_modes_host(self, h_spins, k, tol, max_iter, h_lam, h_V, warm=False, allow_notconv=False):
+        info = SolveInfo()
+        st = self._check(self.lib.moto_lowest_modes_host(self._h, _ptr(h_spins), k, float(tol), int(max_iter), int(warm),
+                                                         _ptr(h_lam), _ptr(h_V), C.byref(info)),
+                         allow=(ENOTCONV,) if allow_notconv else ())
+        return dict(iters=info.iters, converged=bool(info.converged), resid=list(info.resid)[:k],
+                    hvp_count=info.hvp_count, status=st)
+
+    def mmf_step_host(self, h_spins, h_v, dt, h_out):
+        fn = np.zeros(1)
+        self._check(self.lib.moto_mmf_step_host(self._h, _ptr(h_spins), _ptr(h_v), h_v.shape[0], float(dt), _ptr(h_out),
+                                                _ptr(fn)))
+        return h_out, float(fn[0])
+
+
+def spin_context(w, kmax=None, device="cuda:0", stream=None) -> Context:
+    """Context for a workloads.SpinWorkload."""
+    lat = Lattice(KIND_TRI2D, w.Lx, w.Ly, w.pbc_x, w.pbc_y, 0)
+    p = SpinParams(w.J, w.D, w.K, (C.c_double * 3)(*w.B), w.mu)
+    return Context(lat, p, kmax=kmax or w.k, device=device, stream=stream)
+
+
+def cart_context(w, kmax=None, device="cuda:0", stream=None) -> Context:
+    """Context for a workloads.CartWorkload."""
+    lat = Lattice(KIND_CARTESIAN, 0, 0, 1, 1, w.Na)
+    for a in range(2):
+        for b in range(2):
+            lat.cell[a][b] = float(w.cell[a][b])
+    p = MorseParams(w.De, w.alpha, w.r0, w.rc)
+    return Context(lat, p, kmax=kmax or w.k, device=device, stream=stream, fixed=w.fixed)

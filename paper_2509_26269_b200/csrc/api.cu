@@ -1,0 +1,278 @@
+// api.cu -- the C ABI of libmoto.so (include/moto.h): argument checks, workspace carving, dispatch.
+#include <new>
+#include "common.cuh"
+
+static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static int lattice_sites(const moto_lattice* lat) {
+    return lat->kind == MOTO_KIND_TRI2D ? lat->Lx * lat->Ly : lat->n_atoms;
+}
+
+static bool lattice_ok(const moto_lattice* lat) {
+    if (!lat) return false;
+    if (lat->kind == MOTO_KIND_TRI2D) return lat->Lx >= 1 && lat->Ly >= 1 && (long long)lat->Lx * lat->Ly < (1ll << 30);
+    if (lat->kind == MOTO_KIND_CARTESIAN) return lat->n_atoms >= 1;
+    return false;
+}
+
+struct WsLayout { size_t block, c, g, stage, partials, st, cart, total; };
+
+static WsLayout ws_layout(const moto_lattice* lat, int kmax) {
+    WsLayout w;
+    size_t N = (size_t)lattice_sites(lat);
+    w.block = al256((size_t)kmax * N * 3 * sizeof(double));
+    w.c = al256(N * sizeof(double));
+    w.g = al256(N * 3 * sizeof(double));
+    w.stage = al256(N * 3 * sizeof(double));
+    w.partials = al256((size_t)MOTO_RED_BLOCKS * 2 * MOTO_NS * MOTO_NS * sizeof(double));
+    w.st = al256(sizeof(SolverState));
+    w.cart = lat->kind == MOTO_KIND_CARTESIAN ? cart_lists_bytes(lat) : 0;
+    w.total = 6 * w.block + w.c + w.g + w.stage + w.partials + w.st + w.cart;
+    return w;
+}
+
+extern "C" {
+
+const char* moto_version(void) { return "moto-b200 0.1 (sm_100a, fp64)"; }
+
+size_t moto_workspace_bytes(const moto_lattice* lat, int kmax) {
+    if (!lattice_ok(lat) || kmax < 1 || kmax > MOTO_KMAX) return 0;
+    return ws_layout(lat, kmax).total;
+}
+
+moto_status moto_create(const moto_lattice* lat, const void* params, void* d_workspace, size_t ws_bytes, void* cuda_stream,
+                        int kmax, moto_ctx** out) {
+    if (!out) return MOTO_EINVAL;
+    *out = nullptr;
+    if (!lattice_ok(lat) || !params || !d_workspace || kmax < 1 || kmax > MOTO_KMAX) return MOTO_EINVAL;
+    if (((uintptr_t)d_workspace & 255) != 0) return MOTO_EINVAL;
+    WsLayout w = ws_layout(lat, kmax);
+    if (ws_bytes < w.total) return MOTO_EINVAL;
+    moto_ctx* c = new (std::nothrow) moto_ctx;
+    if (!c) return MOTO_ENOMEM;
+    memset(c, 0, sizeof(*c));
+    c->lat = *lat;
+    c->kind = lat->kind;
+    c->N = lattice_sites(lat);
+    c->kmax = kmax;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->ws = (char*)d_workspace;
+    c->ws_bytes = ws_bytes;
+    c->opts.check_every = 8;
+    c->opts.seed = 0x9E3779B97F4A7C15ull;
+    if (c->kind == MOTO_KIND_TRI2D) {
+        c->sp = *(const moto_spin_params*)params;
+        c->lat.d_fixed = nullptr;
+    } else {
+        c->mp = *(const moto_morse_params*)params;
+        if (!(c->mp.rc > 0) || !cart_geometry_ok(lat, c->mp.rc)) { delete c; return MOTO_EINVAL; }
+    }
+    char* p = c->ws;
+    c->X = (double*)p; p += w.block;  c->AX = (double*)p; p += w.block;
+    c->W = (double*)p; p += w.block;  c->AW = (double*)p; p += w.block;
+    c->P = (double*)p; p += w.block;  c->AP = (double*)p; p += w.block;
+    c->c = (double*)p; p += w.c;
+    c->g = (double*)p; p += w.g;
+    c->stage_m = (double*)p; p += w.stage;
+    c->partials = (double*)p; p += w.partials;
+    c->st = (SolverState*)p; p += w.st;
+    if (c->kind == MOTO_KIND_CARTESIAN) cart_lists_carve(c, p);
+    cudaError_t e = cudaHostAlloc((void**)&c->hstat, 2 * sizeof(HostStatus), cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+        if (c->hstat) cudaFreeHost(c->hstat);
+        delete c;
+        return MOTO_ECUDA;
+    }
+    *out = c;
+    return MOTO_OK;
+}
+
+void moto_destroy(moto_ctx* c) {
+    if (!c) return;
+    if (c->ev[0]) cudaEventDestroy(c->ev[0]);
+    if (c->ev[1]) cudaEventDestroy(c->ev[1]);
+    if (c->hstat) cudaFreeHost(c->hstat);
+    delete c;
+}
+
+moto_status moto_set_solver(moto_ctx* c, const moto_solver_opts* o) {
+    if (!c || !o) return MOTO_EINVAL;
+    if (o->guard < 0 || o->check_every < 0 || o->precond_degree < 0) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: negative option");
+    moto_solver_opts n = *o;
+    if (n.check_every == 0) n.check_every = 8;
+    if (n.seed == 0) n.seed = 0x9E3779B97F4A7C15ull;
+    c->opts = n;
+    return MOTO_OK;
+}
+
+const char* moto_last_error(const moto_ctx* c) { return c ? c->err : "null context"; }
+int64_t moto_launch_count(const moto_ctx* c) { return c ? c->launches : 0; }
+
+moto_status moto_energy_grad(moto_ctx* c, const double* d_spins, double* d_E, double* d_g) {
+    if (!c || !d_spins || (!d_E && !d_g)) return c ? moto_fail(c, MOTO_EINVAL, "moto_energy_grad: null argument") : MOTO_EINVAL;
+    if (c->kind == MOTO_KIND_TRI2D) c->launches += spin_energy_grad(c, d_spins, d_E, d_g, nullptr);
+    else { c->launches += cart_build_lists(c, d_spins); c->launches += cart_energy_grad(c, d_spins, d_E, d_g); }
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return MOTO_OK;
+}
+
+moto_status moto_hvp(moto_ctx* c, const double* d_spins, const double* d_V, int k, double* d_HV) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_spins || !d_V || !d_HV || d_V == d_HV) return moto_fail(c, MOTO_EINVAL, "moto_hvp: null or aliased argument");
+    if (k < 1 || k > MOTO_KMAX) return moto_fail(c, MOTO_EINVAL, "moto_hvp: k out of range [1, MOTO_KMAX]");
+    if (c->kind == MOTO_KIND_TRI2D) c->launches += spin_hvp(c, d_spins, nullptr, d_V, k, d_HV, 1, nullptr);
+    else { c->launches += cart_build_lists(c, d_spins); c->launches += cart_hvp(c, d_V, k, d_HV, nullptr); }
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return MOTO_OK;
+}
+
+static moto_status check_overflow(moto_ctx* c) {
+    if (c->kind != MOTO_KIND_CARTESIAN) return MOTO_OK;
+    int ov = 0;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&ov, c->cl.overflow, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (ov) return moto_fail(c, MOTO_ENOMEM, "neighbour capacity MOTO_MAX_NEIGH exceeded");
+    return MOTO_OK;
+}
+
+// solve with the start block already in ctx->X (if warm_start); results left in ctx->X / st->theta
+static moto_status solve_internal(moto_ctx* c, const double* d_spins, int k, double tol, int max_iter, int warm_start,
+                                  moto_solve_info* info) {
+    moto_status s = lobpcg_solve(c, d_spins, k, tol, max_iter, warm_start, info);
+    if (s != MOTO_OK && s != MOTO_ENOTCONV) return s;
+    moto_status s2 = check_overflow(c);
+    if (s2 != MOTO_OK) return s2;
+    c->launches += block_sign_normalise(c, c->X, k);
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return s;
+}
+
+moto_status moto_lowest_modes(moto_ctx* c, const double* d_spins, int k, double tol, int max_iter, int warm_start,
+                              double* d_lambda, double* d_V, moto_solve_info* info) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_spins || !d_lambda || !d_V) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes: null argument");
+    if (k < 1 || k > c->kmax) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes: k out of range [1, kmax]");
+    if (!(tol > 0) || max_iter < 0) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes: tol must be > 0, max_iter >= 0");
+    const size_t bytes = (size_t)k * c->N * 3 * sizeof(double);
+    if (warm_start) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->X, d_V, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    moto_status s = solve_internal(c, d_spins, k, tol, max_iter, warm_start, info);
+    if (s != MOTO_OK && s != MOTO_ENOTCONV) return s;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_V, c->X, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_lambda, c->st->theta, k * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return s;
+}
+
+moto_status moto_mmf_step(moto_ctx* c, const double* d_spins, const double* d_v, int kr, double dt, double* d_out, double* d_fnorm) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_spins || !d_v || !d_out) return moto_fail(c, MOTO_EINVAL, "moto_mmf_step: null argument");
+    if (kr < 1 || kr > MOTO_KMAX) return moto_fail(c, MOTO_EINVAL, "moto_mmf_step: kr out of range");
+    if (c->kind == MOTO_KIND_TRI2D) c->launches += spin_mmf_step(c, d_spins, d_v, kr, dt, d_out, d_fnorm);
+    else { c->launches += cart_build_lists(c, d_spins); c->launches += cart_mmf_step(c, d_spins, d_v, kr, dt, d_out, d_fnorm); }
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return MOTO_OK;
+}
+
+moto_status moto_transport(moto_ctx* c, const double* d_spins_new, double* d_V, int k) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_spins_new || !d_V || k < 1 || k > MOTO_KMAX) return moto_fail(c, MOTO_EINVAL, "moto_transport: bad argument");
+    const size_t bs = (size_t)3 * c->N;
+    int n = 0;
+    if (c->kind == MOTO_KIND_TRI2D) n += spin_project(c, d_spins_new, d_V, k);
+    else n += cart_mask(c, d_V, k);
+    const double* S[MOTO_KMAX];
+    for (int a = 0; a < k; ++a) S[a] = d_V + a * bs;
+    n += block_gram(c, S, k, S, k, c->st->GB, nullptr);
+    n += rr_solve(c, nullptr, c->st->GB, k, k, c->st->theta, c->st->C, /*mode=*/1, nullptr);
+    n += block_apply_coeffs(c, d_V, k, c->st->C, nullptr);
+    c->launches += n;
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return MOTO_OK;
+}
+
+moto_status moto_gram(moto_ctx* c, const double* d_S, int ns, const double* d_T, int nt, double* d_G) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_S || !d_T || !d_G || ns < 1 || nt < 1 || ns > MOTO_NS || nt > 2 * MOTO_NS) return moto_fail(c, MOTO_EINVAL, "moto_gram: bad argument");
+    const size_t bs = (size_t)3 * c->N;
+    const double* S[MOTO_NS]; const double* T[2 * MOTO_NS];
+    for (int i = 0; i < ns; ++i) S[i] = d_S + i * bs;
+    for (int j = 0; j < nt; ++j) T[j] = d_T + j * bs;
+    c->launches += block_gram(c, S, ns, T, nt, d_G, nullptr);
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return MOTO_OK;
+}
+
+moto_status moto_rayleigh_ritz(moto_ctx* c, const double* d_GA, const double* d_GB, int n, int nev, double* d_theta, double* d_C) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_GA || !d_GB || !d_theta || !d_C || n < 1 || n > MOTO_NS || nev < 1 || nev > n)
+        return moto_fail(c, MOTO_EINVAL, "moto_rayleigh_ritz: bad argument");
+    c->launches += rr_solve(c, d_GA, d_GB, n, nev, d_theta, d_C, 0, nullptr);
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return MOTO_OK;
+}
+
+// ------------------------------------------------------------------ host-buffer variants
+moto_status moto_energy_grad_host(moto_ctx* c, const double* h_spins, double* h_E, double* h_g) {
+    if (!c) return MOTO_EINVAL;
+    if (!h_spins || (!h_E && !h_g)) return moto_fail(c, MOTO_EINVAL, "moto_energy_grad_host: null argument");
+    const size_t vb = (size_t)c->N * 3 * sizeof(double);
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->stage_m, h_spins, vb, cudaMemcpyHostToDevice, c->stream));
+    double* dE = c->st->scal + 7;
+    moto_status s = moto_energy_grad(c, c->stage_m, h_E ? dE : nullptr, h_g ? c->AP : nullptr);
+    if (s != MOTO_OK) return s;
+    if (h_E) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_E, dE, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    if (h_g) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_g, c->AP, vb, cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return MOTO_OK;
+}
+
+moto_status moto_hvp_host(moto_ctx* c, const double* h_spins, const double* h_V, int k, double* h_HV) {
+    if (!c) return MOTO_EINVAL;
+    if (!h_spins || !h_V || !h_HV) return moto_fail(c, MOTO_EINVAL, "moto_hvp_host: null argument");
+    if (k < 1 || k > c->kmax) return moto_fail(c, MOTO_EINVAL, "moto_hvp_host: k out of range [1, kmax]");
+    const size_t vb = (size_t)c->N * 3 * sizeof(double);
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->stage_m, h_spins, vb, cudaMemcpyHostToDevice, c->stream));
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->P, h_V, k * vb, cudaMemcpyHostToDevice, c->stream));
+    moto_status s = moto_hvp(c, c->stage_m, c->P, k, c->AP);
+    if (s != MOTO_OK) return s;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_HV, c->AP, k * vb, cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return MOTO_OK;
+}
+
+moto_status moto_lowest_modes_host(moto_ctx* c, const double* h_spins, int k, double tol, int max_iter, int warm_start,
+                                   double* h_lambda, double* h_V, moto_solve_info* info) {
+    if (!c) return MOTO_EINVAL;
+    if (!h_spins || !h_lambda || !h_V) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes_host: null argument");
+    if (k < 1 || k > c->kmax) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes_host: k out of range [1, kmax]");
+    if (!(tol > 0) || max_iter < 0) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes_host: tol must be > 0, max_iter >= 0");
+    const size_t vb = (size_t)c->N * 3 * sizeof(double);
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->stage_m, h_spins, vb, cudaMemcpyHostToDevice, c->stream));
+    if (warm_start) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->X, h_V, k * vb, cudaMemcpyHostToDevice, c->stream));
+    moto_status s = solve_internal(c, c->stage_m, k, tol, max_iter, warm_start, info);
+    if (s != MOTO_OK && s != MOTO_ENOTCONV) return s;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_V, c->X, k * vb, cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_lambda, c->st->theta, k * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return s;
+}
+
+moto_status moto_mmf_step_host(moto_ctx* c, const double* h_spins, const double* h_v, int kr, double dt, double* h_out, double* h_fnorm) {
+    if (!c) return MOTO_EINVAL;
+    if (!h_spins || !h_v || !h_out) return moto_fail(c, MOTO_EINVAL, "moto_mmf_step_host: null argument");
+    if (kr < 1 || kr > c->kmax) return moto_fail(c, MOTO_EINVAL, "moto_mmf_step_host: kr out of range [1, kmax]");
+    const size_t vb = (size_t)c->N * 3 * sizeof(double);
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->stage_m, h_spins, vb, cudaMemcpyHostToDevice, c->stream));
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->P, h_v, kr * vb, cudaMemcpyHostToDevice, c->stream));
+    double* dF = c->st->scal + 7;
+    moto_status s = moto_mmf_step(c, c->stage_m, c->P, kr, dt, c->stage_m, dF);
+    if (s != MOTO_OK) return s;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_out, c->stage_m, vb, cudaMemcpyDeviceToHost, c->stream));
+    if (h_fnorm) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_fnorm, dF, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return MOTO_OK;
+}
+
+}  // extern "C"

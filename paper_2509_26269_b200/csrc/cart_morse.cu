@@ -1,0 +1,320 @@
+// cart_morse.cu -- K7: Cartesian pair-potential gradient + block HVP over a cell-list neighbour
+// structure (the paper's Ni(111) portability case; Morse potential and cell list
+// per BASELINE.json north_star (4) / configs[4]).
+//
+//   g_i     = sum_j phi'(r) n ,                    n = (x_i - x_j)/r (minimum image in-plane, open in z)
+//   (Hv)_i  = sum_j [ phi'' n (n.dv) + (phi'/r)(dv - n (n.dv)) ],  dv = v_i - v_j ,  r < rc
+// masked: fixed atoms carry v = 0 and get a zero output row (the paper's mask Omega).
+//
+// Structure: 2-D cell list over the periodic in-plane cell (the slab is thin in z) -> per-atom
+// neighbour table with the pair coefficients (n, phi'', phi'/r, phi', phi - phi(rc)) stored once per
+// configuration, so every HVP of an eigen-solve is a gather over ~57 stored pairs per atom.
+// Deterministic: cells are sorted by atom id, neighbour order is fixed, reductions are fixed-order.
+#include "common.cuh"
+#include "device_utils.cuh"
+
+void launch_mmf_pass2(moto_ctx* c, const double* x, const double* v, int kr, const double* Fbuf, const double* alpha,
+                      double dt, double* x_out, int retract);
+void launch_final_sum(moto_ctx* c, const double* partials, int nblk, int stride, int nval, double* out, int take_sqrt);
+
+namespace {
+
+constexpr int NC = 7;  // coefficients per pair
+constexpr int MAXC = 4096;  // max cells
+
+struct CartGeom {
+    double a[2][2];    // cell rows
+    double inv[2][2];  // inverse: s = d_xy * inv
+    int ncx, ncy, Na;
+    double De, alpha, r0, rc, phic;
+};
+
+__device__ __forceinline__ void frac(const CartGeom& g, double x, double y, double& s0, double& s1) {
+    s0 = x * g.inv[0][0] + y * g.inv[1][0];
+    s1 = x * g.inv[0][1] + y * g.inv[1][1];
+}
+
+__global__ void k_cell_assign(CartGeom g, const double* __restrict__ x, int* __restrict__ cell_of, int* __restrict__ cell_count) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.Na) return;
+    double s0, s1;
+    frac(g, x[3 * i], x[3 * i + 1], s0, s1);
+    s0 -= floor(s0); s1 -= floor(s1);
+    int cx = min(g.ncx - 1, (int)(s0 * g.ncx)), cy = min(g.ncy - 1, (int)(s1 * g.ncy));
+    int c = cy * g.ncx + cx;
+    cell_of[i] = c;
+    atomicAdd(&cell_count[c], 1);
+}
+
+// single block: exclusive scan of cell counts, then each cell's atom list filled in ascending atom id
+__global__ void k_cell_build(int ncell, int Na, const int* __restrict__ cell_of, const int* __restrict__ cell_count,
+                             int* __restrict__ cell_start, int* __restrict__ cell_atoms) {
+    __shared__ int sstart[MAXC + 1];
+    if (threadIdx.x == 0) {
+        int s = 0;
+        for (int c = 0; c < ncell; ++c) { sstart[c] = s; s += cell_count[c]; }
+        sstart[ncell] = s;
+    }
+    __syncthreads();
+    for (int c = threadIdx.x; c <= ncell; c += blockDim.x) cell_start[c] = sstart[c];
+    // each thread owns a set of cells and scans the atoms in id order (deterministic, O(Na) per thread)
+    for (int c = threadIdx.x; c < ncell; c += blockDim.x) {
+        int w = sstart[c];
+        if (cell_count[c] == 0) continue;
+        for (int i = 0; i < Na; ++i) if (cell_of[i] == c) cell_atoms[w++] = i;
+    }
+}
+
+__device__ __forceinline__ void morse(const CartGeom& g, double r, double& phi, double& dphi, double& d2phi) {
+    double e = exp(-g.alpha * (r - g.r0));
+    phi = g.De * (e * e - 2.0 * e);
+    dphi = g.De * (-2.0 * g.alpha * e * e + 2.0 * g.alpha * e);
+    d2phi = g.De * (4.0 * g.alpha * g.alpha * e * e - 2.0 * g.alpha * g.alpha * e);
+}
+
+// one thread per atom: neighbour table + pair coefficients
+__global__ void k_neighbours(CartGeom g, const double* __restrict__ x, const int* __restrict__ cell_of,
+                             const int* __restrict__ cell_start, const int* __restrict__ cell_atoms, int* __restrict__ nb_count,
+                             int* __restrict__ nb_idx, double* __restrict__ nb_coef, int* __restrict__ overflow) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.Na) return;
+    const double xi = x[3 * i], yi = x[3 * i + 1], zi = x[3 * i + 2];
+    const int c = cell_of[i], cx = c % g.ncx, cy = c / g.ncx;
+    const int nx = min(3, g.ncx), ny = min(3, g.ncy);
+    int cnt = 0;
+    for (int oy = 0; oy < ny; ++oy) {
+        int yy = (cy + oy - (ny == 3 ? 1 : 0) + g.ncy) % g.ncy;
+        for (int ox = 0; ox < nx; ++ox) {
+            int xx = (cx + ox - (nx == 3 ? 1 : 0) + g.ncx) % g.ncx;
+            int cc = yy * g.ncx + xx;
+            for (int t = cell_start[cc]; t < cell_start[cc + 1]; ++t) {
+                int j = cell_atoms[t];
+                if (j == i) continue;
+                double dx = xi - x[3 * j], dy = yi - x[3 * j + 1], dz = zi - x[3 * j + 2];
+                double s0, s1;
+                frac(g, dx, dy, s0, s1);
+                s0 -= rint(s0); s1 -= rint(s1);
+                dx = s0 * g.a[0][0] + s1 * g.a[1][0];
+                dy = s0 * g.a[0][1] + s1 * g.a[1][1];
+                double r2 = dx * dx + dy * dy + dz * dz;
+                if (r2 < g.rc * g.rc) {
+                    if (cnt < MOTO_MAX_NEIGH) {
+                        double r = sqrt(r2), phi, dphi, d2phi;
+                        morse(g, r, phi, dphi, d2phi);
+                        double ir = 1.0 / r;
+                        size_t base = (size_t)i * NC * MOTO_MAX_NEIGH + cnt;
+                        nb_coef[base + 0 * MOTO_MAX_NEIGH] = dx * ir;
+                        nb_coef[base + 1 * MOTO_MAX_NEIGH] = dy * ir;
+                        nb_coef[base + 2 * MOTO_MAX_NEIGH] = dz * ir;
+                        nb_coef[base + 3 * MOTO_MAX_NEIGH] = d2phi;
+                        nb_coef[base + 4 * MOTO_MAX_NEIGH] = dphi * ir;
+                        nb_coef[base + 5 * MOTO_MAX_NEIGH] = dphi;
+                        nb_coef[base + 6 * MOTO_MAX_NEIGH] = phi - g.phic;
+                        nb_idx[(size_t)i * MOTO_MAX_NEIGH + cnt] = j;
+                    }
+                    ++cnt;
+                }
+            }
+        }
+    }
+    if (cnt > MOTO_MAX_NEIGH) { atomicExch(overflow, 1); cnt = MOTO_MAX_NEIGH; }
+    nb_count[i] = cnt;
+}
+
+// warp per atom: E_i = 1/2 sum_j (phi - phi_c),  g_i = sum_j phi' n  (zero row for fixed atoms)
+__global__ void __launch_bounds__(256) k_cart_energy_grad(int Na, const uint8_t* __restrict__ fixed, const int* __restrict__ nb_count,
+                                                          const double* __restrict__ nb_coef, double* __restrict__ g_out,
+                                                          double* __restrict__ e_atom) {
+    int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (i >= Na) return;
+    const double* cf = nb_coef + (size_t)i * NC * MOTO_MAX_NEIGH;
+    double gx = 0, gy = 0, gz = 0, e = 0;
+    for (int n = lane; n < nb_count[i]; n += 32) {
+        double dphi = cf[5 * MOTO_MAX_NEIGH + n];
+        gx = fma(dphi, cf[n], gx); gy = fma(dphi, cf[MOTO_MAX_NEIGH + n], gy); gz = fma(dphi, cf[2 * MOTO_MAX_NEIGH + n], gz);
+        e += cf[6 * MOTO_MAX_NEIGH + n];
+    }
+    gx = warp_sum(gx); gy = warp_sum(gy); gz = warp_sum(gz); e = warp_sum(e);
+    if (lane == 0) {
+        bool fx = fixed && fixed[i];
+        if (g_out) { g_out[3 * i] = fx ? 0.0 : gx; g_out[3 * i + 1] = fx ? 0.0 : gy; g_out[3 * i + 2] = fx ? 0.0 : gz; }
+        e_atom[i] = 0.5 * e;
+    }
+}
+
+// warp per atom, all k columns per pass over the stored pairs
+__global__ void __launch_bounds__(256) k_cart_hvp(int Na, int k, const uint8_t* __restrict__ fixed, const int* __restrict__ nb_count,
+                                                  const int* __restrict__ nb_idx, const double* __restrict__ nb_coef,
+                                                  const double* __restrict__ V, double* __restrict__ HV, const int* __restrict__ done) {
+    if (done && *done) return;
+    int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (i >= Na) return;
+    const bool fxi = fixed && fixed[i];
+    const double* cf = nb_coef + (size_t)i * NC * MOTO_MAX_NEIGH;
+    const int* idx = nb_idx + (size_t)i * MOTO_MAX_NEIGH;
+    double acc[MOTO_KMAX][3];
+#pragma unroll
+    for (int a = 0; a < MOTO_KMAX; ++a) acc[a][0] = acc[a][1] = acc[a][2] = 0.0;
+    if (!fxi) {
+        for (int n = lane; n < nb_count[i]; n += 32) {
+            const int j = idx[n];
+            const bool fxj = fixed && fixed[j];
+            d3 nn = mk3(cf[n], cf[MOTO_MAX_NEIGH + n], cf[2 * MOTO_MAX_NEIGH + n]);
+            const double d2 = cf[3 * MOTO_MAX_NEIGH + n], d1r = cf[4 * MOTO_MAX_NEIGH + n];
+#pragma unroll
+            for (int a = 0; a < MOTO_KMAX; ++a) {
+                if (a < k) {
+                    const double* v = V + (size_t)a * 3 * Na;
+                    d3 dv = ld3(v, i);
+                    if (!fxj) dv = sub3(dv, ld3(v, j));
+                    double nd = dot3(nn, dv);
+                    // phi'' n (n.dv) + (phi'/r)(dv - n (n.dv)) = (phi'' - phi'/r)(n.dv) n + (phi'/r) dv
+                    double w = (d2 - d1r) * nd;
+                    acc[a][0] += fma(w, nn.x, d1r * dv.x);
+                    acc[a][1] += fma(w, nn.y, d1r * dv.y);
+                    acc[a][2] += fma(w, nn.z, d1r * dv.z);
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < MOTO_KMAX; ++a) {
+        if (a < k) {
+            double x = warp_sum(acc[a][0]), y = warp_sum(acc[a][1]), z = warp_sum(acc[a][2]);
+            if (lane == 0) st3(HV + (size_t)a * 3 * Na, i, mk3(x, y, z));
+        }
+    }
+}
+
+__global__ void k_cart_mask(int Na, int k, const uint8_t* __restrict__ fixed, double* __restrict__ V) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= Na || !fixed || !fixed[i]) return;
+    for (int a = 0; a < k; ++a) st3(V + (size_t)a * 3 * Na, i, mk3(0, 0, 0));
+}
+
+// F = -g (masked) ; partial dots alpha_a = F . v_a   (g already in Fbuf, negate in place)
+__global__ void __launch_bounds__(256) k_cart_mmf_pass1(int Na, const double* __restrict__ v, int kr, double* __restrict__ Fbuf,
+                                                        double* __restrict__ partials) {
+    __shared__ double red[32 * MOTO_KMAX];
+    double acc[MOTO_KMAX];
+#pragma unroll
+    for (int a = 0; a < MOTO_KMAX; ++a) acc[a] = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < Na; i += gridDim.x * blockDim.x) {
+        d3 F = scale3(-1.0, ld3(Fbuf, i));
+        st3(Fbuf, i, F);
+#pragma unroll
+        for (int a = 0; a < MOTO_KMAX; ++a)
+            if (a < kr) acc[a] += dot3(F, ld3(v + (size_t)a * 3 * Na, i));
+    }
+    block_sum<MOTO_KMAX>(acc, red);
+    if (threadIdx.x == 0)
+        for (int a = 0; a < MOTO_KMAX; ++a) partials[blockIdx.x * MOTO_KMAX + a] = acc[a];
+}
+
+CartGeom make_geom(const moto_ctx* c) {
+    CartGeom g;
+    for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) g.a[a][b] = c->lat.cell[a][b];
+    double det = g.a[0][0] * g.a[1][1] - g.a[0][1] * g.a[1][0];
+    g.inv[0][0] = g.a[1][1] / det; g.inv[0][1] = -g.a[0][1] / det;
+    g.inv[1][0] = -g.a[1][0] / det; g.inv[1][1] = g.a[0][0] / det;
+    g.ncx = c->cl.ncx; g.ncy = c->cl.ncy; g.Na = c->N;
+    g.De = c->mp.De; g.alpha = c->mp.alpha; g.r0 = c->mp.r0; g.rc = c->mp.rc;
+    double e = exp(-g.alpha * (g.rc - g.r0));
+    g.phic = g.De * (e * e - 2.0 * e);
+    return g;
+}
+
+}  // namespace
+
+// cells: as many as fit with perpendicular width >= rc along each cell vector (at most 64 x 64)
+static void cart_cell_counts(const moto_lattice* lat, double rc, int* ncx, int* ncy, double* h0, double* h1) {
+    const double (*a)[2] = lat->cell;
+    double area = fabs(a[0][0] * a[1][1] - a[0][1] * a[1][0]);
+    double l0 = sqrt(a[0][0] * a[0][0] + a[0][1] * a[0][1]), l1 = sqrt(a[1][0] * a[1][0] + a[1][1] * a[1][1]);
+    *h0 = area / l1;  // width of the cell measured perpendicular to a1-lines (fractional coord 0)
+    *h1 = area / l0;
+    int nx = rc > 0 ? (int)(*h0 / rc) : 1, ny = rc > 0 ? (int)(*h1 / rc) : 1;
+    *ncx = nx < 1 ? 1 : (nx > 64 ? 64 : nx);
+    *ncy = ny < 1 ? 1 : (ny > 64 ? 64 : ny);
+}
+
+bool cart_geometry_ok(const moto_lattice* lat, double rc) {
+    int nx, ny; double h0, h1;
+    const double (*a)[2] = lat->cell;
+    double area = fabs(a[0][0] * a[1][1] - a[0][1] * a[1][0]);
+    if (!(area > 0)) return false;
+    cart_cell_counts(lat, rc, &nx, &ny, &h0, &h1);
+    return rc < 0.5 * h0 && rc < 0.5 * h1;  // minimum image by fractional rounding is exact below half the widths
+}
+
+static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+size_t cart_lists_bytes(const moto_lattice* lat) {
+    size_t Na = (size_t)lat->n_atoms;
+    return al256(Na * 4) * 3 + al256((MAXC + 1) * 4) * 2 + al256(Na * MOTO_MAX_NEIGH * 4) +
+           al256(Na * MOTO_MAX_NEIGH * NC * 8) + 256;
+}
+
+int cart_lists_carve(moto_ctx* c, char* base) {
+    size_t Na = (size_t)c->N;
+    char* p = base;
+    c->cl.cell_of = (int*)p; p += al256(Na * 4);
+    c->cl.cell_atoms = (int*)p; p += al256(Na * 4);
+    c->cl.nb_count = (int*)p; p += al256(Na * 4);
+    c->cl.cell_count = (int*)p; p += al256((MAXC + 1) * 4);
+    c->cl.cell_start = (int*)p; p += al256((MAXC + 1) * 4);
+    c->cl.nb_idx = (int*)p; p += al256(Na * MOTO_MAX_NEIGH * 4);
+    c->cl.nb_coef = (double*)p; p += al256(Na * MOTO_MAX_NEIGH * NC * 8);
+    c->cl.overflow = (int*)p; p += 256;
+    double h0, h1;
+    cart_cell_counts(&c->lat, c->mp.rc, &c->cl.ncx, &c->cl.ncy, &h0, &h1);
+    c->cl.ncell = c->cl.ncx * c->cl.ncy;
+    return 0;
+}
+
+int cart_build_lists(moto_ctx* c, const double* x) {
+    CartGeom g = make_geom(c);
+    const int Na = c->N, ncell = c->cl.ncell;
+    cudaMemsetAsync(c->cl.cell_count, 0, (ncell + 1) * sizeof(int), c->stream);
+    cudaMemsetAsync(c->cl.overflow, 0, sizeof(int), c->stream);
+    k_cell_assign<<<(Na + 127) / 128, 128, 0, c->stream>>>(g, x, c->cl.cell_of, c->cl.cell_count);
+    k_cell_build<<<1, 256, 0, c->stream>>>(ncell, Na, c->cl.cell_of, c->cl.cell_count, c->cl.cell_start, c->cl.cell_atoms);
+    k_neighbours<<<(Na + 63) / 64, 64, 0, c->stream>>>(g, x, c->cl.cell_of, c->cl.cell_start, c->cl.cell_atoms, c->cl.nb_count,
+                                                       c->cl.nb_idx, c->cl.nb_coef, c->cl.overflow);
+    return 3;
+}
+
+int cart_energy_grad(moto_ctx* c, const double* x, double* d_E, double* d_g) {
+    (void)x;
+    const int Na = c->N;
+    double* e_atom = c->c;  // [N] scratch
+    k_cart_energy_grad<<<(Na * 32 + 255) / 256, 256, 0, c->stream>>>(Na, c->lat.d_fixed, c->cl.nb_count, c->cl.nb_coef, d_g, e_atom);
+    int n = 1;
+    if (d_E) { launch_final_sum(c, e_atom, Na, 1, 1, d_E, 0); ++n; }
+    return n;
+}
+
+int cart_hvp(moto_ctx* c, const double* V, int k, double* HV, const int* d_done) {
+    const int Na = c->N;
+    k_cart_hvp<<<(Na * 32 + 255) / 256, 256, 0, c->stream>>>(Na, k, c->lat.d_fixed, c->cl.nb_count, c->cl.nb_idx, c->cl.nb_coef, V, HV, d_done);
+    return 1;
+}
+
+int cart_mask(moto_ctx* c, double* V, int k) {
+    if (!c->lat.d_fixed) return 0;
+    k_cart_mask<<<(c->N + 127) / 128, 128, 0, c->stream>>>(c->N, k, c->lat.d_fixed, V);
+    return 1;
+}
+
+int cart_mmf_step(moto_ctx* c, const double* x, const double* v, int kr, double dt, double* x_out, double* d_fnorm) {
+    const int Na = c->N;
+    int n = cart_energy_grad(c, x, nullptr, c->g);
+    double* alpha = c->st->scal;
+    int blocks = (Na + 255) / 256 < MOTO_RED_BLOCKS ? (Na + 255) / 256 : MOTO_RED_BLOCKS;
+    k_cart_mmf_pass1<<<blocks, 256, 0, c->stream>>>(Na, v, kr, c->g, c->partials);
+    launch_final_sum(c, c->partials, blocks, MOTO_KMAX, MOTO_KMAX, alpha, 0);
+    launch_mmf_pass2(c, x, v, kr, c->g, alpha, dt, x_out, 0);
+    n += 3;
+    if (d_fnorm) { launch_final_sum(c, c->partials, MOTO_RED_BLOCKS, 1, 1, d_fnorm, 1); ++n; }
+    return n;
+}

@@ -1,0 +1,123 @@
+// common.cuh -- context, device-side solver state and launch prototypes shared by the libmoto
+// translation units.  Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include "../../include/moto.h"
+
+#define MOTO_NS MOTO_NSMAX   // 24
+#define MOTO_NUM_SMS 148     // B200
+#define MOTO_RED_BLOCKS 296  // CTAs of every grid-reduction kernel (2 per SM): fixed => deterministic sums
+#define MOTO_MAX_NEIGH 160   // Cartesian: neighbour capacity per atom
+
+// Device-resident LOBPCG state: Gram matrices, Ritz coefficients, residuals, control flags.
+// Lives in the workspace; the host only ever reads the tail (ctl) through a pinned copy.
+struct SolverState {
+    double GA[MOTO_NS * MOTO_NS];
+    double GB[MOTO_NS * MOTO_NS];
+    double C[MOTO_NS * MOTO_KMAX];   // [ns][kb] coefficients of the new X in the basis [X,W,P]
+    double scal[8];                  // scratch scalars: F.v dots, signs ...
+    // ---- tail mirrored to the host (layout == HostStatus)
+    double theta[MOTO_KMAX];
+    double resid[MOTO_KMAX];
+    int done;      // 1 once all wanted residuals <= tol (kernels early-exit)
+    int iter;      // iterations completed
+    int nkeep;     // basis directions kept by the last Rayleigh-Ritz
+    int bad;       // 1 if a NaN/breakdown was seen
+};
+
+struct HostStatus {  // pinned mirror of the control block + residuals
+    double theta[MOTO_KMAX];
+    double resid[MOTO_KMAX];
+    int done, iter, nkeep, bad;
+};
+
+struct CartLists {
+    int ncx, ncy, ncell;
+    int* cell_of;      // [Na]
+    int* cell_count;   // [ncell]
+    int* cell_start;   // [ncell+1]
+    int* cell_atoms;   // [Na] sorted by (cell, atom id)
+    int* nb_count;     // [Na]
+    int* nb_idx;       // [Na][MOTO_MAX_NEIGH] neighbour ids, ascending
+    double* nb_coef;   // [Na][MOTO_MAX_NEIGH][5]: nx, ny, nz, phi'', phi'/r
+    int* overflow;     // [1] set if an atom exceeded MOTO_MAX_NEIGH
+};
+
+struct moto_ctx {
+    moto_lattice lat;
+    int kind;
+    int N;       // sites or atoms
+    int kmax;
+    moto_spin_params sp;
+    moto_morse_params mp;
+    moto_solver_opts opts;
+    cudaStream_t stream;
+    char* ws;
+    size_t ws_bytes;
+    // workspace views
+    double *X, *AX, *W, *AW, *P, *AP;  // [kmax][N][3] each
+    double* c;         // [N]   m_i . g_i
+    double* g;         // [N][3] gradient scratch
+    double* stage_m;   // [N][3] host-variant staging
+    double* partials;  // [MOTO_RED_BLOCKS][2*NS*NS] grid-reduction partials
+    SolverState* st;
+    CartLists cl;
+    HostStatus* hstat;  // pinned
+    cudaEvent_t ev[2];
+    int64_t launches;
+    char err[256];
+};
+
+#define MOTO_CUDA_CHECK(ctx, call)                                                              \
+    do {                                                                                        \
+        cudaError_t e__ = (call);                                                               \
+        if (e__ != cudaSuccess) {                                                               \
+            snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d %s: %s", __FILE__, __LINE__, #call, \
+                     cudaGetErrorString(e__));                                                  \
+            return MOTO_ECUDA;                                                                  \
+        }                                                                                       \
+    } while (0)
+
+static inline moto_status moto_fail(moto_ctx* ctx, moto_status s, const char* msg) {
+    if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s", msg);
+    return s;
+}
+
+// ---- launch wrappers (each returns the number of kernels it enqueued; errors via cudaGetLastError)
+// spin_stencil.cu
+int spin_energy_grad(moto_ctx*, const double* m, double* d_E, double* d_g, double* d_c);
+int spin_curvature(moto_ctx*, const double* m, double* d_c);
+int spin_hvp(moto_ctx*, const double* m, const double* c_or_null, const double* V, int k, double* HV,
+             int project_input, const int* d_done);
+int spin_mmf_step(moto_ctx*, const double* m, const double* v, int kr, double dt, double* m_out, double* d_fnorm);
+int spin_project(moto_ctx*, const double* m, double* V, int k);
+// cart_morse.cu
+int cart_build_lists(moto_ctx*, const double* x);
+int cart_energy_grad(moto_ctx*, const double* x, double* d_E, double* d_g);
+int cart_hvp(moto_ctx*, const double* V, int k, double* HV, const int* d_done);
+int cart_mmf_step(moto_ctx*, const double* x, const double* v, int kr, double dt, double* x_out, double* d_fnorm);
+int cart_mask(moto_ctx*, double* V, int k);
+size_t cart_lists_bytes(const moto_lattice* lat);
+int cart_lists_carve(moto_ctx*, char* base);
+// block_algebra.cu
+int block_gram(moto_ctx*, const double* const* S, int ns, const double* const* T, int nt, double* d_G,
+               const int* d_done);
+int block_gram_lobpcg(moto_ctx*, int kb);
+int block_update(moto_ctx*, int kb);
+int block_residual(moto_ctx*, const double* m_or_null, int kb, int k, double tol);
+int block_random(moto_ctx*, double* X, int kb, uint64_t seed);
+int block_zero(moto_ctx*, double* X, long long n);
+int gram_blocks(const moto_ctx*);
+int rr_solve_lobpcg(moto_ctx*, int kb, int nblk);
+bool cart_geometry_ok(const moto_lattice* lat, double rc);
+int block_apply_coeffs(moto_ctx*, double* V, int k, const double* d_C, double* scratch);
+int block_sign_normalise(moto_ctx*, double* V, int k);
+// rayleigh_ritz.cu
+int rr_solve(moto_ctx*, const double* d_GA, const double* d_GB, int n, int nev, double* d_theta, double* d_C,
+             int mode, SolverState* st_or_null);
+// lobpcg.cu
+moto_status lobpcg_solve(moto_ctx*, const double* d_state, int k, double tol, int max_iter, int warm_start,
+                         moto_solve_info* info);

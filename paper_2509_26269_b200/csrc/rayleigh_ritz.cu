@@ -1,0 +1,215 @@
+// rayleigh_ritz.cu -- K4: single-CTA generalized symmetric eigen-solve  G_A c = theta G_B c  for the
+// LOBPCG basis [X,W,P] (n = 3 kb <= 24), kept on the GPU (BASELINE.json north_star (3); the paper does
+// this host-side inside CuPy).
+//
+// Numerics: G_B is scaled to unit diagonal, diagonalised by cyclic Jacobi (parallel round-robin
+// ordering), directions with eigenvalue <= tau * max are dropped (canonical orthogonalisation: this is
+// what makes the un-orthogonalised basis [X,W,P] safe, incl. P = 0 on the first iteration), the
+// reduced standard problem M^T G_A M is diagonalised by the same Jacobi routine, eigenvalues sorted.
+#include "common.cuh"
+
+namespace {
+
+constexpr int NMAX = MOTO_NS;       // 24
+constexpr int LD = NMAX + 1;        // smem leading dimension
+constexpr int RR_THREADS = 128;
+
+struct JacobiScratch { int p[NMAX / 2], q[NMAX / 2]; double c[NMAX / 2], s[NMAX / 2]; double off, diag; };
+
+// Symmetric eigen-decomposition in shared memory: A (n x n, LD) -> diag(A) = eigenvalues, V = eigenvectors (cols).
+__device__ void jacobi_eig(double* A, double* V, int n, JacobiScratch* js) {
+    const int tid = threadIdx.x, nt = blockDim.x;
+    for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; V[i * LD + j] = (i == j) ? 1.0 : 0.0; }
+    __syncthreads();
+    if (n == 1) return;
+    const int np = (n + 1) & ~1, half = np / 2;
+    for (int sweep = 0; sweep < 30; ++sweep) {
+        if (tid == 0) {
+            double off = 0.0, dg = 0.0;
+            for (int i = 0; i < n; ++i) {
+                dg += A[i * LD + i] * A[i * LD + i];
+                for (int j = i + 1; j < n; ++j) off += A[i * LD + j] * A[i * LD + j];
+            }
+            js->off = off; js->diag = dg;
+        }
+        __syncthreads();
+        if (js->off <= 1e-32 * js->diag || js->off == 0.0) break;
+        for (int r = 0; r < np - 1; ++r) {
+            if (tid < half) {
+                int p, q;
+                if (tid == 0) { p = np - 1; q = r; }
+                else { p = (r + tid) % (np - 1); q = (r - tid + (np - 1)) % (np - 1); }
+                if (p > q) { int t = p; p = q; q = t; }
+                double c = 1.0, s = 0.0;
+                if (q < n) {
+                    double apq = A[p * LD + q];
+                    if (apq != 0.0) {
+                        double app = A[p * LD + p], aqq = A[q * LD + q];
+                        double tau = (aqq - app) / (2.0 * apq);
+                        double t = (tau >= 0.0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
+                        c = 1.0 / sqrt(1.0 + t * t);
+                        s = t * c;
+                    }
+                } else { p = -1; }
+                js->p[tid] = p; js->q[tid] = q; js->c[tid] = c; js->s[tid] = s;
+            }
+            __syncthreads();
+            // columns: A <- A J, V <- V J
+            for (int w = tid; w < half * n; w += nt) {
+                int t = w / n, i = w - t * n, p = js->p[t], q = js->q[t];
+                if (p < 0) continue;
+                double c = js->c[t], s = js->s[t];
+                double aip = A[i * LD + p], aiq = A[i * LD + q];
+                A[i * LD + p] = c * aip - s * aiq; A[i * LD + q] = s * aip + c * aiq;
+                double vip = V[i * LD + p], viq = V[i * LD + q];
+                V[i * LD + p] = c * vip - s * viq; V[i * LD + q] = s * vip + c * viq;
+            }
+            __syncthreads();
+            // rows: A <- J^T A
+            for (int w = tid; w < half * n; w += nt) {
+                int t = w / n, j = w - t * n, p = js->p[t], q = js->q[t];
+                if (p < 0) continue;
+                double c = js->c[t], s = js->s[t];
+                double apj = A[p * LD + j], aqj = A[q * LD + j];
+                A[p * LD + j] = c * apj - s * aqj; A[q * LD + j] = s * apj + c * aqj;
+            }
+            __syncthreads();
+            if (tid < half && js->p[tid] >= 0) { int p = js->p[tid], q = js->q[tid]; A[p * LD + q] = 0.0; A[q * LD + p] = 0.0; }
+            __syncthreads();
+        }
+    }
+    __syncthreads();
+}
+
+// mode 0: Rayleigh-Ritz (theta[nev], C[n][nev]);  mode 1: Loewdin orthonormalisation from G_B only (C[n][n])
+__global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ partials, int nblk, const double* __restrict__ GA_in,
+                                                   const double* __restrict__ GB_in, int n, int nev, double* __restrict__ theta_out,
+                                                   double* __restrict__ C_out, int mode, SolverState* st, double tau) {
+    if (st && st->done) return;
+    __shared__ double A[NMAX * LD], B[NMAX * LD], U[NMAX * LD], M[NMAX * LD], T[NMAX * LD], Z[NMAX * LD];
+    __shared__ double d[NMAX], sig[NMAX], th[NMAX];
+    __shared__ int keep[NMAX], ord[NMAX], na_s, bad_s;
+    __shared__ JacobiScratch js;
+    const int tid = threadIdx.x, nt = blockDim.x;
+
+    // 1. gather G_A, G_B (from grid-reduction partials, fixed order, or from given matrices); symmetrise
+    if (partials) {
+        const int ntc = 2 * n, ne = n * ntc;
+        for (int t = tid; t < 2 * n * n; t += nt) {
+            int which = t / (n * n), e = t - which * n * n, i = e / n, j = e - i * n;
+            int src = i * ntc + which * n + j;
+            double s = 0.0;
+            for (int b = 0; b < nblk; ++b) s += partials[(size_t)b * ne + src];
+            if (which) T[i * LD + j] = s; else U[i * LD + j] = s;  // U <- raw G_B, T <- raw G_A
+        }
+    } else {
+        for (int t = tid; t < n * n; t += nt) {
+            int i = t / n, j = t - i * n;
+            U[i * LD + j] = GB_in[t];
+            T[i * LD + j] = GA_in ? GA_in[t] : 0.0;
+        }
+    }
+    __syncthreads();
+    for (int t = tid; t < n * n; t += nt) {
+        int i = t / n, j = t - i * n;
+        B[i * LD + j] = 0.5 * (U[i * LD + j] + U[j * LD + i]);
+        A[i * LD + j] = 0.5 * (T[i * LD + j] + T[j * LD + i]);
+    }
+    __syncthreads();
+    if (st && partials) {  // keep a copy for diagnostics
+        for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; st->GA[t] = A[i * LD + j]; st->GB[t] = B[i * LD + j]; }
+    }
+    // 2. scale to unit diagonal; non-positive / NaN diagonal => inactive column
+    if (tid < n) {
+        double bii = B[tid * LD + tid];
+        d[tid] = (bii > 1e-300) ? rsqrt(bii) : 0.0;
+    }
+    if (tid == 0) bad_s = 0;
+    __syncthreads();
+    for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; B[i * LD + j] *= d[i] * d[j]; }
+    __syncthreads();
+    // 3. eigen-decomposition of the scaled G_B
+    jacobi_eig(B, U, n, &js);
+    if (tid == 0) {
+        double smax = 0.0;
+        for (int j = 0; j < n; ++j) { sig[j] = B[j * LD + j]; if (sig[j] > smax) smax = sig[j]; }
+        int na = 0;
+        for (int j = 0; j < n; ++j) if (sig[j] > tau * smax && sig[j] > 0.0) keep[na++] = j;
+        na_s = na;
+        if (!(smax == smax)) bad_s = 1;
+    }
+    __syncthreads();
+    const int na = na_s;
+    // M = D U_keep Sigma^{-1/2}   (n x na)
+    for (int t = tid; t < n * na; t += nt) {
+        int i = t / na, l = t - i * na, j = keep[l];
+        M[i * LD + l] = d[i] * U[i * LD + j] * rsqrt(sig[j]);
+    }
+    __syncthreads();
+    if (mode == 1) {
+        // Loewdin: C = M (U_keep)^T D^{-1}... applied to the ORIGINAL vectors: C = D U S^{-1/2} U^T  (n x n)
+        for (int t = tid; t < n * n; t += nt) {
+            int i = t / n, j = t - i * n;
+            double s = 0.0;
+            for (int l = 0; l < na; ++l) s += M[i * LD + l] * U[j * LD + keep[l]];
+            C_out[i * n + j] = s;
+        }
+        if (st && tid == 0) { st->nkeep = na; if (na < n || bad_s) st->bad = 1; }
+        return;
+    }
+    // 4. reduced standard problem  At = M^T A M
+    for (int t = tid; t < n * na; t += nt) {
+        int i = t / na, l = t - i * na;
+        double s = 0.0;
+        for (int j = 0; j < n; ++j) s += A[i * LD + j] * M[j * LD + l];
+        T[i * LD + l] = s;
+    }
+    __syncthreads();
+    for (int t = tid; t < na * na; t += nt) {
+        int a = t / na, b = t - a * na;
+        double s = 0.0;
+        for (int i = 0; i < n; ++i) s += M[i * LD + a] * T[i * LD + b];
+        B[a * LD + b] = s;
+    }
+    __syncthreads();
+    for (int t = tid; t < na * na; t += nt) { int a = t / na, b = t - a * na; A[a * LD + b] = 0.5 * (B[a * LD + b] + B[b * LD + a]); }
+    __syncthreads();
+    jacobi_eig(A, Z, na, &js);
+    // 5. sort ascending
+    if (tid == 0) {
+        for (int j = 0; j < na; ++j) { th[j] = A[j * LD + j]; ord[j] = j; }
+        for (int a = 0; a < na; ++a) {
+            int best = a;
+            for (int b = a + 1; b < na; ++b) if (th[ord[b]] < th[ord[best]]) best = b;
+            int t = ord[a]; ord[a] = ord[best]; ord[best] = t;
+        }
+        if (na < nev) bad_s = 1;
+        for (int a = 0; a < nev && a < na; ++a) if (!(th[ord[a]] == th[ord[a]])) bad_s = 1;
+    }
+    __syncthreads();
+    // 6. C = M Z[:, lowest nev]
+    for (int t = tid; t < n * nev; t += nt) {
+        int i = t / nev, j = t - i * nev;
+        double s = 0.0;
+        if (j < na) { int zj = ord[j]; for (int l = 0; l < na; ++l) s += M[i * LD + l] * Z[l * LD + zj]; }
+        C_out[i * nev + j] = s;
+    }
+    if (tid < nev) theta_out[tid] = (tid < na) ? th[ord[tid]] : 0.0;
+    if (st && tid == 0) { st->nkeep = na; if (bad_s) { st->bad = 1; st->done = 1; } }
+}
+
+}  // namespace
+
+int rr_solve(moto_ctx* c, const double* d_GA, const double* d_GB, int n, int nev, double* d_theta, double* d_C, int mode,
+             SolverState* st) {
+    const double tau = 1e-10;
+    k_rr<<<1, RR_THREADS, 0, c->stream>>>(nullptr, 0, d_GA, d_GB, n, nev, d_theta, d_C, mode, st, tau);
+    return 1;
+}
+
+// LOBPCG flavour: inputs are the Gram partials left in ctx->partials by block_gram_lobpcg
+int rr_solve_lobpcg(moto_ctx* c, int kb, int nblk) {
+    const double tau = 1e-10;
+    k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblk, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau);
+    return 1;
+}

@@ -1,0 +1,269 @@
+// spin_stencil.cu -- K1 (fused gradient + block Riemannian HVP stencil), K6 (reflected-force step +
+// retraction) and the tangent projector for the 2-D triangular spin lattice.
+//
+// The Euclidean Hessian of Eq. 4 is constant: with ordered-pair counting (A1)
+//   (L u)_i = -2 sum_{j in nn(i)} [ J u_j + u_j x D_ij ] - 2 K u_iz z ,   D_ij = D (z x rhat_ij)
+// so  g_i = (L m)_i - mu B,  c_i = m_i . g_i,  and on a tangent vector v (A5)
+//   Hess[v]_i = P_i (L v)_i - c_i v_i ,  P_i = I - m_i m_i^T.
+// For a +- bond pair with unit vector (rx, ry):  u+ x D+ + u- x D-  =  D ( -rx dz, -ry dz, rx dx + ry dy ),
+// d = u+ - u-, which is all the DMI costs.
+//
+// This file holds the generic path (any Lx, Ly, boundary): one thread per site, neighbours through
+// L1/L2.  The TMA-staged fast path lives in spin_stencil_tma.cu.
+#include "common.cuh"
+#include "device_utils.cuh"
+
+namespace {
+
+struct Lat {
+    int Lx, Ly, px, py;
+    double J, D, K, Bx, By, Bz, mu;
+};
+
+__host__ Lat make_lat(const moto_ctx* c) {
+    Lat l;
+    l.Lx = c->lat.Lx; l.Ly = c->lat.Ly; l.px = c->lat.pbc_x; l.py = c->lat.pbc_y;
+    l.J = c->sp.J; l.D = c->sp.D; l.K = c->sp.K; l.mu = c->sp.mu;
+    l.Bx = c->sp.B[0]; l.By = c->sp.B[1]; l.Bz = c->sp.B[2];
+    return l;
+}
+
+// neighbour site index or -1 (open boundary)
+__device__ __forceinline__ long long nb(const Lat& l, int ix, int iy, int dx, int dy) {
+    int jx = ix + dx, jy = iy + dy;
+    if (jx < 0) { if (!l.px) return -1; jx += l.Lx; }
+    if (jx >= l.Lx) { if (!l.px) return -1; jx -= l.Lx; }
+    if (jy < 0) { if (!l.py) return -1; jy += l.Ly; }
+    if (jy >= l.Ly) { if (!l.py) return -1; jy -= l.Ly; }
+    return (long long)jy * l.Lx + jx;
+}
+
+struct Nbrs { long long p1, m1, p2, m2, p3, m3; };  // +-a1, +-a2, +-(a2-a1)
+
+__device__ __forceinline__ Nbrs neighbours(const Lat& l, int ix, int iy) {
+    Nbrs n;
+    n.p1 = nb(l, ix, iy, 1, 0);  n.m1 = nb(l, ix, iy, -1, 0);
+    n.p2 = nb(l, ix, iy, 0, 1);  n.m2 = nb(l, ix, iy, 0, -1);
+    n.p3 = nb(l, ix, iy, -1, 1); n.m3 = nb(l, ix, iy, 1, -1);
+    return n;
+}
+
+#define SQ3H 0.86602540378443864676
+
+// (L u)_i from the six neighbour values (zero where absent) and the site's own u_z
+__device__ __forceinline__ d3 stencil_apply(const Lat& l, d3 up1, d3 um1, d3 up2, d3 um2, d3 up3, d3 um3, double uz) {
+    d3 s = add3(add3(add3(up1, um1), add3(up2, um2)), add3(up3, um3));
+    d3 d1 = sub3(up1, um1), d2 = sub3(up2, um2), d3_ = sub3(up3, um3);
+    // sum_p rx_p d_p , sum_p ry_p d_p  with r1=(1,0), r2=(1/2,s), r3=(-1/2,s)
+    double ax_z = d1.z + 0.5 * (d2.z - d3_.z);          // sum rx dz
+    double ay_z = SQ3H * (d2.z + d3_.z);                // sum ry dz
+    double axy = d1.x + 0.5 * (d2.x - d3_.x) + SQ3H * (d2.y + d3_.y);  // sum (rx dx + ry dy)
+    d3 r;
+    r.x = -2.0 * (l.J * s.x - l.D * ax_z);
+    r.y = -2.0 * (l.J * s.y - l.D * ay_z);
+    r.z = -2.0 * (l.J * s.z + l.D * axy) - 2.0 * l.K * uz;
+    return r;
+}
+
+__device__ __forceinline__ d3 ldn(const double* __restrict__ u, long long j) {
+    return j >= 0 ? ld3(u, j) : mk3(0.0, 0.0, 0.0);
+}
+
+__device__ __forceinline__ d3 stencil_field(const Lat& l, const double* __restrict__ u, const Nbrs& n, double uz) {
+    return stencil_apply(l, ldn(u, n.p1), ldn(u, n.m1), ldn(u, n.p2), ldn(u, n.m2), ldn(u, n.p3), ldn(u, n.m3), uz);
+}
+
+// projected neighbour value  P_j v_j
+__device__ __forceinline__ d3 ldnp(const double* __restrict__ m, const double* __restrict__ v, long long j) {
+    if (j < 0) return mk3(0.0, 0.0, 0.0);
+    return proj3(ld3(m, j), ld3(v, j));
+}
+
+// ---------------------------------------------------------------- energy + gradient (+ c)
+__global__ void __launch_bounds__(256) k_energy_grad(Lat l, const double* __restrict__ m, double* __restrict__ g_out,
+                                                     double* __restrict__ c_out, double* __restrict__ partials) {
+    __shared__ double red[32];
+    const long long N = (long long)l.Lx * l.Ly;
+    double e[1] = {0.0};
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        int iy = (int)(i / l.Lx), ix = (int)(i - (long long)iy * l.Lx);
+        Nbrs n = neighbours(l, ix, iy);
+        d3 mi = ld3(m, i);
+        d3 Lm = stencil_field(l, m, n, mi.z);
+        d3 B = mk3(l.mu * l.Bx, l.mu * l.By, l.mu * l.Bz);
+        d3 g = sub3(Lm, B);
+        double c = dot3(mi, g);
+        e[0] += 0.5 * dot3(mi, Lm) - dot3(mi, B);
+        if (g_out) st3(g_out, i, axpy3(-c, mi, g));
+        if (c_out) c_out[i] = c;
+    }
+    block_sum<1>(e, red);
+    if (threadIdx.x == 0) partials[blockIdx.x] = e[0];
+}
+
+// out[j] = sum_b partials[b*stride + j]  (optionally sqrt); one thread per j, fixed order
+__global__ void k_final_sum(const double* __restrict__ partials, int nblk, int stride, int nval, double* __restrict__ out,
+                            int take_sqrt) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= nval) return;
+    double s = 0.0;
+    for (int b = 0; b < nblk; ++b) s += partials[(size_t)b * stride + j];
+    out[j] = take_sqrt ? sqrt(s) : s;
+}
+
+// ---------------------------------------------------------------- block HVP, generic path
+template <bool HAVE_C, bool PROJECT>
+__global__ void __launch_bounds__(256) k_hvp_generic(Lat l, const double* __restrict__ m, const double* __restrict__ cvec,
+                                                     const double* __restrict__ V, int k, double* __restrict__ HV,
+                                                     const int* __restrict__ done) {
+    if (done && *done) return;
+    const long long N = (long long)l.Lx * l.Ly;
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int iy = (int)(i / l.Lx), ix = (int)(i - (long long)iy * l.Lx);
+    Nbrs n = neighbours(l, ix, iy);
+    d3 mi = ld3(m, i);
+    double c;
+    if (HAVE_C) {
+        c = cvec[i];
+    } else {
+        d3 Lm = stencil_field(l, m, n, mi.z);
+        c = dot3(mi, Lm) - l.mu * (mi.x * l.Bx + mi.y * l.By + mi.z * l.Bz);
+    }
+    for (int a = 0; a < k; ++a) {
+        const double* __restrict__ v = V + (size_t)a * 3 * N;
+        d3 vi = ld3(v, i);
+        d3 Lv;
+        if (PROJECT) {
+            vi = proj3(mi, vi);
+            Lv = stencil_apply(l, ldnp(m, v, n.p1), ldnp(m, v, n.m1), ldnp(m, v, n.p2), ldnp(m, v, n.m2),
+                               ldnp(m, v, n.p3), ldnp(m, v, n.m3), vi.z);
+        } else {
+            Lv = stencil_field(l, v, n, vi.z);
+        }
+        d3 h = axpy3(-c, vi, proj3(mi, Lv));
+        st3(HV + (size_t)a * 3 * N, i, h);
+    }
+}
+
+// ---------------------------------------------------------------- tangent projection of a block, in place
+__global__ void k_project(long long N, const double* __restrict__ m, double* __restrict__ V, int k) {
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    d3 mi = ld3(m, i);
+    for (int a = 0; a < k; ++a) {
+        double* v = V + (size_t)a * 3 * N;
+        st3(v, i, proj3(mi, ld3(v, i)));
+    }
+}
+
+// ---------------------------------------------------------------- K6 reflected-force step
+// pass 1: F = -P g  -> gbuf ; partial dots alpha_a = F . v_a
+__global__ void __launch_bounds__(256) k_mmf_pass1(Lat l, const double* __restrict__ m, const double* __restrict__ v, int kr,
+                                                   double* __restrict__ Fbuf, double* __restrict__ partials) {
+    __shared__ double red[32 * MOTO_KMAX];
+    const long long N = (long long)l.Lx * l.Ly;
+    double acc[MOTO_KMAX];
+#pragma unroll
+    for (int a = 0; a < MOTO_KMAX; ++a) acc[a] = 0.0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        int iy = (int)(i / l.Lx), ix = (int)(i - (long long)iy * l.Lx);
+        Nbrs n = neighbours(l, ix, iy);
+        d3 mi = ld3(m, i);
+        d3 Lm = stencil_field(l, m, n, mi.z);
+        d3 g = sub3(Lm, mk3(l.mu * l.Bx, l.mu * l.By, l.mu * l.Bz));
+        d3 F = scale3(-1.0, proj3(mi, g));
+        st3(Fbuf, i, F);
+#pragma unroll
+        for (int a = 0; a < MOTO_KMAX; ++a)
+            if (a < kr) acc[a] += dot3(F, ld3(v + (size_t)a * 3 * N, i));
+    }
+    block_sum<MOTO_KMAX>(acc, red);
+    if (threadIdx.x == 0)
+        for (int a = 0; a < MOTO_KMAX; ++a) partials[blockIdx.x * MOTO_KMAX + a] = acc[a];
+}
+
+// pass 2: F_mmf = F - 2 sum_a alpha_a v_a ; m' = normalize(m + dt F_mmf) ; partial |F_mmf|^2
+__global__ void __launch_bounds__(256) k_mmf_pass2(long long N, const double* __restrict__ m, const double* __restrict__ v, int kr,
+                                                   const double* __restrict__ Fbuf, const double* __restrict__ alpha, double dt,
+                                                   double* __restrict__ m_out, double* __restrict__ partials, int retract,
+                                                   const uint8_t* __restrict__ fixed) {
+    __shared__ double red[32];
+    double al[MOTO_KMAX];
+#pragma unroll
+    for (int a = 0; a < MOTO_KMAX; ++a) al[a] = (a < kr) ? alpha[a] : 0.0;
+    double f2[1] = {0.0};
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        d3 F = ld3(Fbuf, i);
+#pragma unroll
+        for (int a = 0; a < MOTO_KMAX; ++a)
+            if (a < kr) F = axpy3(-2.0 * al[a], ld3(v + (size_t)a * 3 * N, i), F);
+        if (fixed && fixed[i]) F = mk3(0.0, 0.0, 0.0);
+        f2[0] += dot3(F, F);
+        d3 x = axpy3(dt, F, ld3(m, i));
+        if (retract) x = scale3(1.0 / sqrt(dot3(x, x)), x);
+        st3(m_out, i, x);
+    }
+    block_sum<1>(f2, red);
+    if (threadIdx.x == 0) partials[blockIdx.x] = f2[0];
+}
+
+}  // namespace
+
+// ================================================================ host wrappers
+int spin_energy_grad(moto_ctx* c, const double* m, double* d_E, double* d_g, double* d_c) {
+    Lat l = make_lat(c);
+    k_energy_grad<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, d_g, d_c, c->partials);
+    int n = 1;
+    if (d_E) { k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_E, 0); ++n; }
+    return n;
+}
+
+int spin_curvature(moto_ctx* c, const double* m, double* d_c) { return spin_energy_grad(c, m, nullptr, nullptr, d_c); }
+
+int spin_hvp_tma(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV,
+                 int project_input, const int* d_done);  // spin_stencil_tma.cu; returns 0 if not applicable
+
+int spin_hvp(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input,
+             const int* d_done) {
+    int n = spin_hvp_tma(c, m, cvec, V, k, HV, project_input, d_done);
+    if (n > 0) return n;
+    Lat l = make_lat(c);
+    const long long N = c->N;
+    const int blocks = (int)((N + 255) / 256);
+    if (cvec) {
+        if (project_input) k_hvp_generic<true, true><<<blocks, 256, 0, c->stream>>>(l, m, cvec, V, k, HV, d_done);
+        else k_hvp_generic<true, false><<<blocks, 256, 0, c->stream>>>(l, m, cvec, V, k, HV, d_done);
+    } else {
+        if (project_input) k_hvp_generic<false, true><<<blocks, 256, 0, c->stream>>>(l, m, cvec, V, k, HV, d_done);
+        else k_hvp_generic<false, false><<<blocks, 256, 0, c->stream>>>(l, m, cvec, V, k, HV, d_done);
+    }
+    return 1;
+}
+
+int spin_project(moto_ctx* c, const double* m, double* V, int k) {
+    const long long N = c->N;
+    k_project<<<(int)((N + 255) / 256), 256, 0, c->stream>>>(N, m, V, k);
+    return 1;
+}
+
+int spin_mmf_step(moto_ctx* c, const double* m, const double* v, int kr, double dt, double* m_out, double* d_fnorm) {
+    Lat l = make_lat(c);
+    double* alpha = c->st->scal;  // [KMAX] would overflow scal[8]? KMAX == 8: exactly fits
+    k_mmf_pass1<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, v, kr, c->g, c->partials);
+    k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, MOTO_KMAX, MOTO_KMAX, alpha, 0);
+    k_mmf_pass2<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, m, v, kr, c->g, alpha, dt, m_out, c->partials, 1, nullptr);
+    int n = 3;
+    if (d_fnorm) { k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_fnorm, 1); ++n; }
+    return n;
+}
+
+// shared with cart_morse.cu (declared there as extern)
+void launch_mmf_pass2(moto_ctx* c, const double* x, const double* v, int kr, const double* Fbuf, const double* alpha,
+                      double dt, double* x_out, int retract) {
+    k_mmf_pass2<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, x, v, kr, Fbuf, alpha, dt, x_out, c->partials, retract,
+                                                      c->lat.d_fixed);
+}
+void launch_final_sum(moto_ctx* c, const double* partials, int nblk, int stride, int nval, double* out, int take_sqrt) {
+    k_final_sum<<<(nval + 127) / 128, 128, 0, c->stream>>>(partials, nblk, stride, nval, out, take_sqrt);
+}

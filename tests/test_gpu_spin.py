@@ -1,0 +1,251 @@
+"""GPU parity tests (spin lattice): the CUDA path, called through the C ABI, against the CPU oracle on the
+same seeded inputs.  Tolerances are BASELINE.json north_star's: HVP relative L2 <= 1e-11, eigenvalues
+relative <= 1e-8, lowest-k subspace principal angle <= 1e-6."""
+import numpy as np
+import pytest
+import scipy.linalg
+
+from oracle import spin_oracle as so
+from paper_2509_26269_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+HVP_TOL = 1e-11
+EIG_TOL = 1e-8
+ANGLE_TOL = 1e-6
+
+
+def model_of(w):
+    return so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
+
+
+def dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).cuda()
+
+
+def rel_l2(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+def custom(Lx, Ly, px, py, seed, B=(0.01, -0.02, 0.03), k=2):
+    m = wl.random_spins(Lx, Ly, seed)
+    return wl.SpinWorkload(f"rand{Lx}x{Ly}", Lx, Ly, px, py, 1.0, 0.3, 0.05, B, 1.0, k, seed, m)
+
+
+CASES = [
+    lambda: wl.config0(),
+    lambda: wl.config1(),
+    lambda: custom(37, 23, 0, 0, 1),    # odd sizes, open, ragged tail
+    lambda: custom(64, 50, 1, 0, 2),    # mixed boundaries
+    lambda: custom(130, 70, 0, 1, 3),   # spans several tiles
+    lambda: custom(1, 1, 0, 0, 4),      # degenerate: single spin
+    lambda: custom(2, 3, 1, 1, 5),      # tiny periodic (neighbours alias)
+    lambda: wl.config3_scaled(100),
+]
+
+
+@pytest.mark.parametrize("case", range(len(CASES)))
+def test_energy_grad_parity(moto, case):
+    w = CASES[case]()
+    model = model_of(w)
+    ctx = moto.spin_context(w)
+    E, g = ctx.energy_grad(dev(w.spins))
+    E_ref = so.energy(model, w.spins)
+    g_ref = so.projected_gradient(model, w.spins)
+    assert abs(E.item() - E_ref) <= 1e-12 * max(1.0, abs(E_ref))
+    assert np.max(np.abs(g.cpu().numpy() - g_ref)) <= 1e-12
+
+
+@pytest.mark.parametrize("case", range(len(CASES)))
+@pytest.mark.parametrize("k", [1, 2, 6])
+def test_hvp_parity(moto, case, k):
+    w = CASES[case]()
+    model = model_of(w)
+    ctx = moto.spin_context(w, kmax=8)
+    V = wl.random_block(w.N, k, seed=100 + case)       # NOT tangent: the call must project
+    HV = ctx.hvp(dev(w.spins), dev(V)).cpu().numpy()
+    ref = so.hvp(model, w.spins, V)
+    assert rel_l2(HV, ref) <= HVP_TOL
+    assert np.max(np.abs(np.sum(HV * w.spins[None], axis=2))) <= 1e-12   # tangent output
+
+
+def test_hvp_kmax_and_arg_errors(moto):
+    w = wl.config0()
+    ctx = moto.spin_context(w, kmax=8)
+    V = wl.random_block(w.N, 8, seed=7)
+    HV = ctx.hvp(dev(w.spins), dev(V)).cpu().numpy()
+    assert rel_l2(HV, so.hvp(model_of(w), w.spins, V)) <= HVP_TOL
+    import torch
+    with pytest.raises(moto.MotoError):
+        ctx.hvp(dev(w.spins), dev(wl.random_block(w.N, 9, seed=7)))
+    with pytest.raises(moto.MotoError):
+        v = dev(V)
+        ctx.hvp(dev(w.spins), v, out=v)
+
+
+def test_gram_parity(moto):
+    w = custom(50, 41, 1, 1, 9)
+    ctx = moto.spin_context(w, kmax=8)
+    S = wl.random_block(w.N, 6, seed=1)
+    T = wl.random_block(w.N, 12, seed=2)
+    G = ctx.gram(dev(S), dev(T)).cpu().numpy()
+    ref = S.reshape(6, -1) @ T.reshape(12, -1).T
+    assert np.max(np.abs(G - ref)) <= 1e-11 * np.max(np.abs(ref)) + 1e-10
+
+
+@pytest.mark.parametrize("n,nev", [(3, 1), (6, 2), (9, 3), (18, 6), (24, 8)])
+def test_rayleigh_ritz_vs_lapack(moto, n, nev):
+    rng = np.random.default_rng(n)
+    Q = rng.standard_normal((n, n))
+    GB = Q @ Q.T + 0.1 * np.eye(n)
+    GA = rng.standard_normal((n, n)); GA = GA + GA.T
+    w = wl.config0()
+    ctx = moto.spin_context(w, kmax=8)
+    th, Cm = ctx.rayleigh_ritz(dev(GA), dev(GB), nev)
+    th, Cm = th.cpu().numpy(), Cm.cpu().numpy()
+    ref, Y = scipy.linalg.eigh(GA, GB)
+    assert np.max(np.abs(th - ref[:nev])) <= 1e-11 * np.max(np.abs(ref))
+    assert np.max(np.abs(Cm.T @ GB @ Cm - np.eye(nev))) <= 1e-11
+    assert np.max(np.abs(Cm.T @ GA @ Cm - np.diag(th))) <= 1e-10 * np.max(np.abs(ref))
+
+
+def test_rayleigh_ritz_drops_null_directions(moto):
+    # rank-deficient G_B (duplicate + zero basis vectors), as on the first LOBPCG iteration (P = 0)
+    rng = np.random.default_rng(0)
+    S = rng.standard_normal((40, 6)); S[:, 4] = 0.0; S[:, 5] = S[:, 1]
+    Aop = rng.standard_normal((40, 40)); Aop = Aop + Aop.T
+    GA, GB = S.T @ Aop @ S, S.T @ S
+    w = wl.config0()
+    ctx = moto.spin_context(w, kmax=8)
+    th, Cm = ctx.rayleigh_ritz(dev(GA), dev(GB), 2)
+    Sr = S[:, :4]
+    ref = scipy.linalg.eigh(Sr.T @ Aop @ Sr, Sr.T @ Sr, eigvals_only=True)
+    assert np.max(np.abs(th.cpu().numpy() - ref[:2])) <= 1e-10 * np.max(np.abs(ref))
+
+
+def _check_modes(w, lam, V, lam_ref, V_ref, k):
+    lam = lam.cpu().numpy(); V = V.cpu().numpy()
+    relerr = np.abs(lam - lam_ref[:k]) / np.maximum(np.abs(lam_ref[:k]), 1e-3)
+    assert relerr.max() <= EIG_TOL, (lam, lam_ref)
+    ang = scipy.linalg.subspace_angles(V.reshape(k, -1).T, V_ref[:k].reshape(k, -1).T)
+    assert ang.max() <= ANGLE_TOL, ang
+    G = V.reshape(k, -1) @ V.reshape(k, -1).T
+    assert np.max(np.abs(G - np.eye(k))) <= 1e-10
+    assert np.max(np.abs(np.sum(V * w.spins[None], axis=2))) <= 1e-10
+    for a in range(k):   # sign convention: largest-|component| entry positive
+        f = V[a].ravel()
+        assert f[np.argmax(np.abs(f))] > 0
+
+
+def test_lowest_modes_cfg0(moto):
+    w = wl.config0()
+    lam_ref, V_ref = so.lowest_modes(model_of(w), w.spins, 2, extra=1)
+    ctx = moto.spin_context(w)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=500)
+    assert info["converged"] and max(info["resid"]) <= 1e-9
+    _check_modes(w, lam, V, lam_ref, V_ref, 2)
+    # oracle-side residual of the GPU pair
+    HV = so.hvp(model_of(w), w.spins, V.cpu().numpy())
+    for a in range(2):
+        assert np.linalg.norm(HV[a] - lam[a].item() * V[a].cpu().numpy()) <= 2e-9
+
+
+def test_lowest_modes_cfg1(moto):
+    w = wl.config1()
+    lam_ref, V_ref = so.lowest_modes(model_of(w), w.spins, 2, extra=1)
+    ctx = moto.spin_context(w)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=2000)
+    assert info["converged"], info
+    _check_modes(w, lam, V, lam_ref, V_ref, 2)
+
+
+def test_lowest_modes_guard_and_warm_start(moto):
+    w = wl.config1(L=40)
+    lam_ref, V_ref = so.lowest_modes(model_of(w), w.spins, 3, extra=1)
+    ctx = moto.spin_context(w, kmax=6)
+    ctx.set_solver(guard=3)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 3, tol=1e-9, max_iter=2000)
+    assert info["converged"]
+    _check_modes(w, lam, V, lam_ref, V_ref, 3)
+    # warm start from the converged block: converges at once
+    lam2, V2, info2 = ctx.lowest_modes(dev(w.spins), 3, tol=1e-8, max_iter=50, V0=V)
+    assert info2["converged"] and info2["iters"] <= 2
+    _check_modes(w, lam2, V2, lam_ref, V_ref, 3)
+
+
+def test_lowest_modes_not_converged_status(moto):
+    w = wl.config1(L=40)
+    ctx = moto.spin_context(w)
+    with pytest.raises(moto.MotoError) as e:
+        ctx.lowest_modes(dev(w.spins), 2, tol=1e-12, max_iter=3)
+    assert e.value.status == moto.ENOTCONV
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-12, max_iter=3, allow_notconv=True)
+    assert not info["converged"] and info["iters"] == 3 and np.isfinite(lam.cpu().numpy()).all()
+
+
+def test_ferromagnet_degenerate_pair(moto):
+    # uniform +z: lowest eigenvalue 2K+B exactly doubly degenerate -> compare the 2-d subspace
+    w = wl.config0(sigma=0.0)
+    ctx = moto.spin_context(w)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-10, max_iter=500)
+    assert np.allclose(lam.cpu().numpy(), 0.12, atol=1e-9)
+
+
+def test_mmf_step_parity(moto):
+    for w in (wl.config0(), wl.config1(L=30), custom(37, 23, 0, 0, 1)):
+        model = model_of(w)
+        _, V_ref = so.lowest_modes(model, w.spins, 2)
+        ctx = moto.spin_context(w)
+        for kr in (1, 2):
+            out, fn = ctx.mmf_step(dev(w.spins), dev(V_ref[:kr]), 0.05)
+            ref = so.mmf_step(model, w.spins, V_ref[:kr], 0.05)
+            assert np.max(np.abs(out.cpu().numpy() - ref)) <= 1e-13
+            assert abs(fn.item() - np.linalg.norm(so.mmf_force(model, w.spins, V_ref[:kr]))) <= 1e-12
+        # in place
+        s = dev(w.spins)
+        ctx.mmf_step(s, dev(V_ref[:1]), 0.05, out=s)
+        assert np.max(np.abs(s.cpu().numpy() - so.mmf_step(model, w.spins, V_ref[:1], 0.05))) <= 1e-13
+
+
+def test_transport(moto):
+    w = wl.config1(L=30)
+    model = model_of(w)
+    _, V = so.lowest_modes(model, w.spins, 2)
+    m2 = so.mmf_step(model, w.spins, V[:1], 0.05)
+    ctx = moto.spin_context(w)
+    Vt = ctx.transport(dev(m2), dev(V)).cpu().numpy()
+    assert np.max(np.abs(np.sum(Vt * m2[None], axis=2))) <= 1e-13
+    G = Vt.reshape(2, -1) @ Vt.reshape(2, -1).T
+    assert np.max(np.abs(G - np.eye(2))) <= 1e-12
+    Pv = V - np.sum(V * m2[None], 2, keepdims=True) * m2[None]
+    ang = scipy.linalg.subspace_angles(Vt.reshape(2, -1).T, Pv.reshape(2, -1).T)
+    assert ang.max() <= 1e-10
+
+
+def test_host_variants(moto):
+    w = wl.config1(L=30)
+    model = model_of(w)
+    ctx = moto.spin_context(w)
+    E, g = ctx.energy_grad_host(w.spins, np.zeros_like(w.spins))
+    assert abs(E - so.energy(model, w.spins)) <= 1e-12 * abs(E)
+    assert np.max(np.abs(g - so.projected_gradient(model, w.spins))) <= 1e-12
+    V = wl.random_block(w.N, 2, seed=3)
+    HV = ctx.hvp_host(w.spins, V, np.zeros_like(V))
+    assert rel_l2(HV, so.hvp(model, w.spins, V)) <= HVP_TOL
+    lam = np.zeros(2); Vh = np.zeros((2, w.N, 3))
+    info = ctx.lowest_modes_host(w.spins, 2, 1e-9, 2000, lam, Vh)
+    lam_ref, V_ref = so.lowest_modes(model, w.spins, 2)
+    assert info["converged"] and np.max(np.abs(lam - lam_ref)) <= 1e-8 * np.max(np.abs(lam_ref))
+    out, fn = ctx.mmf_step_host(w.spins, V_ref[:1], 0.05, np.zeros_like(w.spins))
+    assert np.max(np.abs(out - so.mmf_step(model, w.spins, V_ref[:1], 0.05))) <= 1e-13
+
+
+def test_determinism(moto):
+    w = wl.config1(L=40)
+    ctx = moto.spin_context(w)
+    a = ctx.lowest_modes(dev(w.spins), 2, tol=1e-8, max_iter=1000)
+    b = ctx.lowest_modes(dev(w.spins), 2, tol=1e-8, max_iter=1000)
+    assert np.array_equal(a[0].cpu().numpy(), b[0].cpu().numpy())
+    assert np.array_equal(a[1].cpu().numpy(), b[1].cpu().numpy())
+    assert ctx.launch_count > 0
