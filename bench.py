@@ -1,0 +1,305 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement (BASELINE.json metric: lowest-2-mode solve ms & HVPs/s at 10^6 spins;
+HVP GB/s vs HBM peak).
+
+One "step" = one pass of the whole hot path on configs[3] (1000x1000 periodic, ~200 skyrmions, fp64):
+  moto_lowest_modes(k=2, tol=1e-6, cold seeded start)  ->  moto_energy_grad  ->  moto_mmf_step(v1, dt).
+`value` = single-vector HVP applications per second over the timed steps (inputs resident in HBM);
+`e2e`  = the same step through the host-buffer C ABI (H2D of the spins, D2H of lambda, V, m', |F|).
+`roofline` is measured live for the K1 block-HVP kernel in a dedicated region of the same run
+(buffer sets rotated so the footprint exceeds L2).  `cpu_baseline` times the oracle on a bounded sample.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl moto|reference] [--workload cfg3]
+N > 1 (torchrun): N independent replicas (different seeds), no data-path collective ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "HVPs/s over [lowest-2-mode solve + energy_grad + MMF step] at 10^6 spins"
+UNIT = "HVP/s"
+L2_BYTES = 126e6
+
+
+def make_workload(name: str, seed_offset: int = 0):
+    from paper_2509_26269_b200 import workloads as wl
+    if name == "cfg3":
+        return wl.config3(seed=1003 + seed_offset)
+    if name.startswith("cfg3s:"):
+        return wl.config3_scaled(int(name.split(":")[1]), seed=1003 + seed_offset)
+    if name == "cfg1":
+        return wl.config1(seed=1001 + seed_offset)
+    if name == "cfg2":
+        return wl.config2(seed=1002 + seed_offset)
+    raise SystemExit(f"unknown workload {name}")
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=lambda: [self.lines.append(l) for l in self.proc.stdout], daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(L: int = 316, calls: int = 3):
+    """The oracle, as it stands, on a bounded same-density sample of configs[3]; returns HVP/s scaled to 1e6 sites."""
+    from oracle import spin_oracle as so
+    from paper_2509_26269_b200 import workloads as wl
+    import threadpoolctl
+    w = wl.config3_scaled(L)
+    model = so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
+    V = wl.random_block(w.N, 2, seed=5)
+    t0 = time.perf_counter()
+    for _ in range(calls):
+        so.hvp(model, w.spins, V)
+    dt = time.perf_counter() - t0
+    site_hvps = calls * 2 * w.N
+    cores = max([i.get("num_threads", 1) for i in threadpoolctl.threadpool_info()] + [1])
+    return {"value": site_hvps / dt / 1e6, "unit": UNIT, "cores": int(cores), "kind": "oracle",
+            "sample": f"oracle.spin_oracle.hvp (explicit sparse tangent Hessian rebuilt per call, k=2) x{calls} on the "
+                      f"{L}x{L} same-density instance of configs[3]; site-HVPs/s divided by 1e6 sites; {dt:.1f} s of CPU",
+            "host_cpus": os.cpu_count()}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    vals, t_all = [], []
+    for _ in range(args.warmup):
+        oracle_sample(L=100, calls=1)
+    for _ in range(args.steps):
+        t0 = time.perf_counter()
+        r = oracle_sample(L=200, calls=2)
+        t_all.append(time.perf_counter() - t0)
+        vals.append(r["value"])
+    v = float(np.mean(vals))
+    cb = dict(r); cb["value"] = v
+    cb["sample"] = "each step: oracle.spin_oracle.hvp x2 (k=2) on the 200x200 same-density instance of configs[3], scaled by sites to 1e6"
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(t_all)), "higher_is_better": True,
+                      "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": "configs[3] 1000x1000 pbc ~200 skyrmions k=2 (bounded same-density sample)"},
+                      "cpu_baseline": cb,
+                      "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="moto", choices=["moto", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--max-iter", type=int, default=20000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--hvp-reps", type=int, default=60)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2509_26269_b200 as moto
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = make_workload(args.workload, seed_offset=rank)
+    k, tol, dt = w.k, w.tol, w.dt
+    ctx = moto.spin_context(w, kmax=k, device=f"cuda:{local}")
+    N = w.N
+    dev = torch.device("cuda", local)
+    m = torch.as_tensor(w.spins, device=dev)
+    m_out = torch.empty_like(m)
+
+    # ---------------------------------------------------------------- (A) K1 block-HVP kernel alone, cold L2
+    alg_bytes = 24 * N * (1 + 2 * k)
+    nsets = max(2, int(np.ceil(2.5 * L2_BYTES / alg_bytes)) + 1)
+    ms_sets = [m.clone() for _ in range(nsets)]
+    V_sets = [torch.randn(k, N, 3, dtype=torch.float64, device=dev) for _ in range(nsets)]
+    HV_sets = [torch.empty(k, N, 3, dtype=torch.float64, device=dev) for _ in range(nsets)]
+    for i in range(3 * nsets):
+        ctx.hvp(ms_sets[i % nsets], V_sets[i % nsets], out=HV_sets[i % nsets])
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = ctx.launch_count
+    e0.record()
+    for i in range(args.hvp_reps):
+        ctx.hvp(ms_sets[i % nsets], V_sets[i % nsets], out=HV_sets[i % nsets])
+    e1.record()
+    torch.cuda.synchronize()
+    hvp_ms = e0.elapsed_time(e1) / args.hvp_reps
+    hvp_launches = (ctx.launch_count - l0) / args.hvp_reps
+    del ms_sets, V_sets, HV_sets
+    peak, peak_src = measured_peaks()
+    achieved = alg_bytes / (hvp_ms * 1e-3) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "k1_traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get(args.workload)
+
+    # ---------------------------------------------------------------- (B) the step, inputs resident in HBM
+    def step():
+        lam, V, info = ctx.lowest_modes(m, k, tol=tol, max_iter=args.max_iter, allow_notconv=True)
+        E, _ = ctx.energy_grad(m, want_grad=False)
+        _, fn = ctx.mmf_step(m, V[:1], dt, out=m_out)
+        return lam, info, E, fn
+
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    l0 = ctx.launch_count
+    infos = []
+    solve_ms = []
+    e0.record()
+    for _ in range(args.steps):
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record()
+        lam, info, E, fn = step()
+        s1.record()
+        infos.append(info); solve_ms.append((s0, s1))
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    total_ms = e0.elapsed_time(e1)
+    launches = ctx.launch_count - l0
+    hvps = sum(i["hvp_count"] for i in infos)
+    if dist is not None:
+        t = torch.tensor([total_ms, float(hvps)], dtype=torch.float64, device=dev)
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        total_ms, hvps = float(tmax[0]), float(tsum[1])
+    value = hvps / (total_ms * 1e-3)
+
+    # ---------------------------------------------------------------- (C) end to end through the host-buffer ABI
+    h_m = torch.as_tensor(w.spins).pin_memory().numpy()
+    h_lam = torch.zeros(k, dtype=torch.float64).pin_memory().numpy()
+    h_V = torch.zeros(k, N, 3, dtype=torch.float64).pin_memory().numpy()
+    h_out = torch.zeros(N, 3, dtype=torch.float64).pin_memory().numpy()
+
+    def step_host():
+        info = ctx.lowest_modes_host(h_m, k, tol, args.max_iter, h_lam, h_V, allow_notconv=True)
+        E, _ = ctx.energy_grad_host(h_m)
+        _, fn = ctx.mmf_step_host(h_m, h_V[:1], dt, h_out)
+        return info
+
+    step_host()
+    barrier()
+    t0 = time.perf_counter()
+    e2e_hvps = 0
+    n_e2e = max(1, min(args.steps, 3))
+    for _ in range(n_e2e):
+        e2e_hvps += step_host()["hvp_count"]
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s, float(e2e_hvps)], dtype=torch.float64, device=dev)
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        e2e_s, e2e_hvps = float(tmax[0]), float(tsum[1])
+    h2d = 3 * 24 * N + 24 * N          # spins x3 calls + v1
+    d2h = 8 * k + 24 * N * k + 8 + 24 * N + 8
+
+    # ---------------------------------------------------------------- (D) oracle on the host cores (rank 0, N=1)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = oracle_sample()
+
+    if rank == 0:
+        last = infos[-1]
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{w.name} (BASELINE.json configs[3] recipe)" if args.workload == "cfg3" else w.name,
+                       "N": N, "k": k, "tol": tol, "dt": dt, "max_iter": args.max_iter, "start": "cold seeded block",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2_policy": f"solver working set {ctx.workspace_bytes / 1e6:.0f} MB > L2; HVP-only region rotates "
+                                    f"{nsets} buffer sets of {alg_bytes / 1e6:.0f} MB"},
+            "solve": {"ms": float(np.mean([a.elapsed_time(b) for a, b in solve_ms])), "iters": last["iters"],
+                      "converged": last["converged"], "resid": last["resid"], "hvp_count": last["hvp_count"],
+                      "lambda": [float(x) for x in lam.cpu().numpy()],
+                      "peak_incremental_bytes": ctx.workspace_bytes},
+            "hvp_kernel": {"ms": hvp_ms, "block_hvps_per_s": 1e3 / hvp_ms, "hvps_per_s": k * 1e3 / hvp_ms,
+                           "gsite_updates_per_s": N * k / (hvp_ms * 1e-3) / 1e9, "launches_per_call": hvp_launches},
+            "roofline": {"bound": "hbm", "kernel": "K1 block HVP (moto_hvp)", "achieved": achieved, "peak": peak,
+                         "unit": "GB/s", "frac": achieved / peak, "frac_of_8TBs_nominal": achieved / 8000.0,
+                         "traffic": traffic, "algorithmic_bytes": alg_bytes, "peak_source": peak_src},
+            "e2e": {"value": e2e_hvps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": 1e3 * e2e_s / n_e2e, "steps": n_e2e},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -209,7 +209,7 @@ def lowest_modes(model: SpinModel, m: np.ndarray, k: int, extra: int = 0):
     Ht, Bm = tangent_hessian(model, m, dense=True)
     Ht = 0.5 * (Ht + Ht.T)  # "Hermitian part"; Ht is already symmetric to rounding
     lam, Y = scipy.linalg.eigh(Ht, subset_by_index=[0, k + extra - 1])
-    V = (Bm @ Y).T.reshape(k + extra, model.N, 3)
+    V = np.ascontiguousarray((Bm @ Y).T).reshape(k + extra, model.N, 3)
     return lam, V
 
 
@@ -223,7 +223,7 @@ def lowest_modes_sparse(model: SpinModel, m: np.ndarray, k: int, extra: int = 0,
     lam, Y = spla.eigsh(Ht, k=k + extra, sigma=sigma, which="LM", tol=tol)
     order = np.argsort(lam)
     lam, Y = lam[order], Y[:, order]
-    V = (Bm @ Y).T.reshape(k + extra, model.N, 3)
+    V = np.ascontiguousarray((Bm @ Y).T).reshape(k + extra, model.N, 3)
     return lam, V
 
 
