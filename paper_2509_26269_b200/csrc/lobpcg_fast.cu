@@ -1,0 +1,223 @@
+// lobpcg_fast.cu -- fused block-vector algebra of the device-resident LOBPCG for block sizes kb <= 2
+// (the headline case: two lowest modes; Knyazev ref [27] PAPER.md:221).
+//
+// One iteration is TWO streaming kernels and one single-CTA kernel:
+//   K1            AW = Hess[W]                       (+ per-CTA partials of W^T AW)
+//   k_rr          reduce partials -> residual check -> Rayleigh-Ritz on the 3kb x 3kb pencil
+//   k_update_fused  one pass over [X,W,P,AX,AW,AP]:  X' = S C, P' = [W,P] C_wp, AX', AP' by the same
+//                 coefficients, W' = R = AX' - X' Theta, partials of |r_j|^2 AND of every Gram entry the
+//                 next Rayleigh-Ritz needs except W'^T A W' (which needs the next HVP)
+// so no separate Gram pass exists: per iteration the block vectors are read once and written once.
+// W' is re-projected onto the tangent space inside the same pass (see k_update_fused); masked (fixed-atom)
+// rows stay exactly zero because every block is a combination of masked vectors.
+//
+// Reductions are two-stage with
+// a fixed CTA count and fixed order (bit-reproducible, no float atomics).
+#include "common.cuh"
+#include "device_utils.cuh"
+
+namespace {
+
+template <int KB> struct Tri {
+    static constexpr int NS = 3 * KB;
+    static constexpr int NT = NS * (NS + 1) / 2;   // upper triangle of one matrix
+    static constexpr int NK = KB * (KB + 1) / 2;   // W^T A W block
+    static constexpr int NEU = 2 * NT + KB;        // G_B tri, G_A tri, |r_j|^2
+    __host__ __device__ static constexpr int idx(int i, int j) { return i * NS - i * (i - 1) / 2 + (j - i); }
+};
+
+struct Blk6 { double *X, *W, *P, *AX, *AW, *AP; };
+
+
+// Accumulate the Gram entries of S = [s_0..s_{NS-1}], AS = [a_0..] for one scalar element.
+// skip_waw: leave the (W, AW) block untouched (it comes from K1).
+template <int KB, bool SKIP_WAW>
+__device__ __forceinline__ void gram_accum(const double (&s)[3 * KB], const double (&a)[3 * KB], double (&acc)[Tri<KB>::NEU]) {
+    using T = Tri<KB>;
+#pragma unroll
+    for (int i = 0; i < T::NS; ++i)
+#pragma unroll
+        for (int j = i; j < T::NS; ++j) {
+            acc[T::idx(i, j)] = fma(s[i], s[j], acc[T::idx(i, j)]);
+            const bool waw = (i >= KB && i < 2 * KB && j >= KB && j < 2 * KB);
+            if (SKIP_WAW && waw) continue;
+            // G_A(i,j) = s_i . a_j ; for a W column on the right use the symmetric form a_i . s_j (A W' not known yet)
+            const bool jw = (j >= KB && j < 2 * KB);
+            const double v = (SKIP_WAW && jw) ? a[i] * s[j] : s[i] * a[j];
+            acc[T::NT + T::idx(i, j)] += v;
+        }
+}
+
+template <int NV>
+__device__ __forceinline__ void block_reduce_store(double (&acc)[NV], double* __restrict__ out) {
+    __shared__ double red[8][NV];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        double v = warp_sum(acc[i]);
+        if (lane == 0) red[warp][i] = v;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < NV; i += blockDim.x) {
+        double s = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) s += red[w][i];
+        out[i] = s;
+    }
+}
+
+// ---------------------------------------------------------------- full Gram of the six blocks (start-up only)
+template <int KB>
+__global__ void __launch_bounds__(256) k_gram_tri(long long n3, Blk6 b, double* __restrict__ partials, const int* __restrict__ done) {
+    if (*done) return;
+    using T = Tri<KB>;
+    double acc[T::NEU];
+#pragma unroll
+    for (int i = 0; i < T::NEU; ++i) acc[i] = 0.0;
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n3; e += (long long)gridDim.x * blockDim.x) {
+        double s[T::NS], a[T::NS];
+#pragma unroll
+        for (int i = 0; i < KB; ++i) {
+            s[i] = b.X[i * n3 + e]; s[KB + i] = b.W[i * n3 + e]; s[2 * KB + i] = b.P[i * n3 + e];
+            a[i] = b.AX[i * n3 + e]; a[KB + i] = b.AW[i * n3 + e]; a[2 * KB + i] = b.AP[i * n3 + e];
+        }
+        gram_accum<KB, false>(s, a, acc);
+    }
+    block_reduce_store<T::NEU>(acc, partials + (size_t)blockIdx.x * T::NEU);
+}
+
+// ---------------------------------------------------------------- W^T A W partials (generic-K1 path; the TMA K1 fuses this)
+template <int KB>
+__global__ void __launch_bounds__(256) k_dot_waw(long long n3, const double* __restrict__ W, const double* __restrict__ AW,
+                                                 double* __restrict__ partials, const int* __restrict__ done) {
+    if (*done) return;
+    constexpr int NK = Tri<KB>::NK;
+    double acc[NK];
+#pragma unroll
+    for (int i = 0; i < NK; ++i) acc[i] = 0.0;
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n3; e += (long long)gridDim.x * blockDim.x) {
+        double w[KB], a[KB];
+#pragma unroll
+        for (int i = 0; i < KB; ++i) { w[i] = W[i * n3 + e]; a[i] = AW[i * n3 + e]; }
+        int t = 0;
+#pragma unroll
+        for (int i = 0; i < KB; ++i)
+#pragma unroll
+            for (int j = i; j < KB; ++j) { acc[t] = fma(w[i], a[j], acc[t]); ++t; }
+    }
+    block_reduce_store<NK>(acc, partials + (size_t)blockIdx.x * NK);
+}
+
+// ---------------------------------------------------------------- fused update + residual + next Gram
+// C: [3KB][KB] row-major (rows: X, W, P), theta[KB].  In place on all six blocks.  One thread per site
+// (the three components of a site stay together because W' = P_m R needs m_i . r_i).
+//
+// Why W' must be projected every iteration: a radial component rho of X is mapped by the solver-mode
+// operator to -c_i rho (c_i ~ -12 J), so R carries -(c_i + theta) rho and X'' = C_x X' + C_w W' would
+// multiply rho by (1 + 12 C_w) per iteration -- exponential growth from 1e-16 (seen as a residual that
+// stalls at 1e-9 and then creeps up).  With rad(W') = 0 the radial part of X can only shrink.
+//
+// Gram entries that pair W' with a tangent vector (X', P', AX', AP') use R in place of W' = P_m R
+// (t . P_m r = t . r for tangent t); only W'^T W' needs the correction  r_i.r_j - (m.r_i)(m.r_j).
+template <int KB, bool PROJECT>
+__global__ void __launch_bounds__(256) k_update_fused(long long N, Blk6 b, const double* __restrict__ m,
+                                                      const SolverState* __restrict__ st, double* __restrict__ partials) {
+    if (st->done) return;
+    using T = Tri<KB>;
+    __shared__ double sC[3 * KB * KB + KB];
+    for (int t = threadIdx.x; t < 3 * KB * KB + KB; t += blockDim.x) sC[t] = t < 3 * KB * KB ? st->C[t] : st->theta[t - 3 * KB * KB];
+    __syncthreads();
+    double acc[T::NEU];
+#pragma unroll
+    for (int i = 0; i < T::NEU; ++i) acc[i] = 0.0;
+    const long long n3 = 3 * N;
+    for (long long site = blockIdx.x * (long long)blockDim.x + threadIdx.x; site < N; site += (long long)gridDim.x * blockDim.x) {
+        const long long e0 = 3 * site;
+        double in_s[3][T::NS], in_a[3][T::NS], mm[3];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+#pragma unroll
+            for (int i = 0; i < KB; ++i) {
+                in_s[q][i] = b.X[i * n3 + e0 + q]; in_s[q][KB + i] = b.W[i * n3 + e0 + q]; in_s[q][2 * KB + i] = b.P[i * n3 + e0 + q];
+                in_a[q][i] = b.AX[i * n3 + e0 + q]; in_a[q][KB + i] = b.AW[i * n3 + e0 + q]; in_a[q][2 * KB + i] = b.AP[i * n3 + e0 + q];
+            }
+            mm[q] = PROJECT ? m[e0 + q] : 0.0;
+        }
+        double r[3][KB], dm[KB];
+#pragma unroll
+        for (int j = 0; j < KB; ++j) dm[j] = 0.0;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            double s[T::NS], a[T::NS];
+#pragma unroll
+            for (int j = 0; j < KB; ++j) {
+                double p = 0.0, ap = 0.0;
+#pragma unroll
+                for (int i = KB; i < 3 * KB; ++i) { p = fma(sC[i * KB + j], in_s[q][i], p); ap = fma(sC[i * KB + j], in_a[q][i], ap); }
+                double x = p, ax = ap;
+#pragma unroll
+                for (int i = 0; i < KB; ++i) { x = fma(sC[i * KB + j], in_s[q][i], x); ax = fma(sC[i * KB + j], in_a[q][i], ax); }
+                const double rr = fma(-sC[3 * KB * KB + j], x, ax);
+                s[j] = x; s[KB + j] = rr; s[2 * KB + j] = p;
+                a[j] = ax; a[KB + j] = 0.0; a[2 * KB + j] = ap;
+                r[q][j] = rr;
+                dm[j] = fma(mm[q], rr, dm[j]);
+                acc[2 * T::NT + j] = fma(rr, rr, acc[2 * T::NT + j]);
+                b.X[j * n3 + e0 + q] = x; b.P[j * n3 + e0 + q] = p;
+                b.AX[j * n3 + e0 + q] = ax; b.AP[j * n3 + e0 + q] = ap;
+            }
+            gram_accum<KB, true>(s, a, acc);
+        }
+#pragma unroll
+        for (int i = 0; i < KB; ++i)
+#pragma unroll
+            for (int j = i; j < KB; ++j) acc[T::idx(KB + i, KB + j)] -= dm[i] * dm[j];
+#pragma unroll
+        for (int q = 0; q < 3; ++q)
+#pragma unroll
+            for (int j = 0; j < KB; ++j) b.W[j * n3 + e0 + q] = fma(-dm[j], mm[q], r[q][j]);
+    }
+    block_reduce_store<T::NEU>(acc, partials + (size_t)blockIdx.x * T::NEU);
+}
+
+int fast_grid(long long work_items) {
+    long long b = (work_items + 255) / 256;
+    return (int)(b < 1 ? 1 : (b > MOTO_RED_BLOCKS ? MOTO_RED_BLOCKS : b));
+}
+
+Blk6 blocks_of(moto_ctx* c) { Blk6 b; b.X = c->X; b.W = c->W; b.P = c->P; b.AX = c->AX; b.AW = c->AW; b.AP = c->AP; return b; }
+
+}  // namespace
+
+// ================================================================ host side
+int fast_gram_full(moto_ctx* c, int kb, int* nblk_out) {
+    const long long n3 = 3ll * c->N;
+    const int g = fast_grid(n3);
+    *nblk_out = g;
+    if (kb == 1) k_gram_tri<1><<<g, 256, 0, c->stream>>>(n3, blocks_of(c), c->partials, &c->st->done);
+    else k_gram_tri<2><<<g, 256, 0, c->stream>>>(n3, blocks_of(c), c->partials, &c->st->done);
+    return 1;
+}
+
+int fast_dot_waw(moto_ctx* c, int kb, double* partialsK, int* nblk_out) {
+    const long long n3 = 3ll * c->N;
+    const int g = fast_grid(n3);
+    *nblk_out = g;
+    if (kb == 1) k_dot_waw<1><<<g, 256, 0, c->stream>>>(n3, c->W, c->AW, partialsK, &c->st->done);
+    else k_dot_waw<2><<<g, 256, 0, c->stream>>>(n3, c->W, c->AW, partialsK, &c->st->done);
+    return 1;
+}
+
+int fast_update(moto_ctx* c, const double* m_or_null, int kb, int* nblk_out) {
+    const long long N = c->N;
+    const int g = fast_grid(N);
+    *nblk_out = g;
+    Blk6 b = blocks_of(c);
+    if (kb == 1) {
+        if (m_or_null) k_update_fused<1, true><<<g, 256, 0, c->stream>>>(N, b, m_or_null, c->st, c->partials);
+        else k_update_fused<1, false><<<g, 256, 0, c->stream>>>(N, b, m_or_null, c->st, c->partials);
+    } else {
+        if (m_or_null) k_update_fused<2, true><<<g, 256, 0, c->stream>>>(N, b, m_or_null, c->st, c->partials);
+        else k_update_fused<2, false><<<g, 256, 0, c->stream>>>(N, b, m_or_null, c->st, c->partials);
+    }
+    return 1;
+}

@@ -81,25 +81,80 @@ __device__ void jacobi_eig(double* A, double* V, int n, JacobiScratch* js) {
     __syncthreads();
 }
 
+// vals[e] = sum_b partials[b * stride + e]: warps over entries, lanes over CTAs, shuffle tree => fixed order,
+// every load independent (the serial version of this loop was latency-bound on ~300 dependent L2 reads).
+__device__ void reduce_partials(const double* __restrict__ partials, int nblk, int stride, int ne, double* vals) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int e = warp; e < ne; e += nw) {
+        double s = 0.0;
+        for (int b = lane; b < nblk; b += 32) s += partials[(size_t)b * stride + e];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) vals[e] = s;
+    }
+}
+
+struct RRFast {            // inputs of the fused kb <= 2 path (lobpcg_fast.cu); kb == 0: not used
+    const double* partialsK;   // [nblkK][kb(kb+1)/2]  W^T A W from K1 (NULL: already inside the tri partials)
+    int nblkK;
+    int kb;
+    int check;             // 1: finish the residual norms of the last update and decide convergence first; 2: only that
+    int k;                 // wanted columns
+    double tol;
+};
+
 // mode 0: Rayleigh-Ritz (theta[nev], C[n][nev]);  mode 1: Loewdin orthonormalisation from G_B only (C[n][n])
 __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ partials, int nblk, const double* __restrict__ GA_in,
                                                    const double* __restrict__ GB_in, int n, int nev, double* __restrict__ theta_out,
-                                                   double* __restrict__ C_out, int mode, SolverState* st, double tau) {
+                                                   double* __restrict__ C_out, int mode, SolverState* st, double tau, RRFast fz) {
     if (st && st->done) return;
     __shared__ double A[NMAX * LD], B[NMAX * LD], U[NMAX * LD], M[NMAX * LD], T[NMAX * LD], Z[NMAX * LD];
+    __shared__ double vals[NMAX * 2 * NMAX];
     __shared__ double d[NMAX], sig[NMAX], th[NMAX];
-    __shared__ int keep[NMAX], ord[NMAX], na_s, bad_s;
+    __shared__ int keep[NMAX], ord[NMAX], na_s, bad_s, stop_s;
     __shared__ JacobiScratch js;
     const int tid = threadIdx.x, nt = blockDim.x;
 
     // 1. gather G_A, G_B (from grid-reduction partials, fixed order, or from given matrices); symmetrise
-    if (partials) {
+    if (partials && fz.kb > 0) {
+        // upper triangles [G_B | G_A | |r_j|^2] from k_update_fused / k_gram_tri, W^T A W from K1
+        const int kb = fz.kb, nT = n * (n + 1) / 2, nK = kb * (kb + 1) / 2, neu = 2 * nT + kb;
+        reduce_partials(partials, nblk, neu, neu, vals);
+        if (fz.partialsK) reduce_partials(fz.partialsK, fz.nblkK, nK, nK, vals + neu);
+        if (tid == 0) stop_s = 0;
+        __syncthreads();
+        if (fz.check && tid == 0) {
+            bool ok = true, bad = false;
+            for (int a = 0; a < kb; ++a) {
+                double r = sqrt(vals[2 * nT + a]);
+                st->resid[a] = r;
+                if (a < fz.k) { ok = ok && (r <= fz.tol); bad = bad || !(r == r); }
+            }
+            if (bad) { st->bad = 1; st->done = 1; stop_s = 1; }
+            else if (ok) { st->done = 1; stop_s = 1; }
+            else if (fz.check == 1) st->iter += 1;
+        }
+        __syncthreads();
+        if (stop_s || fz.check == 2) return;
+        for (int t = tid; t < n * n; t += nt) {
+            int i = t / n, j = t - i * n;
+            int a = i < j ? i : j, b = i < j ? j : i;
+            int e = a * n - a * (a - 1) / 2 + (b - a);
+            double ga = vals[nT + e];
+            if (fz.partialsK && a >= kb && b < 2 * kb) {   // (W_a', W_b') block
+                int wa = a - kb, wb = b - kb;
+                ga = vals[neu + wa * kb - wa * (wa - 1) / 2 + (wb - wa)];
+            }
+            U[i * LD + j] = vals[e];
+            T[i * LD + j] = ga;
+        }
+    } else if (partials) {
         const int ntc = 2 * n, ne = n * ntc;
+        reduce_partials(partials, nblk, ne, ne, vals);
+        __syncthreads();
         for (int t = tid; t < 2 * n * n; t += nt) {
             int which = t / (n * n), e = t - which * n * n, i = e / n, j = e - i * n;
-            int src = i * ntc + which * n + j;
-            double s = 0.0;
-            for (int b = 0; b < nblk; ++b) s += partials[(size_t)b * ne + src];
+            double s = vals[i * ntc + which * n + j];
             if (which) T[i * LD + j] = s; else U[i * LD + j] = s;  // U <- raw G_B, T <- raw G_A
         }
     } else {
@@ -203,13 +258,23 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
 int rr_solve(moto_ctx* c, const double* d_GA, const double* d_GB, int n, int nev, double* d_theta, double* d_C, int mode,
              SolverState* st) {
     const double tau = 1e-10;
-    k_rr<<<1, RR_THREADS, 0, c->stream>>>(nullptr, 0, d_GA, d_GB, n, nev, d_theta, d_C, mode, st, tau);
+    RRFast fz = {nullptr, 0, 0, 0, 0, 0.0};
+    k_rr<<<1, RR_THREADS, 0, c->stream>>>(nullptr, 0, d_GA, d_GB, n, nev, d_theta, d_C, mode, st, tau, fz);
     return 1;
 }
 
 // LOBPCG flavour: inputs are the Gram partials left in ctx->partials by block_gram_lobpcg
 int rr_solve_lobpcg(moto_ctx* c, int kb, int nblk) {
     const double tau = 1e-10;
-    k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblk, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau);
+    RRFast fz = {nullptr, 0, 0, 0, 0, 0.0};
+    k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblk, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, fz);
+    return 1;
+}
+
+// fused kb <= 2 path: tri partials [nblkU][2 nT + kb] in ctx->partials, optional W^T A W partials, optional check
+int rr_solve_fast(moto_ctx* c, int kb, int nblkU, const double* partialsK, int nblkK, int check, int k, double tol) {
+    const double tau = 1e-10;
+    RRFast fz = {partialsK, nblkK, kb, check, k, tol};
+    k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblkU, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, fz);
     return 1;
 }
