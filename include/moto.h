@@ -71,7 +71,7 @@ typedef struct {
     int32_t guard;          /* extra block columns iterated but not returned            [0]  */
     int32_t check_every;    /* iterations enqueued between host looks at the status     [8]  */
     int32_t precond_degree; /* degree of the Chebyshev polynomial preconditioner, 0=off [0]  */
-    int32_t reserved;
+    int32_t hvp_path;       /* K1 kernel choice: 0 auto, 1 generic (any lattice), 2 TMA-staged (even Lx >= 8) [0] */
     double precond_lo;      /* preconditioner interval [lo, hi] in units of the shift   [auto] */
     double precond_hi;
     uint64_t seed;          /* seed of the counter-based start block when warm_start=0  [0x9E3779B97F4A7C15] */

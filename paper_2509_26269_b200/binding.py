@@ -41,7 +41,7 @@ class MorseParams(C.Structure):
 
 
 class SolverOpts(C.Structure):
-    _fields_ = [("guard", C.c_int32), ("check_every", C.c_int32), ("precond_degree", C.c_int32), ("reserved", C.c_int32),
+    _fields_ = [("guard", C.c_int32), ("check_every", C.c_int32), ("precond_degree", C.c_int32), ("hvp_path", C.c_int32),
                 ("precond_lo", C.c_double), ("precond_hi", C.c_double), ("seed", C.c_uint64)]
 
 
@@ -163,8 +163,8 @@ class Context:
         except Exception:
             pass
 
-    def set_solver(self, guard=0, check_every=8, precond_degree=0, precond_lo=0.0, precond_hi=0.0, seed=0):
-        o = SolverOpts(guard, check_every, precond_degree, 0, precond_lo, precond_hi, seed)
+    def set_solver(self, guard=0, check_every=8, precond_degree=0, precond_lo=0.0, precond_hi=0.0, seed=0, hvp_path=0):
+        o = SolverOpts(guard, check_every, precond_degree, hvp_path, precond_lo, precond_hi, seed)
         self._check(self.lib.moto_set_solver(self._h, C.byref(o)))
 
     @property

@@ -99,7 +99,7 @@ void moto_destroy(moto_ctx* c) {
 
 moto_status moto_set_solver(moto_ctx* c, const moto_solver_opts* o) {
     if (!c || !o) return MOTO_EINVAL;
-    if (o->guard < 0 || o->check_every < 0 || o->precond_degree < 0) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: negative option");
+    if (o->guard < 0 || o->check_every < 0 || o->precond_degree < 0 || o->hvp_path < 0 || o->hvp_path > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: negative option");
     moto_solver_opts n = *o;
     if (n.check_every == 0) n.check_every = 8;
     if (n.seed == 0) n.seed = 0x9E3779B97F4A7C15ull;

@@ -1,4 +1,417 @@
-// spin_stencil_tma.cu -- TMA-staged fast path of K1 (placeholder until the pipelined kernel lands).
+// spin_stencil_tma.cu -- K1, the TMA-staged fast path of the fused gradient + block Riemannian HVP stencil
+// (Eq. 4; Hv PAPER.md:156; projected-gradient Jacobian PAPER.md:162; reading A5).
+//
+// Design (B200, sm_100a): a persistent grid of one CTA per SM.  The lattice is cut into column strips of
+// <= 60 sites; the (strip, row) space is linearised and split evenly over the CTAs, so every CTA streams
+// one or two vertical strip segments top to bottom.  One producer warp drives the TMA engine: each
+// 8-row chunk of every field (m, V_1..V_K; 64 sites = 60 + halo columns, 1536 B per row) is
+// one cp.async.bulk.tensor box landing in a ring of shared-memory row slots guarded by full/empty
+// mbarriers; the two halo rows of a segment are 1-row boxes, out-of-range coordinates zero-fill (that IS
+// the open boundary), periodic wrap in y is a wrapped row coordinate and periodic wrap in x is a 128-byte
+// side box per row.  Eight consumer warps (2 column halves x 4 row pairs) compute two rows per thread from
+// shared memory, so each site is read from HBM once for all K directions and from shared memory 5x instead
+// of 7x.  Results go straight to global memory; c_i (solver mode) and the Chebyshev operand are read
+// directly (no reuse).  Tensor cores are not used: this is a 7-point stencil, HBM-bound.
+//
+// Modes:  API    (moto_hvp)      HV = P (L Pv) - c Pv with c = m.(Lm - mu B) recomputed, input projected
+//         SOLVER (LOBPCG inner)  HV = P (L v) - c v, c given, v tangent; optional per-CTA partials of
+//                                V^T HV and optional three-term epilogue out = alpha (HV - c0 v) + beta u
+#include <cuda.h>
 #include "common.cuh"
+#include "device_utils.cuh"
+#include "stencil_math.cuh"
 
-int spin_hvp_tma(moto_ctx*, const double*, const double*, const double*, int, double*, int, const int*) { return 0; }
+namespace {
+
+constexpr int TXMAX = 60;          // strip width (sites); row box = 64 sites starting at xb - 2 (see x3 below)
+constexpr int ROWD = 192;          // doubles per main row slot (64 sites x 3)
+constexpr int SIDED = 16;          // doubles per side row slot (128 B)
+constexpr int RC = 8;              // rows per chunk
+constexpr int NCW = 8;             // consumer warps
+constexpr int NTHREADS = (NCW + 1) * 32;
+
+template <int K> struct Cfg {
+    static constexpr int F = K + 1;                                  // fields in the ring: m, V_1..V_K
+    static constexpr int ROW_BYTES = F * (ROWD + 2 * SIDED) * 8;     // one row slot, all fields
+    static constexpr int S = (220 * 1024) / (ROW_BYTES * RC) > 8 ? 8 : (220 * 1024) / (ROW_BYTES * RC);  // stages
+    static constexpr int NSLOT = S * RC;
+    static constexpr int MAIN_D = F * NSLOT * ROWD;                  // doubles
+    static constexpr int SIDE_D = F * NSLOT * SIDED;
+    static constexpr int RED_D = NCW * 4;                            // V^T HV reduction scratch
+    static constexpr size_t SMEM = (size_t)(MAIN_D + 2 * SIDE_D + RED_D) * 8 + 2 * S * 8 + 128;
+    static_assert(S >= 3, "ring too shallow");
+};
+
+struct Maps {  // chunk = RC rows, row = 1 row; main = 64 sites, side = 16 doubles
+    CUtensorMap m_chunk, m_row, m_schunk, m_srow;
+    CUtensorMap v_chunk, v_row, v_schunk, v_srow;
+};
+
+struct KParams {
+    Lat l;
+    int nsx;                 // number of strips
+    long long total;         // nsx * Ly strip-rows
+    const double* m;         // for nothing but alignment of the interface (fields come through TMA)
+    const double* cvec;      // [N] (SOLVER)
+    double* out;             // [K][N][3]
+    const double* U;         // [K][N][3] Chebyshev operand or NULL
+    double alpha, c0, beta;  // out = alpha (HV - c0 v) + beta u   (cheb != 0)
+    int cheb;
+    double* waw;             // [grid][K(K+1)/2] or NULL
+    const int* done;
+};
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
+}
+
+__device__ __forceinline__ int strip_x(int i, int Lx, int nsx) { return 2 * (int)(((long long)i * (Lx >> 1)) / nsx); }
+
+__device__ __forceinline__ d3 lds3(const double* p) { return mk3(p[0], p[1], p[2]); }
+
+// ---------------------------------------------------------------------------------------------------------
+template <int K, bool API>
+__global__ void __launch_bounds__(NTHREADS, 1)
+k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
+    using C = Cfg<K>;
+    constexpr int F = C::F, S = C::S, NSLOT = C::NSLOT;
+    constexpr int NK = K * (K + 1) / 2;
+    if (p.done && *p.done) return;
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double* smain = reinterpret_cast<double*>(smem_raw);          // [F][NSLOT][ROWD]
+    double* sL = smain + C::MAIN_D;                               // [F][NSLOT][SIDED]  site Lx-1 at doubles 13..15
+    double* sR = sL + C::SIDE_D;                                  // [F][NSLOT][SIDED]  site 0 at doubles 0..2
+    double* sred = sR + C::SIDE_D;                                // [NCW][4]
+    uint64_t* full = reinterpret_cast<uint64_t*>(sred + C::RED_D);
+    uint64_t* empty = full + S;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const Lat& l = p.l;
+    const int Lx = l.Lx, Ly = l.Ly;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NCW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const long long lo = (p.total * blockIdx.x) / gridDim.x, hi = (p.total * (blockIdx.x + 1)) / gridDim.x;
+
+    if (warp == NCW) {
+        // ================================================================ producer (one lane drives the TMA engine)
+        if (lane == 0) {
+            unsigned n = 0;
+            long long pos = lo;
+            while (pos < hi) {
+                const int sx = (int)(pos / Ly), y_start = (int)(pos - (long long)sx * Ly);
+                const int nrows = (int)((hi - pos) < (long long)(Ly - y_start) ? (hi - pos) : (Ly - y_start));
+                const int xb = strip_x(sx, Lx, p.nsx), xe = (sx + 1 == p.nsx) ? Lx : strip_x(sx + 1, Lx, p.nsx);
+                const bool edgeL = l.px && xb == 0, edgeR = l.px && xe == Lx;
+                const int f_side0 = API ? 0 : 1;   // first field that needs the x-wrap side boxes
+                const int nside = (edgeL ? 1 : 0) + (edgeR ? 1 : 0);
+                const int Q = (nrows + 2 + RC - 1) / RC;
+                for (int j = 0; j < Q; ++j, ++n) {
+                    const unsigned s = n % S, ph = (n / S) & 1u;
+                    mbar_wait(&empty[s], ph ^ 1u);
+                    const int r0 = j * RC - 1;
+                    const int nvalid = (nrows + 1 - r0) < RC ? (nrows + 1 - r0) : RC;
+                    const int y0 = y_start + r0;
+                    const bool chunk_ok = (nvalid == RC) && (!l.py || (y0 >= 0 && y0 + RC <= Ly));
+                    const unsigned bytes = (unsigned)nvalid * (F * ROWD * 8 + nside * (F - f_side0) * SIDED * 8);
+                    mbar_expect_tx(&full[s], bytes);
+                    // TMA needs a 16-byte aligned box start: the inner coordinate (in doubles) must be even, so the box
+                    // starts two sites left of the (even) strip start: sites xb-2 .. xb+61 = halo at 1, strip at 2..w+1, halo at w+2
+                    const int x3 = 3 * (xb - 2);
+                    if (chunk_ok) {
+#pragma unroll
+                        for (int f = 0; f < F; ++f) {
+                            const CUtensorMap* mp = f == 0 ? &maps.m_chunk : &maps.v_chunk;
+                            tma_load_3d(smain + ((size_t)f * NSLOT + s * RC) * ROWD, mp, &full[s], x3, y0, f == 0 ? 0 : f - 1);
+                            if (f >= f_side0) {
+                                const CUtensorMap* ms = f == 0 ? &maps.m_schunk : &maps.v_schunk;
+                                if (edgeL) tma_load_3d(sL + ((size_t)f * NSLOT + s * RC) * SIDED, ms, &full[s], 3 * Lx - SIDED, y0, f == 0 ? 0 : f - 1);
+                                if (edgeR) tma_load_3d(sR + ((size_t)f * NSLOT + s * RC) * SIDED, ms, &full[s], 0, y0, f == 0 ? 0 : f - 1);
+                            }
+                        }
+                    } else {
+                        for (int i = 0; i < nvalid; ++i) {
+                            int y = y0 + i;
+                            if (l.py) { if (y < 0) y += Ly; else if (y >= Ly) y -= Ly; }
+#pragma unroll
+                            for (int f = 0; f < F; ++f) {
+                                const CUtensorMap* mp = f == 0 ? &maps.m_row : &maps.v_row;
+                                tma_load_3d(smain + ((size_t)f * NSLOT + s * RC + i) * ROWD, mp, &full[s], x3, y, f == 0 ? 0 : f - 1);
+                                if (f >= f_side0) {
+                                    const CUtensorMap* ms = f == 0 ? &maps.m_srow : &maps.v_srow;
+                                    if (edgeL) tma_load_3d(sL + ((size_t)f * NSLOT + s * RC + i) * SIDED, ms, &full[s], 3 * Lx - SIDED, y, f == 0 ? 0 : f - 1);
+                                    if (edgeR) tma_load_3d(sR + ((size_t)f * NSLOT + s * RC + i) * SIDED, ms, &full[s], 0, y, f == 0 ? 0 : f - 1);
+                                }
+                            }
+                        }
+                    }
+                }
+                pos += nrows;
+            }
+        }
+        return;
+    }
+
+    // ==================================================================== consumers
+    const int ch = warp & 1, rp = warp >> 1;
+    const int col = ch * 32 + lane;
+    const long long N = (long long)Lx * Ly;
+    double waw[NK > 0 ? NK : 1];
+#pragma unroll
+    for (int t = 0; t < NK; ++t) waw[t] = 0.0;
+    const d3 muB = mk3(l.mu * l.Bx, l.mu * l.By, l.mu * l.Bz);
+
+    unsigned n = 0;
+    long long pos = lo;
+    while (pos < hi) {
+        const int sx = (int)(pos / Ly), y_start = (int)(pos - (long long)sx * Ly);
+        const int nrows = (int)((hi - pos) < (long long)(Ly - y_start) ? (hi - pos) : (Ly - y_start));
+        const int xb = strip_x(sx, Lx, p.nsx), xe = (sx + 1 == p.nsx) ? Lx : strip_x(sx + 1, Lx, p.nsx);
+        const int w = xe - xb;
+        const bool active = col < w;
+        const bool useL = l.px && xb == 0 && col == 0;        // left neighbour comes from the wrap side box
+        const bool useR = l.px && xe == Lx && col == w - 1;   // right neighbour comes from the wrap side box
+        // per-thread column bases (in doubles) and row pitches of the three columns x-1, x, x+1
+        const double* baseL = useL ? sL + 13 : smain + 3 * (col + 1);
+        const double* baseC = smain + 3 * (col + 2);
+        const double* baseR = useR ? sR : smain + 3 * (col + 3);
+        const int pitchL = useL ? SIDED : ROWD, pitchR = useR ? SIDED : ROWD;
+        const int fstrL = useL ? NSLOT * SIDED : NSLOT * ROWD, fstrR = useR ? NSLOT * SIDED : NSLOT * ROWD;
+        const int x = xb + col;
+        const int Q = (nrows + 2 + RC - 1) / RC, nb = (nrows + RC - 1) / RC;
+
+        mbar_wait(&full[n % S], (n / S) & 1u);
+        for (int j = 0; j < nb; ++j) {
+            if (j + 1 < Q) mbar_wait(&full[(n + j + 1) % S], ((n + j + 1) / S) & 1u);
+            const int rA = j * RC + 2 * rp;
+            if (active && rA < nrows) {
+                const bool haveB = rA + 1 < nrows;
+                int slot[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int rr = rA + q;   // = (row index r) + 1, r = rA - 1 + q
+                    slot[q] = (int)((n + rr / RC) % S) * RC + (rr % RC);
+                }
+                const long long siteA = (long long)(y_start + rA) * Lx + x, siteB = siteA + Lx;
+                double cA = 0.0, cB = 0.0;
+                if (!API) { cA = p.cvec[siteA]; if (haveB) cB = p.cvec[siteB]; }
+                // field 0: m.  API: all ten sites (projection of the neighbours + stencil for c); SOLVER: centres only.
+                d3 m0C, m0R, m1L, m1C, m1R, m2L, m2C, m2R, m3L, m3C;
+                m1C = lds3(baseC + slot[1] * ROWD);
+                m2C = lds3(baseC + slot[2] * ROWD);
+                if (API) {
+                    m0C = lds3(baseC + slot[0] * ROWD); m0R = lds3(baseR + slot[0] * pitchR);
+                    m1L = lds3(baseL + slot[1] * pitchL); m1R = lds3(baseR + slot[1] * pitchR);
+                    m2L = lds3(baseL + slot[2] * pitchL); m2R = lds3(baseR + slot[2] * pitchR);
+                    m3L = lds3(baseL + slot[3] * pitchL); m3C = lds3(baseC + slot[3] * ROWD);
+                    const d3 LmA = stencil_apply(l, m1R, m1L, m2C, m0C, m2L, m0R, m1C.z);
+                    const d3 LmB = stencil_apply(l, m2R, m2L, m3C, m1C, m3L, m1R, m2C.z);
+                    cA = dot3(m1C, LmA) - dot3(m1C, muB);
+                    cB = dot3(m2C, LmB) - dot3(m2C, muB);
+                }
+                d3 vA[K], hA[K], vB[K], hB[K];
+#pragma unroll
+                for (int a = 0; a < K; ++a) {
+                    const int f = a + 1;
+                    const double* bL = baseL + f * fstrL;
+                    const double* bC = baseC + f * NSLOT * ROWD;
+                    const double* bR = baseR + f * fstrR;
+                    d3 u0C = lds3(bC + slot[0] * ROWD), u0R = lds3(bR + slot[0] * pitchR);
+                    d3 u1L = lds3(bL + slot[1] * pitchL), u1C = lds3(bC + slot[1] * ROWD), u1R = lds3(bR + slot[1] * pitchR);
+                    d3 u2L = lds3(bL + slot[2] * pitchL), u2C = lds3(bC + slot[2] * ROWD), u2R = lds3(bR + slot[2] * pitchR);
+                    d3 u3L = lds3(bL + slot[3] * pitchL), u3C = lds3(bC + slot[3] * ROWD);
+                    if (API) {
+                        u0C = proj3(m0C, u0C); u0R = proj3(m0R, u0R);
+                        u1L = proj3(m1L, u1L); u1C = proj3(m1C, u1C); u1R = proj3(m1R, u1R);
+                        u2L = proj3(m2L, u2L); u2C = proj3(m2C, u2C); u2R = proj3(m2R, u2R);
+                        u3L = proj3(m3L, u3L); u3C = proj3(m3C, u3C);
+                    }
+                    const d3 LA = stencil_apply(l, u1R, u1L, u2C, u0C, u2L, u0R, u1C.z);
+                    const d3 LB = stencil_apply(l, u2R, u2L, u3C, u1C, u3L, u1R, u2C.z);
+                    vA[a] = u1C; vB[a] = u2C;
+                    hA[a] = axpy3(-cA, u1C, proj3(m1C, LA));
+                    hB[a] = axpy3(-cB, u2C, proj3(m2C, LB));
+                }
+                if (NK > 0 && p.waw) {
+                    int t = 0;
+#pragma unroll
+                    for (int a = 0; a < K; ++a)
+#pragma unroll
+                        for (int b = a; b < K; ++b) {
+                            waw[t] += dot3(vA[a], hA[b]);
+                            if (haveB) waw[t] += dot3(vB[a], hB[b]);
+                            ++t;
+                        }
+                }
+#pragma unroll
+                for (int a = 0; a < K; ++a) {
+                    d3 oA = hA[a], oB = hB[a];
+                    if (p.cheb) {
+                        oA = scale3(p.alpha, axpy3(-p.c0, vA[a], oA));
+                        oB = scale3(p.alpha, axpy3(-p.c0, vB[a], oB));
+                        if (p.U) {
+                            oA = axpy3(p.beta, ld3(p.U + (size_t)a * 3 * N, siteA), oA);
+                            if (haveB) oB = axpy3(p.beta, ld3(p.U + (size_t)a * 3 * N, siteB), oB);
+                        }
+                    }
+                    st3(p.out + (size_t)a * 3 * N, siteA, oA);
+                    if (haveB) st3(p.out + (size_t)a * 3 * N, siteB, oB);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[(n + j) % S]);
+        }
+        if (Q > nb) { __syncwarp(); if (lane == 0) mbar_arrive(&empty[(n + nb) % S]); }
+        n += Q;
+        pos += nrows;
+    }
+
+    if (NK > 0 && p.waw) {  // fixed-order reduction over the 256 consumer threads (named barrier 1: the producer warp has left)
+#pragma unroll
+        for (int t = 0; t < NK; ++t) {
+            const double v = warp_sum(waw[t]);
+            if (lane == 0) sred[warp * 4 + t] = v;
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");
+        if (threadIdx.x < NK) {
+            double s = 0.0;
+            for (int wv = 0; wv < NCW; ++wv) s += sred[wv * 4 + threadIdx.x];
+            p.waw[(size_t)blockIdx.x * NK + threadIdx.x] = s;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)f;
+    }
+    return fn;
+}
+
+// field array [nvec][Ly][3 Lx] fp64 as a 3-D tensor; box = {inner doubles, rows, 1}
+bool encode(CUtensorMap* map, const double* base, int Lx, int Ly, int nvec, int inner, int rows) {
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return false;
+    cuuint64_t gdim[3] = {(cuuint64_t)3 * Lx, (cuuint64_t)Ly, (cuuint64_t)nvec};
+    cuuint64_t gstr[2] = {(cuuint64_t)24 * Lx, (cuuint64_t)24 * Lx * Ly};
+    cuuint32_t box[3] = {(cuuint32_t)inner, (cuuint32_t)rows, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int K, bool API>
+bool launch(moto_ctx* c, const Maps& maps, const KParams& p, int grid) {
+    using C = Cfg<K>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(k_hvp_tma<K, API>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return false;
+        attr_set = true;
+    }
+    k_hvp_tma<K, API><<<grid, NTHREADS, C::SMEM, c->stream>>>(maps, p);
+    return true;
+}
+
+}  // namespace
+
+bool spin_tma_applicable(const moto_ctx* c) {
+    if (c->kind != MOTO_KIND_TRI2D) return false;
+    const int Lx = c->lat.Lx, Ly = c->lat.Ly;
+    if (c->opts.hvp_path == 1) return false;                  // hvp_path = generic
+    if ((Lx & 1) || Lx < 8 || Ly < 1) return false;          // row stride 24 Lx must be a multiple of 16 B; side box needs 16 doubles
+    if (c->opts.hvp_path == 2) return true;                   // hvp_path = tma (forced, tests)
+    return (long long)Lx * Ly >= 16384;                       // small lattices are launch-latency bound: generic kernel
+}
+
+int spin_tma_grid(const moto_ctx* c) {
+    const int Lx = c->lat.Lx, Ly = c->lat.Ly;
+    const int nsx = (Lx + TXMAX - 1) / TXMAX;
+    const long long total = (long long)nsx * Ly;
+    long long g = (total + RC - 1) / RC;
+    return (int)(g > MOTO_NUM_SMS ? MOTO_NUM_SMS : (g < 1 ? 1 : g));
+}
+
+// Extended entry: SOLVER mode when cvec != NULL (input must be tangent), API mode otherwise.
+// waw_partials: optional [spin_tma_grid][k(k+1)/2].  cheb: out = alpha (HV - c0 V) + beta U (U may be NULL).
+// Returns the number of kernels launched, 0 if the path does not apply (caller falls back), -1 on error.
+int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV, const int* d_done,
+                    double* waw_partials, int cheb, double alpha, double c0, double beta, const double* U) {
+    if (!spin_tma_applicable(c)) return 0;
+    if (((uintptr_t)m & 15) || ((uintptr_t)V & 15)) return 0;
+    if (waw_partials && k > 2) return 0;
+    const int Lx = c->lat.Lx, Ly = c->lat.Ly;
+    const size_t bs = (size_t)3 * c->N;
+    int launches = 0;
+    for (int a0 = 0; a0 < k; a0 += 2) {
+        const int kk = (k - a0) >= 2 ? 2 : 1;
+        Maps maps;
+        bool ok = encode(&maps.m_chunk, m, Lx, Ly, 1, ROWD, RC) && encode(&maps.m_row, m, Lx, Ly, 1, ROWD, 1) &&
+                  encode(&maps.m_schunk, m, Lx, Ly, 1, SIDED, RC) && encode(&maps.m_srow, m, Lx, Ly, 1, SIDED, 1) &&
+                  encode(&maps.v_chunk, V + a0 * bs, Lx, Ly, kk, ROWD, RC) && encode(&maps.v_row, V + a0 * bs, Lx, Ly, kk, ROWD, 1) &&
+                  encode(&maps.v_schunk, V + a0 * bs, Lx, Ly, kk, SIDED, RC) && encode(&maps.v_srow, V + a0 * bs, Lx, Ly, kk, SIDED, 1);
+        if (!ok) return launches ? -1 : 0;
+        KParams p;
+        p.l = make_lat(c);
+        p.nsx = (Lx + TXMAX - 1) / TXMAX;
+        p.total = (long long)p.nsx * Ly;
+        p.m = m; p.cvec = cvec; p.out = HV + a0 * bs;
+        p.U = U ? U + a0 * bs : nullptr;
+        p.alpha = alpha; p.c0 = c0; p.beta = beta; p.cheb = cheb;
+        p.waw = waw_partials; p.done = d_done;
+        const int grid = spin_tma_grid(c);
+        bool l_ok;
+        if (cvec) l_ok = kk == 2 ? launch<2, false>(c, maps, p, grid) : launch<1, false>(c, maps, p, grid);
+        else l_ok = kk == 2 ? launch<2, true>(c, maps, p, grid) : launch<1, true>(c, maps, p, grid);
+        if (!l_ok) return launches ? -1 : 0;
+        ++launches;
+    }
+    return launches;
+}
+
+int spin_hvp_tma(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input,
+                 const int* d_done) {
+    // the two combinations the library uses: (no c, project) = API, (c, no project) = SOLVER
+    if ((cvec != nullptr) == (project_input != 0)) return 0;
+    int n = spin_hvp_tma_ex(c, m, cvec, V, k, HV, d_done, nullptr, 0, 0.0, 0.0, 0.0, nullptr);
+    return n < 0 ? 0 : n;
+}

@@ -70,6 +70,58 @@ def test_hvp_parity(moto, case, k):
     assert np.max(np.abs(np.sum(HV * w.spins[None], axis=2))) <= 1e-12   # tangent output
 
 
+# lattices for the TMA-staged K1 path (even Lx >= 8), forced on with hvp_path=2 so that oracle-sized cases run it:
+# several strips + ragged last strip, every boundary combination, segments shorter than a chunk, tiny Ly.
+TMA_CASES = [
+    lambda: wl.config0(),                 # 8x8 periodic: one strip, both wrap side boxes, Ly == chunk
+    lambda: wl.config1(),                 # 70x70 periodic: two strips
+    lambda: custom(64, 50, 1, 0, 2),      # periodic x, open y
+    lambda: custom(130, 70, 0, 1, 3),     # open x, periodic y, three strips
+    lambda: custom(126, 41, 0, 0, 6),     # open, strip boundary at a multiple of 62 + 2
+    lambda: custom(200, 9, 1, 1, 7),      # rows barely more than one chunk
+    lambda: custom(62, 3, 1, 1, 8),       # Ly = 3: wrapped halo rows alias the segment's own rows
+    lambda: custom(10, 2, 1, 1, 9),       # Ly = 2
+    lambda: custom(250, 130, 1, 1, 10),   # > 148 segments' worth of work: CTAs span strip boundaries
+    lambda: wl.config3_scaled(100),
+]
+
+
+@pytest.mark.parametrize("case", range(len(TMA_CASES)))
+@pytest.mark.parametrize("k", [1, 2, 3, 6])
+def test_hvp_tma_parity(moto, case, k):
+    w = TMA_CASES[case]()
+    model = model_of(w)
+    ctx = moto.spin_context(w, kmax=8)
+    ctx.set_solver(hvp_path=2)
+    V = wl.random_block(w.N, k, seed=200 + case)
+    HV = ctx.hvp(dev(w.spins), dev(V)).cpu().numpy()
+    ref = so.hvp(model, w.spins, V)
+    assert rel_l2(HV, ref) <= HVP_TOL
+    assert np.max(np.abs(np.sum(HV * w.spins[None], axis=2))) <= 1e-12
+    # generic path on the same input: the two CUDA kernels agree to rounding
+    ctx.set_solver(hvp_path=1)
+    HV1 = ctx.hvp(dev(w.spins), dev(V)).cpu().numpy()
+    assert rel_l2(HV, HV1) <= 1e-13
+
+
+@pytest.mark.parametrize("case", [0, 1, 2, 3, 5, 8])
+def test_lowest_modes_tma_path(moto, case):
+    # solver mode of the TMA kernel (c given, fused V^T HV partials) inside the LOBPCG
+    w = TMA_CASES[case]()
+    if w.N > 12000:
+        pytest.skip("dense oracle too large")
+    lam_ref, V_ref = so.lowest_modes(model_of(w), w.spins, 2, extra=1)
+    ctx = moto.spin_context(w)
+    ctx.set_solver(hvp_path=2)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=4000)
+    assert info["converged"], info
+    lam = lam.cpu().numpy()
+    assert np.max(np.abs(lam - lam_ref[:2]) / np.maximum(np.abs(lam_ref[:2]), 1e-3)) <= EIG_TOL
+    if lam_ref[2] - lam_ref[1] > 1e-3:
+        ang = scipy.linalg.subspace_angles(V.cpu().numpy().reshape(2, -1).T, V_ref[:2].reshape(2, -1).T)
+        assert ang.max() <= ANGLE_TOL
+
+
 def test_hvp_kmax_and_arg_errors(moto):
     w = wl.config0()
     ctx = moto.spin_context(w, kmax=8)
