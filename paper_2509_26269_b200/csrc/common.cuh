@@ -94,6 +94,11 @@ int spin_hvp(moto_ctx*, const double* m, const double* c_or_null, const double* 
              int project_input, const int* d_done);
 int spin_mmf_step(moto_ctx*, const double* m, const double* v, int kr, double dt, double* m_out, double* d_fnorm);
 int spin_project(moto_ctx*, const double* m, double* V, int k);
+// spin_stencil_tma.cu
+bool spin_tma_applicable(const moto_ctx*);
+int spin_tma_grid(const moto_ctx*);
+int spin_hvp_tma_ex(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double* HV, const int* d_done,
+                    double* waw_partials, int cheb, double alpha, double c0, double beta, const double* U);
 // cart_morse.cu
 int cart_build_lists(moto_ctx*, const double* x);
 int cart_energy_grad(moto_ctx*, const double* x, double* d_E, double* d_g);

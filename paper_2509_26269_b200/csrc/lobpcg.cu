@@ -69,8 +69,13 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     while (!finished) {
         int batch = max_iter - enq < check_every ? max_iter - enq : check_every;
         for (int b = 0; b < batch; ++b) {
-            n += apply_operator(c, d_state, c->W, kb, c->AW);
-            n += fast_dot_waw(c, kb, partialsK, &nblkK);
+            // AW = Hess[W] with the W^T AW partials fused into the TMA kernel's epilogue when that path applies
+            int nk = (c->kind == MOTO_KIND_TRI2D) ? spin_hvp_tma_ex(c, d_state, c->c, c->W, kb, c->AW, &c->st->done, partialsK, 0, 0.0, 0.0, 0.0, nullptr) : 0;
+            if (nk > 0) { n += nk; nblkK = spin_tma_grid(c); }
+            else {
+                n += apply_operator(c, d_state, c->W, kb, c->AW);
+                n += fast_dot_waw(c, kb, partialsK, &nblkK);
+            }
             n += rr_solve_fast(c, kb, nblkU, partialsK, nblkK, /*check=*/1, k, tol);
             n += fast_update(c, m_proj, kb, &nblkU);
         }

@@ -12,28 +12,28 @@ namespace {
 
 constexpr int NMAX = MOTO_NS;       // 24
 constexpr int LD = NMAX + 1;        // smem leading dimension
-constexpr int RR_THREADS = 128;
+constexpr int RR_THREADS = 256;     // gather phase; the dense phase runs on warp 0 alone (warp-level syncs only)
+#define RR_SYNC() __syncwarp()
 
 struct JacobiScratch { int p[NMAX / 2], q[NMAX / 2]; double c[NMAX / 2], s[NMAX / 2]; double off, diag; };
 
 // Symmetric eigen-decomposition in shared memory: A (n x n, LD) -> diag(A) = eigenvalues, V = eigenvectors (cols).
 __device__ void jacobi_eig(double* A, double* V, int n, JacobiScratch* js) {
-    const int tid = threadIdx.x, nt = blockDim.x;
+    const int tid = threadIdx.x, nt = 32;   // called by warp 0 only
     for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; V[i * LD + j] = (i == j) ? 1.0 : 0.0; }
-    __syncthreads();
+    RR_SYNC();
     if (n == 1) return;
     const int np = (n + 1) & ~1, half = np / 2;
     for (int sweep = 0; sweep < 30; ++sweep) {
-        if (tid == 0) {
-            double off = 0.0, dg = 0.0;
-            for (int i = 0; i < n; ++i) {
-                dg += A[i * LD + i] * A[i * LD + i];
-                for (int j = i + 1; j < n; ++j) off += A[i * LD + j] * A[i * LD + j];
-            }
-            js->off = off; js->diag = dg;
+        double off = 0.0, dg = 0.0;
+        for (int t = tid; t < n * n; t += nt) {
+            int i = t / n, j = t - i * n;
+            double a = A[i * LD + j];
+            if (i == j) dg += a * a; else if (j > i) off += a * a;
         }
-        __syncthreads();
-        if (js->off <= 1e-32 * js->diag || js->off == 0.0) break;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { off += __shfl_xor_sync(0xffffffffu, off, o); dg += __shfl_xor_sync(0xffffffffu, dg, o); }
+        if (off <= 1e-30 * dg || off == 0.0) break;   // off-diagonals below 1e-15 of the diagonal scale: rounding level
         for (int r = 0; r < np - 1; ++r) {
             if (tid < half) {
                 int p, q;
@@ -53,7 +53,7 @@ __device__ void jacobi_eig(double* A, double* V, int n, JacobiScratch* js) {
                 } else { p = -1; }
                 js->p[tid] = p; js->q[tid] = q; js->c[tid] = c; js->s[tid] = s;
             }
-            __syncthreads();
+            RR_SYNC();
             // columns: A <- A J, V <- V J
             for (int w = tid; w < half * n; w += nt) {
                 int t = w / n, i = w - t * n, p = js->p[t], q = js->q[t];
@@ -64,7 +64,7 @@ __device__ void jacobi_eig(double* A, double* V, int n, JacobiScratch* js) {
                 double vip = V[i * LD + p], viq = V[i * LD + q];
                 V[i * LD + p] = c * vip - s * viq; V[i * LD + q] = s * vip + c * viq;
             }
-            __syncthreads();
+            RR_SYNC();
             // rows: A <- J^T A
             for (int w = tid; w < half * n; w += nt) {
                 int t = w / n, j = w - t * n, p = js->p[t], q = js->q[t];
@@ -73,24 +73,42 @@ __device__ void jacobi_eig(double* A, double* V, int n, JacobiScratch* js) {
                 double apj = A[p * LD + j], aqj = A[q * LD + j];
                 A[p * LD + j] = c * apj - s * aqj; A[q * LD + j] = s * apj + c * aqj;
             }
-            __syncthreads();
+            RR_SYNC();
             if (tid < half && js->p[tid] >= 0) { int p = js->p[tid], q = js->q[tid]; A[p * LD + q] = 0.0; A[q * LD + p] = 0.0; }
-            __syncthreads();
+            RR_SYNC();
         }
     }
-    __syncthreads();
+    RR_SYNC();
 }
 
-// vals[e] = sum_b partials[b * stride + e]: warps over entries, lanes over CTAs, shuffle tree => fixed order,
-// every load independent (the serial version of this loop was latency-bound on ~300 dependent L2 reads).
-__device__ void reduce_partials(const double* __restrict__ partials, int nblk, int stride, int ne, double* vals) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    for (int e = warp; e < ne; e += nw) {
-        double s = 0.0;
-        for (int b = lane; b < nblk; b += 32) s += partials[(size_t)b * stride + e];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (lane == 0) vals[e] = s;
+// vals[e] = sum_b partials[b * stride + e] in a fixed order with every load independent (the serial version of
+// this loop was latency-bound on ~300 dependent L2 reads).  Thread (g, e) sums the CTAs b = g, g+G, ... with four
+// interleaved accumulators; the G group sums are then added in order.  scratch: >= G * ne doubles of smem.
+__device__ void reduce_partials(const double* __restrict__ partials, int nblk, int stride, int ne, double* vals, double* scratch) {
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int G = (ne <= 64) ? nt / 64 : 1, ne_g = (G > 1) ? 64 : ne;
+    for (int idx = tid; idx < ne_g * G; idx += nt) {
+        const int g = idx / ne_g, e = idx - g * ne_g;
+        if (e >= ne) continue;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        int b = g;
+        for (; b + 3 * G < nblk; b += 4 * G) {
+            a0 += partials[(size_t)b * stride + e];
+            a1 += partials[(size_t)(b + G) * stride + e];
+            a2 += partials[(size_t)(b + 2 * G) * stride + e];
+            a3 += partials[(size_t)(b + 3 * G) * stride + e];
+        }
+        for (; b < nblk; b += G) a0 += partials[(size_t)b * stride + e];
+        const double sum = (a0 + a1) + (a2 + a3);
+        if (G > 1) scratch[g * ne + e] = sum; else vals[e] = sum;
+    }
+    if (G > 1) {
+        __syncthreads();
+        for (int e = tid; e < ne; e += nt) {
+            double sum = 0.0;
+            for (int g = 0; g < G; ++g) sum += scratch[g * ne + e];
+            vals[e] = sum;
+        }
     }
 }
 
@@ -113,14 +131,15 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
     __shared__ double d[NMAX], sig[NMAX], th[NMAX];
     __shared__ int keep[NMAX], ord[NMAX], na_s, bad_s, stop_s;
     __shared__ JacobiScratch js;
-    const int tid = threadIdx.x, nt = blockDim.x;
+    const int tid = threadIdx.x;
+    int nt = blockDim.x;
 
     // 1. gather G_A, G_B (from grid-reduction partials, fixed order, or from given matrices); symmetrise
     if (partials && fz.kb > 0) {
         // upper triangles [G_B | G_A | |r_j|^2] from k_update_fused / k_gram_tri, W^T A W from K1
         const int kb = fz.kb, nT = n * (n + 1) / 2, nK = kb * (kb + 1) / 2, neu = 2 * nT + kb;
-        reduce_partials(partials, nblk, neu, neu, vals);
-        if (fz.partialsK) reduce_partials(fz.partialsK, fz.nblkK, nK, nK, vals + neu);
+        reduce_partials(partials, nblk, neu, neu, vals, Z);
+        if (fz.partialsK) { __syncthreads(); reduce_partials(fz.partialsK, fz.nblkK, nK, nK, vals + neu, Z); }
         if (tid == 0) stop_s = 0;
         __syncthreads();
         if (fz.check && tid == 0) {
@@ -150,7 +169,7 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         }
     } else if (partials) {
         const int ntc = 2 * n, ne = n * ntc;
-        reduce_partials(partials, nblk, ne, ne, vals);
+        reduce_partials(partials, nblk, ne, ne, vals, Z);
         __syncthreads();
         for (int t = tid; t < 2 * n * n; t += nt) {
             int which = t / (n * n), e = t - which * n * n, i = e / n, j = e - i * n;
@@ -171,6 +190,9 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         A[i * LD + j] = 0.5 * (T[i * LD + j] + T[j * LD + i]);
     }
     __syncthreads();
+    // ---- dense phase: warp 0 alone, warp-level synchronisation only
+    if (tid >= 32) return;
+    nt = 32;
     if (st && partials) {  // keep a copy for diagnostics
         for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; st->GA[t] = A[i * LD + j]; st->GB[t] = B[i * LD + j]; }
     }
@@ -180,9 +202,9 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         d[tid] = (bii > 1e-300) ? rsqrt(bii) : 0.0;
     }
     if (tid == 0) bad_s = 0;
-    __syncthreads();
+    RR_SYNC();
     for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; B[i * LD + j] *= d[i] * d[j]; }
-    __syncthreads();
+    RR_SYNC();
     // 3. eigen-decomposition of the scaled G_B
     jacobi_eig(B, U, n, &js);
     if (tid == 0) {
@@ -193,14 +215,14 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         na_s = na;
         if (!(smax == smax)) bad_s = 1;
     }
-    __syncthreads();
+    RR_SYNC();
     const int na = na_s;
     // M = D U_keep Sigma^{-1/2}   (n x na)
     for (int t = tid; t < n * na; t += nt) {
         int i = t / na, l = t - i * na, j = keep[l];
         M[i * LD + l] = d[i] * U[i * LD + j] * rsqrt(sig[j]);
     }
-    __syncthreads();
+    RR_SYNC();
     if (mode == 1) {
         // Loewdin: C = M (U_keep)^T D^{-1}... applied to the ORIGINAL vectors: C = D U S^{-1/2} U^T  (n x n)
         for (int t = tid; t < n * n; t += nt) {
@@ -219,16 +241,16 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         for (int j = 0; j < n; ++j) s += A[i * LD + j] * M[j * LD + l];
         T[i * LD + l] = s;
     }
-    __syncthreads();
+    RR_SYNC();
     for (int t = tid; t < na * na; t += nt) {
         int a = t / na, b = t - a * na;
         double s = 0.0;
         for (int i = 0; i < n; ++i) s += M[i * LD + a] * T[i * LD + b];
         B[a * LD + b] = s;
     }
-    __syncthreads();
+    RR_SYNC();
     for (int t = tid; t < na * na; t += nt) { int a = t / na, b = t - a * na; A[a * LD + b] = 0.5 * (B[a * LD + b] + B[b * LD + a]); }
-    __syncthreads();
+    RR_SYNC();
     jacobi_eig(A, Z, na, &js);
     // 5. sort ascending
     if (tid == 0) {
@@ -241,7 +263,7 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         if (na < nev) bad_s = 1;
         for (int a = 0; a < nev && a < na; ++a) if (!(th[ord[a]] == th[ord[a]])) bad_s = 1;
     }
-    __syncthreads();
+    RR_SYNC();
     // 6. C = M Z[:, lowest nev]
     for (int t = tid; t < n * nev; t += nt) {
         int i = t / nev, j = t - i * nev;

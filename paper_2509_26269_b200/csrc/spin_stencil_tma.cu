@@ -3,7 +3,8 @@
 //
 // Design (B200, sm_100a): a persistent grid of one CTA per SM.  The lattice is cut into column strips of
 // <= 60 sites; the (strip, row) space is linearised and split evenly over the CTAs, so every CTA streams
-// one or two vertical strip segments top to bottom.  One producer warp drives the TMA engine: each
+// one or two vertical strip segments top to bottom.  One producer warp drives the TMA engine (its 32 lanes
+// issue the boxes of a stage in parallel): each
 // 8-row chunk of every field (m, V_1..V_K; 64 sites = 60 + halo columns, 1536 B per row) is
 // one cp.async.bulk.tensor box landing in a ring of shared-memory row slots guarded by full/empty
 // mbarriers; the two halo rows of a segment are 1-row boxes, out-of-range coordinates zero-fill (that IS
@@ -30,21 +31,29 @@ constexpr int RC = 8;              // rows per chunk
 constexpr int NCW = 8;             // consumer warps
 constexpr int NTHREADS = (NCW + 1) * 32;
 
-template <int K> struct Cfg {
+constexpr int CROWD = 64;          // doubles per c row slot (SOLVER mode: c_i rides the ring too)
+constexpr int SMEM_BUDGET = 231 * 1024;
+
+template <int K, bool API> struct Cfg {
     static constexpr int F = K + 1;                                  // fields in the ring: m, V_1..V_K
-    static constexpr int ROW_BYTES = F * (ROWD + 2 * SIDED) * 8;     // one row slot, all fields
-    static constexpr int S = (220 * 1024) / (ROW_BYTES * RC) > 8 ? 8 : (220 * 1024) / (ROW_BYTES * RC);  // stages
+    static constexpr int FS0 = API ? 0 : 1;                          // first field with x-wrap side boxes (SOLVER: m needs none)
+    static constexpr int NFS = F - FS0;
+    static constexpr int ROW_BYTES = (F * ROWD + 2 * NFS * SIDED + (API ? 0 : CROWD)) * 8;   // one row slot, everything
+    static constexpr int S = SMEM_BUDGET / (ROW_BYTES * RC) > 8 ? 8 : SMEM_BUDGET / (ROW_BYTES * RC);  // stages
     static constexpr int NSLOT = S * RC;
     static constexpr int MAIN_D = F * NSLOT * ROWD;                  // doubles
-    static constexpr int SIDE_D = F * NSLOT * SIDED;
+    static constexpr int SIDE_D = NFS * NSLOT * SIDED;
+    static constexpr int C_D = API ? 0 : NSLOT * CROWD;
     static constexpr int RED_D = NCW * 4;                            // V^T HV reduction scratch
-    static constexpr size_t SMEM = (size_t)(MAIN_D + 2 * SIDE_D + RED_D) * 8 + 2 * S * 8 + 128;
+    static constexpr size_t SMEM = (size_t)(MAIN_D + 2 * SIDE_D + C_D + RED_D) * 8 + 2 * S * 8;
     static_assert(S >= 3, "ring too shallow");
+    static_assert(SMEM <= 232448, "over the 227 KB per-CTA limit");
 };
 
 struct Maps {  // chunk = RC rows, row = 1 row; main = 64 sites, side = 16 doubles
     CUtensorMap m_chunk, m_row, m_schunk, m_srow;
     CUtensorMap v_chunk, v_row, v_schunk, v_srow;
+    CUtensorMap c_chunk, c_row;   // c [1][Ly][Lx] fp64, box 64 wide (SOLVER)
 };
 
 struct KParams {
@@ -59,6 +68,9 @@ struct KParams {
     int cheb;
     double* waw;             // [grid][K(K+1)/2] or NULL
     const int* done;
+#ifdef MOTO_K1_TIMING
+    unsigned long long* dbg;   // [grid][4]: smid, t_start, t_first_data, t_end (globaltimer ns)
+#endif
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -96,16 +108,17 @@ __device__ __forceinline__ d3 lds3(const double* p) { return mk3(p[0], p[1], p[2
 template <int K, bool API>
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
-    using C = Cfg<K>;
-    constexpr int F = C::F, S = C::S, NSLOT = C::NSLOT;
+    using C = Cfg<K, API>;
+    constexpr int F = C::F, S = C::S, NSLOT = C::NSLOT, FS0 = C::FS0, NFS = C::NFS;
     constexpr int NK = K * (K + 1) / 2;
     if (p.done && *p.done) return;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* smain = reinterpret_cast<double*>(smem_raw);          // [F][NSLOT][ROWD]
-    double* sL = smain + C::MAIN_D;                               // [F][NSLOT][SIDED]  site Lx-1 at doubles 13..15
-    double* sR = sL + C::SIDE_D;                                  // [F][NSLOT][SIDED]  site 0 at doubles 0..2
-    double* sred = sR + C::SIDE_D;                                // [NCW][4]
+    double* sL = smain + C::MAIN_D;                               // [NFS][NSLOT][SIDED]  site Lx-1 at doubles 13..15
+    double* sR = sL + C::SIDE_D;                                  // [NFS][NSLOT][SIDED]  site 0 at doubles 0..2
+    double* sc = sR + C::SIDE_D;                                  // [NSLOT][CROWD]       c_i (SOLVER)
+    double* sred = sc + C::C_D;                                   // [NCW][4]
     uint64_t* full = reinterpret_cast<uint64_t*>(sred + C::RED_D);
     uint64_t* empty = full + S;
 
@@ -120,62 +133,65 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     __syncthreads();
 
     const long long lo = (p.total * blockIdx.x) / gridDim.x, hi = (p.total * (blockIdx.x + 1)) / gridDim.x;
+#ifdef MOTO_K1_TIMING
+    if (threadIdx.x == 0) {
+        unsigned long long t; unsigned sm;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
+        p.dbg[blockIdx.x * 4 + 0] = sm; p.dbg[blockIdx.x * 4 + 1] = t;
+    }
+#endif
 
     if (warp == NCW) {
-        // ================================================================ producer (one lane drives the TMA engine)
-        if (lane == 0) {
-            unsigned n = 0;
-            long long pos = lo;
-            while (pos < hi) {
-                const int sx = (int)(pos / Ly), y_start = (int)(pos - (long long)sx * Ly);
-                const int nrows = (int)((hi - pos) < (long long)(Ly - y_start) ? (hi - pos) : (Ly - y_start));
-                const int xb = strip_x(sx, Lx, p.nsx), xe = (sx + 1 == p.nsx) ? Lx : strip_x(sx + 1, Lx, p.nsx);
-                const bool edgeL = l.px && xb == 0, edgeR = l.px && xe == Lx;
-                const int f_side0 = API ? 0 : 1;   // first field that needs the x-wrap side boxes
-                const int nside = (edgeL ? 1 : 0) + (edgeR ? 1 : 0);
-                const int Q = (nrows + 2 + RC - 1) / RC;
-                for (int j = 0; j < Q; ++j, ++n) {
-                    const unsigned s = n % S, ph = (n / S) & 1u;
+        // ================================================================ producer warp: all 32 lanes issue TMA boxes
+        // kinds of box per row (or per chunk): F main fields, NFS left-wrap sides, NFS right-wrap sides, c (SOLVER)
+        constexpr int KINDS = F + 2 * NFS + (API ? 0 : 1);
+        if (lane < 10) asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&maps.m_chunk + lane)) : "memory");
+        unsigned n = 0;
+        long long pos = lo;
+        while (pos < hi) {
+            const int sx = (int)(pos / Ly), y_start = (int)(pos - (long long)sx * Ly);
+            const int nrows = (int)((hi - pos) < (long long)(Ly - y_start) ? (hi - pos) : (Ly - y_start));
+            const int xb = strip_x(sx, Lx, p.nsx), xe = (sx + 1 == p.nsx) ? Lx : strip_x(sx + 1, Lx, p.nsx);
+            const bool edgeL = l.px && xb == 0, edgeR = l.px && xe == Lx;
+            const int nside = (edgeL ? 1 : 0) + (edgeR ? 1 : 0);
+            const int Q = (nrows + 2 + RC - 1) / RC;
+            // TMA needs a 16-byte aligned box start: the inner coordinate (in doubles) must be even, so the box
+            // starts two sites left of the (even) strip start: sites xb-2 .. xb+61 = halo at 1, strip at 2..w+1, halo at w+2
+            const int x3 = 3 * (xb - 2);
+            for (int j = 0; j < Q; ++j, ++n) {
+                const unsigned s = n % S, ph = (n / S) & 1u;
+                const int r0 = j * RC - 1;
+                const int nvalid = (nrows + 1 - r0) < RC ? (nrows + 1 - r0) : RC;
+                const int y0 = y_start + r0;
+                const bool chunk_ok = (nvalid == RC) && (!l.py || (y0 >= 0 && y0 + RC <= Ly));
+                if (lane == 0) {
                     mbar_wait(&empty[s], ph ^ 1u);
-                    const int r0 = j * RC - 1;
-                    const int nvalid = (nrows + 1 - r0) < RC ? (nrows + 1 - r0) : RC;
-                    const int y0 = y_start + r0;
-                    const bool chunk_ok = (nvalid == RC) && (!l.py || (y0 >= 0 && y0 + RC <= Ly));
-                    const unsigned bytes = (unsigned)nvalid * (F * ROWD * 8 + nside * (F - f_side0) * SIDED * 8);
-                    mbar_expect_tx(&full[s], bytes);
-                    // TMA needs a 16-byte aligned box start: the inner coordinate (in doubles) must be even, so the box
-                    // starts two sites left of the (even) strip start: sites xb-2 .. xb+61 = halo at 1, strip at 2..w+1, halo at w+2
-                    const int x3 = 3 * (xb - 2);
-                    if (chunk_ok) {
-#pragma unroll
-                        for (int f = 0; f < F; ++f) {
-                            const CUtensorMap* mp = f == 0 ? &maps.m_chunk : &maps.v_chunk;
-                            tma_load_3d(smain + ((size_t)f * NSLOT + s * RC) * ROWD, mp, &full[s], x3, y0, f == 0 ? 0 : f - 1);
-                            if (f >= f_side0) {
-                                const CUtensorMap* ms = f == 0 ? &maps.m_schunk : &maps.v_schunk;
-                                if (edgeL) tma_load_3d(sL + ((size_t)f * NSLOT + s * RC) * SIDED, ms, &full[s], 3 * Lx - SIDED, y0, f == 0 ? 0 : f - 1);
-                                if (edgeR) tma_load_3d(sR + ((size_t)f * NSLOT + s * RC) * SIDED, ms, &full[s], 0, y0, f == 0 ? 0 : f - 1);
-                            }
+                    mbar_expect_tx(&full[s], (unsigned)nvalid * (F * ROWD * 8 + nside * NFS * SIDED * 8 + (API ? 0 : CROWD * 8)));
+                }
+                __syncwarp();
+                const int nops = (chunk_ok ? 1 : nvalid) * KINDS;
+                for (int t = lane; t < nops; t += 32) {
+                    const int i = t / KINDS, kind = t - i * KINDS;     // i: row inside the stage (0 on the chunk path)
+                    int y = y0 + i;
+                    if (!chunk_ok && l.py) { if (y < 0) y += Ly; else if (y >= Ly) y -= Ly; }
+                    const int slot = s * RC + i;
+                    if (kind < F) {
+                        const int f = kind;
+                        const CUtensorMap* mp = f == 0 ? (chunk_ok ? &maps.m_chunk : &maps.m_row) : (chunk_ok ? &maps.v_chunk : &maps.v_row);
+                        tma_load_3d(smain + ((size_t)f * NSLOT + slot) * ROWD, mp, &full[s], x3, y, f == 0 ? 0 : f - 1);
+                    } else if (kind < F + 2 * NFS) {
+                        const int q = kind - F, right = q >= NFS, fi = right ? q - NFS : q, f = fi + FS0;
+                        if (right ? edgeR : edgeL) {
+                            const CUtensorMap* ms = f == 0 ? (chunk_ok ? &maps.m_schunk : &maps.m_srow) : (chunk_ok ? &maps.v_schunk : &maps.v_srow);
+                            tma_load_3d((right ? sR : sL) + ((size_t)fi * NSLOT + slot) * SIDED, ms, &full[s], right ? 0 : 3 * Lx - SIDED, y,
+                                        f == 0 ? 0 : f - 1);
                         }
                     } else {
-                        for (int i = 0; i < nvalid; ++i) {
-                            int y = y0 + i;
-                            if (l.py) { if (y < 0) y += Ly; else if (y >= Ly) y -= Ly; }
-#pragma unroll
-                            for (int f = 0; f < F; ++f) {
-                                const CUtensorMap* mp = f == 0 ? &maps.m_row : &maps.v_row;
-                                tma_load_3d(smain + ((size_t)f * NSLOT + s * RC + i) * ROWD, mp, &full[s], x3, y, f == 0 ? 0 : f - 1);
-                                if (f >= f_side0) {
-                                    const CUtensorMap* ms = f == 0 ? &maps.m_srow : &maps.v_srow;
-                                    if (edgeL) tma_load_3d(sL + ((size_t)f * NSLOT + s * RC + i) * SIDED, ms, &full[s], 3 * Lx - SIDED, y, f == 0 ? 0 : f - 1);
-                                    if (edgeR) tma_load_3d(sR + ((size_t)f * NSLOT + s * RC + i) * SIDED, ms, &full[s], 0, y, f == 0 ? 0 : f - 1);
-                                }
-                            }
-                        }
+                        tma_load_3d(sc + (size_t)slot * CROWD, chunk_ok ? &maps.c_chunk : &maps.c_row, &full[s], xb - 2, y, 0);
                     }
                 }
-                pos += nrows;
             }
+            pos += nrows;
         }
         return;
     }
@@ -209,6 +225,9 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         const int Q = (nrows + 2 + RC - 1) / RC, nb = (nrows + RC - 1) / RC;
 
         mbar_wait(&full[n % S], (n / S) & 1u);
+#ifdef MOTO_K1_TIMING
+        if (threadIdx.x == 0 && pos == lo) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); p.dbg[blockIdx.x * 4 + 2] = t; }
+#endif
         for (int j = 0; j < nb; ++j) {
             if (j + 1 < Q) mbar_wait(&full[(n + j + 1) % S], ((n + j + 1) / S) & 1u);
             const int rA = j * RC + 2 * rp;
@@ -222,7 +241,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                 }
                 const long long siteA = (long long)(y_start + rA) * Lx + x, siteB = siteA + Lx;
                 double cA = 0.0, cB = 0.0;
-                if (!API) { cA = p.cvec[siteA]; if (haveB) cB = p.cvec[siteB]; }
+                if (!API) { cA = sc[slot[1] * CROWD + col + 2]; cB = sc[slot[2] * CROWD + col + 2]; }
                 // field 0: m.  API: all ten sites (projection of the neighbours + stencil for c); SOLVER: centres only.
                 d3 m0C, m0R, m1L, m1C, m1R, m2L, m2C, m2R, m3L, m3C;
                 m1C = lds3(baseC + slot[1] * ROWD);
@@ -241,9 +260,9 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
 #pragma unroll
                 for (int a = 0; a < K; ++a) {
                     const int f = a + 1;
-                    const double* bL = baseL + f * fstrL;
+                    const double* bL = baseL + (useL ? f - FS0 : f) * fstrL;
                     const double* bC = baseC + f * NSLOT * ROWD;
-                    const double* bR = baseR + f * fstrR;
+                    const double* bR = baseR + (useR ? f - FS0 : f) * fstrR;
                     d3 u0C = lds3(bC + slot[0] * ROWD), u0R = lds3(bR + slot[0] * pitchR);
                     d3 u1L = lds3(bL + slot[1] * pitchL), u1C = lds3(bC + slot[1] * ROWD), u1R = lds3(bR + slot[1] * pitchR);
                     d3 u2L = lds3(bL + slot[2] * pitchL), u2C = lds3(bC + slot[2] * ROWD), u2R = lds3(bR + slot[2] * pitchR);
@@ -294,6 +313,9 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         pos += nrows;
     }
 
+#ifdef MOTO_K1_TIMING
+    if (threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); p.dbg[blockIdx.x * 4 + 3] = t; }
+#endif
     if (NK > 0 && p.waw) {  // fixed-order reduction over the 256 consumer threads (named barrier 1: the producer warp has left)
 #pragma unroll
         for (int t = 0; t < NK; ++t) {
@@ -328,12 +350,12 @@ EncodeTiledFn get_encode() {
     return fn;
 }
 
-// field array [nvec][Ly][3 Lx] fp64 as a 3-D tensor; box = {inner doubles, rows, 1}
-bool encode(CUtensorMap* map, const double* base, int Lx, int Ly, int nvec, int inner, int rows) {
+// field array [nvec][Ly][ncomp Lx] fp64 as a 3-D tensor; box = {inner doubles, rows, 1}
+bool encode(CUtensorMap* map, const double* base, int Lx, int Ly, int nvec, int inner, int rows, int ncomp = 3) {
     EncodeTiledFn enc = get_encode();
     if (!enc) return false;
-    cuuint64_t gdim[3] = {(cuuint64_t)3 * Lx, (cuuint64_t)Ly, (cuuint64_t)nvec};
-    cuuint64_t gstr[2] = {(cuuint64_t)24 * Lx, (cuuint64_t)24 * Lx * Ly};
+    cuuint64_t gdim[3] = {(cuuint64_t)ncomp * Lx, (cuuint64_t)Ly, (cuuint64_t)nvec};
+    cuuint64_t gstr[2] = {(cuuint64_t)8 * ncomp * Lx, (cuuint64_t)8 * ncomp * Lx * Ly};
     cuuint32_t box[3] = {(cuuint32_t)inner, (cuuint32_t)rows, 1};
     cuuint32_t estr[3] = {1, 1, 1};
     return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -342,7 +364,7 @@ bool encode(CUtensorMap* map, const double* base, int Lx, int Ly, int nvec, int 
 
 template <int K, bool API>
 bool launch(moto_ctx* c, const Maps& maps, const KParams& p, int grid) {
-    using C = Cfg<K>;
+    using C = Cfg<K, API>;
     static bool attr_set = false;
     if (!attr_set) {
         if (cudaFuncSetAttribute(k_hvp_tma<K, API>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return false;
@@ -377,7 +399,7 @@ int spin_tma_grid(const moto_ctx* c) {
 int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV, const int* d_done,
                     double* waw_partials, int cheb, double alpha, double c0, double beta, const double* U) {
     if (!spin_tma_applicable(c)) return 0;
-    if (((uintptr_t)m & 15) || ((uintptr_t)V & 15)) return 0;
+    if (((uintptr_t)m & 15) || ((uintptr_t)V & 15) || ((uintptr_t)cvec & 15)) return 0;
     if (waw_partials && k > 2) return 0;
     const int Lx = c->lat.Lx, Ly = c->lat.Ly;
     const size_t bs = (size_t)3 * c->N;
@@ -385,10 +407,12 @@ int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const doub
     for (int a0 = 0; a0 < k; a0 += 2) {
         const int kk = (k - a0) >= 2 ? 2 : 1;
         Maps maps;
+        memset(&maps, 0, sizeof(maps));
         bool ok = encode(&maps.m_chunk, m, Lx, Ly, 1, ROWD, RC) && encode(&maps.m_row, m, Lx, Ly, 1, ROWD, 1) &&
                   encode(&maps.m_schunk, m, Lx, Ly, 1, SIDED, RC) && encode(&maps.m_srow, m, Lx, Ly, 1, SIDED, 1) &&
                   encode(&maps.v_chunk, V + a0 * bs, Lx, Ly, kk, ROWD, RC) && encode(&maps.v_row, V + a0 * bs, Lx, Ly, kk, ROWD, 1) &&
                   encode(&maps.v_schunk, V + a0 * bs, Lx, Ly, kk, SIDED, RC) && encode(&maps.v_srow, V + a0 * bs, Lx, Ly, kk, SIDED, 1);
+        if (ok && cvec) ok = encode(&maps.c_chunk, cvec, Lx, Ly, 1, CROWD, RC, 1) && encode(&maps.c_row, cvec, Lx, Ly, 1, CROWD, 1, 1);
         if (!ok) return launches ? -1 : 0;
         KParams p;
         p.l = make_lat(c);
@@ -398,6 +422,9 @@ int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const doub
         p.U = U ? U + a0 * bs : nullptr;
         p.alpha = alpha; p.c0 = c0; p.beta = beta; p.cheb = cheb;
         p.waw = waw_partials; p.done = d_done;
+#ifdef MOTO_K1_TIMING
+        p.dbg = (unsigned long long*)(c->partials + 100000);
+#endif
         const int grid = spin_tma_grid(c);
         bool l_ok;
         if (cvec) l_ok = kk == 2 ? launch<2, false>(c, maps, p, grid) : launch<1, false>(c, maps, p, grid);
