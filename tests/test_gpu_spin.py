@@ -301,3 +301,55 @@ def test_determinism(moto):
     assert np.array_equal(a[0].cpu().numpy(), b[0].cpu().numpy())
     assert np.array_equal(a[1].cpu().numpy(), b[1].cpu().numpy())
     assert ctx.launch_count > 0
+
+
+# ---------------------------------------------------------------- full size: BASELINE.json configs[3], the bench configuration
+@pytest.fixture(scope="module")
+def cfg3_full():
+    return wl.config3()
+
+
+def _golden_eigs(L):
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg3_lowest_eigs.txt")
+    for line in open(path):
+        if line.startswith(f"L={L} "):
+            return np.array([float(x) for x in line.split()[2:]])
+    raise KeyError(L)
+
+
+def test_cfg3_full_size_hvp_parity(moto, cfg3_full):
+    # the launch configuration bench.py times (TMA path, k = 2, 10^6 spins) against the oracle's explicit sparse Hessian
+    w = cfg3_full
+    ctx = moto.spin_context(w, kmax=2)
+    V = wl.random_block(w.N, 2, seed=33)
+    HV = ctx.hvp(dev(w.spins), dev(V)).cpu().numpy()
+    ref = so.hvp(model_of(w), w.spins, V)
+    assert rel_l2(HV, ref) <= HVP_TOL
+    assert np.max(np.abs(HV - ref)) <= 1e-11 * np.max(np.abs(ref))
+
+
+def test_cfg3_full_size_lowest_modes_vs_golden(moto, cfg3_full):
+    # eigenvalues against the oracle's ARPACK shift-invert values stored by tests/golden/make_cfg3_eigs.py;
+    # lambda_3 - lambda_2 = 1.0e-4, so the subspace test is the oracle-side residual (reading A10), not an angle
+    w = cfg3_full
+    gold = _golden_eigs(1000)
+    ctx = moto.spin_context(w, kmax=2)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-6, max_iter=20000)
+    assert info["converged"], info
+    lam = lam.cpu().numpy(); V = V.cpu().numpy()
+    assert np.max(np.abs(lam - gold[:2]) / np.abs(gold[:2])) <= EIG_TOL, (lam, gold[:2])
+    HV = so.hvp(model_of(w), w.spins, V)
+    for a in range(2):
+        assert np.linalg.norm(HV[a] - lam[a] * V[a]) <= 2e-6
+    assert np.max(np.abs(V.reshape(2, -1) @ V.reshape(2, -1).T - np.eye(2))) <= 1e-10
+    assert np.max(np.abs(np.sum(V * w.spins[None], axis=2))) <= 1e-10
+
+
+def test_cfg3_scaled_316_vs_golden(moto):
+    w = wl.config3_scaled(316)
+    gold = _golden_eigs(316)
+    ctx = moto.spin_context(w, kmax=2)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-7, max_iter=20000)
+    assert info["converged"], info
+    assert np.max(np.abs(lam.cpu().numpy() - gold[:2]) / np.abs(gold[:2])) <= EIG_TOL
