@@ -91,7 +91,7 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_sample(L: int = 316, calls: int = 3):
+def oracle_sample(L: int = 632, calls: int = 6):
     """The oracle, as it stands, on a bounded same-density sample of configs[3]; returns HVP/s scaled to 1e6 sites."""
     from oracle import spin_oracle as so
     from paper_2509_26269_b200 import workloads as wl

@@ -15,7 +15,7 @@ static bool lattice_ok(const moto_lattice* lat) {
     return false;
 }
 
-struct WsLayout { size_t block, c, g, stage, partials, st, cart, total; };
+struct WsLayout { size_t block, c, g, stage, partials, st, cart, total; int nblocks; };
 
 static WsLayout ws_layout(const moto_lattice* lat, int kmax) {
     WsLayout w;
@@ -27,7 +27,8 @@ static WsLayout ws_layout(const moto_lattice* lat, int kmax) {
     w.partials = al256((size_t)MOTO_RED_BLOCKS * 2 * MOTO_NS * MOTO_NS * sizeof(double));
     w.st = al256(sizeof(SolverState));
     w.cart = lat->kind == MOTO_KIND_CARTESIAN ? cart_lists_bytes(lat) : 0;
-    w.total = 6 * w.block + w.c + w.g + w.stage + w.partials + w.st + w.cart;
+    w.nblocks = lat->kind == MOTO_KIND_TRI2D ? 8 : 6;   // spin lattices: + two Chebyshev ping-pong blocks
+    w.total = w.nblocks * w.block + w.c + w.g + w.stage + w.partials + w.st + w.cart;
     return w;
 }
 
@@ -71,6 +72,7 @@ moto_status moto_create(const moto_lattice* lat, const void* params, void* d_wor
     c->X = (double*)p; p += w.block;  c->AX = (double*)p; p += w.block;
     c->W = (double*)p; p += w.block;  c->AW = (double*)p; p += w.block;
     c->P = (double*)p; p += w.block;  c->AP = (double*)p; p += w.block;
+    if (w.nblocks == 8) { c->T1 = (double*)p; p += w.block; c->T2 = (double*)p; p += w.block; }
     c->c = (double*)p; p += w.c;
     c->g = (double*)p; p += w.g;
     c->stage_m = (double*)p; p += w.stage;

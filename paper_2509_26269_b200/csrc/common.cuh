@@ -11,6 +11,7 @@
 #define MOTO_NUM_SMS 148     // B200
 #define MOTO_RED_BLOCKS 296  // CTAs of every grid-reduction kernel (2 per SM): fixed => deterministic sums
 #define MOTO_MAX_NEIGH 160   // Cartesian: neighbour capacity per atom
+#define MOTO_CHEB_MAX 256    // largest degree of the Chebyshev spectral transformation
 
 // Device-resident LOBPCG state: Gram matrices, Ritz coefficients, residuals, control flags.
 // Lives in the workspace; the host only ever reads the tail (ctl) through a pinned copy.
@@ -19,6 +20,8 @@ struct SolverState {
     double GB[MOTO_NS * MOTO_NS];
     double C[MOTO_NS * MOTO_KMAX];   // [ns][kb] coefficients of the new X in the basis [X,W,P]
     double scal[8];                  // scratch scalars: F.v dots, signs ...
+    double cheb[MOTO_CHEB_MAX][4];   // per-step {alpha, c0, beta, -} of the Chebyshev recurrence (k_cheb_coef)
+    double cheb_ab[4];               // a, b, a_L, scale of the current transformation
     // ---- tail mirrored to the host (layout == HostStatus)
     double theta[MOTO_KMAX];
     double resid[MOTO_KMAX];
@@ -26,12 +29,14 @@ struct SolverState {
     int iter;      // iterations completed
     int nkeep;     // basis directions kept by the last Rayleigh-Ritz
     int bad;       // 1 if a NaN/breakdown was seen
+    long long nhvp;  // single-vector HVP applications so far
 };
 
 struct HostStatus {  // pinned mirror of the control block + residuals
     double theta[MOTO_KMAX];
     double resid[MOTO_KMAX];
     int done, iter, nkeep, bad;
+    long long nhvp;
 };
 
 struct CartLists {
@@ -59,6 +64,7 @@ struct moto_ctx {
     size_t ws_bytes;
     // workspace views
     double *X, *AX, *W, *AW, *P, *AP;  // [kmax][N][3] each
+    double *T1, *T2;   // [kmax][N][3] ping-pong blocks of the Chebyshev recurrence (spin lattices)
     double* c;         // [N]   m_i . g_i
     double* g;         // [N][3] gradient scratch
     double* stage_m;   // [N][3] host-variant staging
@@ -98,7 +104,7 @@ int spin_project(moto_ctx*, const double* m, double* V, int k);
 bool spin_tma_applicable(const moto_ctx*);
 int spin_tma_grid(const moto_ctx*);
 int spin_hvp_tma_ex(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double* HV, const int* d_done,
-                    double* waw_partials, int cheb, double alpha, double c0, double beta, const double* U);
+                    double* waw_partials, int cheb, double alpha, double c0, double beta, const double* U, const double* d_coef);
 // cart_morse.cu
 int cart_build_lists(moto_ctx*, const double* x);
 int cart_energy_grad(moto_ctx*, const double* x, double* d_E, double* d_g);

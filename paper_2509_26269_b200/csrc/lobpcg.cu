@@ -20,9 +20,11 @@ static int project_block(moto_ctx* c, const double* d_state, double* V, int kb) 
 
 // lobpcg_fast.cu / rayleigh_ritz.cu
 int fast_gram_full(moto_ctx*, int kb, int* nblk_out);
-int fast_dot_waw(moto_ctx*, int kb, double* partialsK, int* nblk_out);
+int fast_dot_waw(moto_ctx*, int kb, const double* W, const double* AW, double* partialsK, int* nblk_out);
+int fast_negc_max(moto_ctx*, double* partial_max, int* nmax_out);
+int fast_cheb_coef(moto_ctx*, int k, int d, double margin, double lnorm, double hi_user, const double* partial_max, int nmax);
 int fast_update(moto_ctx*, const double* m_or_null, int kb, int* nblk_out);
-int rr_solve_fast(moto_ctx*, int kb, int nblkU, const double* partialsK, int nblkK, int check, int k, double tol);
+int rr_solve_fast(moto_ctx*, int kb, int nblkU, const double* partialsK, int nblkK, int check, int k, double tol, int hvp_inc);
 
 static moto_status finish(moto_ctx* c, int k, int kb, int enq, const HostStatus& last, moto_solve_info* info) {
     MOTO_CUDA_CHECK(c, cudaGetLastError());
@@ -31,57 +33,125 @@ static moto_status finish(moto_ctx* c, int k, int kb, int enq, const HostStatus&
         info->iters = iters;
         info->converged = (last.done && !last.bad) ? 1 : 0;
         for (int a = 0; a < MOTO_KMAX; ++a) info->resid[a] = a < k ? last.resid[a] : 0.0;
-        info->hvp_count = (int64_t)kb * (1 + iters);
+        info->hvp_count = last.nhvp > 0 ? (int64_t)last.nhvp : (int64_t)kb * (1 + iters);
     }
     if (last.bad) return moto_fail(c, MOTO_ECUDA, "moto_lowest_modes: numerical breakdown (NaN or rank loss) in Rayleigh-Ritz");
     if (!last.done) return moto_fail(c, MOTO_ENOTCONV, "moto_lowest_modes: max_iter reached; outputs hold the best iterate");
     return MOTO_OK;
 }
 
-// Fused path for kb <= 2 (lobpcg_fast.cu): per iteration  K1 -> k_rr (check + Rayleigh-Ritz) -> k_update_fused.
+// ------------------------------------------------------------------------------------------------------------
+// Fused path for kb <= 2 (lobpcg_fast.cu): per iteration  op(W) -> k_rr (check + Rayleigh-Ritz) -> k_update_fused.
+//
+// op is either the Hessian itself (one K1 launch with the W^T AW partials fused in) or, on spin lattices with the
+// TMA K1 path, the Chebyshev spectral transformation -p_d(A): d fused three-term K1 launches whose coefficients
+// live on the device (k_cheb_coef), so each outer iteration moves 176 B/site per Hessian application instead of
+// the ~700 B/site of a full LOBPCG iteration.  The transformation is fixed for a phase of `phase_len` iterations;
+// between phases the true A-Ritz values and A-residuals are recomputed (that is also the only convergence test
+// while transformed), the interval [a, b] is re-centred on them and LOBPCG restarts from the current X.
+// The host never waits per iteration: it enqueues whole phases and looks at a pinned status copy one batch behind.
+struct FastCtx {
+    moto_ctx* c; const double* state; const double* m_proj; int k, kb; double tol;
+    double* partialsK; int nblkU, nblkK; int n;   // n: kernels enqueued
+    int degree;      // 0: op = A
+};
+
+// OV = op(V), with the V^T OV partials left in partialsK.  V = X goes to AX, V = W goes to AW.
+static void fast_apply(FastCtx& f, const double* V, double* OV) {
+    moto_ctx* c = f.c;
+    if (f.degree == 0) {
+        int nk = (c->kind == MOTO_KIND_TRI2D) ? spin_hvp_tma_ex(c, f.state, c->c, V, f.kb, OV, &c->st->done, f.partialsK, 0, 0.0, 0.0, 0.0, nullptr, nullptr) : 0;
+        if (nk > 0) { f.n += nk; f.nblkK = spin_tma_grid(c); return; }
+        f.n += apply_operator(c, f.state, V, f.kb, OV);
+        f.n += fast_dot_waw(c, f.kb, V, OV, f.partialsK, &f.nblkK);
+        return;
+    }
+    // Chebyshev recurrence Y_0 = V, Y_1 -> T1, Y_2 -> T2, Y_3 -> T1 (in place over its own three-term operand) ...
+    const double* in = V; const double* prev = nullptr;
+    for (int i = 1; i <= f.degree; ++i) {
+        double* out = (i == f.degree) ? OV : ((i & 1) ? c->T1 : c->T2);
+        f.n += spin_hvp_tma_ex(c, f.state, c->c, in, f.kb, out, &c->st->done, nullptr, 1, 0.0, 0.0, 0.0, prev, &c->st->cheb[i - 1][0]);
+        prev = in; in = out;
+        if (i == 1) prev = V;
+    }
+    f.n += fast_dot_waw(c, f.kb, V, OV, f.partialsK, &f.nblkK);
+}
+
+// (re)start LOBPCG on span(X) for the current op: OX = op(X), Rayleigh-Ritz on X alone, first fused update (W = R)
+static void fast_phase_start(FastCtx& f) {
+    moto_ctx* c = f.c;
+    const size_t bs = (size_t)3 * c->N;
+    fast_apply(f, c->X, c->AX);
+    f.n += block_zero(c, c->W, (long long)f.kb * bs);
+    f.n += block_zero(c, c->AW, (long long)f.kb * bs);
+    f.n += block_zero(c, c->P, (long long)f.kb * bs);
+    f.n += block_zero(c, c->AP, (long long)f.kb * bs);
+    f.n += fast_gram_full(c, f.kb, &f.nblkU);
+    f.n += rr_solve_fast(c, f.kb, f.nblkU, nullptr, 0, /*check=*/0, f.k, f.tol, f.kb * (f.degree ? f.degree : 1));
+    f.n += fast_update(c, f.m_proj, f.kb, &f.nblkU);
+}
+
+static void fast_iterate(FastCtx& f, int check_mode) {
+    moto_ctx* c = f.c;
+    fast_apply(f, c->W, c->AW);
+    f.n += rr_solve_fast(c, f.kb, f.nblkU, f.partialsK, f.nblkK, check_mode, f.k, f.tol, f.kb * (f.degree ? f.degree : 1));
+    f.n += fast_update(c, f.m_proj, f.kb, &f.nblkU);
+}
+
 static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, int kb, double tol, int max_iter, int warm_start,
                                      moto_solve_info* info) {
     const size_t bs = (size_t)3 * c->N;
     const int check_every = c->opts.check_every > 0 ? c->opts.check_every : 8;
-    double* partialsK = c->partials + (size_t)MOTO_RED_BLOCKS * 64;   // after the [<=296][<=44] tri partials
-    const double* m_proj = (c->kind == MOTO_KIND_TRI2D) ? d_state : nullptr;
-    int n = 0, nblkU = 0, nblkK = 0;
+    FastCtx f;
+    f.c = c; f.state = d_state; f.k = k; f.kb = kb; f.tol = tol; f.n = 0; f.nblkU = f.nblkK = 0; f.degree = 0;
+    f.partialsK = c->partials + (size_t)MOTO_RED_BLOCKS * 64;   // after the [<=296][<=44] tri partials
+    f.m_proj = (c->kind == MOTO_KIND_TRI2D) ? d_state : nullptr;
+    double* pmax = c->partials + (size_t)MOTO_RED_BLOCKS * 128;
 
-    if (c->kind == MOTO_KIND_TRI2D) n += spin_curvature(c, d_state, c->c);
-    else n += cart_build_lists(c, d_state);
+    // spectral transformation: precond_degree 0 = auto (32 where the TMA K1 applies), < 0 = off
+    int degree = c->opts.precond_degree;
+    const bool can_filter = c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && 3ll * kb * 8 <= 2ll * c->N;
+    if (degree == 0) degree = can_filter ? 32 : 0;
+    if (degree < 0 || !can_filter) degree = 0;
+    if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
+    const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.02;
+    const int phase_len = 10, plain_start = 30;
+    const double lnorm = 12.0 * fabs(c->sp.J) + 12.0 * fabs(c->sp.D) + 2.0 * fabs(c->sp.K);
+
+    if (c->kind == MOTO_KIND_TRI2D) f.n += spin_curvature(c, d_state, c->c);
+    else f.n += cart_build_lists(c, d_state);
     MOTO_CUDA_CHECK(c, cudaMemsetAsync(c->st, 0, sizeof(SolverState), c->stream));
-    if (!warm_start) n += block_random(c, c->X, kb, c->opts.seed);
-    else if (kb > k) n += block_random(c, c->X + (size_t)k * bs, kb - k, c->opts.seed ^ 0x5bd1e995u);
-    n += project_block(c, d_state, c->X, kb);
-    n += apply_operator(c, d_state, c->X, kb, c->AX);
-    n += block_zero(c, c->W, (long long)kb * bs);
-    n += block_zero(c, c->AW, (long long)kb * bs);
-    n += block_zero(c, c->P, (long long)kb * bs);
-    n += block_zero(c, c->AP, (long long)kb * bs);
-    // start-up: Rayleigh-Ritz on span(X) alone, then the first fused update produces W = R and the Gram partials
-    n += fast_gram_full(c, kb, &nblkU);
-    n += rr_solve_fast(c, kb, nblkU, nullptr, 0, /*check=*/0, k, tol);
-    n += fast_update(c, m_proj, kb, &nblkU);
+    int nmax = 0;
+    if (degree > 0) f.n += fast_negc_max(c, pmax, &nmax);
+    if (!warm_start) f.n += block_random(c, c->X, kb, c->opts.seed);
+    else if (kb > k) f.n += block_random(c, c->X + (size_t)k * bs, kb - k, c->opts.seed ^ 0x5bd1e995u);
+    f.n += project_block(c, d_state, c->X, kb);
+    fast_phase_start(f);
 
-    int enq = 0, slot = 0, pending = 0;
-    bool finished = false;
+    int enq = 0, slot = 0, pending = 0, in_phase = 0;
+    bool finished = false, transformed = false;
     HostStatus last; memset(&last, 0, sizeof(last));
     while (!finished) {
         int batch = max_iter - enq < check_every ? max_iter - enq : check_every;
         for (int b = 0; b < batch; ++b) {
-            // AW = Hess[W] with the W^T AW partials fused into the TMA kernel's epilogue when that path applies
-            int nk = (c->kind == MOTO_KIND_TRI2D) ? spin_hvp_tma_ex(c, d_state, c->c, c->W, kb, c->AW, &c->st->done, partialsK, 0, 0.0, 0.0, 0.0, nullptr) : 0;
-            if (nk > 0) { n += nk; nblkK = spin_tma_grid(c); }
-            else {
-                n += apply_operator(c, d_state, c->W, kb, c->AW);
-                n += fast_dot_waw(c, kb, partialsK, &nblkK);
+            if (degree > 0 && ((!transformed && enq + b >= plain_start) || (transformed && in_phase >= phase_len))) {
+                // phase boundary: true A-Ritz pairs and residuals of the current X, convergence test, new interval
+                f.degree = 0;
+                fast_phase_start(f);
+                f.n += rr_solve_fast(c, kb, f.nblkU, nullptr, 0, /*check=*/2, k, tol, 0);
+                f.n += fast_cheb_coef(c, k, degree, margin, lnorm, c->opts.precond_hi, pmax, nmax);
+                f.degree = degree;
+                fast_phase_start(f);
+                transformed = true; in_phase = 0;
             }
-            n += rr_solve_fast(c, kb, nblkU, partialsK, nblkK, /*check=*/1, k, tol);
-            n += fast_update(c, m_proj, kb, &nblkU);
+            fast_iterate(f, transformed ? 3 : 1);
+            ++in_phase;
         }
         enq += batch;
-        if (enq >= max_iter)   // final look at the residuals of the last update (no solve follows: done or not, X stays)
-            n += rr_solve_fast(c, kb, nblkU, nullptr, 0, /*check=*/2, k, tol);
+        if (enq >= max_iter) {   // final look: residuals of the last update if op = A, else a last A-phase start
+            if (transformed) { f.degree = 0; fast_phase_start(f); }
+            f.n += rr_solve_fast(c, kb, f.nblkU, nullptr, 0, /*check=*/2, k, tol, 0);
+        }
         MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&c->hstat[slot], &c->st->theta, sizeof(HostStatus), cudaMemcpyDeviceToHost, c->stream));
         MOTO_CUDA_CHECK(c, cudaEventRecord(c->ev[slot], c->stream));
         if (pending) {
@@ -96,8 +166,8 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     MOTO_CUDA_CHECK(c, cudaEventSynchronize(c->ev[slot ^ 1]));
     last = c->hstat[slot ^ 1];
     // keep the returned block exactly tangent / masked (rounding drift of the recurrences)
-    n += project_block(c, d_state, c->X, k);
-    c->launches += n;
+    f.n += project_block(c, d_state, c->X, k);
+    c->launches += f.n;
     return finish(c, k, kb, enq, last, info);
 }
 

@@ -179,6 +179,53 @@ __global__ void __launch_bounds__(256) k_update_fused(long long N, Blk6 b, const
     block_reduce_store<T::NEU>(acc, partials + (size_t)blockIdx.x * T::NEU);
 }
 
+// ---------------------------------------------------------------- Chebyshev spectral transformation (coefficients)
+// p(lambda) = scaled Chebyshev polynomial of degree d that is <= 1 in magnitude on [a, b] and grows below a
+// (Zhou & Saad's scaled three-term form, p(a_L) = 1).  LOBPCG is run on -p(A): same eigenvectors, lowest
+// eigenvalues of A <-> lowest of -p(A), relative gaps d^2 times wider as long as d^2 (a - lambda) <~ (b - a)/4.
+// a = theta_k + margin from the current A-Ritz values (theta_k >= lambda_k, so the wanted pairs stay below a),
+// b = max_i(-c_i) + ||L||  >= lambda_max (Gershgorin-type bound), a_L = theta_1.  All on the device.
+__global__ void k_negc_max(long long N, const double* __restrict__ c, double* __restrict__ partial_max) {
+    __shared__ double sm[8];
+    double v = -1e300;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) v = fmax(v, -c[i]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) v = fmax(v, sm[w]);
+        partial_max[blockIdx.x] = v;
+    }
+}
+
+__global__ void k_cheb_coef(SolverState* st, int k, int d, double margin, double lnorm, double hi_user,
+                            const double* __restrict__ partial_max, int nmax) {
+    if (st->done || threadIdx.x != 0) return;
+    double b = hi_user;
+    if (!(b > 0.0)) {
+        double mx = -1e300;
+        for (int i = 0; i < nmax; ++i) mx = fmax(mx, partial_max[i]);
+        b = mx + lnorm;
+    }
+    const double aL = st->theta[0];
+    double a = st->theta[k - 1] + margin;
+    if (a > 0.5 * (aL + b)) a = 0.5 * (aL + b);   // crude early Ritz values: keep the interval sane
+    const double e = 0.5 * (b - a), c0 = 0.5 * (b + a), sig1 = e / (aL - c0);
+    double sig = sig1;
+    st->cheb_ab[0] = a; st->cheb_ab[1] = b; st->cheb_ab[2] = aL; st->cheb_ab[3] = (double)d;
+    for (int i = 1; i <= d; ++i) {
+        double alpha, beta;
+        if (i == 1) { alpha = sig1 / e; beta = 0.0; }
+        else {
+            const double sn = 1.0 / (2.0 / sig1 - sig);
+            alpha = 2.0 * sn / e; beta = -sig * sn; sig = sn;
+        }
+        if (i == d) { alpha = -alpha; beta = -beta; }   // the transformed operator is -p(A)
+        st->cheb[i - 1][0] = alpha; st->cheb[i - 1][1] = c0; st->cheb[i - 1][2] = beta; st->cheb[i - 1][3] = 0.0;
+    }
+}
+
 int fast_grid(long long work_items) {
     long long b = (work_items + 255) / 256;
     return (int)(b < 1 ? 1 : (b > MOTO_RED_BLOCKS ? MOTO_RED_BLOCKS : b));
@@ -198,12 +245,12 @@ int fast_gram_full(moto_ctx* c, int kb, int* nblk_out) {
     return 1;
 }
 
-int fast_dot_waw(moto_ctx* c, int kb, double* partialsK, int* nblk_out) {
+int fast_dot_waw(moto_ctx* c, int kb, const double* W, const double* AW, double* partialsK, int* nblk_out) {
     const long long n3 = 3ll * c->N;
     const int g = fast_grid(n3);
     *nblk_out = g;
-    if (kb == 1) k_dot_waw<1><<<g, 256, 0, c->stream>>>(n3, c->W, c->AW, partialsK, &c->st->done);
-    else k_dot_waw<2><<<g, 256, 0, c->stream>>>(n3, c->W, c->AW, partialsK, &c->st->done);
+    if (kb == 1) k_dot_waw<1><<<g, 256, 0, c->stream>>>(n3, W, AW, partialsK, &c->st->done);
+    else k_dot_waw<2><<<g, 256, 0, c->stream>>>(n3, W, AW, partialsK, &c->st->done);
     return 1;
 }
 
@@ -219,5 +266,17 @@ int fast_update(moto_ctx* c, const double* m_or_null, int kb, int* nblk_out) {
         if (m_or_null) k_update_fused<2, true><<<g, 256, 0, c->stream>>>(N, b, m_or_null, c->st, c->partials);
         else k_update_fused<2, false><<<g, 256, 0, c->stream>>>(N, b, m_or_null, c->st, c->partials);
     }
+    return 1;
+}
+
+int fast_negc_max(moto_ctx* c, double* partial_max, int* nmax_out) {
+    const int g = fast_grid(c->N);
+    *nmax_out = g;
+    k_negc_max<<<g, 256, 0, c->stream>>>((long long)c->N, c->c, partial_max);
+    return 1;
+}
+
+int fast_cheb_coef(moto_ctx* c, int k, int d, double margin, double lnorm, double hi_user, const double* partial_max, int nmax) {
+    k_cheb_coef<<<1, 32, 0, c->stream>>>(c->st, k, d, margin, lnorm, hi_user, partial_max, nmax);
     return 1;
 }

@@ -116,7 +116,9 @@ struct RRFast {            // inputs of the fused kb <= 2 path (lobpcg_fast.cu);
     const double* partialsK;   // [nblkK][kb(kb+1)/2]  W^T A W from K1 (NULL: already inside the tri partials)
     int nblkK;
     int kb;
-    int check;             // 1: finish the residual norms of the last update and decide convergence first; 2: only that
+    int check;             // 1: finish the residual norms of the last update and decide convergence first; 2: only that;
+                           // 3: count the iteration without testing (transformed operator: its residuals are not A's)
+    int hvp_inc;           // single-vector HVPs the caller spent since the previous Rayleigh-Ritz
     int k;                 // wanted columns
     double tol;
 };
@@ -142,7 +144,8 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         if (fz.partialsK) { __syncthreads(); reduce_partials(fz.partialsK, fz.nblkK, nK, nK, vals + neu, Z); }
         if (tid == 0) stop_s = 0;
         __syncthreads();
-        if (fz.check && tid == 0) {
+        if (fz.check == 3 && tid == 0) st->iter += 1;
+        if ((fz.check == 1 || fz.check == 2) && tid == 0) {
             bool ok = true, bad = false;
             for (int a = 0; a < kb; ++a) {
                 double r = sqrt(vals[2 * nT + a]);
@@ -155,6 +158,7 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         }
         __syncthreads();
         if (stop_s || fz.check == 2) return;
+        if (tid == 0) st->nhvp += fz.hvp_inc;
         for (int t = tid; t < n * n; t += nt) {
             int i = t / n, j = t - i * n;
             int a = i < j ? i : j, b = i < j ? j : i;
@@ -280,7 +284,7 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
 int rr_solve(moto_ctx* c, const double* d_GA, const double* d_GB, int n, int nev, double* d_theta, double* d_C, int mode,
              SolverState* st) {
     const double tau = 1e-10;
-    RRFast fz = {nullptr, 0, 0, 0, 0, 0.0};
+    RRFast fz = {nullptr, 0, 0, 0, 0, 0, 0.0};
     k_rr<<<1, RR_THREADS, 0, c->stream>>>(nullptr, 0, d_GA, d_GB, n, nev, d_theta, d_C, mode, st, tau, fz);
     return 1;
 }
@@ -288,15 +292,15 @@ int rr_solve(moto_ctx* c, const double* d_GA, const double* d_GB, int n, int nev
 // LOBPCG flavour: inputs are the Gram partials left in ctx->partials by block_gram_lobpcg
 int rr_solve_lobpcg(moto_ctx* c, int kb, int nblk) {
     const double tau = 1e-10;
-    RRFast fz = {nullptr, 0, 0, 0, 0, 0.0};
+    RRFast fz = {nullptr, 0, 0, 0, 0, 0, 0.0};
     k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblk, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, fz);
     return 1;
 }
 
 // fused kb <= 2 path: tri partials [nblkU][2 nT + kb] in ctx->partials, optional W^T A W partials, optional check
-int rr_solve_fast(moto_ctx* c, int kb, int nblkU, const double* partialsK, int nblkK, int check, int k, double tol) {
+int rr_solve_fast(moto_ctx* c, int kb, int nblkU, const double* partialsK, int nblkK, int check, int k, double tol, int hvp_inc) {
     const double tau = 1e-10;
-    RRFast fz = {partialsK, nblkK, kb, check, k, tol};
+    RRFast fz = {partialsK, nblkK, kb, check, hvp_inc, k, tol};
     k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblkU, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, fz);
     return 1;
 }

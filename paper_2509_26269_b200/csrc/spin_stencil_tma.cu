@@ -66,6 +66,7 @@ struct KParams {
     const double* U;         // [K][N][3] Chebyshev operand or NULL
     double alpha, c0, beta;  // out = alpha (HV - c0 v) + beta u   (cheb != 0)
     int cheb;
+    const double* coef;      // optional device triple {alpha, c0, beta} overriding the three scalars (device-resident recurrence)
     double* waw;             // [grid][K(K+1)/2] or NULL
     const int* done;
 #ifdef MOTO_K1_TIMING
@@ -204,6 +205,8 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
 #pragma unroll
     for (int t = 0; t < NK; ++t) waw[t] = 0.0;
     const d3 muB = mk3(l.mu * l.Bx, l.mu * l.By, l.mu * l.Bz);
+    const bool use_coef = !API && p.cheb && p.coef;
+    const double ch_alpha = use_coef ? p.coef[0] : p.alpha, ch_c0 = use_coef ? p.coef[1] : p.c0, ch_beta = use_coef ? p.coef[2] : p.beta;
 
     unsigned n = 0;
     long long pos = lo;
@@ -240,6 +243,16 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                     slot[q] = (int)((n + rr / RC) % S) * RC + (rr % RC);
                 }
                 const long long siteA = (long long)(y_start + rA) * Lx + x, siteB = siteA + Lx;
+                // the three-term operand is read straight from global memory (no reuse): issue the loads before the
+                // shared-memory phase so their latency overlaps this block's arithmetic
+                d3 uA[K], uB[K];
+                if (!API && p.cheb && p.U) {
+#pragma unroll
+                    for (int a = 0; a < K; ++a) {
+                        uA[a] = ld3(p.U + (size_t)a * 3 * N, siteA);
+                        uB[a] = haveB ? ld3(p.U + (size_t)a * 3 * N, siteB) : mk3(0.0, 0.0, 0.0);
+                    }
+                }
                 double cA = 0.0, cB = 0.0;
                 if (!API) { cA = sc[slot[1] * CROWD + col + 2]; cB = sc[slot[2] * CROWD + col + 2]; }
                 // field 0: m.  API: all ten sites (projection of the neighbours + stencil for c); SOLVER: centres only.
@@ -293,12 +306,12 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
 #pragma unroll
                 for (int a = 0; a < K; ++a) {
                     d3 oA = hA[a], oB = hB[a];
-                    if (p.cheb) {
-                        oA = scale3(p.alpha, axpy3(-p.c0, vA[a], oA));
-                        oB = scale3(p.alpha, axpy3(-p.c0, vB[a], oB));
+                    if (!API && p.cheb) {
+                        oA = scale3(ch_alpha, axpy3(-ch_c0, vA[a], oA));
+                        oB = scale3(ch_alpha, axpy3(-ch_c0, vB[a], oB));
                         if (p.U) {
-                            oA = axpy3(p.beta, ld3(p.U + (size_t)a * 3 * N, siteA), oA);
-                            if (haveB) oB = axpy3(p.beta, ld3(p.U + (size_t)a * 3 * N, siteB), oB);
+                            oA = axpy3(ch_beta, uA[a], oA);
+                            oB = axpy3(ch_beta, uB[a], oB);
                         }
                     }
                     st3(p.out + (size_t)a * 3 * N, siteA, oA);
@@ -397,7 +410,7 @@ int spin_tma_grid(const moto_ctx* c) {
 // waw_partials: optional [spin_tma_grid][k(k+1)/2].  cheb: out = alpha (HV - c0 V) + beta U (U may be NULL).
 // Returns the number of kernels launched, 0 if the path does not apply (caller falls back), -1 on error.
 int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV, const int* d_done,
-                    double* waw_partials, int cheb, double alpha, double c0, double beta, const double* U) {
+                    double* waw_partials, int cheb, double alpha, double c0, double beta, const double* U, const double* d_coef) {
     if (!spin_tma_applicable(c)) return 0;
     if (((uintptr_t)m & 15) || ((uintptr_t)V & 15) || ((uintptr_t)cvec & 15)) return 0;
     if (waw_partials && k > 2) return 0;
@@ -420,7 +433,7 @@ int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const doub
         p.total = (long long)p.nsx * Ly;
         p.m = m; p.cvec = cvec; p.out = HV + a0 * bs;
         p.U = U ? U + a0 * bs : nullptr;
-        p.alpha = alpha; p.c0 = c0; p.beta = beta; p.cheb = cheb;
+        p.alpha = alpha; p.c0 = c0; p.beta = beta; p.cheb = cheb; p.coef = d_coef;
         p.waw = waw_partials; p.done = d_done;
 #ifdef MOTO_K1_TIMING
         p.dbg = (unsigned long long*)(c->partials + 100000);
@@ -439,6 +452,6 @@ int spin_hvp_tma(moto_ctx* c, const double* m, const double* cvec, const double*
                  const int* d_done) {
     // the two combinations the library uses: (no c, project) = API, (c, no project) = SOLVER
     if ((cvec != nullptr) == (project_input != 0)) return 0;
-    int n = spin_hvp_tma_ex(c, m, cvec, V, k, HV, d_done, nullptr, 0, 0.0, 0.0, 0.0, nullptr);
+    int n = spin_hvp_tma_ex(c, m, cvec, V, k, HV, d_done, nullptr, 0, 0.0, 0.0, 0.0, nullptr, nullptr);
     return n < 0 ? 0 : n;
 }
