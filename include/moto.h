@@ -70,10 +70,12 @@ typedef struct { double De, alpha, r0, rc; } moto_morse_params;
 typedef struct {
     int32_t guard;          /* extra block columns iterated but not returned            [0]  */
     int32_t check_every;    /* iterations enqueued between host looks at the status     [8]  */
-    int32_t precond_degree; /* degree of the Chebyshev polynomial preconditioner, 0=off [0]  */
+    int32_t precond_degree; /* degree d of the Chebyshev spectral transformation -p_d(A) LOBPCG runs on:
+                               0 = auto (40 on spin lattices that take the TMA K1 path and kb <= 2, else off),
+                               -1 = off (plain LOBPCG on A, the paper's solver), 1..256 = degree          [0]  */
     int32_t hvp_path;       /* K1 kernel choice: 0 auto, 1 generic (any lattice), 2 TMA-staged (even Lx >= 8) [0] */
-    double precond_lo;      /* preconditioner interval [lo, hi] in units of the shift   [auto] */
-    double precond_hi;
+    double precond_lo;      /* margin: the damped interval starts at theta_k + margin           [0 -> 0.01] */
+    double precond_hi;      /* upper end b >= lambda_max of the damped interval    [0 -> max(-c_i) + ||L||] */
     uint64_t seed;          /* seed of the counter-based start block when warm_start=0  [0x9E3779B97F4A7C15] */
 } moto_solver_opts;
 

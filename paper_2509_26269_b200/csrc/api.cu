@@ -1,4 +1,5 @@
 // api.cu -- the C ABI of libmoto.so (include/moto.h): argument checks, workspace carving, dispatch.
+#include <math.h>
 #include <new>
 #include "common.cuh"
 
@@ -13,6 +14,36 @@ static bool lattice_ok(const moto_lattice* lat) {
     if (lat->kind == MOTO_KIND_TRI2D) return lat->Lx >= 1 && lat->Ly >= 1 && (long long)lat->Lx * lat->Ly < (1ll << 30);
     if (lat->kind == MOTO_KIND_CARTESIAN) return lat->n_atoms >= 1;
     return false;
+}
+
+// Upper bound on lambda_max of the constant Euclidean Hessian L of Eq. 4 on the infinite
+// triangular lattice (a finite open or periodic lattice is a compression / sub-sampling of it, so the bound holds).
+// Fourier symbol: L(q) = a(q) I3 + i [w(q)]x - 2 K z z^T with a(q) = -4 J sum_p cos(q.r_p), w(q) = 4 sum_p sin(q.r_p) D_p
+// over the three bond pairs; eigenvalues of i[w]x are {0, +-|w|}, so lambda_max(L) <= max_q (a + |w|) + 2|K|.
+// Used for the upper end b = max_i(-c_i) + lambda_max(L) of the Chebyshev interval (Weyl + compression to the
+// tangent space).  The symbol is smooth; a 512 x 512 grid plus a second-derivative allowance is a safe maximum.
+static double stencil_lmax_bound(const moto_spin_params& sp) {
+    const double rx[3] = {1.0, 0.5, -0.5}, ry[3] = {0.0, 0.86602540378443864676, 0.86602540378443864676};
+    const int G = 512;
+    const double two_pi = 6.283185307179586476925;
+    double best = -1e300;
+    for (int i = 0; i < G; ++i)
+        for (int j = 0; j < G; ++j) {
+            // q = q1 b1 + q2 b2 with q.a1 = 2 pi i/G, q.a2 = 2 pi j/G  => phases of the three bonds
+            const double t1 = two_pi * i / G, t2 = two_pi * j / G;
+            const double ph[3] = {t1, t2, t2 - t1};
+            double a = 0.0, wx = 0.0, wy = 0.0;
+            for (int p = 0; p < 3; ++p) {
+                a += -4.0 * sp.J * cos(ph[p]);
+                // D_p = D (z x r_p) = D (-ry, rx, 0)
+                wx += 4.0 * sin(ph[p]) * sp.D * (-ry[p]);
+                wy += 4.0 * sin(ph[p]) * sp.D * (rx[p]);
+            }
+            const double v = a + sqrt(wx * wx + wy * wy);
+            if (v > best) best = v;
+        }
+    const double h = two_pi / G;   // grid spacing in each phase; |second derivatives| <= 12 (|J| + |D|)
+    return best + 0.25 * h * h * 12.0 * (fabs(sp.J) + fabs(sp.D)) * 2.0 + 2.0 * fabs(sp.K);
 }
 
 struct WsLayout { size_t block, c, g, stage, partials, st, cart, total; int nblocks; };
@@ -63,6 +94,7 @@ moto_status moto_create(const moto_lattice* lat, const void* params, void* d_wor
     c->opts.seed = 0x9E3779B97F4A7C15ull;
     if (c->kind == MOTO_KIND_TRI2D) {
         c->sp = *(const moto_spin_params*)params;
+        c->lmax_L = stencil_lmax_bound(c->sp);
         c->lat.d_fixed = nullptr;
     } else {
         c->mp = *(const moto_morse_params*)params;
@@ -101,7 +133,7 @@ void moto_destroy(moto_ctx* c) {
 
 moto_status moto_set_solver(moto_ctx* c, const moto_solver_opts* o) {
     if (!c || !o) return MOTO_EINVAL;
-    if (o->guard < 0 || o->check_every < 0 || o->precond_degree < 0 || o->hvp_path < 0 || o->hvp_path > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: negative option");
+    if (o->guard < 0 || o->check_every < 0 || o->precond_degree < -1 || o->hvp_path < 0 || o->hvp_path > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: negative option");
     moto_solver_opts n = *o;
     if (n.check_every == 0) n.check_every = 8;
     if (n.seed == 0) n.seed = 0x9E3779B97F4A7C15ull;

@@ -57,6 +57,7 @@ struct moto_ctx {
     int N;       // sites or atoms
     int kmax;
     moto_spin_params sp;
+    double lmax_L;     // upper bound on the top eigenvalue of the constant stencil operator L (spin lattices)
     moto_morse_params mp;
     moto_solver_opts opts;
     cudaStream_t stream;

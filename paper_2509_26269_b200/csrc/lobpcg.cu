@@ -6,6 +6,7 @@
 // (convergence, breakdown, basis truncation) is taken on the device: kernels read SolverState::done and
 // return at once when it is set, so the host enqueues iterations in batches without waiting on any of
 // them; it only looks at a pinned copy of the status after each batch, one batch behind the GPU.
+#include <stdlib.h>
 #include "common.cuh"
 
 static int apply_operator(moto_ctx* c, const double* d_state, const double* V, int kb, double* AV) {
@@ -22,6 +23,7 @@ static int project_block(moto_ctx* c, const double* d_state, double* V, int kb) 
 int fast_gram_full(moto_ctx*, int kb, int* nblk_out);
 int fast_dot_waw(moto_ctx*, int kb, const double* W, const double* AW, double* partialsK, int* nblk_out);
 int fast_negc_max(moto_ctx*, double* partial_max, int* nmax_out);
+int fast_acheck(moto_ctx*, int kb, int k, double tol, const double* d_T, double* partials);
 int fast_cheb_coef(moto_ctx*, int k, int d, double margin, double lnorm, double hi_user, const double* partial_max, int nmax);
 int fast_update(moto_ctx*, const double* m_or_null, int kb, int* nblk_out);
 int rr_solve_fast(moto_ctx*, int kb, int nblkU, const double* partialsK, int nblkK, int check, int k, double tol, int hvp_inc);
@@ -108,15 +110,18 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     f.m_proj = (c->kind == MOTO_KIND_TRI2D) ? d_state : nullptr;
     double* pmax = c->partials + (size_t)MOTO_RED_BLOCKS * 128;
 
-    // spectral transformation: precond_degree 0 = auto (32 where the TMA K1 applies), < 0 = off
+    // spectral transformation: precond_degree 0 = auto (40 where the TMA K1 applies), < 0 = off
     int degree = c->opts.precond_degree;
     const bool can_filter = c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && 3ll * kb * 8 <= 2ll * c->N;
-    if (degree == 0) degree = can_filter ? 32 : 0;
+    if (degree == 0) degree = can_filter ? 40 : 0;
     if (degree < 0 || !can_filter) degree = 0;
     if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
-    const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.02;
-    const int phase_len = 10, plain_start = 30;
-    const double lnorm = 12.0 * fabs(c->sp.J) + 12.0 * fabs(c->sp.D) + 2.0 * fabs(c->sp.K);
+    const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.01;
+    int phase_len = 20, plain_start = 20;
+    const int acheck_every = 4;
+    if (const char* e = getenv("MOTO_PHASE_LEN")) phase_len = atoi(e);      // tuning hooks (not part of the ABI)
+    if (const char* e = getenv("MOTO_PLAIN_START")) plain_start = atoi(e);
+    const double lnorm = c->lmax_L;   // b = max_i(-c_i) + lambda_max(L) >= lambda_max(Hess)
 
     if (c->kind == MOTO_KIND_TRI2D) f.n += spin_curvature(c, d_state, c->c);
     else f.n += cart_build_lists(c, d_state);
@@ -146,6 +151,11 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
             }
             fast_iterate(f, transformed ? 3 : 1);
             ++in_phase;
+            if (transformed && in_phase < phase_len && in_phase % acheck_every == 0) {
+                // cheap convergence test between restarts: T1 = A X, |A x_j - (x_j.A x_j) x_j| (T1/T2 are free between applies)
+                f.n += spin_hvp_tma_ex(c, d_state, c->c, c->X, kb, c->T1, &c->st->done, nullptr, 0, 0.0, 0.0, 0.0, nullptr, nullptr);
+                f.n += fast_acheck(c, kb, k, tol, c->T1, pmax + 1024);
+            }
         }
         enq += batch;
         if (enq >= max_iter) {   // final look: residuals of the last update if op = A, else a last A-phase start

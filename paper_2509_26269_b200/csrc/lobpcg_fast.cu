@@ -226,6 +226,56 @@ __global__ void k_cheb_coef(SolverState* st, int k, int d, double margin, double
     }
 }
 
+// ---------------------------------------------------------------- A-residual check while LOBPCG runs on -p(A)
+// partials[blk][3 KB]: x_j.x_j, x_j.t_j, t_j.t_j with T = A X; then |A x - theta x|^2 = tt - 2 theta xt + theta^2 xx,
+// theta = xt / xx.  (|r|^2 ~ tol^2 = 1e-12 against tt ~ 1e-2: nine digits of head-room left in fp64.)
+template <int KB>
+__global__ void __launch_bounds__(256) k_acheck_dots(long long n3, const double* __restrict__ X, const double* __restrict__ T,
+                                                     double* __restrict__ partials, const int* __restrict__ done) {
+    if (*done) return;
+    double acc[3 * KB];
+#pragma unroll
+    for (int i = 0; i < 3 * KB; ++i) acc[i] = 0.0;
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n3; e += (long long)gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int j = 0; j < KB; ++j) {
+            const double x = X[j * n3 + e], t = T[j * n3 + e];
+            acc[3 * j] = fma(x, x, acc[3 * j]); acc[3 * j + 1] = fma(x, t, acc[3 * j + 1]); acc[3 * j + 2] = fma(t, t, acc[3 * j + 2]);
+        }
+    }
+    block_reduce_store<3 * KB>(acc, partials + (size_t)blockIdx.x * 3 * KB);
+}
+
+__global__ void k_acheck_final(const double* __restrict__ partials, int nblk, int kb, int k, double tol, SolverState* st) {
+    if (st->done) return;
+    __shared__ double v[3 * MOTO_KMAX];
+    const int e = threadIdx.x >> 5, lane = threadIdx.x & 31;   // one warp per entry
+    if (e < 3 * kb) {
+        double s = 0.0;
+        for (int b = lane; b < nblk; b += 32) s += partials[(size_t)b * 3 * kb + e];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) v[e] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        bool ok = true;
+        double th[MOTO_KMAX], rs[MOTO_KMAX];
+        for (int j = 0; j < kb; ++j) {
+            const double xx = v[3 * j], xt = v[3 * j + 1], tt = v[3 * j + 2];
+            th[j] = xt / xx;
+            const double r2 = (tt - 2.0 * th[j] * xt + th[j] * th[j] * xx) / xx;
+            rs[j] = sqrt(r2 > 0.0 ? r2 : 0.0);
+            if (j < k) ok = ok && (rs[j] <= tol) && (r2 == r2);
+        }
+        st->nhvp += kb;
+        if (ok) {
+            for (int j = 0; j < kb; ++j) { st->theta[j] = th[j]; st->resid[j] = rs[j]; }
+            st->done = 1;
+        }
+    }
+}
+
 int fast_grid(long long work_items) {
     long long b = (work_items + 255) / 256;
     return (int)(b < 1 ? 1 : (b > MOTO_RED_BLOCKS ? MOTO_RED_BLOCKS : b));
@@ -279,4 +329,14 @@ int fast_negc_max(moto_ctx* c, double* partial_max, int* nmax_out) {
 int fast_cheb_coef(moto_ctx* c, int k, int d, double margin, double lnorm, double hi_user, const double* partial_max, int nmax) {
     k_cheb_coef<<<1, 32, 0, c->stream>>>(c->st, k, d, margin, lnorm, hi_user, partial_max, nmax);
     return 1;
+}
+
+// T = A X must already be in d_T.  Sets done (and theta, resid) when every wanted A-residual is below tol.
+int fast_acheck(moto_ctx* c, int kb, int k, double tol, const double* d_T, double* partials) {
+    const long long n3 = 3ll * c->N;
+    const int g = fast_grid(n3);
+    if (kb == 1) k_acheck_dots<1><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, partials, &c->st->done);
+    else k_acheck_dots<2><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, partials, &c->st->done);
+    k_acheck_final<<<1, 32 * 3 * kb, 0, c->stream>>>(partials, g, kb, k, tol, c->st);
+    return 2;
 }
