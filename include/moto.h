@@ -136,6 +136,14 @@ moto_status moto_gram(moto_ctx* ctx, const double* d_S, int ns, const double* d_
 moto_status moto_rayleigh_ritz(moto_ctx* ctx, const double* d_GA, const double* d_GB, int n, int nev,
                                double* d_theta, double* d_C);
 
+/* One step of the three-term recurrence the transformed solver is made of (the kernel that dominates
+ * moto_lowest_modes), exported so it can be tested and timed alone:
+ *   d_out = alpha (Hess[V] - c0 V) + beta U      (U may be NULL: beta ignored; d_out may alias d_U, not d_V)
+ * kind 0 only.  V must be tangent (it is NOT re-projected: solver mode, reading A24); c_i = m_i.g_i is recomputed
+ * from d_spins when refresh_c != 0, else the values cached in the workspace by the previous call are used. */
+moto_status moto_hvp_three_term(moto_ctx* ctx, const double* d_spins, const double* d_V, int k, double alpha, double c0,
+                                double beta, const double* d_U, double* d_out, int refresh_c);
+
 /* Host-buffer variants (end-to-end path): same semantics, all array arguments are HOST pointers
  * (pinned or pageable); the library stages them through its workspace (host->device, compute,
  * device->host) and synchronises the stream before returning. */

@@ -62,6 +62,8 @@ _SIGS = {
     "moto_lowest_modes": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
                                     C.POINTER(SolveInfo)]),
     "moto_mmf_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p, C.c_void_p]),
+    "moto_hvp_three_term": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p,
+                                      C.c_void_p, C.c_int]),
     "moto_transport": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "moto_gram": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
     "moto_rayleigh_ritz": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
@@ -192,6 +194,18 @@ class Context:
         HV = out if out is not None else self._empty(k, self.N, 3)
         self._check(self.lib.moto_hvp(self._h, _ptr(spins), _ptr(V), k, _ptr(HV)))
         return HV
+
+    def hvp_three_term(self, spins, V, alpha, c0, beta, U=None, out=None, refresh_c=True):
+        """moto_hvp_three_term: out = alpha (Hess[V] - c0 V) + beta U for tangent V (solver mode)."""
+        _dev_f64(spins, (self.N, 3))
+        k = V.shape[0]
+        _dev_f64(V, (k, self.N, 3))
+        if U is not None:
+            _dev_f64(U, (k, self.N, 3))
+        out = out if out is not None else self._empty(k, self.N, 3)
+        self._check(self.lib.moto_hvp_three_term(self._h, _ptr(spins), _ptr(V), k, float(alpha), float(c0), float(beta), _ptr(U),
+                                                 _ptr(out), int(bool(refresh_c))))
+        return out
 
     def lowest_modes(self, spins, k, tol, max_iter=200, V0=None, allow_notconv=False):
         """moto_lowest_modes -> (lam [k], V [k][N][3], info dict)."""

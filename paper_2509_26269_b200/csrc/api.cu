@@ -226,6 +226,20 @@ moto_status moto_transport(moto_ctx* c, const double* d_spins_new, double* d_V, 
     return MOTO_OK;
 }
 
+moto_status moto_hvp_three_term(moto_ctx* c, const double* d_spins, const double* d_V, int k, double alpha, double c0, double beta,
+                                const double* d_U, double* d_out, int refresh_c) {
+    if (!c) return MOTO_EINVAL;
+    if (c->kind != MOTO_KIND_TRI2D) return moto_fail(c, MOTO_ESTATE, "moto_hvp_three_term: spin lattices only");
+    if (!d_spins || !d_V || !d_out || d_V == d_out) return moto_fail(c, MOTO_EINVAL, "moto_hvp_three_term: null or aliased argument");
+    if (k < 1 || k > MOTO_KMAX) return moto_fail(c, MOTO_EINVAL, "moto_hvp_three_term: k out of range [1, MOTO_KMAX]");
+    if (refresh_c) c->launches += spin_curvature(c, d_spins, c->c);
+    int n = spin_hvp_tma_ex(c, d_spins, c->c, d_V, k, d_out, nullptr, nullptr, 1, alpha, c0, beta, d_U, nullptr);
+    if (n <= 0) n = spin_hvp_three_term_generic(c, d_spins, c->c, d_V, k, alpha, c0, beta, d_U, d_out);
+    c->launches += n;
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return MOTO_OK;
+}
+
 moto_status moto_gram(moto_ctx* c, const double* d_S, int ns, const double* d_T, int nt, double* d_G) {
     if (!c) return MOTO_EINVAL;
     if (!d_S || !d_T || !d_G || ns < 1 || nt < 1 || ns > MOTO_NS || nt > 2 * MOTO_NS) return moto_fail(c, MOTO_EINVAL, "moto_gram: bad argument");

@@ -117,6 +117,27 @@ __global__ void __launch_bounds__(256) k_hvp_generic(Lat l, const double* __rest
     }
 }
 
+// three-term step on the generic path: out = alpha (Hess[v] - c0 v) + beta u, solver mode (c given, v tangent)
+__global__ void __launch_bounds__(256) k_three_term_generic(Lat l, const double* __restrict__ m, const double* __restrict__ cvec,
+                                                            const double* __restrict__ V, int k, double alpha, double c0, double beta,
+                                                            const double* U, double* out) {
+    const long long N = (long long)l.Lx * l.Ly;
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int iy = (int)(i / l.Lx), ix = (int)(i - (long long)iy * l.Lx);
+    Nbrs n = neighbours(l, ix, iy);
+    d3 mi = ld3(m, i);
+    const double c = cvec[i];
+    for (int a = 0; a < k; ++a) {
+        const double* __restrict__ v = V + (size_t)a * 3 * N;
+        d3 vi = ld3(v, i);
+        d3 h = axpy3(-c, vi, proj3(mi, stencil_field(l, v, n, vi.z)));
+        d3 o = scale3(alpha, axpy3(-c0, vi, h));
+        if (U) o = axpy3(beta, ld3(U + (size_t)a * 3 * N, i), o);
+        st3(out + (size_t)a * 3 * N, i, o);
+    }
+}
+
 // ---------------------------------------------------------------- tangent projection of a block, in place
 __global__ void k_project(long long N, const double* __restrict__ m, double* __restrict__ V, int k) {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -209,6 +230,14 @@ int spin_hvp(moto_ctx* c, const double* m, const double* cvec, const double* V, 
         if (project_input) k_hvp_generic<false, true><<<blocks, 256, 0, c->stream>>>(l, m, cvec, V, k, HV, d_done);
         else k_hvp_generic<false, false><<<blocks, 256, 0, c->stream>>>(l, m, cvec, V, k, HV, d_done);
     }
+    return 1;
+}
+
+int spin_hvp_three_term_generic(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double alpha, double c0,
+                                double beta, const double* U, double* out) {
+    Lat l = make_lat(c);
+    const long long N = c->N;
+    k_three_term_generic<<<(int)((N + 255) / 256), 256, 0, c->stream>>>(l, m, cvec, V, k, alpha, c0, beta, U, out);
     return 1;
 }
 

@@ -353,3 +353,30 @@ def test_cfg3_scaled_316_vs_golden(moto):
     lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-7, max_iter=20000)
     assert info["converged"], info
     assert np.max(np.abs(lam.cpu().numpy() - gold[:2]) / np.abs(gold[:2])) <= EIG_TOL
+
+
+@pytest.mark.parametrize("case", [1, 2, 3, 5, 6, 8])
+@pytest.mark.parametrize("path", [1, 2])
+def test_hvp_three_term_parity(moto, case, path):
+    # the recurrence step of the transformed solver: out = alpha (Hess[V] - c0 V) + beta U, tangent V, solver mode
+    w = TMA_CASES[case]()
+    model = model_of(w)
+    ctx = moto.spin_context(w, kmax=8)
+    ctx.set_solver(hvp_path=path)
+    rng = np.random.default_rng(case)
+    for k in (1, 2, 3):
+        V = wl.random_block(w.N, k, seed=300 + case)
+        V = V - np.sum(V * w.spins[None], axis=2, keepdims=True) * w.spins[None]     # tangent input
+        U = wl.random_block(w.N, k, seed=400 + case)
+        alpha, c0, beta = rng.uniform(-2, 2), rng.uniform(-1, 20), rng.uniform(-2, 2)
+        HV = so.hvp(model, w.spins, V)
+        ref = alpha * (HV - c0 * V) + beta * U
+        out = ctx.hvp_three_term(dev(w.spins), dev(V), alpha, c0, beta, U=dev(U)).cpu().numpy()
+        assert rel_l2(out, ref) <= HVP_TOL
+        # no operand, cached c
+        out2 = ctx.hvp_three_term(dev(w.spins), dev(V), alpha, c0, 0.0, refresh_c=False).cpu().numpy()
+        assert rel_l2(out2, alpha * (HV - c0 * V)) <= HVP_TOL
+        # in place over the operand (what the solver does from the third step on)
+        Ud = dev(U)
+        ctx.hvp_three_term(dev(w.spins), dev(V), alpha, c0, beta, U=Ud, out=Ud, refresh_c=False)
+        assert rel_l2(Ud.cpu().numpy(), ref) <= HVP_TOL
