@@ -107,12 +107,13 @@ __device__ __forceinline__ d3 lds3(const double* p) { return mk3(p[0], p[1], p[2
 
 // ---------------------------------------------------------------------------------------------------------
 template <int K, bool API>
-__global__ void __launch_bounds__(NTHREADS, 1)
+__global__ void __launch_bounds__(NTHREADS, 1)   // registers are granted per 4 warps: 9 warps count as 12 => 168 regs/thread
 k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     using C = Cfg<K, API>;
     constexpr int F = C::F, S = C::S, NSLOT = C::NSLOT, FS0 = C::FS0, NFS = C::NFS;
     constexpr int NK = K * (K + 1) / 2;
-    if (p.done && *p.done) return;
+    // programmatic dependent launch: let the next K1 in the stream start its prologue as soon as this CTA's SM frees up
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* smain = reinterpret_cast<double*>(smem_raw);          // [F][NSLOT][ROWD]
@@ -131,7 +132,11 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NCW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (warp == NCW && lane < 10) asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&maps.m_chunk + lane)) : "memory");
     __syncthreads();
+    // everything above overlapped the tail of the previous kernel; nothing it wrote has been touched yet
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (p.done && *p.done) return;
 
     const long long lo = (p.total * blockIdx.x) / gridDim.x, hi = (p.total * (blockIdx.x + 1)) / gridDim.x;
 #ifdef MOTO_K1_TIMING
@@ -146,7 +151,6 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         // ================================================================ producer warp: all 32 lanes issue TMA boxes
         // kinds of box per row (or per chunk): F main fields, NFS left-wrap sides, NFS right-wrap sides, c (SOLVER)
         constexpr int KINDS = F + 2 * NFS + (API ? 0 : 1);
-        if (lane < 10) asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&maps.m_chunk + lane)) : "memory");
         unsigned n = 0;
         long long pos = lo;
         while (pos < hi) {
@@ -231,7 +235,26 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
 #ifdef MOTO_K1_TIMING
         if (threadIdx.x == 0 && pos == lo) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); p.dbg[blockIdx.x * 4 + 2] = t; }
 #endif
+        // The three-term operand U is read straight from global memory (no reuse, so it does not ride the ring); its
+        // loads are issued one block ahead so that a whole block of arithmetic hides their latency (issuing them at the
+        // top of the same block left the warps on the long scoreboard).  out may alias U: a site's U is read and
+        // written by the same thread, one block apart.
+        const bool use_u = !API && p.cheb && p.U;
+        d3 uA[K], uB[K], nA[K], nB[K];
+        auto load_u = [&](int jb, d3 (&ua)[K], d3 (&ub)[K]) {
+            const int r = jb * RC + 2 * rp;
+            if (use_u && active && r < nrows) {
+                const long long sA = (long long)(y_start + r) * Lx + x;
+#pragma unroll
+                for (int a = 0; a < K; ++a) {
+                    ua[a] = ld3(p.U + (size_t)a * 3 * N, sA);
+                    ub[a] = (r + 1 < nrows) ? ld3(p.U + (size_t)a * 3 * N, sA + Lx) : mk3(0.0, 0.0, 0.0);
+                }
+            }
+        };
+        load_u(0, uA, uB);
         for (int j = 0; j < nb; ++j) {
+            if (j + 1 < nb) load_u(j + 1, nA, nB);
             if (j + 1 < Q) mbar_wait(&full[(n + j + 1) % S], ((n + j + 1) / S) & 1u);
             const int rA = j * RC + 2 * rp;
             if (active && rA < nrows) {
@@ -243,16 +266,6 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                     slot[q] = (int)((n + rr / RC) % S) * RC + (rr % RC);
                 }
                 const long long siteA = (long long)(y_start + rA) * Lx + x, siteB = siteA + Lx;
-                // the three-term operand is read straight from global memory (no reuse): issue the loads before the
-                // shared-memory phase so their latency overlaps this block's arithmetic
-                d3 uA[K], uB[K];
-                if (!API && p.cheb && p.U) {
-#pragma unroll
-                    for (int a = 0; a < K; ++a) {
-                        uA[a] = ld3(p.U + (size_t)a * 3 * N, siteA);
-                        uB[a] = haveB ? ld3(p.U + (size_t)a * 3 * N, siteB) : mk3(0.0, 0.0, 0.0);
-                    }
-                }
                 double cA = 0.0, cB = 0.0;
                 if (!API) { cA = sc[slot[1] * CROWD + col + 2]; cB = sc[slot[2] * CROWD + col + 2]; }
                 // field 0: m.  API: all ten sites (projection of the neighbours + stencil for c); SOLVER: centres only.
@@ -317,6 +330,10 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                     st3(p.out + (size_t)a * 3 * N, siteA, oA);
                     if (haveB) st3(p.out + (size_t)a * 3 * N, siteB, oB);
                 }
+            }
+            if (use_u) {
+#pragma unroll
+                for (int a = 0; a < K; ++a) { uA[a] = nA[a]; uB[a] = nB[a]; }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[(n + j) % S]);
@@ -383,8 +400,14 @@ bool launch(moto_ctx* c, const Maps& maps, const KParams& p, int grid) {
         if (cudaFuncSetAttribute(k_hvp_tma<K, API>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return false;
         attr_set = true;
     }
-    k_hvp_tma<K, API><<<grid, NTHREADS, C::SMEM, c->stream>>>(maps, p);
-    return true;
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(NTHREADS); cfg.dynamicSmemBytes = C::SMEM; cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_hvp_tma<K, API>, maps, p) == cudaSuccess;
 }
 
 }  // namespace
