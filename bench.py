@@ -210,10 +210,13 @@ def main():
     peak, peak_src = measured_peaks()
     achieved = alg_bytes / (tt_ms * 1e-3) / 1e9
     achieved_api = alg_bytes_api / (hvp_ms * 1e-3) / 1e9
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "k1_traffic.json")
-    if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(args.workload)
+    traffic = None   # dram__bytes_read + dram__bytes_write of the roofline kernel from the committed ncu --set full capture
+    tp = os.path.join(ROOT, "profiles", "r01_k1_traffic.csv")
+    if os.path.exists(tp) and args.workload == "cfg3":
+        for line in open(tp).read().splitlines()[1:]:
+            f = line.split(",")
+            if f[0] == "cfg3" and "three-term" in line:
+                traffic = float(f[-3]) + float(f[-2])
 
     # ---------------------------------------------------------------- (B) the step, inputs resident in HBM
     def step():
