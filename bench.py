@@ -134,6 +134,102 @@ def run_reference(args):
                       "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
+def run_report(args):
+    """`--report`: the per-config table BASELINE.json north_star asks for (five configs, 1 GPU): HVPs/s, Gsite-updates/s,
+    time to the lowest-k modes, MMF loop, peak incremental memory, with the oracle timed beside it (cpu_baseline leg:
+    bounded, as it stands).  Prints markdown; `profiles/r01_five_configs.md` is a committed copy of one run."""
+    import torch
+    import paper_2509_26269_b200 as moto
+    from paper_2509_26269_b200 import workloads as wl
+    dev = torch.device("cuda", 0)
+    peak, _ = measured_peaks()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(fn, reps):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        ev0.record()
+        for _ in range(reps):
+            fn()
+        ev1.record()
+        torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1) / reps
+
+    rows, orows = [], []
+    cfgs = [("0", wl.config0(), 0), ("1", wl.config1(), 0), ("2", wl.config2(), 100), ("3", wl.config3(), 200), ("4", wl.config4(), 100)]
+    for name, w, nsteps in cfgs:
+        cart = hasattr(w, "positions")
+        ctx = moto.cart_context(w, kmax=w.k) if cart else moto.spin_context(w, kmax=w.k)
+        if cart:
+            ctx.set_solver(guard=2) if w.k + 2 <= ctx.kmax else None
+        N = ctx.N
+        x = torch.as_tensor(w.positions if cart else w.spins, device=dev)
+        V = torch.randn(w.k, N, 3, dtype=torch.float64, device=dev)
+        HV = torch.empty_like(V)
+        hvp_ms = timed(lambda: ctx.hvp(x, V, out=HV), 50)
+        alg = 24 * N * (1 + 2 * w.k)
+        tol = w.tol
+        lam, Vm, info = ctx.lowest_modes(x, w.k, tol=tol, max_iter=20000, allow_notconv=True)   # warm-up (JIT-free, but first-touch)
+        torch.cuda.synchronize()
+        ev0.record()
+        lam, Vm, info = ctx.lowest_modes(x, w.k, tol=tol, max_iter=20000, allow_notconv=True)
+        ev1.record(); torch.cuda.synchronize()
+        solve_ms = ev0.elapsed_time(ev1)
+        # MMF loop: re-solve (warm start, transported block) -> energy/gradient -> reflected step along v1
+        mmf = ""
+        if nsteps:
+            xm, Vw = x.clone(), Vm.clone()
+            torch.cuda.synchronize(); ev0.record()
+            tot_it = 0
+            for _ in range(nsteps):
+                lam_s, Vw, inf_s = ctx.lowest_modes(xm, w.k, tol=tol, max_iter=20000, V0=Vw, allow_notconv=True)
+                tot_it += inf_s["iters"]
+                xm, fn = ctx.mmf_step(xm, Vw[:1].contiguous(), w.dt, out=xm)
+                if not cart:
+                    ctx.transport(xm, Vw)
+            ev1.record(); torch.cuda.synchronize()
+            l = lam_s.cpu().numpy()
+            mmf = f"{nsteps} steps, {ev0.elapsed_time(ev1):.0f} ms ({ev0.elapsed_time(ev1) / nsteps:.2f} ms/step, {tot_it} solver iterations), final \\|F_mmf\\| = {fn.item():.3e}, λ₁, λ₂ = {l[0]:.5f}, {l[1]:.5f}"
+        gbs = alg / (hvp_ms * 1e-3) / 1e9
+        rows.append(f"| {name} | {N} | {w.k} | {hvp_ms * 1e3:.1f} | {w.k * 1e3 / hvp_ms:.3g} | {N * w.k / (hvp_ms * 1e-3) / 1e9:.3g} | "
+                    f"{gbs:.0f} ({gbs / peak:.2f} of measured, {gbs / 8000:.2f} of 8 TB/s{'' if N >= 500000 else '; below L2 size: latency-bound'}) | "
+                    f"{solve_ms:.2f} | {info['iters']} | {info['hvp_count']} | {max(info['resid']):.1e} | {ctx.workspace_bytes / 1e6:.1f} | {mmf or '—'} |")
+        # ---- oracle beside it (cpu_baseline leg, bounded)
+        if not args.no_cpu_baseline:
+            if cart:
+                from oracle import cart_oracle as co
+                mdl = co.MorseModel(w.cell, w.De, w.alpha, w.r0, w.rc, w.fixed)
+                t0 = time.perf_counter(); co.hvp(mdl, w.positions, V.cpu().numpy()); t_h = time.perf_counter() - t0
+                t0 = time.perf_counter(); lr, _ = co.lowest_modes(mdl, w.positions, w.k); t_s = time.perf_counter() - t0
+                how = "dense eigh 2421²"
+            else:
+                from oracle import spin_oracle as so
+                mdl = so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
+                t0 = time.perf_counter(); so.hvp(mdl, w.spins, V.cpu().numpy()); t_h = time.perf_counter() - t0
+                if N <= 5000:
+                    t0 = time.perf_counter(); lr, _ = so.lowest_modes(mdl, w.spins, w.k); t_s = time.perf_counter() - t0
+                    how = f"dense eigh {2 * N}²"
+                elif N <= 70000:
+                    t0 = time.perf_counter(); lr, _ = so.lowest_modes_sparse(mdl, w.spins, w.k, extra=2); t_s = time.perf_counter() - t0
+                    how = "ARPACK shift-invert (sparse LU)"
+                else:
+                    lr, t_s, how = None, float("nan"), "ARPACK shift-invert: ~70 min on 8 cores (tests/golden/make_cfg3_eigs.py), not re-run here"
+            err = "" if lr is None else f"{np.max(np.abs(lam.cpu().numpy() - lr[:w.k]) / np.maximum(np.abs(lr[:w.k]), 1e-3)):.1e}"
+            orows.append(f"| {name} | {t_h * 1e3:.0f} | {t_s:.2f} | {how} | {err} |")
+        ctx.close()
+    import threadpoolctl
+    cores = max([i.get("num_threads", 1) for i in threadpoolctl.threadpool_info()] + [1])
+    print("| cfg | N | k | moto_hvp µs | HVP/s | Gsite-updates/s | HVP GB/s (algorithmic 24N(1+2k)) | lowest-k solve ms | iters | HVPs | max resid | peak incremental MB | MMF loop |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+    print("\n".join(rows))
+    if orows:
+        print(f"\nOracle on the host ({cores} BLAS threads, {os.cpu_count()} CPUs), as it stands — a baseline, not the target:\n")
+        print("| cfg | oracle HVP ms (explicit Hessian rebuilt) | oracle lowest-k s | how | max rel. eigenvalue difference GPU vs oracle |")
+        print("|---|---|---|---|---|")
+        print("\n".join(orows))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -144,9 +240,12 @@ def main():
     ap.add_argument("--max-iter", type=int, default=20000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--hvp-reps", type=int, default=60)
+    ap.add_argument("--report", action="store_true", help="five-config table (markdown) instead of the JSON line")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.report:
+        return run_report(args)
 
     import torch
     import paper_2509_26269_b200 as moto
