@@ -134,6 +134,18 @@ def run_reference(args):
                       "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
+def reduce_over_ranks(dist, elapsed, units, device):
+    """Replicas-only multi-GPU accounting: time = MAX over ranks, work = SUM over ranks.
+    `dist` is torch.distributed (already initialised) or None; no data-path collective exists anywhere else."""
+    if dist is None:
+        return float(elapsed), float(units)
+    import torch
+    t = torch.tensor([float(elapsed), float(units)], dtype=torch.float64, device=device)
+    tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+    return float(tmax[0]), float(tsum[1])
+
+
 def run_report(args):
     """`--report`: the per-config table BASELINE.json north_star asks for (five configs, 1 GPU): HVPs/s, Gsite-updates/s,
     time to the lowest-k modes, MMF loop, peak incremental memory, with the oracle timed beside it (cpu_baseline leg:
@@ -346,10 +358,7 @@ def main():
     launches = ctx.launch_count - l0
     hvps = sum(i["hvp_count"] for i in infos)
     if dist is not None:
-        t = torch.tensor([total_ms, float(hvps)], dtype=torch.float64, device=dev)
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        total_ms, hvps = float(tmax[0]), float(tsum[1])
+        total_ms, hvps = reduce_over_ranks(dist, total_ms, hvps, dev)
     value = hvps / (total_ms * 1e-3)
 
     # ---------------------------------------------------------------- (C) end to end through the host-buffer ABI
@@ -374,10 +383,7 @@ def main():
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     if dist is not None:
-        t = torch.tensor([e2e_s, float(e2e_hvps)], dtype=torch.float64, device=dev)
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        e2e_s, e2e_hvps = float(tmax[0]), float(tsum[1])
+        e2e_s, e2e_hvps = reduce_over_ranks(dist, e2e_s, e2e_hvps, dev)
     h2d = 3 * 24 * N + 24 * N          # spins x3 calls + v1
     d2h = 8 * k + 24 * N * k + 8 + 24 * N + 8
 
