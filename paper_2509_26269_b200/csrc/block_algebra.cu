@@ -137,15 +137,15 @@ __global__ void __launch_bounds__(256) k_residual(long long N, int kb, const dou
 __global__ void k_check(const double* __restrict__ partials, int nblk, int kb, int k, double tol, SolverState* st) {
     if (st->done) return;
     __shared__ double r[MOTO_KMAX];
-    int j = threadIdx.x;
+    const int j = threadIdx.x >> 5, lane = threadIdx.x & 31;   // one warp per column, lanes over CTAs, fixed order
     if (j < kb) {
         double s = 0.0;
-        for (int b = 0; b < nblk; ++b) s += partials[b * MOTO_KMAX + j];
-        r[j] = sqrt(s);
-        st->resid[j] = r[j];
+        for (int b = lane; b < nblk; b += 32) s += partials[b * MOTO_KMAX + j];
+        s = warp_sum(s);
+        if (lane == 0) { r[j] = sqrt(s); st->resid[j] = r[j]; }
     }
     __syncthreads();
-    if (j == 0) {
+    if (threadIdx.x == 0) {
         bool ok = true, bad = false;
         for (int a = 0; a < k; ++a) { ok = ok && (r[a] <= tol); bad = bad || !(r[a] == r[a]); }
         if (bad) { st->bad = 1; st->done = 1; }
@@ -296,7 +296,7 @@ int block_update(moto_ctx* c, int kb) {
 int block_residual(moto_ctx* c, const double* m_or_null, int kb, int k, double tol) {
     k_residual<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, kb, m_or_null, c->kind == MOTO_KIND_CARTESIAN ? c->lat.d_fixed : nullptr,
                                                        c->X, c->AX, c->W, c->st, c->partials);
-    k_check<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, kb, k, tol, c->st);
+    k_check<<<1, 32 * kb, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, kb, k, tol, c->st);
     return 2;
 }
 

@@ -13,27 +13,34 @@ namespace {
 constexpr int NMAX = MOTO_NS;       // 24
 constexpr int LD = NMAX + 1;        // smem leading dimension
 constexpr int RR_THREADS = 256;     // gather phase; the dense phase runs on warp 0 alone (warp-level syncs only)
-#define RR_SYNC() __syncwarp()
+// dense phase: one warp (warp-level syncs) for n <= 8, the whole CTA for larger pencils (more rotations per round)
+#define RR_SYNC() do { if (wide) __syncthreads(); else __syncwarp(); } while (0)
 
 struct JacobiScratch { int p[NMAX / 2], q[NMAX / 2]; double c[NMAX / 2], s[NMAX / 2]; double off, diag; };
 
 // Symmetric eigen-decomposition in shared memory: A (n x n, LD) -> diag(A) = eigenvalues, V = eigenvectors (cols).
-__device__ void jacobi_eig(double* A, double* V, int n, JacobiScratch* js) {
-    const int tid = threadIdx.x, nt = 32;   // called by warp 0 only
+__device__ void jacobi_eig(double* A, double* V, int n, JacobiScratch* js, bool wide) {
+    const int tid = threadIdx.x, nt = wide ? blockDim.x : 32;
     for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; V[i * LD + j] = (i == j) ? 1.0 : 0.0; }
     RR_SYNC();
     if (n == 1) return;
     const int np = (n + 1) & ~1, half = np / 2;
     for (int sweep = 0; sweep < 30; ++sweep) {
         double off = 0.0, dg = 0.0;
-        for (int t = tid; t < n * n; t += nt) {
-            int i = t / n, j = t - i * n;
-            double a = A[i * LD + j];
-            if (i == j) dg += a * a; else if (j > i) off += a * a;
-        }
+        if (tid < 32) {   // warp 0 sums (n*n <= 576 entries), everyone reads the verdict
+            for (int t = tid; t < n * n; t += 32) {
+                int i = t / n, j = t - i * n;
+                double a = A[i * LD + j];
+                if (i == j) dg += a * a; else if (j > i) off += a * a;
+            }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) { off += __shfl_xor_sync(0xffffffffu, off, o); dg += __shfl_xor_sync(0xffffffffu, dg, o); }
-        if (off <= 1e-30 * dg || off == 0.0) break;   // off-diagonals below 1e-15 of the diagonal scale: rounding level
+            for (int o = 16; o > 0; o >>= 1) { off += __shfl_xor_sync(0xffffffffu, off, o); dg += __shfl_xor_sync(0xffffffffu, dg, o); }
+            if (tid == 0) { js->off = off; js->diag = dg; }
+        }
+        RR_SYNC();
+        off = js->off; dg = js->diag;
+        RR_SYNC();
+        if (off <= 1e-30 * dg || off == 0.0) break;   // off-diagonals below 1e-15 of the diagonal scale: rounding level   // off-diagonals below 1e-15 of the diagonal scale: rounding level
         for (int r = 0; r < np - 1; ++r) {
             if (tid < half) {
                 int p, q;
@@ -194,9 +201,9 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         A[i * LD + j] = 0.5 * (T[i * LD + j] + T[j * LD + i]);
     }
     __syncthreads();
-    // ---- dense phase: warp 0 alone, warp-level synchronisation only
-    if (tid >= 32) return;
-    nt = 32;
+    // ---- dense phase: warp 0 alone for small pencils (warp-level synchronisation only), the whole CTA otherwise
+    const bool wide = n > 8;
+    if (!wide) { if (tid >= 32) return; nt = 32; }
     if (st && partials) {  // keep a copy for diagnostics
         for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; st->GA[t] = A[i * LD + j]; st->GB[t] = B[i * LD + j]; }
     }
@@ -210,7 +217,7 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
     for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; B[i * LD + j] *= d[i] * d[j]; }
     RR_SYNC();
     // 3. eigen-decomposition of the scaled G_B
-    jacobi_eig(B, U, n, &js);
+    jacobi_eig(B, U, n, &js, wide);
     if (tid == 0) {
         double smax = 0.0;
         for (int j = 0; j < n; ++j) { sig[j] = B[j * LD + j]; if (sig[j] > smax) smax = sig[j]; }
@@ -255,7 +262,7 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
     RR_SYNC();
     for (int t = tid; t < na * na; t += nt) { int a = t / na, b = t - a * na; A[a * LD + b] = 0.5 * (B[a * LD + b] + B[b * LD + a]); }
     RR_SYNC();
-    jacobi_eig(A, Z, na, &js);
+    jacobi_eig(A, Z, na, &js, wide);
     // 5. sort ascending
     if (tid == 0) {
         for (int j = 0; j < na; ++j) { th[j] = A[j * LD + j]; ord[j] = j; }

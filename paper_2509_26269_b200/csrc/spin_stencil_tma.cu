@@ -27,8 +27,8 @@ namespace {
 constexpr int TXMAX = 60;          // strip width (sites); row box = 64 sites starting at xb - 2 (see x3 below)
 constexpr int ROWD = 192;          // doubles per main row slot (64 sites x 3)
 constexpr int SIDED = 16;          // doubles per side row slot (128 B)
-constexpr int RC = 8;              // rows per chunk
-constexpr int NCW = 8;             // consumer warps
+constexpr int RC = 10;             // rows per chunk (= 2 rows per consumer row-pair x 5)
+constexpr int NCW = 10;            // consumer warps: 10 + 1 producer = 11 warps, registers are granted per 4 warps (12)
 constexpr int NTHREADS = (NCW + 1) * 32;
 
 constexpr int CROWD = 64;          // doubles per c row slot (SOLVER mode: c_i rides the ring too)
