@@ -46,7 +46,7 @@ static double stencil_lmax_bound(const moto_spin_params& sp) {
     return best + 0.25 * h * h * 12.0 * (fabs(sp.J) + fabs(sp.D)) * 2.0 + 2.0 * fabs(sp.K);
 }
 
-struct WsLayout { size_t block, c, g, stage, partials, st, cart, total; int nblocks; };
+struct WsLayout { size_t block, c, g, stage, partials, st, flags, cart, total; int nblocks; };
 
 static WsLayout ws_layout(const moto_lattice* lat, int kmax) {
     WsLayout w;
@@ -59,7 +59,8 @@ static WsLayout ws_layout(const moto_lattice* lat, int kmax) {
     w.st = al256(sizeof(SolverState));
     w.cart = lat->kind == MOTO_KIND_CARTESIAN ? cart_lists_bytes(lat) : 0;
     w.nblocks = lat->kind == MOTO_KIND_TRI2D ? 8 : 6;   // spin lattices: + two Chebyshev ping-pong blocks
-    w.total = w.nblocks * w.block + w.c + w.g + w.stage + w.partials + w.st + w.cart;
+    w.flags = 4096;
+    w.total = w.nblocks * w.block + w.c + w.g + w.stage + w.partials + w.st + w.flags + w.cart;
     return w;
 }
 
@@ -110,8 +111,10 @@ moto_status moto_create(const moto_lattice* lat, const void* params, void* d_wor
     c->stage_m = (double*)p; p += w.stage;
     c->partials = (double*)p; p += w.partials;
     c->st = (SolverState*)p; p += w.st;
+    c->flags = (unsigned long long*)p; p += w.flags;
     if (c->kind == MOTO_KIND_CARTESIAN) cart_lists_carve(c, p);
     cudaError_t e = cudaHostAlloc((void**)&c->hstat, 2 * sizeof(HostStatus), cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->flags, 0, w.flags, c->stream);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming);
     if (e != cudaSuccess) {

@@ -68,7 +68,12 @@ static void fast_apply(FastCtx& f, const double* V, double* OV) {
         f.n += fast_dot_waw(c, f.kb, V, OV, f.partialsK, &f.nblkK);
         return;
     }
-    // Chebyshev recurrence Y_0 = V, Y_1 -> T1, Y_2 -> T2, Y_3 -> T1 (in place over its own three-term operand) ...
+    // the whole recurrence in one persistent cooperative launch (neighbour-flag synchronised steps) when it fits ...
+    if (f.degree >= 2 && !getenv("MOTO_NO_MULTISTEP")) {
+        int nk = spin_cheb_multistep(c, f.state, c->c, V, f.kb, f.degree, OV, &c->st->cheb[0][0], &c->st->done);
+        if (nk > 0) { f.n += nk; f.n += fast_dot_waw(c, f.kb, V, OV, f.partialsK, &f.nblkK); return; }
+    }
+    // ... else one launch per step: Y_0 = V, Y_1 -> T1, Y_2 -> T2, Y_3 -> T1 (in place over its own three-term operand) ...
     const double* in = V; const double* prev = nullptr;
     for (int i = 1; i <= f.degree; ++i) {
         double* out = (i == f.degree) ? OV : ((i & 1) ? c->T1 : c->T2);
@@ -117,7 +122,8 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     if (degree < 0 || !can_filter) degree = 0;
     if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
     const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.01;
-    int phase_len = 20, plain_start = 20;
+    // cold start: 20 plain iterations first so that theta_k (hence a) means something; a warm start already has it
+    int phase_len = 20, plain_start = warm_start ? 0 : 20;
     const int acheck_every = 4;
     if (const char* e = getenv("MOTO_PHASE_LEN")) phase_len = atoi(e);      // tuning hooks (not part of the ABI)
     if (const char* e = getenv("MOTO_PLAIN_START")) plain_start = atoi(e);

@@ -45,15 +45,16 @@ template <int K, bool API> struct Cfg {
     static constexpr int SIDE_D = NFS * NSLOT * SIDED;
     static constexpr int C_D = API ? 0 : NSLOT * CROWD;
     static constexpr int RED_D = NCW * 4;                            // V^T HV reduction scratch
-    static constexpr size_t SMEM = (size_t)(MAIN_D + 2 * SIDE_D + C_D + RED_D) * 8 + 2 * S * 8;
+    static constexpr size_t SMEM = (size_t)(MAIN_D + 2 * SIDE_D + C_D + RED_D) * 8 + 2 * S * 8 + 64 * 4;
     static_assert(S >= 3, "ring too shallow");
     static_assert(SMEM <= 232448, "over the 227 KB per-CTA limit");
 };
 
-struct Maps {  // chunk = RC rows, row = 1 row; main = 64 sites, side = 16 doubles
+struct VSet { CUtensorMap chunk, row, schunk, srow; };   // chunk = RC rows, row = 1 row; main = 64 sites, side = 16 doubles
+struct Maps {
     CUtensorMap m_chunk, m_row, m_schunk, m_srow;
-    CUtensorMap v_chunk, v_row, v_schunk, v_srow;
     CUtensorMap c_chunk, c_row;   // c [1][Ly][Lx] fp64, box 64 wide (SOLVER)
+    VSet vset[3];                 // [0] the input block; [1], [2] the ping-pong blocks T1, T2 of a multi-step launch
 };
 
 struct KParams {
@@ -69,6 +70,16 @@ struct KParams {
     const double* coef;      // optional device triple {alpha, c0, beta} overriding the three scalars (device-resident recurrence)
     double* waw;             // [grid][K(K+1)/2] or NULL
     const int* done;
+    // multi-step launch (nsteps > 1): the whole Chebyshev recurrence Y_1..Y_nsteps in one persistent cooperative kernel.
+    // Y_i goes to T1 (i odd) / T2 (i even), the last one to `out`; step i reads Y_{i-1} through TMA (halo) and Y_{i-2}
+    // directly; coefficients of step i at coef + 4 (i - 1).  CTAs synchronise with the few neighbours whose sites they
+    // read as halo through release/acquire flags (no grid-wide barrier, no launch gap between steps).
+    int nsteps;
+    const double* V0;        // the input block (three-term operand of step 2)
+    double *T1, *T2;
+    unsigned long long* flags;   // [grid] last step finished by each CTA, as epoch + step
+    unsigned long long epoch;
+    int* err;                // set when a neighbour wait times out
 #ifdef MOTO_K1_TIMING
     unsigned long long* dbg;   // [grid][4]: smid, t_start, t_first_data, t_end (globaltimer ns)
 #endif
@@ -123,6 +134,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     double* sred = sc + C::C_D;                                   // [NCW][4]
     uint64_t* full = reinterpret_cast<uint64_t*>(sred + C::RED_D);
     uint64_t* empty = full + S;
+    int* sdep = reinterpret_cast<int*>(empty + S);                // [0] = count, [1..] = CTAs this one exchanges halos with
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const Lat& l = p.l;
@@ -133,6 +145,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == NCW && lane < 10) asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&maps.m_chunk + lane)) : "memory");
+    const int nsteps = (!API && p.nsteps > 1) ? p.nsteps : 1;
     __syncthreads();
     // everything above overlapped the tail of the previous kernel; nothing it wrote has been touched yet
     asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -151,7 +164,59 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         // ================================================================ producer warp: all 32 lanes issue TMA boxes
         // kinds of box per row (or per chunk): F main fields, NFS left-wrap sides, NFS right-wrap sides, c (SOLVER)
         constexpr int KINDS = F + 2 * NFS + (API ? 0 : 1);
+        if (nsteps > 1) {   // CTAs whose sites this CTA reads as halo (and which read its sites): same strip above/below, strips left/right
+            if (lane == 0) {
+                int nd = 0;
+                auto cta_of = [&](long long idx) {
+                    long long b = idx * gridDim.x / p.total;
+                    while (b + 1 < (long long)gridDim.x && (p.total * (b + 1)) / gridDim.x <= idx) ++b;
+                    while (b > 0 && (p.total * b) / gridDim.x > idx) --b;
+                    return (int)b;
+                };
+                auto add = [&](int c) { for (int i = 1; i <= nd; ++i) if (sdep[i] == c) return; if (nd < 60) sdep[++nd] = c; };
+                auto add_rows = [&](int sx2, int ya, int yb) {   // rows [ya, yb] of strip sx2
+                    const int c0 = cta_of((long long)sx2 * Ly + ya), c1 = cta_of((long long)sx2 * Ly + yb);
+                    for (int c = c0; c <= c1; ++c) add(c);
+                };
+                add((int)blockIdx.x);
+                long long q = lo;
+                while (q < hi) {
+                    const int sx = (int)(q / Ly), y0 = (int)(q - (long long)sx * Ly);
+                    const int nr = (int)((hi - q) < (long long)(Ly - y0) ? (hi - q) : (Ly - y0)), y1 = y0 + nr;   // rows [y0, y1)
+                    const int ya = y0 > 0 ? y0 - 1 : 0, yb = y1 < Ly ? y1 : Ly - 1;
+                    for (int ds = -1; ds <= 1; ++ds) {
+                        int s2 = sx + ds;
+                        if (s2 < 0) { if (!l.px) continue; s2 += p.nsx; }
+                        if (s2 >= p.nsx) { if (!l.px) continue; s2 -= p.nsx; }
+                        add_rows(s2, ya, yb);
+                        if (l.py && y0 == 0) add_rows(s2, Ly - 1, Ly - 1);
+                        if (l.py && y1 == Ly) add_rows(s2, 0, 0);
+                    }
+                    q += nr;
+                }
+                sdep[0] = nd;
+            }
+            __syncwarp();
+        }
         unsigned n = 0;
+        for (int step = 1; step <= nsteps; ++step) {
+        const VSet& vs = maps.vset[step == 1 ? 0 : (((step - 1) & 1) ? 1 : 2)];   // Y_{step-1}: the input, T1 (odd) or T2 (even)
+        if (step > 1) {   // wait until every halo partner has published step - 1 (bounded spin: a lost partner must not hang the GPU)
+            const int nd = sdep[0];
+            const unsigned long long want = p.epoch + (unsigned long long)(step - 1);
+            for (int d = lane; d < nd; d += 32) {
+                const unsigned long long* f = p.flags + sdep[1 + d];
+                unsigned long long v; int spins = 0;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(f) : "memory");
+                    if (v >= want) break;
+                    __nanosleep(64);
+                } while (++spins < (1 << 22));
+                if (v < want) *p.err = 1;
+            }
+            __syncwarp();
+            asm volatile("fence.proxy.async;" ::: "memory");   // generic-proxy writes of the partners -> this CTA's TMA reads
+        }
         long long pos = lo;
         while (pos < hi) {
             const int sx = (int)(pos / Ly), y_start = (int)(pos - (long long)sx * Ly);
@@ -182,12 +247,12 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                     const int slot = s * RC + i;
                     if (kind < F) {
                         const int f = kind;
-                        const CUtensorMap* mp = f == 0 ? (chunk_ok ? &maps.m_chunk : &maps.m_row) : (chunk_ok ? &maps.v_chunk : &maps.v_row);
+                        const CUtensorMap* mp = f == 0 ? (chunk_ok ? &maps.m_chunk : &maps.m_row) : (chunk_ok ? &vs.chunk : &vs.row);
                         tma_load_3d(smain + ((size_t)f * NSLOT + slot) * ROWD, mp, &full[s], x3, y, f == 0 ? 0 : f - 1);
                     } else if (kind < F + 2 * NFS) {
                         const int q = kind - F, right = q >= NFS, fi = right ? q - NFS : q, f = fi + FS0;
                         if (right ? edgeR : edgeL) {
-                            const CUtensorMap* ms = f == 0 ? (chunk_ok ? &maps.m_schunk : &maps.m_srow) : (chunk_ok ? &maps.v_schunk : &maps.v_srow);
+                            const CUtensorMap* ms = f == 0 ? (chunk_ok ? &maps.m_schunk : &maps.m_srow) : (chunk_ok ? &vs.schunk : &vs.srow);
                             tma_load_3d((right ? sR : sL) + ((size_t)fi * NSLOT + slot) * SIDED, ms, &full[s], right ? 0 : 3 * Lx - SIDED, y,
                                         f == 0 ? 0 : f - 1);
                         }
@@ -198,6 +263,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
             }
             pos += nrows;
         }
+        }   // step
         return;
     }
 
@@ -210,9 +276,18 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     for (int t = 0; t < NK; ++t) waw[t] = 0.0;
     const d3 muB = mk3(l.mu * l.Bx, l.mu * l.By, l.mu * l.Bz);
     const bool use_coef = !API && p.cheb && p.coef;
-    const double ch_alpha = use_coef ? p.coef[0] : p.alpha, ch_c0 = use_coef ? p.coef[1] : p.c0, ch_beta = use_coef ? p.coef[2] : p.beta;
 
     unsigned n = 0;
+    for (int step = 1; step <= nsteps; ++step) {
+    // per-step operands: coefficients, three-term operand Y_{step-2} (same-site, same-thread data), destination
+    const double* cf = use_coef ? p.coef + 4 * (step - 1) : nullptr;
+    const double ch_alpha = cf ? cf[0] : p.alpha, ch_c0 = cf ? cf[1] : p.c0, ch_beta = cf ? cf[2] : p.beta;
+    const double* Ustep = p.U;
+    double* outp = p.out;
+    if (nsteps > 1) {
+        Ustep = step == 1 ? nullptr : (step == 2 ? p.V0 : ((step & 1) ? p.T1 : p.T2));     // Y_{step-2}
+        outp = step == nsteps ? p.out : ((step & 1) ? p.T1 : p.T2);                          // Y_step (in place over Y_{step-2})
+    }
     long long pos = lo;
     while (pos < hi) {
         const int sx = (int)(pos / Ly), y_start = (int)(pos - (long long)sx * Ly);
@@ -239,7 +314,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         // loads are issued one block ahead so that a whole block of arithmetic hides their latency (issuing them at the
         // top of the same block left the warps on the long scoreboard).  out may alias U: a site's U is read and
         // written by the same thread, one block apart.
-        const bool use_u = !API && p.cheb && p.U;
+        const bool use_u = !API && p.cheb && Ustep;
         d3 uA[K], uB[K], nA[K], nB[K];
         auto load_u = [&](int jb, d3 (&ua)[K], d3 (&ub)[K]) {
             const int r = jb * RC + 2 * rp;
@@ -247,8 +322,8 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                 const long long sA = (long long)(y_start + r) * Lx + x;
 #pragma unroll
                 for (int a = 0; a < K; ++a) {
-                    ua[a] = ld3(p.U + (size_t)a * 3 * N, sA);
-                    ub[a] = (r + 1 < nrows) ? ld3(p.U + (size_t)a * 3 * N, sA + Lx) : mk3(0.0, 0.0, 0.0);
+                    ua[a] = ld3(Ustep + (size_t)a * 3 * N, sA);
+                    ub[a] = (r + 1 < nrows) ? ld3(Ustep + (size_t)a * 3 * N, sA + Lx) : mk3(0.0, 0.0, 0.0);
                 }
             }
         };
@@ -322,13 +397,13 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                     if (!API && p.cheb) {
                         oA = scale3(ch_alpha, axpy3(-ch_c0, vA[a], oA));
                         oB = scale3(ch_alpha, axpy3(-ch_c0, vB[a], oB));
-                        if (p.U) {
+                        if (Ustep) {
                             oA = axpy3(ch_beta, uA[a], oA);
                             oB = axpy3(ch_beta, uB[a], oB);
                         }
                     }
-                    st3(p.out + (size_t)a * 3 * N, siteA, oA);
-                    if (haveB) st3(p.out + (size_t)a * 3 * N, siteB, oB);
+                    st3(outp + (size_t)a * 3 * N, siteA, oA);
+                    if (haveB) st3(outp + (size_t)a * 3 * N, siteB, oB);
                 }
             }
             if (use_u) {
@@ -342,6 +417,15 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         n += Q;
         pos += nrows;
     }
+    if (nsteps > 1) {   // publish "this CTA has finished step": every consumer's stores first, then one release store
+        __threadfence();
+        asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");
+        if (threadIdx.x == 0) {
+            const unsigned long long v = p.epoch + (unsigned long long)step;
+            asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p.flags + blockIdx.x), "l"(v) : "memory");
+        }
+    }
+    }   // step
 
 #ifdef MOTO_K1_TIMING
     if (threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); p.dbg[blockIdx.x * 4 + 3] = t; }
@@ -392,6 +476,11 @@ bool encode(CUtensorMap* map, const double* base, int Lx, int Ly, int nvec, int 
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+bool encode_vset(VSet* v, const double* base, int Lx, int Ly, int nvec) {
+    return encode(&v->chunk, base, Lx, Ly, nvec, ROWD, RC) && encode(&v->row, base, Lx, Ly, nvec, ROWD, 1) &&
+           encode(&v->schunk, base, Lx, Ly, nvec, SIDED, RC) && encode(&v->srow, base, Lx, Ly, nvec, SIDED, 1);
+}
+
 template <int K, bool API>
 bool launch(moto_ctx* c, const Maps& maps, const KParams& p, int grid) {
     using C = Cfg<K, API>;
@@ -404,8 +493,13 @@ bool launch(moto_ctx* c, const Maps& maps, const KParams& p, int grid) {
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3(grid); cfg.blockDim = dim3(NTHREADS); cfg.dynamicSmemBytes = C::SMEM; cfg.stream = c->stream;
     cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    if (p.nsteps > 1) {   // CTAs wait on each other's flags: they must all be resident
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+    } else {
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+    }
     cfg.attrs = attr; cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, k_hvp_tma<K, API>, maps, p) == cudaSuccess;
 }
@@ -446,8 +540,7 @@ int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const doub
         memset(&maps, 0, sizeof(maps));
         bool ok = encode(&maps.m_chunk, m, Lx, Ly, 1, ROWD, RC) && encode(&maps.m_row, m, Lx, Ly, 1, ROWD, 1) &&
                   encode(&maps.m_schunk, m, Lx, Ly, 1, SIDED, RC) && encode(&maps.m_srow, m, Lx, Ly, 1, SIDED, 1) &&
-                  encode(&maps.v_chunk, V + a0 * bs, Lx, Ly, kk, ROWD, RC) && encode(&maps.v_row, V + a0 * bs, Lx, Ly, kk, ROWD, 1) &&
-                  encode(&maps.v_schunk, V + a0 * bs, Lx, Ly, kk, SIDED, RC) && encode(&maps.v_srow, V + a0 * bs, Lx, Ly, kk, SIDED, 1);
+                  encode_vset(&maps.vset[0], V + a0 * bs, Lx, Ly, kk);
         if (ok && cvec) ok = encode(&maps.c_chunk, cvec, Lx, Ly, 1, CROWD, RC, 1) && encode(&maps.c_row, cvec, Lx, Ly, 1, CROWD, 1, 1);
         if (!ok) return launches ? -1 : 0;
         KParams p;
@@ -458,6 +551,7 @@ int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const doub
         p.U = U ? U + a0 * bs : nullptr;
         p.alpha = alpha; p.c0 = c0; p.beta = beta; p.cheb = cheb; p.coef = d_coef;
         p.waw = waw_partials; p.done = d_done;
+        p.nsteps = 1; p.V0 = nullptr; p.T1 = p.T2 = nullptr; p.flags = nullptr; p.epoch = 0; p.err = nullptr;
 #ifdef MOTO_K1_TIMING
         p.dbg = (unsigned long long*)(c->partials + 100000);
 #endif
@@ -469,6 +563,53 @@ int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const doub
         ++launches;
     }
     return launches;
+}
+
+template <int K>
+static int coop_limit_of() {
+    using C = Cfg<K, false>;
+    int dev = 0, sms = 0, per_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(k_hvp_tma<K, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return -1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_hvp_tma<K, false>, NTHREADS, C::SMEM) != cudaSuccess) return -1;
+    return sms * per_sm;
+}
+int spin_tma_coop_limit(int k) { return k == 2 ? coop_limit_of<2>() : coop_limit_of<1>(); }
+
+// The whole Chebyshev recurrence of one operator application in ONE persistent cooperative launch:
+// OUT = Y_d with Y_0 = V, Y_i = alpha_i (Hess[Y_{i-1}] - c0 Y_{i-1}) + beta_i Y_{i-2}, coefficients at d_coef + 4 (i - 1)
+// (device memory), Y_1..Y_{d-1} in the context's T1/T2 blocks.  k <= 2, d >= 2.  Returns launches or 0 if not applicable.
+int spin_cheb_multistep(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
+                        const double* d_coef, const int* d_done) {
+    if (!spin_tma_applicable(c) || k > 2 || d < 2 || !c->T1 || !cvec) return 0;
+    if (((uintptr_t)m & 15) || ((uintptr_t)V & 15) || ((uintptr_t)cvec & 15)) return 0;
+    const int Lx = c->lat.Lx, Ly = c->lat.Ly;
+    const int grid = spin_tma_grid(c);
+    if (c->coop_max_ctas == 0) c->coop_max_ctas = spin_tma_coop_limit(k);
+    if (grid > c->coop_max_ctas) return 0;
+    Maps maps;
+    memset(&maps, 0, sizeof(maps));
+    bool ok = encode(&maps.m_chunk, m, Lx, Ly, 1, ROWD, RC) && encode(&maps.m_row, m, Lx, Ly, 1, ROWD, 1) &&
+              encode(&maps.m_schunk, m, Lx, Ly, 1, SIDED, RC) && encode(&maps.m_srow, m, Lx, Ly, 1, SIDED, 1) &&
+              encode(&maps.c_chunk, cvec, Lx, Ly, 1, CROWD, RC, 1) && encode(&maps.c_row, cvec, Lx, Ly, 1, CROWD, 1, 1) &&
+              encode_vset(&maps.vset[0], V, Lx, Ly, k) && encode_vset(&maps.vset[1], c->T1, Lx, Ly, k) &&
+              encode_vset(&maps.vset[2], c->T2, Lx, Ly, k);
+    if (!ok) return 0;
+    KParams p;
+    p.l = make_lat(c);
+    p.nsx = (Lx + TXMAX - 1) / TXMAX;
+    p.total = (long long)p.nsx * Ly;
+    p.m = m; p.cvec = cvec; p.out = OUT; p.U = nullptr;
+    p.alpha = p.c0 = p.beta = 0.0; p.cheb = 1; p.coef = d_coef;
+    p.waw = nullptr; p.done = d_done;
+    p.nsteps = d; p.V0 = V; p.T1 = c->T1; p.T2 = c->T2;
+    p.flags = c->flags; c->epoch += 1024; p.epoch = c->epoch; p.err = &c->st->bad;
+#ifdef MOTO_K1_TIMING
+    p.dbg = (unsigned long long*)(c->partials + 100000);
+#endif
+    const bool l_ok = k == 2 ? launch<2, false>(c, maps, p, grid) : launch<1, false>(c, maps, p, grid);
+    return l_ok ? 1 : 0;
 }
 
 int spin_hvp_tma(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input,

@@ -380,3 +380,22 @@ def test_hvp_three_term_parity(moto, case, path):
         Ud = dev(U)
         ctx.hvp_three_term(dev(w.spins), dev(V), alpha, c0, beta, U=Ud, out=Ud, refresh_c=False)
         assert rel_l2(Ud.cpu().numpy(), ref) <= HVP_TOL
+
+
+@pytest.mark.parametrize("case", [1, 3, 8])
+def test_multistep_recurrence_is_bitwise_the_stepwise_one(moto, case, monkeypatch):
+    # The persistent cooperative launch that runs the whole Chebyshev recurrence with neighbour-flag synchronisation
+    # must give exactly the bits of the one-launch-per-step path (same arithmetic, different scheduling).
+    w = TMA_CASES[case]()
+    out = []
+    for single in (False, True):
+        if single:
+            monkeypatch.setenv("MOTO_NO_MULTISTEP", "1")
+        else:
+            monkeypatch.delenv("MOTO_NO_MULTISTEP", raising=False)
+        ctx = moto.spin_context(w)
+        ctx.set_solver(hvp_path=2, precond_degree=24)
+        lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-8, max_iter=400, allow_notconv=True)
+        out.append((lam.cpu().numpy(), V.cpu().numpy(), info["iters"], info["hvp_count"]))
+    assert out[0][2] == out[1][2] and out[0][3] == out[1][3]
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
