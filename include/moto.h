@@ -144,6 +144,16 @@ moto_status moto_rayleigh_ritz(moto_ctx* ctx, const double* d_GA, const double* 
 moto_status moto_hvp_three_term(moto_ctx* ctx, const double* d_spins, const double* d_V, int k, double alpha, double c0,
                                 double beta, const double* d_U, double* d_out, int refresh_c);
 
+/* The operator the transformed solver runs LOBPCG on, exported so it can be tested and timed alone:
+ *   d_out = -p_d(Hess) V ,  p_d = Chebyshev polynomial of degree d scaled so that p_d(a_L) = 1, |p_d| <= 1 on [a, b]
+ * (Zhou-Saad three-term form: sigma_1 = e/(a_L - c0), e = (b-a)/2, c0 = (b+a)/2;  Y_1 = (sigma_1/e)(A - c0) V,
+ *  Y_{i+1} = (2 sigma_{i+1}/e)(A - c0) Y_i - sigma_i sigma_{i+1} Y_{i-1}, sigma_{i+1} = 1/(2/sigma_1 - sigma_i)).
+ * kind 0 only, k <= 2, 1 <= d <= 256, V tangent (solver mode), a_L < a < b.  On lattices that take the TMA K1 path
+ * the whole recurrence is ONE persistent cooperative launch; otherwise d launches.  d_out must not alias d_V.
+ * refresh_c as in moto_hvp_three_term. */
+moto_status moto_cheb_apply(moto_ctx* ctx, const double* d_spins, const double* d_V, int k, int d, double a, double b,
+                            double a_L, double* d_out, int refresh_c);
+
 /* Host-buffer variants (end-to-end path): same semantics, all array arguments are HOST pointers
  * (pinned or pageable); the library stages them through its workspace (host->device, compute,
  * device->host) and synchronises the stream before returning. */

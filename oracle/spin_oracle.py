@@ -249,3 +249,28 @@ def mmf_force(model: SpinModel, m: np.ndarray, v: np.ndarray) -> np.ndarray:
 def mmf_step(model: SpinModel, m: np.ndarray, v: np.ndarray, dt: float) -> np.ndarray:
     x = m + dt * mmf_force(model, m, v)
     return x / np.linalg.norm(x, axis=1, keepdims=True)
+
+
+# ---- O11 the spectral transformation the GPU solver runs LOBPCG on (a solver device, not in the paper: DESIGN.md 5):
+#      -p_d(H_t), p_d(x) = T_d(l(x)) / T_d(l(a_L)),  l(x) = (2x - a - b)/(b - a),  T_d the Chebyshev polynomial.
+#      Written here as the DEFINITION through the dense eigen-decomposition (no three-term recurrence).
+def chebyshev_T(d: int, x: np.ndarray) -> np.ndarray:
+    x = np.asarray(x, dtype=np.float64)
+    out = np.empty_like(x)
+    inside = np.abs(x) <= 1.0
+    out[inside] = np.cos(d * np.arccos(x[inside]))
+    xo = x[~inside]
+    out[~inside] = np.sign(xo) ** d * np.cosh(d * np.arccosh(np.abs(xo)))
+    return out
+
+
+def transformed_operator_apply(model: SpinModel, m: np.ndarray, V: np.ndarray, d: int, a: float, b: float, a_L: float):
+    """-p_d(Hess) V for tangent-projected V ([k][N][3]), via eigh of the explicit tangent Hessian."""
+    Ht, Bm = tangent_hessian(model, m, dense=True)
+    lam, Y = scipy.linalg.eigh(0.5 * (Ht + Ht.T))
+    ell = lambda x: (2.0 * x - a - b) / (b - a)
+    pl = chebyshev_T(d, ell(lam)) / chebyshev_T(d, np.array([ell(a_L)]))[0]
+    k = V.shape[0]
+    coeff = Y.T @ (Bm.T @ V.reshape(k, -1).T)            # 2N x k
+    out = -(Bm @ (Y @ (pl[:, None] * coeff)))
+    return np.ascontiguousarray(out.T).reshape(k, model.N, 3)

@@ -64,6 +64,7 @@ _SIGS = {
     "moto_mmf_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p, C.c_void_p]),
     "moto_hvp_three_term": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p,
                                       C.c_void_p, C.c_int]),
+    "moto_cheb_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_int]),
     "moto_transport": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "moto_gram": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
     "moto_rayleigh_ritz": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
@@ -205,6 +206,16 @@ class Context:
         out = out if out is not None else self._empty(k, self.N, 3)
         self._check(self.lib.moto_hvp_three_term(self._h, _ptr(spins), _ptr(V), k, float(alpha), float(c0), float(beta), _ptr(U),
                                                  _ptr(out), int(bool(refresh_c))))
+        return out
+
+    def cheb_apply(self, spins, V, d, a, b, a_L, out=None, refresh_c=True):
+        """moto_cheb_apply: out = -p_d(Hess) V (the transformed operator of the solver), tangent V, k <= 2."""
+        _dev_f64(spins, (self.N, 3))
+        k = V.shape[0]
+        _dev_f64(V, (k, self.N, 3))
+        out = out if out is not None else self._empty(k, self.N, 3)
+        self._check(self.lib.moto_cheb_apply(self._h, _ptr(spins), _ptr(V), k, int(d), float(a), float(b), float(a_L), _ptr(out),
+                                             int(bool(refresh_c))))
         return out
 
     def lowest_modes(self, spins, k, tol, max_iter=200, V0=None, allow_notconv=False):

@@ -243,6 +243,33 @@ moto_status moto_hvp_three_term(moto_ctx* c, const double* d_spins, const double
     return MOTO_OK;
 }
 
+moto_status moto_cheb_apply(moto_ctx* c, const double* d_spins, const double* d_V, int k, int d, double a, double b, double a_L,
+                            double* d_out, int refresh_c) {
+    if (!c) return MOTO_EINVAL;
+    if (c->kind != MOTO_KIND_TRI2D) return moto_fail(c, MOTO_ESTATE, "moto_cheb_apply: spin lattices only");
+    if (!d_spins || !d_V || !d_out || d_V == d_out) return moto_fail(c, MOTO_EINVAL, "moto_cheb_apply: null or aliased argument");
+    if (k < 1 || k > 2 || k > c->kmax || d < 1 || d > MOTO_CHEB_MAX || !(a_L < a) || !(a < b))
+        return moto_fail(c, MOTO_EINVAL, "moto_cheb_apply: need 1 <= k <= min(2, kmax), 1 <= d <= 256, a_L < a < b");
+    int n = refresh_c ? spin_curvature(c, d_spins, c->c) : 0;
+    MOTO_CUDA_CHECK(c, cudaMemsetAsync(&c->st->done, 0, 4 * sizeof(int), c->stream));
+    n += fast_cheb_coef_explicit(c, d, a, b, a_L);
+    int nk = d >= 2 ? spin_cheb_multistep(c, d_spins, c->c, d_V, k, d, d_out, &c->st->cheb[0][0], nullptr) : 0;
+    if (nk > 0) n += nk;
+    else {
+        const double* in = d_V; const double* prev = nullptr;
+        for (int i = 1; i <= d; ++i) {
+            double* out = (i == d) ? d_out : ((i & 1) ? c->T1 : c->T2);
+            int m = spin_hvp_tma_ex(c, d_spins, c->c, in, k, out, nullptr, nullptr, 1, 0.0, 0.0, 0.0, prev, &c->st->cheb[i - 1][0]);
+            if (m <= 0) return moto_fail(c, MOTO_ESTATE, "moto_cheb_apply: needs the TMA K1 path (even Lx >= 8; hvp_path != 1)");
+            n += m;
+            prev = in; in = out;
+        }
+    }
+    c->launches += n;
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return MOTO_OK;
+}
+
 moto_status moto_gram(moto_ctx* c, const double* d_S, int ns, const double* d_T, int nt, double* d_G) {
     if (!c) return MOTO_EINVAL;
     if (!d_S || !d_T || !d_G || ns < 1 || nt < 1 || ns > MOTO_NS || nt > 2 * MOTO_NS) return moto_fail(c, MOTO_EINVAL, "moto_gram: bad argument");

@@ -135,6 +135,8 @@ int rr_solve_lobpcg(moto_ctx*, int kb, int nblk);
 bool cart_geometry_ok(const moto_lattice* lat, double rc);
 int block_apply_coeffs(moto_ctx*, double* V, int k, const double* d_C, double* scratch);
 int block_sign_normalise(moto_ctx*, double* V, int k);
+// lobpcg_fast.cu
+int fast_cheb_coef_explicit(moto_ctx* c, int d, double a, double b, double aL);
 // rayleigh_ritz.cu
 int rr_solve(moto_ctx*, const double* d_GA, const double* d_GB, int n, int nev, double* d_theta, double* d_C,
              int mode, SolverState* st_or_null);

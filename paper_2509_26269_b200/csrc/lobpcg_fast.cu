@@ -199,18 +199,19 @@ __global__ void k_negc_max(long long N, const double* __restrict__ c, double* __
     }
 }
 
+// explicit == 1: interval given (a = margin, b = hi_user, a_L = lnorm): the moto_cheb_apply building block
 __global__ void k_cheb_coef(SolverState* st, int k, int d, double margin, double lnorm, double hi_user,
-                            const double* __restrict__ partial_max, int nmax) {
+                            const double* __restrict__ partial_max, int nmax, int explicit_ab) {
     if (st->done || threadIdx.x != 0) return;
     double b = hi_user;
-    if (!(b > 0.0)) {
+    if (!explicit_ab && !(b > 0.0)) {
         double mx = -1e300;
         for (int i = 0; i < nmax; ++i) mx = fmax(mx, partial_max[i]);
         b = mx + lnorm;
     }
-    const double aL = st->theta[0];
-    double a = st->theta[k - 1] + margin;
-    if (a > 0.5 * (aL + b)) a = 0.5 * (aL + b);   // crude early Ritz values: keep the interval sane
+    const double aL = explicit_ab ? lnorm : st->theta[0];
+    double a = explicit_ab ? margin : st->theta[k - 1] + margin;
+    if (!explicit_ab && a > 0.5 * (aL + b)) a = 0.5 * (aL + b);   // crude early Ritz values: keep the interval sane
     const double e = 0.5 * (b - a), c0 = 0.5 * (b + a), sig1 = e / (aL - c0);
     double sig = sig1;
     st->cheb_ab[0] = a; st->cheb_ab[1] = b; st->cheb_ab[2] = aL; st->cheb_ab[3] = (double)d;
@@ -327,7 +328,12 @@ int fast_negc_max(moto_ctx* c, double* partial_max, int* nmax_out) {
 }
 
 int fast_cheb_coef(moto_ctx* c, int k, int d, double margin, double lnorm, double hi_user, const double* partial_max, int nmax) {
-    k_cheb_coef<<<1, 32, 0, c->stream>>>(c->st, k, d, margin, lnorm, hi_user, partial_max, nmax);
+    k_cheb_coef<<<1, 32, 0, c->stream>>>(c->st, k, d, margin, lnorm, hi_user, partial_max, nmax, 0);
+    return 1;
+}
+
+int fast_cheb_coef_explicit(moto_ctx* c, int d, double a, double b, double aL) {
+    k_cheb_coef<<<1, 32, 0, c->stream>>>(c->st, 1, d, a, aL, b, nullptr, 0, 1);
     return 1;
 }
 

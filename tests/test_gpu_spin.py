@@ -399,3 +399,42 @@ def test_multistep_recurrence_is_bitwise_the_stepwise_one(moto, case, monkeypatc
         out.append((lam.cpu().numpy(), V.cpu().numpy(), info["iters"], info["hvp_count"]))
     assert out[0][2] == out[1][2] and out[0][3] == out[1][3]
     assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+
+
+@pytest.mark.parametrize("path", [1, 2])
+def test_lowest_mode_k1_and_zero_iterations(moto, path):
+    # block size 1 (the paper's default single minimum mode) on both K1 paths; max_iter = 0 returns the
+    # Rayleigh-Ritz of the start block with ENOTCONV and finite outputs
+    w = wl.config1(L=40)
+    lam_ref, V_ref = so.lowest_modes(model_of(w), w.spins, 1, extra=1)
+    ctx = moto.spin_context(w)
+    ctx.set_solver(hvp_path=path)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 1, tol=1e-9, max_iter=4000)
+    assert info["converged"], info
+    assert abs(lam.item() - lam_ref[0]) <= EIG_TOL * abs(lam_ref[0])
+    ang = scipy.linalg.subspace_angles(V.cpu().numpy().reshape(1, -1).T, V_ref[:1].reshape(1, -1).T)
+    assert ang.max() <= ANGLE_TOL
+    lam0, V0, info0 = ctx.lowest_modes(dev(w.spins), 1, tol=1e-9, max_iter=0, allow_notconv=True)
+    assert not info0["converged"] and info0["iters"] == 0 and np.isfinite(lam0.cpu().numpy()).all()
+
+
+CHEB_CASES = [lambda: wl.config0(), lambda: custom(24, 16, 1, 0, 21), lambda: custom(62, 10, 0, 1, 22), lambda: custom(130, 6, 1, 1, 23)]
+
+
+@pytest.mark.parametrize("case", range(len(CHEB_CASES)))
+@pytest.mark.parametrize("d", [1, 2, 3, 8, 40])
+def test_cheb_apply_parity(moto, case, d):
+    # the transformed operator -p_d(Hess) of the solver (one persistent multi-step launch for d >= 2) against its
+    # definition through the oracle's dense eigen-decomposition (lattices small enough for a full dense eigh)
+    w = CHEB_CASES[case]()
+    model = model_of(w)
+    ctx = moto.spin_context(w, kmax=2)
+    ctx.set_solver(hvp_path=2)
+    lam_ref, _ = so.lowest_modes(model, w.spins, 2)
+    a, b, aL = lam_ref[1] + 0.05, lam_ref[1] + 25.0, lam_ref[0]
+    for k in (1, 2):
+        V = wl.random_block(w.N, k, seed=500 + case)
+        V = V - np.sum(V * w.spins[None], axis=2, keepdims=True) * w.spins[None]
+        out = ctx.cheb_apply(dev(w.spins), dev(V), d, a, b, aL).cpu().numpy()
+        ref = so.transformed_operator_apply(model, w.spins, V, d, a, b, aL)
+        assert rel_l2(out, ref) <= 1e-10, rel_l2(out, ref)

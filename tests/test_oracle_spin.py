@@ -263,3 +263,25 @@ def test_mmf_force_vanishes_only_at_stationary_point():
     m = np.zeros((16, 3)); m[:, 2] = 1
     v = np.zeros((1, 16, 3)); v[0, :, 0] = 0.25
     assert np.max(np.abs(so.mmf_step(model, m, v, 0.1) - m)) < 1e-15
+
+
+def test_transformed_operator_definition_pins():
+    # Chebyshev T_d against numpy's own evaluation and closed forms; -p_1(H) = -(H - c0)/(a_L - c0) exactly
+    x = np.linspace(-2.5, 2.5, 41)
+    for d in (1, 2, 3, 7):
+        ref = np.polynomial.chebyshev.chebval(x, [0] * d + [1])
+        assert np.max(np.abs(so.chebyshev_T(d, x) - ref) / np.maximum(1, np.abs(ref))) < 1e-12
+    assert np.allclose(so.chebyshev_T(2, x), 2 * x * x - 1)
+    w = wl.config0()
+    model = so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
+    V = wl.random_block(w.N, 2, seed=3)
+    a, b, aL = 0.3, 19.0, 0.1
+    HV = so.hvp(model, w.spins, V)
+    PV = V - np.sum(V * w.spins[None], axis=2, keepdims=True) * w.spins[None]
+    c0 = 0.5 * (a + b)
+    ref1 = -(HV - c0 * PV) / (aL - c0)
+    assert np.max(np.abs(so.transformed_operator_apply(model, w.spins, V, 1, a, b, aL) - ref1)) < 1e-12
+    # p_d(a_L) = 1: an eigenvector with eigenvalue a_L is mapped to minus itself
+    lam, Vm = so.lowest_modes(model, w.spins, 1)
+    out = so.transformed_operator_apply(model, w.spins, Vm, 5, lam[0] + 0.2, 19.0, lam[0])
+    assert np.max(np.abs(out + Vm)) < 1e-10
