@@ -201,6 +201,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         unsigned n = 0;
         for (int step = 1; step <= nsteps; ++step) {
         const VSet& vs = maps.vset[step == 1 ? 0 : (((step - 1) & 1) ? 1 : 2)];   // Y_{step-1}: the input, T1 (odd) or T2 (even)
+        const bool rev = nsteps > 1 && !(step & 1);   // even steps sweep every segment bottom-up (see the consumers)
         if (step > 1) {   // wait until every halo partner has published step - 1 (bounded spin: a lost partner must not hang the GPU)
             const int nd = sdep[0];
             const unsigned long long want = p.epoch + (unsigned long long)(step - 1);
@@ -232,7 +233,10 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                 const unsigned s = n % S, ph = (n / S) & 1u;
                 const int r0 = j * RC - 1;
                 const int nvalid = (nrows + 1 - r0) < RC ? (nrows + 1 - r0) : RC;
-                const int y0 = y_start + r0;
+                // forward: row index r lives at y = y_start + r; reversed: at y = y_end - 1 - r, and a chunk box (ascending y)
+                // then holds descending r, so row i of the stage sits in slot RC - 1 - i
+                const int y_end = y_start + nrows;
+                const int y0 = rev ? y_end - r0 - RC : y_start + r0;          // first (lowest-y) row of the full chunk box
                 const bool chunk_ok = (nvalid == RC) && (!l.py || (y0 >= 0 && y0 + RC <= Ly));
                 if (lane == 0) {
                     mbar_wait(&empty[s], ph ^ 1u);
@@ -242,9 +246,9 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                 const int nops = (chunk_ok ? 1 : nvalid) * KINDS;
                 for (int t = lane; t < nops; t += 32) {
                     const int i = t / KINDS, kind = t - i * KINDS;     // i: row inside the stage (0 on the chunk path)
-                    int y = y0 + i;
+                    int y = chunk_ok ? y0 : (rev ? y_end - 1 - (r0 + i) : y_start + r0 + i);
                     if (!chunk_ok && l.py) { if (y < 0) y += Ly; else if (y >= Ly) y -= Ly; }
-                    const int slot = s * RC + i;
+                    const int slot = s * RC + (chunk_ok ? 0 : (rev ? RC - 1 - i : i));
                     if (kind < F) {
                         const int f = kind;
                         const CUtensorMap* mp = f == 0 ? (chunk_ok ? &maps.m_chunk : &maps.m_row) : (chunk_ok ? &vs.chunk : &vs.row);
@@ -288,19 +292,30 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         Ustep = step == 1 ? nullptr : (step == 2 ? p.V0 : ((step & 1) ? p.T1 : p.T2));     // Y_{step-2}
         outp = step == nsteps ? p.out : ((step & 1) ? p.T1 : p.T2);                          // Y_step (in place over Y_{step-2})
     }
+    // Even steps of a multi-step launch sweep bottom-up: the rows a CTA wrote (and read) last in step i are the first it
+    // touches in step i + 1, so a good part of the 176 MB/step footprint is still in the 126 MB L2.  A reversed sweep is
+    // the same code on the point-reflected lattice: row order reversed, left and right neighbours swapped, D -> -D
+    // (the stencil is inversion symmetric up to the sign of the DMI vectors, D_{-delta} = -D_delta).
+    const bool rev = nsteps > 1 && !(step & 1);
+    Lat ls = p.l;
+    if (rev) ls.D = -ls.D;
     long long pos = lo;
     while (pos < hi) {
         const int sx = (int)(pos / Ly), y_start = (int)(pos - (long long)sx * Ly);
         const int nrows = (int)((hi - pos) < (long long)(Ly - y_start) ? (hi - pos) : (Ly - y_start));
+        const int y_end = y_start + nrows;
         const int xb = strip_x(sx, Lx, p.nsx), xe = (sx + 1 == p.nsx) ? Lx : strip_x(sx + 1, Lx, p.nsx);
         const int w = xe - xb;
         const bool active = col < w;
-        const bool useL = l.px && xb == 0 && col == 0;        // left neighbour comes from the wrap side box
-        const bool useR = l.px && xe == Lx && col == w - 1;   // right neighbour comes from the wrap side box
-        // per-thread column bases (in doubles) and row pitches of the three columns x-1, x, x+1
-        const double* baseL = useL ? sL + 13 : smain + 3 * (col + 1);
+        const bool wrapL = l.px && xb == 0 && col == 0;        // x - 1 comes from the wrap side box
+        const bool wrapR = l.px && xe == Lx && col == w - 1;   // x + 1 comes from the wrap side box
+        // per-thread column bases (in doubles) and row pitches of the three columns; "L" is x - 1 on a forward sweep, x + 1 reversed
+        const double* colM = wrapL ? sL + 13 : smain + 3 * (col + 1);   // x - 1
         const double* baseC = smain + 3 * (col + 2);
-        const double* baseR = useR ? sR : smain + 3 * (col + 3);
+        const double* colP = wrapR ? sR : smain + 3 * (col + 3);         // x + 1
+        const bool useL = rev ? wrapR : wrapL, useR = rev ? wrapL : wrapR;
+        const double* baseL = rev ? colP : colM;
+        const double* baseR = rev ? colM : colP;
         const int pitchL = useL ? SIDED : ROWD, pitchR = useR ? SIDED : ROWD;
         const int fstrL = useL ? NSLOT * SIDED : NSLOT * ROWD, fstrR = useR ? NSLOT * SIDED : NSLOT * ROWD;
         const int x = xb + col;
@@ -319,11 +334,12 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         auto load_u = [&](int jb, d3 (&ua)[K], d3 (&ub)[K]) {
             const int r = jb * RC + 2 * rp;
             if (use_u && active && r < nrows) {
-                const long long sA = (long long)(y_start + r) * Lx + x;
+                const long long sA = (long long)(rev ? y_end - 1 - r : y_start + r) * Lx + x;
+                const long long dB = rev ? -(long long)Lx : (long long)Lx;
 #pragma unroll
                 for (int a = 0; a < K; ++a) {
                     ua[a] = ld3(Ustep + (size_t)a * 3 * N, sA);
-                    ub[a] = (r + 1 < nrows) ? ld3(Ustep + (size_t)a * 3 * N, sA + Lx) : mk3(0.0, 0.0, 0.0);
+                    ub[a] = (r + 1 < nrows) ? ld3(Ustep + (size_t)a * 3 * N, sA + dB) : mk3(0.0, 0.0, 0.0);
                 }
             }
         };
@@ -338,9 +354,9 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     const int rr = rA + q;   // = (row index r) + 1, r = rA - 1 + q
-                    slot[q] = (int)((n + rr / RC) % S) * RC + (rr % RC);
+                    slot[q] = (int)((n + rr / RC) % S) * RC + (rev ? RC - 1 - rr % RC : rr % RC);
                 }
-                const long long siteA = (long long)(y_start + rA) * Lx + x, siteB = siteA + Lx;
+                const long long siteA = (long long)(rev ? y_end - 1 - rA : y_start + rA) * Lx + x, siteB = rev ? siteA - Lx : siteA + Lx;
                 double cA = 0.0, cB = 0.0;
                 if (!API) { cA = sc[slot[1] * CROWD + col + 2]; cB = sc[slot[2] * CROWD + col + 2]; }
                 // field 0: m.  API: all ten sites (projection of the neighbours + stencil for c); SOLVER: centres only.
@@ -352,8 +368,8 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                     m1L = lds3(baseL + slot[1] * pitchL); m1R = lds3(baseR + slot[1] * pitchR);
                     m2L = lds3(baseL + slot[2] * pitchL); m2R = lds3(baseR + slot[2] * pitchR);
                     m3L = lds3(baseL + slot[3] * pitchL); m3C = lds3(baseC + slot[3] * ROWD);
-                    const d3 LmA = stencil_apply(l, m1R, m1L, m2C, m0C, m2L, m0R, m1C.z);
-                    const d3 LmB = stencil_apply(l, m2R, m2L, m3C, m1C, m3L, m1R, m2C.z);
+                    const d3 LmA = stencil_apply(ls, m1R, m1L, m2C, m0C, m2L, m0R, m1C.z);
+                    const d3 LmB = stencil_apply(ls, m2R, m2L, m3C, m1C, m3L, m1R, m2C.z);
                     cA = dot3(m1C, LmA) - dot3(m1C, muB);
                     cB = dot3(m2C, LmB) - dot3(m2C, muB);
                 }
@@ -374,8 +390,8 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                         u2L = proj3(m2L, u2L); u2C = proj3(m2C, u2C); u2R = proj3(m2R, u2R);
                         u3L = proj3(m3L, u3L); u3C = proj3(m3C, u3C);
                     }
-                    const d3 LA = stencil_apply(l, u1R, u1L, u2C, u0C, u2L, u0R, u1C.z);
-                    const d3 LB = stencil_apply(l, u2R, u2L, u3C, u1C, u3L, u1R, u2C.z);
+                    const d3 LA = stencil_apply(ls, u1R, u1L, u2C, u0C, u2L, u0R, u1C.z);
+                    const d3 LB = stencil_apply(ls, u2R, u2L, u3C, u1C, u3L, u1R, u2C.z);
                     vA[a] = u1C; vB[a] = u2C;
                     hA[a] = axpy3(-cA, u1C, proj3(m1C, LA));
                     hB[a] = axpy3(-cB, u2C, proj3(m2C, LB));
