@@ -170,6 +170,10 @@ def run_report(args):
 
     rows, orows = [], []
     cfgs = [("0", wl.config0(), 0), ("1", wl.config1(), 0), ("2", wl.config2(), 100), ("3", wl.config3(), 200), ("4", wl.config4(), 100)]
+    # the paper's own Fig. 2 workload class: a random spin configuration at 10^6 spins, same J, D, K, B
+    rnd = wl.random_spins(1000, 1000, 7)
+    cfgs.append(("R (random spins, PAPER.md:84)", wl.SpinWorkload("rand1000", 1000, 1000, 1, 1, 1.0, 0.3, 0.05, (0.0, 0.0, 0.02), 1.0, 2, 7, rnd,
+                                                                    tol=1e-6), 0))
     for name, w, nsteps in cfgs:
         cart = hasattr(w, "positions")
         ctx = moto.cart_context(w, kmax=w.k) if cart else moto.spin_context(w, kmax=w.k)
@@ -225,8 +229,10 @@ def run_report(args):
                 elif N <= 70000:
                     t0 = time.perf_counter(); lr, _ = so.lowest_modes_sparse(mdl, w.spins, w.k, extra=2); t_s = time.perf_counter() - t0
                     how = "ARPACK shift-invert (sparse LU)"
-                else:
+                elif name == "3":
                     lr, t_s, how = None, float("nan"), "ARPACK shift-invert: ~70 min on 8 cores (tests/golden/make_cfg3_eigs.py), not re-run here"
+                else:
+                    lr, t_s, how = None, float("nan"), "not run (2e6 unknowns; the GPU pair is checked by its oracle-side residual in the tests for cfg 3)"
             err = "" if lr is None else f"{np.max(np.abs(lam.cpu().numpy() - lr[:w.k]) / np.maximum(np.abs(lr[:w.k]), 1e-3)):.1e}"
             orows.append(f"| {name} | {t_h * 1e3:.0f} | {t_s:.2f} | {how} | {err} |")
         ctx.close()
