@@ -124,7 +124,8 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.01;
     // cold start: 20 plain iterations first so that theta_k (hence a) means something; a warm start already has it
     int phase_len = 20, plain_start = warm_start ? 0 : 20;
-    const int acheck_every = 4;
+    int acheck_every = 4;
+    if (const char* e = getenv("MOTO_ACHECK_EVERY")) acheck_every = atoi(e) > 0 ? atoi(e) : 4;
     if (const char* e = getenv("MOTO_PHASE_LEN")) phase_len = atoi(e);      // tuning hooks (not part of the ABI)
     if (const char* e = getenv("MOTO_PLAIN_START")) plain_start = atoi(e);
     const double lnorm = c->lmax_L;   // b = max_i(-c_i) + lambda_max(L) >= lambda_max(Hess)
@@ -187,6 +188,101 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     return finish(c, k, kb, enq, last, info);
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Block sizes kb > 2 on spin lattices that take the TMA K1 path: the generic block algebra (k_gram, k_update,
+// k_residual) run on the same Chebyshev-transformed operator -p_d(A) as the fused path, two columns per persistent
+// multi-step K1 launch.  Same phase structure: A-Ritz pairs + A-residual test + new interval at every boundary.
+static int gen_apply(moto_ctx* c, const double* d_state, const double* V, int kb, double* OV, int degree) {
+    if (degree == 0) return apply_operator(c, d_state, V, kb, OV);
+    const size_t bs = (size_t)3 * c->N;
+    int n = 0;
+    for (int a0 = 0; a0 < kb; a0 += 2) {
+        const int kk = kb - a0 >= 2 ? 2 : 1;
+        int nk = degree >= 2 ? spin_cheb_multistep(c, d_state, c->c, V + a0 * bs, kk, degree, OV + a0 * bs, &c->st->cheb[0][0], &c->st->done) : 0;
+        if (nk > 0) { n += nk; continue; }
+        const double* in = V + a0 * bs; const double* prev = nullptr;
+        for (int i = 1; i <= degree; ++i) {
+            double* out = (i == degree) ? OV + a0 * bs : ((i & 1) ? c->T1 : c->T2);
+            n += spin_hvp_tma_ex(c, d_state, c->c, in, kk, out, &c->st->done, nullptr, 1, 0.0, 0.0, 0.0, prev, &c->st->cheb[i - 1][0]);
+            prev = in; in = out;
+        }
+    }
+    return n;
+}
+
+static int gen_phase_start(moto_ctx* c, const double* d_state, int kb, int k, double tol, int degree, int nblk) {
+    const size_t bs = (size_t)3 * c->N;
+    int n = gen_apply(c, d_state, c->X, kb, c->AX, degree);
+    n += block_zero(c, c->W, (long long)kb * bs);
+    n += block_zero(c, c->AW, (long long)kb * bs);
+    n += block_zero(c, c->P, (long long)kb * bs);
+    n += block_zero(c, c->AP, (long long)kb * bs);
+    n += block_gram_lobpcg(c, kb);
+    n += rr_solve_lobpcg(c, kb, nblk);
+    n += block_update(c, kb);
+    n += block_residual(c, d_state, kb, k, degree ? -1.0 : tol);   // transformed residuals never decide convergence
+    return n;
+}
+
+static moto_status lobpcg_solve_generic_filtered(moto_ctx* c, const double* d_state, int k, int kb, double tol, int max_iter,
+                                                 int warm_start, int degree, moto_solve_info* info) {
+    const size_t bs = (size_t)3 * c->N;
+    const int check_every = c->opts.check_every > 0 ? c->opts.check_every : 8;
+    const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.01;
+    const int phase_len = 20, plain_start = warm_start ? 0 : 20;
+    double* pmax = c->g;   // [<= 296] block maxima of -c_i (the gradient scratch is free during a solve; the Gram partials fill c->partials)
+    int n = 0, nmax = 0;
+    n += spin_curvature(c, d_state, c->c);
+    MOTO_CUDA_CHECK(c, cudaMemsetAsync(c->st, 0, sizeof(SolverState), c->stream));
+    n += fast_negc_max(c, pmax, &nmax);
+    if (!warm_start) n += block_random(c, c->X, kb, c->opts.seed);
+    else if (kb > k) n += block_random(c, c->X + (size_t)k * bs, kb - k, c->opts.seed ^ 0x5bd1e995u);
+    n += project_block(c, d_state, c->X, kb);
+    const int nblk = gram_blocks(c);
+    n += gen_phase_start(c, d_state, kb, k, tol, 0, nblk);
+
+    int enq = 0, slot = 0, pending = 0, in_phase = 0, cur_degree = 0;
+    long long hv = kb;
+    bool finished = false;
+    HostStatus last; memset(&last, 0, sizeof(last));
+    while (!finished) {
+        int batch = max_iter - enq < check_every ? max_iter - enq : check_every;
+        for (int b = 0; b < batch; ++b) {
+            if ((cur_degree == 0 && enq + b >= plain_start) || (cur_degree > 0 && in_phase >= phase_len)) {
+                if (cur_degree > 0) { n += gen_phase_start(c, d_state, kb, k, tol, 0, nblk); hv += kb; }   // A-Ritz pairs, A-residual test
+                n += fast_cheb_coef(c, k, degree, margin, c->lmax_L, c->opts.precond_hi, pmax, nmax);
+                n += gen_phase_start(c, d_state, kb, k, tol, degree, nblk);
+                hv += (long long)kb * degree;
+                cur_degree = degree; in_phase = 0;
+            }
+            n += gen_apply(c, d_state, c->W, kb, c->AW, cur_degree);
+            n += block_gram_lobpcg(c, kb);
+            n += rr_solve_lobpcg(c, kb, nblk);
+            n += block_update(c, kb);
+            n += block_residual(c, d_state, kb, k, cur_degree ? -1.0 : tol);
+            hv += (long long)kb * (cur_degree ? cur_degree : 1);
+            ++in_phase;
+        }
+        enq += batch;
+        if (enq >= max_iter && cur_degree > 0) { n += gen_phase_start(c, d_state, kb, k, tol, 0, nblk); hv += kb; }
+        MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&c->hstat[slot], &c->st->theta, sizeof(HostStatus), cudaMemcpyDeviceToHost, c->stream));
+        MOTO_CUDA_CHECK(c, cudaEventRecord(c->ev[slot], c->stream));
+        if (pending) {
+            MOTO_CUDA_CHECK(c, cudaEventSynchronize(c->ev[slot ^ 1]));
+            last = c->hstat[slot ^ 1];
+            if (last.done) finished = true;
+        }
+        pending = 1;
+        slot ^= 1;
+        if (enq >= max_iter) finished = true;
+    }
+    MOTO_CUDA_CHECK(c, cudaEventSynchronize(c->ev[slot ^ 1]));
+    last = c->hstat[slot ^ 1];
+    c->launches += n;
+    last.nhvp = hv;   // enqueued applications (an upper bound when the device stopped early inside the last batch)
+    return finish(c, k, kb, enq, last, info);
+}
+
 moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, int max_iter, int warm_start,
                          moto_solve_info* info) {
     int kb = k + (c->opts.guard > 0 ? c->opts.guard : 0);
@@ -195,6 +291,13 @@ moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, 
     if (3ll * kb > dof) kb = (int)(dof / 3 > 0 ? dof / 3 : 1);
     if (kb < k) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes: k too large for this system (need 3k <= dof)");
     if (kb <= 2 && max_iter > 0) return lobpcg_solve_fast(c, d_state, k, kb, tol, max_iter, warm_start, info);
+    // kb > 2: the transformation is opt-in (precond_degree > 0): at the sizes where such blocks are used here (cfg 2,
+    // 65 536 sites) the recurrence steps are launch-latency bound and plain LOBPCG is as fast
+    if (max_iter > 0 && c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && c->opts.precond_degree > 0) {
+        int degree = c->opts.precond_degree;
+        if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
+        return lobpcg_solve_generic_filtered(c, d_state, k, kb, tol, max_iter, warm_start, degree, info);
+    }
     const size_t bs = (size_t)3 * c->N;
     const int check_every = c->opts.check_every > 0 ? c->opts.check_every : 8;
     const double* m_proj = (c->kind == MOTO_KIND_TRI2D) ? d_state : nullptr;

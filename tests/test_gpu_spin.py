@@ -443,3 +443,14 @@ def test_cheb_apply_parity(moto, case, d):
         out = ctx.cheb_apply(dev(w.spins), dev(V), d, a, b, aL).cpu().numpy()
         ref = so.transformed_operator_apply(model, w.spins, V, d, a, b, aL)
         assert rel_l2(out, ref) <= 1e-10, rel_l2(out, ref)
+
+
+def test_transformed_generic_path_kb_gt_2(moto):
+    # block sizes above 2 (guard columns) on the transformed operator: opt-in through precond_degree > 0
+    w = wl.config1(L=40)
+    lam_ref, V_ref = so.lowest_modes(model_of(w), w.spins, 3, extra=1)
+    ctx = moto.spin_context(w, kmax=5)
+    ctx.set_solver(guard=2, hvp_path=2, precond_degree=16)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 3, tol=1e-9, max_iter=2000)
+    assert info["converged"], info
+    _check_modes(w, lam, V, lam_ref, V_ref, 3)
