@@ -454,3 +454,29 @@ def test_transformed_generic_path_kb_gt_2(moto):
     lam, V, info = ctx.lowest_modes(dev(w.spins), 3, tol=1e-9, max_iter=2000)
     assert info["converged"], info
     _check_modes(w, lam, V, lam_ref, V_ref, 3)
+
+
+def test_building_block_argument_errors_and_fallbacks(moto):
+    import torch
+    w = custom(37, 23, 0, 0, 1)              # odd Lx: the TMA path does not apply
+    ctx = moto.spin_context(w, kmax=3)
+    x = dev(w.spins)
+    V = wl.random_block(w.N, 3, seed=5)
+    V = V - np.sum(V * w.spins[None], axis=2, keepdims=True) * w.spins[None]
+    # three-term step falls back to the generic kernel and still matches the oracle
+    out = ctx.hvp_three_term(x, dev(V), 0.5, 3.0, -0.25, U=dev(V)).cpu().numpy()
+    HV = so.hvp(model_of(w), w.spins, V)
+    assert rel_l2(out, 0.5 * (HV - 3.0 * V) - 0.25 * V) <= HVP_TOL
+    # the transformed operator needs the TMA path: a status code, never a silent CPU fallback
+    with pytest.raises(moto.MotoError) as e:
+        ctx.cheb_apply(x, dev(V[:2]), 4, -0.1, 18.0, -0.2)
+    assert e.value.status == moto.ESTATE
+    w2 = wl.config1(L=40)
+    ctx2 = moto.spin_context(w2, kmax=2)
+    V2 = dev(wl.random_block(w2.N, 2, seed=6))
+    for bad in (dict(d=0), dict(d=300), dict(a=-0.3), dict(b=-0.5)):     # degree range, a_L < a < b
+        kw = dict(d=4, a=-0.1, b=18.0, a_L=-0.2); kw.update(bad)
+        with pytest.raises(moto.MotoError):
+            ctx2.cheb_apply(dev(w2.spins), V2, kw["d"], kw["a"], kw["b"], kw["a_L"])
+    with pytest.raises(moto.MotoError):
+        ctx2.cheb_apply(dev(w2.spins), V2, 4, -0.1, 18.0, -0.2, out=V2)   # aliasing
