@@ -517,7 +517,9 @@ bool launch(moto_ctx* c, const Maps& maps, const KParams& p, int grid) {
         attr[0].val.programmaticStreamSerializationAllowed = 1;
     }
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k_hvp_tma<K, API>, maps, p) == cudaSuccess;
+    if (cudaLaunchKernelEx(&cfg, k_hvp_tma<K, API>, maps, p) == cudaSuccess) return true;
+    (void)cudaGetLastError();   // the caller falls back to another path: do not leave the launch error sticky
+    return false;
 }
 
 }  // namespace
