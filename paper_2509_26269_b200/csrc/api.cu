@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of libmoto.so (include/moto.h): argument checks, workspace carving, dispatch.
 #include <math.h>
+#include <stdlib.h>
 #include <new>
 #include "common.cuh"
 
@@ -253,7 +254,8 @@ moto_status moto_cheb_apply(moto_ctx* c, const double* d_spins, const double* d_
     int n = refresh_c ? spin_curvature(c, d_spins, c->c) : 0;
     MOTO_CUDA_CHECK(c, cudaMemsetAsync(&c->st->done, 0, 4 * sizeof(int), c->stream));
     n += fast_cheb_coef_explicit(c, d, a, b, a_L);
-    int nk = d >= 2 ? spin_cheb_multistep(c, d_spins, c->c, d_V, k, d, d_out, &c->st->cheb[0][0], nullptr) : 0;
+    // MOTO_NO_MULTISTEP: test hook, forces one launch per step (the multi-step == step-wise test compares the two)
+    int nk = (d >= 2 && !getenv("MOTO_NO_MULTISTEP")) ? spin_cheb_multistep(c, d_spins, c->c, d_V, k, d, d_out, &c->st->cheb[0][0], nullptr) : 0;
     if (nk > 0) n += nk;
     else {
         const double* in = d_V; const double* prev = nullptr;

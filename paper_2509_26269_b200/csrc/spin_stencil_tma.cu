@@ -3,20 +3,21 @@
 //
 // Design (B200, sm_100a): a persistent grid of one CTA per SM.  The lattice is cut into column strips of
 // <= 60 sites; the (strip, row) space is linearised and split evenly over the CTAs, so every CTA streams
-// one or two vertical strip segments top to bottom.  One producer warp drives the TMA engine (its 32 lanes
-// issue the boxes of a stage in parallel): each
-// 8-row chunk of every field (m, V_1..V_K; 64 sites = 60 + halo columns, 1536 B per row) is
-// one cp.async.bulk.tensor box landing in a ring of shared-memory row slots guarded by full/empty
-// mbarriers; the two halo rows of a segment are 1-row boxes, out-of-range coordinates zero-fill (that IS
-// the open boundary), periodic wrap in y is a wrapped row coordinate and periodic wrap in x is a 128-byte
-// side box per row.  Eight consumer warps (2 column halves x 4 row pairs) compute two rows per thread from
-// shared memory, so each site is read from HBM once for all K directions and from shared memory 5x instead
-// of 7x.  Results go straight to global memory; c_i (solver mode) and the Chebyshev operand are read
-// directly (no reuse).  Tensor cores are not used: this is a 7-point stencil, HBM-bound.
+// one or two vertical strip segments.  One producer warp drives the TMA engine (its 32 lanes issue the boxes of a
+// stage in parallel): each 10-row chunk of every field (m, V_1..V_K; 64 sites = 60 + halo columns, 1536 B per row;
+// in solver mode also c_i) is one cp.async.bulk.tensor box landing in a ring of shared-memory row slots guarded by
+// full/empty mbarriers; the two halo rows of a segment are 1-row boxes, out-of-range coordinates zero-fill (that IS
+// the open boundary), periodic wrap in y is a wrapped row coordinate and periodic wrap in x is a 128-byte side box
+// per row.  Ten consumer warps (2 column halves x 5 row pairs) compute two rows per thread from shared memory, so
+// each site is read from HBM once for all K directions and from shared memory 5x instead of 7x.  Results go straight
+// to global memory; the three-term operand is read directly one block ahead (no reuse).  Tensor cores are not used:
+// this is a 7-point stencil, HBM-bound.
 //
 // Modes:  API    (moto_hvp)      HV = P (L Pv) - c Pv with c = m.(Lm - mu B) recomputed, input projected
-//         SOLVER (LOBPCG inner)  HV = P (L v) - c v, c given, v tangent; optional per-CTA partials of
-//                                V^T HV and optional three-term epilogue out = alpha (HV - c0 v) + beta u
+//         SOLVER (LOBPCG inner)  HV = P (L v) - c v, c given, v tangent; optional per-CTA partials of V^T HV and
+//                                optional three-term epilogue out = alpha (HV - c0 v) + beta u
+//         MULTI-STEP (solver)    the whole Chebyshev recurrence in one cooperative launch: per-step neighbour flags,
+//                                ping-pong blocks, alternating sweep direction (see KParams and DESIGN.md 5)
 #include <cuda.h>
 #include "common.cuh"
 #include "device_utils.cuh"
@@ -61,7 +62,6 @@ struct KParams {
     Lat l;
     int nsx;                 // number of strips
     long long total;         // nsx * Ly strip-rows
-    const double* m;         // for nothing but alignment of the interface (fields come through TMA)
     const double* cvec;      // [N] (SOLVER)
     double* out;             // [K][N][3]
     const double* U;         // [K][N][3] Chebyshev operand or NULL
@@ -565,7 +565,7 @@ int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const doub
         p.l = make_lat(c);
         p.nsx = (Lx + TXMAX - 1) / TXMAX;
         p.total = (long long)p.nsx * Ly;
-        p.m = m; p.cvec = cvec; p.out = HV + a0 * bs;
+        p.cvec = cvec; p.out = HV + a0 * bs;
         p.U = U ? U + a0 * bs : nullptr;
         p.alpha = alpha; p.c0 = c0; p.beta = beta; p.cheb = cheb; p.coef = d_coef;
         p.waw = waw_partials; p.done = d_done;
@@ -618,7 +618,7 @@ int spin_cheb_multistep(moto_ctx* c, const double* m, const double* cvec, const 
     p.l = make_lat(c);
     p.nsx = (Lx + TXMAX - 1) / TXMAX;
     p.total = (long long)p.nsx * Ly;
-    p.m = m; p.cvec = cvec; p.out = OUT; p.U = nullptr;
+    p.cvec = cvec; p.out = OUT; p.U = nullptr;
     p.alpha = p.c0 = p.beta = 0.0; p.cheb = 1; p.coef = d_coef;
     p.waw = nullptr; p.done = d_done;
     p.nsteps = d; p.V0 = V; p.T1 = c->T1; p.T2 = c->T2;
