@@ -480,3 +480,16 @@ def test_building_block_argument_errors_and_fallbacks(moto):
             ctx2.cheb_apply(dev(w2.spins), V2, kw["d"], kw["a"], kw["b"], kw["a_L"])
     with pytest.raises(moto.MotoError):
         ctx2.cheb_apply(dev(w2.spins), V2, 4, -0.1, 18.0, -0.2, out=V2)   # aliasing
+
+
+def test_guard_column_on_the_fused_path(moto):
+    # k = 1 with one guard column: block size 2 on the fused (and, with hvp_path=2, transformed) path; only column 0 is returned
+    w = wl.config1(L=40)
+    lam_ref, V_ref = so.lowest_modes(model_of(w), w.spins, 1, extra=1)
+    ctx = moto.spin_context(w, kmax=2)
+    ctx.set_solver(guard=1, hvp_path=2)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 1, tol=1e-9, max_iter=3000)
+    assert info["converged"], info
+    assert V.shape[0] == 1 and abs(lam.item() - lam_ref[0]) <= EIG_TOL * abs(lam_ref[0])
+    ang = scipy.linalg.subspace_angles(V.cpu().numpy().reshape(1, -1).T, V_ref[:1].reshape(1, -1).T)
+    assert ang.max() <= ANGLE_TOL
