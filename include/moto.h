@@ -124,6 +124,27 @@ moto_status moto_lowest_modes(moto_ctx* ctx, const double* d_spins, int k, doubl
 moto_status moto_mmf_step(moto_ctx* ctx, const double* d_spins, const double* d_v, int kr, double dt,
                           double* d_spins_out, double* d_fnorm);
 
+/* Outer minimum-mode-following loop with the paper's termination test (Alg. 1 l.9-14; SURVEY 8(f) f2,
+ * fixed step instead of a line search):
+ *   repeat:  (lambda, V) <- lowest k modes at x (warm-started from the transported V of the previous step)
+ *            F_mmf = F - 2 (F.v_1) v_1                                  (Eq. 2; v_1 only)
+ *            if ||F_mmf||_2 <= tau_F and lambda_1 < 0 < lambda_2: stop, x is an index-1 saddle
+ *            x <- R(x + dt F_mmf)                                        (retraction for spins)
+ * d_state [N][3] in/out; d_V [k][N][3]: start block if warm_start, holds the modes at the final x on return; k >= 2
+ * (the test needs lambda_2).  info->steps = updates applied, info->converged = the test held at the returned x.
+ * Returns MOTO_ENOTCONV if max_steps was reached without the test holding (outputs valid), or the solver's status if an
+ * inner solve failed.  Synchronises the stream once per step (two scalars and k eigenvalues come back). */
+typedef struct {
+    int32_t steps;              /* updates applied */
+    int32_t converged;          /* 1: ||F_mmf|| <= tau_F and lambda_1 < 0 < lambda_2 at the returned state */
+    double fnorm;               /* ||F_mmf||_2 at the returned state */
+    double lambda[MOTO_KMAX];   /* lowest eigenvalues at the returned state */
+    int64_t hvp_count;          /* single-vector HVPs over all inner solves */
+    int64_t solver_iters;       /* LOBPCG iterations over all inner solves */
+} moto_mmf_info;
+moto_status moto_mmf_run(moto_ctx* ctx, double* d_state, int k, double dt, int max_steps, double tau_F, double tol, int max_iter,
+                         int warm_start, double* d_V, moto_mmf_info* info);
+
 /* Vector transport for warm starts after m -> m' (reading A17): V <- orthonormalise(P_{m'} V), in place. */
 moto_status moto_transport(moto_ctx* ctx, const double* d_spins_new, double* d_V, int k);
 

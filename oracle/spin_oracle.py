@@ -274,3 +274,19 @@ def transformed_operator_apply(model: SpinModel, m: np.ndarray, V: np.ndarray, d
     coeff = Y.T @ (Bm.T @ V.reshape(k, -1).T)            # 2N x k
     out = -(Bm @ (Y @ (pl[:, None] * coeff)))
     return np.ascontiguousarray(out.T).reshape(k, model.N, 3)
+
+
+# ---- O12 outer MMF loop with the paper's termination test (Alg. 1 l.9-14), fixed step dt
+def mmf_run(model: SpinModel, m: np.ndarray, k: int, dt: float, max_steps: int, tau_F: float):
+    """repeat: lowest-k modes (dense eigh) -> F_mmf with v_1 -> stop if |F_mmf| <= tau_F and lam_1 < 0 < lam_2 -> step.
+    Returns (m, lam, steps applied, converged, |F_mmf| at the returned state)."""
+    m = m.copy()
+    for step in range(max_steps + 1):
+        lam, V = lowest_modes(model, m, k)
+        F = mmf_force(model, m, V[:1])
+        fn = float(np.linalg.norm(F))
+        if fn <= tau_F and lam[0] < 0.0 < lam[1]:
+            return m, lam, step, True, fn
+        if step == max_steps:
+            return m, lam, step, False, fn
+        m = mmf_step(model, m, V[:1], dt)

@@ -45,6 +45,11 @@ class SolverOpts(C.Structure):
                 ("precond_lo", C.c_double), ("precond_hi", C.c_double), ("seed", C.c_uint64)]
 
 
+class MmfInfo(C.Structure):
+    _fields_ = [("steps", C.c_int32), ("converged", C.c_int32), ("fnorm", C.c_double), ("lam", C.c_double * KMAX),
+                ("hvp_count", C.c_int64), ("solver_iters", C.c_int64)]
+
+
 class SolveInfo(C.Structure):
     _fields_ = [("iters", C.c_int32), ("converged", C.c_int32), ("resid", C.c_double * KMAX), ("hvp_count", C.c_int64)]
 
@@ -65,6 +70,8 @@ _SIGS = {
     "moto_hvp_three_term": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p,
                                       C.c_void_p, C.c_int]),
     "moto_cheb_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_int]),
+    "moto_mmf_run": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
+                               C.c_void_p, C.POINTER(MmfInfo)]),
     "moto_transport": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "moto_gram": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
     "moto_rayleigh_ritz": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
@@ -243,6 +250,19 @@ class Context:
         fn = self._empty(1) if want_fnorm else None
         self._check(self.lib.moto_mmf_step(self._h, _ptr(spins), _ptr(v), kr, float(dt), _ptr(out), _ptr(fn)))
         return out, fn
+
+    def mmf_run(self, state, k, dt, max_steps, tau_F, tol, max_iter=20000, V0=None):
+        """moto_mmf_run: outer MMF loop with the saddle test; `state` is updated in place.  -> (V, info dict)."""
+        _dev_f64(state, (self.N, 3))
+        if V0 is not None:
+            V, warm = _dev_f64(V0, (k, self.N, 3)).clone(), 1
+        else:
+            V, warm = self._empty(k, self.N, 3), 0
+        info = MmfInfo()
+        st = self._check(self.lib.moto_mmf_run(self._h, _ptr(state), k, float(dt), int(max_steps), float(tau_F), float(tol),
+                                               int(max_iter), warm, _ptr(V), C.byref(info)), allow=(ENOTCONV,))
+        return V, dict(steps=info.steps, converged=bool(info.converged), fnorm=info.fnorm, lam=list(info.lam)[:k],
+                       hvp_count=info.hvp_count, solver_iters=info.solver_iters, status=st)
 
     def transport(self, spins_new, V):
         k = V.shape[0]

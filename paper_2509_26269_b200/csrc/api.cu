@@ -213,6 +213,44 @@ moto_status moto_mmf_step(moto_ctx* c, const double* d_spins, const double* d_v,
     return MOTO_OK;
 }
 
+moto_status moto_mmf_run(moto_ctx* c, double* d_state, int k, double dt, int max_steps, double tau_F, double tol, int max_iter,
+                         int warm_start, double* d_V, moto_mmf_info* info) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_state || !d_V) return moto_fail(c, MOTO_EINVAL, "moto_mmf_run: null argument");
+    if (k < 2 || k > c->kmax) return moto_fail(c, MOTO_EINVAL, "moto_mmf_run: k out of range [2, kmax] (the saddle test needs lambda_2)");
+    if (!(tol > 0) || max_iter < 0 || max_steps < 0 || !(tau_F >= 0)) return moto_fail(c, MOTO_EINVAL, "moto_mmf_run: bad tolerance or cap");
+    const size_t vb = (size_t)c->N * 3 * sizeof(double);
+    double* d_lam = c->st->scal;          // [k] device scratch (k <= 8)
+    double* d_fn = c->st->cheb_ab;        // scalar scratch (rewritten by the next solve)
+    double h_lam[MOTO_KMAX], h_fn = 0.0;
+    moto_mmf_info out; memset(&out, 0, sizeof(out));
+    moto_status st = MOTO_OK;
+    int warm = warm_start;
+    for (int step = 0;; ++step) {
+        moto_solve_info si;
+        st = moto_lowest_modes(c, d_state, k, tol, max_iter, warm, d_lam, d_V, &si);
+        out.hvp_count += si.hvp_count; out.solver_iters += si.iters;
+        if (st != MOTO_OK && st != MOTO_ENOTCONV) break;
+        MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_lam, d_lam, k * sizeof(double), cudaMemcpyDeviceToHost, c->stream));   // before the step reuses scal
+        // candidate update into the staging vector; ||F_mmf|| of the CURRENT state comes with it
+        st = moto_mmf_step(c, d_state, d_V, 1, dt, c->stage_m, d_fn);
+        if (st != MOTO_OK) break;
+        MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&h_fn, d_fn, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+        out.fnorm = h_fn;
+        for (int a = 0; a < k; ++a) out.lambda[a] = h_lam[a];
+        out.steps = step;
+        if (h_fn <= tau_F && h_lam[0] < 0.0 && h_lam[1] > 0.0) { out.converged = 1; st = MOTO_OK; break; }
+        if (step >= max_steps) { st = moto_fail(c, MOTO_ENOTCONV, "moto_mmf_run: max_steps reached before the saddle test held"); break; }
+        MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_state, c->stage_m, vb, cudaMemcpyDeviceToDevice, c->stream));
+        moto_status t = moto_transport(c, d_state, d_V, k);
+        if (t != MOTO_OK) { st = t; break; }
+        warm = 1;
+    }
+    if (info) *info = out;
+    return st;
+}
+
 moto_status moto_transport(moto_ctx* c, const double* d_spins_new, double* d_V, int k) {
     if (!c) return MOTO_EINVAL;
     if (!d_spins_new || !d_V || k < 1 || k > MOTO_KMAX) return moto_fail(c, MOTO_EINVAL, "moto_transport: bad argument");

@@ -92,3 +92,25 @@ def test_bad_geometry_rejected(moto):
     w.cell = np.array([[10.0, 0.0], [0.0, 10.0]])   # rc = 6 > half the cell width
     with pytest.raises(moto.MotoError):
         moto.cart_context(w)
+
+
+def test_mmf_run_cartesian_matches_stepwise_calls(moto, slab):
+    # the outer loop on Cartesian atoms (identity retraction, masked modes): moto_mmf_run == the same calls made one by one,
+    # and its first step == the oracle's step fed the same mode
+    w, mdl = slab
+    ctx = moto.cart_context(w, kmax=4)
+    ctx.set_solver(guard=2)
+    x = dev(w.positions)
+    V, info = ctx.mmf_run(x, 2, 0.05, 2, 0.0, tol=1e-9, max_iter=5000)
+    assert info["steps"] == 2 and not info["converged"]
+    y = dev(w.positions)
+    lam, Vs, _ = ctx.lowest_modes(y, 2, tol=1e-9, max_iter=5000)
+    first = co.mmf_step(mdl, w.positions, Vs[:1].cpu().numpy(), 0.05)
+    for s in range(2):
+        y, _ = ctx.mmf_step(y, Vs[:1].contiguous(), 0.05)
+        if s == 0:
+            assert np.max(np.abs(y.cpu().numpy() - first)) <= 1e-12
+        ctx.transport(y, Vs)
+        lam, Vs, _ = ctx.lowest_modes(y, 2, tol=1e-9, max_iter=5000, V0=Vs)
+    assert np.max(np.abs(x.cpu().numpy() - y.cpu().numpy())) <= 1e-9
+    assert np.array_equal(x.cpu().numpy()[w.fixed == 1], w.positions[w.fixed == 1])

@@ -493,3 +493,31 @@ def test_guard_column_on_the_fused_path(moto):
     assert V.shape[0] == 1 and abs(lam.item() - lam_ref[0]) <= EIG_TOL * abs(lam_ref[0])
     ang = scipy.linalg.subspace_angles(V.cpu().numpy().reshape(1, -1).T, V_ref[:1].reshape(1, -1).T)
     assert ang.max() <= ANGLE_TOL
+
+
+def test_mmf_run_outer_loop(moto):
+    # moto_mmf_run against the oracle's loop: a few steps on small lattices (the trajectory is only compared while the
+    # modes are well separated), and the termination semantics
+    w = wl.config1(L=12, R=2.5)
+    model = model_of(w)
+    m_ref, lam_ref, steps_ref, conv_ref, fn_ref = so.mmf_run(model, w.spins, 2, 0.05, 3, 0.0)
+    ctx = moto.spin_context(w, kmax=2)
+    x = dev(w.spins)
+    V, info = ctx.mmf_run(x, 2, 0.05, 3, 0.0, tol=1e-11, max_iter=5000)
+    assert info["steps"] == 3 and not info["converged"] and info["status"] == moto.ENOTCONV
+    assert np.max(np.abs(x.cpu().numpy() - m_ref)) <= 1e-7
+    assert np.max(np.abs(np.array(info["lam"]) - lam_ref)) <= 1e-7 and abs(info["fnorm"] - fn_ref) <= 1e-6 * fn_ref
+    # huge tau_F: a state with lambda_1 < 0 < lambda_2 is accepted at once and left untouched ...
+    lam0, _ = so.lowest_modes(model, w.spins, 2)
+    if lam0[0] < 0.0 < lam0[1]:
+        x2 = dev(w.spins)
+        _, info2 = ctx.mmf_run(x2, 2, 0.05, 5, 1e9, tol=1e-9, max_iter=5000)
+        assert info2["converged"] and info2["steps"] == 0 and info2["status"] == moto.OK
+        assert np.array_equal(x2.cpu().numpy(), w.spins)
+    # ... and a state with only positive curvatures never is
+    wf = wl.config0(sigma=0.05)
+    ctxf = moto.spin_context(wf, kmax=2)
+    _, info3 = ctxf.mmf_run(dev(wf.spins), 2, 0.05, 2, 1e9, tol=1e-9, max_iter=2000)
+    assert not info3["converged"] and info3["steps"] == 2
+    with pytest.raises(moto.MotoError):
+        ctx.mmf_run(dev(w.spins), 1, 0.05, 2, 1e-3, tol=1e-9)      # k = 1: no lambda_2

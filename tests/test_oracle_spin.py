@@ -285,3 +285,26 @@ def test_transformed_operator_definition_pins():
     lam, Vm = so.lowest_modes(model, w.spins, 1)
     out = so.transformed_operator_apply(model, w.spins, Vm, 5, lam[0] + 0.2, 19.0, lam[0])
     assert np.max(np.abs(out + Vm)) < 1e-10
+
+
+def test_mmf_run_termination_logic():
+    # the loop is the composition of pinned pieces; here: the test is evaluated BEFORE a step, the cap counts applied
+    # steps, and a state without a negative mode can never be declared a saddle
+    w = wl.config1(L=12, R=2.5)
+    model = so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
+    lam0, V0 = so.lowest_modes(model, w.spins, 2)
+    m1, lam1, steps, conv, fn = so.mmf_run(model, w.spins, 2, 0.05, 3, 0.0)
+    assert steps == 3 and not conv
+    ref = w.spins
+    for _ in range(3):
+        _, V = so.lowest_modes(model, ref, 2)
+        ref = so.mmf_step(model, ref, V[:1], 0.05)
+    assert np.max(np.abs(m1 - ref)) < 1e-12
+    if lam0[0] < 0.0 < lam0[1]:
+        m2, _, steps2, conv2, _ = so.mmf_run(model, w.spins, 2, 0.05, 3, 1e9)
+        assert steps2 == 0 and conv2 and np.array_equal(m2, w.spins)
+    wf = wl.config0(sigma=0.05)                     # tilted ferromagnet: all curvatures positive
+    mf = so.SpinModel(wf.Lx, wf.Ly, 1, 1, wf.J, wf.D, wf.K, wf.B, wf.mu)
+    assert so.lowest_modes(mf, wf.spins, 2)[0][0] > 0
+    _, _, steps3, conv3, _ = so.mmf_run(mf, wf.spins, 2, 0.05, 2, 1e9)
+    assert steps3 == 2 and not conv3
