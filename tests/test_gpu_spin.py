@@ -521,3 +521,31 @@ def test_mmf_run_outer_loop(moto):
     assert not info3["converged"] and info3["steps"] == 2
     with pytest.raises(moto.MotoError):
         ctx.mmf_run(dev(w.spins), 1, 0.05, 2, 1e-3, tol=1e-9)      # k = 1: no lambda_2
+
+
+@pytest.mark.parametrize("params", [(-0.7, -0.5, -0.2, (0.3, -0.1, 0.2), 1.7), (0.4, 1.1, 0.3, (0.0, 0.0, -0.5), 0.6)])
+def test_other_parameter_signs(moto, params):
+    # antiferromagnetic exchange, negative / dominant DMI, easy-plane anisotropy, tilted field, mu != 1: HVP parity on both
+    # K1 paths, and the transformed solver (whose upper spectral bound b = max(-c) + lambda_max(L) must hold for any signs)
+    J, D, K, B, mu = params
+    m = wl.random_spins(40, 30, 11)
+    w = wl.SpinWorkload("signs", 40, 30, 1, 0, J, D, K, B, mu, 2, 11, m)
+    model = model_of(w)
+    V = wl.random_block(w.N, 2, seed=12)
+    ref = so.hvp(model, w.spins, V)
+    for path in (1, 2):
+        ctx = moto.spin_context(w, kmax=2)
+        ctx.set_solver(hvp_path=path)
+        assert rel_l2(ctx.hvp(dev(w.spins), dev(V)).cpu().numpy(), ref) <= HVP_TOL
+        E, g = ctx.energy_grad(dev(w.spins))
+        assert abs(E.item() - so.energy(model, w.spins)) <= 1e-12 * abs(so.energy(model, w.spins))
+    lam_ref, V_ref = so.lowest_modes(model, w.spins, 2, extra=1)
+    lam, Vm, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=6000)
+    assert info["converged"], info
+    assert np.max(np.abs(lam.cpu().numpy() - lam_ref[:2]) / np.maximum(np.abs(lam_ref[:2]), 1e-3)) <= EIG_TOL
+    # the bound itself: the whole spectrum lies below max(-c) + lambda_max(L) evaluated by the oracle's pieces
+    Ht, _ = so.tangent_hessian(model, w.spins, dense=True)
+    lam_max = np.linalg.eigvalsh(0.5 * (Ht + Ht.T))[-1]
+    c = so.curvature_scalar(w.spins, so.gradient(model, w.spins))
+    Lmax = np.linalg.eigvalsh(so.euclid_hessian(model).toarray())[-1]
+    assert lam_max <= np.max(-c) + Lmax + 1e-9
