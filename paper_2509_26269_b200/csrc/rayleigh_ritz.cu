@@ -12,80 +12,163 @@ namespace {
 
 constexpr int NMAX = MOTO_NS;       // 24
 constexpr int LD = NMAX + 1;        // smem leading dimension
-constexpr int RR_THREADS = 256;     // gather phase; the dense phase runs on warp 0 alone (warp-level syncs only)
-// dense phase: one warp (warp-level syncs) for n <= 8, the whole CTA for larger pencils (more rotations per round)
-#define RR_SYNC() do { if (wide) __syncthreads(); else __syncwarp(); } while (0)
+constexpr int RR_THREADS = 256;     // smallest block; pencils with more than 256 padded entries get one thread per entry
+constexpr int RR_THREADS_MAX = NMAX * NMAX;
 
-struct JacobiScratch { int p[NMAX / 2], q[NMAX / 2]; double c[NMAX / 2], s[NMAX / 2]; double off, diag; };
+struct JacobiScratch { double off, diag; int dummy_col; };
 
-// Symmetric eigen-decomposition in shared memory: A (n x n, LD) -> diag(A) = eigenvalues, V = eigenvectors (cols).
-__device__ void jacobi_eig(double* A, double* V, int n, JacobiScratch* js, bool wide) {
-    const int tid = threadIdx.x, nt = wide ? blockDim.x : 32;
-    for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; V[i * LD + j] = (i == j) ? 1.0 : 0.0; }
-    RR_SYNC();
+// ---- cyclic Jacobi, tournament (Brent-Luk) ordering with FIXED pair positions: the rotations of a round always act on
+// the position pairs (0,1), (2,3), ..., and after every round rows and columns are permuted by bl_next so that over
+// np - 1 rounds every two indices meet once.  Because positions are fixed, every address a thread touches is
+// loop-invariant: thread (i, j) forms entry (i, j) of J^T A J and of V J straight from the previous buffers (four
+// entries of A, two of V) and writes them to the permuted position of the other buffer of a ping-pong pair.  A round
+// is [one thread per pair: rotation] barrier [one thread per entry: apply] barrier.  Entries (i, j) and (j, i) are
+// computed by the same expression, so A stays exactly symmetric.  An odd n is padded with a zero row/column whose
+// rotations are exact identities (a_pq = 0).
+
+__device__ __forceinline__ int bl_next(int x, int np) {   // the index at position x moves to position bl_next(x)
+    const int h = np / 2;
+    if (x == 0 || h == 1) return x;
+    if (x & 1) return (x == 1) ? 2 : x - 2;               // bottom row shifts left, its head moves up to top[1]
+    return (x == 2 * h - 2) ? 2 * h - 1 : x + 2;          // top row shifts right, its tail drops to the bottom
+}
+
+__device__ __forceinline__ double rcp_approx(double x) { double y; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y; }
+__device__ __forceinline__ float rcp_approx_f(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float sqrt_approx_f(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// Rotation (c, s), t = s / c the smaller root of  apq t^2 + (aqq - app) t - apq = 0, that annihilates A[p][q].
+// A rotation round is a chain of dependent operations on one thread and fp64 operations have ~4x the latency of fp32
+// ones here, IEEE fp64 division and square root ~100x: so the textbook formula is evaluated in fp32 as a seed and
+// refined in fp64 by two Newton steps on the quadratic itself (sharing one approximate reciprocal), and
+// c = (1 + t^2)^{-1/2} by one cubically convergent step from an fp32 seed.  Both end at rounding level, and c, s are
+// formed from the same t, so the rotation is orthogonal to rounding whatever t is (checked against LAPACK in the tests).
+__device__ __forceinline__ void rr_angle(double app, double aqq, double apq, double& c, double& s) {
+    c = 1.0; s = 0.0;
+    if (apq == 0.0) return;
+    const double dlt = aqq - app;
+    const float tau = (float)(dlt * rcp_approx(2.0 * apq));   // +-inf when |dlt| >> |apq|: seed 0, Newton lands on apq / dlt
+    const float den = fabsf(tau) + sqrt_approx_f(fmaf(tau, tau, 1.0f));
+    double t = (double)copysignf(rcp_approx_f(den), tau);
+    if (!(fabsf(tau) < 3.0e38f)) t = 0.0;
+    const double r = rcp_approx(fma(2.0 * apq, t, dlt));
+    t = fma(-fma(fma(apq, t, dlt), t, -apq), r, t);
+    t = fma(-fma(fma(apq, t, dlt), t, -apq), r, t);
+    if (!(fabs(t) <= 1.0000001)) {                            // guard (NaN / overflow corner): the textbook formula
+        const double tq = dlt / (2.0 * apq);
+        t = (tq >= 0.0 ? 1.0 : -1.0) / (fabs(tq) + sqrt(1.0 + tq * tq));
+    }
+    const double x = fma(t, t, 1.0);                          // in [1, 2]
+    const double y = (double)rsqrtf((float)x);
+    const double e = fma(-x * y, y, 1.0);
+    c = fma(y * e, fma(0.375, e, 0.5), y);
+    s = t * c;
+}
+
+// A (n x n, symmetric) -> eigenvalues on the diagonal of A, eigenvectors in the matching columns of V (order arbitrary).
+// A2, V2: scratch of the same shape; rc, rs: NMAX / 2 doubles each.  blockDim.x >= np * np, np = n rounded up to even.
+// All threads of the CTA must call.
+__device__ void jacobi_eig(double* A, double* V, double* A2, double* V2, int n, JacobiScratch* js, double* rc, double* rs) {
+    const int tid = threadIdx.x;
+    const int np = (n + 1) & ~1, h = np / 2;
+    const bool act = tid < np * np;
+    const int i = act ? tid / np : 0, j = act ? tid - i * np : 0;
+    if (act) {
+        if (i >= n || j >= n) A[i * LD + j] = 0.0;
+        V[i * LD + j] = (i == j) ? 1.0 : 0.0;
+    }
+    __syncthreads();
     if (n == 1) return;
-    const int np = (n + 1) & ~1, half = np / 2;
+    // loop-invariant addressing of this thread
+    const int lo = i < j ? i : j, hi = i < j ? j : i;
+    const int pr = lo & ~1, pc = hi & ~1, pv = j & ~1;
+    const bool rowp = !(lo & 1), colp = !(hi & 1), vp = !(j & 1), same_pair = (pr == pc) && (lo != hi);
+    const int src_pp = pr * LD + pc, dst_a = bl_next(i, np) * LD + bl_next(j, np);
+    const int src_v = i * LD + pv, dst_v = i * LD + bl_next(j, np);
+    double *Ac = A, *An = A2, *Vc = V, *Vn = V2;
     for (int sweep = 0; sweep < 30; ++sweep) {
-        double off = 0.0, dg = 0.0;
-        if (tid < 32) {   // warp 0 sums (n*n <= 576 entries), everyone reads the verdict
-            for (int t = tid; t < n * n; t += 32) {
-                int i = t / n, j = t - i * n;
-                double a = A[i * LD + j];
-                if (i == j) dg += a * a; else if (j > i) off += a * a;
+        if (tid < 32) {
+            double off = 0.0, dg = 0.0;
+            for (int t = tid; t < np * np; t += 32) {
+                int a = t / np, b = t - a * np;
+                double x = Ac[a * LD + b];
+                if (a == b) dg += x * x; else if (b > a) off += x * x;
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) { off += __shfl_xor_sync(0xffffffffu, off, o); dg += __shfl_xor_sync(0xffffffffu, dg, o); }
             if (tid == 0) { js->off = off; js->diag = dg; }
         }
-        RR_SYNC();
-        off = js->off; dg = js->diag;
-        RR_SYNC();
-        if (off <= 1e-30 * dg || off == 0.0) break;   // off-diagonals below 1e-15 of the diagonal scale: rounding level   // off-diagonals below 1e-15 of the diagonal scale: rounding level
+        __syncthreads();
+        const double off = js->off, dg = js->diag;
+        __syncthreads();
+        if (off <= 1e-30 * dg || off == 0.0) break;   // off-diagonals below 1e-15 of the diagonal scale: rounding level
         for (int r = 0; r < np - 1; ++r) {
-            if (tid < half) {
-                int p, q;
-                if (tid == 0) { p = np - 1; q = r; }
-                else { p = (r + tid) % (np - 1); q = (r - tid + (np - 1)) % (np - 1); }
-                if (p > q) { int t = p; p = q; q = t; }
-                double c = 1.0, s = 0.0;
-                if (q < n) {
-                    double apq = A[p * LD + q];
-                    if (apq != 0.0) {
-                        double app = A[p * LD + p], aqq = A[q * LD + q];
-                        double tau = (aqq - app) / (2.0 * apq);
-                        double t = (tau >= 0.0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
-                        c = 1.0 / sqrt(1.0 + t * t);
-                        s = t * c;
-                    }
-                } else { p = -1; }
-                js->p[tid] = p; js->q[tid] = q; js->c[tid] = c; js->s[tid] = s;
+            if (tid < h) {
+                double c, s;
+                rr_angle(Ac[(2 * tid) * LD + 2 * tid], Ac[(2 * tid + 1) * LD + 2 * tid + 1], Ac[(2 * tid) * LD + 2 * tid + 1], c, s);
+                rc[tid] = c; rs[tid] = s;
             }
-            RR_SYNC();
-            // columns: A <- A J, V <- V J
-            for (int w = tid; w < half * n; w += nt) {
-                int t = w / n, i = w - t * n, p = js->p[t], q = js->q[t];
-                if (p < 0) continue;
-                double c = js->c[t], s = js->s[t];
-                double aip = A[i * LD + p], aiq = A[i * LD + q];
-                A[i * LD + p] = c * aip - s * aiq; A[i * LD + q] = s * aip + c * aiq;
-                double vip = V[i * LD + p], viq = V[i * LD + q];
-                V[i * LD + p] = c * vip - s * viq; V[i * LD + q] = s * vip + c * viq;
+            __syncthreads();
+            if (act) {
+                const double cr = rc[lo >> 1], sr = rs[lo >> 1], cc = rc[hi >> 1], sc = rs[hi >> 1];
+                const double a_pp = Ac[src_pp], a_pq = Ac[src_pp + 1], a_qp = Ac[src_pp + LD], a_qq = Ac[src_pp + LD + 1];
+                const double b_p = colp ? cc * a_pp - sc * a_pq : sc * a_pp + cc * a_pq;   // (A J)[pr][hi]
+                const double b_q = colp ? cc * a_qp - sc * a_qq : sc * a_qp + cc * a_qq;   // (A J)[pr+1][hi]
+                double anew = rowp ? cr * b_p - sr * b_q : sr * b_p + cr * b_q;           // (J^T A J)[lo][hi]
+                if (same_pair) anew = 0.0;      // the annihilated entry (exact zeros let the sweep test reach its floor)
+                An[dst_a] = anew;
+                const double cv = rc[j >> 1], sv = rs[j >> 1];
+                const double v_p = Vc[src_v], v_q = Vc[src_v + 1];
+                Vn[dst_v] = vp ? cv * v_p - sv * v_q : sv * v_p + cv * v_q;               // (V J)[i][j]
             }
-            RR_SYNC();
-            // rows: A <- J^T A
-            for (int w = tid; w < half * n; w += nt) {
-                int t = w / n, j = w - t * n, p = js->p[t], q = js->q[t];
-                if (p < 0) continue;
-                double c = js->c[t], s = js->s[t];
-                double apj = A[p * LD + j], aqj = A[q * LD + j];
-                A[p * LD + j] = c * apj - s * aqj; A[q * LD + j] = s * apj + c * aqj;
-            }
-            RR_SYNC();
-            if (tid < half && js->p[tid] >= 0) { int p = js->p[tid], q = js->q[tid]; A[p * LD + q] = 0.0; A[q * LD + p] = 0.0; }
-            RR_SYNC();
+            __syncthreads();
+            double* t = Ac; Ac = An; An = t;
+            t = Vc; Vc = Vn; Vn = t;
         }
     }
-    RR_SYNC();
+    if (Ac != A) {   // uniform
+        if (act) { A[i * LD + j] = Ac[i * LD + j]; V[i * LD + j] = Vc[i * LD + j]; }
+        __syncthreads();
+    }
+    if (np != n) {   // the padding index ended at some position: move the pair at position n into its place
+        if (tid < np && V[n * LD + tid] != 0.0) js->dummy_col = tid;   // its eigenvector is e_n exactly
+        __syncthreads();
+        const int jd = js->dummy_col;
+        if (jd != n) {
+            if (tid < n) V[tid * LD + jd] = V[tid * LD + n];
+            if (tid == 0) A[jd * LD + jd] = A[n * LD + n];
+        }
+        __syncthreads();
+    }
+}
+
+// Cholesky whitening of the unit-diagonal G_B (every direction kept): B = L L^T in place, Linv = L^{-1} into U,
+// returns false (uniformly) when a pivot falls below thr, in which case the caller takes the eigen-decomposition path
+// with its rank truncation.  B is destroyed either way only below/at the failing step, so the caller re-scales it.
+__device__ bool chol_whiten(double* B, double* Lw, double* U, int n, double thr) {
+    const int tid = threadIdx.x;
+    const bool act = tid < n * n;
+    const int i = act ? tid / n : 0, k = act ? tid - i * n : 0;
+    for (int j = 0; j < n; ++j) {
+        const double piv = B[j * LD + j];
+        if (!(piv > thr)) return false;
+        if (act && i > j && k > j) B[i * LD + k] -= B[i * LD + j] * B[k * LD + j] / piv;
+        __syncthreads();
+    }
+    if (act) Lw[i * LD + k] = (i >= k) ? B[i * LD + k] * rsqrt(B[k * LD + k]) : 0.0;
+    __syncthreads();
+    if (tid < n) {       // column tid of L^{-1} by forward substitution
+        const int c = tid;
+        for (int r = 0; r < c; ++r) U[r * LD + c] = 0.0;
+        U[c * LD + c] = 1.0 / Lw[c * LD + c];
+        for (int r = c + 1; r < n; ++r) {
+            double s = 0.0;
+            for (int q = c; q < r; ++q) s = fma(Lw[r * LD + q], U[q * LD + c], s);
+            U[r * LD + c] = -s / Lw[r * LD + r];
+        }
+    }
+    __syncthreads();
+    return true;
 }
 
 // vals[e] = sum_b partials[b * stride + e] in a fixed order with every load independent (the serial version of
@@ -131,13 +214,13 @@ struct RRFast {            // inputs of the fused kb <= 2 path (lobpcg_fast.cu);
 };
 
 // mode 0: Rayleigh-Ritz (theta[nev], C[n][nev]);  mode 1: Loewdin orthonormalisation from G_B only (C[n][n])
-__global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ partials, int nblk, const double* __restrict__ GA_in,
+__global__ void __launch_bounds__(RR_THREADS_MAX) k_rr(const double* __restrict__ partials, int nblk, const double* __restrict__ GA_in,
                                                    const double* __restrict__ GB_in, int n, int nev, double* __restrict__ theta_out,
-                                                   double* __restrict__ C_out, int mode, SolverState* st, double tau, RRFast fz) {
+                                                   double* __restrict__ C_out, int mode, SolverState* st, double tau, double chol_thr, RRFast fz) {
     if (st && st->done) return;
     __shared__ double A[NMAX * LD], B[NMAX * LD], U[NMAX * LD], M[NMAX * LD], T[NMAX * LD], Z[NMAX * LD];
     __shared__ double vals[NMAX * 2 * NMAX];
-    __shared__ double d[NMAX], sig[NMAX], th[NMAX];
+    __shared__ double d[NMAX], sig[NMAX], th[NMAX], rc_s[NMAX + 1], rs_s[NMAX + 1];
     __shared__ int keep[NMAX], ord[NMAX], na_s, bad_s, stop_s;
     __shared__ JacobiScratch js;
     const int tid = threadIdx.x;
@@ -201,9 +284,7 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         A[i * LD + j] = 0.5 * (T[i * LD + j] + T[j * LD + i]);
     }
     __syncthreads();
-    // ---- dense phase: warp 0 alone for small pencils (warp-level synchronisation only), the whole CTA otherwise
-    const bool wide = n > 8;
-    if (!wide) { if (tid >= 32) return; nt = 32; }
+    // ---- dense phase
     if (st && partials) {  // keep a copy for diagnostics
         for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; st->GA[t] = A[i * LD + j]; st->GB[t] = B[i * LD + j]; }
     }
@@ -213,11 +294,25 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         d[tid] = (bii > 1e-300) ? rsqrt(bii) : 0.0;
     }
     if (tid == 0) bad_s = 0;
-    RR_SYNC();
+    __syncthreads();
     for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; B[i * LD + j] *= d[i] * d[j]; }
-    RR_SYNC();
-    // 3. eigen-decomposition of the scaled G_B
-    jacobi_eig(B, U, n, &js, wide);
+    __syncthreads();
+    // 3. whitening of the scaled G_B.  n > 8, Rayleigh-Ritz mode: Cholesky when every pivot clears chol_thr ...
+    bool whitened = false;
+    if (mode == 0 && chol_thr > 0.0) {
+        for (int t = tid; t < n * n; t += nt) { int i = t / n, j = t - i * n; Z[i * LD + j] = B[i * LD + j]; }
+        __syncthreads();
+        whitened = chol_whiten(Z, T, U, n, chol_thr);
+        if (whitened) {   // M = D L^{-T}  (n x n), every direction kept
+            for (int t = tid; t < n * n; t += nt) { int i = t / n, l = t - i * n; M[i * LD + l] = d[i] * U[l * LD + i]; }
+            if (tid < n) { keep[tid] = tid; sig[tid] = 1.0; }
+            if (tid == 0) na_s = n;
+        }
+        __syncthreads();
+    }
+    // ... otherwise eigen-decomposition of the scaled G_B with rank truncation (canonical orthogonalisation)
+    if (!whitened) {
+    jacobi_eig(B, U, T, Z, n, &js, rc_s, rs_s);
     if (tid == 0) {
         double smax = 0.0;
         for (int j = 0; j < n; ++j) { sig[j] = B[j * LD + j]; if (sig[j] > smax) smax = sig[j]; }
@@ -226,14 +321,15 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         na_s = na;
         if (!(smax == smax)) bad_s = 1;
     }
-    RR_SYNC();
-    const int na = na_s;
+    __syncthreads();
     // M = D U_keep Sigma^{-1/2}   (n x na)
-    for (int t = tid; t < n * na; t += nt) {
-        int i = t / na, l = t - i * na, j = keep[l];
+    for (int t = tid; t < n * na_s; t += nt) {
+        int i = t / na_s, l = t - i * na_s, j = keep[l];
         M[i * LD + l] = d[i] * U[i * LD + j] * rsqrt(sig[j]);
     }
-    RR_SYNC();
+    __syncthreads();
+    }
+    const int na = na_s;
     if (mode == 1) {
         // Loewdin: C = M (U_keep)^T D^{-1}... applied to the ORIGINAL vectors: C = D U S^{-1/2} U^T  (n x n)
         for (int t = tid; t < n * n; t += nt) {
@@ -252,17 +348,17 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         for (int j = 0; j < n; ++j) s += A[i * LD + j] * M[j * LD + l];
         T[i * LD + l] = s;
     }
-    RR_SYNC();
+    __syncthreads();
     for (int t = tid; t < na * na; t += nt) {
         int a = t / na, b = t - a * na;
         double s = 0.0;
         for (int i = 0; i < n; ++i) s += M[i * LD + a] * T[i * LD + b];
         B[a * LD + b] = s;
     }
-    RR_SYNC();
+    __syncthreads();
     for (int t = tid; t < na * na; t += nt) { int a = t / na, b = t - a * na; A[a * LD + b] = 0.5 * (B[a * LD + b] + B[b * LD + a]); }
-    RR_SYNC();
-    jacobi_eig(A, Z, na, &js, wide);
+    __syncthreads();
+    jacobi_eig(A, Z, B, T, na, &js, rc_s, rs_s);
     // 5. sort ascending
     if (tid == 0) {
         for (int j = 0; j < na; ++j) { th[j] = A[j * LD + j]; ord[j] = j; }
@@ -274,7 +370,7 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
         if (na < nev) bad_s = 1;
         for (int a = 0; a < nev && a < na; ++a) if (!(th[ord[a]] == th[ord[a]])) bad_s = 1;
     }
-    RR_SYNC();
+    __syncthreads();
     // 6. C = M Z[:, lowest nev]
     for (int t = tid; t < n * nev; t += nt) {
         int i = t / nev, j = t - i * nev;
@@ -288,11 +384,16 @@ __global__ void __launch_bounds__(RR_THREADS) k_rr(const double* __restrict__ pa
 
 }  // namespace
 
+// block of the launch: 256 threads for n <= 8, one thread per entry (rounded to warps) above
+static inline int rr_threads(int n) { int np = (n + 1) & ~1, t = (np * np + 31) & ~31; return t > RR_THREADS ? t : RR_THREADS; }
+// pivots of the unit-diagonal G_B below this send the pencil to the truncating eigen-decomposition path
+static const double CHOL_THR = 1e-8;
+
 int rr_solve(moto_ctx* c, const double* d_GA, const double* d_GB, int n, int nev, double* d_theta, double* d_C, int mode,
              SolverState* st) {
     const double tau = 1e-10;
     RRFast fz = {nullptr, 0, 0, 0, 0, 0, 0.0};
-    k_rr<<<1, RR_THREADS, 0, c->stream>>>(nullptr, 0, d_GA, d_GB, n, nev, d_theta, d_C, mode, st, tau, fz);
+    k_rr<<<1, rr_threads(n), 0, c->stream>>>(nullptr, 0, d_GA, d_GB, n, nev, d_theta, d_C, mode, st, tau, CHOL_THR, fz);
     return 1;
 }
 
@@ -300,7 +401,7 @@ int rr_solve(moto_ctx* c, const double* d_GA, const double* d_GB, int n, int nev
 int rr_solve_lobpcg(moto_ctx* c, int kb, int nblk) {
     const double tau = 1e-10;
     RRFast fz = {nullptr, 0, 0, 0, 0, 0, 0.0};
-    k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblk, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, fz);
+    k_rr<<<1, rr_threads(3 * kb), 0, c->stream>>>(c->partials, nblk, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, CHOL_THR, fz);
     return 1;
 }
 
@@ -308,6 +409,6 @@ int rr_solve_lobpcg(moto_ctx* c, int kb, int nblk) {
 int rr_solve_fast(moto_ctx* c, int kb, int nblkU, const double* partialsK, int nblkK, int check, int k, double tol, int hvp_inc) {
     const double tau = 1e-10;
     RRFast fz = {partialsK, nblkK, kb, check, hvp_inc, k, tol};
-    k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblkU, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, fz);
+    k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblkU, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, CHOL_THR, fz);
     return 1;
 }

@@ -176,6 +176,29 @@ def test_rayleigh_ritz_drops_null_directions(moto):
     assert np.max(np.abs(th.cpu().numpy() - ref[:2])) <= 1e-10 * np.max(np.abs(ref))
 
 
+@pytest.mark.parametrize("n,nbad", [(18, 3), (21, 1), (24, 6), (9, 2), (15, 0)])
+def test_rayleigh_ritz_wide_pencils_rank_deficient(moto, n, nbad):
+    # n > 8 takes the one-thread-per-entry path: Cholesky whitening when G_B is well conditioned, the truncating
+    # eigen-decomposition when it is not (nbad dependent basis vectors: zero columns and duplicates)
+    rng = np.random.default_rng(100 + n)
+    S = rng.standard_normal((60, n))
+    for b in range(nbad):
+        if b % 2 == 0: S[:, n - 1 - b] = 0.0
+        else: S[:, n - 1 - b] = S[:, b] * 1.5
+    Aop = rng.standard_normal((60, 60)); Aop = Aop + Aop.T
+    GA, GB = S.T @ Aop @ S, S.T @ S
+    nev = n // 3
+    w = wl.config0()
+    ctx = moto.spin_context(w, kmax=8)
+    th, Cm = ctx.rayleigh_ritz(dev(GA), dev(GB), nev)
+    th, Cm = th.cpu().numpy(), Cm.cpu().numpy()
+    Sr = S[:, :n - nbad]
+    ref = scipy.linalg.eigh(Sr.T @ Aop @ Sr, Sr.T @ Sr, eigvals_only=True)
+    assert np.max(np.abs(th - ref[:nev])) <= 1e-10 * np.max(np.abs(ref))
+    assert np.max(np.abs(Cm.T @ GB @ Cm - np.eye(nev))) <= 1e-10
+    assert np.max(np.abs(Cm.T @ GA @ Cm - np.diag(th))) <= 1e-9 * np.max(np.abs(ref))
+
+
 def _check_modes(w, lam, V, lam_ref, V_ref, k):
     lam = lam.cpu().numpy(); V = V.cpu().numpy()
     relerr = np.abs(lam - lam_ref[:k]) / np.maximum(np.abs(lam_ref[:k]), 1e-3)
