@@ -67,6 +67,87 @@ __global__ void k_gram_final(const double* __restrict__ partials, int nblk, int 
     G[e] = s;
 }
 
+// ---------------------------------------------------------------- K3 for the LOBPCG basis: symmetric, register-tiled
+// Upper triangles of G_B = S^T S and G_A = S^T (A S) for S = [X,W,P] (n = 3 kb columns).  k_gram above spends two
+// shared-memory loads per multiply-add and forms all n x 2n products; here a thread owns one 3 x 3 tile (I <= J) of
+// both matrices for a slice of the staged chunk: nine loads feed eighteen multiply-adds, and only the nb (nb + 1) / 2
+// upper tiles exist.  Threads = tiles x slices; slices are summed in a fixed order at the end.
+// Output per CTA: [G_B upper triangle (nT) | G_A upper triangle (nT)], entry (a <= b) at a n - a (a - 1) / 2 + (b - a).
+struct GramPtrs { const double* s[MOTO_NS]; const double* as[MOTO_NS]; };
+constexpr int GS_THREADS = 256;
+constexpr int GS_QPER = 4;        // flat elements per slice per staged chunk
+
+__global__ void __launch_bounds__(GS_THREADS) k_gram_sym(GramPtrs P, int n, int nslice, long long n3,
+                                                         double* __restrict__ partials, const int* __restrict__ done) {
+    if (done && *done) return;
+    extern __shared__ double sm[];
+    const int nb = n / 3, ntile = nb * (nb + 1) / 2, NR = 2 * n + 1, Q = nslice * GS_QPER;
+    const int t = threadIdx.x;
+    const int tile = t % ntile, slice = t / ntile;
+    const bool act = slice < nslice;
+    int I = 0, rem = tile;
+    while (rem >= nb - I) { rem -= nb - I; ++I; }
+    const int J = I + rem;
+    double gb[9], ga[9];
+#pragma unroll
+    for (int x = 0; x < 9; ++x) { gb[x] = 0.0; ga[x] = 0.0; }
+    const long long nchunk = (n3 + Q - 1) / Q;
+    for (long long ch = blockIdx.x; ch < nchunk; ch += gridDim.x) {
+        const long long base = ch * Q;
+        for (int idx = t; idx < 2 * n * Q; idx += GS_THREADS) {
+            const int row = idx / Q, q = idx - row * Q;
+            const long long e = base + q;
+            double val = 0.0;
+            if (e < n3) val = (row < n) ? P.s[row][e] : P.as[row - n][e];
+            sm[q * NR + row] = val;
+        }
+        __syncthreads();
+        if (act) {
+#pragma unroll
+            for (int u = 0; u < GS_QPER; ++u) {
+                const double* r = sm + (slice + u * nslice) * NR;
+                double si[3], sj[3], aj[3];
+#pragma unroll
+                for (int a = 0; a < 3; ++a) { si[a] = r[3 * I + a]; sj[a] = r[3 * J + a]; aj[a] = r[n + 3 * J + a]; }
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b) { gb[a * 3 + b] = fma(si[a], sj[b], gb[a * 3 + b]); ga[a * 3 + b] = fma(si[a], aj[b], ga[a * 3 + b]); }
+            }
+        }
+        __syncthreads();
+    }
+    // slices -> one partial per CTA, fixed order
+    double* red = sm;    // [GS_THREADS][18]
+#pragma unroll
+    for (int x = 0; x < 9; ++x) { red[t * 18 + x] = act ? gb[x] : 0.0; red[t * 18 + 9 + x] = act ? ga[x] : 0.0; }
+    __syncthreads();
+    const int nT = n * (n + 1) / 2;
+    for (int o = t; o < ntile * 18; o += GS_THREADS) {
+        const int tl = o / 18, x = o - tl * 18, which = x / 9, ab = x - which * 9, a = ab / 3, b = ab - a * 3;
+        int I2 = 0, rem2 = tl;
+        while (rem2 >= nb - I2) { rem2 -= nb - I2; ++I2; }
+        const int i = 3 * I2 + a, j = 3 * (I2 + rem2) + b;
+        if (i > j) continue;    // lower half of a diagonal tile
+        double sum = 0.0;
+        for (int sl = 0; sl < nslice; ++sl) sum += red[(sl * ntile + tl) * 18 + x];
+        partials[(size_t)blockIdx.x * (2 * nT) + which * nT + i * n - i * (i - 1) / 2 + (j - i)] = sum;
+    }
+}
+
+// out[e] = sum_b partials[b][e]: one warp per entry, lanes stride over the CTAs, fixed shuffle tree
+__global__ void __launch_bounds__(256) k_reduce_partials(const double* __restrict__ partials, int nblk, int ne, double* __restrict__ out,
+                                                         const int* __restrict__ done) {
+    if (done && *done) return;
+    const int e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (e >= ne) return;
+    double s = 0.0;
+    for (int b = lane; b < nblk; b += 32) s += partials[(size_t)b * ne + e];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) out[e] = s;
+}
+
 // ---------------------------------------------------------------- K5 block update, element-wise, in place
 //   X' = [X,W,P] C ; P' = [W,P] C_{W,P rows} ; same coefficients on AX, AW, AP (PAPER.md ref [27])
 template <int KB>
@@ -265,17 +346,29 @@ int block_gram(moto_ctx* c, const double* const* S, int ns, const double* const*
     return 1;
 }
 
-// Gram of the LOBPCG basis: S = [X,W,P] (3kb), T = [S, AS] (6kb); partials stay in ctx->partials for rr_solve.
-// Returns the number of partial blocks through *nblk_out semantics: blocks = min(nchunk, MOTO_RED_BLOCKS).
+// Gram of the LOBPCG basis S = [X,W,P] (n = 3 kb): upper triangles of S^T S and S^T (A S), summed over the CTAs into
+// gram_reduced(c) = [G_B tri | G_A tri] for rr_solve_lobpcg.
+double* gram_reduced(const moto_ctx* c) { return c->partials + (size_t)(MOTO_RED_BLOCKS - 1) * 2 * MOTO_NS * MOTO_NS; }
+
 int block_gram_lobpcg(moto_ctx* c, int kb) {
     const size_t bs = (size_t)3 * c->N;
-    const double* S[MOTO_NS]; const double* T[2 * MOTO_NS];
+    GramPtrs P;
     for (int j = 0; j < kb; ++j) {
-        S[j] = c->X + j * bs; S[kb + j] = c->W + j * bs; S[2 * kb + j] = c->P + j * bs;
-        T[3 * kb + j] = c->AX + j * bs; T[4 * kb + j] = c->AW + j * bs; T[5 * kb + j] = c->AP + j * bs;
+        P.s[j] = c->X + j * bs; P.s[kb + j] = c->W + j * bs; P.s[2 * kb + j] = c->P + j * bs;
+        P.as[j] = c->AX + j * bs; P.as[kb + j] = c->AW + j * bs; P.as[2 * kb + j] = c->AP + j * bs;
     }
-    for (int j = 0; j < 3 * kb; ++j) T[j] = S[j];
-    return block_gram(c, S, 3 * kb, T, 6 * kb, nullptr, &c->st->done);
+    const int n = 3 * kb, ntile = kb * (kb + 1) / 2, nT = n * (n + 1) / 2;
+    int nslice = GS_THREADS / ntile;
+    if (nslice > 32) nslice = 32;
+    const long long n3 = 3ll * c->N;
+    const int Q = nslice * GS_QPER;
+    const long long nchunk = (n3 + Q - 1) / Q;
+    const int blocks = (int)(nchunk < MOTO_RED_BLOCKS ? nchunk : MOTO_RED_BLOCKS);
+    size_t smem = (size_t)Q * (2 * n + 1) * sizeof(double), smem_red = (size_t)GS_THREADS * 18 * sizeof(double);
+    if (smem < smem_red) smem = smem_red;
+    k_gram_sym<<<blocks, GS_THREADS, smem, c->stream>>>(P, n, nslice, n3, c->partials, &c->st->done);
+    k_reduce_partials<<<(2 * nT * 32 + 255) / 256, 256, 0, c->stream>>>(c->partials, blocks, 2 * nT, gram_reduced(c), &c->st->done);
+    return 2;
 }
 
 int gram_blocks(const moto_ctx* c) {

@@ -131,6 +131,7 @@ int block_residual(moto_ctx*, const double* m_or_null, int kb, int k, double tol
 int block_random(moto_ctx*, double* X, int kb, uint64_t seed);
 int block_zero(moto_ctx*, double* X, long long n);
 int gram_blocks(const moto_ctx*);
+double* gram_reduced(const moto_ctx*);   // [G_B upper triangle | G_A upper triangle] left by block_gram_lobpcg
 int rr_solve_lobpcg(moto_ctx*, int kb, int nblk);
 bool cart_geometry_ok(const moto_lattice* lat, double rc);
 int block_apply_coeffs(moto_ctx*, double* V, int k, const double* d_C, double* scratch);

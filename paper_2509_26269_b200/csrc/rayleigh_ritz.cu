@@ -261,6 +261,16 @@ __global__ void __launch_bounds__(RR_THREADS_MAX) k_rr(const double* __restrict_
             U[i * LD + j] = vals[e];
             T[i * LD + j] = ga;
         }
+    } else if (partials && nblk < 0) {
+        // already reduced upper triangles [G_B | G_A] (block_gram_lobpcg)
+        const int nT = n * (n + 1) / 2;
+        for (int t = tid; t < n * n; t += nt) {
+            int i = t / n, j = t - i * n;
+            int a = i < j ? i : j, b = i < j ? j : i;
+            int e = a * n - a * (a - 1) / 2 + (b - a);
+            U[i * LD + j] = partials[e];
+            T[i * LD + j] = partials[nT + e];
+        }
     } else if (partials) {
         const int ntc = 2 * n, ne = n * ntc;
         reduce_partials(partials, nblk, ne, ne, vals, Z);
@@ -397,11 +407,11 @@ int rr_solve(moto_ctx* c, const double* d_GA, const double* d_GB, int n, int nev
     return 1;
 }
 
-// LOBPCG flavour: inputs are the Gram partials left in ctx->partials by block_gram_lobpcg
-int rr_solve_lobpcg(moto_ctx* c, int kb, int nblk) {
+// LOBPCG flavour: inputs are the reduced Gram triangles left by block_gram_lobpcg
+int rr_solve_lobpcg(moto_ctx* c, int kb, int /*nblk*/) {
     const double tau = 1e-10;
     RRFast fz = {nullptr, 0, 0, 0, 0, 0, 0.0};
-    k_rr<<<1, rr_threads(3 * kb), 0, c->stream>>>(c->partials, nblk, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, CHOL_THR, fz);
+    k_rr<<<1, rr_threads(3 * kb), 0, c->stream>>>(gram_reduced(c), -1, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, CHOL_THR, fz);
     return 1;
 }
 
