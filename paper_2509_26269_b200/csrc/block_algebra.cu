@@ -76,6 +76,7 @@ __global__ void k_gram_final(const double* __restrict__ partials, int nblk, int 
 struct GramPtrs { const double* s[MOTO_NS]; const double* as[MOTO_NS]; };
 constexpr int GS_THREADS = 256;
 constexpr int GS_QPER = 4;        // flat elements per slice per staged chunk
+constexpr int GS_LMAX = 10;       // staged values per thread per chunk: 2 n Q / 256 <= 9.4 for every kb <= 8
 
 __global__ void __launch_bounds__(GS_THREADS) k_gram_sym(GramPtrs P, int n, int nslice, long long n3,
                                                          double* __restrict__ partials, const int* __restrict__ done) {
@@ -92,16 +93,38 @@ __global__ void __launch_bounds__(GS_THREADS) k_gram_sym(GramPtrs P, int n, int 
 #pragma unroll
     for (int x = 0; x < 9; ++x) { gb[x] = 0.0; ga[x] = 0.0; }
     const long long nchunk = (n3 + Q - 1) / Q;
-    for (long long ch = blockIdx.x; ch < nchunk; ch += gridDim.x) {
-        const long long base = ch * Q;
-        for (int idx = t; idx < 2 * n * Q; idx += GS_THREADS) {
+    const int tot = 2 * n * Q;                 // staged values per chunk (<= GS_LMAX per thread)
+    // chunk ch + gridDim.x is fetched into registers (all loads in flight at once) while chunk ch is multiplied
+    // per-thread staging slots (chunk-invariant): source pointer at q = 0 of the chunk, flat offset q, smem offset
+    double v[GS_LMAX];
+    const double* gp[GS_LMAX];
+    int qo[GS_LMAX];       // (q << 16) | smem offset; -1: no slot
+#pragma unroll
+    for (int u = 0; u < GS_LMAX; ++u) {
+        const int idx = t + u * GS_THREADS;
+        qo[u] = -1; gp[u] = nullptr;
+        if (idx < tot) {
             const int row = idx / Q, q = idx - row * Q;
-            const long long e = base + q;
-            double val = 0.0;
-            if (e < n3) val = (row < n) ? P.s[row][e] : P.as[row - n][e];
-            sm[q * NR + row] = val;
+            gp[u] = ((row < n) ? P.s[row] : P.as[row - n]) + q;
+            qo[u] = (q << 16) | (q * NR + row);
         }
+    }
+    auto fetch = [&](long long ch) {
+        const long long base = ch * Q;
+        const bool full = base + Q <= n3;
+#pragma unroll
+        for (int u = 0; u < GS_LMAX; ++u) {
+            v[u] = 0.0;
+            if (qo[u] >= 0 && (full || base + (qo[u] >> 16) < n3)) v[u] = gp[u][base];
+        }
+    };
+    if (blockIdx.x < nchunk) fetch(blockIdx.x);
+    for (long long ch = blockIdx.x; ch < nchunk; ch += gridDim.x) {
+#pragma unroll
+        for (int u = 0; u < GS_LMAX; ++u)
+            if (qo[u] >= 0) sm[qo[u] & 0xffff] = v[u];
         __syncthreads();
+        if (ch + gridDim.x < nchunk) fetch(ch + gridDim.x);
         if (act) {
 #pragma unroll
             for (int u = 0; u < GS_QPER; ++u) {

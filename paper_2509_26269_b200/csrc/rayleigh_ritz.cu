@@ -152,7 +152,10 @@ __device__ bool chol_whiten(double* B, double* Lw, double* U, int n, double thr)
     for (int j = 0; j < n; ++j) {
         const double piv = B[j * LD + j];
         if (!(piv > thr)) return false;
-        if (act && i > j && k > j) B[i * LD + k] -= B[i * LD + j] * B[k * LD + j] / piv;
+        double rpiv = rcp_approx(piv);          // piv in (thr, ~n]: two Newton steps reach rounding level
+        rpiv = rpiv * fma(-piv, rpiv, 2.0);
+        rpiv = rpiv * fma(-piv, rpiv, 2.0);
+        if (act && i > j && k > j) B[i * LD + k] = fma(-B[i * LD + j] * rpiv, B[k * LD + j], B[i * LD + k]);
         __syncthreads();
     }
     if (act) Lw[i * LD + k] = (i >= k) ? B[i * LD + k] * rsqrt(B[k * LD + k]) : 0.0;
@@ -369,17 +372,18 @@ __global__ void __launch_bounds__(RR_THREADS_MAX) k_rr(const double* __restrict_
     for (int t = tid; t < na * na; t += nt) { int a = t / na, b = t - a * na; A[a * LD + b] = 0.5 * (B[a * LD + b] + B[b * LD + a]); }
     __syncthreads();
     jacobi_eig(A, Z, B, T, na, &js, rc_s, rs_s);
-    // 5. sort ascending
-    if (tid == 0) {
-        for (int j = 0; j < na; ++j) { th[j] = A[j * LD + j]; ord[j] = j; }
-        for (int a = 0; a < na; ++a) {
-            int best = a;
-            for (int b = a + 1; b < na; ++b) if (th[ord[b]] < th[ord[best]]) best = b;
-            int t = ord[a]; ord[a] = ord[best]; ord[best] = t;
+    // 5. sort ascending: thread j ranks eigenvalue j (ties by index; NaNs rank last and flag the solve)
+    if (tid < na) {
+        const double x = A[tid * LD + tid];
+        int rank = 0;
+        for (int b = 0; b < na; ++b) {
+            const double y = A[b * LD + b];
+            if (y < x || (y == x && b < tid) || (!(x == x) && (y == y || b < tid))) ++rank;
         }
-        if (na < nev) bad_s = 1;
-        for (int a = 0; a < nev && a < na; ++a) if (!(th[ord[a]] == th[ord[a]])) bad_s = 1;
+        th[tid] = x; ord[rank] = tid;
+        if (rank < nev && !(x == x)) bad_s = 1;
     }
+    if (tid == 0 && na < nev) bad_s = 1;
     __syncthreads();
     // 6. C = M Z[:, lowest nev]
     for (int t = tid; t < n * nev; t += nt) {
