@@ -77,6 +77,10 @@ typedef struct {
     double precond_lo;      /* margin: the damped interval starts at theta_k + margin           [0 -> 0.01] */
     double precond_hi;      /* upper end b >= lambda_max of the damped interval    [0 -> max(-c_i) + ||L||] */
     uint64_t seed;          /* seed of the counter-based start block when warm_start=0  [0x9E3779B97F4A7C15] */
+    int32_t method;         /* 0 = block LOBPCG, 1 = thick-restart Lanczos with full re-orthogonalisation
+                               (single start vector, guard / precond_* ignored)          [0]  */
+    int32_t ncv;            /* Lanczos basis size m, k + 2 <= m <= min(24, S kmax - 1, dof - 1) with S = 8 blocks
+                               (spin lattices) or 6 (Cartesian) of the workspace; 0 = the largest that fits   [0]  */
 } moto_solver_opts;
 
 typedef struct {

@@ -103,6 +103,7 @@ moto_status moto_create(const moto_lattice* lat, const void* params, void* d_wor
         if (!(c->mp.rc > 0) || !cart_geometry_ok(lat, c->mp.rc)) { delete c; return MOTO_EINVAL; }
     }
     char* p = c->ws;
+    c->block_bytes = w.block; c->nblocks = w.nblocks;
     c->X = (double*)p; p += w.block;  c->AX = (double*)p; p += w.block;
     c->W = (double*)p; p += w.block;  c->AW = (double*)p; p += w.block;
     c->P = (double*)p; p += w.block;  c->AP = (double*)p; p += w.block;
@@ -138,6 +139,7 @@ void moto_destroy(moto_ctx* c) {
 moto_status moto_set_solver(moto_ctx* c, const moto_solver_opts* o) {
     if (!c || !o) return MOTO_EINVAL;
     if (o->guard < 0 || o->check_every < 0 || o->precond_degree < -1 || o->hvp_path < 0 || o->hvp_path > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: negative option");
+    if (o->method < 0 || o->method > 1 || o->ncv < 0 || o->ncv > MOTO_LZ_MAX) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: method must be 0 or 1, ncv in 0..24");
     moto_solver_opts n = *o;
     if (n.check_every == 0) n.check_every = 8;
     if (n.seed == 0) n.seed = 0x9E3779B97F4A7C15ull;

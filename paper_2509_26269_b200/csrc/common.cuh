@@ -9,6 +9,7 @@
 
 #define MOTO_NS MOTO_NSMAX   // 24
 #define MOTO_NUM_SMS 148     // B200
+#define MOTO_LZ_MAX 24       // largest Lanczos basis (the single-CTA Jacobi solves up to MOTO_NS = 24)
 #define MOTO_RED_BLOCKS 296  // CTAs of every grid-reduction kernel (2 per SM): fixed => deterministic sums
 #define MOTO_MAX_NEIGH 160   // Cartesian: neighbour capacity per atom
 #define MOTO_CHEB_MAX 256    // largest degree of the Chebyshev spectral transformation
@@ -22,6 +23,12 @@ struct SolverState {
     double scal[8];                  // scratch scalars: F.v dots, signs ...
     double cheb[MOTO_CHEB_MAX][4];   // per-step {alpha, c0, beta, -} of the Chebyshev recurrence (k_cheb_coef)
     double cheb_ab[4];               // a, b, a_L, scale of the current transformation
+    // ---- thick-restart Lanczos (lanczos.cu)
+    double lz_T[MOTO_LZ_MAX * MOTO_LZ_MAX];   // projected matrix V^T A V: tridiagonal, bordered-diagonal after a restart
+    double lz_Y[MOTO_LZ_MAX * MOTO_KMAX];     // [m][k] Ritz coefficients of the restart
+    double lz_h[MOTO_LZ_MAX + 1];             // Gram-Schmidt coefficients of the current pass
+    double lz_beta, lz_rbeta;                 // ||u|| of the current step and its reciprocal
+    int lz_cycle, lz_pad;                     // index of the last restart cycle whose Rayleigh-Ritz ran
     // ---- tail mirrored to the host (layout == HostStatus)
     double theta[MOTO_KMAX];
     double resid[MOTO_KMAX];
@@ -63,6 +70,8 @@ struct moto_ctx {
     cudaStream_t stream;
     char* ws;
     size_t ws_bytes;
+    size_t block_bytes;   // stride between the [kmax][N][3] blocks X, AX, W, AW, P, AP(, T1, T2)
+    int nblocks;
     // workspace views
     double *X, *AX, *W, *AW, *P, *AP;  // [kmax][N][3] each
     double *T1, *T2;   // [kmax][N][3] ping-pong blocks of the Chebyshev recurrence (spin lattices)
@@ -141,6 +150,9 @@ int fast_cheb_coef_explicit(moto_ctx* c, int d, double a, double b, double aL);
 // rayleigh_ritz.cu
 int rr_solve(moto_ctx*, const double* d_GA, const double* d_GB, int n, int nev, double* d_theta, double* d_C,
              int mode, SolverState* st_or_null);
+// lanczos.cu
+moto_status lanczos_solve(moto_ctx*, const double* d_state, int k, double tol, int max_iter, int warm_start,
+                          moto_solve_info* info);
 // lobpcg.cu
 moto_status lobpcg_solve(moto_ctx*, const double* d_state, int k, double tol, int max_iter, int warm_start,
                          moto_solve_info* info);

@@ -282,6 +282,7 @@ static moto_status lobpcg_solve_generic_filtered(moto_ctx* c, const double* d_st
 
 moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, int max_iter, int warm_start,
                          moto_solve_info* info) {
+    if (c->opts.method == 1) return lanczos_solve(c, d_state, k, tol, max_iter, warm_start, info);
     int kb = k + (c->opts.guard > 0 ? c->opts.guard : 0);
     if (kb > c->kmax) kb = c->kmax;
     const long long dof = (c->kind == MOTO_KIND_TRI2D) ? 2ll * c->N : 3ll * c->N;

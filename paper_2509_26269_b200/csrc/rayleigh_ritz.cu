@@ -396,6 +396,55 @@ __global__ void __launch_bounds__(RR_THREADS_MAX) k_rr(const double* __restrict_
     if (st && tid == 0) { st->nkeep = na; if (bad_s) { st->bad = 1; st->done = 1; } }
 }
 
+// ---- Rayleigh-Ritz step of the thick-restart Lanczos (lanczos.cu): eigen-decomposition of the m x m projected matrix
+// T, the k smallest Ritz values, their coefficient vectors Y = S[:, :k] for the restart, the residual estimates
+// |beta s_{m-1,i}| (Lanczos relation A V = V T + beta v_m e_m^T), the stop test, and the bordered-diagonal T of the
+// restarted basis [x_1 .. x_k, v_m].
+__global__ void __launch_bounds__(RR_THREADS_MAX) k_lz_ritz(SolverState* st, int m, int k, double tol, int cycle) {
+    if (st->done) return;
+    __shared__ double A[NMAX * LD], Z[NMAX * LD], A2[NMAX * LD], Z2[NMAX * LD];
+    __shared__ double rc_s[NMAX + 1], rs_s[NMAX + 1];
+    __shared__ int ord[NMAX];
+    __shared__ JacobiScratch js;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    for (int t = tid; t < m * m; t += nt) {
+        int i = t / m, j = t - i * m;
+        A[i * LD + j] = 0.5 * (st->lz_T[i * MOTO_LZ_MAX + j] + st->lz_T[j * MOTO_LZ_MAX + i]);
+    }
+    __syncthreads();
+    jacobi_eig(A, Z, A2, Z2, m, &js, rc_s, rs_s);
+    if (tid < m) {
+        const double x = A[tid * LD + tid];
+        int rank = 0;
+        for (int b = 0; b < m; ++b) {
+            const double y = A[b * LD + b];
+            if (y < x || (y == x && b < tid) || (!(x == x) && (y == y || b < tid))) ++rank;
+        }
+        ord[rank] = tid;
+    }
+    __syncthreads();
+    const double beta = st->lz_beta;
+    if (tid == 0) {
+        bool ok = true, bad = false;
+        for (int a = 0; a < k; ++a) {
+            const double th = A[ord[a] * LD + ord[a]], r = fabs(beta * Z[(m - 1) * LD + ord[a]]);
+            st->theta[a] = th; st->resid[a] = r;
+            ok = ok && (r <= tol); bad = bad || !(r == r) || !(th == th);
+        }
+        st->lz_cycle = cycle;
+        if (bad) { st->bad = 1; st->done = 1; } else if (ok) st->done = 1;
+    }
+    for (int t = tid; t < m * k; t += nt) { int l = t / k, a = t - l * k; st->lz_Y[t] = Z[l * LD + ord[a]]; }
+    for (int t = tid; t < m * m; t += nt) {
+        int i = t / m, j = t - i * m;
+        double v = 0.0;
+        if (i == j && i < k) v = A[ord[i] * LD + ord[i]];
+        else if (i == k && j < k) v = beta * Z[(m - 1) * LD + ord[j]];
+        else if (j == k && i < k) v = beta * Z[(m - 1) * LD + ord[i]];
+        st->lz_T[i * MOTO_LZ_MAX + j] = v;
+    }
+}
+
 }  // namespace
 
 // block of the launch: 256 threads for n <= 8, one thread per entry (rounded to warps) above
@@ -424,5 +473,11 @@ int rr_solve_fast(moto_ctx* c, int kb, int nblkU, const double* partialsK, int n
     const double tau = 1e-10;
     RRFast fz = {partialsK, nblkK, kb, check, hvp_inc, k, tol};
     k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblkU, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, CHOL_THR, fz);
+    return 1;
+}
+
+// Lanczos flavour (lanczos.cu)
+int lz_ritz(moto_ctx* c, int m, int k, double tol, int cycle) {
+    k_lz_ritz<<<1, rr_threads(m), 0, c->stream>>>(c->st, m, k, tol, cycle);
     return 1;
 }

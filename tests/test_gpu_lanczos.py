@@ -1,0 +1,144 @@
+"""GPU parity tests of the HVP-Lanczos variant (moto_solver_opts.method = 1) against
+oracle/lanczos_oracle.py (same algorithm, same start vector, same basis size) and against the dense oracle."""
+import numpy as np
+import pytest
+import scipy.linalg
+
+from oracle import cart_oracle as co
+from oracle import lanczos_oracle as lo
+from oracle import spin_oracle as so
+from paper_2509_26269_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+EIG_TOL = 1e-8
+ANGLE_TOL = 1e-6
+
+
+def model_of(w):
+    return so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
+
+
+def dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).cuda()
+
+
+def custom(Lx, Ly, px, py, seed, B=(0.01, -0.02, 0.03), k=2):
+    m = wl.random_spins(Lx, Ly, seed)
+    return wl.SpinWorkload(f"rand{Lx}x{Ly}", Lx, Ly, px, py, 1.0, 0.3, 0.05, B, 1.0, k, seed, m)
+
+
+def start_block(w, k, seed):
+    """[k][N][3] with the start vector in column 0 and zeros elsewhere: the library sums the columns."""
+    V0 = np.zeros((k, w.N, 3))
+    V0[0] = wl.random_block(w.N, 1, seed=seed)[0]
+    return V0
+
+
+LZ_CASES = [
+    (lambda: wl.config0(), 2, 2, 1e-9),                 # 8x8, basis 15
+    (lambda: custom(37, 23, 0, 0, 1), 2, 2, 1e-9),      # generic K1 path (odd Lx), open boundaries
+    (lambda: custom(64, 50, 1, 0, 2), 2, 2, 1e-9),      # TMA K1 path, mixed boundaries
+    (lambda: wl.config1(L=40), 3, 3, 1e-9),             # k = 3, basis 23
+    (lambda: wl.config1(L=40), 1, 2, 1e-9),             # k = 1
+]
+
+
+@pytest.mark.parametrize("case", range(len(LZ_CASES)))
+def test_lanczos_matches_its_oracle_step_for_step(moto, case):
+    mk, k, kmax, tol = LZ_CASES[case]
+    w = mk()
+    m = min(24, 8 * kmax - 1)
+    V0 = start_block(w, k, seed=11 + case)
+    theta_o, V_o, info_o = lo.lowest_modes_lanczos(model_of(w), w.spins, k, V0[0], m, tol)
+    assert info_o["converged"]
+    ctx = moto.spin_context(w, kmax=kmax)
+    ctx.set_solver(method=1)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), k, tol=tol, max_iter=100000, V0=dev(V0))
+    assert info["converged"], info
+    # same algorithm, same start, same basis size: the number of Lanczos steps agrees (restart cycles are discrete)
+    assert info["iters"] == info_o["steps"], (info["iters"], info_o["steps"])
+    lam = lam.cpu().numpy(); V = V.cpu().numpy()
+    assert np.max(np.abs(lam - theta_o) / np.maximum(np.abs(theta_o), 1e-3)) <= EIG_TOL
+    ang = scipy.linalg.subspace_angles(V.reshape(k, -1).T, V_o.reshape(k, -1).T)
+    assert ang.max() <= ANGLE_TOL
+    # reported residuals are the true ones and meet the tolerance; oracle-side residual of the GPU pairs
+    assert max(info["resid"]) <= tol * (1 + 1e-6) + 1e-13
+    HV = so.hvp(model_of(w), w.spins, V)
+    for a in range(k):
+        assert abs(np.linalg.norm(HV[a] - lam[a] * V[a]) - info["resid"][a]) <= 1e-12 + 1e-3 * tol
+    # and against the dense eigendecomposition
+    lam_ref, V_ref = so.lowest_modes(model_of(w), w.spins, k, extra=1)
+    assert np.max(np.abs(lam - lam_ref[:k]) / np.maximum(np.abs(lam_ref[:k]), 1e-3)) <= EIG_TOL
+    assert scipy.linalg.subspace_angles(V.reshape(k, -1).T, V_ref[:k].reshape(k, -1).T).max() <= ANGLE_TOL
+    assert np.max(np.abs(V.reshape(k, -1) @ V.reshape(k, -1).T - np.eye(k))) <= 1e-10
+    assert np.max(np.abs(np.sum(V * w.spins[None], axis=2))) <= 1e-10
+
+
+def test_lanczos_cold_start_cfg1_and_agreement_with_lobpcg(moto):
+    w = wl.config1()
+    ctx = moto.spin_context(w)
+    lam_b, V_b, info_b = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=5000)
+    ctx.set_solver(method=1)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=100000)
+    assert info["converged"] and info_b["converged"]
+    assert np.max(np.abs((lam - lam_b).cpu().numpy())) <= 1e-9
+    ang = scipy.linalg.subspace_angles(V.cpu().numpy().reshape(2, -1).T, V_b.cpu().numpy().reshape(2, -1).T)
+    assert ang.max() <= ANGLE_TOL
+    assert info["hvp_count"] == info["iters"] + 2
+    # smaller basis on request
+    ctx.set_solver(method=1, ncv=8)
+    lam8, V8, info8 = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=100000)
+    assert info8["converged"] and np.max(np.abs((lam8 - lam_b).cpu().numpy())) <= 1e-9
+    assert (info8["iters"] - 8) % 6 == 0          # 8 steps, then cycles of ncv - k
+
+
+def test_lanczos_cap_and_errors(moto):
+    w = wl.config1(L=40)
+    ctx = moto.spin_context(w)
+    ctx.set_solver(method=1)
+    with pytest.raises(moto.MotoError) as e:
+        ctx.lowest_modes(dev(w.spins), 2, tol=1e-13, max_iter=20)
+    assert e.value.status == moto.ENOTCONV
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-13, max_iter=20, allow_notconv=True)
+    assert not info["converged"] and info["iters"] == 15 + 13 and np.isfinite(lam.cpu().numpy()).all()
+    assert np.isfinite(info["resid"]).all() and max(info["resid"]) > 1e-13
+    with pytest.raises(moto.MotoError):
+        ctx.set_solver(method=2)
+    with pytest.raises(moto.MotoError):
+        ctx.set_solver(method=1, ncv=25)
+    ctx.set_solver(method=1, ncv=3)               # needs k + 2 <= ncv
+    with pytest.raises(moto.MotoError) as e:
+        ctx.lowest_modes(dev(w.spins), 2, tol=1e-8, max_iter=100)
+    assert e.value.status == moto.EINVAL
+    # a single spin has two degrees of freedom: no room for a Krylov basis
+    w1 = custom(1, 1, 0, 0, 4)
+    c1 = moto.spin_context(w1)
+    c1.set_solver(method=1)
+    with pytest.raises(moto.MotoError):
+        c1.lowest_modes(dev(w1.spins), 1, tol=1e-8, max_iter=10)
+
+
+def test_lanczos_cartesian(moto):
+    w = wl.config4()
+    mdl = co.MorseModel(w.cell, w.De, w.alpha, w.r0, w.rc, fixed=w.fixed)
+    lam_ref, V_ref = co.lowest_modes(mdl, w.positions, 2)
+    ctx = moto.cart_context(w)
+    ctx.set_solver(method=1)
+    lam, V, info = ctx.lowest_modes(dev(w.positions), 2, tol=1e-8, max_iter=200000)
+    assert info["converged"], info
+    lam = lam.cpu().numpy(); V = V.cpu().numpy()
+    assert np.max(np.abs(lam - lam_ref[:2]) / np.maximum(np.abs(lam_ref[:2]), 1e-3)) <= EIG_TOL
+    assert scipy.linalg.subspace_angles(V.reshape(2, -1).T, V_ref[:2].reshape(2, -1).T).max() <= ANGLE_TOL
+    assert np.max(np.abs(V[:, w.fixed.astype(bool)])) == 0.0
+
+
+def test_lanczos_deterministic(moto):
+    w = wl.config1(L=40)
+    ctx = moto.spin_context(w)
+    ctx.set_solver(method=1)
+    a = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=100000)
+    b = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=100000)
+    assert a[2]["iters"] == b[2]["iters"]
+    assert np.array_equal(a[0].cpu().numpy(), b[0].cpu().numpy()) and np.array_equal(a[1].cpu().numpy(), b[1].cpu().numpy())
