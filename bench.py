@@ -168,7 +168,7 @@ def run_report(args):
         torch.cuda.synchronize()
         return ev0.elapsed_time(ev1) / reps
 
-    rows, orows = [], []
+    rows, orows, lrows = [], [], []
     cfgs = [("0", wl.config0(), 0), ("1", wl.config1(), 0), ("2", wl.config2(), 100), ("3", wl.config3(), 200), ("4", wl.config4(), 100)]
     # the paper's own Fig. 2 workload class: a random spin configuration at 10^6 spins, same J, D, K, B
     rnd = wl.random_spins(1000, 1000, 7)
@@ -192,6 +192,17 @@ def run_report(args):
         lam, Vm, info = ctx.lowest_modes(x, w.k, tol=tol, max_iter=20000, allow_notconv=True)
         ev1.record(); torch.cuda.synchronize()
         solve_ms = ev0.elapsed_time(ev1)
+        # the Lanczos variant on the same input (moto_solver_opts.method = 1; plain operator, cap 20000 steps)
+        ctx.set_solver(method=1)
+        ctx.lowest_modes(x, w.k, tol=tol, max_iter=20000, allow_notconv=True)
+        torch.cuda.synchronize()
+        ev0.record()
+        lam_z, _, info_z = ctx.lowest_modes(x, w.k, tol=tol, max_iter=20000, allow_notconv=True)
+        ev1.record(); torch.cuda.synchronize()
+        lrows.append(f"| {name} | {N} | {w.k} | {min(24, (6 if cart else 8) * ctx.kmax - 1)} | {ev0.elapsed_time(ev1):.2f} | {info_z['iters']} | "
+                     f"{'yes' if info_z['converged'] else 'no (cap)'} | {max(info_z['resid']):.1e} | "
+                     f"{np.max(np.abs((lam_z - lam).cpu().numpy())):.1e} |")
+        ctx.set_solver(guard=2) if (cart and w.k + 2 <= ctx.kmax) else ctx.set_solver()
         # MMF loop: re-solve (warm start, transported block) -> energy/gradient -> reflected step along v1
         mmf = ""
         if nsteps:
@@ -241,6 +252,10 @@ def run_report(args):
     print("| cfg | N | k | moto_hvp µs | HVP/s | Gsite-updates/s | HVP GB/s (algorithmic 24N(1+2k)) | lowest-k solve ms | iters | HVPs | max resid | peak incremental MB | MMF loop |")
     print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
     print("\n".join(rows))
+    print("\nHVP-Lanczos variant (`moto_solver_opts.method = 1`: thick-restart, full re-orthogonalisation, plain operator; PAPER.md:84):\n")
+    print("| cfg | N | k | basis m | solve ms | Lanczos steps (= HVPs) | converged | max true resid | max abs(lambda - LOBPCG's) |")
+    print("|---|---|---|---|---|---|---|---|---|")
+    print("\n".join(lrows))
     if orows:
         print(f"\nOracle on the host ({cores} BLAS threads, {os.cpu_count()} CPUs), as it stands — a baseline, not the target:\n")
         print("| cfg | oracle HVP ms (explicit Hessian rebuilt) | oracle lowest-k s | how | max rel. eigenvalue difference GPU vs oracle |")

@@ -28,22 +28,26 @@ struct LzBasis {
     __host__ __device__ double* vec(int i) const { return base + (size_t)(i / kmax) * block_stride + (size_t)(i % kmax) * (size_t)n3; }
 };
 
-// partials[blk][i] = sum over this CTA's elements of v_i[e] u[e] (i <= j), partials[blk][LZ_NRM] = sum u[e]^2;  u = v_{j+1}
-__global__ void __launch_bounds__(LZ_THREADS) k_lz_dots(LzBasis B, int j, double* __restrict__ partials, const int* __restrict__ stop) {
-    if (*stop) return;
-    const double* vp[MOTO_LZ_MAX];
+constexpr int LZ_U = 4;          // flat elements per thread per trip (independent loads in flight)
+
+// acc[i] += v_i[e] * ue for the LZ_U elements of this trip (i <= j); the i-loop is unrolled so acc stays in registers
+__device__ __forceinline__ void lz_dot_trip(const LzBasis& B, int j, long long e0, long long stride, const double (&ue)[LZ_U],
+                                            double (&acc)[MOTO_LZ_MAX]) {
 #pragma unroll
-    for (int i = 0; i < MOTO_LZ_MAX; ++i) vp[i] = (i <= j) ? B.vec(i) : nullptr;
-    const double* u = B.vec(j + 1);
-    double acc[MOTO_LZ_MAX], an = 0.0;
+    for (int i = 0; i < MOTO_LZ_MAX; ++i) {
+        if (i <= j) {
+            const double* p = B.vec(i);
+            double v[LZ_U];
 #pragma unroll
-    for (int i = 0; i < MOTO_LZ_MAX; ++i) acc[i] = 0.0;
-    for (long long e = blockIdx.x * (long long)LZ_THREADS + threadIdx.x; e < B.n3; e += (long long)gridDim.x * LZ_THREADS) {
-        const double ue = u[e];
-        an = fma(ue, ue, an);
+            for (int u = 0; u < LZ_U; ++u) { const long long e = e0 + u * stride; v[u] = (e < B.n3) ? p[e] : 0.0; }
 #pragma unroll
-        for (int i = 0; i < MOTO_LZ_MAX; ++i) if (i <= j) acc[i] = fma(vp[i][e], ue, acc[i]);
+            for (int u = 0; u < LZ_U; ++u) acc[i] = fma(v[u], ue[u], acc[i]);
+        }
     }
+}
+
+// CTA sums of acc[0..j] and an -> partials[blk][0..j], partials[blk][MOTO_LZ_MAX]
+__device__ __forceinline__ void lz_block_sums(int j, const double (&acc)[MOTO_LZ_MAX], double an, double* __restrict__ partials) {
     __shared__ double red[LZ_THREADS / 32][MOTO_LZ_MAX + 1];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
@@ -68,61 +72,58 @@ __global__ void __launch_bounds__(LZ_THREADS) k_lz_dots(LzBasis B, int j, double
     }
 }
 
+// partials[blk][i] = sum over this CTA's elements of v_i[e] u[e] (i <= j), partials[blk][MOTO_LZ_MAX] = sum u[e]^2;  u = v_{j+1}
+__global__ void __launch_bounds__(LZ_THREADS) k_lz_dots(LzBasis B, int j, double* __restrict__ partials, const int* __restrict__ stop) {
+    if (*stop) return;
+    const double* u = B.vec(j + 1);
+    double acc[MOTO_LZ_MAX], an = 0.0;
+#pragma unroll
+    for (int i = 0; i < MOTO_LZ_MAX; ++i) acc[i] = 0.0;
+    const long long stride = (long long)gridDim.x * LZ_THREADS;
+    for (long long e0 = blockIdx.x * (long long)LZ_THREADS + threadIdx.x; e0 < B.n3; e0 += LZ_U * stride) {
+        double ue[LZ_U];
+#pragma unroll
+        for (int t = 0; t < LZ_U; ++t) { const long long e = e0 + t * stride; ue[t] = (e < B.n3) ? u[e] : 0.0; an = fma(ue[t], ue[t], an); }
+        lz_dot_trip(B, j, e0, stride, ue, acc);
+    }
+    lz_block_sums(j, acc, an, partials);
+}
+
 // pass 1: u <- u - V h and partials of V^T u, ||u||^2 of the updated u;   pass 2: v_{j+1} = (u - V h) * (1 / beta)
 template <int PASS>
 __global__ void __launch_bounds__(LZ_THREADS) k_lz_upd(LzBasis B, int j, SolverState* st, double* __restrict__ partials) {
     if (st->done) return;
-    const double* vp[MOTO_LZ_MAX];
     __shared__ double h[MOTO_LZ_MAX];
     if (threadIdx.x < MOTO_LZ_MAX) h[threadIdx.x] = (threadIdx.x <= j) ? st->lz_h[threadIdx.x] : 0.0;
     __syncthreads();
-#pragma unroll
-    for (int i = 0; i < MOTO_LZ_MAX; ++i) vp[i] = (i <= j) ? B.vec(i) : nullptr;
     double* u = B.vec(j + 1);
     const double scale = (PASS == 2) ? st->lz_rbeta : 1.0;
     double acc[MOTO_LZ_MAX], an = 0.0;
 #pragma unroll
     for (int i = 0; i < MOTO_LZ_MAX; ++i) acc[i] = 0.0;
-    for (long long e = blockIdx.x * (long long)LZ_THREADS + threadIdx.x; e < B.n3; e += (long long)gridDim.x * LZ_THREADS) {
-        double ue = u[e];
-        double v[MOTO_LZ_MAX];
+    const long long stride = (long long)gridDim.x * LZ_THREADS;
+    for (long long e0 = blockIdx.x * (long long)LZ_THREADS + threadIdx.x; e0 < B.n3; e0 += LZ_U * stride) {
+        double ue[LZ_U];
 #pragma unroll
-        for (int i = 0; i < MOTO_LZ_MAX; ++i) v[i] = (i <= j) ? vp[i][e] : 0.0;
+        for (int t = 0; t < LZ_U; ++t) { const long long e = e0 + t * stride; ue[t] = (e < B.n3) ? u[e] : 0.0; }
+        for (int i = 0; i <= j; ++i) {          // runtime loop: LZ_U independent loads per basis vector
+            const double* p = B.vec(i);
+            const double hi = h[i];
+            double v[LZ_U];
 #pragma unroll
-        for (int i = 0; i < MOTO_LZ_MAX; ++i) if (i <= j) ue = fma(-h[i], v[i], ue);
+            for (int t = 0; t < LZ_U; ++t) { const long long e = e0 + t * stride; v[t] = (e < B.n3) ? p[e] : 0.0; }
+#pragma unroll
+            for (int t = 0; t < LZ_U; ++t) ue[t] = fma(-hi, v[t], ue[t]);
+        }
+#pragma unroll
+        for (int t = 0; t < LZ_U; ++t) { const long long e = e0 + t * stride; if (e < B.n3) u[e] = ue[t] * scale; }
         if (PASS == 1) {
-            u[e] = ue;
-            an = fma(ue, ue, an);
 #pragma unroll
-            for (int i = 0; i < MOTO_LZ_MAX; ++i) if (i <= j) acc[i] = fma(v[i], ue, acc[i]);
-        } else {
-            u[e] = ue * scale;
+            for (int t = 0; t < LZ_U; ++t) an = fma(ue[t], ue[t], an);
+            lz_dot_trip(B, j, e0, stride, ue, acc);      // second read of the basis at these elements (cache-resident)
         }
     }
-    if (PASS == 1) {
-        __shared__ double red[LZ_THREADS / 32][MOTO_LZ_MAX + 1];
-        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-        for (int i = 0; i < MOTO_LZ_MAX; ++i) {
-            if (i <= j) {
-                double s = acc[i];
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-                if (lane == 0) red[warp][i] = s;
-            }
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) an += __shfl_xor_sync(0xffffffffu, an, o);
-        if (lane == 0) red[warp][MOTO_LZ_MAX] = an;
-        __syncthreads();
-        const int t = threadIdx.x;
-        if (t <= j || t == MOTO_LZ_MAX) {
-            double s = 0.0;
-#pragma unroll
-            for (int w = 0; w < LZ_THREADS / 32; ++w) s += red[w][t];
-            partials[(size_t)blockIdx.x * (MOTO_LZ_MAX + 1) + t] = s;
-        }
-    }
+    if (PASS == 1) lz_block_sums(j, acc, an, partials);
 }
 
 // One CTA, one warp per entry: sums the CTA partials in a fixed order and does the scalar bookkeeping of the step.
