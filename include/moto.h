@@ -149,6 +149,33 @@ typedef struct {
 moto_status moto_mmf_run(moto_ctx* ctx, double* d_state, int k, double dt, int max_steps, double tau_F, double tol, int max_iter,
                          int warm_start, double* d_V, moto_mmf_info* info);
 
+/* Two-sided minimum-mode descent (Alg. 1 l.15-18; Suppl. Note 1 b(iii)).
+ * moto_relax: "RelaxDownHill" with a deterministic optimiser.  The paper names the class ("L-BFGS/CG") and nothing else;
+ *   this is Riemannian Polak-Ribiere+ conjugate gradients with backtracking (reading A25):
+ *     trial x_t = R(x + a d), a = alpha, alpha/2, ... (<= 40);  accepted when g_t.d <= 0.5 |g.d| and
+ *     (E_t <= E + 1e-4 a g.d  or  E_t <= E + 1e-10 |E|);  beta = max(0, (g_t.g_t - g_t.g)/(g.g));
+ *     d <- -g_t + beta T(d) (T = tangent projection at x_t for spins, identity for atoms; reset to -g_t if not a descent
+ *     direction);  alpha <- 2a if the first trial was accepted, else a.  g = tangent-projected / masked gradient.
+ *   d_state [N][3] in/out (unit spins / positions).  Stops when ||g||_2 <= tau_F (MOTO_OK, converged = 1), after
+ *   max_steps accepted steps or when no step along -g is acceptable (MOTO_ENOTCONV; d_state = best iterate, info valid).
+ *   alpha0 > 0: first trial step.  Synchronises the stream once per trial (four scalars come back).  Uses the solver
+ *   blocks of the workspace as scratch: modes left there by an earlier solve are overwritten (user arrays are not).
+ * moto_two_sided_descent: seeds x_saddle + s eta v_min, s = +1 then -1 (retracted for spins), each relaxed as above into
+ *   d_min_plus / d_min_minus [N][3] (must not alias the inputs or each other); info[2] (host, may be NULL) in that order.
+ *   Returns MOTO_ENOTCONV if either branch did not converge (both outputs valid). */
+typedef struct {
+    int32_t steps;       /* accepted steps */
+    int32_t converged;   /* 1: ||g|| <= tau_F at the returned state */
+    int32_t evals;       /* energy + gradient evaluations (one per trial, plus the first) */
+    int32_t pad_;
+    double energy;       /* E at the returned state */
+    double gnorm;        /* ||g||_2 at the returned state */
+    double alpha;        /* trial step the next iteration would start from */
+} moto_relax_info;
+moto_status moto_relax(moto_ctx* ctx, double* d_state, int max_steps, double tau_F, double alpha0, moto_relax_info* info);
+moto_status moto_two_sided_descent(moto_ctx* ctx, const double* d_saddle, const double* d_vmin, double eta, int max_steps,
+                                   double tau_F, double alpha0, double* d_min_plus, double* d_min_minus, moto_relax_info* info);
+
 /* Vector transport for warm starts after m -> m' (reading A17): V <- orthonormalise(P_{m'} V), in place. */
 moto_status moto_transport(moto_ctx* ctx, const double* d_spins_new, double* d_V, int k);
 

@@ -50,6 +50,15 @@ class MmfInfo(C.Structure):
                 ("hvp_count", C.c_int64), ("solver_iters", C.c_int64)]
 
 
+class RelaxInfo(C.Structure):
+    _fields_ = [("steps", C.c_int32), ("converged", C.c_int32), ("evals", C.c_int32), ("pad_", C.c_int32),
+                ("energy", C.c_double), ("gnorm", C.c_double), ("alpha", C.c_double)]
+
+    def as_dict(self, status=0):
+        return dict(steps=self.steps, converged=bool(self.converged), evals=self.evals, energy=self.energy, gnorm=self.gnorm,
+                    alpha=self.alpha, status=status)
+
+
 class SolveInfo(C.Structure):
     _fields_ = [("iters", C.c_int32), ("converged", C.c_int32), ("resid", C.c_double * KMAX), ("hvp_count", C.c_int64)]
 
@@ -72,6 +81,9 @@ _SIGS = {
     "moto_cheb_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_int]),
     "moto_mmf_run": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
                                C.c_void_p, C.POINTER(MmfInfo)]),
+    "moto_relax": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double, C.POINTER(RelaxInfo)]),
+    "moto_two_sided_descent": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_double, C.c_double,
+                                         C.c_void_p, C.c_void_p, C.POINTER(RelaxInfo)]),
     "moto_transport": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "moto_gram": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
     "moto_rayleigh_ritz": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
@@ -265,6 +277,24 @@ class Context:
                                                int(max_iter), warm, _ptr(V), C.byref(info)), allow=(ENOTCONV,))
         return V, dict(steps=info.steps, converged=bool(info.converged), fnorm=info.fnorm, lam=list(info.lam)[:k],
                        hvp_count=info.hvp_count, solver_iters=info.solver_iters, status=st)
+
+    def relax(self, state, max_steps, tau_F, alpha0):
+        """moto_relax: relax `state` downhill in place (CG + backtracking).  -> info dict."""
+        _dev_f64(state, (self.N, 3))
+        info = RelaxInfo()
+        st = self._check(self.lib.moto_relax(self._h, _ptr(state), int(max_steps), float(tau_F), float(alpha0), C.byref(info)),
+                         allow=(ENOTCONV,))
+        return info.as_dict(st)
+
+    def two_sided_descent(self, saddle, vmin, eta, max_steps, tau_F, alpha0):
+        """moto_two_sided_descent -> (x_min(+eta), x_min(-eta), [info dict, info dict])."""
+        _dev_f64(saddle, (self.N, 3))
+        _dev_f64(vmin, (self.N, 3))
+        xp, xm = self._empty(self.N, 3), self._empty(self.N, 3)
+        info = (RelaxInfo * 2)()
+        st = self._check(self.lib.moto_two_sided_descent(self._h, _ptr(saddle), _ptr(vmin), float(eta), int(max_steps), float(tau_F),
+                                                         float(alpha0), _ptr(xp), _ptr(xm), info), allow=(ENOTCONV,))
+        return xp, xm, [info[0].as_dict(st), info[1].as_dict(st)]
 
     def transport(self, spins_new, V):
         k = V.shape[0]

@@ -253,6 +253,32 @@ moto_status moto_mmf_run(moto_ctx* c, double* d_state, int k, double dt, int max
     return st;
 }
 
+moto_status moto_relax(moto_ctx* c, double* d_state, int max_steps, double tau_F, double alpha0, moto_relax_info* info) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_state) return moto_fail(c, MOTO_EINVAL, "moto_relax: null argument");
+    if (max_steps < 0 || !(tau_F >= 0) || !(alpha0 > 0)) return moto_fail(c, MOTO_EINVAL, "moto_relax: need max_steps >= 0, tau_F >= 0, alpha0 > 0");
+    return relax_run(c, d_state, max_steps, tau_F, alpha0, info);
+}
+
+moto_status moto_two_sided_descent(moto_ctx* c, const double* d_saddle, const double* d_vmin, double eta, int max_steps, double tau_F,
+                                   double alpha0, double* d_min_plus, double* d_min_minus, moto_relax_info* info) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_saddle || !d_vmin || !d_min_plus || !d_min_minus) return moto_fail(c, MOTO_EINVAL, "moto_two_sided_descent: null argument");
+    if (d_min_plus == d_min_minus || d_min_plus == d_saddle || d_min_minus == d_saddle || d_min_plus == d_vmin || d_min_minus == d_vmin)
+        return moto_fail(c, MOTO_EINVAL, "moto_two_sided_descent: outputs must not alias the inputs or each other");
+    if (max_steps < 0 || !(tau_F >= 0) || !(alpha0 > 0) || !(eta == eta)) return moto_fail(c, MOTO_EINVAL, "moto_two_sided_descent: need max_steps >= 0, tau_F >= 0, alpha0 > 0");
+    moto_status worst = MOTO_OK;
+    for (int b = 0; b < 2; ++b) {
+        double* out = b == 0 ? d_min_plus : d_min_minus;
+        moto_status s = relax_seed(c, d_saddle, d_vmin, b == 0 ? eta : -eta, out);   // Alg. 1 l.16
+        if (s != MOTO_OK) return s;
+        s = relax_run(c, out, max_steps, tau_F, alpha0, info ? info + b : nullptr);   // Alg. 1 l.17
+        if (s != MOTO_OK && s != MOTO_ENOTCONV) return s;
+        if (s == MOTO_ENOTCONV) worst = s;
+    }
+    return worst;
+}
+
 moto_status moto_transport(moto_ctx* c, const double* d_spins_new, double* d_V, int k) {
     if (!c) return MOTO_EINVAL;
     if (!d_spins_new || !d_V || k < 1 || k > MOTO_KMAX) return moto_fail(c, MOTO_EINVAL, "moto_transport: bad argument");

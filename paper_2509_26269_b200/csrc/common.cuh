@@ -153,6 +153,9 @@ int rr_solve(moto_ctx*, const double* d_GA, const double* d_GB, int n, int nev, 
 // lanczos.cu
 moto_status lanczos_solve(moto_ctx*, const double* d_state, int k, double tol, int max_iter, int warm_start,
                           moto_solve_info* info);
+// relax.cu
+moto_status relax_run(moto_ctx*, double* d_state, int max_steps, double tau_F, double alpha0, moto_relax_info* info);
+moto_status relax_seed(moto_ctx*, const double* d_saddle, const double* d_v, double s_eta, double* d_out);
 // lobpcg.cu
 moto_status lobpcg_solve(moto_ctx*, const double* d_state, int k, double tol, int max_iter, int warm_start,
                          moto_solve_info* info);

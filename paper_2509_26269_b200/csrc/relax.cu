@@ -1,0 +1,138 @@
+// relax.cu -- two-sided minimum-mode descent (Alg. 1 l.15-18; Suppl. Note 1 b(iii), PAPER.md:307;
+// SURVEY 8(f) f2): seeds x_saddle +- eta v_min, each relaxed downhill "using a deterministic optimizer (e.g., L-BFGS/CG)".
+// The paper gives no more than that; the optimiser is reading A25 of DESIGN.md: Riemannian Polak-Ribiere+ conjugate
+// gradients with backtracking,
+//   trial x_t = R(x + a d), a = alpha, alpha/2, ...;  accept if g_t.d <= SIGMA |g.d| and (Armijo or E_t <= E + EPS_E |E|)
+//   beta = max(0, (g_t.g_t - g_t.g)/(g.g));  d <- -g_t + beta T(d)  (T = tangent projection at x_t / identity for atoms)
+//   alpha <- 2a if the first trial was accepted else a;  stop at |g| <= tau_F.
+// Every vector operation runs here (energy + gradient through the K1/K7 kernels, the three dots of a trial in one Gram
+// launch, trial state and direction update in two streaming kernels); the host sees four scalars per trial
+// (E_t, g_t.g_t, g_t.g, g_t.d) and takes the accept/reject decision.
+#include "common.cuh"
+#include "device_utils.cuh"
+
+#define RELAX_C1 1e-4
+#define RELAX_EPS_E 1e-10
+#define RELAX_SIGMA 0.5
+#define RELAX_MAX_BACKTRACKS 40
+
+namespace {
+
+// x_t = R(x + a d): per-site renormalisation for spins (A7), identity for atoms (d is zero on fixed atoms)
+__global__ void __launch_bounds__(256) k_relax_trial(long long N, const double* __restrict__ x, const double* __restrict__ d, double a,
+                                                     double* __restrict__ xt, int retract) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        d3 y = axpy3(a, ld3(d, i), ld3(x, i));
+        if (retract) y = scale3(1.0 / sqrt(dot3(y, y)), y);
+        st3(xt, i, y);
+    }
+}
+
+// d <- -g_t + beta T(d)
+__global__ void __launch_bounds__(256) k_relax_dir(long long N, const double* __restrict__ xt, const double* __restrict__ gt, double beta,
+                                                   double* __restrict__ d, int project) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        d3 di = mk3(0.0, 0.0, 0.0);
+        if (beta != 0.0) {                       // beta == 0: d may be uninitialised, never read it
+            di = ld3(d, i);
+            if (project) di = proj3(ld3(xt, i), di);
+        }
+        d3 g = ld3(gt, i);
+        st3(d, i, mk3(fma(beta, di.x, -g.x), fma(beta, di.y, -g.y), fma(beta, di.z, -g.z)));
+    }
+}
+
+int grid_for(long long N) {
+    long long b = (N + 255) / 256;
+    return (int)(b < 4 * MOTO_NUM_SMS ? (b > 0 ? b : 1) : 4 * MOTO_NUM_SMS);
+}
+
+// E and gradient at x, then the dots of g_new with [g_new, g_old, d]; four scalars to the host, one synchronisation
+moto_status eval_point(moto_ctx* c, const double* x, double* g_new, const double* g_old, const double* d, double* h4) {
+    double* dE = c->st->scal;          // [0] E, [1..3] dots
+    moto_status s = moto_energy_grad(c, x, dE, g_new);
+    if (s != MOTO_OK) return s;
+    const double* S[1] = {g_new};
+    const double* T[3] = {g_new, g_old ? g_old : g_new, d ? d : g_new};
+    c->launches += block_gram(c, S, 1, T, 3, dE + 1, nullptr);
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h4, dE, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (c->kind == MOTO_KIND_CARTESIAN) {
+        int ov = 0;
+        MOTO_CUDA_CHECK(c, cudaMemcpy(&ov, c->cl.overflow, sizeof(int), cudaMemcpyDeviceToHost));
+        if (ov) return moto_fail(c, MOTO_ENOMEM, "neighbour capacity MOTO_MAX_NEIGH exceeded");
+    }
+    return MOTO_OK;
+}
+
+}  // namespace
+
+// d_state in/out.  Scratch: g = ctx->g, g_t = W, d = AW, x_t = stage_m (no solver is running).
+moto_status relax_run(moto_ctx* c, double* d_state, int max_steps, double tau_F, double alpha0, moto_relax_info* info) {
+    const long long N = c->N;
+    const size_t vb = (size_t)N * 3 * sizeof(double);
+    const int spin = c->kind == MOTO_KIND_TRI2D;
+    const int grid = grid_for(N);
+    double *g = c->g, *gt = c->W, *d = c->AW, *xt = c->stage_m;
+    moto_relax_info out; memset(&out, 0, sizeof(out));
+    double h[4];
+    moto_status s = eval_point(c, d_state, g, nullptr, nullptr, h);
+    if (s != MOTO_OK) return s;
+    out.evals = 1;
+    double E = h[0], gg = h[1], slope = -gg, alpha = alpha0;
+    k_relax_dir<<<grid, 256, 0, c->stream>>>(N, d_state, g, 0.0, d, 0);   // d = -g (beta = 0: the old d is not read into the result)
+    c->launches += 1;
+    bool steepest = true;
+    moto_status ret = MOTO_OK;
+    for (;;) {
+        if (!(gg == gg)) { ret = moto_fail(c, MOTO_ESTATE, "moto_relax: NaN gradient"); break; }
+        if (sqrt(gg) <= tau_F) { out.converged = 1; break; }
+        if (out.steps >= max_steps) { ret = moto_fail(c, MOTO_ENOTCONV, "moto_relax: max_steps reached"); break; }
+        double a = alpha;
+        bool accepted = false, first = true;
+        for (int bt = 0; bt < RELAX_MAX_BACKTRACKS; ++bt) {
+            k_relax_trial<<<grid, 256, 0, c->stream>>>(N, d_state, d, a, xt, spin);
+            c->launches += 1;
+            s = eval_point(c, xt, gt, g, d, h);
+            if (s != MOTO_OK) return s;
+            out.evals += 1;
+            const double Et = h[0], gtd = h[3];
+            if (gtd <= RELAX_SIGMA * fabs(slope) && (Et <= E + RELAX_C1 * a * slope || Et <= E + RELAX_EPS_E * fabs(E))) { accepted = true; break; }
+            a *= 0.5;
+            first = false;
+        }
+        if (!accepted) {
+            if (steepest) { ret = moto_fail(c, MOTO_ENOTCONV, "moto_relax: stalled (no acceptable step along -g)"); break; }
+            k_relax_dir<<<grid, 256, 0, c->stream>>>(N, d_state, g, 0.0, d, 0);
+            c->launches += 1;
+            slope = -gg; steepest = true;
+            continue;
+        }
+        const double Et = h[0], gtgt = h[1], gtg = h[2], gtd = h[3];
+        double beta = (gtgt - gtg) / gg;
+        if (!(beta > 0.0)) beta = 0.0;
+        double new_slope = -gtgt + beta * gtd;
+        if (new_slope >= 0.0) { beta = 0.0; new_slope = -gtgt; }
+        k_relax_dir<<<grid, 256, 0, c->stream>>>(N, xt, gt, beta, d, spin);
+        c->launches += 1;
+        steepest = beta == 0.0;
+        MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_state, xt, vb, cudaMemcpyDeviceToDevice, c->stream));
+        double* t = g; g = gt; gt = t;
+        E = Et; gg = gtgt; slope = new_slope;
+        alpha = first ? 2.0 * a : a;
+        out.steps += 1;
+    }
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    out.energy = E; out.gnorm = sqrt(gg); out.alpha = alpha;
+    if (info) *info = out;
+    return ret;
+}
+
+moto_status relax_seed(moto_ctx* c, const double* d_saddle, const double* d_v, double s_eta, double* d_out) {
+    k_relax_trial<<<grid_for(c->N), 256, 0, c->stream>>>((long long)c->N, d_saddle, d_v, s_eta, d_out, c->kind == MOTO_KIND_TRI2D);
+    c->launches += 1;
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return MOTO_OK;
+}

@@ -57,6 +57,7 @@ def test_struct_sizes_match_header():
     assert C.sizeof(b.SolveInfo) == 8 + 8 * b.KMAX + 8
     assert C.sizeof(b.SolverOpts) == 16 + 16 + 8 + 8   # + method, ncv
     assert C.sizeof(b.Lattice) == 24 + 32 + 8
+    assert C.sizeof(b.RelaxInfo) == 16 + 24
 
 
 def test_product_path_does_not_import_oracle():

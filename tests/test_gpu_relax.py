@@ -1,0 +1,158 @@
+"""GPU parity tests of moto_relax / moto_two_sided_descent (Alg. 1 l.15-18) against
+oracle/relax_oracle.py: the first steps of the trajectory (decisions far above rounding) step for step, the end points
+(minima are attractors, so they agree to the gradient tolerance over the curvature), closed forms, error paths."""
+import numpy as np
+import pytest
+
+from oracle import cart_oracle as co
+from oracle import relax_oracle as ro
+from oracle import spin_oracle as so
+from paper_2509_26269_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def spin_model(w):
+    return so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
+
+
+def cart_model(w):
+    return co.MorseModel(w.cell, w.De, w.alpha, w.r0, w.rc, w.fixed)
+
+
+def dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).cuda()
+
+
+@pytest.mark.parametrize("steps", [1, 2, 5, 12])
+def test_first_steps_match_oracle_spins(moto, steps):
+    # same start, same number of accepted steps: state, energy, |g|, evaluation count and next alpha agree to rounding
+    w = wl.config1(L=14, R=3.0)          # TMA-ineligible size -> generic K1; 70x70 below takes the TMA path
+    mdl = spin_model(w)
+    ref, iref = ro.relax_downhill(*ro.spin_ops(mdl), w.spins, steps, 0.0, 0.05)
+    ctx = moto.spin_context(w, kmax=2)
+    x = dev(w.spins)
+    info = ctx.relax(x, steps, 0.0, 0.05)
+    assert info["steps"] == iref["steps"] == steps and not info["converged"] and info["status"] == moto.binding.ENOTCONV
+    assert info["evals"] == iref["evals"] and info["alpha"] == iref["alpha"]
+    assert abs(info["energy"] - iref["energy"]) <= 1e-12 * abs(iref["energy"])
+    assert abs(info["gnorm"] - iref["gnorm"]) <= 1e-10 * iref["gnorm"]
+    assert np.max(np.abs(x.cpu().numpy() - ref)) <= 1e-11
+
+
+def test_relax_skyrmion_end_point(moto):
+    # 40x40 skyrmion + noise (configs[1] recipe, TMA K1 path): both sides reach the same minimum.  The relaxed skyrmion has
+    # translation modes with lambda ~ 0 (Goldstone; oracle eigenvalues ~1e-12 at the relaxed 70x70 state), so the STATE is
+    # only fixed up to a drift along them (observed 0.08 between the two end points at equal energy): compare what is
+    # unique -- the energy, and stationarity checked by the oracle on the GPU's end point.
+    w = wl.config1(L=40)
+    mdl = spin_model(w)
+    ref, iref = ro.relax_downhill(*ro.spin_ops(mdl), w.spins, 4000, 1e-6, 0.05)
+    ctx = moto.spin_context(w, kmax=2)
+    x = dev(w.spins)
+    info = ctx.relax(x, 4000, 1e-6, 0.05)
+    assert iref["converged"] and info["converged"] and info["status"] == 0
+    xh = x.cpu().numpy()
+    assert np.max(np.abs(np.linalg.norm(xh, axis=1) - 1.0)) <= 1e-14
+    assert abs(info["energy"] - iref["energy"]) <= 1e-11 * abs(iref["energy"])
+    assert np.linalg.norm(so.projected_gradient(mdl, xh)) <= 1.01e-6          # oracle-side check of the GPU's end point
+    assert abs(info["energy"] - so.energy(mdl, xh)) <= 1e-12 * abs(info["energy"])
+
+
+def test_ferromagnet_closed_form(moto):
+    # perturbed +z state relaxes to the ferromagnet: E = -N (6J + K + mu B) (ordered pairs, A1)
+    w = wl.config0()
+    ctx = moto.spin_context(w, kmax=2)
+    x = dev(w.spins)
+    info = ctx.relax(x, 2000, 1e-10, 0.05)
+    assert info["converged"]
+    assert abs(info["energy"] - (-w.N * (6 * w.J + w.K + w.mu * w.B[2]))) <= 1e-10
+    assert np.max(np.abs(x.cpu().numpy() - np.array([0.0, 0.0, 1.0]))) <= 1e-9
+
+
+def test_two_sided_descent_spins(moto):
+    w = wl.config1(L=12)
+    mdl = spin_model(w)
+    lam, V = so.lowest_modes(mdl, w.spins, 1)
+    res = ro.two_sided_descent(*ro.spin_ops(mdl), w.spins, V[0], 0.1, 3000, 1e-6, 0.05)
+    ctx = moto.spin_context(w, kmax=2)
+    xp, xm, infos = ctx.two_sided_descent(dev(w.spins), dev(V[0]), 0.1, 3000, 1e-6, 0.05)
+    for x, info, (xr, ir) in zip((xp, xm), infos, res):
+        xh = x.cpu().numpy()
+        assert info["converged"] and ir["converged"]
+        assert abs(info["energy"] - ir["energy"]) <= 1e-10 * abs(ir["energy"])
+        assert np.linalg.norm(so.projected_gradient(mdl, xh)) <= 1.01e-6
+        assert np.max(np.abs(np.linalg.norm(xh, axis=1) - 1.0)) <= 1e-14
+    # the seeds themselves: one accepted step from the seed is the same as the oracle's first step from its seed
+    xs, _, _ = ctx.two_sided_descent(dev(w.spins), dev(V[0]), 0.1, 0, 1e-6, 0.05)
+    seed = w.spins + 0.1 * V[0]
+    seed /= np.linalg.norm(seed, axis=1, keepdims=True)
+    assert np.max(np.abs(xs.cpu().numpy() - seed)) <= 1e-15
+
+
+def test_cartesian_first_steps_and_trimer(moto):
+    w = wl.config4()
+    mdl = cart_model(w)
+    ref, iref = ro.relax_downhill(*ro.cart_ops(mdl), w.positions, 3, 0.0, 0.05)
+    ctx = moto.cart_context(w)
+    x = dev(w.positions)
+    info = ctx.relax(x, 3, 0.0, 0.05)
+    assert info["steps"] == 3 and info["evals"] == iref["evals"]
+    assert abs(info["energy"] - iref["energy"]) <= 1e-12 * abs(iref["energy"])
+    xh = x.cpu().numpy()
+    assert np.max(np.abs(xh - ref)) <= 1e-11
+    assert np.all(xh[w.fixed == 1] == w.positions[w.fixed == 1])              # frozen atoms never move
+    # Morse trimer: equilateral triangle with edge r0, E = 3 (-De - phi(rc))
+    t = wl.small_cluster(3, seed=1)
+    t.positions[:] = np.array([[20.0, 20.0, 20.0], [23.1, 20.2, 19.9], [21.3, 22.9, 20.3]])
+    ctx3 = moto.cart_context(t)
+    x3 = dev(t.positions)
+    info3 = ctx3.relax(x3, 5000, 1e-10, 0.1)
+    p = x3.cpu().numpy()
+    r = np.array([np.linalg.norm(p[i] - p[j]) for i, j in ((0, 1), (0, 2), (1, 2))])
+    assert info3["converged"] and np.max(np.abs(r - t.r0)) <= 1e-8
+    assert abs(info3["energy"] - 3 * (-t.De - cart_model(t).phi(t.rc))) <= 1e-12
+
+
+def test_relax_already_converged_and_errors(moto):
+    w = wl.config0(sigma=0.0)            # exact ferromagnet: g = 0
+    ctx = moto.spin_context(w, kmax=2)
+    x = dev(w.spins)
+    info = ctx.relax(x, 10, 1e-12, 0.05)
+    assert info["converged"] and info["steps"] == 0 and info["evals"] == 1
+    assert np.array_equal(x.cpu().numpy(), w.spins)
+    with pytest.raises(moto.binding.MotoError):
+        ctx.relax(x, 10, 1e-12, 0.0)     # alpha0 must be > 0
+    with pytest.raises(moto.binding.MotoError):
+        ctx.relax(x, -1, 1e-12, 0.1)
+    import ctypes as C
+    lib = moto.load_library()
+    p = C.c_void_p(x.data_ptr())
+    assert lib.moto_two_sided_descent(ctx._h, p, p, 0.1, 10, 1e-6, 0.05, p, p, None) == moto.binding.EINVAL   # aliased
+
+
+def test_relax_is_deterministic(moto):
+    w = wl.config1(L=20)
+    ctx = moto.spin_context(w, kmax=2)
+    a, b = dev(w.spins), dev(w.spins)
+    ia = ctx.relax(a, 40, 0.0, 0.05)
+    ib = ctx.relax(b, 40, 0.0, 0.05)
+    assert ia == ib and np.array_equal(a.cpu().numpy(), b.cpu().numpy())
+
+
+def test_relax_full_size_properties(moto):
+    # configs[3] (10^6 spins), the launch configuration the bench times: 25 accepted steps; what the oracle can check at
+    # this size is the returned state itself -- its energy and projected-gradient norm, recomputed by the oracle
+    w = wl.config3()
+    mdl = spin_model(w)
+    E0 = so.energy(mdl, w.spins)
+    ctx = moto.spin_context(w, kmax=2)
+    x = dev(w.spins)
+    info = ctx.relax(x, 25, 0.0, 0.05)
+    xh = x.cpu().numpy()
+    assert info["steps"] == 25 and info["energy"] < E0
+    assert abs(info["energy"] - so.energy(mdl, xh)) <= 1e-12 * abs(E0)
+    gn = np.linalg.norm(so.projected_gradient(mdl, xh))
+    assert abs(info["gnorm"] - gn) <= 1e-10 * gn
+    assert np.max(np.abs(np.linalg.norm(xh, axis=1) - 1.0)) <= 1e-14
