@@ -113,6 +113,7 @@ int spin_hvp(moto_ctx*, const double* m, const double* c_or_null, const double* 
              int project_input, const int* d_done);
 int spin_mmf_step(moto_ctx*, const double* m, const double* v, int kr, double dt, double* m_out, double* d_fnorm);
 int spin_project(moto_ctx*, const double* m, double* V, int k);
+int spin_relax_eval(moto_ctx*, const double* x, const double* d, double a, const double* g_old, double* xt, double* gt, double* d_out4);
 int spin_hvp_three_term_generic(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double alpha, double c0,
                                 double beta, const double* U, double* out);
 // spin_stencil_tma.cu

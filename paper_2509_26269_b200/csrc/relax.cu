@@ -5,9 +5,10 @@
 //   trial x_t = R(x + a d), a = alpha, alpha/2, ...;  accept if g_t.d <= SIGMA |g.d| and (Armijo or E_t <= E + EPS_E |E|)
 //   beta = max(0, (g_t.g_t - g_t.g)/(g.g));  d <- -g_t + beta T(d)  (T = tangent projection at x_t / identity for atoms)
 //   alpha <- 2a if the first trial was accepted else a;  stop at |g| <= tau_F.
-// Every vector operation runs here (energy + gradient through the K1/K7 kernels, the three dots of a trial in one Gram
-// launch, trial state and direction update in two streaming kernels); the host sees four scalars per trial
-// (E_t, g_t.g_t, g_t.g, g_t.d) and takes the accept/reject decision.
+// Every vector operation runs on the device.  Spins: a trial is ONE fused pass (k_relax_eval in spin_stencil.cu: retraction
+// recomputed at the site and its neighbours, stencil gradient, projection and the four sums E_t, g_t.g_t, g_t.g, g_t.d;
+// 120 B/site) plus the direction update (96 B/site) once a step is accepted.  Atoms: trial kernel, neighbour lists + K7
+// gradient, one Gram launch.  The host sees four scalars per trial and takes the accept/reject decision.
 #include "common.cuh"
 #include "device_utils.cuh"
 
@@ -47,14 +48,22 @@ int grid_for(long long N) {
     return (int)(b < 4 * MOTO_NUM_SMS ? (b > 0 ? b : 1) : 4 * MOTO_NUM_SMS);
 }
 
-// E and gradient at x, then the dots of g_new with [g_new, g_old, d]; four scalars to the host, one synchronisation
-moto_status eval_point(moto_ctx* c, const double* x, double* g_new, const double* g_old, const double* d, double* h4) {
+// One evaluation: trial point x_t = R(x + a d) (d != nullptr) or x itself (d == nullptr); leaves g_new = gradient there and
+// brings {E, g_new.g_new, g_new.g_old, g_new.d} to the host with one synchronisation.
+// Spins: one fused pass (k_relax_eval, spin_stencil.cu).  Atoms: trial kernel, neighbour lists + K7 gradient, one Gram launch.
+moto_status eval_point(moto_ctx* c, const double* x, const double* d, double a, const double* g_old, double* xt, double* g_new,
+                       double* h4) {
     double* dE = c->st->scal;          // [0] E, [1..3] dots
-    moto_status s = moto_energy_grad(c, x, dE, g_new);
-    if (s != MOTO_OK) return s;
-    const double* S[1] = {g_new};
-    const double* T[3] = {g_new, g_old ? g_old : g_new, d ? d : g_new};
-    c->launches += block_gram(c, S, 1, T, 3, dE + 1, nullptr);
+    int fused = c->kind == MOTO_KIND_TRI2D ? spin_relax_eval(c, x, d, a, g_old, xt, g_new, dE) : 0;
+    c->launches += fused;
+    if (!fused) {
+        if (d) { k_relax_trial<<<grid_for(c->N), 256, 0, c->stream>>>((long long)c->N, x, d, a, xt, c->kind == MOTO_KIND_TRI2D); c->launches += 1; }
+        moto_status s = moto_energy_grad(c, d ? xt : x, dE, g_new);
+        if (s != MOTO_OK) return s;
+        const double* S[1] = {g_new};
+        const double* T[3] = {g_new, g_old ? g_old : g_new, d ? d : g_new};
+        c->launches += block_gram(c, S, 1, T, 3, dE + 1, nullptr);
+    }
     MOTO_CUDA_CHECK(c, cudaGetLastError());
     MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h4, dE, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
@@ -68,20 +77,24 @@ moto_status eval_point(moto_ctx* c, const double* x, double* g_new, const double
 
 }  // namespace
 
-// d_state in/out.  Scratch: g = ctx->g, g_t = W, d = AW, x_t = stage_m (no solver is running).
+// d_state in/out.  Scratch (no solver is running): g, g_t = ctx->g / W (swapped on acceptance), d = AW, and the current and
+// trial states ping-pong between stage_m and P, so an accepted step costs no copy; d_state is written once at the end.
 moto_status relax_run(moto_ctx* c, double* d_state, int max_steps, double tau_F, double alpha0, moto_relax_info* info) {
     const long long N = c->N;
     const size_t vb = (size_t)N * 3 * sizeof(double);
     const int spin = c->kind == MOTO_KIND_TRI2D;
     const int grid = grid_for(N);
-    double *g = c->g, *gt = c->W, *d = c->AW, *xt = c->stage_m;
+    double *g = c->g, *gt = c->W, *d = c->AW;
+    double* bufs[2] = {c->stage_m, c->P};
+    int which = 0;
+    const double* x = d_state;
     moto_relax_info out; memset(&out, 0, sizeof(out));
     double h[4];
-    moto_status s = eval_point(c, d_state, g, nullptr, nullptr, h);
+    moto_status s = eval_point(c, x, nullptr, 0.0, nullptr, nullptr, g, h);
     if (s != MOTO_OK) return s;
     out.evals = 1;
     double E = h[0], gg = h[1], slope = -gg, alpha = alpha0;
-    k_relax_dir<<<grid, 256, 0, c->stream>>>(N, d_state, g, 0.0, d, 0);   // d = -g (beta = 0: the old d is not read into the result)
+    k_relax_dir<<<grid, 256, 0, c->stream>>>(N, x, g, 0.0, d, 0);   // d = -g (beta = 0: the old d is never read)
     c->launches += 1;
     bool steepest = true;
     moto_status ret = MOTO_OK;
@@ -89,12 +102,11 @@ moto_status relax_run(moto_ctx* c, double* d_state, int max_steps, double tau_F,
         if (!(gg == gg)) { ret = moto_fail(c, MOTO_ESTATE, "moto_relax: NaN gradient"); break; }
         if (sqrt(gg) <= tau_F) { out.converged = 1; break; }
         if (out.steps >= max_steps) { ret = moto_fail(c, MOTO_ENOTCONV, "moto_relax: max_steps reached"); break; }
+        double* xt = bufs[which];
         double a = alpha;
         bool accepted = false, first = true;
         for (int bt = 0; bt < RELAX_MAX_BACKTRACKS; ++bt) {
-            k_relax_trial<<<grid, 256, 0, c->stream>>>(N, d_state, d, a, xt, spin);
-            c->launches += 1;
-            s = eval_point(c, xt, gt, g, d, h);
+            s = eval_point(c, x, d, a, g, xt, gt, h);
             if (s != MOTO_OK) return s;
             out.evals += 1;
             const double Et = h[0], gtd = h[3];
@@ -104,7 +116,7 @@ moto_status relax_run(moto_ctx* c, double* d_state, int max_steps, double tau_F,
         }
         if (!accepted) {
             if (steepest) { ret = moto_fail(c, MOTO_ENOTCONV, "moto_relax: stalled (no acceptable step along -g)"); break; }
-            k_relax_dir<<<grid, 256, 0, c->stream>>>(N, d_state, g, 0.0, d, 0);
+            k_relax_dir<<<grid, 256, 0, c->stream>>>(N, x, g, 0.0, d, 0);
             c->launches += 1;
             slope = -gg; steepest = true;
             continue;
@@ -117,12 +129,13 @@ moto_status relax_run(moto_ctx* c, double* d_state, int max_steps, double tau_F,
         k_relax_dir<<<grid, 256, 0, c->stream>>>(N, xt, gt, beta, d, spin);
         c->launches += 1;
         steepest = beta == 0.0;
-        MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_state, xt, vb, cudaMemcpyDeviceToDevice, c->stream));
+        x = xt; which ^= 1;
         double* t = g; g = gt; gt = t;
         E = Et; gg = gtgt; slope = new_slope;
         alpha = first ? 2.0 * a : a;
         out.steps += 1;
     }
+    if (x != d_state) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_state, x, vb, cudaMemcpyDeviceToDevice, c->stream));
     MOTO_CUDA_CHECK(c, cudaGetLastError());
     MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
     out.energy = E; out.gnorm = sqrt(gg); out.alpha = alpha;

@@ -72,6 +72,83 @@ __global__ void __launch_bounds__(256) k_energy_grad(Lat l, const double* __rest
     if (threadIdx.x == 0) partials[blockIdx.x] = e[0];
 }
 
+// ---------------------------------------------------------------- fused line-search trial of moto_relax (relax.cu)
+// One pass per trial: a CTA stages the 32 x 8 site tile plus its one-site halo of the TRIAL state x_t = R(x + a d) in shared
+// memory (retraction computed once per staged site: 340 for 256 sites), applies the stencil from there, and emits x_t,
+// g_t = P_t (L x_t - mu B) and the partial sums of E_t, g_t.g_t, g_t.g, g_t.d: 120 B/site, the trial state never makes a round
+// trip through HBM before the stencil.  (Recomputing x_t at the seven sites per thread straight from global memory was
+// 3x slower than the plain gradient: 14 strided site loads per thread.)
+// TRIAL = false: plain evaluation at x (d, g ignored, nothing retracted, x_t not written).
+#define RT_W 32
+#define RT_H 8
+template <bool TRIAL>
+__global__ void __launch_bounds__(RT_W * RT_H) k_relax_eval(Lat l, const double* __restrict__ x, const double* __restrict__ d, double a,
+                                                            const double* __restrict__ g_old, double* __restrict__ xt_out,
+                                                            double* __restrict__ gt_out, double* __restrict__ partials) {
+    __shared__ double tile[RT_H + 2][RT_W + 2][3];
+    __shared__ double red[32 * 4];
+    const int tx0 = blockIdx.x * RT_W, ty0 = blockIdx.y * RT_H;
+    for (int cell = threadIdx.x; cell < (RT_W + 2) * (RT_H + 2); cell += RT_W * RT_H) {
+        const int ly = cell / (RT_W + 2), lx = cell - ly * (RT_W + 2);
+        int gx = tx0 + lx - 1, gy = ty0 + ly - 1;
+        bool ok = true;
+        if (gx < 0 || gx >= l.Lx) { if (l.px) gx = ((gx % l.Lx) + l.Lx) % l.Lx; else ok = false; }
+        if (gy < 0 || gy >= l.Ly) { if (l.py) gy = ((gy % l.Ly) + l.Ly) % l.Ly; else ok = false; }
+        d3 y = mk3(0.0, 0.0, 0.0);                     // absent neighbour (open boundary) contributes 0
+        if (ok) {
+            const long long j = (long long)gy * l.Lx + gx;
+            y = ld3(x, j);
+            if (TRIAL) {
+                y = axpy3(a, ld3(d, j), y);
+                y = scale3(1.0 / sqrt(dot3(y, y)), y);
+            }
+        }
+        tile[ly][lx][0] = y.x; tile[ly][lx][1] = y.y; tile[ly][lx][2] = y.z;
+    }
+    __syncthreads();
+    const int lx = threadIdx.x % RT_W, ly = threadIdx.x / RT_W;
+    const int gx = tx0 + lx, gy = ty0 + ly;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    if (gx < l.Lx && gy < l.Ly) {
+        const long long i = (long long)gy * l.Lx + gx;
+        auto T = [&](int yy, int xx) { return mk3(tile[yy][xx][0], tile[yy][xx][1], tile[yy][xx][2]); };
+        const d3 mi = T(ly + 1, lx + 1);
+        // +-a1 = (+-1, 0), +-a2 = (0, +-1), +-(a2 - a1) = (-+1, +-1)
+        const d3 Lm = stencil_apply(l, T(ly + 1, lx + 2), T(ly + 1, lx), T(ly + 2, lx + 1), T(ly, lx + 1), T(ly + 2, lx), T(ly, lx + 2), mi.z);
+        const d3 B = mk3(l.mu * l.Bx, l.mu * l.By, l.mu * l.Bz);
+        const d3 g = sub3(Lm, B);
+        const d3 pg = axpy3(-dot3(mi, g), mi, g);
+        acc[0] = 0.5 * dot3(mi, Lm) - dot3(mi, B);
+        acc[1] = dot3(pg, pg);
+        if (TRIAL) {
+            acc[2] = dot3(pg, ld3(g_old, i));
+            acc[3] = dot3(pg, ld3(d, i));
+            st3(xt_out, i, mi);
+        }
+        st3(gt_out, i, pg);
+    }
+    block_sum<4>(acc, red);
+    if (threadIdx.x == 0) {
+        const size_t b = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
+        for (int j = 0; j < 4; ++j) partials[b * 4 + j] = acc[j];
+    }
+}
+
+// out[j] = sum_b partials[b*4 + j], j < 4: 256 strided rows per value (coalesced), then a shared-memory tree; fixed order
+__global__ void __launch_bounds__(1024) k_final_sum4(const double* __restrict__ partials, int nblk, double* __restrict__ out) {
+    __shared__ double sm[1024];
+    const int j = threadIdx.x & 3, r = threadIdx.x >> 2;
+    double s = 0.0;
+    for (int b = r; b < nblk; b += 256) s += partials[(size_t)b * 4 + j];
+    sm[threadIdx.x] = s;
+    __syncthreads();
+    for (int off = 512; off >= 4; off >>= 1) {
+        if (threadIdx.x < off) sm[threadIdx.x] += sm[threadIdx.x + off];
+        __syncthreads();
+    }
+    if (threadIdx.x < 4) out[threadIdx.x] = sm[threadIdx.x];
+}
+
 // out[j] = sum_b partials[b*stride + j]  (optionally sqrt); one thread per j, fixed order
 __global__ void k_final_sum(const double* __restrict__ partials, int nblk, int stride, int nval, double* __restrict__ out,
                             int take_sqrt) {
@@ -209,6 +286,17 @@ int spin_energy_grad(moto_ctx* c, const double* m, double* d_E, double* d_g, dou
     int n = 1;
     if (d_E) { k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_E, 0); ++n; }
     return n;
+}
+
+// d_out4 = {E_t, g_t.g_t, g_t.g, g_t.d} (device); d == nullptr: plain evaluation at x (out4[2], [3] = 0)
+int spin_relax_eval(moto_ctx* c, const double* x, const double* d, double a, const double* g_old, double* xt, double* gt, double* d_out4) {
+    Lat l = make_lat(c);
+    dim3 grid((l.Lx + RT_W - 1) / RT_W, (l.Ly + RT_H - 1) / RT_H);
+    if ((size_t)grid.x * grid.y * 4 > (size_t)MOTO_RED_BLOCKS * 2 * MOTO_NS * MOTO_NS || grid.y > 65535) return 0;   // partials capacity: caller takes the three-pass route
+    if (d) k_relax_eval<true><<<grid, RT_W * RT_H, 0, c->stream>>>(l, x, d, a, g_old, xt, gt, c->partials);
+    else k_relax_eval<false><<<grid, RT_W * RT_H, 0, c->stream>>>(l, x, nullptr, 0.0, nullptr, nullptr, gt, c->partials);
+    k_final_sum4<<<1, 1024, 0, c->stream>>>(c->partials, (int)(grid.x * grid.y), d_out4);
+    return 2;
 }
 
 int spin_curvature(moto_ctx* c, const double* m, double* d_c) { return spin_energy_grad(c, m, nullptr, nullptr, d_c); }
