@@ -168,7 +168,7 @@ def run_report(args):
         torch.cuda.synchronize()
         return ev0.elapsed_time(ev1) / reps
 
-    rows, orows, lrows = [], [], []
+    rows, orows, lrows, xrows = [], [], [], []
     cfgs = [("0", wl.config0(), 0), ("1", wl.config1(), 0), ("2", wl.config2(), 100), ("3", wl.config3(), 200), ("4", wl.config4(), 100)]
     # the paper's own Fig. 2 workload class: a random spin configuration at 10^6 spins, same J, D, K, B
     rnd = wl.random_spins(1000, 1000, 7)
@@ -218,6 +218,26 @@ def run_report(args):
             ev1.record(); torch.cuda.synchronize()
             l = lam_s.cpu().numpy()
             mmf = f"{nsteps} steps, {ev0.elapsed_time(ev1):.0f} ms ({ev0.elapsed_time(ev1) / nsteps:.2f} ms/step, {tot_it} solver iterations), final \\|F_mmf\\| = {fn.item():.3e}, λ₁, λ₂ = {l[0]:.5f}, {l[1]:.5f}"
+        # two-sided descent's RelaxDownHill (moto_relax, Alg. 1 l.17): bounded run from the config's start state
+        xr = x.clone()
+        ctx.relax(xr.clone(), 20, 0.0, 0.05)
+        torch.cuda.synchronize(); ev0.record()
+        rinfo = ctx.relax(xr, 2000, 1e-6, 0.05)
+        ev1.record(); torch.cuda.synchronize()
+        relax_ms = ev0.elapsed_time(ev1)
+        o_us = ""
+        if not args.no_cpu_baseline:
+            from oracle import relax_oracle as ro
+            if cart:
+                from oracle import cart_oracle as co
+                ops = ro.cart_ops(co.MorseModel(w.cell, w.De, w.alpha, w.r0, w.rc, w.fixed))
+            else:
+                from oracle import spin_oracle as so
+                ops = ro.spin_ops(so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu))
+            t0 = time.perf_counter(); _, oi = ro.relax_downhill(*ops, w.positions if cart else w.spins, 3, 0.0, 0.05); t_r = time.perf_counter() - t0
+            o_us = f"{1e6 * t_r / oi['evals']:.0f}"
+        xrows.append(f"| {name} | {N} | {rinfo['steps']} | {rinfo['evals']} | {relax_ms:.2f} | {1e3 * relax_ms / rinfo['evals']:.1f} | "
+                     f"{'yes' if rinfo['converged'] else 'no (cap 2000)'} | {rinfo['gnorm']:.1e} | {rinfo['energy']:.6f} | {o_us} |")
         gbs = alg / (hvp_ms * 1e-3) / 1e9
         rows.append(f"| {name} | {N} | {w.k} | {hvp_ms * 1e3:.1f} | {w.k * 1e3 / hvp_ms:.3g} | {N * w.k / (hvp_ms * 1e-3) / 1e9:.3g} | "
                     f"{gbs:.0f} ({gbs / peak:.2f} of measured, {gbs / 8000:.2f} of 8 TB/s{'' if N >= 500000 else '; below L2 size: latency-bound'}) | "
@@ -256,6 +276,11 @@ def run_report(args):
     print("| cfg | N | k | basis m | solve ms | Lanczos steps (= HVPs) | converged | max true resid | max abs(lambda - LOBPCG's) |")
     print("|---|---|---|---|---|---|---|---|---|")
     print("\n".join(lrows))
+    print("\nRelaxDownHill of the two-sided descent (`moto_relax`, Alg. 1 l.17: PR+ CG with backtracking, tau_F = 1e-6, alpha0 = 0.05, cap 2000 steps; "
+          "one evaluation = energy + gradient + 3 dots at a trial point; oracle = oracle/relax_oracle.py, first 3 steps):\n")
+    print("| cfg | N | accepted steps | evaluations | ms | µs / evaluation | converged | final \\|g\\| | final E | oracle µs / evaluation |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    print("\n".join(xrows))
     if orows:
         print(f"\nOracle on the host ({cores} BLAS threads, {os.cpu_count()} CPUs), as it stands — a baseline, not the target:\n")
         print("| cfg | oracle HVP ms (explicit Hessian rebuilt) | oracle lowest-k s | how | max rel. eigenvalue difference GPU vs oracle |")

@@ -151,7 +151,7 @@ moto_status moto_mmf_run(moto_ctx* ctx, double* d_state, int k, double dt, int m
 
 /* Two-sided minimum-mode descent (Alg. 1 l.15-18; Suppl. Note 1 b(iii)).
  * moto_relax: "RelaxDownHill" with a deterministic optimiser.  The paper names the class ("L-BFGS/CG") and nothing else;
- *   this is Riemannian Polak-Ribiere+ conjugate gradients with backtracking (reading A25):
+ *   this is Riemannian Polak-Ribiere+ conjugate gradients with backtracking (reading A26):
  *     trial x_t = R(x + a d), a = alpha, alpha/2, ... (<= 40);  accepted when g_t.d <= 0.5 |g.d| and
  *     (E_t <= E + 1e-4 a g.d  or  E_t <= E + 1e-10 |E|);  beta = max(0, (g_t.g_t - g_t.g)/(g.g));
  *     d <- -g_t + beta T(d) (T = tangent projection at x_t for spins, identity for atoms; reset to -g_t if not a descent

@@ -5,7 +5,7 @@
                    PAPER.md:275 (Alg. 1 l.17), :307 (Suppl. Note 1 b(iii))
 
 The paper names the optimiser class and nothing else (no line search, no constants), so the algorithm below is the
-reading DESIGN.md lists as A25 -- Riemannian Polak-Ribiere+ nonlinear conjugate gradients with backtracking:
+reading DESIGN.md lists as A26 -- Riemannian Polak-Ribiere+ nonlinear conjugate gradients with backtracking:
 
   d_0 = -g_0                                   g = tangent-projected / masked gradient
   trial  x_t = R(x + a d),  a = alpha, alpha/2, alpha/4, ...  (at most MAX_BACKTRACKS)

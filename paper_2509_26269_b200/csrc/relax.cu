@@ -1,6 +1,6 @@
 // relax.cu -- two-sided minimum-mode descent (Alg. 1 l.15-18; Suppl. Note 1 b(iii), PAPER.md:307;
 // SURVEY 8(f) f2): seeds x_saddle +- eta v_min, each relaxed downhill "using a deterministic optimizer (e.g., L-BFGS/CG)".
-// The paper gives no more than that; the optimiser is reading A25 of DESIGN.md: Riemannian Polak-Ribiere+ conjugate
+// The paper gives no more than that; the optimiser is reading A26 of DESIGN.md: Riemannian Polak-Ribiere+ conjugate
 // gradients with backtracking,
 //   trial x_t = R(x + a d), a = alpha, alpha/2, ...;  accept if g_t.d <= SIGMA |g.d| and (Armijo or E_t <= E + EPS_E |E|)
 //   beta = max(0, (g_t.g_t - g_t.g)/(g.g));  d <- -g_t + beta T(d)  (T = tangent projection at x_t / identity for atoms)
