@@ -249,3 +249,62 @@ def small_cluster(n: int, seed: int, box: float = 9.0) -> CartWorkload:
     cell = np.array([[60.0, 0.0], [0.0, 60.0]])
     return CartWorkload(f"cluster{n}", pos, np.zeros(n, dtype=np.uint8), cell, De=0.4205, alpha=1.4199, r0=2.780,
                         rc=6.0, k=2, seed=seed)
+
+
+# ---- general neighbour shells: stand-in for the paper's tabulated Pd/Fe/Ir(111) couplings
+def shell_table(rcut: float, J1: float = 1.0, D1: float = 0.3, Dz1: float = 0.05, kF: float = 1.7):
+    """All lattice offsets (dx, dy) != 0 with |dx a1 + dy a2| <= rcut, with synthetic, inversion-symmetric couplings that
+    have the structure of a tabulated metallic film (the DFT tables of PAPER.md:328-616 are garbled and the UppASD inputs
+    are not in the container): oscillating, decaying exchange J(r) = J1 cos(kF (r - 1)) / r^3, an in-plane Neel-type DMI
+    D1 / r^3 (z x rhat) and an out-of-plane component Dz1 / r^3 with the sign of the bond's half-plane (so D(-d) = -D(d)).
+    rcut = 1 gives the six nearest neighbours with J1, D1 (z x rhat) + sign * Dz1 z.  rcut = 10 gives 366 neighbours.
+    Returns offsets [n][2] int32, J [n], D [n][3]."""
+    R = int(np.ceil(rcut * 2 / np.sqrt(3.0))) + 1
+    offs, Js, Ds = [], [], []
+    for dy in range(-R, R + 1):
+        for dx in range(-2 * R, 2 * R + 1):
+            if dx == 0 and dy == 0:
+                continue
+            x, y = dx + 0.5 * dy, dy * np.sqrt(3.0) / 2.0
+            r = float(np.hypot(x, y))
+            if r > rcut + 1e-9:
+                continue
+            sgn = 1.0 if (dy > 0 or (dy == 0 and dx > 0)) else -1.0
+            offs.append((dx, dy))
+            Js.append(J1 * np.cos(kF * (r - 1.0)) / r ** 3)
+            Ds.append((D1 / r ** 3 * (-y / r), D1 / r ** 3 * (x / r), sgn * Dz1 / r ** 3))
+    return np.array(offs, dtype=np.int32), np.array(Js), np.array(Ds)
+
+
+@dataclass
+class ShellWorkload:
+    name: str
+    Lx: int
+    Ly: int
+    pbc_x: int
+    pbc_y: int
+    offsets: np.ndarray   # [n][2] int32
+    Jd: np.ndarray        # [n]
+    Dd: np.ndarray        # [n][3]
+    K: float
+    B: tuple
+    mu: float
+    k: int
+    seed: int
+    spins: np.ndarray
+    tol: float = 1e-8
+
+    @property
+    def N(self) -> int:
+        return self.Lx * self.Ly
+
+
+def config_shells(L: int = 100, rcut: float = 10.0, seed: int = 1005, R: float = 5.0, sigma: float = 0.02, pbc: int = 1) -> ShellWorkload:
+    """The paper's real workload class: L x L periodic lattice, couplings over every shell within rcut
+    (366 neighbours per site at rcut = 10), one Neel skyrmion of radius R at the centre plus seeded noise (configs[1] recipe)."""
+    rng = np.random.default_rng(seed)
+    centre = np.array([_site_xy(L // 2, L // 2)])
+    spins = add_noise(skyrmion_texture(L, L, pbc, pbc, centre, R), sigma, rng)
+    offs, Js, Ds = shell_table(rcut)
+    return ShellWorkload(f"shells{L}_rc{rcut:g}", L, L, pbc, pbc, offs, Js, Ds, K=0.05, B=(0.0, 0.0, 0.02), mu=1.0, k=2, seed=seed,
+                         spins=spins)
