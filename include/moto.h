@@ -102,6 +102,17 @@ void moto_destroy(moto_ctx* ctx);
 moto_status moto_set_solver(moto_ctx* ctx, const moto_solver_opts* opts);
 const char* moto_last_error(const moto_ctx* ctx);
 
+/* General neighbour shells (Eq. 4, is written for arbitrary pairs and the paper's
+ * Pd/Fe/Ir(111) workload tabulates J_ij and three-component D_ij over ~340 neighbours per site):
+ * replace the nearest-neighbour J, D of moto_spin_params by a translation-invariant table over lattice offsets,
+ *   J_ij = h_J[t], D_ij = h_D[t][0..2]  for  j = i + (h_offsets[t][0], h_offsets[t][1])   (K, B, mu stay as created).
+ * All three arrays are HOST pointers, copied (n <= 512).  The table must hold distinct non-zero offsets and be inversion
+ * symmetric, J(-d) = J(d), D(-d) = -D(d) (the same bond seen from its other end, reading A2), else MOTO_EINVAL.  Ordered
+ * pairs are counted as printed (reading A1).  n = 0 returns to the nearest-neighbour model.  Kind 0 only.  Every call
+ * (energy_grad, hvp, lowest_modes, mmf_step, mmf_run, relax, ...) then runs on the table through the warp-per-site K1 of
+ * spin_shells.cu; the TMA path and with it moto_cheb_apply / the Chebyshev transformation are not available. */
+moto_status moto_set_shells(moto_ctx* ctx, int n, const int32_t* h_offsets, const double* h_J, const double* h_D);
+
 /* E(m) and its gradient.  d_E: [1] device.  d_g: [N][3] device, may be NULL.
  * kind 0: d_g = tangent-projected gradient P g = g - (m.g) m ("forces ... understood as
  *         tangent-projected").   kind 1: Euclidean gradient, rows of fixed atoms zero. */

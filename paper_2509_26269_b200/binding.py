@@ -71,6 +71,7 @@ _SIGS = {
     "moto_destroy": (None, [C.c_void_p]),
     "moto_set_solver": (C.c_int, [C.c_void_p, C.POINTER(SolverOpts)]),
     "moto_last_error": (C.c_char_p, [C.c_void_p]),
+    "moto_set_shells": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "moto_energy_grad": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "moto_hvp": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
     "moto_lowest_modes": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
@@ -190,6 +191,14 @@ class Context:
         """method: 0 block LOBPCG, 1 thick-restart Lanczos (ncv = basis size, 0 = largest the workspace holds)."""
         o = SolverOpts(guard, check_every, precond_degree, hvp_path, precond_lo, precond_hi, seed, method, ncv)
         self._check(self.lib.moto_set_solver(self._h, C.byref(o)))
+
+    def set_shells(self, offsets, J, D):
+        """moto_set_shells: host tables offsets [n][2] int32, J [n], D [n][3] (n = 0 / empty: back to nearest neighbours)."""
+        off = np.ascontiguousarray(offsets, dtype=np.int32).reshape(-1, 2)
+        Jh = np.ascontiguousarray(J, dtype=np.float64).reshape(-1)
+        Dh = np.ascontiguousarray(D, dtype=np.float64).reshape(-1, 3)
+        assert off.shape[0] == Jh.shape[0] == Dh.shape[0]
+        self._check(self.lib.moto_set_shells(self._h, int(off.shape[0]), off.ctypes.data, Jh.ctypes.data, Dh.ctypes.data))
 
     @property
     def launch_count(self) -> int:
@@ -357,3 +366,12 @@ def cart_context(w, kmax=None, device="cuda:0", stream=None) -> Context:
             lat.cell[a][b] = float(w.cell[a][b])
     p = MorseParams(w.De, w.alpha, w.r0, w.rc)
     return Context(lat, p, kmax=kmax or w.k, device=device, stream=stream, fixed=w.fixed)
+
+
+def shell_context(w, kmax=None, device="cuda:0", stream=None) -> Context:
+    """Context for a workloads.ShellWorkload: a spin lattice whose couplings come from the neighbour table (moto_set_shells)."""
+    lat = Lattice(KIND_TRI2D, w.Lx, w.Ly, w.pbc_x, w.pbc_y, 0)
+    p = SpinParams(0.0, 0.0, w.K, (C.c_double * 3)(*w.B), w.mu)
+    ctx = Context(lat, p, kmax=kmax or w.k, device=device, stream=stream)
+    ctx.set_shells(w.offsets, w.Jd, w.Dd)
+    return ctx

@@ -47,7 +47,7 @@ static double stencil_lmax_bound(const moto_spin_params& sp) {
     return best + 0.25 * h * h * 12.0 * (fabs(sp.J) + fabs(sp.D)) * 2.0 + 2.0 * fabs(sp.K);
 }
 
-struct WsLayout { size_t block, c, g, stage, partials, st, flags, cart, total; int nblocks; };
+struct WsLayout { size_t block, c, g, stage, partials, st, flags, shell, cart, total; int nblocks; };
 
 static WsLayout ws_layout(const moto_lattice* lat, int kmax) {
     WsLayout w;
@@ -61,7 +61,8 @@ static WsLayout ws_layout(const moto_lattice* lat, int kmax) {
     w.cart = lat->kind == MOTO_KIND_CARTESIAN ? cart_lists_bytes(lat) : 0;
     w.nblocks = lat->kind == MOTO_KIND_TRI2D ? 8 : 6;   // spin lattices: + two Chebyshev ping-pong blocks
     w.flags = 4096;
-    w.total = w.nblocks * w.block + w.c + w.g + w.stage + w.partials + w.st + w.flags + w.cart;
+    w.shell = lat->kind == MOTO_KIND_TRI2D ? al256((size_t)MOTO_MAX_SHELLS * (2 * sizeof(int) + 4 * sizeof(double))) : 0;
+    w.total = w.nblocks * w.block + w.c + w.g + w.stage + w.partials + w.st + w.flags + w.shell + w.cart;
     return w;
 }
 
@@ -114,6 +115,7 @@ moto_status moto_create(const moto_lattice* lat, const void* params, void* d_wor
     c->partials = (double*)p; p += w.partials;
     c->st = (SolverState*)p; p += w.st;
     c->flags = (unsigned long long*)p; p += w.flags;
+    if (w.shell) { c->sh_jd = (double*)p; c->sh_off = (int*)(p + (size_t)MOTO_MAX_SHELLS * 4 * sizeof(double)); p += w.shell; }
     if (c->kind == MOTO_KIND_CARTESIAN) cart_lists_carve(c, p);
     cudaError_t e = cudaHostAlloc((void**)&c->hstat, 2 * sizeof(HostStatus), cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->flags, 0, w.flags, c->stream);
@@ -145,6 +147,13 @@ moto_status moto_set_solver(moto_ctx* c, const moto_solver_opts* o) {
     if (n.seed == 0) n.seed = 0x9E3779B97F4A7C15ull;
     c->opts = n;
     return MOTO_OK;
+}
+
+moto_status moto_set_shells(moto_ctx* c, int n, const int32_t* h_offsets, const double* h_J, const double* h_D) {
+    if (!c) return MOTO_EINVAL;
+    if (c->kind != MOTO_KIND_TRI2D) return moto_fail(c, MOTO_ESTATE, "moto_set_shells: spin lattices only");
+    if (n < 0 || n > MOTO_MAX_SHELLS || (n > 0 && (!h_offsets || !h_J || !h_D))) return moto_fail(c, MOTO_EINVAL, "moto_set_shells: need 0 <= n <= 512 and non-null tables");
+    return shell_set(c, n, h_offsets, h_J, h_D);
 }
 
 const char* moto_last_error(const moto_ctx* c) { return c ? c->err : "null context"; }

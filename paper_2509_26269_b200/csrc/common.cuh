@@ -12,6 +12,7 @@
 #define MOTO_LZ_MAX 24       // largest Lanczos basis (the single-CTA Jacobi solves up to MOTO_NS = 24)
 #define MOTO_RED_BLOCKS 296  // CTAs of every grid-reduction kernel (2 per SM): fixed => deterministic sums
 #define MOTO_MAX_NEIGH 160   // Cartesian: neighbour capacity per atom
+#define MOTO_MAX_SHELLS 512 // largest neighbour table of moto_set_shells
 #define MOTO_CHEB_MAX 256    // largest degree of the Chebyshev spectral transformation
 
 // Device-resident LOBPCG state: Gram matrices, Ritz coefficients, residuals, control flags.
@@ -84,6 +85,9 @@ struct moto_ctx {
     double* partials;  // [MOTO_RED_BLOCKS][2*NS*NS] grid-reduction partials
     SolverState* st;
     CartLists cl;
+    int nsh;           // > 0: general neighbour shells (moto_set_shells) replace the nearest-neighbour J, D of sp
+    int* sh_off;       // [MOTO_MAX_SHELLS][2] device
+    double* sh_jd;     // [MOTO_MAX_SHELLS][4] device: J, Dx, Dy, Dz
     HostStatus* hstat;  // pinned
     cudaEvent_t ev[2];
     int64_t launches;
@@ -124,6 +128,13 @@ int spin_cheb_multistep(moto_ctx*, const double* m, const double* cvec, const do
                         const double* d_coef, const int* d_done);
 int spin_hvp_tma_ex(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double* HV, const int* d_done,
                     double* waw_partials, int cheb, double alpha, double c0, double beta, const double* U, const double* d_coef);
+// spin_shells.cu
+int shell_energy_grad(moto_ctx*, const double* m, double* d_E, double* d_g, double* d_c);
+int shell_hvp(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input, const int* d_done);
+int shell_three_term(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double alpha, double c0, double beta,
+                     const double* U, double* out);
+int shell_mmf_pass1(moto_ctx*, const double* m, const double* v, int kr);
+moto_status shell_set(moto_ctx*, int n, const int32_t* h_off, const double* h_J, const double* h_D);
 // cart_morse.cu
 int cart_build_lists(moto_ctx*, const double* x);
 int cart_energy_grad(moto_ctx*, const double* x, double* d_E, double* d_g);

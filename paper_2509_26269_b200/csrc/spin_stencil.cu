@@ -281,6 +281,7 @@ __global__ void __launch_bounds__(256) k_mmf_pass2(long long N, const double* __
 
 // ================================================================ host wrappers
 int spin_energy_grad(moto_ctx* c, const double* m, double* d_E, double* d_g, double* d_c) {
+    if (c->nsh > 0) return shell_energy_grad(c, m, d_E, d_g, d_c);
     Lat l = make_lat(c);
     k_energy_grad<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, d_g, d_c, c->partials);
     int n = 1;
@@ -290,6 +291,7 @@ int spin_energy_grad(moto_ctx* c, const double* m, double* d_E, double* d_g, dou
 
 // d_out4 = {E_t, g_t.g_t, g_t.g, g_t.d} (device); d == nullptr: plain evaluation at x (out4[2], [3] = 0)
 int spin_relax_eval(moto_ctx* c, const double* x, const double* d, double a, const double* g_old, double* xt, double* gt, double* d_out4) {
+    if (c->nsh > 0) return 0;   // general shells: the one-site halo tile does not apply, caller takes the three-pass route
     Lat l = make_lat(c);
     dim3 grid((l.Lx + RT_W - 1) / RT_W, (l.Ly + RT_H - 1) / RT_H);
     if ((size_t)grid.x * grid.y * 4 > (size_t)MOTO_RED_BLOCKS * 2 * MOTO_NS * MOTO_NS || grid.y > 65535) return 0;   // partials capacity: caller takes the three-pass route
@@ -306,6 +308,7 @@ int spin_hvp_tma(moto_ctx* c, const double* m, const double* cvec, const double*
 
 int spin_hvp(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input,
              const int* d_done) {
+    if (c->nsh > 0) return shell_hvp(c, m, cvec, V, k, HV, project_input, d_done);
     int n = spin_hvp_tma(c, m, cvec, V, k, HV, project_input, d_done);
     if (n > 0) return n;
     Lat l = make_lat(c);
@@ -323,6 +326,7 @@ int spin_hvp(moto_ctx* c, const double* m, const double* cvec, const double* V, 
 
 int spin_hvp_three_term_generic(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double alpha, double c0,
                                 double beta, const double* U, double* out) {
+    if (c->nsh > 0) return shell_three_term(c, m, cvec, V, k, alpha, c0, beta, U, out);
     Lat l = make_lat(c);
     const long long N = c->N;
     k_three_term_generic<<<(int)((N + 255) / 256), 256, 0, c->stream>>>(l, m, cvec, V, k, alpha, c0, beta, U, out);
@@ -338,10 +342,12 @@ int spin_project(moto_ctx* c, const double* m, double* V, int k) {
 int spin_mmf_step(moto_ctx* c, const double* m, const double* v, int kr, double dt, double* m_out, double* d_fnorm) {
     Lat l = make_lat(c);
     double* alpha = c->st->scal;  // [KMAX] would overflow scal[8]? KMAX == 8: exactly fits
-    k_mmf_pass1<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, v, kr, c->g, c->partials);
+    int n0 = 1;
+    if (c->nsh > 0) n0 = shell_mmf_pass1(c, m, v, kr);
+    else k_mmf_pass1<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, v, kr, c->g, c->partials);
     k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, MOTO_KMAX, MOTO_KMAX, alpha, 0);
     k_mmf_pass2<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, m, v, kr, c->g, alpha, dt, m_out, c->partials, 1, nullptr);
-    int n = 3;
+    int n = 2 + n0;
     if (d_fnorm) { k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_fnorm, 1); ++n; }
     return n;
 }

@@ -525,7 +525,7 @@ bool launch(moto_ctx* c, const Maps& maps, const KParams& p, int grid) {
 }  // namespace
 
 bool spin_tma_applicable(const moto_ctx* c) {
-    if (c->kind != MOTO_KIND_TRI2D) return false;
+    if (c->kind != MOTO_KIND_TRI2D || c->nsh > 0) return false;   // general neighbour shells take spin_shells.cu
     const int Lx = c->lat.Lx, Ly = c->lat.Ly;
     if (c->opts.hvp_path == 1) return false;                  // hvp_path = generic
     if ((Lx & 1) || Lx < 8 || Ly < 1) return false;          // row stride 24 Lx must be a multiple of 16 B; side box needs 16 doubles

@@ -1,0 +1,159 @@
+"""GPU parity tests of the general-neighbour-shell path (moto_set_shells) against oracle/shell_oracle.py,
+and against the library's own nearest-neighbour kernels on the six-neighbour table."""
+import ctypes as C
+
+import numpy as np
+import pytest
+import scipy.linalg
+
+from oracle import relax_oracle as ro
+from oracle import shell_oracle as sh
+from oracle import spin_oracle as so
+from paper_2509_26269_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).cuda()
+
+
+def rel_l2(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+def model_of(w):
+    return sh.ShellModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.offsets, w.Jd, w.Dd, w.K, w.B, w.mu)
+
+
+def shell_workload(Lx, Ly, pbc, rcut, seed, B=(0.01, -0.02, 0.03), **kw):
+    offs, J, D = wl.shell_table(rcut, **kw)
+    return wl.ShellWorkload(f"sh{Lx}x{Ly}", Lx, Ly, pbc[0], pbc[1], offs, J, D, K=0.05, B=B, mu=1.0, k=2, seed=seed,
+                            spins=wl.random_spins(Lx, Ly, seed))
+
+
+@pytest.mark.parametrize("Lx,Ly,pbc,rcut", [(12, 12, (1, 1), 3.0), (13, 9, (0, 0), 3.0), (16, 7, (1, 0), 2.0), (5, 4, (1, 1), 3.0),
+                                             (40, 33, (0, 1), 4.5)])
+def test_energy_grad_hvp_parity(moto, Lx, Ly, pbc, rcut):
+    # random spins (the paper's "random spin configurations"); 5x4 periodic with rcut 3: offsets wrap more than once
+    w = shell_workload(Lx, Ly, pbc, rcut, seed=Lx + Ly)
+    mdl = model_of(w)
+    ctx = moto.shell_context(w, kmax=8)
+    E, g = ctx.energy_grad(dev(w.spins))
+    E_ref = sh.energy(mdl, w.spins)
+    assert abs(E.item() - E_ref) <= 1e-12 * max(1.0, abs(E_ref))
+    assert np.max(np.abs(g.cpu().numpy() - sh.projected_gradient(mdl, w.spins))) <= 1e-12
+    for k in (1, 2, 5):
+        V = wl.random_block(w.N, k, seed=k)          # not tangent: the API projects
+        HV = ctx.hvp(dev(w.spins), dev(V)).cpu().numpy()
+        assert rel_l2(HV, sh.hvp(mdl, w.spins, V)) <= 1e-11
+        assert np.max(np.abs(np.sum(HV * w.spins[None], axis=2))) <= 1e-12     # output tangent
+
+
+def test_six_neighbour_table_equals_nearest_neighbour_kernels(moto):
+    # rcut = 1, Dz = 0 is the model of configs[0..3]: the table path must agree with the stencil kernels (generic and TMA)
+    for L, path in ((14, 1), (64, 2)):
+        base = wl.config1(L=L)
+        offs, J, D = wl.shell_table(1.0, Dz1=0.0)
+        w = wl.ShellWorkload("nn", L, L, 1, 1, offs, J, D, base.K, base.B, base.mu, 2, 0, base.spins)
+        nn = moto.spin_context(base, kmax=2)
+        nn.set_solver(hvp_path=path)
+        st = moto.shell_context(w, kmax=2)
+        x, V = dev(base.spins), dev(wl.random_block(base.N, 2, 4))
+        E0, g0 = nn.energy_grad(x)
+        E1, g1 = st.energy_grad(x)
+        assert abs(E0.item() - E1.item()) <= 1e-12 * abs(E0.item())
+        assert np.max(np.abs((g0 - g1).cpu().numpy())) <= 1e-12
+        assert rel_l2(st.hvp(x, V).cpu().numpy(), nn.hvp(x, V).cpu().numpy()) <= 1e-12
+        # n = 0 switches the table off again: bit-identical to the nearest-neighbour context?  J = D = 0 there, so compare
+        # against a context created with J, D and an emptied table instead
+        nn2 = moto.spin_context(base, kmax=2)
+        nn2.set_solver(hvp_path=path)
+        nn2.set_shells(offs, J, D)
+        nn2.set_shells(np.zeros((0, 2), np.int32), np.zeros(0), np.zeros((0, 3)))
+        assert np.array_equal(nn2.hvp(x, V).cpu().numpy(), nn.hvp(x, V).cpu().numpy())
+
+
+@pytest.mark.parametrize("method", [0, 1])
+def test_lowest_modes_vs_dense_oracle(moto, method):
+    w = wl.config_shells(L=18, rcut=3.0)
+    mdl = model_of(w)
+    lam_ref, V_ref = sh.lowest_modes(mdl, w.spins, 2, extra=1)
+    ctx = moto.shell_context(w, kmax=2)
+    ctx.set_solver(method=method)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=20000)
+    assert info["converged"]
+    lam, V = lam.cpu().numpy(), V.cpu().numpy()
+    assert np.max(np.abs(lam - lam_ref[:2]) / np.maximum(np.abs(lam_ref[:2]), 1e-3)) <= 1e-8
+    gap = lam_ref[2] - lam_ref[1]
+    ang = scipy.linalg.subspace_angles(V.reshape(2, -1).T, V_ref[:2].reshape(2, -1).T)
+    if gap > 1e-3:
+        assert np.max(ang) <= 1e-6
+    res = sh.hvp(mdl, w.spins, V) - lam[:, None, None] * V            # oracle-side residual of the GPU's pairs
+    assert np.max(np.linalg.norm(res.reshape(2, -1), axis=1)) <= 2e-9
+
+
+def test_mmf_step_and_relax_parity(moto):
+    w = wl.config_shells(L=14, rcut=3.0)
+    mdl = model_of(w)
+    lam, V = sh.lowest_modes(mdl, w.spins, 1)
+    ctx = moto.shell_context(w, kmax=2)
+    out, fn = ctx.mmf_step(dev(w.spins), dev(V), 0.05)
+    assert np.max(np.abs(out.cpu().numpy() - sh.mmf_step(mdl, w.spins, V, 0.05))) <= 1e-13
+    ops = ((lambda m: sh.energy(mdl, m)), (lambda m: sh.projected_gradient(mdl, m))) + ro.spin_ops(so.SpinModel(1, 1, 0, 0, 0, 0, 0, (0, 0, 0)))[2:]
+    ref, iref = ro.relax_downhill(*ops, w.spins, 6, 0.0, 0.05)
+    x = dev(w.spins)
+    info = ctx.relax(x, 6, 0.0, 0.05)
+    assert info["steps"] == 6 and info["evals"] == iref["evals"] and info["alpha"] == iref["alpha"]
+    assert abs(info["energy"] - iref["energy"]) <= 1e-12 * abs(iref["energy"])
+    assert np.max(np.abs(x.cpu().numpy() - ref)) <= 1e-11
+
+
+def test_full_size_366_neighbours(moto):
+    # the paper's workload class: 100 x 100 periodic, every shell within 10 lattice constants (366 neighbours)
+    w = wl.config_shells()
+    assert len(w.offsets) == 366 and w.N == 10000
+    mdl = model_of(w)
+    ctx = moto.shell_context(w, kmax=2)
+    x = dev(w.spins)
+    E, g = ctx.energy_grad(x)
+    assert abs(E.item() - sh.energy(mdl, w.spins)) <= 1e-12 * abs(E.item())
+    assert np.max(np.abs(g.cpu().numpy() - sh.projected_gradient(mdl, w.spins))) <= 1e-12
+    V = wl.random_block(w.N, 2, 8)
+    assert rel_l2(ctx.hvp(x, dev(V)).cpu().numpy(), sh.hvp(mdl, w.spins, V)) <= 1e-11
+    lam, Vm, info = ctx.lowest_modes(x, 2, tol=1e-8, max_iter=20000)
+    assert info["converged"]
+    lam, Vm = lam.cpu().numpy(), Vm.cpu().numpy()
+    res = sh.hvp(mdl, w.spins, Vm) - lam[:, None, None] * Vm
+    assert np.max(np.linalg.norm(res.reshape(2, -1), axis=1)) <= 2e-8
+    # "lowest-ness" at this size is not pinned (shift-invert on the 14.7 M-nonzero explicit Hessian takes minutes): it is
+    # checked with the same 366-neighbour table on a 36 x 36 lattice, where the dense oracle is exact
+    w2 = wl.config_shells(L=36)
+    mdl2 = model_of(w2)
+    lam_ref, V_ref = sh.lowest_modes(mdl2, w2.spins, 2, extra=1)
+    ctx2 = moto.shell_context(w2, kmax=2)
+    lam2, V2, info2 = ctx2.lowest_modes(dev(w2.spins), 2, tol=1e-9, max_iter=20000)
+    assert info2["converged"]
+    assert np.max(np.abs(lam2.cpu().numpy() - lam_ref[:2]) / np.maximum(np.abs(lam_ref[:2]), 1e-3)) <= 1e-8
+    if lam_ref[2] - lam_ref[1] > 1e-3:
+        assert np.max(scipy.linalg.subspace_angles(V2.cpu().numpy().reshape(2, -1).T, V_ref[:2].reshape(2, -1).T)) <= 1e-6
+
+
+def test_set_shells_errors(moto):
+    w = shell_workload(8, 8, (1, 1), 2.0, seed=1)
+    ctx = moto.shell_context(w, kmax=2)
+    lib = moto.load_library()
+    with pytest.raises(moto.binding.MotoError):
+        ctx.set_shells(w.offsets[:-1], w.Jd[:-1], w.Dd[:-1])                # inversion partner missing
+    D2 = w.Dd.copy(); D2[0, 2] += 0.1
+    with pytest.raises(moto.binding.MotoError):
+        ctx.set_shells(w.offsets, w.Jd, D2)                                 # D(-d) != -D(d)
+    with pytest.raises(moto.binding.MotoError):
+        ctx.set_shells(np.vstack([w.offsets, [[0, 0]]]), np.append(w.Jd, 1.0), np.vstack([w.Dd, [[0, 0, 0]]]))
+    assert lib.moto_set_shells(ctx._h, 513, None, None, None) == moto.binding.EINVAL
+    with pytest.raises(moto.binding.MotoError):                             # the Chebyshev building block needs the TMA path
+        ctx.cheb_apply(dev(w.spins), dev(wl.random_block(w.N, 1, 1)), 4, 0.0, 20.0, -1.0)
+    cart = moto.cart_context(wl.small_cluster(5, seed=2))
+    off = np.ascontiguousarray(w.offsets, np.int32)
+    assert lib.moto_set_shells(cart._h, len(off), off.ctypes.data, w.Jd.ctypes.data, np.ascontiguousarray(w.Dd).ctypes.data) == moto.binding.ESTATE
