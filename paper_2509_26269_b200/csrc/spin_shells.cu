@@ -22,17 +22,37 @@ __device__ __forceinline__ d3 cross3(d3 u, d3 D) { return mk3(u.y * D.z - u.z * 
 // neighbour site of (ix, iy) at table entry t, or -1 (open boundary)
 __device__ __forceinline__ long long shell_nb(const Lat& l, const ShellTab& tb, int t, int ix, int iy) {
     int jx = ix + tb.off[2 * t], jy = iy + tb.off[2 * t + 1];
-    if (jx < 0 || jx >= l.Lx) { if (!l.px) return -1; jx %= l.Lx; if (jx < 0) jx += l.Lx; }
-    if (jy < 0 || jy >= l.Ly) { if (!l.py) return -1; jy %= l.Ly; if (jy < 0) jy += l.Ly; }
+    if (jx < 0 || jx >= l.Lx) {      // one conditional add covers |dx| <= Lx; the division only runs for longer offsets
+        if (!l.px) return -1;
+        jx += jx < 0 ? l.Lx : -l.Lx;
+        if (jx < 0 || jx >= l.Lx) { jx %= l.Lx; if (jx < 0) jx += l.Lx; }
+    }
+    if (jy < 0 || jy >= l.Ly) {
+        if (!l.py) return -1;
+        jy += jy < 0 ? l.Ly : -l.Ly;
+        if (jy < 0 || jy >= l.Ly) { jy %= l.Ly; if (jy < 0) jy += l.Ly; }
+    }
     return (long long)jy * l.Lx + jx;
+}
+
+// the CTA's copy of the table in shared memory (20 KB at 512 entries): no dependent global loads in the neighbour loop
+struct ShellSmem { double jd[MOTO_MAX_SHELLS * 4]; int off[MOTO_MAX_SHELLS * 2]; };
+__device__ __forceinline__ ShellTab stage_table(const ShellTab& tb, ShellSmem& sm) {
+    for (int t = threadIdx.x; t < 4 * tb.n; t += blockDim.x) sm.jd[t] = tb.jd[t];
+    for (int t = threadIdx.x; t < 2 * tb.n; t += blockDim.x) sm.off[t] = tb.off[t];
+    __syncthreads();
+    ShellTab r; r.n = tb.n; r.off = sm.off; r.jd = sm.jd;
+    return r;
 }
 
 __device__ __forceinline__ d3 warp_sum3(d3 v) { return mk3(warp_sum(v.x), warp_sum(v.y), warp_sum(v.z)); }
 
 // energy partials + tangent-projected gradient (+ c)
-__global__ void __launch_bounds__(256) k_shell_energy_grad(Lat l, ShellTab tb, const double* __restrict__ m, double* __restrict__ g_out,
+__global__ void __launch_bounds__(256) k_shell_energy_grad(Lat l, ShellTab tbg, const double* __restrict__ m, double* __restrict__ g_out,
                                                            double* __restrict__ c_out, double* __restrict__ partials) {
     __shared__ double red[32];
+    __shared__ ShellSmem ssm;
+    const ShellTab tb = stage_table(tbg, ssm);
     const long long N = (long long)l.Lx * l.Ly;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double e[1] = {0.0};
@@ -77,12 +97,14 @@ __global__ void __launch_bounds__(1024) k_shell_final_sum(const double* __restri
 
 // block HVP.  PROJECT: API mode (neighbours projected, P_j v_j).  cvec == nullptr: c from the same pass over m.
 // CHEB: three-term epilogue out = alpha (Hess[v] - c0 v) + beta u (solver mode).
-template <bool PROJECT, bool CHEB>
-__global__ void __launch_bounds__(256) k_shell_hvp(Lat l, ShellTab tb, const double* __restrict__ m, const double* __restrict__ cvec,
+template <bool PROJECT, bool CHEB, int KT>   // KT: compile-time bound on k (1, 2 or MOTO_KMAX): accumulators and unrolling
+__global__ void __launch_bounds__(256) k_shell_hvp(Lat l, ShellTab tbg, const double* __restrict__ m, const double* __restrict__ cvec,
                                                    const double* __restrict__ V, int k, double* __restrict__ HV,
                                                    const int* __restrict__ done, double alpha, double c0, double beta,
                                                    const double* U) {
     if (done && *done) return;
+    __shared__ ShellSmem ssm;
+    const ShellTab tb = stage_table(tbg, ssm);
     const long long N = (long long)l.Lx * l.Ly;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const bool need_c = cvec == nullptr;
@@ -90,9 +112,11 @@ __global__ void __launch_bounds__(256) k_shell_hvp(Lat l, ShellTab tb, const dou
     for (long long i = (long long)blockIdx.x * 8 + warp; i < N; i += (long long)gridDim.x * 8) {
         const int iy = (int)(i / l.Lx), ix = (int)(i - (long long)iy * l.Lx);
         d3 accm = mk3(0.0, 0.0, 0.0);
-        d3 acc[MOTO_KMAX];
+        d3 acc[KT];
 #pragma unroll
-        for (int a = 0; a < MOTO_KMAX; ++a) acc[a] = mk3(0.0, 0.0, 0.0);
+        for (int a = 0; a < KT; ++a) acc[a] = mk3(0.0, 0.0, 0.0);
+        // (unrolling this loop by four with the absent neighbours predicated instead of skipped was slower, 46 -> 62 us at
+        //  k = 2: more registers, fewer resident warps)
         for (int t = lane; t < tb.n; t += 32) {
             const long long j = shell_nb(l, tb, t, ix, iy);
             if (j < 0) continue;
@@ -102,7 +126,7 @@ __global__ void __launch_bounds__(256) k_shell_hvp(Lat l, ShellTab tb, const dou
             if (PROJECT || need_c) mj = ld3(m, j);
             if (need_c) accm = add3(accm, axpy3(J, mj, cross3(mj, D)));
 #pragma unroll
-            for (int a = 0; a < MOTO_KMAX; ++a) {
+            for (int a = 0; a < KT; ++a) {
                 if (a < k) {
                     d3 vj = ld3(V + (size_t)a * 3 * N, j);
                     if (PROJECT) vj = proj3(mj, vj);
@@ -112,12 +136,12 @@ __global__ void __launch_bounds__(256) k_shell_hvp(Lat l, ShellTab tb, const dou
         }
         if (need_c) accm = warp_sum3(accm);
 #pragma unroll
-        for (int a = 0; a < MOTO_KMAX; ++a)
+        for (int a = 0; a < KT; ++a)
             if (a < k) acc[a] = warp_sum3(acc[a]);
         // lanes 0..k-1 finish one direction each (the sums are in every lane after the xor tree)
         d3 mine = mk3(0.0, 0.0, 0.0);
 #pragma unroll
-        for (int a = 0; a < MOTO_KMAX; ++a)
+        for (int a = 0; a < KT; ++a)
             if (a == lane) mine = acc[a];
         if (lane < k) {
             const d3 mi = ld3(m, i);
@@ -180,14 +204,17 @@ int shell_energy_grad(moto_ctx* c, const double* m, double* d_E, double* d_g, do
 
 int shell_hvp(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input, const int* d_done) {
     const int grid = shell_grid(c);
-    if (project_input) k_shell_hvp<true, false><<<grid, 256, 0, c->stream>>>(make_lat(c), tab_of(c), m, cvec, V, k, HV, d_done, 0.0, 0.0, 0.0, nullptr);
-    else k_shell_hvp<false, false><<<grid, 256, 0, c->stream>>>(make_lat(c), tab_of(c), m, cvec, V, k, HV, d_done, 0.0, 0.0, 0.0, nullptr);
+#define SHELL_HVP(P, KT) k_shell_hvp<P, false, KT><<<grid, 256, 0, c->stream>>>(make_lat(c), tab_of(c), m, cvec, V, k, HV, d_done, 0.0, 0.0, 0.0, nullptr)
+    if (project_input) { if (k == 1) SHELL_HVP(true, 1); else if (k == 2) SHELL_HVP(true, 2); else SHELL_HVP(true, MOTO_KMAX); }
+    else { if (k == 1) SHELL_HVP(false, 1); else if (k == 2) SHELL_HVP(false, 2); else SHELL_HVP(false, MOTO_KMAX); }
+#undef SHELL_HVP
     return 1;
 }
 
 int shell_three_term(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double alpha, double c0, double beta,
                      const double* U, double* out) {
-    k_shell_hvp<false, true><<<shell_grid(c), 256, 0, c->stream>>>(make_lat(c), tab_of(c), m, cvec, V, k, out, nullptr, alpha, c0, beta, U);
+    if (k <= 2) k_shell_hvp<false, true, 2><<<shell_grid(c), 256, 0, c->stream>>>(make_lat(c), tab_of(c), m, cvec, V, k, out, nullptr, alpha, c0, beta, U);
+    else k_shell_hvp<false, true, MOTO_KMAX><<<shell_grid(c), 256, 0, c->stream>>>(make_lat(c), tab_of(c), m, cvec, V, k, out, nullptr, alpha, c0, beta, U);
     return 1;
 }
 
