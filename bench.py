@@ -174,9 +174,13 @@ def run_report(args):
     rnd = wl.random_spins(1000, 1000, 7)
     cfgs.append(("R (random spins, PAPER.md:84)", wl.SpinWorkload("rand1000", 1000, 1000, 1, 1, 1.0, 0.3, 0.05, (0.0, 0.0, 0.02), 1.0, 2, 7, rnd,
                                                                     tol=1e-6), 0))
+    # the paper's real workload class: 100 x 100 periodic, couplings tabulated over every shell within 10 lattice
+    # constants (366 neighbours per site; synthetic table) -- SURVEY 8(f) f4, moto_set_shells
+    cfgs.append(("S (366-neighbour shells, PAPER.md:96)", wl.config_shells(), 0))
     for name, w, nsteps in cfgs:
         cart = hasattr(w, "positions")
-        ctx = moto.cart_context(w, kmax=w.k) if cart else moto.spin_context(w, kmax=w.k)
+        shells = hasattr(w, "offsets")
+        ctx = moto.cart_context(w, kmax=w.k) if cart else (moto.shell_context(w, kmax=w.k) if shells else moto.spin_context(w, kmax=w.k))
         if cart:
             ctx.set_solver(guard=2) if w.k + 2 <= ctx.kmax else None
         N = ctx.N
@@ -231,6 +235,12 @@ def run_report(args):
             if cart:
                 from oracle import cart_oracle as co
                 ops = ro.cart_ops(co.MorseModel(w.cell, w.De, w.alpha, w.r0, w.rc, w.fixed))
+            elif shells:
+                from oracle import shell_oracle as sho
+                from oracle import spin_oracle as so
+                smdl = sho.ShellModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.offsets, w.Jd, w.Dd, w.K, w.B, w.mu)
+                ops = ((lambda m_: sho.energy(smdl, m_)), (lambda m_: sho.projected_gradient(smdl, m_))) + \
+                    ro.spin_ops(so.SpinModel(1, 1, 0, 0, 0.0, 0.0, 0.0, (0.0, 0.0, 0.0)))[2:]
             else:
                 from oracle import spin_oracle as so
                 ops = ro.spin_ops(so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu))
@@ -250,6 +260,11 @@ def run_report(args):
                 t0 = time.perf_counter(); co.hvp(mdl, w.positions, V.cpu().numpy()); t_h = time.perf_counter() - t0
                 t0 = time.perf_counter(); lr, _ = co.lowest_modes(mdl, w.positions, w.k); t_s = time.perf_counter() - t0
                 how = "dense eigh 2421²"
+            elif shells:
+                from oracle import shell_oracle as sho
+                mdl = sho.ShellModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.offsets, w.Jd, w.Dd, w.K, w.B, w.mu)
+                t0 = time.perf_counter(); sho.hvp(mdl, w.spins, V.cpu().numpy()); t_h = time.perf_counter() - t0
+                lr, t_s, how = None, float("nan"), "not run (shift-invert on the 14.7 M-nonzero explicit Hessian: minutes); dense oracle parity at 36x36 in tests/test_gpu_shells.py"
             else:
                 from oracle import spin_oracle as so
                 mdl = so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
