@@ -132,6 +132,20 @@ moto_status moto_hvp(moto_ctx* ctx, const double* d_spins, const double* d_V, in
 moto_status moto_lowest_modes(moto_ctx* ctx, const double* d_spins, int k, double tol, int max_iter,
                               int warm_start, double* d_lambda, double* d_V, moto_solve_info* info);
 
+/* Population solve (Alg. 1 l.3-5: the explorer evaluates (lambda_1, lambda_2) once per candidate per
+ * generation, P = 24 in the paper): moto_lowest_modes on P independent problems at once.
+ * ctxs[p] are P DISTINCT contexts (same or different lattices), each created on its OWN stream -- on small lattices a solve is
+ * a chain of launch-latency-bound kernels, and the P chains overlap on the GPU only through separate streams (contexts that
+ * share a stream are still solved correctly, one after the other).  The library runs one host thread per context (at most 32
+ * at a time); every array argument is a HOST array of P device pointers / P structs, entry p with the meaning it has in
+ * moto_lowest_modes.  Inputs must be complete on the device before the call (the contexts' streams are not ordered against
+ * the stream that produced them).  statuses [P] (host, may be NULL) receives each problem's status; the return value is MOTO_OK,
+ * MOTO_ENOTCONV if some problem hit max_iter (and none failed), else the first failure.  Results are bit-identical to P
+ * separate moto_lowest_modes calls. */
+moto_status moto_lowest_modes_batch(moto_ctx* const* ctxs, int P, const double* const* d_spins, int k, double tol, int max_iter,
+                                    int warm_start, double* const* d_lambda, double* const* d_V, moto_solve_info* infos,
+                                    int32_t* statuses);
+
 /* One reflected-force step (Eq. 2; Alg. 1 l.11-12):
  * F = -grad (tangent-projected / masked), F_mmf = F - 2 sum_a (F.v_a) v_a over the kr columns given,
  * kind 0: m' = normalize(m + dt F_mmf) per site (retraction);  kind 1: x' = x + dt F_mmf.

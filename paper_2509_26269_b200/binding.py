@@ -76,6 +76,8 @@ _SIGS = {
     "moto_hvp": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
     "moto_lowest_modes": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
                                     C.POINTER(SolveInfo)]),
+    "moto_lowest_modes_batch": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
+                                          C.c_void_p, C.c_void_p]),
     "moto_mmf_step": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p, C.c_void_p]),
     "moto_hvp_three_term": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p,
                                       C.c_void_p, C.c_int]),
@@ -349,6 +351,33 @@ class Context:
         self._check(self.lib.moto_mmf_step_host(self._h, _ptr(h_spins), _ptr(h_v), h_v.shape[0], float(dt), _ptr(h_out),
                                                 _ptr(fn)))
         return h_out, float(fn[0])
+
+
+def lowest_modes_batch(ctxs, spins, k, tol, max_iter=200, V0=None, allow_notconv=False):
+    """moto_lowest_modes_batch over P contexts (each on its own stream) -> ([lam_p], [V_p], [info dict_p]).
+    Synchronises the device first: the contexts' streams are not ordered against the stream that produced the inputs."""
+    import torch
+    P = len(ctxs)
+    lib = load_library()
+    lams = [c._empty(k) for c in ctxs]
+    Vs = [(_dev_f64(V0[p], (k, c.N, 3)).clone() if V0 is not None else c._empty(k, c.N, 3)) for p, c in enumerate(ctxs)]
+    for p, c in enumerate(ctxs):
+        _dev_f64(spins[p], (c.N, 3))
+    torch.cuda.synchronize()
+    H = (C.c_void_p * P)(*[c._h for c in ctxs])
+    S = (C.c_void_p * P)(*[_ptr(s) for s in spins])
+    L = (C.c_void_p * P)(*[_ptr(t) for t in lams])
+    VV = (C.c_void_p * P)(*[_ptr(t) for t in Vs])
+    infos = (SolveInfo * P)()
+    sts = (C.c_int32 * P)()
+    st = lib.moto_lowest_modes_batch(H, P, S, k, float(tol), int(max_iter), 1 if V0 is not None else 0, L, VV, infos, sts)
+    for p, c in enumerate(ctxs):
+        c._check(sts[p], allow=(ENOTCONV,) if allow_notconv else ())
+    if st not in (OK, ENOTCONV):
+        raise MotoError(st, "moto_lowest_modes_batch failed")
+    out = [dict(iters=i.iters, converged=bool(i.converged), resid=list(i.resid)[:k], hvp_count=i.hvp_count, status=sts[p])
+           for p, i in enumerate(infos)]
+    return lams, Vs, out
 
 
 def spin_context(w, kmax=None, device="cuda:0", stream=None) -> Context:

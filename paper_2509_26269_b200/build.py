@@ -14,7 +14,7 @@ LIB = os.path.join(HERE, "libmoto.so")
 SOURCES = ["api.cu", "lobpcg.cu", "lobpcg_fast.cu", "block_algebra.cu", "rayleigh_ritz.cu", "lanczos.cu", "relax.cu", "spin_stencil.cu", "spin_stencil_tma.cu", "spin_shells.cu",
            "cart_morse.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math=false",
-              "-Xcompiler", "-fPIC,-O2", "-shared", "-cudart", "static"]
+              "-Xcompiler", "-fPIC,-O2", "-shared", "-cudart", "static", "-lpthread"]
 
 
 def _nvcc() -> str:

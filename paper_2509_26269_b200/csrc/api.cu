@@ -1,4 +1,7 @@
 // api.cu -- the C ABI of libmoto.so (include/moto.h): argument checks, workspace carving, dispatch.
+#include <atomic>
+#include <thread>
+#include <vector>
 #include <math.h>
 #include <stdlib.h>
 #include <new>
@@ -212,6 +215,39 @@ moto_status moto_lowest_modes(moto_ctx* c, const double* d_spins, int k, double 
     MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_lambda, c->st->theta, k * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
     return s;
+}
+
+// Population solve: P independent problems, one host thread per context (at most 32 at a time) so that their launch-latency-bound
+// kernel sequences overlap on the GPU through the contexts' own streams.
+moto_status moto_lowest_modes_batch(moto_ctx* const* ctxs, int P, const double* const* d_spins, int k, double tol, int max_iter,
+                                    int warm_start, double* const* d_lambda, double* const* d_V, moto_solve_info* infos,
+                                    int32_t* statuses) {
+    if (!ctxs || !d_spins || !d_lambda || !d_V || P < 1 || P > 4096) return MOTO_EINVAL;
+    for (int p = 0; p < P; ++p) {
+        if (!ctxs[p]) return MOTO_EINVAL;
+        for (int q = 0; q < p; ++q)
+            if (ctxs[q] == ctxs[p]) return moto_fail(ctxs[p], MOTO_EINVAL, "moto_lowest_modes_batch: the same context appears twice");
+    }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return MOTO_ECUDA;
+    std::vector<int32_t> st(P, (int32_t)MOTO_OK);
+    std::atomic<int> next(0);
+    auto worker = [&]() {
+        cudaSetDevice(dev);
+        for (int p = next.fetch_add(1); p < P; p = next.fetch_add(1))
+            st[p] = (int32_t)moto_lowest_modes(ctxs[p], d_spins[p], k, tol, max_iter, warm_start, d_lambda[p], d_V[p], infos ? infos + p : nullptr);
+    };
+    const int nthreads = P < 32 ? P : 32;
+    std::vector<std::thread> pool;
+    pool.reserve(nthreads);
+    for (int t = 0; t < nthreads; ++t) pool.emplace_back(worker);
+    for (auto& t : pool) t.join();
+    moto_status worst = MOTO_OK;
+    for (int p = 0; p < P; ++p) {
+        if (statuses) statuses[p] = st[p];
+        if (st[p] != MOTO_OK && (worst == MOTO_OK || worst == MOTO_ENOTCONV)) worst = (moto_status)st[p];
+    }
+    return worst;
 }
 
 moto_status moto_mmf_step(moto_ctx* c, const double* d_spins, const double* d_v, int kr, double dt, double* d_out, double* d_fnorm) {
