@@ -296,6 +296,32 @@ def run_report(args):
     print("| cfg | N | accepted steps | evaluations | ms | µs / evaluation | converged | final \\|g\\| | final E | oracle µs / evaluation |")
     print("|---|---|---|---|---|---|---|---|---|---|")
     print("\n".join(xrows))
+    # population solve (Alg. 1 l.3-5): P = 24 candidates, sequential calls vs moto_lowest_modes_batch
+    prow = []
+    for label, make, mk in (("70x70 nearest-neighbour (configs[1] recipe, seeds 3000..)", lambda p_: wl.config1(seed=3000 + p_), moto.spin_context),
+                            ("100x100, 366-neighbour shells (seeds 3000..)", lambda p_: wl.config_shells(seed=3000 + p_), moto.shell_context)):
+        P = 24
+        wsP = [make(p_) for p_ in range(P)]
+        ctxP = [mk(w_, kmax=2, stream=torch.cuda.Stream()) for w_ in wsP]
+        xsP = [torch.as_tensor(w_.spins, device=dev) for w_ in wsP]
+        t_seq = t_b = 0.0
+        for _ in range(2):
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            for c_, x_ in zip(ctxP, xsP):
+                c_.lowest_modes(x_, 2, tol=1e-8, max_iter=20000)
+            torch.cuda.synchronize(); t_seq = time.perf_counter() - t0
+        for _ in range(2):
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            _, _, infP = moto.lowest_modes_batch(ctxP, xsP, 2, 1e-8, max_iter=20000)
+            torch.cuda.synchronize(); t_b = time.perf_counter() - t0
+        prow.append(f"| {label} | {P} | {1e3 * t_seq:.1f} | {P / t_seq:.0f} | {1e3 * t_b:.1f} | {P / t_b:.0f} | {t_seq / t_b:.2f} | "
+                    f"{sum(i_['iters'] for i_ in infP)} | {'yes' if all(i_['converged'] for i_ in infP) else 'no'} |")
+        for c_ in ctxP:
+            c_.close()
+    print("\nPopulation solve (`moto_lowest_modes_batch`, k = 2, tol 1e-8, wall clock incl. host; one host thread and one stream per candidate):\n")
+    print("| workload | P | sequential ms | solves/s | batch ms | solves/s | speed-up | solver iterations (all) | all converged |")
+    print("|---|---|---|---|---|---|---|---|---|")
+    print("\n".join(prow))
     if orows:
         print(f"\nOracle on the host ({cores} BLAS threads, {os.cpu_count()} CPUs), as it stands — a baseline, not the target:\n")
         print("| cfg | oracle HVP ms (explicit Hessian rebuilt) | oracle lowest-k s | how | max rel. eigenvalue difference GPU vs oracle |")
