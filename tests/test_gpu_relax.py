@@ -156,3 +156,36 @@ def test_relax_full_size_properties(moto):
     gn = np.linalg.norm(so.projected_gradient(mdl, xh))
     assert abs(info["gnorm"] - gn) <= 1e-10 * gn
     assert np.max(np.abs(np.linalg.norm(xh, axis=1) - 1.0)) <= 1e-14
+
+
+def test_certified_edge_skyrmion_collapse(moto):
+    # The bilayer kernel + certification end to end (Alg. 1 l.9-18): moto_mmf_run climbs from a small
+    # skyrmion to the collapse saddle, moto_two_sided_descent relaxes both sides.  The saddle is an attractor of the MMF
+    # iteration and the minima of the descent, so GPU and oracle must arrive at the same three states: compare energies,
+    # curvatures and states to what the stopping tolerances allow; one minimum is the ferromagnet (closed-form energy).
+    w = wl.config1(L=12, R=2.0, sigma=0.0)
+    mdl = spin_model(w)
+    m_ref, lam_ref, steps_ref, conv_ref, fn_ref = so.mmf_run(mdl, w.spins, 2, 0.1, 4000, 1e-4)
+    assert conv_ref
+    ctx = moto.spin_context(w, kmax=2)
+    x = dev(w.spins)
+    V, info = ctx.mmf_run(x, 2, 0.1, 4000, 1e-4, tol=1e-9, max_iter=5000)
+    assert info["converged"] and info["fnorm"] <= 1e-4 and info["lam"][0] < 0.0 < info["lam"][1]
+    assert abs(info["steps"] - steps_ref) <= 2
+    xs = x.cpu().numpy()
+    assert np.max(np.abs(xs - m_ref)) <= 1e-2                                  # |dm| <~ tau_F / lambda_2 = 1e-4 / 0.038
+    assert abs(so.energy(mdl, xs) - so.energy(mdl, m_ref)) <= 1e-7 * abs(so.energy(mdl, m_ref))
+    assert np.max(np.abs(np.array(info["lam"]) - lam_ref) / np.abs(lam_ref)) <= 1e-3
+    # oracle-side check of the GPU's saddle: stationary for the reflected force, index 1
+    lam_chk, V_chk = so.lowest_modes(mdl, xs, 2)
+    assert np.linalg.norm(so.mmf_force(mdl, xs, V_chk[:1])) <= 1.1e-4 and lam_chk[0] < 0.0 < lam_chk[1]
+    xp, xm, infos = ctx.two_sided_descent(x, V[0].contiguous(), 0.1, 6000, 1e-6, 0.05)
+    res = ro.two_sided_descent(*ro.spin_ops(mdl), m_ref, V_chk[0], 0.1, 6000, 1e-6, 0.05)
+    E_gpu = sorted(i["energy"] for i in infos)
+    E_ref = sorted(i["energy"] for _, i in res)
+    assert all(i["converged"] for i in infos)
+    E_fm = -w.N * (6 * w.J + w.K + w.mu * w.B[2])
+    assert abs(E_gpu[0] - E_fm) <= 1e-9                                        # the ferromagnet, closed form
+    assert abs(E_gpu[1] - E_ref[1]) <= 1e-9 * abs(E_ref[1])                    # the skyrmion minimum
+    fm = (xp if infos[0]["energy"] < infos[1]["energy"] else xm).cpu().numpy()
+    assert np.max(np.abs(fm - np.array([0.0, 0.0, 1.0]))) <= 1e-5

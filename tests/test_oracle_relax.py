@@ -96,3 +96,23 @@ def test_two_sided_descent_spin_seeds_on_manifold():
         assert info["converged"] and info["energy"] < E0
         assert np.max(np.abs(np.linalg.norm(x, axis=1) - 1.0)) < 1e-14
         assert np.linalg.norm(so.projected_gradient(mdl, x)) <= 1e-6
+
+
+def test_certified_edge_skyrmion_collapse():
+    # Alg. 1 l.9-18 end to end on the oracle side: minimum-mode following from a small skyrmion climbs to the collapse saddle
+    # (lambda_1 < 0 < lambda_2, |F_mmf| <= tau_F), the two-sided descent from it ends in two different minima, one of which
+    # is the ferromagnet with the closed-form energy -N (6J + K + mu B).  12 x 12 periodic, configs[0] parameters.
+    w = wl.config1(L=12, R=2.0, sigma=0.0)
+    mdl = so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
+    m, lam, steps, conv, fn = so.mmf_run(mdl, w.spins, 2, 0.1, 4000, 1e-4)
+    assert conv and fn <= 1e-4 and lam[0] < 0.0 < lam[1]
+    E_saddle = so.energy(mdl, m)
+    lam2, V = so.lowest_modes(mdl, m, 2)
+    res = ro.two_sided_descent(*ro.spin_ops(mdl), m, V[0], 0.1, 6000, 1e-6, 0.05)
+    E = sorted(info["energy"] for _, info in res)
+    assert all(info["converged"] for _, info in res)
+    E_fm = -w.N * (6 * w.J + w.K + w.mu * w.B[2])
+    assert abs(E[0] - E_fm) < 1e-9                       # one branch: the ferromagnet (closed form)
+    assert E[1] < E_saddle - 1.0 and E[1] > E_fm + 1.0   # the other: a distinct minimum below the saddle (the skyrmion)
+    fm = min(res, key=lambda r: r[1]["energy"])[0]
+    assert np.max(np.abs(fm - np.array([0.0, 0.0, 1.0]))) < 1e-5
