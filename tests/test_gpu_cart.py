@@ -114,3 +114,42 @@ def test_mmf_run_cartesian_matches_stepwise_calls(moto, slab):
         lam, Vs, _ = ctx.lowest_modes(y, 2, tol=1e-9, max_iter=5000, V0=Vs)
     assert np.max(np.abs(x.cpu().numpy() - y.cpu().numpy())) <= 1e-9
     assert np.array_equal(x.cpu().numpy()[w.fixed == 1], w.positions[w.fixed == 1])
+
+
+def test_heptamer_certified_edge(moto, slab):
+    # The paper's portability case end to end (Alg. 1 l.9-18): relax the Ni(111) slab + heptamer to its
+    # reference minimum, displace the heptamer (seeded), climb with moto_mmf_run to an index-1 saddle, descend on both sides.
+    # The oracle cannot follow 2000 outer steps (a dense 2421^2 eigen-solve each), so it checks what is unique about the
+    # three end states: stationarity (its own gradient / reflected force), the index (its own dense eigenvalues, which must
+    # equal the GPU's), and that one branch returns to the reference minimum.
+    w, mdl = slab
+    ctx = moto.cart_context(w)
+    x = dev(w.positions)
+    rinfo = ctx.relax(x, 5000, 1e-6, 0.05)
+    assert rinfo["converged"]
+    x0 = x.clone()
+    rng = np.random.default_rng(5)
+    d = np.zeros_like(w.positions)
+    top = np.arange(w.Na - 7, w.Na)                       # the heptamer atoms
+    d[top] = 0.15 * rng.standard_normal((7, 3))
+    d[top, 2] *= 0.2
+    x = x0 + dev(d)
+    V, info = ctx.mmf_run(x, 2, 0.04, 6000, 1e-4, tol=1e-8, max_iter=5000)
+    assert info["converged"] and info["lam"][0] < 0.0 < info["lam"][1]
+    xs = x.cpu().numpy()
+    lam_ref, V_ref = co.lowest_modes(mdl, xs, 2)
+    assert lam_ref[0] < 0.0 < lam_ref[1]
+    assert np.max(np.abs(np.array(info["lam"]) - lam_ref) / np.abs(lam_ref)) <= 1e-6
+    assert np.linalg.norm(co.mmf_force(mdl, xs, V_ref[:1])) <= 1.1e-4
+    E_saddle, E_min = co.energy(mdl, xs), co.energy(mdl, x0.cpu().numpy())
+    assert abs(E_min - rinfo["energy"]) <= 1e-11 * abs(E_min)
+    assert 0.05 < E_saddle - E_min < 1.0                  # a barrier of a few tenths of an eV
+    xp, xm, infos = ctx.two_sided_descent(x, V[0].contiguous(), 0.1, 8000, 1e-6, 0.05)
+    assert all(i["converged"] for i in infos)
+    ends = sorted(zip([i["energy"] for i in infos], [xp.cpu().numpy(), xm.cpu().numpy()]), key=lambda t: t[0])
+    for E, y in ends:
+        assert np.linalg.norm(co.gradient(mdl, y)) <= 1.1e-6 and abs(co.energy(mdl, y) - E) <= 1e-11 * abs(E)
+        assert E < E_saddle - 0.01
+        assert np.all(y[w.fixed == 1] == w.positions[w.fixed == 1])
+    assert abs(ends[0][0] - E_min) <= 1e-9 and np.max(np.abs(ends[0][1] - x0.cpu().numpy())) <= 1e-4   # back to the reference minimum
+    assert np.max(np.abs(ends[1][1] - x0.cpu().numpy())) > 0.5                                          # a different minimum
