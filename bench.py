@@ -324,10 +324,10 @@ def run_report(args):
     print("\n".join(prow))
     # the bilayer kernel + certification end to end (Alg. 1 l.9-18): climb to an index-1 saddle, descend on both sides
     erows = []
-    def edge(label, ctx_, x_, dt_, tauF):
+    def edge(label, ctx_, x_, dt_, tauF, cap=8000):
         torch.cuda.synchronize(); t0 = time.perf_counter()
         E0, _ = ctx_.energy_grad(x_)
-        Vs_, mi = ctx_.mmf_run(x_, 2, dt_, 8000, tauF, tol=1e-8 if tauF < 1e-3 else 1e-7, max_iter=5000)
+        Vs_, mi = ctx_.mmf_run(x_, 2, dt_, cap, tauF, tol=1e-8 if cap == 8000 else 1e-6, max_iter=20000)
         torch.cuda.synchronize(); t_m = time.perf_counter() - t0
         Es, _ = ctx_.energy_grad(x_)
         if mi["converged"]:
@@ -337,7 +337,7 @@ def run_report(args):
             ends = f"{inf2[0]['energy']:.6f} ({inf2[0]['steps']} steps), {inf2[1]['energy']:.6f} ({inf2[1]['steps']} steps)"
         else:
             t_d, ends = float("nan"), "—"
-        erows.append(f"| {label} | {mi['steps']} | {'yes' if mi['converged'] else 'no (cap 8000)'} | {mi['fnorm']:.1e} | {mi['lam'][0]:.4f}, {mi['lam'][1]:.4f} | "
+        erows.append(f"| {label} | {mi['steps']} | {'yes' if mi['converged'] else f'no (cap {cap})'} | {mi['fnorm']:.1e} | {mi['lam'][0]:.4f}, {mi['lam'][1]:.4f} | "
                      f"{Es.item():.6f} | {1e3 * t_m:.0f} | {mi['hvp_count']} | {ends} | {1e3 * t_d:.0f} |")
     for L_ in (12, 64):
         w_ = wl.config1(L=L_, R=2.0, sigma=0.0)
@@ -351,6 +351,10 @@ def run_report(args):
     d_ = np.zeros_like(w_.positions); top_ = np.arange(w_.Na - 7, w_.Na)
     d_[top_] = 0.15 * np.random.default_rng(5).standard_normal((7, 3)); d_[top_, 2] *= 0.2
     edge("Ni(111) heptamer (configs[4] relaxed, adatoms displaced sigma = 0.15 A, seed 5), dt = 0.04, tau_F = 1e-4", c_, x_ + torch.as_tensor(d_, device=dev), 0.04, 1e-4)
+    c_.close()
+    w_ = wl.config3()
+    c_ = moto.spin_context(w_, kmax=2)
+    edge("configs[3] (10^6 spins, 200 skyrmions): 200 outer steps, dt = 0.05, tol 1e-6 (tau_F = 0: never stops early)", c_, torch.as_tensor(w_.spins, device=dev), 0.05, 0.0, cap=200)
     c_.close()
     print("\nBilayer kernel + certification end to end (`moto_mmf_run` -> `moto_two_sided_descent`, Alg. 1 l.9-18; wall clock incl. host):\n")
     print("| start | outer MMF steps | saddle test met | \\|F_mmf\\| | λ₁, λ₂ at the end | E at the end | climb ms | HVPs | energies of the two descents | descent ms |")

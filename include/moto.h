@@ -161,6 +161,10 @@ moto_status moto_mmf_step(moto_ctx* ctx, const double* d_spins, const double* d_
  *            x <- R(x + dt F_mmf)                                        (retraction for spins)
  * d_state [N][3] in/out; d_V [k][N][3]: start block if warm_start, holds the modes at the final x on return; k >= 2
  * (the test needs lambda_2).  info->steps = updates applied, info->converged = the test held at the returned x.
+ * With the block LOBPCG solver the per-step re-solve converges v_1 only (the reflected force needs nothing else); the other
+ * k-1 columns are iterated and warm-started with it as guard columns, which leaves a Ritz value theta_2 >= lambda_2.  All k
+ * columns are converged to tol where lambda_2 decides -- when ||F_mmf|| <= tau_F with lambda_1 < 0 < theta_2, and at the last
+ * step -- so the test and the returned eigenvalues always use converged pairs.  (Lanczos: all k columns every step.)
  * Returns MOTO_ENOTCONV if max_steps was reached without the test holding (outputs valid), or the solver's status if an
  * inner solve failed.  Synchronises the stream once per step (two scalars and k eigenvalues come back). */
 typedef struct {

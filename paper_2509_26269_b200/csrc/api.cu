@@ -260,6 +260,27 @@ moto_status moto_mmf_step(moto_ctx* c, const double* d_spins, const double* d_v,
     return MOTO_OK;
 }
 
+// Re-solve for moto_mmf_run: a block of kb columns is iterated and warm-started as a whole, but only the first one has to
+// meet tol (the reflected force needs v_1 alone, Eq. 2; lambda_2 is only needed for the sign test at the very end).  The other
+// columns ride along as guard columns: they speed up v_1 (its convergence then depends on the gap to lambda_{kb+1}) and leave
+// Ritz values theta_2.. >= lambda_2.. in d_lambda.  Block LOBPCG only.
+static moto_status solve_first_column(moto_ctx* c, const double* d_state, int kb, double tol, int max_iter, int warm, double* d_lambda,
+                                      double* d_V, moto_solve_info* info) {
+    const size_t bytes = (size_t)kb * c->N * 3 * sizeof(double);
+    if (warm) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->X, d_V, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    const int guard0 = c->opts.guard;
+    c->opts.guard = kb - 1;
+    c->keep_guard = warm;
+    moto_status s = solve_internal(c, d_state, 1, tol, max_iter, warm, info);
+    c->opts.guard = guard0;
+    c->keep_guard = 0;
+    if (s != MOTO_OK && s != MOTO_ENOTCONV) return s;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_V, c->X, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_lambda, c->st->theta, kb * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return s;
+}
+
 moto_status moto_mmf_run(moto_ctx* c, double* d_state, int k, double dt, int max_steps, double tau_F, double tol, int max_iter,
                          int warm_start, double* d_V, moto_mmf_info* info) {
     if (!c) return MOTO_EINVAL;
@@ -273,21 +294,34 @@ moto_status moto_mmf_run(moto_ctx* c, double* d_state, int k, double dt, int max
     moto_mmf_info out; memset(&out, 0, sizeof(out));
     moto_status st = MOTO_OK;
     int warm = warm_start;
+    // block LOBPCG: per step only v_1 is converged (solve_first_column); all k columns are converged where lambda_2 decides
+    const bool first_only = c->opts.method == 0 && max_iter > 0;
     for (int step = 0;; ++step) {
         moto_solve_info si;
-        st = moto_lowest_modes(c, d_state, k, tol, max_iter, warm, d_lam, d_V, &si);
-        out.hvp_count += si.hvp_count; out.solver_iters += si.iters;
+        bool full = !first_only;
+        st = first_only ? solve_first_column(c, d_state, k, tol, max_iter, warm, d_lam, d_V, &si)
+                        : moto_lowest_modes(c, d_state, k, tol, max_iter, warm, d_lam, d_V, &si);
+        for (;;) {
+            out.hvp_count += si.hvp_count; out.solver_iters += si.iters;
+            if (st != MOTO_OK && st != MOTO_ENOTCONV) break;
+            MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_lam, d_lam, k * sizeof(double), cudaMemcpyDeviceToHost, c->stream));   // before the step reuses scal
+            // candidate update into the staging vector; ||F_mmf|| of the CURRENT state comes with it
+            st = moto_mmf_step(c, d_state, d_V, 1, dt, c->stage_m, d_fn);
+            if (st != MOTO_OK) break;
+            MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&h_fn, d_fn, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+            MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+            // the cheap solve left theta_2 >= lambda_2: the saddle test can only hold if theta_2 > 0; then (and on the last
+            // step, so that the returned eigenvalues are the converged ones) all k columns are converged and the test redone
+            const bool need_full = !full && ((h_fn <= tau_F && h_lam[0] < 0.0 && h_lam[1] > 0.0) || step >= max_steps);
+            if (!need_full) break;
+            st = moto_lowest_modes(c, d_state, k, tol, max_iter, 1, d_lam, d_V, &si);
+            full = true;
+        }
         if (st != MOTO_OK && st != MOTO_ENOTCONV) break;
-        MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_lam, d_lam, k * sizeof(double), cudaMemcpyDeviceToHost, c->stream));   // before the step reuses scal
-        // candidate update into the staging vector; ||F_mmf|| of the CURRENT state comes with it
-        st = moto_mmf_step(c, d_state, d_V, 1, dt, c->stage_m, d_fn);
-        if (st != MOTO_OK) break;
-        MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&h_fn, d_fn, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-        MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
         out.fnorm = h_fn;
         for (int a = 0; a < k; ++a) out.lambda[a] = h_lam[a];
         out.steps = step;
-        if (h_fn <= tau_F && h_lam[0] < 0.0 && h_lam[1] > 0.0) { out.converged = 1; st = MOTO_OK; break; }
+        if (full && h_fn <= tau_F && h_lam[0] < 0.0 && h_lam[1] > 0.0) { out.converged = 1; st = MOTO_OK; break; }
         if (step >= max_steps) { st = moto_fail(c, MOTO_ENOTCONV, "moto_mmf_run: max_steps reached before the saddle test held"); break; }
         MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_state, c->stage_m, vb, cudaMemcpyDeviceToDevice, c->stream));
         moto_status t = moto_transport(c, d_state, d_V, k);

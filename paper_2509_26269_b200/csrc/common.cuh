@@ -85,6 +85,7 @@ struct moto_ctx {
     double* partials;  // [MOTO_RED_BLOCKS][2*NS*NS] grid-reduction partials
     SolverState* st;
     CartLists cl;
+    int keep_guard;    // internal: a warm start also carries the guard columns (moto_mmf_run's v_1-only re-solves)
     int nsh;           // > 0: general neighbour shells (moto_set_shells) replace the nearest-neighbour J, D of sp
     int* sh_off;       // [MOTO_MAX_SHELLS][2] device
     double* sh_jd;     // [MOTO_MAX_SHELLS][4] device: J, Dx, Dy, Dz

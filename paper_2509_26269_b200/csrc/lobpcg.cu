@@ -133,7 +133,7 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     int nmax = 0;
     if (degree > 0) f.n += fast_negc_max(c, pmax, &nmax);
     if (!warm_start) f.n += block_random(c, c->X, kb, c->opts.seed);
-    else if (kb > k) f.n += block_random(c, c->X + (size_t)k * bs, kb - k, c->opts.seed ^ 0x5bd1e995u);
+    else if (kb > k && !c->keep_guard) f.n += block_random(c, c->X + (size_t)k * bs, kb - k, c->opts.seed ^ 0x5bd1e995u);
     f.n += project_block(c, d_state, c->X, kb);
     fast_phase_start(f);
 
@@ -233,7 +233,7 @@ static moto_status lobpcg_solve_generic_filtered(moto_ctx* c, const double* d_st
     MOTO_CUDA_CHECK(c, cudaMemsetAsync(c->st, 0, sizeof(SolverState), c->stream));
     n += fast_negc_max(c, pmax, &nmax);
     if (!warm_start) n += block_random(c, c->X, kb, c->opts.seed);
-    else if (kb > k) n += block_random(c, c->X + (size_t)k * bs, kb - k, c->opts.seed ^ 0x5bd1e995u);
+    else if (kb > k && !c->keep_guard) n += block_random(c, c->X + (size_t)k * bs, kb - k, c->opts.seed ^ 0x5bd1e995u);
     n += project_block(c, d_state, c->X, kb);
     const int nblk = gram_blocks(c);
     n += gen_phase_start(c, d_state, kb, k, tol, 0, nblk);
@@ -308,7 +308,7 @@ moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, 
 
     // start block
     if (!warm_start) n += block_random(c, c->X, kb, c->opts.seed);
-    else if (kb > k) {  // guard columns are always fresh
+    else if (kb > k && !c->keep_guard) {  // guard columns are fresh unless the caller warm-starts them too (moto_mmf_run)
         n += block_random(c, c->X + (size_t)k * bs, kb - k, c->opts.seed ^ 0x5bd1e995u);
     }
     n += project_block(c, d_state, c->X, kb);
