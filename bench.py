@@ -324,10 +324,13 @@ def run_report(args):
     print("\n".join(prow))
     # the bilayer kernel + certification end to end (Alg. 1 l.9-18): climb to an index-1 saddle, descend on both sides
     erows = []
-    def edge(label, ctx_, x_, dt_, tauF, cap=8000):
+    def edge(label, ctx_, x_, dt_, tauF, cap=8000, cg=None):
         torch.cuda.synchronize(); t0 = time.perf_counter()
         E0, _ = ctx_.energy_grad(x_)
-        Vs_, mi = ctx_.mmf_run(x_, 2, dt_, cap, tauF, tol=1e-8 if cap == 8000 else 1e-6, max_iter=20000)
+        if cg:
+            Vs_, mi = ctx_.mmf_run_cg(x_, 2, cg[0], cg[1], cap, tauF, tol=1e-8, max_iter=20000)
+        else:
+            Vs_, mi = ctx_.mmf_run(x_, 2, dt_, cap, tauF, tol=1e-8 if cap == 8000 else 1e-6, max_iter=20000)
         torch.cuda.synchronize(); t_m = time.perf_counter() - t0
         Es, _ = ctx_.energy_grad(x_)
         if mi["converged"]:
@@ -343,6 +346,7 @@ def run_report(args):
         w_ = wl.config1(L=L_, R=2.0, sigma=0.0)
         c_ = moto.spin_context(w_, kmax=2)
         edge(f"skyrmion collapse, {L_}x{L_} periodic (configs[1] recipe, R = 2, no noise), dt = 0.1, tau_F = 1e-4", c_, torch.as_tensor(w_.spins, device=dev), 0.1, 1e-4)
+        edge(f"same start, CG step rule (`moto_mmf_run_cg`, delta = 0.05, s_max = 1)", c_, torch.as_tensor(w_.spins, device=dev), 0.0, 1e-4, cap=2000, cg=(0.05, 1.0))
         c_.close()
     w_ = wl.config4()
     c_ = moto.cart_context(w_)
@@ -351,6 +355,7 @@ def run_report(args):
     d_ = np.zeros_like(w_.positions); top_ = np.arange(w_.Na - 7, w_.Na)
     d_[top_] = 0.15 * np.random.default_rng(5).standard_normal((7, 3)); d_[top_, 2] *= 0.2
     edge("Ni(111) heptamer (configs[4] relaxed, adatoms displaced sigma = 0.15 A, seed 5), dt = 0.04, tau_F = 1e-4", c_, x_ + torch.as_tensor(d_, device=dev), 0.04, 1e-4)
+    edge("same start, CG step rule (`moto_mmf_run_cg`, delta = 0.02, s_max = 0.3)", c_, x_ + torch.as_tensor(d_, device=dev), 0.0, 1e-4, cap=2000, cg=(0.02, 0.3))
     c_.close()
     w_ = wl.config3()
     c_ = moto.spin_context(w_, kmax=2)

@@ -178,6 +178,20 @@ typedef struct {
 moto_status moto_mmf_run(moto_ctx* ctx, double* d_state, int k, double dt, int max_steps, double tau_F, double tol, int max_iter,
                          int warm_start, double* d_V, moto_mmf_info* info);
 
+/* The same outer loop with a conjugate-gradient step rule (Alg. 1 l.12: "x <- R_x(x + alpha F_mmf)  > Lbfgs/CG", PAPER.md:262;
+ * SURVEY 8(f) f2).  F_mmf is not the gradient of a function, so there is no energy line search; reading A28 is the
+ * translation step of the dimer method: Polak-Ribiere+ conjugate directions on the reflected force with a one-trial secant
+ * line search on the force component along the direction,
+ *   dh = d/|d|, f0 = F_mmf(x).dh;  trial x_t = R(x + delta dh), f1 = F_mmf(x_t).dh;  C = (f0 - f1)/delta;
+ *   s = f0/C if C > 0 else smax, clipped to [-smax, smax];  x <- R(x + s dh);
+ *   beta = max(0, F_new.(F_new - F)/(F.F));  d <- F_new + beta T(d)      (T: tangent projection for spins, identity for atoms)
+ * i.e. two minimum-mode solves per iteration (v_1-only re-solves as in moto_mmf_run) instead of one, and an order of
+ * magnitude fewer iterations.  delta: trial displacement, smax: largest displacement per iteration, both in the 2-norm of
+ * the whole configuration.  d_scratch: caller-owned device scratch [4][N][3].  Other arguments, outputs, termination test
+ * and return values as moto_mmf_run; info->steps counts iterations. */
+moto_status moto_mmf_run_cg(moto_ctx* ctx, double* d_state, int k, double delta, double smax, int max_steps, double tau_F, double tol,
+                            int max_iter, int warm_start, double* d_V, double* d_scratch, moto_mmf_info* info);
+
 /* Two-sided minimum-mode descent (Alg. 1 l.15-18; Suppl. Note 1 b(iii)).
  * moto_relax: "RelaxDownHill" with a deterministic optimiser.  The paper names the class ("L-BFGS/CG") and nothing else;
  *   this is Riemannian Polak-Ribiere+ conjugate gradients with backtracking (reading A26):

@@ -87,6 +87,8 @@ _SIGS = {
     "moto_relax": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double, C.POINTER(RelaxInfo)]),
     "moto_two_sided_descent": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_double, C.c_double,
                                          C.c_void_p, C.c_void_p, C.POINTER(RelaxInfo)]),
+    "moto_mmf_run_cg": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
+                                  C.c_void_p, C.c_void_p, C.POINTER(MmfInfo)]),
     "moto_transport": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "moto_gram": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
     "moto_rayleigh_ritz": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
@@ -286,6 +288,20 @@ class Context:
         info = MmfInfo()
         st = self._check(self.lib.moto_mmf_run(self._h, _ptr(state), k, float(dt), int(max_steps), float(tau_F), float(tol),
                                                int(max_iter), warm, _ptr(V), C.byref(info)), allow=(ENOTCONV,))
+        return V, dict(steps=info.steps, converged=bool(info.converged), fnorm=info.fnorm, lam=list(info.lam)[:k],
+                       hvp_count=info.hvp_count, solver_iters=info.solver_iters, status=st)
+
+    def mmf_run_cg(self, state, k, delta, smax, max_steps, tau_F, tol, max_iter=20000, V0=None):
+        """moto_mmf_run_cg: outer MMF loop with the CG step rule; `state` is updated in place.  -> (V, info dict)."""
+        _dev_f64(state, (self.N, 3))
+        if V0 is not None:
+            V, warm = _dev_f64(V0, (k, self.N, 3)).clone(), 1
+        else:
+            V, warm = self._empty(k, self.N, 3), 0
+        scratch = self._empty(4, self.N, 3)
+        info = MmfInfo()
+        st = self._check(self.lib.moto_mmf_run_cg(self._h, _ptr(state), k, float(delta), float(smax), int(max_steps), float(tau_F),
+                                                  float(tol), int(max_iter), warm, _ptr(V), _ptr(scratch), C.byref(info)), allow=(ENOTCONV,))
         return V, dict(steps=info.steps, converged=bool(info.converged), fnorm=info.fnorm, lam=list(info.lam)[:k],
                        hvp_count=info.hvp_count, solver_iters=info.solver_iters, status=st)
 

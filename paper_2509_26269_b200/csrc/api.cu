@@ -264,7 +264,7 @@ moto_status moto_mmf_step(moto_ctx* c, const double* d_spins, const double* d_v,
 // meet tol (the reflected force needs v_1 alone, Eq. 2; lambda_2 is only needed for the sign test at the very end).  The other
 // columns ride along as guard columns: they speed up v_1 (its convergence then depends on the gap to lambda_{kb+1}) and leave
 // Ritz values theta_2.. >= lambda_2.. in d_lambda.  Block LOBPCG only.
-static moto_status solve_first_column(moto_ctx* c, const double* d_state, int kb, double tol, int max_iter, int warm, double* d_lambda,
+static moto_status solve_first_column_impl(moto_ctx* c, const double* d_state, int kb, double tol, int max_iter, int warm, double* d_lambda,
                                       double* d_V, moto_solve_info* info) {
     const size_t bytes = (size_t)kb * c->N * 3 * sizeof(double);
     if (warm) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->X, d_V, bytes, cudaMemcpyDeviceToDevice, c->stream));
@@ -299,7 +299,7 @@ moto_status moto_mmf_run(moto_ctx* c, double* d_state, int k, double dt, int max
     for (int step = 0;; ++step) {
         moto_solve_info si;
         bool full = !first_only;
-        st = first_only ? solve_first_column(c, d_state, k, tol, max_iter, warm, d_lam, d_V, &si)
+        st = first_only ? solve_first_column_impl(c, d_state, k, tol, max_iter, warm, d_lam, d_V, &si)
                         : moto_lowest_modes(c, d_state, k, tol, max_iter, warm, d_lam, d_V, &si);
         for (;;) {
             out.hvp_count += si.hvp_count; out.solver_iters += si.iters;
@@ -330,6 +330,16 @@ moto_status moto_mmf_run(moto_ctx* c, double* d_state, int k, double dt, int max
     }
     if (info) *info = out;
     return st;
+}
+
+moto_status moto_mmf_run_cg(moto_ctx* c, double* d_state, int k, double delta, double smax, int max_steps, double tau_F, double tol,
+                            int max_iter, int warm_start, double* d_V, double* d_scratch, moto_mmf_info* info) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_state || !d_V || !d_scratch) return moto_fail(c, MOTO_EINVAL, "moto_mmf_run_cg: null argument");
+    if (k < 2 || k > c->kmax) return moto_fail(c, MOTO_EINVAL, "moto_mmf_run_cg: k out of range [2, kmax] (the saddle test needs lambda_2)");
+    if (!(tol > 0) || max_iter < 0 || max_steps < 0 || !(tau_F >= 0) || !(delta > 0) || !(smax > 0))
+        return moto_fail(c, MOTO_EINVAL, "moto_mmf_run_cg: bad tolerance, cap or step length");
+    return mmf_cg_run(c, d_state, k, delta, smax, max_steps, tau_F, tol, max_iter, warm_start, d_V, d_scratch, info);
 }
 
 moto_status moto_relax(moto_ctx* c, double* d_state, int max_steps, double tau_F, double alpha0, moto_relax_info* info) {
@@ -501,3 +511,9 @@ moto_status moto_mmf_step_host(moto_ctx* c, const double* h_spins, const double*
 }
 
 }  // extern "C"
+
+// C++-linkage entry for relax.cu (moto_mmf_run_cg)
+moto_status solve_first_column(moto_ctx* c, const double* d_state, int kb, double tol, int max_iter, int warm, double* d_lambda, double* d_V,
+                               moto_solve_info* info) {
+    return solve_first_column_impl(c, d_state, kb, tol, max_iter, warm, d_lambda, d_V, info);
+}

@@ -85,6 +85,7 @@ struct moto_ctx {
     double* partials;  // [MOTO_RED_BLOCKS][2*NS*NS] grid-reduction partials
     SolverState* st;
     CartLists cl;
+    double* fmmf_out;  // internal: when set, moto_mmf_step also writes the reflected force F_mmf [N][3] there (moto_mmf_run_cg)
     int keep_guard;    // internal: a warm start also carries the guard columns (moto_mmf_run's v_1-only re-solves)
     int nsh;           // > 0: general neighbour shells (moto_set_shells) replace the nearest-neighbour J, D of sp
     int* sh_off;       // [MOTO_MAX_SHELLS][2] device
@@ -168,6 +169,10 @@ moto_status lanczos_solve(moto_ctx*, const double* d_state, int k, double tol, i
                           moto_solve_info* info);
 // relax.cu
 moto_status relax_run(moto_ctx*, double* d_state, int max_steps, double tau_F, double alpha0, moto_relax_info* info);
+moto_status mmf_cg_run(moto_ctx*, double* d_state, int k, double delta, double smax, int max_steps, double tau_F, double tol, int max_iter,
+                       int warm_start, double* d_V, double* d_scratch, moto_mmf_info* info);
+moto_status solve_first_column(moto_ctx*, const double* d_state, int kb, double tol, int max_iter, int warm, double* d_lambda, double* d_V,
+                               moto_solve_info* info);   // api.cu
 moto_status relax_seed(moto_ctx*, const double* d_saddle, const double* d_v, double s_eta, double* d_out);
 // lobpcg.cu
 moto_status lobpcg_solve(moto_ctx*, const double* d_state, int k, double tol, int max_iter, int warm_start,

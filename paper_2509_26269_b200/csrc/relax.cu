@@ -29,9 +29,9 @@ __global__ void __launch_bounds__(256) k_relax_trial(long long N, const double* 
     }
 }
 
-// d <- -g_t + beta T(d)
+// d <- sg g_t + beta T(d)   (sg = -1: descent on the gradient, moto_relax;  sg = +1: g_t is a force, moto_mmf_run_cg)
 __global__ void __launch_bounds__(256) k_relax_dir(long long N, const double* __restrict__ xt, const double* __restrict__ gt, double beta,
-                                                   double* __restrict__ d, int project) {
+                                                   double* __restrict__ d, int project, double sg = -1.0) {
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
         d3 di = mk3(0.0, 0.0, 0.0);
         if (beta != 0.0) {                       // beta == 0: d may be uninitialised, never read it
@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(256) k_relax_dir(long long N, const double* __
             if (project) di = proj3(ld3(xt, i), di);
         }
         d3 g = ld3(gt, i);
-        st3(d, i, mk3(fma(beta, di.x, -g.x), fma(beta, di.y, -g.y), fma(beta, di.z, -g.z)));
+        st3(d, i, mk3(fma(beta, di.x, sg * g.x), fma(beta, di.y, sg * g.y), fma(beta, di.z, sg * g.z)));
     }
 }
 
@@ -148,4 +148,109 @@ moto_status relax_seed(moto_ctx* c, const double* d_saddle, const double* d_v, d
     c->launches += 1;
     MOTO_CUDA_CHECK(c, cudaGetLastError());
     return MOTO_OK;
+}
+
+// ================================================================ outer MMF loop with a conjugate-gradient step rule
+// (Alg. 1 l.12 "Lbfgs/CG"; reading A28): PR+ conjugate directions on the reflected force, one-trial secant line
+// search on the force component along the direction (the translation step of the dimer method).  Two MinMode solves per
+// iteration (trial point, new point), v_1-only re-solves with warm-started guard columns as in moto_mmf_run.
+namespace {
+
+struct ForceEval { double lam[MOTO_KMAX]; double fn; };
+
+// F_mmf at y into F_out; V (k columns, modes at the previously evaluated point) is transported to y and re-solved
+moto_status eval_force(moto_ctx* c, const double* y, int k, double tol, int max_iter, int warm, int transport, double* d_V, double* F_out,
+                       bool full, ForceEval* fe, moto_mmf_info* acc) {
+    double* d_lam = c->st->scal;
+    double* d_fn = c->st->cheb_ab;
+    if (transport) { moto_status t = moto_transport(c, y, d_V, k); if (t != MOTO_OK) return t; }
+    moto_solve_info si;
+    moto_status s = (c->opts.method == 0 && !full && max_iter > 0) ? solve_first_column(c, y, k, tol, max_iter, warm, d_lam, d_V, &si)
+                                                                   : moto_lowest_modes(c, y, k, tol, max_iter, warm, d_lam, d_V, &si);
+    acc->hvp_count += si.hvp_count; acc->solver_iters += si.iters;
+    if (s != MOTO_OK && s != MOTO_ENOTCONV) return s;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(fe->lam, d_lam, k * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    c->fmmf_out = F_out;
+    s = moto_mmf_step(c, y, d_V, 1, 0.0, c->stage_m, d_fn);      // dt = 0: only the force and its norm are wanted
+    c->fmmf_out = nullptr;
+    if (s != MOTO_OK) return s;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&fe->fn, d_fn, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return MOTO_OK;
+}
+
+moto_status dots(moto_ctx* c, const double* a, const double* b0, const double* b1, const double* b2, int nb, double* h) {
+    const double* S[1] = {a};
+    const double* T[3] = {b0, b1 ? b1 : b0, b2 ? b2 : b0};
+    c->launches += block_gram(c, S, 1, T, nb, c->st->scal, nullptr);
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h, c->st->scal, nb * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return MOTO_OK;
+}
+
+}  // namespace
+
+moto_status mmf_cg_run(moto_ctx* c, double* d_state, int k, double delta, double smax, int max_steps, double tau_F, double tol, int max_iter,
+                       int warm_start, double* d_V, double* d_scratch, moto_mmf_info* info) {
+    const long long N = c->N;
+    const size_t n3 = (size_t)3 * N, vb = n3 * sizeof(double);
+    const int spin = c->kind == MOTO_KIND_TRI2D;
+    const int grid = grid_for(N);
+    double *F = d_scratch, *d = d_scratch + n3, *Fn = d_scratch + 2 * n3, *xt = d_scratch + 3 * n3;
+    moto_mmf_info out; memset(&out, 0, sizeof(out));
+    ForceEval fe;
+    moto_status st = eval_force(c, d_state, k, tol, max_iter, warm_start, 0, d_V, F, false, &fe, &out);
+    if (st != MOTO_OK) return st;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d, F, vb, cudaMemcpyDeviceToDevice, c->stream));
+    bool full = c->opts.method != 0;
+    moto_status ret = MOTO_OK;
+    double h[3];
+    for (int step = 0;; ++step) {
+        // saddle test; lambda_2 decides only on converged pairs (see moto_mmf_run)
+        if (!full && ((fe.fn <= tau_F && fe.lam[0] < 0.0 && fe.lam[1] > 0.0) || step >= max_steps)) {
+            st = eval_force(c, d_state, k, tol, max_iter, 1, 0, d_V, F, true, &fe, &out);
+            if (st != MOTO_OK) return st;
+            full = true;
+        }
+        out.steps = step; out.fnorm = fe.fn;
+        for (int a = 0; a < k; ++a) out.lambda[a] = fe.lam[a];
+        if (full && fe.fn <= tau_F && fe.lam[0] < 0.0 && fe.lam[1] > 0.0) { out.converged = 1; break; }
+        if (step >= max_steps) { ret = moto_fail(c, MOTO_ENOTCONV, "moto_mmf_run_cg: max_steps reached before the saddle test held"); break; }
+        full = c->opts.method != 0;
+        st = dots(c, F, F, d, nullptr, 2, h);                         // F.F, F.d
+        if (st != MOTO_OK) return st;
+        const double FF = h[0], Fd = h[1];
+        st = dots(c, d, d, nullptr, nullptr, 1, h);                   // d.d
+        if (st != MOTO_OK) return st;
+        const double dn = sqrt(h[0]);
+        if (!(dn > 0.0) || !(FF > 0.0)) { ret = moto_fail(c, MOTO_ESTATE, "moto_mmf_run_cg: zero force"); break; }
+        const double f0 = Fd / dn;
+        k_relax_trial<<<grid, 256, 0, c->stream>>>(N, d_state, d, delta / dn, xt, spin);
+        c->launches += 1;
+        ForceEval ft;
+        st = eval_force(c, xt, k, tol, max_iter, 1, 1, d_V, Fn, false, &ft, &out);
+        if (st != MOTO_OK) return st;
+        st = dots(c, Fn, d, nullptr, nullptr, 1, h);                  // F_t.d  (F_t is tangent at x_t: transporting d changes nothing)
+        if (st != MOTO_OK) return st;
+        const double f1 = h[0] / dn;
+        const double Cv = (f0 - f1) / delta;
+        double s = Cv > 0.0 ? f0 / Cv : smax;
+        s = s > smax ? smax : (s < -smax ? -smax : s);
+        k_relax_trial<<<grid, 256, 0, c->stream>>>(N, d_state, d, s / dn, d_state, spin);   // in place: element-wise
+        c->launches += 1;
+        st = eval_force(c, d_state, k, tol, max_iter, 1, 1, d_V, Fn, false, &fe, &out);
+        if (st != MOTO_OK) return st;
+        st = dots(c, Fn, Fn, F, nullptr, 2, h);                       // F_new.F_new, F_new.F
+        if (st != MOTO_OK) return st;
+        double beta = (h[0] - h[1]) / FF;
+        if (!(beta > 0.0)) beta = 0.0;
+        k_relax_dir<<<grid, 256, 0, c->stream>>>(N, d_state, Fn, beta, d, spin, 1.0);
+        c->launches += 1;
+        double* t = F; F = Fn; Fn = t;
+    }
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (info) *info = out;
+    return ret;
 }

@@ -256,7 +256,7 @@ __global__ void __launch_bounds__(256) k_mmf_pass1(Lat l, const double* __restri
 __global__ void __launch_bounds__(256) k_mmf_pass2(long long N, const double* __restrict__ m, const double* __restrict__ v, int kr,
                                                    const double* __restrict__ Fbuf, const double* __restrict__ alpha, double dt,
                                                    double* __restrict__ m_out, double* __restrict__ partials, int retract,
-                                                   const uint8_t* __restrict__ fixed) {
+                                                   const uint8_t* __restrict__ fixed, double* __restrict__ F_out) {
     __shared__ double red[32];
     double al[MOTO_KMAX];
 #pragma unroll
@@ -269,6 +269,7 @@ __global__ void __launch_bounds__(256) k_mmf_pass2(long long N, const double* __
             if (a < kr) F = axpy3(-2.0 * al[a], ld3(v + (size_t)a * 3 * N, i), F);
         if (fixed && fixed[i]) F = mk3(0.0, 0.0, 0.0);
         f2[0] += dot3(F, F);
+        if (F_out) st3(F_out, i, F);          // the reflected force itself (moto_mmf_run_cg)
         d3 x = axpy3(dt, F, ld3(m, i));
         if (retract) x = scale3(1.0 / sqrt(dot3(x, x)), x);
         st3(m_out, i, x);
@@ -346,7 +347,7 @@ int spin_mmf_step(moto_ctx* c, const double* m, const double* v, int kr, double 
     if (c->nsh > 0) n0 = shell_mmf_pass1(c, m, v, kr);
     else k_mmf_pass1<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, v, kr, c->g, c->partials);
     k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, MOTO_KMAX, MOTO_KMAX, alpha, 0);
-    k_mmf_pass2<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, m, v, kr, c->g, alpha, dt, m_out, c->partials, 1, nullptr);
+    k_mmf_pass2<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, m, v, kr, c->g, alpha, dt, m_out, c->partials, 1, nullptr, c->fmmf_out);
     int n = 2 + n0;
     if (d_fnorm) { k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_fnorm, 1); ++n; }
     return n;
@@ -356,7 +357,7 @@ int spin_mmf_step(moto_ctx* c, const double* m, const double* v, int kr, double 
 void launch_mmf_pass2(moto_ctx* c, const double* x, const double* v, int kr, const double* Fbuf, const double* alpha,
                       double dt, double* x_out, int retract) {
     k_mmf_pass2<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, x, v, kr, Fbuf, alpha, dt, x_out, c->partials, retract,
-                                                      c->lat.d_fixed);
+                                                      c->lat.d_fixed, c->fmmf_out);
 }
 void launch_final_sum(moto_ctx* c, const double* partials, int nblk, int stride, int nval, double* out, int take_sqrt) {
     k_final_sum<<<(nval + 127) / 128, 128, 0, c->stream>>>(partials, nblk, stride, nval, out, take_sqrt);

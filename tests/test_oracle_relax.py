@@ -116,3 +116,29 @@ def test_certified_edge_skyrmion_collapse():
     assert E[1] < E_saddle - 1.0 and E[1] > E_fm + 1.0   # the other: a distinct minimum below the saddle (the skyrmion)
     fm = min(res, key=lambda r: r[1]["energy"])[0]
     assert np.max(np.abs(fm - np.array([0.0, 0.0, 1.0]))) < 1e-5
+
+
+def test_cg_mmf_double_well_and_same_saddle_as_fixed_step():
+    # oracle/mmf_cg_oracle.py (outer loop with the CG step rule, reading A28).  (i) 2-D double well with the analytic Hessian as
+    # MinMode: from (0.4, 0.3) the loop must reach the index-1 saddle at the origin.  (ii) on the 12 x 12 lattice it must reach the
+    # saddle the fixed-step loop reaches (same energy and curvatures), in an order of magnitude fewer MinMode solves.
+    from oracle import mmf_cg_oracle as mc
+
+    def minmode(p):
+        lam, U = np.linalg.eigh(np.array([[12.0 * p[0] ** 2 - 4.0, 0.0], [0.0, 2.0]]))
+        return lam, U.T
+    force = lambda p: -np.array([4.0 * p[0] * (p[0] ** 2 - 1.0), 2.0 * p[1]])
+    x, lam, steps, conv, fn, evals = mc.mmf_run_cg(minmode, force, lambda x: x, lambda x, d: d, np.array([0.4, 0.3]), 0.01, 0.2, 100, 1e-10)
+    assert conv and steps < 20 and evals == 2 * steps + 1
+    assert np.max(np.abs(x)) < 1e-10 and abs(lam[0] + 4.0) < 1e-9 and abs(lam[1] - 2.0) < 1e-12
+    w = wl.config1(L=12, R=2.0, sigma=0.0)
+    mdl = so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
+    _, _, retract, transport = ro.spin_ops(mdl)
+    x, lam, steps, conv, fn, evals = mc.mmf_run_cg(lambda m: so.lowest_modes(mdl, m, 2), lambda m: -so.projected_gradient(mdl, m), retract,
+                                                   transport, w.spins, 0.05, 1.0, 400, 1e-4)
+    assert conv and fn <= 1e-4 and steps < 200
+    m_fix, lam_fix, steps_fix, conv_fix, _ = so.mmf_run(mdl, w.spins, 2, 0.1, 4000, 1e-4)
+    assert conv_fix and evals < steps_fix / 5
+    assert abs(so.energy(mdl, x) - so.energy(mdl, m_fix)) < 1e-6
+    assert np.max(np.abs(lam - lam_fix) / np.abs(lam_fix)) < 1e-3
+    assert np.max(np.abs(x - m_fix)) < 1e-2
