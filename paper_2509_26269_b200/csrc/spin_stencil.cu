@@ -149,14 +149,18 @@ __global__ void __launch_bounds__(1024) k_final_sum4(const double* __restrict__ 
     if (threadIdx.x < 4) out[threadIdx.x] = sm[threadIdx.x];
 }
 
-// out[j] = sum_b partials[b*stride + j]  (optionally sqrt); one thread per j, fixed order
-__global__ void k_final_sum(const double* __restrict__ partials, int nblk, int stride, int nval, double* __restrict__ out,
-                            int take_sqrt) {
-    int j = blockIdx.x * blockDim.x + threadIdx.x;
+// out[j] = sum_b partials[b*stride + j]  (optionally sqrt): one WARP per j (lanes stride over b, then a shuffle tree); fixed order.
+// Launch with FS_GRID(nval) blocks of 256 threads.  (One thread per j took 17 us for 296 partials, 40 us for the 1607
+// per-atom energies of the Cartesian path.)
+#define FS_GRID(nval) (((nval) + 7) / 8)
+__global__ void __launch_bounds__(256) k_final_sum(const double* __restrict__ partials, int nblk, int stride, int nval,
+                                                   double* __restrict__ out, int take_sqrt) {
+    const int j = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (j >= nval) return;
     double s = 0.0;
-    for (int b = 0; b < nblk; ++b) s += partials[(size_t)b * stride + j];
-    out[j] = take_sqrt ? sqrt(s) : s;
+    for (int b = lane; b < nblk; b += 32) s += partials[(size_t)b * stride + j];
+    s = warp_sum(s);
+    if (lane == 0) out[j] = take_sqrt ? sqrt(s) : s;
 }
 
 // ---------------------------------------------------------------- block HVP, generic path
@@ -286,7 +290,7 @@ int spin_energy_grad(moto_ctx* c, const double* m, double* d_E, double* d_g, dou
     Lat l = make_lat(c);
     k_energy_grad<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, d_g, d_c, c->partials);
     int n = 1;
-    if (d_E) { k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_E, 0); ++n; }
+    if (d_E) { k_final_sum<<<FS_GRID(1), 256, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_E, 0); ++n; }
     return n;
 }
 
@@ -346,10 +350,10 @@ int spin_mmf_step(moto_ctx* c, const double* m, const double* v, int kr, double 
     int n0 = 1;
     if (c->nsh > 0) n0 = shell_mmf_pass1(c, m, v, kr);
     else k_mmf_pass1<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, v, kr, c->g, c->partials);
-    k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, MOTO_KMAX, MOTO_KMAX, alpha, 0);
+    k_final_sum<<<FS_GRID(MOTO_KMAX), 256, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, MOTO_KMAX, MOTO_KMAX, alpha, 0);
     k_mmf_pass2<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, m, v, kr, c->g, alpha, dt, m_out, c->partials, 1, nullptr, c->fmmf_out);
     int n = 2 + n0;
-    if (d_fnorm) { k_final_sum<<<1, 32, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_fnorm, 1); ++n; }
+    if (d_fnorm) { k_final_sum<<<FS_GRID(1), 256, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_fnorm, 1); ++n; }
     return n;
 }
 
@@ -360,5 +364,5 @@ void launch_mmf_pass2(moto_ctx* c, const double* x, const double* v, int kr, con
                                                       c->lat.d_fixed, c->fmmf_out);
 }
 void launch_final_sum(moto_ctx* c, const double* partials, int nblk, int stride, int nval, double* out, int take_sqrt) {
-    k_final_sum<<<(nval + 127) / 128, 128, 0, c->stream>>>(partials, nblk, stride, nval, out, take_sqrt);
+    k_final_sum<<<FS_GRID(nval), 256, 0, c->stream>>>(partials, nblk, stride, nval, out, take_sqrt);
 }
