@@ -60,3 +60,17 @@ def test_batch_mixed_lattices_notconv_and_errors(moto):
     assert lib.moto_lowest_modes_batch(H, 2, S, 2, 1e-8, 10, 0, S, S, None, None) == moto.binding.EINVAL    # same context twice
     assert lib.moto_lowest_modes_batch(None, 2, S, 2, 1e-8, 10, 0, S, S, None, None) == moto.binding.EINVAL
     assert lib.moto_lowest_modes_batch(H, 0, S, 2, 1e-8, 10, 0, S, S, None, None) == moto.binding.EINVAL
+
+
+def test_batch_more_problems_than_threads(moto):
+    # P = 40 > 32 host threads: the worker queue must hand every problem out exactly once
+    import torch
+    ws = [wl.config0(seed=5000 + p) for p in range(40)]
+    ctxs = [moto.spin_context(w, kmax=2, stream=torch.cuda.Stream()) for w in ws]
+    xs = [dev(w.spins) for w in ws]
+    lams, Vs, infos = moto.lowest_modes_batch(ctxs, xs, 2, 1e-9, max_iter=5000)
+    for p, w in enumerate(ws):
+        mdl = so.SpinModel(w.Lx, w.Ly, w.pbc_x, w.pbc_y, w.J, w.D, w.K, w.B, w.mu)
+        lam_ref, _ = so.lowest_modes(mdl, w.spins, 2)
+        assert infos[p]["converged"]
+        assert np.max(np.abs(lams[p].cpu().numpy() - lam_ref) / np.maximum(np.abs(lam_ref), 1e-3)) <= 1e-8
