@@ -201,7 +201,8 @@ moto_status moto_mmf_run_cg(moto_ctx* ctx, double* d_state, int k, double delta,
  *     direction);  alpha <- 2a if the first trial was accepted, else a.  g = tangent-projected / masked gradient.
  *   d_state [N][3] in/out (unit spins / positions).  Stops when ||g||_2 <= tau_F (MOTO_OK, converged = 1), after
  *   max_steps accepted steps or when no step along -g is acceptable (MOTO_ENOTCONV; d_state = best iterate, info valid).
- *   alpha0 > 0: first trial step.  Synchronises the stream once per trial (four scalars come back).  Uses the solver
+ *   alpha0 > 0: first trial step.  Spin lattices: the accept/reject decisions are taken on the device, the host looks at the
+ *   state once per eight trials; atoms (and general shells): one synchronisation per trial (four scalars come back).  Uses the solver
  *   blocks of the workspace as scratch: modes left there by an earlier solve are overwritten (user arrays are not).
  * moto_two_sided_descent: seeds x_saddle + s eta v_min, s = +1 then -1 (retracted for spins), each relaxed as above into
  *   d_min_plus / d_min_minus [N][3] (must not alias the inputs or each other); info[2] (host, may be NULL) in that order.

@@ -40,6 +40,19 @@ struct SolverState {
     long long nhvp;  // single-vector HVP applications so far
 };
 
+// Device-resident line-search state of moto_relax on spin lattices (relax.cu): the accept/reject decision of a trial is taken by
+// k_relax_decide, the next trial reads its step, buffers and direction mode from here -- no host look per trial.
+struct RelaxDev {
+    double E, gg, slope, alpha, a, beta, tau;
+    int cur, gcur;        // current state buffer (0 = the caller's array, 1, 2 = workspace), current gradient buffer (0, 1)
+    int steepest, first, bt, steps, evals, max_steps;
+    int status;           // 0 running, 1 converged, 2 max_steps, 3 stalled, 4 NaN
+    int dir_mode;         // what k_relax_dir does next: 0 nothing, 1 d <- -g + beta T(d), 2 d <- -g
+    double* x[3];
+    double* g[2];
+    double* d;
+};
+
 struct HostStatus {  // pinned mirror of the control block + residuals
     double theta[MOTO_KMAX];
     double resid[MOTO_KMAX];
@@ -120,6 +133,8 @@ int spin_hvp(moto_ctx*, const double* m, const double* c_or_null, const double* 
 int spin_mmf_step(moto_ctx*, const double* m, const double* v, int kr, double dt, double* m_out, double* d_fnorm);
 int spin_project(moto_ctx*, const double* m, double* V, int k);
 int spin_relax_eval(moto_ctx*, const double* x, const double* d, double a, const double* g_old, double* xt, double* gt, double* d_out4);
+int spin_relax_nblk(const moto_ctx*);
+int spin_relax_eval_dev(moto_ctx*, const RelaxDev* rs, int* nblk_out);   // trial described by the device state; partials left in ctx->partials
 int spin_hvp_three_term_generic(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double alpha, double c0,
                                 double beta, const double* U, double* out);
 // spin_stencil_tma.cu

@@ -8,7 +8,9 @@
 // Every vector operation runs on the device.  Spins: a trial is ONE fused pass (k_relax_eval in spin_stencil.cu: retraction
 // recomputed at the site and its neighbours, stencil gradient, projection and the four sums E_t, g_t.g_t, g_t.g, g_t.d;
 // 120 B/site) plus the direction update (96 B/site) once a step is accepted.  Atoms: trial kernel, neighbour lists + K7
-// gradient, one Gram launch.  The host sees four scalars per trial and takes the accept/reject decision.
+// gradient, one Gram launch, and the host reads four scalars per trial and decides.  On spin lattices the decision is taken
+// on the device as well (k_relax_decide, same arithmetic): eval -> decide -> direction update are enqueued eight trials at a
+// time and the host only looks at the state between batches (relax_run_device).
 #include "common.cuh"
 #include "device_utils.cuh"
 
@@ -77,9 +79,122 @@ moto_status eval_point(moto_ctx* c, const double* x, const double* d, double a, 
 
 }  // namespace
 
+// ---------------------------------------------------------------- device-resident line search (spin lattices, fused trial kernel)
+namespace {
+
+// sums the four partial columns of the last evaluation, then ONE thread takes the decision the host loop of relax_run_host
+// takes (same arithmetic, same order), and leaves the next trial's description in *rs
+__global__ void __launch_bounds__(1024) k_relax_decide(const double* __restrict__ partials, int nblk, RelaxDev* rs, int init) {
+    __shared__ double sm[1024];
+    if (rs->status) return;
+    const int j = threadIdx.x & 3, r = threadIdx.x >> 2;
+    double s = 0.0;
+    for (int b = r; b < nblk; b += 256) s += partials[(size_t)b * 4 + j];
+    sm[threadIdx.x] = s;
+    __syncthreads();
+    for (int off = 512; off >= 4; off >>= 1) {
+        if (threadIdx.x < off) sm[threadIdx.x] += sm[threadIdx.x + off];
+        __syncthreads();
+    }
+    if (threadIdx.x != 0) return;
+    if (init) {
+        rs->E = sm[0]; rs->gg = sm[1]; rs->slope = -sm[1];
+        rs->a = rs->alpha; rs->steepest = 1; rs->first = 1; rs->bt = 0; rs->evals = 1; rs->steps = 0;
+        rs->dir_mode = 2;
+    } else {
+        rs->evals += 1;
+        const double Et = sm[0], gtgt = sm[1], gtg = sm[2], gtd = sm[3], a = rs->a, E = rs->E, slope = rs->slope;
+        const bool acc = gtd <= RELAX_SIGMA * fabs(slope) && (Et <= E + RELAX_C1 * a * slope || Et <= E + RELAX_EPS_E * fabs(E));
+        if (acc) {
+            double beta = (gtgt - gtg) / rs->gg;
+            if (!(beta > 0.0)) beta = 0.0;
+            double new_slope = -gtgt + beta * gtd;
+            if (new_slope >= 0.0) { beta = 0.0; new_slope = -gtgt; }
+            rs->beta = beta; rs->steepest = beta == 0.0;
+            rs->cur = rs->cur == 1 ? 2 : 1; rs->gcur ^= 1;
+            rs->E = Et; rs->gg = gtgt; rs->slope = new_slope;
+            rs->alpha = rs->first ? 2.0 * a : a;
+            rs->steps += 1;
+            rs->a = rs->alpha; rs->first = 1; rs->bt = 0;
+            rs->dir_mode = 1;
+        } else {
+            rs->a = 0.5 * a; rs->first = 0; rs->bt += 1; rs->dir_mode = 0;
+            if (rs->bt >= RELAX_MAX_BACKTRACKS) {
+                if (rs->steepest) { rs->status = 3; return; }
+                rs->dir_mode = 2; rs->slope = -rs->gg; rs->steepest = 1; rs->a = rs->alpha; rs->first = 1; rs->bt = 0;
+            }
+            return;
+        }
+    }
+    const double gg = rs->gg;
+    if (!(gg == gg)) rs->status = 4;
+    else if (sqrt(gg) <= rs->tau) rs->status = 1;
+    else if (rs->steps >= rs->max_steps) rs->status = 2;
+}
+
+__global__ void __launch_bounds__(256) k_relax_dir_dev(long long N, const RelaxDev* __restrict__ rs) {
+    const int mode = rs->dir_mode;
+    if (mode == 0 || rs->status) return;
+    const double* __restrict__ xt = rs->x[rs->cur];
+    const double* __restrict__ gt = rs->g[rs->gcur];
+    double* __restrict__ d = rs->d;
+    const double beta = mode == 1 ? rs->beta : 0.0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        d3 di = mk3(0.0, 0.0, 0.0);
+        if (beta != 0.0) di = proj3(ld3(xt, i), ld3(d, i));
+        const d3 g = ld3(gt, i);
+        st3(d, i, mk3(fma(beta, di.x, -g.x), fma(beta, di.y, -g.y), fma(beta, di.z, -g.z)));
+    }
+}
+
+}  // namespace
+
+// Spin lattices with the fused trial kernel: a trial is eval -> decide -> (direction update) with nothing coming back to the
+// host; the host enqueues eight trials at a time and then looks at the state once.
+static moto_status relax_run_device(moto_ctx* c, double* d_state, int max_steps, double tau_F, double alpha0, moto_relax_info* info, int nblk) {
+    const long long N = c->N;
+    const size_t vb = (size_t)N * 3 * sizeof(double);
+    const int grid = grid_for(N);
+    RelaxDev* rs = reinterpret_cast<RelaxDev*>(c->st->lz_T);   // solver scratch: no solve runs during a relaxation
+    static_assert(sizeof(RelaxDev) <= sizeof(double) * MOTO_LZ_MAX * MOTO_LZ_MAX, "RelaxDev does not fit its scratch");
+    RelaxDev h; memset(&h, 0, sizeof(h));
+    h.alpha = alpha0; h.tau = tau_F; h.max_steps = max_steps;
+    h.x[0] = d_state; h.x[1] = c->stage_m; h.x[2] = c->P; h.g[0] = c->g; h.g[1] = c->W; h.d = c->AW;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(rs, &h, sizeof(h), cudaMemcpyHostToDevice, c->stream));
+    c->launches += spin_relax_eval(c, d_state, nullptr, 0.0, nullptr, nullptr, c->g, c->st->scal);
+    k_relax_decide<<<1, 1024, 0, c->stream>>>(c->partials, nblk, rs, 1);
+    k_relax_dir_dev<<<grid, 256, 0, c->stream>>>(N, rs);
+    c->launches += 2;
+    for (;;) {
+        MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&h, rs, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+        MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+        if (h.status) break;
+        for (int b = 0; b < 8; ++b) {
+            int nb = 0;
+            c->launches += spin_relax_eval_dev(c, rs, &nb);
+            k_relax_decide<<<1, 1024, 0, c->stream>>>(c->partials, nb, rs, 0);
+            k_relax_dir_dev<<<grid, 256, 0, c->stream>>>(N, rs);
+            c->launches += 2;
+        }
+        MOTO_CUDA_CHECK(c, cudaGetLastError());
+    }
+    if (h.cur != 0) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_state, h.x[h.cur], vb, cudaMemcpyDeviceToDevice, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (info) {
+        memset(info, 0, sizeof(*info));
+        info->steps = h.steps; info->converged = h.status == 1; info->evals = h.evals;
+        info->energy = h.E; info->gnorm = sqrt(h.gg); info->alpha = h.alpha;
+    }
+    if (h.status == 1) return MOTO_OK;
+    if (h.status == 2) return moto_fail(c, MOTO_ENOTCONV, "moto_relax: max_steps reached");
+    if (h.status == 3) return moto_fail(c, MOTO_ENOTCONV, "moto_relax: stalled (no acceptable step along -g)");
+    return moto_fail(c, MOTO_ESTATE, "moto_relax: NaN gradient");
+}
+
 // d_state in/out.  Scratch (no solver is running): g, g_t = ctx->g / W (swapped on acceptance), d = AW, and the current and
 // trial states ping-pong between stage_m and P, so an accepted step costs no copy; d_state is written once at the end.
 moto_status relax_run(moto_ctx* c, double* d_state, int max_steps, double tau_F, double alpha0, moto_relax_info* info) {
+    if (const int nblk = spin_relax_nblk(c)) return relax_run_device(c, d_state, max_steps, tau_F, alpha0, info, nblk);
     const long long N = c->N;
     const size_t vb = (size_t)N * 3 * sizeof(double);
     const int spin = c->kind == MOTO_KIND_TRI2D;

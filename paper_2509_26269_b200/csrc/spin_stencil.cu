@@ -84,9 +84,15 @@ __global__ void __launch_bounds__(256) k_energy_grad(Lat l, const double* __rest
 template <bool TRIAL>
 __global__ void __launch_bounds__(RT_W * RT_H) k_relax_eval(Lat l, const double* __restrict__ x, const double* __restrict__ d, double a,
                                                             const double* __restrict__ g_old, double* __restrict__ xt_out,
-                                                            double* __restrict__ gt_out, double* __restrict__ partials) {
+                                                            double* __restrict__ gt_out, double* __restrict__ partials,
+                                                            const RelaxDev* __restrict__ rs = nullptr) {
     __shared__ double tile[RT_H + 2][RT_W + 2][3];
     __shared__ double red[32 * 4];
+    if (rs) {   // device-resident line search: the trial is described by the state k_relax_decide left
+        if (rs->status) return;
+        x = rs->x[rs->cur]; xt_out = rs->x[rs->cur == 1 ? 2 : 1]; d = rs->d; a = rs->a;
+        g_old = rs->g[rs->gcur]; gt_out = rs->g[rs->gcur ^ 1];
+    }
     const int tx0 = blockIdx.x * RT_W, ty0 = blockIdx.y * RT_H;
     for (int cell = threadIdx.x; cell < (RT_W + 2) * (RT_H + 2); cell += RT_W * RT_H) {
         const int ly = cell / (RT_W + 2), lx = cell - ly * (RT_W + 2);
@@ -304,6 +310,24 @@ int spin_relax_eval(moto_ctx* c, const double* x, const double* d, double a, con
     else k_relax_eval<false><<<grid, RT_W * RT_H, 0, c->stream>>>(l, x, nullptr, 0.0, nullptr, nullptr, gt, c->partials);
     k_final_sum4<<<1, 1024, 0, c->stream>>>(c->partials, (int)(grid.x * grid.y), d_out4);
     return 2;
+}
+
+// number of CTAs (= rows of partials) of the fused trial kernel, 0 if it does not apply to this context
+int spin_relax_nblk(const moto_ctx* c) {
+    if (c->kind != MOTO_KIND_TRI2D || c->nsh > 0) return 0;
+    const long long gx = (c->lat.Lx + RT_W - 1) / RT_W, gy = (c->lat.Ly + RT_H - 1) / RT_H;
+    if ((size_t)gx * gy * 4 > (size_t)MOTO_RED_BLOCKS * 2 * MOTO_NS * MOTO_NS || gy > 65535) return 0;
+    return (int)(gx * gy);
+}
+
+int spin_relax_eval_dev(moto_ctx* c, const RelaxDev* rs, int* nblk_out) {
+    if (c->nsh > 0) return 0;
+    Lat l = make_lat(c);
+    dim3 grid((l.Lx + RT_W - 1) / RT_W, (l.Ly + RT_H - 1) / RT_H);
+    if ((size_t)grid.x * grid.y * 4 > (size_t)MOTO_RED_BLOCKS * 2 * MOTO_NS * MOTO_NS || grid.y > 65535) return 0;
+    k_relax_eval<true><<<grid, RT_W * RT_H, 0, c->stream>>>(l, nullptr, nullptr, 0.0, nullptr, nullptr, nullptr, c->partials, rs);
+    *nblk_out = (int)(grid.x * grid.y);
+    return 1;
 }
 
 int spin_curvature(moto_ctx* c, const double* m, double* d_c) { return spin_energy_grad(c, m, nullptr, nullptr, d_c); }
