@@ -11,10 +11,12 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmoto.so")
-SOURCES = ["api.cu", "lobpcg.cu", "lobpcg_fast.cu", "block_algebra.cu", "rayleigh_ritz.cu", "lanczos.cu", "relax.cu", "spin_stencil.cu", "spin_stencil_tma.cu", "spin_shells.cu",
-           "cart_morse.cu"]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math=false",
-              "-Xcompiler", "-fPIC,-O2", "-shared", "-cudart", "static", "-lpthread"]
+SOURCES = ["api.cu", "lobpcg.cu", "lobpcg_fast.cu", "block_algebra.cu", "rayleigh_ritz.cu", "lanczos.cu", "relax.cu", "spin_stencil.cu", "spin_stencil_tma.cu",
+           "spin_cheb2_tma.cu", "spin_shells.cu", "cart_morse.cu"]
+ARCH_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a"]
+COMPILE_FLAGS = ARCH_FLAGS + ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-O2"]
+LINK_FLAGS = ARCH_FLAGS + ["-shared", "-cudart", "static", "-lpthread"]
+OBJ_DIR = os.path.join(HERE, "build")   # git-ignored
 
 
 def _nvcc() -> str:
@@ -33,16 +35,29 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """One nvcc -c per translation unit (in parallel), then one link into libmoto.so."""
     if not force and not needs_build():
         return LIB
-    flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
-    cmd = [_nvcc()] + flags + (["-Xptxas", "-v"] if verbose else []) + [os.path.join(CSRC, s) for s in SOURCES] + \
-          ["-o", LIB]
+    from concurrent.futures import ThreadPoolExecutor
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    nvcc = _nvcc()
+
+    def compile_one(src):
+        obj = os.path.join(OBJ_DIR, src + ".o")
+        cmd = [nvcc] + COMPILE_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
+        return obj, r.stderr
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 4)) as ex:
+        results = list(ex.map(compile_one, SOURCES))
+    if verbose:
+        print("".join(err for _, err in results))
+    cmd = [nvcc] + LINK_FLAGS + [obj for obj, _ in results] + ["-o", LIB]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
-    if verbose:
-        print(r.stderr)
+        raise RuntimeError("nvcc link failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
     return LIB
 
 

@@ -3,7 +3,6 @@
 #include <thread>
 #include <vector>
 #include <math.h>
-#include <stdlib.h>
 #include <new>
 #include "common.cuh"
 
@@ -62,7 +61,7 @@ static WsLayout ws_layout(const moto_lattice* lat, int kmax) {
     w.partials = al256((size_t)MOTO_RED_BLOCKS * 2 * MOTO_NS * MOTO_NS * sizeof(double));
     w.st = al256(sizeof(SolverState));
     w.cart = lat->kind == MOTO_KIND_CARTESIAN ? cart_lists_bytes(lat) : 0;
-    w.nblocks = lat->kind == MOTO_KIND_TRI2D ? 8 : 6;   // spin lattices: + two Chebyshev ping-pong blocks
+    w.nblocks = lat->kind == MOTO_KIND_TRI2D ? 10 : 6;   // spin lattices: + four rotating blocks of the Chebyshev recurrence
     w.flags = 4096;
     w.shell = lat->kind == MOTO_KIND_TRI2D ? al256((size_t)MOTO_MAX_SHELLS * (2 * sizeof(int) + 4 * sizeof(double))) : 0;
     w.total = w.nblocks * w.block + w.c + w.g + w.stage + w.partials + w.st + w.flags + w.shell + w.cart;
@@ -111,7 +110,10 @@ moto_status moto_create(const moto_lattice* lat, const void* params, void* d_wor
     c->X = (double*)p; p += w.block;  c->AX = (double*)p; p += w.block;
     c->W = (double*)p; p += w.block;  c->AW = (double*)p; p += w.block;
     c->P = (double*)p; p += w.block;  c->AP = (double*)p; p += w.block;
-    if (w.nblocks == 8) { c->T1 = (double*)p; p += w.block; c->T2 = (double*)p; p += w.block; }
+    if (w.nblocks == 10) {
+        c->T1 = (double*)p; p += w.block; c->T2 = (double*)p; p += w.block;
+        c->T3 = (double*)p; p += w.block; c->T4 = (double*)p; p += w.block;
+    }
     c->c = (double*)p; p += w.c;
     c->g = (double*)p; p += w.g;
     c->stage_m = (double*)p; p += w.stage;
@@ -145,6 +147,7 @@ moto_status moto_set_solver(moto_ctx* c, const moto_solver_opts* o) {
     if (!c || !o) return MOTO_EINVAL;
     if (o->guard < 0 || o->check_every < 0 || o->precond_degree < -1 || o->hvp_path < 0 || o->hvp_path > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: negative option");
     if (o->method < 0 || o->method > 1 || o->ncv < 0 || o->ncv > MOTO_LZ_MAX) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: method must be 0 or 1, ncv in 0..24");
+    if (o->cheb_mode < 0 || o->cheb_mode > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: cheb_mode must be 0, 1 or 2");
     moto_solver_opts n = *o;
     if (n.check_every == 0) n.check_every = 8;
     if (n.seed == 0) n.seed = 0x9E3779B97F4A7C15ull;
@@ -409,19 +412,9 @@ moto_status moto_cheb_apply(moto_ctx* c, const double* d_spins, const double* d_
     int n = refresh_c ? spin_curvature(c, d_spins, c->c) : 0;
     MOTO_CUDA_CHECK(c, cudaMemsetAsync(&c->st->done, 0, 4 * sizeof(int), c->stream));
     n += fast_cheb_coef_explicit(c, d, a, b, a_L);
-    // MOTO_NO_MULTISTEP: test hook, forces one launch per step (the multi-step == step-wise test compares the two)
-    int nk = (d >= 2 && !getenv("MOTO_NO_MULTISTEP")) ? spin_cheb_multistep(c, d_spins, c->c, d_V, k, d, d_out, &c->st->cheb[0][0], nullptr) : 0;
-    if (nk > 0) n += nk;
-    else {
-        const double* in = d_V; const double* prev = nullptr;
-        for (int i = 1; i <= d; ++i) {
-            double* out = (i == d) ? d_out : ((i & 1) ? c->T1 : c->T2);
-            int m = spin_hvp_tma_ex(c, d_spins, c->c, in, k, out, nullptr, nullptr, 1, 0.0, 0.0, 0.0, prev, &c->st->cheb[i - 1][0]);
-            if (m <= 0) return moto_fail(c, MOTO_ESTATE, "moto_cheb_apply: needs the TMA K1 path (even Lx >= 8; hvp_path != 1)");
-            n += m;
-            prev = in; in = out;
-        }
-    }
+    const int nk = spin_cheb_recurrence(c, d_spins, c->c, d_V, k, d, d_out, &c->st->cheb[0][0], nullptr);
+    if (nk <= 0) return moto_fail(c, MOTO_ESTATE, "moto_cheb_apply: needs the TMA K1 path (even Lx >= 8; hvp_path != 1)");
+    n += nk;
     c->launches += n;
     MOTO_CUDA_CHECK(c, cudaGetLastError());
     return MOTO_OK;

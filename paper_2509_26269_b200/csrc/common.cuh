@@ -88,10 +88,12 @@ struct moto_ctx {
     int nblocks;
     // workspace views
     double *X, *AX, *W, *AW, *P, *AP;  // [kmax][N][3] each
-    double *T1, *T2;   // [kmax][N][3] ping-pong blocks of the Chebyshev recurrence (spin lattices)
+    double *T1, *T2, *T3, *T4;   // [kmax][N][3] rotating blocks of the Chebyshev recurrence (spin lattices; the one-step-per-pass
+                                 // kernel ping-pongs between T1 and T2, the two-step kernel rotates through all four)
     unsigned long long* flags;   // [MOTO_NUM_SMS] per-CTA step flags of the multi-step K1 (zeroed at create)
     unsigned long long epoch;    // flag base of the latest multi-step launch
     int coop_max_ctas;           // co-resident CTAs of the multi-step K1 (cooperative launch limit)
+    int coop2_max_ctas;          // the same for the two-steps-per-pass K1 (spin_cheb2_tma.cu)
     double* c;         // [N]   m_i . g_i
     double* g;         // [N][3] gradient scratch
     double* stage_m;   // [N][3] host-variant staging
@@ -143,6 +145,11 @@ int spin_tma_grid(const moto_ctx*);
 int spin_tma_coop_limit(int k);
 int spin_cheb_multistep(moto_ctx*, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
                         const double* d_coef, const int* d_done);
+// spin_cheb2_tma.cu
+int spin_cheb2_multistep(moto_ctx*, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
+                         const double* d_coef, const int* d_done);
+int spin_cheb_recurrence(moto_ctx*, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
+                         const double* d_coef, const int* d_done);
 int spin_hvp_tma_ex(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double* HV, const int* d_done,
                     double* waw_partials, int cheb, double alpha, double c0, double beta, const double* U, const double* d_coef);
 // spin_shells.cu

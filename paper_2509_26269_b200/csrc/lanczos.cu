@@ -207,7 +207,7 @@ moto_status lanczos_solve(moto_ctx* c, const double* d_state, int k, double tol,
                           moto_solve_info* info) {
     const long long n3 = 3ll * c->N;
     const long long dof = (c->kind == MOTO_KIND_TRI2D) ? 2ll * c->N : 3ll * c->N;
-    int m = c->nblocks * c->kmax - 1;
+    int m = (c->nblocks > 8 ? 8 : c->nblocks) * c->kmax - 1;   // the basis lives in the first eight blocks (six for atoms)
     if (m > MOTO_LZ_MAX) m = MOTO_LZ_MAX;
     if (c->opts.ncv > 0 && c->opts.ncv < m) m = c->opts.ncv;
     if (m > dof - 1) m = (int)(dof - 1);

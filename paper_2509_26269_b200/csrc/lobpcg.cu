@@ -56,6 +56,7 @@ struct FastCtx {
     moto_ctx* c; const double* state; const double* m_proj; int k, kb; double tol;
     double* partialsK; int nblkU, nblkK; int n;   // n: kernels enqueued
     int degree;      // 0: op = A
+    bool failed;     // a recurrence launch failed: the blocks hold nothing usable
 };
 
 // OV = op(V), with the V^T OV partials left in partialsK.  V = X goes to AX, V = W goes to AW.
@@ -68,19 +69,11 @@ static void fast_apply(FastCtx& f, const double* V, double* OV) {
         f.n += fast_dot_waw(c, f.kb, V, OV, f.partialsK, &f.nblkK);
         return;
     }
-    // the whole recurrence in one persistent cooperative launch (neighbour-flag synchronised steps) when it fits ...
-    if (f.degree >= 2 && !getenv("MOTO_NO_MULTISTEP")) {   // (the variable exists for the multi-step == step-wise test)
-        int nk = spin_cheb_multistep(c, f.state, c->c, V, f.kb, f.degree, OV, &c->st->cheb[0][0], &c->st->done);
-        if (nk > 0) { f.n += nk; f.n += fast_dot_waw(c, f.kb, V, OV, f.partialsK, &f.nblkK); return; }
-    }
-    // ... else one launch per step: Y_0 = V, Y_1 -> T1, Y_2 -> T2, Y_3 -> T1 (in place over its own three-term operand) ...
-    const double* in = V; const double* prev = nullptr;
-    for (int i = 1; i <= f.degree; ++i) {
-        double* out = (i == f.degree) ? OV : ((i & 1) ? c->T1 : c->T2);
-        f.n += spin_hvp_tma_ex(c, f.state, c->c, in, f.kb, out, &c->st->done, nullptr, 1, 0.0, 0.0, 0.0, prev, &c->st->cheb[i - 1][0]);
-        prev = in; in = out;
-        if (i == 1) prev = V;
-    }
+    // the whole recurrence: two steps per pass in one persistent cooperative launch when it fits (spin_cheb2_tma.cu), else one
+    // step per pass, else one launch per step (moto_solver_opts.cheb_mode)
+    const int nk = spin_cheb_recurrence(c, f.state, c->c, V, f.kb, f.degree, OV, &c->st->cheb[0][0], &c->st->done);
+    if (nk <= 0) { f.failed = true; return; }
+    f.n += nk;
     f.n += fast_dot_waw(c, f.kb, V, OV, f.partialsK, &f.nblkK);
 }
 
@@ -110,7 +103,7 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     const size_t bs = (size_t)3 * c->N;
     const int check_every = c->opts.check_every > 0 ? c->opts.check_every : 8;
     FastCtx f;
-    f.c = c; f.state = d_state; f.k = k; f.kb = kb; f.tol = tol; f.n = 0; f.nblkU = f.nblkK = 0; f.degree = 0;
+    f.c = c; f.state = d_state; f.k = k; f.kb = kb; f.tol = tol; f.n = 0; f.nblkU = f.nblkK = 0; f.degree = 0; f.failed = false;
     f.partialsK = c->partials + (size_t)MOTO_RED_BLOCKS * 64;   // after the [<=296][<=44] tri partials
     f.m_proj = (c->kind == MOTO_KIND_TRI2D) ? d_state : nullptr;
     double* pmax = c->partials + (size_t)MOTO_RED_BLOCKS * 128;
@@ -162,6 +155,7 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
             }
         }
         enq += batch;
+        if (f.failed) { c->launches += f.n; return moto_fail(c, MOTO_ECUDA, "moto_lowest_modes: a launch of the Chebyshev recurrence failed"); }
         if (enq >= max_iter) {   // final look: residuals of the last update if op = A, else a last A-phase start
             if (transformed) { f.degree = 0; fast_phase_start(f); }
             f.n += rr_solve_fast(c, kb, f.nblkU, nullptr, 0, /*check=*/2, k, tol, 0);
@@ -195,14 +189,9 @@ static int gen_apply(moto_ctx* c, const double* d_state, const double* V, int kb
     int n = 0;
     for (int a0 = 0; a0 < kb; a0 += 2) {
         const int kk = kb - a0 >= 2 ? 2 : 1;
-        int nk = degree >= 2 ? spin_cheb_multistep(c, d_state, c->c, V + a0 * bs, kk, degree, OV + a0 * bs, &c->st->cheb[0][0], &c->st->done) : 0;
-        if (nk > 0) { n += nk; continue; }
-        const double* in = V + a0 * bs; const double* prev = nullptr;
-        for (int i = 1; i <= degree; ++i) {
-            double* out = (i == degree) ? OV + a0 * bs : ((i & 1) ? c->T1 : c->T2);
-            n += spin_hvp_tma_ex(c, d_state, c->c, in, kk, out, &c->st->done, nullptr, 1, 0.0, 0.0, 0.0, prev, &c->st->cheb[i - 1][0]);
-            prev = in; in = out;
-        }
+        const int nk = spin_cheb_recurrence(c, d_state, c->c, V + a0 * bs, kk, degree, OV + a0 * bs, &c->st->cheb[0][0], &c->st->done);
+        if (nk <= 0) return -1000000;   // reported by the caller as a failed solve
+        n += nk;
     }
     return n;
 }
@@ -261,6 +250,7 @@ static moto_status lobpcg_solve_generic_filtered(moto_ctx* c, const double* d_st
             ++in_phase;
         }
         enq += batch;
+        if (n < 0) return moto_fail(c, MOTO_ECUDA, "moto_lowest_modes: a launch of the Chebyshev recurrence failed");
         if (enq >= max_iter && cur_degree > 0) { n += gen_phase_start(c, d_state, kb, k, tol, 0, nblk); hv += kb; }
         MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&c->hstat[slot], &c->st->theta, sizeof(HostStatus), cudaMemcpyDeviceToHost, c->stream));
         MOTO_CUDA_CHECK(c, cudaEventRecord(c->ev[slot], c->stream));

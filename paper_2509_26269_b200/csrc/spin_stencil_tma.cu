@@ -18,21 +18,18 @@
 //                                optional three-term epilogue out = alpha (HV - c0 v) + beta u
 //         MULTI-STEP (solver)    the whole Chebyshev recurrence in one cooperative launch: per-step neighbour flags,
 //                                ping-pong blocks, alternating sweep direction (see KParams and DESIGN.md 5)
-#include <cuda.h>
 #include "common.cuh"
 #include "device_utils.cuh"
 #include "stencil_math.cuh"
+#include "tma_utils.cuh"
 
 namespace {
 
-constexpr int TXMAX = 60;          // strip width (sites); row box = 64 sites starting at xb - 2 (see x3 below)
-constexpr int ROWD = 192;          // doubles per main row slot (64 sites x 3)
-constexpr int SIDED = 16;          // doubles per side row slot (128 B)
+using namespace tma;   // TXMAX, ROWD, SIDED, CROWD, mbarrier / TMA wrappers, tensor-map encoding
 constexpr int RC = 10;             // rows per chunk (= 2 rows per consumer row-pair x 5)
 constexpr int NCW = 10;            // consumer warps: 10 + 1 producer = 11 warps, registers are granted per 4 warps (12)
 constexpr int NTHREADS = (NCW + 1) * 32;
 
-constexpr int CROWD = 64;          // doubles per c row slot (SOLVER mode: c_i rides the ring too)
 constexpr int SMEM_BUDGET = 231 * 1024;
 
 template <int K, bool API> struct Cfg {
@@ -80,39 +77,7 @@ struct KParams {
     unsigned long long* flags;   // [grid] last step finished by each CTA, as epoch + step
     unsigned long long epoch;
     int* err;                // set when a neighbour wait times out
-#ifdef MOTO_K1_TIMING
-    unsigned long long* dbg;   // [grid][4]: smid, t_start, t_first_data, t_end (globaltimer ns)
-#endif
 };
-
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra DONE;\n"
-        "bra LAB_WAIT;\n"
-        "DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-                 ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
-                 : "memory");
-}
-
-__device__ __forceinline__ int strip_x(int i, int Lx, int nsx) { return 2 * (int)(((long long)i * (Lx >> 1)) / nsx); }
 
 __device__ __forceinline__ d3 lds3(const double* p) { return mk3(p[0], p[1], p[2]); }
 
@@ -152,13 +117,6 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     if (p.done && *p.done) return;
 
     const long long lo = (p.total * blockIdx.x) / gridDim.x, hi = (p.total * (blockIdx.x + 1)) / gridDim.x;
-#ifdef MOTO_K1_TIMING
-    if (threadIdx.x == 0) {
-        unsigned long long t; unsigned sm;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
-        p.dbg[blockIdx.x * 4 + 0] = sm; p.dbg[blockIdx.x * 4 + 1] = t;
-    }
-#endif
 
     if (warp == NCW) {
         // ================================================================ producer warp: all 32 lanes issue TMA boxes
@@ -167,15 +125,12 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         if (nsteps > 1) {   // CTAs whose sites this CTA reads as halo (and which read its sites): same strip above/below, strips left/right
             if (lane == 0) {
                 int nd = 0;
-                auto cta_of = [&](long long idx) {
-                    long long b = idx * gridDim.x / p.total;
-                    while (b + 1 < (long long)gridDim.x && (p.total * (b + 1)) / gridDim.x <= idx) ++b;
-                    while (b > 0 && (p.total * b) / gridDim.x > idx) --b;
-                    return (int)b;
+                auto add = [&](int c) {   // a partner beyond the capacity of sdep would be a silent race: report it instead
+                    for (int i = 1; i <= nd; ++i) if (sdep[i] == c) return;
+                    if (nd < 60) sdep[++nd] = c; else *p.err = 1;
                 };
-                auto add = [&](int c) { for (int i = 1; i <= nd; ++i) if (sdep[i] == c) return; if (nd < 60) sdep[++nd] = c; };
                 auto add_rows = [&](int sx2, int ya, int yb) {   // rows [ya, yb] of strip sx2
-                    const int c0 = cta_of((long long)sx2 * Ly + ya), c1 = cta_of((long long)sx2 * Ly + yb);
+                    const int c0 = cta_of((long long)sx2 * Ly + ya, p.total, gridDim.x), c1 = cta_of((long long)sx2 * Ly + yb, p.total, gridDim.x);
                     for (int c = c0; c <= c1; ++c) add(c);
                 };
                 add((int)blockIdx.x);
@@ -322,9 +277,6 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         const int Q = (nrows + 2 + RC - 1) / RC, nb = (nrows + RC - 1) / RC;
 
         mbar_wait(&full[n % S], (n / S) & 1u);
-#ifdef MOTO_K1_TIMING
-        if (threadIdx.x == 0 && pos == lo) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); p.dbg[blockIdx.x * 4 + 2] = t; }
-#endif
         // The three-term operand U is read straight from global memory (no reuse, so it does not ride the ring); its
         // loads are issued one block ahead so that a whole block of arithmetic hides their latency (issuing them at the
         // top of the same block left the warps on the long scoreboard).  out may alias U: a site's U is read and
@@ -443,9 +395,6 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     }
     }   // step
 
-#ifdef MOTO_K1_TIMING
-    if (threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); p.dbg[blockIdx.x * 4 + 3] = t; }
-#endif
     if (NK > 0 && p.waw) {  // fixed-order reduction over the 256 consumer threads (named barrier 1: the producer warp has left)
 #pragma unroll
         for (int t = 0; t < NK; ++t) {
@@ -462,34 +411,6 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn lookup_encode() {
-    void* f = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
-        return (EncodeTiledFn)f;
-    return nullptr;
-}
-EncodeTiledFn get_encode() {
-    static const EncodeTiledFn fn = lookup_encode();   // thread-safe one-time initialisation (moto_lowest_modes_batch runs host threads)
-    return fn;
-}
-
-// field array [nvec][Ly][ncomp Lx] fp64 as a 3-D tensor; box = {inner doubles, rows, 1}
-bool encode(CUtensorMap* map, const double* base, int Lx, int Ly, int nvec, int inner, int rows, int ncomp = 3) {
-    EncodeTiledFn enc = get_encode();
-    if (!enc) return false;
-    cuuint64_t gdim[3] = {(cuuint64_t)ncomp * Lx, (cuuint64_t)Ly, (cuuint64_t)nvec};
-    cuuint64_t gstr[2] = {(cuuint64_t)8 * ncomp * Lx, (cuuint64_t)8 * ncomp * Lx * Ly};
-    cuuint32_t box[3] = {(cuuint32_t)inner, (cuuint32_t)rows, 1};
-    cuuint32_t estr[3] = {1, 1, 1};
-    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
 bool encode_vset(VSet* v, const double* base, int Lx, int Ly, int nvec) {
     return encode(&v->chunk, base, Lx, Ly, nvec, ROWD, RC) && encode(&v->row, base, Lx, Ly, nvec, ROWD, 1) &&
            encode(&v->schunk, base, Lx, Ly, nvec, SIDED, RC) && encode(&v->srow, base, Lx, Ly, nvec, SIDED, 1);
@@ -498,11 +419,8 @@ bool encode_vset(VSet* v, const double* base, int Lx, int Ly, int nvec) {
 template <int K, bool API>
 bool launch(moto_ctx* c, const Maps& maps, const KParams& p, int grid) {
     using C = Cfg<K, API>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(k_hvp_tma<K, API>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return false;
-        attr_set = true;
-    }
+    static std::atomic<unsigned long long> attr_seen{0};   // per device, thread-safe
+    if (!ensure_smem_attr(k_hvp_tma<K, API>, C::SMEM, attr_seen)) return false;
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3(grid); cfg.blockDim = dim3(NTHREADS); cfg.dynamicSmemBytes = C::SMEM; cfg.stream = c->stream;
@@ -568,9 +486,6 @@ int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const doub
         p.alpha = alpha; p.c0 = c0; p.beta = beta; p.cheb = cheb; p.coef = d_coef;
         p.waw = waw_partials; p.done = d_done;
         p.nsteps = 1; p.V0 = nullptr; p.T1 = p.T2 = nullptr; p.flags = nullptr; p.epoch = 0; p.err = nullptr;
-#ifdef MOTO_K1_TIMING
-        p.dbg = (unsigned long long*)(c->partials + 100000);
-#endif
         const int grid = spin_tma_grid(c);
         bool l_ok;
         if (cvec) l_ok = kk == 2 ? launch<2, false>(c, maps, p, grid) : launch<1, false>(c, maps, p, grid);
@@ -621,9 +536,6 @@ int spin_cheb_multistep(moto_ctx* c, const double* m, const double* cvec, const 
     p.waw = nullptr; p.done = d_done;
     p.nsteps = d; p.V0 = V; p.T1 = c->T1; p.T2 = c->T2;
     p.flags = c->flags; c->epoch += 1024; p.epoch = c->epoch; p.err = &c->st->bad;
-#ifdef MOTO_K1_TIMING
-    p.dbg = (unsigned long long*)(c->partials + 100000);
-#endif
     const bool l_ok = k == 2 ? launch<2, false>(c, maps, p, grid) : launch<1, false>(c, maps, p, grid);
     return l_ok ? 1 : 0;
 }

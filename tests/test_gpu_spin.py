@@ -405,28 +405,32 @@ def test_hvp_three_term_parity(moto, case, path):
         assert rel_l2(Ud.cpu().numpy(), ref) <= HVP_TOL
 
 
-@pytest.mark.parametrize("case", [1, 3, 8])
-def test_multistep_recurrence_matches_the_stepwise_one(moto, case, monkeypatch):
-    # The persistent cooperative launch that runs the whole Chebyshev recurrence (neighbour-flag synchronisation, every
-    # second step swept bottom-up on the point-reflected stencil) against the one-launch-per-step path: same
-    # arithmetic up to the summation order inside the stencil, so agreement to rounding, and the same solve.
+@pytest.mark.parametrize("case", range(len(TMA_CASES)))
+def test_multistep_recurrence_matches_the_stepwise_one(moto, case):
+    # The three ways the degree-d recurrence is launched (moto_solver_opts.cheb_mode): 0 = two steps per pass with the
+    # intermediate step kept in shared memory and a redundantly computed halo ring (spin_cheb2_tma.cu; plus one single
+    # step when d is odd), 1 = one step per pass in one cooperative launch (neighbour-flag synchronisation, every second
+    # step swept bottom-up on the point-reflected stencil), 2 = d dependent launches.  Same arithmetic per site up to the
+    # summation order inside the stencil of a reversed sweep, so agreement to rounding, and the same solve.
     w = TMA_CASES[case]()
-    V = wl.random_block(w.N, 2, seed=77)
-    V = V - np.sum(V * w.spins[None], axis=2, keepdims=True) * w.spins[None]
-    outs, sols = [], []
-    for single in (False, True):
-        if single:
-            monkeypatch.setenv("MOTO_NO_MULTISTEP", "1")
-        else:
-            monkeypatch.delenv("MOTO_NO_MULTISTEP", raising=False)
+    outs, sols = {}, {}
+    for mode in (0, 1, 2):
         ctx = moto.spin_context(w)
-        ctx.set_solver(hvp_path=2, precond_degree=24)
-        outs.append(ctx.cheb_apply(dev(w.spins), dev(V), 24, -0.1, 18.6, -0.16).cpu().numpy())
-        lam, Vm, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-8, max_iter=400, allow_notconv=True)
-        sols.append((lam.cpu().numpy(), info))
-    assert rel_l2(outs[0], outs[1]) <= 1e-13
-    assert sols[0][1]["converged"] == sols[1][1]["converged"]
-    assert np.max(np.abs(sols[0][0] - sols[1][0])) <= 1e-9 * np.max(np.abs(sols[1][0]))
+        ctx.set_solver(hvp_path=2, precond_degree=24, cheb_mode=mode)
+        for k in (1, 2):
+            V = wl.random_block(w.N, k, seed=77 + k)
+            V = V - np.sum(V * w.spins[None], axis=2, keepdims=True) * w.spins[None]
+            for d in (2, 3, 24, 25):
+                outs[mode, k, d] = ctx.cheb_apply(dev(w.spins), dev(V), d, -0.1, 18.6, -0.16).cpu().numpy()
+        if w.N >= 400:
+            lam, Vm, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-8, max_iter=400, allow_notconv=True)
+            sols[mode] = (lam.cpu().numpy(), info)
+    for (mode, k, d), o in outs.items():
+        assert np.isfinite(o).all()
+        assert rel_l2(o, outs[2, k, d]) <= 1e-13, (mode, k, d, rel_l2(o, outs[2, k, d]))
+    for mode in sols:
+        assert sols[mode][1]["converged"] == sols[2][1]["converged"]
+        assert np.max(np.abs(sols[mode][0] - sols[2][0])) <= 1e-9 * np.max(np.abs(sols[2][0]))
 
 
 @pytest.mark.parametrize("path", [1, 2])
