@@ -81,9 +81,10 @@ typedef struct {
                                (single start vector, guard / precond_* ignored)          [0]  */
     int32_t ncv;            /* Lanczos basis size m, k + 2 <= m <= min(24, S kmax - 1, dof - 1) with S = 8 blocks
                                (spin lattices) or 6 (Cartesian) of the workspace; 0 = the largest that fits   [0]  */
-    int32_t cheb_mode;      /* how the degree-d recurrence of -p_d(A) is launched on the TMA K1 path: 0 = auto (two steps per
-                               pass in one persistent cooperative launch, spin_cheb2_tma.cu), 1 = one step per pass in one
-                               cooperative launch, 2 = d dependent launches.  All three give bit-identical results.   [0]  */
+    int32_t cheb_mode;      /* how the degree-d recurrence of -p_d(A) is launched on the TMA K1 path: 0 = auto (= 1, the fastest
+                               as measured at 10^6 spins), 1 = one step per pass in one persistent cooperative launch,
+                               2 = d dependent launches, 3 = two steps per pass in one cooperative launch with the intermediate
+                               step kept in shared memory (spin_cheb2_tma.cu).  All give the same results to rounding.  [0]  */
     int32_t reserved_;      /* must be 0 */
 } moto_solver_opts;
 

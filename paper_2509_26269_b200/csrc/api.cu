@@ -147,7 +147,7 @@ moto_status moto_set_solver(moto_ctx* c, const moto_solver_opts* o) {
     if (!c || !o) return MOTO_EINVAL;
     if (o->guard < 0 || o->check_every < 0 || o->precond_degree < -1 || o->hvp_path < 0 || o->hvp_path > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: negative option");
     if (o->method < 0 || o->method > 1 || o->ncv < 0 || o->ncv > MOTO_LZ_MAX) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: method must be 0 or 1, ncv in 0..24");
-    if (o->cheb_mode < 0 || o->cheb_mode > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: cheb_mode must be 0, 1 or 2");
+    if (o->cheb_mode < 0 || o->cheb_mode > 3) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: cheb_mode must be 0..3");
     moto_solver_opts n = *o;
     if (n.check_every == 0) n.check_every = 8;
     if (n.seed == 0) n.seed = 0x9E3779B97F4A7C15ull;

@@ -416,9 +416,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
             pos += nrows;
         }
         // publish "this CTA has finished pass": every consumer's stores first, then one release store
-        __threadfence();
+        // (one fence by the publishing thread after the CTA barrier covers every consumer's stores by cumulativity -- the
+        // pattern of a cooperative-groups grid sync; a fence per thread cost ~2 us per step)
         asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");
         if (threadIdx.x == 0) {
+            __threadfence();
             const unsigned long long v = p.epoch + (unsigned long long)pass;
             asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p.flags + blockIdx.x), "l"(v) : "memory");
         }
@@ -495,14 +497,14 @@ int spin_cheb2_multistep(moto_ctx* c, const double* m, const double* cvec, const
 }
 
 // The whole degree-d recurrence OUT = Y_d (Y_0 = V, coefficients at d_coef + 4 (i - 1), device memory) by the fastest path
-// the context allows (moto_solver_opts.cheb_mode): two steps per pass (+ one single step when d is odd), else one
-// cooperative launch with one step per pass, else d dependent launches.  k <= 2, V tangent, d >= 1.
+// the context allows (moto_solver_opts.cheb_mode): one cooperative launch with one step per pass (auto: the fastest as
+// measured at 10^6 spins), two steps per pass (+ one single step when d is odd) on request, else d dependent launches.  k <= 2, V tangent, d >= 1.
 // Returns the number of launches, or -1 if the TMA K1 path does not apply / a launch failed (nothing usable in OUT).
 int spin_cheb_recurrence(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
                          const double* d_coef, const int* d_done) {
     const int mode = c->opts.cheb_mode;
     double* T[4] = {c->T1, c->T2, c->T3, c->T4};
-    if (mode == 0 && d >= 2) {
+    if (mode == 3 && d >= 2) {
         const int de = d & ~1;
         // odd d: Y_{d-1} goes to the block it would occupy in the rotation, the last step is a single launch
         int n = spin_cheb2_multistep(c, m, cvec, V, k, de, de == d ? OUT : T[(de - 1) & 3], d_coef, d_done);
@@ -513,7 +515,7 @@ int spin_cheb_recurrence(moto_ctx* c, const double* m, const double* cvec, const
             return n1 > 0 ? n + n1 : -1;
         }
     }
-    if (mode <= 1 && d >= 2) {
+    if ((mode <= 1 || mode == 3) && d >= 2) {
         const int n = spin_cheb_multistep(c, m, cvec, V, k, d, OUT, d_coef, d_done);
         if (n > 0) return n;
     }

@@ -227,6 +227,10 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     }
 
     // ==================================================================== consumers
+    // Address arithmetic is hoisted out of the block loop: per sub-segment a thread fixes where its three stencil columns
+    // live (the main row box or, on the edge strips of a periodic lattice, a wrap side box: offset, row pitch and field
+    // stride of each), per block only the four row-slot indices change.  (The first version recomputed slots, pitches and
+    // 64-bit site indices per load: 330 of its 800 instructions per block were integer work.)
     const int ch = warp & 1, rp = warp >> 1;
     const int col = ch * 32 + lane;
     const long long N = (long long)Lx * Ly;
@@ -235,6 +239,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     for (int t = 0; t < NK; ++t) waw[t] = 0.0;
     const d3 muB = mk3(l.mu * l.Bx, l.mu * l.By, l.mu * l.Bz);
     const bool use_coef = !API && p.cheb && p.coef;
+    struct Role { int off, pitch, fstr; };   // doubles: field-0 / slot-0 offset from smain, row-slot pitch, field stride
 
     unsigned n = 0;
     for (int step = 1; step <= nsteps; ++step) {
@@ -247,6 +252,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         Ustep = step == 1 ? nullptr : (step == 2 ? p.V0 : ((step & 1) ? p.T1 : p.T2));     // Y_{step-2}
         outp = step == nsteps ? p.out : ((step & 1) ? p.T1 : p.T2);                          // Y_step (in place over Y_{step-2})
     }
+    const bool use_u = !API && p.cheb && Ustep;
     // Even steps of a multi-step launch sweep bottom-up: the rows a CTA wrote (and read) last in step i are the first it
     // touches in step i + 1, so a good part of the 176 MB/step footprint is still in the 126 MB L2.  A reversed sweep is
     // the same code on the point-reflected lattice: row order reversed, left and right neighbours swapped, D -> -D
@@ -264,62 +270,60 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         const bool active = col < w;
         const bool wrapL = l.px && xb == 0 && col == 0;        // x - 1 comes from the wrap side box
         const bool wrapR = l.px && xe == Lx && col == w - 1;   // x + 1 comes from the wrap side box
-        // per-thread column bases (in doubles) and row pitches of the three columns; "L" is x - 1 on a forward sweep, x + 1 reversed
-        const double* colM = wrapL ? sL + 13 : smain + 3 * (col + 1);   // x - 1
-        const double* baseC = smain + 3 * (col + 2);
-        const double* colP = wrapR ? sR : smain + 3 * (col + 3);         // x + 1
-        const bool useL = rev ? wrapR : wrapL, useR = rev ? wrapL : wrapR;
-        const double* baseL = rev ? colP : colM;
-        const double* baseR = rev ? colM : colP;
-        const int pitchL = useL ? SIDED : ROWD, pitchR = useR ? SIDED : ROWD;
-        const int fstrL = useL ? NSLOT * SIDED : NSLOT * ROWD, fstrR = useR ? NSLOT * SIDED : NSLOT * ROWD;
-        const int x = xb + col;
+        Role rM, rC, rP;                                        // columns x - 1, x, x + 1
+        rC.off = 3 * (col + 2); rC.pitch = ROWD; rC.fstr = NSLOT * ROWD;
+        rM.off = 3 * (col + 1); rM.pitch = ROWD; rM.fstr = NSLOT * ROWD;
+        rP.off = 3 * (col + 3); rP.pitch = ROWD; rP.fstr = NSLOT * ROWD;
+        if (wrapL) { rM.off = (int)(sL - smain) + 13 - FS0 * NSLOT * SIDED; rM.pitch = SIDED; rM.fstr = NSLOT * SIDED; }
+        if (wrapR) { rP.off = (int)(sR - smain) - FS0 * NSLOT * SIDED; rP.pitch = SIDED; rP.fstr = NSLOT * SIDED; }
+        const Role rL = rev ? rP : rM, rR = rev ? rM : rP;     // stencil frame of the sweep
         const int Q = (nrows + 2 + RC - 1) / RC, nb = (nrows + RC - 1) / RC;
+        // this thread's first site and the step to its second row / to the next block, in doubles
+        const long long e0 = 3 * ((long long)(rev ? y_end - 1 - 2 * rp : y_start + 2 * rp) * Lx + xb + col);
+        const long long eRow = rev ? -3ll * Lx : 3ll * Lx, eBlk = RC * eRow;
 
         mbar_wait(&full[n % S], (n / S) & 1u);
-        // The three-term operand U is read straight from global memory (no reuse, so it does not ride the ring); its
-        // loads are issued one block ahead so that a whole block of arithmetic hides their latency (issuing them at the
-        // top of the same block left the warps on the long scoreboard).  out may alias U: a site's U is read and
-        // written by the same thread, one block apart.
-        const bool use_u = !API && p.cheb && Ustep;
-        d3 uA[K], uB[K], nA[K], nB[K];
-        auto load_u = [&](int jb, d3 (&ua)[K], d3 (&ub)[K]) {
+        // The three-term operand U is read straight from global memory (no reuse, so it does not ride the ring): the loads
+        // for block j + 1 are issued at the end of block j, into the registers block j has just finished with, and have
+        // the stencil arithmetic of block j + 1 to arrive in.  out may alias U: a site's U is read and written by the same thread.
+        d3 uA[K], uB[K];
+        auto load_u = [&](int jb) {
             const int r = jb * RC + 2 * rp;
             if (use_u && active && r < nrows) {
-                const long long sA = (long long)(rev ? y_end - 1 - r : y_start + r) * Lx + x;
-                const long long dB = rev ? -(long long)Lx : (long long)Lx;
+                const double* up = Ustep + e0 + (long long)jb * eBlk;
 #pragma unroll
                 for (int a = 0; a < K; ++a) {
-                    ua[a] = ld3(Ustep + (size_t)a * 3 * N, sA);
-                    ub[a] = (r + 1 < nrows) ? ld3(Ustep + (size_t)a * 3 * N, sA + dB) : mk3(0.0, 0.0, 0.0);
+                    uA[a] = ld3(up + (size_t)a * 3 * N, 0);
+                    uB[a] = (r + 1 < nrows) ? ld3(up + (size_t)a * 3 * N + eRow, 0) : mk3(0.0, 0.0, 0.0);
                 }
             }
         };
-        load_u(0, uA, uB);
+        load_u(0);
+        int cur = (int)(n % S);
         for (int j = 0; j < nb; ++j) {
-            if (j + 1 < nb) load_u(j + 1, nA, nB);
-            if (j + 1 < Q) mbar_wait(&full[(n + j + 1) % S], ((n + j + 1) / S) & 1u);
+            const int nxt = cur + 1 == S ? 0 : cur + 1;
+            if (j + 1 < Q) mbar_wait(&full[nxt], ((n + j + 1) / S) & 1u);
             const int rA = j * RC + 2 * rp;
             if (active && rA < nrows) {
                 const bool haveB = rA + 1 < nrows;
-                int slot[4];
+                int sr[4];   // row slots of stencil rows rA - 1 .. rA + 2 (stage rows 2 rp .. 2 rp + 3, the last ones in the next stage)
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    const int rr = rA + q;   // = (row index r) + 1, r = rA - 1 + q
-                    slot[q] = (int)((n + rr / RC) % S) * RC + (rev ? RC - 1 - rr % RC : rr % RC);
+                    const int t = 2 * rp + q;
+                    sr[q] = t < RC ? cur * RC + (rev ? RC - 1 - t : t) : nxt * RC + (rev ? RC - 1 - (t - RC) : t - RC);
                 }
-                const long long siteA = (long long)(rev ? y_end - 1 - rA : y_start + rA) * Lx + x, siteB = rev ? siteA - Lx : siteA + Lx;
+                double* oA_p = outp + e0 + (long long)j * eBlk;
                 double cA = 0.0, cB = 0.0;
-                if (!API) { cA = sc[slot[1] * CROWD + col + 2]; cB = sc[slot[2] * CROWD + col + 2]; }
+                if (!API) { cA = sc[sr[1] * CROWD + col + 2]; cB = sc[sr[2] * CROWD + col + 2]; }
                 // field 0: m.  API: all ten sites (projection of the neighbours + stencil for c); SOLVER: centres only.
                 d3 m0C, m0R, m1L, m1C, m1R, m2L, m2C, m2R, m3L, m3C;
-                m1C = lds3(baseC + slot[1] * ROWD);
-                m2C = lds3(baseC + slot[2] * ROWD);
+                m1C = lds3(smain + rC.off + sr[1] * ROWD);
+                m2C = lds3(smain + rC.off + sr[2] * ROWD);
                 if (API) {
-                    m0C = lds3(baseC + slot[0] * ROWD); m0R = lds3(baseR + slot[0] * pitchR);
-                    m1L = lds3(baseL + slot[1] * pitchL); m1R = lds3(baseR + slot[1] * pitchR);
-                    m2L = lds3(baseL + slot[2] * pitchL); m2R = lds3(baseR + slot[2] * pitchR);
-                    m3L = lds3(baseL + slot[3] * pitchL); m3C = lds3(baseC + slot[3] * ROWD);
+                    m0C = lds3(smain + rC.off + sr[0] * ROWD); m0R = lds3(smain + rR.off + sr[0] * rR.pitch);
+                    m1L = lds3(smain + rL.off + sr[1] * rL.pitch); m1R = lds3(smain + rR.off + sr[1] * rR.pitch);
+                    m2L = lds3(smain + rL.off + sr[2] * rL.pitch); m2R = lds3(smain + rR.off + sr[2] * rR.pitch);
+                    m3L = lds3(smain + rL.off + sr[3] * rL.pitch); m3C = lds3(smain + rC.off + sr[3] * ROWD);
                     const d3 LmA = stencil_apply(ls, m1R, m1L, m2C, m0C, m2L, m0R, m1C.z);
                     const d3 LmB = stencil_apply(ls, m2R, m2L, m3C, m1C, m3L, m1R, m2C.z);
                     cA = dot3(m1C, LmA) - dot3(m1C, muB);
@@ -328,14 +332,13 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                 d3 vA[K], hA[K], vB[K], hB[K];
 #pragma unroll
                 for (int a = 0; a < K; ++a) {
-                    const int f = a + 1;
-                    const double* bL = baseL + (useL ? f - FS0 : f) * fstrL;
-                    const double* bC = baseC + f * NSLOT * ROWD;
-                    const double* bR = baseR + (useR ? f - FS0 : f) * fstrR;
-                    d3 u0C = lds3(bC + slot[0] * ROWD), u0R = lds3(bR + slot[0] * pitchR);
-                    d3 u1L = lds3(bL + slot[1] * pitchL), u1C = lds3(bC + slot[1] * ROWD), u1R = lds3(bR + slot[1] * pitchR);
-                    d3 u2L = lds3(bL + slot[2] * pitchL), u2C = lds3(bC + slot[2] * ROWD), u2R = lds3(bR + slot[2] * pitchR);
-                    d3 u3L = lds3(bL + slot[3] * pitchL), u3C = lds3(bC + slot[3] * ROWD);
+                    const double* bL = smain + rL.off + (a + 1) * rL.fstr;
+                    const double* bC = smain + rC.off + (a + 1) * rC.fstr;
+                    const double* bR = smain + rR.off + (a + 1) * rR.fstr;
+                    d3 u0C = lds3(bC + sr[0] * ROWD), u0R = lds3(bR + sr[0] * rR.pitch);
+                    d3 u1L = lds3(bL + sr[1] * rL.pitch), u1C = lds3(bC + sr[1] * ROWD), u1R = lds3(bR + sr[1] * rR.pitch);
+                    d3 u2L = lds3(bL + sr[2] * rL.pitch), u2C = lds3(bC + sr[2] * ROWD), u2R = lds3(bR + sr[2] * rR.pitch);
+                    d3 u3L = lds3(bL + sr[3] * rL.pitch), u3C = lds3(bC + sr[3] * ROWD);
                     if (API) {
                         u0C = proj3(m0C, u0C); u0R = proj3(m0R, u0R);
                         u1L = proj3(m1L, u1L); u1C = proj3(m1C, u1C); u1R = proj3(m1R, u1R);
@@ -370,32 +373,32 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                             oB = axpy3(ch_beta, uB[a], oB);
                         }
                     }
-                    st3(outp + (size_t)a * 3 * N, siteA, oA);
-                    if (haveB) st3(outp + (size_t)a * 3 * N, siteB, oB);
+                    st3(oA_p + (size_t)a * 3 * N, 0, oA);
+                    if (haveB) st3(oA_p + (size_t)a * 3 * N + eRow, 0, oB);
                 }
             }
-            if (use_u) {
-#pragma unroll
-                for (int a = 0; a < K; ++a) { uA[a] = nA[a]; uB[a] = nB[a]; }
-            }
+            if (j + 1 < nb) load_u(j + 1);
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[(n + j) % S]);
+            if (lane == 0) mbar_arrive(&empty[cur]);
+            cur = nxt;
         }
-        if (Q > nb) { __syncwarp(); if (lane == 0) mbar_arrive(&empty[(n + nb) % S]); }
+        if (Q > nb) { __syncwarp(); if (lane == 0) mbar_arrive(&empty[cur]); }
         n += Q;
         pos += nrows;
     }
     if (nsteps > 1) {   // publish "this CTA has finished step": every consumer's stores first, then one release store
-        __threadfence();
+        // (one fence by the publishing thread after the CTA barrier covers every consumer's stores by cumulativity -- the
+        // pattern of a cooperative-groups grid sync; a fence per thread cost ~2 us per step)
         asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");
         if (threadIdx.x == 0) {
+            __threadfence();
             const unsigned long long v = p.epoch + (unsigned long long)step;
             asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p.flags + blockIdx.x), "l"(v) : "memory");
         }
     }
     }   // step
 
-    if (NK > 0 && p.waw) {  // fixed-order reduction over the 256 consumer threads (named barrier 1: the producer warp has left)
+    if (NK > 0 && p.waw) {  // fixed-order reduction over the 320 consumer threads (named barrier 1: the producer warp has left)
 #pragma unroll
         for (int t = 0; t < NK; ++t) {
             const double v = warp_sum(waw[t]);

@@ -407,14 +407,14 @@ def test_hvp_three_term_parity(moto, case, path):
 
 @pytest.mark.parametrize("case", range(len(TMA_CASES)))
 def test_multistep_recurrence_matches_the_stepwise_one(moto, case):
-    # The three ways the degree-d recurrence is launched (moto_solver_opts.cheb_mode): 0 = two steps per pass with the
+    # The three ways the degree-d recurrence is launched (moto_solver_opts.cheb_mode): 3 = two steps per pass with the
     # intermediate step kept in shared memory and a redundantly computed halo ring (spin_cheb2_tma.cu; plus one single
     # step when d is odd), 1 = one step per pass in one cooperative launch (neighbour-flag synchronisation, every second
     # step swept bottom-up on the point-reflected stencil), 2 = d dependent launches.  Same arithmetic per site up to the
     # summation order inside the stencil of a reversed sweep, so agreement to rounding, and the same solve.
     w = TMA_CASES[case]()
     outs, sols = {}, {}
-    for mode in (0, 1, 2):
+    for mode in (1, 2, 3):
         ctx = moto.spin_context(w)
         ctx.set_solver(hvp_path=2, precond_degree=24, cheb_mode=mode)
         for k in (1, 2):
