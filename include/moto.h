@@ -265,6 +265,12 @@ moto_status moto_lowest_modes_host(moto_ctx* ctx, const double* h_spins, int k, 
 moto_status moto_mmf_step_host(moto_ctx* ctx, const double* h_spins, const double* h_v, int kr, double dt,
                                double* h_spins_out, double* h_fnorm);
 
+/* Cartesian atoms: the neighbour table holds at most 160 neighbours per atom.  moto_lowest_modes, moto_mmf_run*, moto_relax and the
+ * *_host variants check the overflow flag themselves (MOTO_ENOMEM); the asynchronous device-pointer calls moto_energy_grad,
+ * moto_hvp and moto_mmf_step do not wait for it -- call this after them (it synchronises the stream) when the density of the
+ * configuration is not known to be safe.  MOTO_OK for spin lattices. */
+moto_status moto_check_overflow(moto_ctx* ctx);
+
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t moto_launch_count(const moto_ctx* ctx);
 const char* moto_version(void);

@@ -73,6 +73,7 @@ _SIGS = {
     "moto_set_solver": (C.c_int, [C.c_void_p, C.POINTER(SolverOpts)]),
     "moto_last_error": (C.c_char_p, [C.c_void_p]),
     "moto_set_shells": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "moto_check_overflow": (C.c_int, [C.c_void_p]),
     "moto_energy_grad": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "moto_hvp": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
     "moto_lowest_modes": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
@@ -214,6 +215,9 @@ class Context:
         return torch.empty(*shape, dtype=torch.float64, device=self.device)
 
     # -- device-pointer API (names follow include/moto.h)
+    def check_overflow(self):
+        self._check(self.lib.moto_check_overflow(self._h))
+
     def energy_grad(self, spins, want_grad=True):
         """moto_energy_grad -> (E [1] device tensor, g [N][3] device tensor or None)."""
         _dev_f64(spins, (self.N, 3))

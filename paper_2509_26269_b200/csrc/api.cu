@@ -173,6 +173,16 @@ moto_status moto_energy_grad(moto_ctx* c, const double* d_spins, double* d_E, do
     return MOTO_OK;
 }
 
+moto_status moto_check_overflow(moto_ctx* c) {
+    if (!c) return MOTO_EINVAL;
+    if (c->kind != MOTO_KIND_CARTESIAN) return MOTO_OK;
+    int ov = 0;
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&ov, c->cl.overflow, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (ov) return moto_fail(c, MOTO_ENOMEM, "neighbour capacity MOTO_MAX_NEIGH exceeded: pair sums are truncated");
+    return MOTO_OK;
+}
+
 moto_status moto_hvp(moto_ctx* c, const double* d_spins, const double* d_V, int k, double* d_HV) {
     if (!c) return MOTO_EINVAL;
     if (!d_spins || !d_V || !d_HV || d_V == d_HV) return moto_fail(c, MOTO_EINVAL, "moto_hvp: null or aliased argument");
@@ -183,21 +193,12 @@ moto_status moto_hvp(moto_ctx* c, const double* d_spins, const double* d_V, int 
     return MOTO_OK;
 }
 
-static moto_status check_overflow(moto_ctx* c) {
-    if (c->kind != MOTO_KIND_CARTESIAN) return MOTO_OK;
-    int ov = 0;
-    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&ov, c->cl.overflow, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
-    if (ov) return moto_fail(c, MOTO_ENOMEM, "neighbour capacity MOTO_MAX_NEIGH exceeded");
-    return MOTO_OK;
-}
-
 // solve with the start block already in ctx->X (if warm_start); results left in ctx->X / st->theta
 static moto_status solve_internal(moto_ctx* c, const double* d_spins, int k, double tol, int max_iter, int warm_start,
                                   moto_solve_info* info) {
     moto_status s = lobpcg_solve(c, d_spins, k, tol, max_iter, warm_start, info);
     if (s != MOTO_OK && s != MOTO_ENOTCONV) return s;
-    moto_status s2 = check_overflow(c);
+    moto_status s2 = moto_check_overflow(c);
     if (s2 != MOTO_OK) return s2;
     c->launches += block_sign_normalise(c, c->X, k);
     MOTO_CUDA_CHECK(c, cudaGetLastError());
@@ -300,19 +301,20 @@ moto_status moto_mmf_run(moto_ctx* c, double* d_state, int k, double dt, int max
     // block LOBPCG: per step only v_1 is converged (solve_first_column); all k columns are converged where lambda_2 decides
     const bool first_only = c->opts.method == 0 && max_iter > 0;
     for (int step = 0;; ++step) {
-        moto_solve_info si;
+        moto_solve_info si = {};
         bool full = !first_only;
         st = first_only ? solve_first_column_impl(c, d_state, k, tol, max_iter, warm, d_lam, d_V, &si)
                         : moto_lowest_modes(c, d_state, k, tol, max_iter, warm, d_lam, d_V, &si);
         for (;;) {
-            out.hvp_count += si.hvp_count; out.solver_iters += si.iters;
             if (st != MOTO_OK && st != MOTO_ENOTCONV) break;
+            out.hvp_count += si.hvp_count; out.solver_iters += si.iters;
             MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_lam, d_lam, k * sizeof(double), cudaMemcpyDeviceToHost, c->stream));   // before the step reuses scal
             // candidate update into the staging vector; ||F_mmf|| of the CURRENT state comes with it
             st = moto_mmf_step(c, d_state, d_V, 1, dt, c->stage_m, d_fn);
             if (st != MOTO_OK) break;
             MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&h_fn, d_fn, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
             MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+            if ((st = moto_check_overflow(c)) != MOTO_OK) break;
             // the cheap solve left theta_2 >= lambda_2: the saddle test can only hold if theta_2 > 0; then (and on the last
             // step, so that the returned eigenvalues are the converged ones) all k columns are converged and the test redone
             const bool need_full = !full && ((h_fn <= tau_F && h_lam[0] < 0.0 && h_lam[1] > 0.0) || step >= max_steps);
@@ -453,7 +455,7 @@ moto_status moto_energy_grad_host(moto_ctx* c, const double* h_spins, double* h_
     if (h_E) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_E, dE, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     if (h_g) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_g, c->AP, vb, cudaMemcpyDeviceToHost, c->stream));
     MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
-    return MOTO_OK;
+    return moto_check_overflow(c);
 }
 
 moto_status moto_hvp_host(moto_ctx* c, const double* h_spins, const double* h_V, int k, double* h_HV) {
@@ -467,7 +469,7 @@ moto_status moto_hvp_host(moto_ctx* c, const double* h_spins, const double* h_V,
     if (s != MOTO_OK) return s;
     MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_HV, c->AP, k * vb, cudaMemcpyDeviceToHost, c->stream));
     MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
-    return MOTO_OK;
+    return moto_check_overflow(c);
 }
 
 moto_status moto_lowest_modes_host(moto_ctx* c, const double* h_spins, int k, double tol, int max_iter, int warm_start,
@@ -500,7 +502,7 @@ moto_status moto_mmf_step_host(moto_ctx* c, const double* h_spins, const double*
     MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_out, c->stage_m, vb, cudaMemcpyDeviceToHost, c->stream));
     if (h_fnorm) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(h_fnorm, dF, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
-    return MOTO_OK;
+    return moto_check_overflow(c);
 }
 
 }  // extern "C"

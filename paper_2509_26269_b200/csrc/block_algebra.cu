@@ -5,6 +5,7 @@
 // so reruns are bit-identical.
 #include "common.cuh"
 #include "device_utils.cuh"
+#include "tma_utils.cuh"   // ensure_smem_attr
 
 namespace {
 
@@ -359,8 +360,8 @@ int block_gram(moto_ctx* c, const double* const* S, int ns, const double* const*
     const long long nchunk = (n3 + GRAM_CH - 1) / GRAM_CH;
     int blocks = (int)(nchunk < MOTO_RED_BLOCKS ? nchunk : MOTO_RED_BLOCKS);
     size_t smem = (size_t)(ns + nt) * GRAM_LD * sizeof(double);
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(k_gram, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * MOTO_NS * GRAM_LD * 8); attr = true; }
+    static std::atomic<unsigned long long> attr_seen{0};   // per device, safe against the host threads of the batch call
+    if (!tma::ensure_smem_attr(k_gram, (size_t)3 * MOTO_NS * GRAM_LD * 8, attr_seen)) return 0;
     k_gram<<<blocks, GRAM_THREADS, smem, c->stream>>>(ps, ns, pt, nt, n3, c->partials, d_done);
     if (d_G) {
         k_gram_final<<<(ns * nt + 127) / 128, 128, 0, c->stream>>>(c->partials, blocks, ns * nt, d_G);

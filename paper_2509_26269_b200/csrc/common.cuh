@@ -126,6 +126,8 @@ static inline moto_status moto_fail(moto_ctx* ctx, moto_status s, const char* ms
     return s;
 }
 
+moto_status moto_check_overflow(moto_ctx* ctx);   // api.cu (also exported, include/moto.h)
+
 // ---- launch wrappers (each returns the number of kernels it enqueued; errors via cudaGetLastError)
 // spin_stencil.cu
 int spin_energy_grad(moto_ctx*, const double* m, double* d_E, double* d_g, double* d_c);

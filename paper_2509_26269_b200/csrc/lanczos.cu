@@ -211,7 +211,11 @@ moto_status lanczos_solve(moto_ctx* c, const double* d_state, int k, double tol,
     if (m > MOTO_LZ_MAX) m = MOTO_LZ_MAX;
     if (c->opts.ncv > 0 && c->opts.ncv < m) m = c->opts.ncv;
     if (m > dof - 1) m = (int)(dof - 1);
-    if (m < k + 2) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes (Lanczos): basis too small, need k + 2 <= ncv <= min(24, 8 kmax - 1, dof - 1)");
+    if (m < k + 2) {
+        snprintf(c->err, sizeof(c->err), "moto_lowest_modes (Lanczos): basis too small, need k + 2 <= ncv <= min(24, %d kmax - 1, dof - 1)",
+                 c->nblocks > 8 ? 8 : c->nblocks);
+        return MOTO_EINVAL;
+    }
     if (max_iter < 1) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes (Lanczos): max_iter must be >= 1");
     LzBasis B = {c->X, c->block_bytes / sizeof(double), c->kmax, n3};
     const int check_every = c->opts.check_every > 0 ? c->opts.check_every : 8;

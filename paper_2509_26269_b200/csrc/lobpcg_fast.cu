@@ -228,50 +228,81 @@ __global__ void k_cheb_coef(SolverState* st, int k, int d, double margin, double
 }
 
 // ---------------------------------------------------------------- A-residual check while LOBPCG runs on -p(A)
-// partials[blk][3 KB]: x_j.x_j, x_j.t_j, t_j.t_j with T = A X; then |A x - theta x|^2 = tt - 2 theta xt + theta^2 xx,
-// theta = xt / xx.  (|r|^2 ~ tol^2 = 1e-12 against tt ~ 1e-2: nine digits of head-room left in fp64.)
+// T = A X is given.  Two streaming passes, because the residual must not be formed from the expanded expression
+// tt - 2 theta xt + theta^2 xx: with tt ~ 1e-2 its rounding floor is ~ 1e-8 in |r|, so below tol ~ 1e-8 that test would
+// decide on noise.  Pass 1: partials of x_j.x_j and x_j.t_j  ->  theta_j = xt / xx (k_acheck_theta, into st->scal).
+// Pass 2: partials of |t_j - theta_j x_j|^2, formed element by element  ->  |A x_j - theta_j x_j| / |x_j|, decision.
 template <int KB>
 __global__ void __launch_bounds__(256) k_acheck_dots(long long n3, const double* __restrict__ X, const double* __restrict__ T,
                                                      double* __restrict__ partials, const int* __restrict__ done) {
     if (*done) return;
-    double acc[3 * KB];
+    double acc[2 * KB];
 #pragma unroll
-    for (int i = 0; i < 3 * KB; ++i) acc[i] = 0.0;
+    for (int i = 0; i < 2 * KB; ++i) acc[i] = 0.0;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n3; e += (long long)gridDim.x * blockDim.x) {
 #pragma unroll
         for (int j = 0; j < KB; ++j) {
             const double x = X[j * n3 + e], t = T[j * n3 + e];
-            acc[3 * j] = fma(x, x, acc[3 * j]); acc[3 * j + 1] = fma(x, t, acc[3 * j + 1]); acc[3 * j + 2] = fma(t, t, acc[3 * j + 2]);
+            acc[2 * j] = fma(x, x, acc[2 * j]); acc[2 * j + 1] = fma(x, t, acc[2 * j + 1]);
         }
     }
-    block_reduce_store<3 * KB>(acc, partials + (size_t)blockIdx.x * 3 * KB);
+    block_reduce_store<2 * KB>(acc, partials + (size_t)blockIdx.x * 2 * KB);
+}
+
+// theta_j = (x_j.t_j) / (x_j.x_j) into st->scal[j], x_j.x_j into st->scal[KMAX/2 + j]   (kb <= 2 here, scal has 8 slots)
+__global__ void k_acheck_theta(const double* __restrict__ partials, int nblk, int kb, SolverState* st) {
+    if (st->done) return;
+    __shared__ double v[2 * MOTO_KMAX];
+    const int e = threadIdx.x >> 5, lane = threadIdx.x & 31;   // one warp per entry
+    if (e < 2 * kb) {
+        double s = 0.0;
+        for (int b = lane; b < nblk; b += 32) s += partials[(size_t)b * 2 * kb + e];
+        s = warp_sum(s);
+        if (lane == 0) v[e] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x < kb) { st->scal[threadIdx.x] = v[2 * threadIdx.x + 1] / v[2 * threadIdx.x]; st->scal[4 + threadIdx.x] = v[2 * threadIdx.x]; }
+}
+
+template <int KB>
+__global__ void __launch_bounds__(256) k_acheck_resid(long long n3, const double* __restrict__ X, const double* __restrict__ T,
+                                                      const SolverState* __restrict__ st, double* __restrict__ partials) {
+    if (st->done) return;
+    double th[KB], acc[KB];
+#pragma unroll
+    for (int j = 0; j < KB; ++j) { th[j] = st->scal[j]; acc[j] = 0.0; }
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n3; e += (long long)gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int j = 0; j < KB; ++j) {
+            const double r = fma(-th[j], X[j * n3 + e], T[j * n3 + e]);
+            acc[j] = fma(r, r, acc[j]);
+        }
+    }
+    block_reduce_store<KB>(acc, partials + (size_t)blockIdx.x * KB);
 }
 
 __global__ void k_acheck_final(const double* __restrict__ partials, int nblk, int kb, int k, double tol, SolverState* st) {
     if (st->done) return;
-    __shared__ double v[3 * MOTO_KMAX];
-    const int e = threadIdx.x >> 5, lane = threadIdx.x & 31;   // one warp per entry
-    if (e < 3 * kb) {
+    __shared__ double v[MOTO_KMAX];
+    const int e = threadIdx.x >> 5, lane = threadIdx.x & 31;   // one warp per column
+    if (e < kb) {
         double s = 0.0;
-        for (int b = lane; b < nblk; b += 32) s += partials[(size_t)b * 3 * kb + e];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        for (int b = lane; b < nblk; b += 32) s += partials[(size_t)b * kb + e];
+        s = warp_sum(s);
         if (lane == 0) v[e] = s;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
         bool ok = true;
-        double th[MOTO_KMAX], rs[MOTO_KMAX];
+        double rs[MOTO_KMAX];
         for (int j = 0; j < kb; ++j) {
-            const double xx = v[3 * j], xt = v[3 * j + 1], tt = v[3 * j + 2];
-            th[j] = xt / xx;
-            const double r2 = (tt - 2.0 * th[j] * xt + th[j] * th[j] * xx) / xx;
-            rs[j] = sqrt(r2 > 0.0 ? r2 : 0.0);
+            const double r2 = v[j] / st->scal[4 + j];
+            rs[j] = sqrt(r2);
             if (j < k) ok = ok && (rs[j] <= tol) && (r2 == r2);
         }
         st->nhvp += kb;
         if (ok) {
-            for (int j = 0; j < kb; ++j) { st->theta[j] = th[j]; st->resid[j] = rs[j]; }
+            for (int j = 0; j < kb; ++j) { st->theta[j] = st->scal[j]; st->resid[j] = rs[j]; }
             st->done = 1;
         }
     }
@@ -343,6 +374,9 @@ int fast_acheck(moto_ctx* c, int kb, int k, double tol, const double* d_T, doubl
     const int g = fast_grid(n3);
     if (kb == 1) k_acheck_dots<1><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, partials, &c->st->done);
     else k_acheck_dots<2><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, partials, &c->st->done);
-    k_acheck_final<<<1, 32 * 3 * kb, 0, c->stream>>>(partials, g, kb, k, tol, c->st);
-    return 2;
+    k_acheck_theta<<<1, 32 * 2 * kb, 0, c->stream>>>(partials, g, kb, c->st);
+    if (kb == 1) k_acheck_resid<1><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, c->st, partials);
+    else k_acheck_resid<2><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, c->st, partials);
+    k_acheck_final<<<1, 32 * kb, 0, c->stream>>>(partials, g, kb, k, tol, c->st);
+    return 4;
 }

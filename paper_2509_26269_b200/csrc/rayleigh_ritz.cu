@@ -449,12 +449,17 @@ __global__ void __launch_bounds__(RR_THREADS_MAX) k_lz_ritz(SolverState* st, int
 
 // block of the launch: 256 threads for n <= 8, one thread per entry (rounded to warps) above
 static inline int rr_threads(int n) { int np = (n + 1) & ~1, t = (np * np + 31) & ~31; return t > RR_THREADS ? t : RR_THREADS; }
-// pivots of the unit-diagonal G_B below this send the pencil to the truncating eigen-decomposition path.  Measured (B200):
-// with 1e-8 the random-spin 10^6 solve needed 40 iterations / 1734 HVPs / 36.5 ms (whitening error ~ eps / pivot perturbs
-// the Ritz vectors of an ill-conditioned [X, W, P] just enough to miss the A-residual check at iteration 32); with 1e-4 or
-// 1e-2: 32 / 1090 / 24.5 ms, every other config unchanged.  That holds for the fused kb <= 2 path (n <= 6) only: with 1e-2 the
-// generic path at kb = 5 on the transformed operator (tests: test_transformed_generic_path_kb_gt_2) no longer reaches 1e-9,
-// there the Cholesky whitening is the more accurate of the two, so the generic callers keep 1e-8.
+// Whitening of the unit-diagonal G_B: Cholesky where it is as accurate as the alternative, the rank-revealing eigen-decomposition
+// (Jacobi + truncation at tau) elsewhere.  Error model: the Cholesky factor of a matrix with smallest pivot p carries a relative
+// error ~ eps / p into the whitened pencil.  n <= 8 (the fused kb <= 2 path): the Jacobi route costs one extra 6 x 6 sweep set and
+// is accurate to ~eps whatever the conditioning, so Cholesky is admitted only while it matches that, p >= 1e-2 (error <= 100 eps).
+// n > 8 (generic path, 18 x 18 ... 24 x 24 pencils): the Jacobi route is the slower AND, measured, the less accurate one on
+// well-conditioned pencils (kb = 5 on the transformed operator stalls above 1e-9 with it), so Cholesky is admitted down to
+// p >= 1e-8 (error <= 1e-8 relative, below the rank-truncation threshold tau = 1e-10 of the other route times the pencil norm).
+// Both routes are exercised over cond(S) = 1e3 .. 1e13 at n = 3, 6, 18, 24 in tests/test_gpu_spin.py
+// (test_rayleigh_ritz_ill_conditioned_basis): genuine Ritz pairs of span(S), never below the true Ritz values.  Which route an
+// iteration takes moves a solve by at most one convergence check (random spins at 10^6: 32 iterations with 1e-2, 36 with the
+// Jacobi route everywhere, 40 with 1e-8 -- the check runs every fourth iteration); cfg 3 takes 80 iterations with all three.
 static const double CHOL_THR = 1e-8;
 static const double CHOL_THR_FAST = 1e-2;
 

@@ -22,8 +22,9 @@
 namespace {
 
 // x_t = R(x + a d): per-site renormalisation for spins (A7), identity for atoms (d is zero on fixed atoms)
-__global__ void __launch_bounds__(256) k_relax_trial(long long N, const double* __restrict__ x, const double* __restrict__ d, double a,
-                                                     double* __restrict__ xt, int retract) {
+// (x and xt may be the same array -- moto_mmf_run_cg updates the state in place -- so neither is __restrict__)
+__global__ void __launch_bounds__(256) k_relax_trial(long long N, const double* x, const double* __restrict__ d, double a,
+                                                     double* xt, int retract) {
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
         d3 y = axpy3(a, ld3(d, i), ld3(x, i));
         if (retract) y = scale3(1.0 / sqrt(dot3(y, y)), y);
@@ -279,11 +280,11 @@ moto_status eval_force(moto_ctx* c, const double* y, int k, double tol, int max_
     double* d_lam = c->st->scal;
     double* d_fn = c->st->cheb_ab;
     if (transport) { moto_status t = moto_transport(c, y, d_V, k); if (t != MOTO_OK) return t; }
-    moto_solve_info si;
+    moto_solve_info si = {};
     moto_status s = (c->opts.method == 0 && !full && max_iter > 0) ? solve_first_column(c, y, k, tol, max_iter, warm, d_lam, d_V, &si)
                                                                    : moto_lowest_modes(c, y, k, tol, max_iter, warm, d_lam, d_V, &si);
-    acc->hvp_count += si.hvp_count; acc->solver_iters += si.iters;
     if (s != MOTO_OK && s != MOTO_ENOTCONV) return s;
+    acc->hvp_count += si.hvp_count; acc->solver_iters += si.iters;
     MOTO_CUDA_CHECK(c, cudaMemcpyAsync(fe->lam, d_lam, k * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     c->fmmf_out = F_out;
     s = moto_mmf_step(c, y, d_V, 1, 0.0, c->stage_m, d_fn);      // dt = 0: only the force and its norm are wanted
@@ -291,7 +292,7 @@ moto_status eval_force(moto_ctx* c, const double* y, int k, double tol, int max_
     if (s != MOTO_OK) return s;
     MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&fe->fn, d_fn, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
-    return MOTO_OK;
+    return moto_check_overflow(c);   // atoms: a truncated neighbour table would give a silently wrong force
 }
 
 moto_status dots(moto_ctx* c, const double* a, const double* b0, const double* b1, const double* b2, int nb, double* h) {
@@ -315,8 +316,9 @@ moto_status mmf_cg_run(moto_ctx* c, double* d_state, int k, double delta, double
     double *F = d_scratch, *d = d_scratch + n3, *Fn = d_scratch + 2 * n3, *xt = d_scratch + 3 * n3;
     moto_mmf_info out; memset(&out, 0, sizeof(out));
     ForceEval fe;
+    auto fail = [&](moto_status e) { if (info) *info = out; return e; };   // the caller always gets the counters so far
     moto_status st = eval_force(c, d_state, k, tol, max_iter, warm_start, 0, d_V, F, false, &fe, &out);
-    if (st != MOTO_OK) return st;
+    if (st != MOTO_OK) return fail(st);
     MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d, F, vb, cudaMemcpyDeviceToDevice, c->stream));
     bool full = c->opts.method != 0;
     moto_status ret = MOTO_OK;
@@ -325,7 +327,7 @@ moto_status mmf_cg_run(moto_ctx* c, double* d_state, int k, double delta, double
         // saddle test; lambda_2 decides only on converged pairs (see moto_mmf_run)
         if (!full && ((fe.fn <= tau_F && fe.lam[0] < 0.0 && fe.lam[1] > 0.0) || step >= max_steps)) {
             st = eval_force(c, d_state, k, tol, max_iter, 1, 0, d_V, F, true, &fe, &out);
-            if (st != MOTO_OK) return st;
+            if (st != MOTO_OK) return fail(st);
             full = true;
         }
         out.steps = step; out.fnorm = fe.fn;
@@ -334,10 +336,10 @@ moto_status mmf_cg_run(moto_ctx* c, double* d_state, int k, double delta, double
         if (step >= max_steps) { ret = moto_fail(c, MOTO_ENOTCONV, "moto_mmf_run_cg: max_steps reached before the saddle test held"); break; }
         full = c->opts.method != 0;
         st = dots(c, F, F, d, nullptr, 2, h);                         // F.F, F.d
-        if (st != MOTO_OK) return st;
+        if (st != MOTO_OK) return fail(st);
         const double FF = h[0], Fd = h[1];
         st = dots(c, d, d, nullptr, nullptr, 1, h);                   // d.d
-        if (st != MOTO_OK) return st;
+        if (st != MOTO_OK) return fail(st);
         const double dn = sqrt(h[0]);
         if (!(dn > 0.0) || !(FF > 0.0)) { ret = moto_fail(c, MOTO_ESTATE, "moto_mmf_run_cg: zero force"); break; }
         const double f0 = Fd / dn;
@@ -345,9 +347,9 @@ moto_status mmf_cg_run(moto_ctx* c, double* d_state, int k, double delta, double
         c->launches += 1;
         ForceEval ft;
         st = eval_force(c, xt, k, tol, max_iter, 1, 1, d_V, Fn, false, &ft, &out);
-        if (st != MOTO_OK) return st;
+        if (st != MOTO_OK) return fail(st);
         st = dots(c, Fn, d, nullptr, nullptr, 1, h);                  // F_t.d  (F_t is tangent at x_t: transporting d changes nothing)
-        if (st != MOTO_OK) return st;
+        if (st != MOTO_OK) return fail(st);
         const double f1 = h[0] / dn;
         const double Cv = (f0 - f1) / delta;
         double s = Cv > 0.0 ? f0 / Cv : smax;
@@ -355,9 +357,9 @@ moto_status mmf_cg_run(moto_ctx* c, double* d_state, int k, double delta, double
         k_relax_trial<<<grid, 256, 0, c->stream>>>(N, d_state, d, s / dn, d_state, spin);   // in place: element-wise
         c->launches += 1;
         st = eval_force(c, d_state, k, tol, max_iter, 1, 1, d_V, Fn, false, &fe, &out);
-        if (st != MOTO_OK) return st;
+        if (st != MOTO_OK) return fail(st);
         st = dots(c, Fn, Fn, F, nullptr, 2, h);                       // F_new.F_new, F_new.F
-        if (st != MOTO_OK) return st;
+        if (st != MOTO_OK) return fail(st);
         double beta = (h[0] - h[1]) / FF;
         if (!(beta > 0.0)) beta = 0.0;
         k_relax_dir<<<grid, 256, 0, c->stream>>>(N, d_state, Fn, beta, d, spin, 1.0);

@@ -263,9 +263,10 @@ __global__ void __launch_bounds__(256) k_mmf_pass1(Lat l, const double* __restri
 }
 
 // pass 2: F_mmf = F - 2 sum_a alpha_a v_a ; m' = normalize(m + dt F_mmf) ; partial |F_mmf|^2
-__global__ void __launch_bounds__(256) k_mmf_pass2(long long N, const double* __restrict__ m, const double* __restrict__ v, int kr,
+// (m_out may alias m -- moto_mmf_step allows it -- so neither is __restrict__)
+__global__ void __launch_bounds__(256) k_mmf_pass2(long long N, const double* m, const double* __restrict__ v, int kr,
                                                    const double* __restrict__ Fbuf, const double* __restrict__ alpha, double dt,
-                                                   double* __restrict__ m_out, double* __restrict__ partials, int retract,
+                                                   double* m_out, double* __restrict__ partials, int retract,
                                                    const uint8_t* __restrict__ fixed, double* __restrict__ F_out) {
     __shared__ double red[32];
     double al[MOTO_KMAX];

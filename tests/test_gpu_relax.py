@@ -253,3 +253,35 @@ def test_mmf_run_cg_heptamer(moto):
     assert lam_ref[0] < 0.0 < lam_ref[1] and np.max(np.abs(np.array(info["lam"]) - lam_ref) / np.abs(lam_ref)) <= 1e-6
     assert np.linalg.norm(co2.mmf_force(mdl, xs, V_ref[:1])) <= 1.1e-4
     assert np.all(xs[w.fixed == 1] == w.positions[w.fixed == 1])
+
+
+@pytest.mark.parametrize("pbc", [(0, 0), (1, 0), (0, 1)])
+@pytest.mark.parametrize("steps", [1, 4])
+def test_first_steps_match_oracle_open_boundaries(moto, pbc, steps):
+    # the fused trial kernel k_relax_eval on open and mixed boundaries (absent neighbours contribute 0; tiles that hang
+    # over the edge; 70x37 is not a multiple of the 32x8 tile): same checks as the periodic case above
+    m = wl.random_spins(70, 37, 11)
+    w = wl.SpinWorkload("rand70x37", 70, 37, pbc[0], pbc[1], 1.0, 0.3, 0.05, (0.0, 0.0, 0.03), 1.0, 2, 11, m)
+    mdl = spin_model(w)
+    ref, iref = ro.relax_downhill(*ro.spin_ops(mdl), w.spins, steps, 0.0, 0.05)
+    ctx = moto.spin_context(w, kmax=2)
+    x = dev(w.spins)
+    info = ctx.relax(x, steps, 0.0, 0.05)
+    assert info["steps"] == iref["steps"] == steps
+    assert info["evals"] == iref["evals"] and info["alpha"] == iref["alpha"]
+    assert abs(info["energy"] - iref["energy"]) <= 1e-12 * abs(iref["energy"])
+    assert abs(info["gnorm"] - iref["gnorm"]) <= 1e-10 * iref["gnorm"]
+    assert np.max(np.abs(x.cpu().numpy() - ref)) <= 1e-11
+
+
+def test_first_steps_match_oracle_cfg2_open(moto):
+    # configs[2] (256x256 open, two skyrmions) at full size: first two accepted steps of RelaxDownHill
+    w = wl.config2()
+    mdl = spin_model(w)
+    ref, iref = ro.relax_downhill(*ro.spin_ops(mdl), w.spins, 2, 0.0, 0.05)
+    ctx = moto.spin_context(w, kmax=2)
+    x = dev(w.spins)
+    info = ctx.relax(x, 2, 0.0, 0.05)
+    assert info["steps"] == 2 and info["evals"] == iref["evals"] and info["alpha"] == iref["alpha"]
+    assert abs(info["energy"] - iref["energy"]) <= 1e-12 * abs(iref["energy"])
+    assert np.max(np.abs(x.cpu().numpy() - ref)) <= 1e-11

@@ -364,7 +364,7 @@ def test_cfg3_full_size_lowest_modes_vs_golden(moto, cfg3_full):
     assert np.max(np.abs(lam - gold[:2]) / np.abs(gold[:2])) <= EIG_TOL, (lam, gold[:2])
     HV = so.hvp(model_of(w), w.spins, V)
     for a in range(2):
-        assert np.linalg.norm(HV[a] - lam[a] * V[a]) <= 2e-6
+        assert np.linalg.norm(HV[a] - lam[a] * V[a]) <= 1e-6 * (1 + 1e-3)      # the stated tol; 1e-3 for the oracle's own rounding
     assert np.max(np.abs(V.reshape(2, -1) @ V.reshape(2, -1).T - np.eye(2))) <= 1e-10
     assert np.max(np.abs(np.sum(V * w.spins[None], axis=2))) <= 1e-10
 
@@ -576,3 +576,135 @@ def test_other_parameter_signs(moto, params):
     c = so.curvature_scalar(w.spins, so.gradient(model, w.spins))
     Lmax = np.linalg.eigvalsh(so.euclid_hessian(model).toarray())[-1]
     assert lam_max <= np.max(-c) + Lmax + 1e-9
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# BASELINE.json configs[2] at full size: 256x256 OPEN lattice, two skyrmions, k = 6, then MMF steps with a re-solve per
+# step (8(c) "O-sparse (cfg 2, 3)").  65 536 sites takes the TMA K1 path with open boundaries on both
+# axes (out-of-range box coordinates zero-fill) and the generic kb > 2 LOBPCG (k_gram_sym, k_update, k_residual, 18x18 pencils).
+@pytest.fixture(scope="module")
+def cfg2_full():
+    w = wl.config2()
+    lam_ref, V_ref = so.lowest_modes_sparse(model_of(w), w.spins, 6, extra=2)
+    return w, lam_ref, V_ref
+
+
+def test_cfg2_full_size_hvp_parity_k6(moto, cfg2_full):
+    w, _, _ = cfg2_full
+    model = model_of(w)
+    ctx = moto.spin_context(w, kmax=8)
+    V = wl.random_block(w.N, 6, seed=44)               # not tangent: the call projects
+    ref = so.hvp(model, w.spins, V)
+    for path in (0, 2, 1):                              # auto (= TMA at this size), TMA forced, generic
+        ctx.set_solver(hvp_path=path)
+        HV = ctx.hvp(dev(w.spins), dev(V)).cpu().numpy()
+        assert rel_l2(HV, ref) <= HVP_TOL, path
+        assert np.max(np.abs(HV - ref)) <= 1e-11 * np.max(np.abs(ref)), path
+        assert np.max(np.abs(np.sum(HV * w.spins[None], axis=2))) <= 1e-12
+    E, g = ctx.energy_grad(dev(w.spins))
+    assert abs(E.item() - so.energy(model, w.spins)) <= 1e-12 * abs(so.energy(model, w.spins))
+    assert np.max(np.abs(g.cpu().numpy() - so.projected_gradient(model, w.spins))) <= 1e-12
+
+
+def test_cfg2_full_size_lowest_modes_k6(moto, cfg2_full):
+    # eigenvalues one by one at 1e-8 relative (floor 1e-3, reading A23); eigenvectors as subspaces (reading A10): the angle to
+    # the oracle's lowest-6 space where the gap after mode 6 allows it, containment in the oracle's lowest-8 space otherwise;
+    # and the oracle-side residual of every returned pair
+    w, lam_ref, V_ref = cfg2_full
+    ctx = moto.spin_context(w, kmax=8)
+    ctx.set_solver(guard=2)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 6, tol=w.tol, max_iter=20000)
+    assert info["converged"], info
+    lam = lam.cpu().numpy(); V = V.cpu().numpy()
+    assert np.max(np.abs(lam - lam_ref[:6]) / np.maximum(np.abs(lam_ref[:6]), 1e-3)) <= EIG_TOL, (lam, lam_ref)
+    Vf = V.reshape(6, -1).T
+    gap = lam_ref[6] - lam_ref[5]
+    if gap > 1e-2 * abs(lam_ref[5]):
+        assert scipy.linalg.subspace_angles(Vf, V_ref[:6].reshape(6, -1).T).max() <= ANGLE_TOL
+    else:
+        Q = np.linalg.qr(V_ref.reshape(8, -1).T)[0]
+        assert np.linalg.norm(Vf - Q @ (Q.T @ Vf), 2) <= ANGLE_TOL
+    HV = so.hvp(model_of(w), w.spins, V)
+    for a in range(6):
+        assert np.linalg.norm(HV[a] - lam[a] * V[a]) <= w.tol * (1 + 1e-3), a
+    assert np.max(np.abs(Vf.T @ Vf - np.eye(6))) <= 1e-10
+    assert np.max(np.abs(np.sum(V * w.spins[None], axis=2))) <= 1e-10
+
+
+def test_cfg2_full_size_first_mmf_steps(moto, cfg2_full):
+    # the first 3 of configs[2]'s 100 MMF steps (dt = 0.05, re-solve per step, warm start from the transported block): per
+    # step the oracle is fed the GPU's own v_1 (SURVEY 8(c) "MMF trajectory": only single steps are pinned) and must
+    # reproduce the new state to 1e-13 and |F_mmf|; the re-solved pairs are checked by their oracle-side residuals
+    w, lam_ref, _ = cfg2_full
+    model = model_of(w)
+    ctx = moto.spin_context(w, kmax=8)
+    ctx.set_solver(guard=2)
+    x = dev(w.spins)
+    V0 = None
+    for step in range(3):
+        lam, V, info = ctx.lowest_modes(x, 6, tol=w.tol, max_iter=20000, V0=V0)
+        assert info["converged"], (step, info)
+        xh, Vh, lh = x.cpu().numpy(), V.cpu().numpy(), lam.cpu().numpy()
+        if step == 0:
+            assert np.max(np.abs(lh - lam_ref[:6]) / np.maximum(np.abs(lam_ref[:6]), 1e-3)) <= EIG_TOL
+        HV = so.hvp(model, xh, Vh[:2])
+        for a in range(2):
+            assert np.linalg.norm(HV[a] - lh[a] * Vh[a]) <= w.tol * (1 + 1e-3)
+        xn, fn = ctx.mmf_step(x, V[:1].contiguous(), w.dt)
+        ref = so.mmf_step(model, xh, Vh[:1], w.dt)
+        assert np.max(np.abs(xn.cpu().numpy() - ref)) <= 1e-13
+        assert abs(fn.item() - np.linalg.norm(so.mmf_force(model, xh, Vh[:1]))) <= 1e-12 * max(1.0, fn.item())
+        x = xn
+        V0 = V.clone()
+        ctx.transport(x, V0)
+
+
+def test_transformed_solve_oracle_side_residual_at_1e9(moto):
+    # LOBPCG on -p_d(A) (the default fused path where the TMA K1 applies) decides convergence on |A x - theta x| of A itself.
+    # At tol = 1e-9 that decision sits far below what an expanded-form residual could resolve (tt - 2 theta xt + theta^2 xx
+    # has a rounding floor ~1e-8): the oracle recomputes the residual of every returned pair and it must meet the tolerance.
+    for w in (wl.config3_scaled(100), wl.config1()):
+        model = model_of(w)
+        ctx = moto.spin_context(w, kmax=2)
+        ctx.set_solver(hvp_path=2)
+        lam, V, info = ctx.lowest_modes(dev(w.spins), 2, tol=1e-9, max_iter=20000)
+        assert info["converged"], info
+        lam = lam.cpu().numpy(); V = V.cpu().numpy()
+        HV = so.hvp(model, w.spins, V)
+        for a in range(2):
+            r = np.linalg.norm(HV[a] - lam[a] * V[a])
+            assert r <= 1e-9 * (1 + 1e-3), (w.name, a, r, info["resid"])
+            assert abs(r - info["resid"][a]) <= 1e-3 * 1e-9 + 1e-3 * r      # the reported residual is the true one
+        lam_ref, _ = so.lowest_modes(model, w.spins, 2)
+        assert np.max(np.abs(lam - lam_ref[:2]) / np.maximum(np.abs(lam_ref[:2]), 1e-3)) <= EIG_TOL
+
+
+@pytest.mark.parametrize("n,nev", [(6, 2), (3, 1), (18, 6), (24, 8)])
+@pytest.mark.parametrize("cond", [1e3, 1e6, 1e10, 1e13])
+def test_rayleigh_ritz_ill_conditioned_basis(moto, n, nev, cond):
+    # K4 on the kind of pencil a converging LOBPCG produces: S = [X, W, P] with nearly dependent columns (W, P -> span X),
+    # cond(S) up to 1e13 before the rank truncation at 1e-10 of the largest eigenvalue of the scaled G_B sets in.  Truth:
+    # Ritz values of A on span(S) from a QR of S itself (backward stable, never forms S^T S).  Forming the Gram matrices
+    # costs cond(S)^2 eps in the small directions, which the kernel must turn into a dropped direction, not into garbage:
+    # the lowest Ritz values may then only move UP (a subspace of span S), by at most what the dropped directions held.
+    rng = np.random.default_rng(int(np.log10(cond)) * 100 + n)
+    N = 80
+    Q0 = np.linalg.qr(rng.standard_normal((N, n)))[0]
+    sv = np.logspace(0, -np.log10(cond), n)
+    S = (Q0 * sv) @ np.linalg.qr(rng.standard_normal((n, n)))[0]
+    Aop = rng.standard_normal((N, N)); Aop = Aop + Aop.T
+    GA, GB = S.T @ Aop @ S, S.T @ S
+    w = wl.config0()
+    ctx = moto.spin_context(w, kmax=8)
+    th, Cm = ctx.rayleigh_ritz(dev(GA), dev(GB), nev)
+    th, Cm = th.cpu().numpy(), Cm.cpu().numpy()
+    assert np.isfinite(th).all() and np.isfinite(Cm).all()
+    Qs = np.linalg.qr(S)[0]
+    full = np.linalg.eigvalsh(Qs.T @ Aop @ Qs)
+    # every returned pair is a genuine Ritz pair of span(S): orthonormal in the S metric, Rayleigh quotient = theta
+    Y = S @ Cm
+    assert np.max(np.abs(Y.T @ Y - np.eye(nev))) <= 1e-6
+    assert np.max(np.abs(np.diag(Y.T @ Aop @ Y) - th)) <= 1e-6 * np.max(np.abs(full))
+    assert np.all(th >= full[:nev] - 1e-8 * np.max(np.abs(full)))             # Cauchy interlacing: never below the truth
+    if cond <= 1e3:                  # cond(G_B) = 1e6 < 1e10: no direction is dropped, the answer is the truth itself
+        assert np.max(np.abs(th - full[:nev])) <= 1e-8 * np.max(np.abs(full))
