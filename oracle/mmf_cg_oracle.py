@@ -18,7 +18,9 @@ one-trial secant line search on the force component along the direction:
 
 Written against callables so that the loop can be pinned on a plain 2-D function with an analytic Hessian
 (tests/test_oracle_relax.py) and on the spin lattice, where it must reach the saddle the fixed-step loop
-(spin_oracle.mmf_run) reaches.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline legs may import this file.
+(spin_oracle.mmf_run) reaches.  Parity status: pinned step by step on the quadratic saddle x^T diag(-1, 2, 3) x / 2 with its
+analytic minimum mode (the secant step in closed form, its clip at smax, the negative-curvature branch, beta of linear CG,
+exactness after three steps) and at the end point on the lattice.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline legs may import this file.
 """
 from __future__ import annotations
 

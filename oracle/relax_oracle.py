@@ -26,8 +26,10 @@ Written against four callables (energy, gradient, retract, transport) so that th
 quadratic in R^n (tests/test_oracle_relax.py: minimiser == numpy.linalg.solve), on the ferromagnet (closed-form
 energy -N(6J + K + mu B)), on a Morse trimer (bond lengths r0) and on a 2-D double well for the two-sided descent.
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline legs may import this file; it shares no code with
-the CUDA path.  Parity status: pinned (end points); the step-by-step trajectory is compared with the CUDA path only
-while the accept/reject decisions sit well above rounding.
+the CUDA path.  Parity status: pinned -- end points as above, and step by step (tests/test_oracle_relax.py): a 1-D sequence
+derived by hand from the rule (a rejected overshoot, a doubled step, two restarts to steepest descent, evaluation counts),
+and the direction update against textbook linear CG after an exact step (beta, signs).  The trajectory is compared with the
+CUDA path only while the accept/reject decisions sit well above rounding.
 """
 from __future__ import annotations
 

@@ -142,3 +142,94 @@ def test_cg_mmf_double_well_and_same_saddle_as_fixed_step():
     assert abs(so.energy(mdl, x) - so.energy(mdl, m_fix)) < 1e-6
     assert np.max(np.abs(lam - lam_fix) / np.abs(lam_fix)) < 1e-3
     assert np.max(np.abs(x - m_fix)) < 1e-2
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Step-level pins of the two conjugate-gradient loops (readings A26, A28).  End-point pins alone cannot see a wrong beta, a
+# wrong sign in the restart test, a wrong step-doubling rule or a wrong secant clip (all still converge); these do.
+def test_relax_one_dimensional_sequence_by_hand():
+    # f = x^2/2 from x0 = 1 with alpha0 = 3; every number is an exact binary fraction, derived by hand from the rule of A26:
+    # step 1  g = 1, d = -1, slope = -1.  a = 3: x_t = -2, g_t.d = 2 > 1/2 |slope|: REJECTED (overshoot).  a = 3/2: x_t = -1/2,
+    #         g_t.d = 1/2 <= 1/2, E_t = 1/8 <= 1/2 - 1.5e-4: accepted at the SECOND trial -> alpha stays 3/2.  evals = 3.
+    #         beta = (1/4 + 1/2)/1 = 3/4; new slope = -1/4 + 3/4 * 1/2 = +1/8 >= 0 -> restart: beta = 0, d = +1/2, slope = -1/4.
+    # step 2  a = 3/2: x_t = 1/4, g_t.d = 1/8 <= 1/8, E_t = 1/32 <= 1/8 - 3.75e-5: accepted at the FIRST trial -> alpha = 3.  evals = 4.
+    #         beta = (1/16 + 1/8)/(1/4) = 3/4; new slope = -1/16 + 3/4 * 1/8 = +1/32 >= 0 -> restart: d = -1/4, slope = -1/16.
+    # step 3  a = 3: x_t = -1/2, g_t.d = 1/8 > 1/32: rejected.  a = 3/2: x_t = -1/8, g_t.d = 1/32 <= 1/32, E_t = 1/128: accepted at
+    #         the second trial -> alpha = 3/2.  evals = 6.
+    ops = _flat_ops(lambda x: float(0.5 * x @ x), lambda x: x.copy())
+    want_x = [-0.5, 0.25, -0.125]
+    want_alpha = [1.5, 3.0, 1.5]
+    want_evals = [3, 4, 6]
+    for n in (1, 2, 3):
+        trace = []
+        x, info = ro.relax_downhill(*ops, np.array([1.0]), n, 0.0, 3.0, trace=trace)
+        assert x[0] == want_x[n - 1] and info["alpha"] == want_alpha[n - 1] and info["evals"] == want_evals[n - 1]
+        assert info["steps"] == n and info["energy"] == 0.5 * want_x[n - 1] ** 2 and info["gnorm"] == abs(want_x[n - 1])
+    assert trace == [(0.125, 0.5, 1.5), (0.03125, 0.25, 1.5), (0.0078125, 0.125, 1.5)]
+
+
+def test_relax_direction_update_is_linear_cg_after_an_exact_step():
+    # On an SPD quadratic with an EXACT first step (alpha0 = g.g / g^T A g, accepted at the first trial: g_1.d_0 = 0) the new
+    # gradient is orthogonal to the old one, so PR+ beta = g_1.g_1 / g_0.g_0 = the beta of LINEAR conjugate gradients and
+    # d_1 = -g_1 + beta_1 d_0 is the CG direction.  x_1 and the direction of x_2 - x_1 are pinned against the textbook
+    # recurrence written out below (numpy only); the second step's length is one of 2 alpha0 / 2^j.
+    rng = np.random.default_rng(5)
+    n = 9
+    Q = rng.standard_normal((n, n)); A = Q @ Q.T + np.eye(n)
+    b = rng.standard_normal(n)
+    x0 = rng.standard_normal(n)
+    ops = _flat_ops(lambda x: float(0.5 * x @ A @ x - b @ x), lambda x: A @ x - b)
+    r0 = b - A @ x0                                  # linear CG (Hestenes-Stiefel), two steps
+    p0 = r0
+    a0 = (r0 @ r0) / (p0 @ A @ p0)
+    x1_cg = x0 + a0 * p0
+    r1 = r0 - a0 * (A @ p0)
+    beta1 = (r1 @ r1) / (r0 @ r0)
+    p1 = r1 + beta1 * p0
+    x1, i1 = ro.relax_downhill(*ops, x0, 1, 0.0, a0)
+    assert i1["evals"] == 2 and i1["alpha"] == 2.0 * a0                   # first trial accepted -> doubled
+    assert np.max(np.abs(x1 - x1_cg)) <= 1e-14 * np.max(np.abs(x1_cg))
+    trace = []
+    x2, i2 = ro.relax_downhill(*ops, x0, 2, 0.0, a0, trace=trace)
+    step = x2 - x1
+    a1 = trace[1][2]
+    assert any(a1 == 2.0 * a0 / 2 ** j for j in range(8))
+    assert np.max(np.abs(step / a1 - p1)) <= 1e-12 * np.max(np.abs(p1))    # beta and the sign of every term of d_1
+    # and with exact steps throughout (a 2-D quadratic where 2 alpha0 happens to be exact is not needed: restart the loop from
+    # x_1 with the exact CG step length instead) the iterates are those of linear CG
+    a1_cg = (r1 @ r1) / (p1 @ A @ p1)
+    assert ops[0](x1 + a1_cg * p1) <= ops[0](x2) + 1e-15                  # the exact CG step is at least as good as the accepted one
+
+
+def test_mmf_cg_secant_step_closed_form_clip_and_negative_curvature():
+    # Quadratic saddle f = x^T A x / 2, A = diag(-1, 2, 3), analytic MinMode v_1 = e_1: F_mmf = -|A| x is LINEAR, so the secant
+    # estimate C = (f0 - f1)/delta equals dh^T |A| dh whatever delta is and s = f0 / C is the exact zero of the force along dh:
+    # x_1 = x_0 + [(F.dh)/(dh^T |A| dh)] dh with dh = F/|F| -- the first step of linear CG on |A|.  Three such steps reach the
+    # saddle (3-D).  With smax below that length the step is exactly smax dh.  With a wrong mode (e_2) the effective Hessian
+    # along dh = e_1 is negative, C < 0, and the step is +smax along dh.
+    from oracle import mmf_cg_oracle as mo
+    A = np.diag([-1.0, 2.0, 3.0]); absA = np.diag([1.0, 2.0, 3.0])
+    mm = lambda x: (np.array([-1.0, 2.0]), np.stack([np.array([1.0, 0.0, 0.0]), np.array([0.0, 1.0, 0.0])]))
+    force = lambda x: -A @ x
+    flat = ((lambda x: x), (lambda x, d: d))
+    x0 = np.array([0.5, -0.25, 0.125])
+    F0 = -absA @ x0
+    dh = F0 / np.linalg.norm(F0)
+    s_exact = (F0 @ dh) / (dh @ absA @ dh)
+    for delta in (1e-3, 0.05):
+        trace = []
+        x1, lam, steps, conv, fn, evals = mo.mmf_run_cg(mm, force, *flat, x0, delta, 10.0, 1, 0.0, trace=trace)
+        assert steps == 1 and evals == 3
+        assert abs(trace[0][1] - s_exact) <= 1e-10 * s_exact
+        assert np.max(np.abs(x1 - (x0 + s_exact * dh))) <= 1e-10
+    r1 = -absA @ (x0 + s_exact * dh)                                        # linear CG beta on |A| (gradient of the next point)
+    assert abs(trace[0][2] - (r1 @ r1) / (F0 @ F0)) <= 1e-9                 # PR+ = FR after an exact step (F_1 . F_0 = 0)
+    x3, lam, steps, conv, fn, evals = mo.mmf_run_cg(mm, force, *flat, x0, 1e-3, 10.0, 3, 0.0)
+    assert np.max(np.abs(x3)) <= 1e-9                                       # n = 3: CG is exact after three steps
+    xc, *_ = mo.mmf_run_cg(mm, force, *flat, x0, 1e-3, 0.01, 1, 0.0)
+    assert np.max(np.abs(xc - (x0 + 0.01 * dh))) <= 1e-16                   # clipped to smax
+    mm_wrong = lambda x: (np.array([-1.0, 2.0]), np.stack([np.array([0.0, 1.0, 0.0]), np.array([1.0, 0.0, 0.0])]))
+    xe = np.array([0.5, 0.0, 0.0])                                          # F = (0.5, 0, 0): dh = e_1, effective curvature -1
+    trace = []
+    xn, *_ = mo.mmf_run_cg(mm_wrong, force, *flat, xe, 1e-3, 0.02, 1, 0.0, trace=trace)
+    assert trace[0][1] == 0.02 and np.max(np.abs(xn - np.array([0.52, 0.0, 0.0]))) <= 1e-16
