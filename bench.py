@@ -7,7 +7,7 @@ One "step" = one pass of the whole hot path on configs[3] (1000x1000 periodic, ~
 `value` = single-vector HVP applications per second over the timed steps (inputs resident in HBM);
 `e2e`  = the same step through the host-buffer C ABI (H2D of the spins, D2H of lambda, V, m', |F|).
 `roofline` is measured live for the K1 block-HVP kernel in a dedicated region of the same run
-(buffer sets rotated so the footprint exceeds L2).  `cpu_baseline` times the oracle on a bounded sample.
+(buffer sets rotated so the footprint exceeds L2); `roofline.frac` counts SURVEY 8(d)'s 24 (1 + 2k) bytes per site per block-HVP.  `cpu_baseline` times the oracle on a bounded sample.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl moto|reference] [--workload cfg3]
 N > 1 (torchrun): N independent replicas (different seeds), no data-path collective ("replicas only").
@@ -91,7 +91,10 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_sample(L: int = 632, calls: int = 6):
+ORACLE_SAMPLE = dict(L=400, calls=10)   # the bounded sample BOTH arms time (cpu_baseline leg and --impl reference)
+
+
+def oracle_sample(L: int = ORACLE_SAMPLE["L"], calls: int = ORACLE_SAMPLE["calls"]):
     """The oracle, as it stands, on a bounded same-density sample of configs[3]; returns HVP/s scaled to 1e6 sites."""
     from oracle import spin_oracle as so
     from paper_2509_26269_b200 import workloads as wl
@@ -111,25 +114,37 @@ def oracle_sample(L: int = 632, calls: int = 6):
             "host_cpus": os.cpu_count()}
 
 
+def bench_config(args, world: int):
+    """The `config` object of the JSON line -- one definition for both arms (own and --impl reference)."""
+    from paper_2509_26269_b200 import workloads as wl
+    name = args.workload
+    label = {"cfg3": "cfg3_1000x1000_pbc_200skyrmions (BASELINE.json configs[3] recipe)"}.get(name, name)
+    N = 1000 * 1000 if name == "cfg3" else None
+    return {"workload": label, "N": N, "k": 2, "tol": 1e-6, "dt": 0.05, "max_iter": args.max_iter, "start": "cold seeded block",
+            "parallelism": "replicas only" if world > 1 else "1 GPU",
+            "l2_policy": "solver working set ~540 MB > 126 MB L2; kernel-only regions rotate buffer sets of 120-176 MB each (> 2.5 x L2 in total)",
+            "solver": "LOBPCG on the Chebyshev-transformed operator -p_40(A) (library default), A-residual <= tol"}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     vals, t_all = [], []
     for _ in range(args.warmup):
-        oracle_sample(L=100, calls=1)
+        oracle_sample(calls=1)
     for _ in range(args.steps):
         t0 = time.perf_counter()
-        r = oracle_sample(L=200, calls=2)
+        r = oracle_sample()
         t_all.append(time.perf_counter() - t0)
         vals.append(r["value"])
     v = float(np.mean(vals))
     cb = dict(r); cb["value"] = v
-    cb["sample"] = "each step: oracle.spin_oracle.hvp x2 (k=2) on the 200x200 same-density instance of configs[3], scaled by sites to 1e6"
+    cb["sample"] = "each step: " + r["sample"]
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
                       "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(t_all)), "higher_is_better": True,
                       "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                      "config": {"workload": "configs[3] 1000x1000 pbc ~200 skyrmions k=2 (bounded same-density sample)"},
+                      "config": bench_config(args, 1),
                       "cpu_baseline": cb,
                       "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
@@ -462,13 +477,24 @@ def main():
     achieved = alg_bytes / (tt_ms * 1e-3) / 1e9
     achieved_ms = alg_bytes_ms / (ms_ms * 1e-3) / 1e9
     achieved_api = alg_bytes_api / (hvp_ms * 1e-3) / 1e9
-    traffic = None   # dram__bytes_read + dram__bytes_write of the roofline kernel from the committed ncu --set full capture
-    tp = os.path.join(ROOT, "profiles", "r01_k1_traffic.csv")
-    if os.path.exists(tp) and args.workload == "cfg3":
-        for line in open(tp).read().splitlines()[1:]:
-            f = line.split(",")
-            if f[0] == "cfg3" and "multi-step" in line:
-                traffic = float(f[-3]) + float(f[-2])
+    # DRAM traffic of the roofline kernel: bench.py cannot run ncu, so the number comes from the committed `ncu --set full`
+    # capture of THIS kernel -- and only if the capture was taken from the kernel source that is being timed now (the CSV
+    # records the sha256 of spin_stencil_tma.cu); a stale capture gives traffic = null instead of a wrong number.
+    traffic, traffic_source = None, None
+    tp = os.path.join(ROOT, "profiles", "r02_k1_traffic.csv")
+    src = os.path.join(ROOT, "paper_2509_26269_b200", "csrc", "spin_stencil_tma.cu")
+    if os.path.exists(tp) and os.path.exists(src) and args.workload == "cfg3":
+        import hashlib
+        sha = hashlib.sha256(open(src, "rb").read()).hexdigest()[:16]
+        rows = [l.split(",") for l in open(tp).read().splitlines() if l and not l.startswith("#")]
+        hdr, rows = rows[0], rows[1:]
+        for f in rows:
+            r_ = dict(zip(hdr, f))
+            if r_.get("launch") == "multi-step d=40" and r_.get("kernel_src_sha16") == sha:
+                traffic = float(r_["dram_bytes_read"]) + float(r_["dram_bytes_write"])
+                traffic_source = f"profiles/r02_k1_traffic.csv (ncu --set full capture, kernel source sha16 {sha} = the source timed here)"
+        if traffic is None:
+            traffic_source = "none: profiles/r02_k1_traffic.csv was captured from a different kernel source"
 
     # ---------------------------------------------------------------- (B) the step, inputs resident in HBM
     def step():
@@ -535,16 +561,13 @@ def main():
 
     if rank == 0:
         last = infos[-1]
+        cfg = bench_config(args, world)
+        cfg.update({"N": N, "k": k, "tol": tol, "dt": dt}) if args.workload != "cfg3" else None
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{w.name} (BASELINE.json configs[3] recipe)" if args.workload == "cfg3" else w.name,
-                       "N": N, "k": k, "tol": tol, "dt": dt, "max_iter": args.max_iter, "start": "cold seeded block",
-                       "parallelism": "replicas only" if world > 1 else "1 GPU",
-                       "l2_policy": f"solver working set {ctx.workspace_bytes / 1e6:.0f} MB > L2; kernel-only regions rotate "
-                                    f"{nsets} buffer sets of {alg_bytes_api / 1e6:.0f}-{alg_bytes / 1e6:.0f} MB",
-                       "solver": "LOBPCG on the Chebyshev-transformed operator -p_40(A) (library default), A-residual <= tol"},
+            "config": cfg,
             "solve": {"ms": float(np.mean([a.elapsed_time(b) for a, b in solve_ms])), "iters": last["iters"],
                       "converged": last["converged"], "resid": last["resid"], "hvp_count": last["hvp_count"],
                       "lambda": [float(x) for x in lam.cpu().numpy()],
@@ -554,17 +577,30 @@ def main():
                            "gsite_updates_per_s": N * k / (hvp_ms * 1e-3) / 1e9, "launches_per_call": hvp_launches,
                            "algorithmic_bytes": alg_bytes_api, "achieved_gbs": achieved_api, "frac_of_measured_peak": achieved_api / peak,
                            "frac_of_8TBs_nominal": achieved_api / 8000.0},
+            # `frac` is in the survey's unit: 24 (1 + 2k) N algorithmic bytes per block-HVP (read m, V; write HV),
+            # d block-HVPs per launch.  The recurrence really moves more (c and the three-term operand: 128 B/site for the first
+            # step, 176 for the others): that figure rides along as frac_recurrence_bytes.
             "roofline": {"bound": "hbm",
                          "kernel": f"k_hvp_tma<2,0> persistent multi-step launch (moto_cheb_apply, degree {deg}): the operator application "
-                                   "of the transformed solver, > 80 % of the step's GPU time",
-                         "achieved": achieved_ms, "peak": peak, "unit": "GB/s", "frac": achieved_ms / peak,
-                         "frac_of_8TBs_nominal": achieved_ms / 8000.0, "traffic": traffic, "algorithmic_bytes": alg_bytes_ms,
+                                   "of the transformed solver, ~80 % of the step's GPU time",
+                         "achieved": deg * alg_bytes_api / (ms_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": deg * alg_bytes_api / (ms_ms * 1e-3) / 1e9 / peak,
+                         "frac_of_8TBs_nominal": deg * alg_bytes_api / (ms_ms * 1e-3) / 1e9 / 8000.0,
+                         "algorithmic_bytes": deg * alg_bytes_api, "algorithmic_bytes_per_site_per_step": 24 * (1 + 2 * k),
+                         "achieved_recurrence_bytes": achieved_ms, "frac_recurrence_bytes": achieved_ms / peak,
+                         "recurrence_bytes": alg_bytes_ms,
+                         "traffic": traffic, "traffic_source": traffic_source,
                          "ms": ms_ms, "us_per_step": 1e3 * ms_ms / deg, "hvps_per_s": k * deg * 1e3 / ms_ms,
                          "gsite_updates_per_s": N * k * deg / (ms_ms * 1e-3) / 1e9, "launches_per_call": ms_launches,
                          "peak_source": peak_src,
+                         "kernel_hvp": {"call": "moto_hvp, k_hvp_tma<2,1> (the kernel north_star names: input projected, c recomputed)",
+                                        "ms": hvp_ms, "algorithmic_bytes": alg_bytes_api, "achieved": achieved_api,
+                                        "frac": achieved_api / peak, "frac_of_8TBs_nominal": achieved_api / 8000.0},
                          "single_step": {"call": "moto_hvp_three_term (one recurrence step per launch, programmatic dependent launch)",
-                                         "ms": tt_ms, "algorithmic_bytes": alg_bytes, "achieved": achieved, "frac": achieved / peak,
-                                         "frac_of_8TBs_nominal": achieved / 8000.0, "launches_per_call": tt_launches}},
+                                         "ms": tt_ms, "algorithmic_bytes": alg_bytes_api, "achieved": alg_bytes_api / (tt_ms * 1e-3) / 1e9,
+                                         "frac": alg_bytes_api / (tt_ms * 1e-3) / 1e9 / peak,
+                                         "recurrence_bytes": alg_bytes, "frac_recurrence_bytes": achieved / peak,
+                                         "launches_per_call": tt_launches}},
             "e2e": {"value": e2e_hvps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": 1e3 * e2e_s / n_e2e, "steps": n_e2e},
             "gpu_launches": int(launches),

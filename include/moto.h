@@ -85,7 +85,9 @@ typedef struct {
                                as measured at 10^6 spins), 1 = one step per pass in one persistent cooperative launch,
                                2 = d dependent launches, 3 = two steps per pass in one cooperative launch with the intermediate
                                step kept in shared memory (spin_cheb2_tma.cu).  All give the same results to rounding.  [0]  */
-    int32_t reserved_;      /* must be 0 */
+    int32_t persistent;     /* the whole solve as ONE persistent cooperative kernel (nearest-neighbour spin lattices up to 32 768
+                               sites that do not take the transformed path, k <= 2, no guard columns): 0 / 1 = where it applies,
+                               2 = never (the multi-launch solver)                                                    [0]  */
 } moto_solver_opts;
 
 typedef struct {
@@ -139,10 +141,15 @@ moto_status moto_lowest_modes(moto_ctx* ctx, const double* d_spins, int k, doubl
 
 /* Population solve (Alg. 1 l.3-5: the explorer evaluates (lambda_1, lambda_2) once per candidate per
  * generation, P = 24 in the paper): moto_lowest_modes on P independent problems at once.
- * ctxs[p] are P DISTINCT contexts (same or different lattices), each created on its OWN stream -- on small lattices a solve is
- * a chain of launch-latency-bound kernels, and the P chains overlap on the GPU only through separate streams (contexts that
- * share a stream are still solved correctly, one after the other).  The library runs one host thread per context (at most 32
- * at a time); every array argument is a HOST array of P device pointers / P structs, entry p with the meaning it has in
+ * ctxs[p] are P DISTINCT contexts; every array argument is a HOST array of P device pointers / P structs, entry p with the
+ * meaning it has in moto_lowest_modes.
+ * Batched path: when all contexts describe the same nearest-neighbour spin lattice (size, boundaries, parameters) small enough
+ * for the persistent solver (moto_solver_opts.persistent; k <= 2), the P solves run inside ONE cooperative kernel launch per 24
+ * problems on ctxs[0]'s stream: problem index = a grid dimension, a barrier among the CTAs of one problem only, one
+ * Rayleigh-Ritz per problem and iteration on the device, problems finish at their own iteration counts.
+ * Otherwise (different lattices, atoms, general shells, larger lattices): one host thread per context (at most 32 at a time),
+ * each driving the multi-launch solver on its context's own stream, so that the P launch chains overlap -- create the
+ * contexts on their OWN streams for that; in
  * moto_lowest_modes.  Inputs must be complete on the device before the call (the contexts' streams are not ordered against
  * the stream that produced them).  statuses [P] (host, may be NULL) receives each problem's status; the return value is MOTO_OK,
  * MOTO_ENOTCONV if some problem hit max_iter (and none failed), else the first failure.  Results are bit-identical to P

@@ -43,7 +43,7 @@ class MorseParams(C.Structure):
 class SolverOpts(C.Structure):
     _fields_ = [("guard", C.c_int32), ("check_every", C.c_int32), ("precond_degree", C.c_int32), ("hvp_path", C.c_int32),
                 ("precond_lo", C.c_double), ("precond_hi", C.c_double), ("seed", C.c_uint64), ("method", C.c_int32), ("ncv", C.c_int32),
-                ("cheb_mode", C.c_int32), ("reserved_", C.c_int32)]
+                ("cheb_mode", C.c_int32), ("persistent", C.c_int32)]
 
 
 class MmfInfo(C.Structure):
@@ -193,9 +193,9 @@ class Context:
             pass
 
     def set_solver(self, guard=0, check_every=8, precond_degree=0, precond_lo=0.0, precond_hi=0.0, seed=0, hvp_path=0,
-                   method=0, ncv=0, cheb_mode=0):
+                   method=0, ncv=0, cheb_mode=0, persistent=0):
         """method: 0 block LOBPCG, 1 thick-restart Lanczos (ncv = basis size, 0 = largest the workspace holds)."""
-        o = SolverOpts(guard, check_every, precond_degree, hvp_path, precond_lo, precond_hi, seed, method, ncv, cheb_mode, 0)
+        o = SolverOpts(guard, check_every, precond_degree, hvp_path, precond_lo, precond_hi, seed, method, ncv, cheb_mode, persistent)
         self._check(self.lib.moto_set_solver(self._h, C.byref(o)))
 
     def set_shells(self, offsets, J, D):

@@ -147,6 +147,7 @@ moto_status moto_set_solver(moto_ctx* c, const moto_solver_opts* o) {
     if (!c || !o) return MOTO_EINVAL;
     if (o->guard < 0 || o->check_every < 0 || o->precond_degree < -1 || o->hvp_path < 0 || o->hvp_path > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: negative option");
     if (o->method < 0 || o->method > 1 || o->ncv < 0 || o->ncv > MOTO_LZ_MAX) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: method must be 0 or 1, ncv in 0..24");
+    if (o->persistent < 0 || o->persistent > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: persistent must be 0, 1 or 2");
     if (o->cheb_mode < 0 || o->cheb_mode > 3) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: cheb_mode must be 0..3");
     moto_solver_opts n = *o;
     if (n.check_every == 0) n.check_every = 8;
@@ -211,6 +212,13 @@ moto_status moto_lowest_modes(moto_ctx* c, const double* d_spins, int k, double 
     if (!d_spins || !d_lambda || !d_V) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes: null argument");
     if (k < 1 || k > c->kmax) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes: k out of range [1, kmax]");
     if (!(tol > 0) || max_iter < 0) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes: tol must be > 0, max_iter >= 0");
+    if (persistent_applicable(c, k, max_iter)) {   // small lattice: the whole solve in one persistent kernel (same code as the batch)
+        moto_ctx* one[1] = {c};
+        const double* sp[1] = {d_spins};
+        double* lam[1] = {d_lambda};
+        double* vv[1] = {d_V};
+        return persistent_solve(one, 1, sp, k, tol, max_iter, warm_start, lam, vv, info, nullptr);
+    }
     const size_t bytes = (size_t)k * c->N * 3 * sizeof(double);
     if (warm_start) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->X, d_V, bytes, cudaMemcpyDeviceToDevice, c->stream));
     moto_status s = solve_internal(c, d_spins, k, tol, max_iter, warm_start, info);
@@ -232,6 +240,15 @@ moto_status moto_lowest_modes_batch(moto_ctx* const* ctxs, int P, const double* 
         for (int q = 0; q < p; ++q)
             if (ctxs[q] == ctxs[p]) return moto_fail(ctxs[p], MOTO_EINVAL, "moto_lowest_modes_batch: the same context appears twice");
     }
+    // batched path: every problem on the same small nearest-neighbour lattice -> one persistent kernel for all of them
+    bool same = tol > 0 && max_iter >= 1 && k >= 1;
+    for (int p = 0; p < P && same; ++p) {
+        const moto_ctx* a = ctxs[0]; const moto_ctx* b = ctxs[p];
+        same = d_spins[p] && d_lambda[p] && d_V[p] && persistent_applicable(b, k, max_iter) && b->lat.Lx == a->lat.Lx && b->lat.Ly == a->lat.Ly &&
+               b->lat.pbc_x == a->lat.pbc_x && b->lat.pbc_y == a->lat.pbc_y && memcmp(&b->sp, &a->sp, sizeof(moto_spin_params)) == 0 &&
+               b->opts.seed == a->opts.seed;
+    }
+    if (same) return persistent_solve(ctxs, P, d_spins, k, tol, max_iter, warm_start, d_lambda, d_V, infos, statuses);
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return MOTO_ECUDA;
     std::vector<int32_t> st(P, (int32_t)MOTO_OK);

@@ -30,6 +30,7 @@ struct SolverState {
     double lz_h[MOTO_LZ_MAX + 1];             // Gram-Schmidt coefficients of the current pass
     double lz_beta, lz_rbeta;                 // ||u|| of the current step and its reciprocal
     int lz_cycle, lz_pad;                     // index of the last restart cycle whose Rayleigh-Ritz ran
+    unsigned long long pbar;                  // barrier counter of the persistent small-lattice solver (lobpcg_persistent.cu)
     // ---- tail mirrored to the host (layout == HostStatus)
     double theta[MOTO_KMAX];
     double resid[MOTO_KMAX];
@@ -198,6 +199,10 @@ moto_status mmf_cg_run(moto_ctx*, double* d_state, int k, double delta, double s
 moto_status solve_first_column(moto_ctx*, const double* d_state, int kb, double tol, int max_iter, int warm, double* d_lambda, double* d_V,
                                moto_solve_info* info);   // api.cu
 moto_status relax_seed(moto_ctx*, const double* d_saddle, const double* d_v, double s_eta, double* d_out);
+// lobpcg_persistent.cu
+bool persistent_applicable(const moto_ctx*, int k, int max_iter);
+moto_status persistent_solve(moto_ctx* const* ctxs, int P, const double* const* d_spins, int k, double tol, int max_iter, int warm_start,
+                             double* const* d_lambda, double* const* d_V, moto_solve_info* infos, int32_t* statuses);
 // lobpcg.cu
 moto_status lobpcg_solve(moto_ctx*, const double* d_state, int k, double tol, int max_iter, int warm_start,
                          moto_solve_info* info);

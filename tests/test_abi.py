@@ -55,7 +55,7 @@ def test_struct_sizes_match_header():
     assert C.sizeof(b.SpinParams) == 7 * 8
     assert C.sizeof(b.MorseParams) == 4 * 8
     assert C.sizeof(b.SolveInfo) == 8 + 8 * b.KMAX + 8
-    assert C.sizeof(b.SolverOpts) == 16 + 16 + 8 + 8 + 8   # + method, ncv, cheb_mode, reserved_
+    assert C.sizeof(b.SolverOpts) == 16 + 16 + 8 + 8 + 8   # + method, ncv, cheb_mode, persistent
     assert C.sizeof(b.Lattice) == 24 + 32 + 8
     assert C.sizeof(b.RelaxInfo) == 16 + 24
 
