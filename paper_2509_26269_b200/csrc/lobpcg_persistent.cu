@@ -100,16 +100,21 @@ struct RRs {
 // eigen-decomposition of the symmetric n x n matrix A (n <= 6) by round-robin parallel Jacobi: A -> diagonal, V = eigenvectors
 // (columns).  All 32 lanes of one warp call it; T is scratch.
 __device__ void warp_jacobi(double* A, double* V, double* T, double* cs, double* sn, int* partner, int n, int lane) {
-    for (int t = lane; t < NM * NM; t += 32) V[t] = (t / NM == t % NM) ? 1.0 : 0.0;
+    // lane owns the matrix entries e = lane and lane + 32 of the NM x NM array (row e / NM, column e % NM: constant divisors)
+    const int e0 = lane, e1 = lane + 32;
+    const int i0 = e0 / NM, j0 = e0 % NM, i1 = e1 / NM, j1 = e1 % NM;
+    const bool in0 = i0 < n && j0 < n, in1 = e1 < NM * NM && i1 < n && j1 < n;
+    V[e0] = (i0 == j0) ? 1.0 : 0.0;
+    if (e1 < NM * NM) V[e1] = (i1 == j1) ? 1.0 : 0.0;
     __syncwarp();
     const int np = (n + 1) & ~1;
-    for (int sweep = 0; sweep < 12; ++sweep) {
-        double off = 0.0;
-        for (int t = lane; t < n * n; t += 32) { const int i = t / n, j = t - i * n; if (i != j) off += A[i * NM + j] * A[i * NM + j]; }
-        double dg = 0.0;
-        if (lane < n) dg = A[lane * NM + lane] * A[lane * NM + lane];
+    for (int sweep = 0; sweep < 10 && np >= 2; ++sweep) {
+        double off = 0.0, dg = 0.0;
+        if (in0) { const double v = A[e0] * A[e0]; if (i0 == j0) dg += v; else off += v; }
+        if (in1) { const double v = A[e1] * A[e1]; if (i1 == j1) dg += v; else off += v; }
         off = warp_sum(off); dg = warp_sum(dg);
-        if (!(off > 1e-34 * dg) || np < 2) break;        // converged (or NaN: the caller flags it)
+        if (!(off > 1e-30 * dg)) break;
+        // off-diagonal part at rounding level of the diagonal (or NaN: the caller flags it)
         for (int r = 0; r < np - 1; ++r) {
             // pairs of round r: (np - 1, r) and ((r + i) mod (np - 1), (r - i) mod (np - 1)), i = 1 .. np/2 - 1
             if (lane < np / 2) {
@@ -117,13 +122,13 @@ __device__ void warp_jacobi(double* A, double* V, double* T, double* cs, double*
                 if (lane == 0) { p = np - 1; q = r; }
                 else { p = (r + lane) % (np - 1); q = (r - lane + (np - 1)) % (np - 1); }
                 if (p > q) { const int t = p; p = q; q = t; }
-                double c = 1.0, s = 0.0;
                 if (q < n) {
-                    const double apq = A[p * NM + q], app = A[p * NM + p], aqq = A[q * NM + q];
+                    const double apq = A[p * NM + q], dd = A[q * NM + q] - A[p * NM + p];
+                    double c = 1.0, s = 0.0;
                     if (fabs(apq) > 1e-300) {
-                        const double tau = (aqq - app) / (2.0 * apq);
-                        const double t = (tau >= 0.0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
-                        c = 1.0 / sqrt(1.0 + t * t); s = t * c;
+                        // tan of the rotation angle: the smaller root of t^2 + (dd / apq) t - 1 = 0, cancellation-free form
+                        const double t = (dd >= 0.0 ? 2.0 : -2.0) * apq / (fabs(dd) + sqrt(fma(dd, dd, 4.0 * apq * apq)));
+                        c = rsqrt(fma(t, t, 1.0)); s = t * c;
                     }
                     // column p of J: (c at p, -s at q); column q: (s at p, c at q)
                     cs[p] = c; sn[p] = -s; partner[p] = q;
@@ -132,20 +137,16 @@ __device__ void warp_jacobi(double* A, double* V, double* T, double* cs, double*
             }
             __syncwarp();
             // T = J^T A : T(i, l) = cs_i A(i, l) + sn_i A(partner_i, l)
-            for (int t = lane; t < n * n; t += 32) {
-                const int i = t / n, l = t - i * n;
-                T[i * NM + l] = cs[i] * A[i * NM + l] + sn[i] * A[partner[i] * NM + l];
-            }
+            if (in0) T[e0] = cs[i0] * A[e0] + sn[i0] * A[partner[i0] * NM + j0];
+            if (in1) T[e1] = cs[i1] * A[e1] + sn[i1] * A[partner[i1] * NM + j1];
             __syncwarp();
             // A = T J : A(i, j) = T(i, j) cs_j + T(i, partner_j) sn_j ;  V = V J likewise
-            double va[2];
-            for (int t = lane, u = 0; t < n * n; t += 32, ++u) {
-                const int i = t / n, j = t - i * n;
-                A[i * NM + j] = T[i * NM + j] * cs[j] + T[i * NM + partner[j]] * sn[j];
-                va[u] = V[i * NM + j] * cs[j] + V[i * NM + partner[j]] * sn[j];
-            }
+            double v0 = 0.0, v1 = 0.0;
+            if (in0) { A[e0] = T[e0] * cs[j0] + T[i0 * NM + partner[j0]] * sn[j0]; v0 = V[e0] * cs[j0] + V[i0 * NM + partner[j0]] * sn[j0]; }
+            if (in1) { A[e1] = T[e1] * cs[j1] + T[i1 * NM + partner[j1]] * sn[j1]; v1 = V[e1] * cs[j1] + V[i1 * NM + partner[j1]] * sn[j1]; }
             __syncwarp();
-            for (int t = lane, u = 0; t < n * n; t += 32, ++u) { const int i = t / n, j = t - i * n; V[i * NM + j] = va[u]; }
+            if (in0) V[e0] = v0;
+            if (in1) V[e1] = v1;
             __syncwarp();
         }
     }
@@ -248,15 +249,21 @@ __device__ void warp_rr(RRs& s, int n, int nev, double* theta, double* C, int la
     __syncwarp();
 }
 
-// sum of nv values over the chunks of one problem, in chunk order (lane-strided, then a shuffle tree): the same for every
-// CTA of the problem and for every cpp.  out[v] valid after the trailing __syncthreads.
-__device__ void reduce_chunks(const double* part, int nchunk, int nv, double* out) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
-    for (int v = warp; v < nv; v += nw) {
+// Sum of nv (<= 64) values over the chunks of one problem in a fixed order that depends on nchunk only (so it is the same
+// for every CTA of the problem and for every cpp): thread (v, g) adds the chunks g, g + G, ... (all loads of the CTA in
+// flight together), then thread v combines the G group sums in order.  out[v] valid after the trailing __syncthreads.
+__device__ void reduce_chunks(const double* part, int nchunk, int nv, double* out, double* scratch /*[PT]*/) {
+    const int G = PT / nv, v = threadIdx.x % nv, g = threadIdx.x / nv;
+    if (g < G) {
         double s = 0.0;
-        for (int ch = lane; ch < nchunk; ch += 32) s += __ldcg(part + (size_t)ch * nv + v);
-        s = warp_sum(s);
-        if (lane == 0) out[v] = s;
+        for (int ch = g; ch < nchunk; ch += G) s += __ldcg(part + (size_t)ch * nv + v);
+        scratch[g * nv + v] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x < nv) {
+        double s = 0.0;
+        for (int gg = 0; gg < G; ++gg) s += scratch[gg * nv + threadIdx.x];
+        out[threadIdx.x] = s;
     }
     __syncthreads();
 }
@@ -268,6 +275,7 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
     __shared__ double sC[3 * KB * KB + KB];
     __shared__ double sval[NEU + NK];
     __shared__ double ssign[KB];
+    __shared__ double sscr[PT];
     __shared__ RRs rr;
     __shared__ int s_stop;
     const int prob = blockIdx.x / q.cpp, jc = blockIdx.x - prob * q.cpp;
@@ -356,8 +364,8 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
     bool done = false, bad = false;
     for (int it = 0;; ++it) {
         // ------------------------------------------------------------ R: partial sums, residual test, Rayleigh-Ritz
-        reduce_chunks(partU[parity], q.nchunk, NEU, sval);
-        if (it > 0) reduce_chunks(partK, q.nchunk, NK, sval + NEU);
+        reduce_chunks(partU[parity], q.nchunk, NEU, sval, sscr);
+        if (it > 0) reduce_chunks(partK, q.nchunk, NK, sval + NEU, sscr);
         if (tid == 0) {
             int stop = 0;
             if (it > 0) {
