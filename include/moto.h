@@ -232,6 +232,24 @@ moto_status moto_relax(moto_ctx* ctx, double* d_state, int max_steps, double tau
 moto_status moto_two_sided_descent(moto_ctx* ctx, const double* d_saddle, const double* d_vmin, double eta, int max_steps,
                                    double tau_F, double alpha0, double* d_min_plus, double* d_min_minus, moto_relax_info* info);
 
+/* The L-BFGS variants of the two loops above -- the paper's primary optimiser ("We employ a GPU implementation of
+ * LBFGS ... and a nonlinear conjugate-gradient (CG) variant for comparison"; Alg. 1 l.12, l.17).  The paper calls
+ * a library routine and prints no algorithm; readings A29, A30:
+ * moto_relax_lbfgs: RelaxDownHill.  History of at most m pairs s = T(a d), y = g_new - T(g_old), all transported to the current
+ *   tangent space at every accepted step (projection for spins, identity for atoms); d = -H g by the two-loop recursion with
+ *   H_0 = (s.y / y.y) I of the newest pair, d = -g while the history is empty; a pair is kept only if s.y > 1e-10 |s| |y|;
+ *   acceptance test of moto_relax (reading A26) on trial steps a = a_0, a_0/2, ... with a_0 = 1 (alpha0-scaled first-step
+ *   length while the history is empty); a direction that is not downhill or along which every trial fails drops the history.
+ *   d_scratch: caller-owned device scratch [2 m + 5][N][3].  info / return values as moto_relax.  One synchronisation per trial.
+ * moto_mmf_run_lbfgs: the outer climb, x <- R(x + p), p = H F_mmf with pairs s = T(p), y = -(F_new - T(F_old)), H_0 = alpha0 I
+ *   while the history is empty, |p|_2 capped at smax, history dropped if F.p <= 0.  ONE minimum-mode solve per iteration
+ *   (moto_mmf_run_cg spends two).  d_scratch: [2 m + 4][N][3].  Other arguments, termination test, info and return values as
+ *   moto_mmf_run.  1 <= m <= 8. */
+moto_status moto_relax_lbfgs(moto_ctx* ctx, double* d_state, int max_steps, double tau_F, double alpha0, int m, double* d_scratch,
+                             moto_relax_info* info);
+moto_status moto_mmf_run_lbfgs(moto_ctx* ctx, double* d_state, int k, double alpha0, double smax, int max_steps, double tau_F, double tol,
+                               int max_iter, int warm_start, int m, double* d_V, double* d_scratch, moto_mmf_info* info);
+
 /* Vector transport for warm starts after m -> m' (reading A17): V <- orthonormalise(P_{m'} V), in place. */
 moto_status moto_transport(moto_ctx* ctx, const double* d_spins_new, double* d_V, int k);
 

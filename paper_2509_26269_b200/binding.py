@@ -91,6 +91,9 @@ _SIGS = {
                                          C.c_void_p, C.c_void_p, C.POINTER(RelaxInfo)]),
     "moto_mmf_run_cg": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
                                   C.c_void_p, C.c_void_p, C.POINTER(MmfInfo)]),
+    "moto_relax_lbfgs": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int, C.c_void_p, C.POINTER(RelaxInfo)]),
+    "moto_mmf_run_lbfgs": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
+                                     C.c_int, C.c_void_p, C.c_void_p, C.POINTER(MmfInfo)]),
     "moto_transport": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "moto_gram": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
     "moto_rayleigh_ritz": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
@@ -309,6 +312,30 @@ class Context:
                                                   float(tol), int(max_iter), warm, _ptr(V), _ptr(scratch), C.byref(info)), allow=(ENOTCONV,))
         return V, dict(steps=info.steps, converged=bool(info.converged), fnorm=info.fnorm, lam=list(info.lam)[:k],
                        hvp_count=info.hvp_count, solver_iters=info.solver_iters, status=st)
+
+    def mmf_run_lbfgs(self, state, k, alpha0, smax, max_steps, tau_F, tol, max_iter=20000, V0=None, m=8):
+        """moto_mmf_run_lbfgs: outer MMF loop with the L-BFGS step rule; `state` is updated in place.  -> (V, info dict)."""
+        _dev_f64(state, (self.N, 3))
+        if V0 is not None:
+            V, warm = _dev_f64(V0, (k, self.N, 3)).clone(), 1
+        else:
+            V, warm = self._empty(k, self.N, 3), 0
+        scratch = self._empty(2 * m + 4, self.N, 3)
+        info = MmfInfo()
+        st = self._check(self.lib.moto_mmf_run_lbfgs(self._h, _ptr(state), k, float(alpha0), float(smax), int(max_steps), float(tau_F),
+                                                     float(tol), int(max_iter), warm, int(m), _ptr(V), _ptr(scratch), C.byref(info)),
+                         allow=(ENOTCONV,))
+        return V, dict(steps=info.steps, converged=bool(info.converged), fnorm=info.fnorm, lam=list(info.lam)[:k],
+                       hvp_count=info.hvp_count, solver_iters=info.solver_iters, status=st)
+
+    def relax_lbfgs(self, state, max_steps, tau_F, alpha0, m=8):
+        """moto_relax_lbfgs: relax `state` downhill in place (L-BFGS, history m).  -> info dict."""
+        _dev_f64(state, (self.N, 3))
+        scratch = self._empty(2 * m + 5, self.N, 3)
+        info = RelaxInfo()
+        st = self._check(self.lib.moto_relax_lbfgs(self._h, _ptr(state), int(max_steps), float(tau_F), float(alpha0), int(m), _ptr(scratch),
+                                                   C.byref(info)), allow=(ENOTCONV,))
+        return info.as_dict(st)
 
     def relax(self, state, max_steps, tau_F, alpha0):
         """moto_relax: relax `state` downhill in place (CG + backtracking).  -> info dict."""

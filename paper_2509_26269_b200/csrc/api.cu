@@ -371,6 +371,25 @@ moto_status moto_relax(moto_ctx* c, double* d_state, int max_steps, double tau_F
     return relax_run(c, d_state, max_steps, tau_F, alpha0, info);
 }
 
+moto_status moto_relax_lbfgs(moto_ctx* c, double* d_state, int max_steps, double tau_F, double alpha0, int m, double* d_scratch,
+                             moto_relax_info* info) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_state || !d_scratch) return moto_fail(c, MOTO_EINVAL, "moto_relax_lbfgs: null argument");
+    if (max_steps < 0 || !(tau_F >= 0) || !(alpha0 > 0) || m < 1 || m > 8)
+        return moto_fail(c, MOTO_EINVAL, "moto_relax_lbfgs: need max_steps >= 0, tau_F >= 0, alpha0 > 0, 1 <= m <= 8");
+    return relax_lbfgs_run(c, d_state, max_steps, tau_F, alpha0, m, d_scratch, info);
+}
+
+moto_status moto_mmf_run_lbfgs(moto_ctx* c, double* d_state, int k, double alpha0, double smax, int max_steps, double tau_F, double tol,
+                               int max_iter, int warm_start, int m, double* d_V, double* d_scratch, moto_mmf_info* info) {
+    if (!c) return MOTO_EINVAL;
+    if (!d_state || !d_V || !d_scratch) return moto_fail(c, MOTO_EINVAL, "moto_mmf_run_lbfgs: null argument");
+    if (k < 2 || k > c->kmax) return moto_fail(c, MOTO_EINVAL, "moto_mmf_run_lbfgs: k out of range [2, kmax] (the saddle test needs lambda_2)");
+    if (!(tol > 0) || max_iter < 0 || max_steps < 0 || !(tau_F >= 0) || !(alpha0 > 0) || !(smax > 0) || m < 1 || m > 8)
+        return moto_fail(c, MOTO_EINVAL, "moto_mmf_run_lbfgs: bad tolerance, cap, step length or history size (1 <= m <= 8)");
+    return mmf_lbfgs_run(c, d_state, k, alpha0, smax, max_steps, tau_F, tol, max_iter, warm_start, m, d_V, d_scratch, info);
+}
+
 moto_status moto_two_sided_descent(moto_ctx* c, const double* d_saddle, const double* d_vmin, double eta, int max_steps, double tau_F,
                                    double alpha0, double* d_min_plus, double* d_min_minus, moto_relax_info* info) {
     if (!c) return MOTO_EINVAL;

@@ -196,6 +196,9 @@ moto_status lanczos_solve(moto_ctx*, const double* d_state, int k, double tol, i
 moto_status relax_run(moto_ctx*, double* d_state, int max_steps, double tau_F, double alpha0, moto_relax_info* info);
 moto_status mmf_cg_run(moto_ctx*, double* d_state, int k, double delta, double smax, int max_steps, double tau_F, double tol, int max_iter,
                        int warm_start, double* d_V, double* d_scratch, moto_mmf_info* info);
+moto_status relax_lbfgs_run(moto_ctx*, double* d_state, int max_steps, double tau_F, double alpha0, int M, double* d_scratch, moto_relax_info* info);
+moto_status mmf_lbfgs_run(moto_ctx*, double* d_state, int k, double alpha0, double smax, int max_steps, double tau_F, double tol, int max_iter,
+                          int warm_start, int M, double* d_V, double* d_scratch, moto_mmf_info* info);
 moto_status solve_first_column(moto_ctx*, const double* d_state, int kb, double tol, int max_iter, int warm, double* d_lambda, double* d_V,
                                moto_solve_info* info);   // api.cu
 moto_status relax_seed(moto_ctx*, const double* d_saddle, const double* d_v, double s_eta, double* d_out);

@@ -371,3 +371,281 @@ moto_status mmf_cg_run(moto_ctx* c, double* d_state, int k, double delta, double
     if (info) *info = out;
     return ret;
 }
+
+// ================================================================ L-BFGS variants (readings A29, A30; "We employ a
+// GPU implementation of LBFGS ... and a nonlinear conjugate-gradient (CG) variant for comparison", :262, :275)
+// The inverse-Hessian product is evaluated in the span of {q, s_1..s_n, y_1..y_n}: ONE Gram launch gives every inner
+// product the two-loop recursion needs (the pairs are re-transported at every step, so their inner products change and are
+// recomputed anyway), the recursion itself then runs on coefficient vectors on the host (it synchronises once per trial
+// already), and ONE pass forms the direction as a linear combination.  Per accepted step: transport of the history (one
+// projection pass over 2n vectors), new pair (one pass), Gram (one pass), combination (one pass).
+namespace {
+
+constexpr int LB_MAX = 8;                       // largest history M
+constexpr int LB_NV = 2 * LB_MAX + 1;
+constexpr double LB_CURV_EPS = 1e-10;
+
+struct LinComb { const double* v[LB_NV]; double coef[LB_NV]; int n; };
+
+__global__ void __launch_bounds__(256) k_lincomb(long long n3, LinComb lc, double* __restrict__ out) {
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n3; e += (long long)gridDim.x * blockDim.x) {
+        double s = 0.0;
+        for (int b = 0; b < lc.n; ++b) s = fma(lc.coef[b], lc.v[b][e], s);
+        out[e] = s;
+    }
+}
+
+// new pair at the accepted point xt:  s = a T(d),  y = sy (g_t - T(g))   (T = tangent projection at xt for spins, identity for atoms)
+__global__ void __launch_bounds__(256) k_lbfgs_pair(long long N, const double* __restrict__ xt, const double* __restrict__ d, double a,
+                                                    const double* __restrict__ gt, const double* __restrict__ g, double sy, int project,
+                                                    double* __restrict__ s_out, double* __restrict__ y_out) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        d3 di = ld3(d, i), gi = ld3(g, i);
+        if (project) { const d3 x = ld3(xt, i); di = proj3(x, di); gi = proj3(x, gi); }
+        const d3 gn = ld3(gt, i);
+        st3(s_out, i, scale3(a, di));
+        st3(y_out, i, scale3(sy, sub3(gn, gi)));
+    }
+}
+
+struct LbfgsHist {
+    double* S[LB_MAX]; double* Y[LB_MAX];   // slot storage
+    int order[LB_MAX + 1];                  // slots in use, oldest first
+    int n, M;
+};
+
+// r = H q in coefficients over {q, S[order[0..n)], Y[order[0..n)]}; G: Gram of that basis, row-major (2n+1)^2, index 0 = q,
+// 1 + i = s_i, 1 + n + i = y_i (i in history order).  gamma0: H_0 = gamma0 I when the history is empty.
+void lbfgs_coeffs(const double* G, int n, double gamma0, double* r /*[2n+1]*/) {
+    const int nb = 2 * n + 1;
+    double q[LB_NV], al[LB_MAX];
+    for (int b = 0; b < nb; ++b) q[b] = 0.0;
+    q[0] = 1.0;
+    if (n == 0) { r[0] = gamma0; return; }
+    auto dot = [&](int row, const double* cf) { double s = 0.0; for (int b = 0; b < nb; ++b) s += cf[b] * G[row * nb + b]; return s; };
+    for (int i = n - 1; i >= 0; --i) {
+        const double rho = 1.0 / G[(1 + i) * nb + (1 + n + i)];
+        al[i] = rho * dot(1 + i, q);
+        q[1 + n + i] -= al[i];
+    }
+    const double gamma = G[(1 + n - 1) * nb + (1 + n + n - 1)] / G[(1 + n + n - 1) * nb + (1 + n + n - 1)];
+    for (int b = 0; b < nb; ++b) r[b] = gamma * q[b];
+    for (int i = 0; i < n; ++i) {
+        const double rho = 1.0 / G[(1 + i) * nb + (1 + n + i)];
+        const double be = rho * dot(1 + n + i, r);
+        r[1 + i] += al[i] - be;
+    }
+}
+
+// Gram of {q, S, Y} to the host (one launch pair + one synchronisation)
+moto_status lbfgs_gram(moto_ctx* c, const LbfgsHist& h, const double* q, double* G_host, double* d_G) {
+    const int nb = 2 * h.n + 1;
+    const double* B[LB_NV];
+    B[0] = q;
+    for (int i = 0; i < h.n; ++i) { B[1 + i] = h.S[h.order[i]]; B[1 + h.n + i] = h.Y[h.order[i]]; }
+    c->launches += block_gram(c, B, nb, B, nb, d_G, nullptr);
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    MOTO_CUDA_CHECK(c, cudaMemcpyAsync(G_host, d_G, (size_t)nb * nb * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return MOTO_OK;
+}
+
+// drop pairs whose curvature s.y is not safely positive (they would break positive definiteness); newest pair last.
+// Returns true if the basis changed (the caller then rebuilds G by deleting rows / columns -- done here in place).
+bool lbfgs_prune_newest(LbfgsHist& h, double* G) {
+    if (h.n == 0) return false;
+    const int n = h.n, nb = 2 * n + 1, i = n - 1;
+    const double sy = G[(1 + i) * nb + (1 + n + i)], ss = G[(1 + i) * nb + (1 + i)], yy = G[(1 + n + i) * nb + (1 + n + i)];
+    if (sy > LB_CURV_EPS * sqrt(ss) * sqrt(yy)) return false;
+    // delete rows / columns (1 + i) and (1 + n + i)
+    double T[LB_NV * LB_NV];
+    int keep[LB_NV], nk = 0;
+    for (int b = 0; b < nb; ++b) if (b != 1 + i && b != 1 + n + i) keep[nk++] = b;
+    for (int a = 0; a < nk; ++a) for (int b = 0; b < nk; ++b) T[a * nk + b] = G[keep[a] * nb + keep[b]];
+    memcpy(G, T, sizeof(double) * nk * nk);
+    h.n = n - 1;
+    return true;
+}
+
+void lbfgs_push_slot(LbfgsHist& h, int* slot_out) {
+    // slot for a new pair: a free one, or the oldest (which is dropped)
+    bool used[LB_MAX] = {false};
+    for (int i = 0; i < h.n; ++i) used[h.order[i]] = true;
+    if (h.n == h.M) { *slot_out = h.order[0]; for (int i = 1; i < h.n; ++i) h.order[i - 1] = h.order[i]; h.n -= 1; }
+    else { int s = 0; while (used[s]) ++s; *slot_out = s; }
+    h.order[h.n] = *slot_out;
+    h.n += 1;
+}
+
+moto_status lbfgs_direction(moto_ctx* c, const LbfgsHist& h, const double* q, const double* r, double sign, double* out) {
+    LinComb lc;
+    lc.n = 2 * h.n + 1;
+    lc.v[0] = q; lc.coef[0] = sign * r[0];
+    for (int i = 0; i < h.n; ++i) {
+        lc.v[1 + i] = h.S[h.order[i]]; lc.coef[1 + i] = sign * r[1 + i];
+        lc.v[1 + h.n + i] = h.Y[h.order[i]]; lc.coef[1 + h.n + i] = sign * r[1 + h.n + i];
+    }
+    k_lincomb<<<grid_for(c->N), 256, 0, c->stream>>>(3ll * c->N, lc, out);
+    c->launches += 1;
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    return MOTO_OK;
+}
+
+}  // namespace
+
+// RelaxDownHill with L-BFGS (reading A29).  d_scratch: [2 M + 5][N][3].
+moto_status relax_lbfgs_run(moto_ctx* c, double* d_state, int max_steps, double tau_F, double alpha0, int M, double* d_scratch,
+                            moto_relax_info* info) {
+    const long long N = c->N;
+    const size_t n3 = (size_t)3 * N, vb = n3 * sizeof(double);
+    const int spin = c->kind == MOTO_KIND_TRI2D;
+    LbfgsHist h; memset(&h, 0, sizeof(h));
+    h.M = M;
+    for (int i = 0; i < M; ++i) { h.S[i] = d_scratch + (size_t)i * n3; h.Y[i] = d_scratch + (size_t)(M + i) * n3; }
+    double* bufs[2] = {d_scratch + (size_t)(2 * M) * n3, d_scratch + (size_t)(2 * M + 1) * n3};
+    double *g = d_scratch + (size_t)(2 * M + 2) * n3, *gt = d_scratch + (size_t)(2 * M + 3) * n3, *d = d_scratch + (size_t)(2 * M + 4) * n3;
+    double* d_G = c->partials + 150000;           // device scratch for the Gram matrix (beyond the reduction partials in use)
+    int which = 0;
+    const double* x = d_state;
+    moto_relax_info out; memset(&out, 0, sizeof(out));
+    double hv[4], G[LB_NV * LB_NV], r[LB_NV];
+    moto_status s = eval_point(c, x, nullptr, 0.0, nullptr, nullptr, g, hv);
+    if (s != MOTO_OK) return s;
+    out.evals = 1;
+    double E = hv[0], gg = hv[1], alpha = alpha0;
+    moto_status ret = MOTO_OK;
+    for (;;) {
+        if (!(gg == gg)) { ret = moto_fail(c, MOTO_ESTATE, "moto_relax_lbfgs: NaN gradient"); break; }
+        if (sqrt(gg) <= tau_F) { out.converged = 1; break; }
+        if (out.steps >= max_steps) { ret = moto_fail(c, MOTO_ENOTCONV, "moto_relax_lbfgs: max_steps reached"); break; }
+        double* xt = bufs[which];
+        bool accepted = false, first = true;
+        double a = 0.0;
+        int npairs = 0;
+        for (;;) {
+            npairs = h.n;
+            double slope;
+            if (npairs) {
+                s = lbfgs_gram(c, h, g, G, d_G);
+                if (s != MOTO_OK) return s;
+                while (lbfgs_prune_newest(h, G)) {}
+                npairs = h.n;
+            }
+            if (npairs) {
+                lbfgs_coeffs(G, npairs, 1.0, r);
+                const int nb = 2 * npairs + 1;
+                slope = 0.0;
+                for (int b = 0; b < nb; ++b) slope -= r[b] * G[b];          // g.d = -sum_b r_b <g, basis_b>
+                if (!(slope < 0.0)) { h.n = 0; continue; }                   // not a descent direction: drop the history
+                s = lbfgs_direction(c, h, g, r, -1.0, d);
+                if (s != MOTO_OK) return s;
+            } else {
+                k_relax_dir<<<grid_for(N), 256, 0, c->stream>>>(N, x, g, 0.0, d, 0);   // d = -g
+                c->launches += 1;
+                slope = -gg;
+            }
+            a = npairs ? 1.0 : alpha;
+            first = true;
+            for (int bt = 0; bt < RELAX_MAX_BACKTRACKS; ++bt) {
+                s = eval_point(c, x, d, a, g, xt, gt, hv);
+                if (s != MOTO_OK) return s;
+                out.evals += 1;
+                const double Et = hv[0], gtd = hv[3];
+                if (gtd <= RELAX_SIGMA * fabs(slope) && (Et <= E + RELAX_C1 * a * slope || Et <= E + RELAX_EPS_E * fabs(E))) { accepted = true; break; }
+                a *= 0.5;
+                first = false;
+            }
+            if (accepted || !npairs) break;
+            h.n = 0;                                                          // every trial along the quasi-Newton direction rejected
+        }
+        if (!accepted) { ret = moto_fail(c, MOTO_ENOTCONV, "moto_relax_lbfgs: stalled (no acceptable step along -g)"); break; }
+        if (!npairs) alpha = first ? 2.0 * a : a;
+        // history to the new tangent space, then the new pair (its curvature is tested with the next Gram)
+        if (spin && h.n > 0)
+            for (int i = 0; i < h.n; ++i) { c->launches += spin_project(c, xt, h.S[h.order[i]], 1); c->launches += spin_project(c, xt, h.Y[h.order[i]], 1); }
+        int slot;
+        lbfgs_push_slot(h, &slot);
+        k_lbfgs_pair<<<grid_for(N), 256, 0, c->stream>>>(N, xt, d, a, gt, g, 1.0, spin, h.S[slot], h.Y[slot]);
+        c->launches += 1;
+        x = xt; which ^= 1;
+        double* t = g; g = gt; gt = t;
+        E = hv[0]; gg = hv[1];
+        out.steps += 1;
+    }
+    if (x != d_state) MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_state, x, vb, cudaMemcpyDeviceToDevice, c->stream));
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    out.energy = E; out.gnorm = sqrt(gg); out.alpha = alpha;
+    if (info) *info = out;
+    return ret;
+}
+
+// Outer climb with the L-BFGS step rule (reading A30).  d_scratch: [2 M + 4][N][3].
+moto_status mmf_lbfgs_run(moto_ctx* c, double* d_state, int k, double alpha0, double smax, int max_steps, double tau_F, double tol,
+                          int max_iter, int warm_start, int M, double* d_V, double* d_scratch, moto_mmf_info* info) {
+    const long long N = c->N;
+    const size_t n3 = (size_t)3 * N;
+    const int spin = c->kind == MOTO_KIND_TRI2D;
+    LbfgsHist h; memset(&h, 0, sizeof(h));
+    h.M = M;
+    for (int i = 0; i < M; ++i) { h.S[i] = d_scratch + (size_t)i * n3; h.Y[i] = d_scratch + (size_t)(M + i) * n3; }
+    double *F = d_scratch + (size_t)(2 * M) * n3, *Fn = d_scratch + (size_t)(2 * M + 1) * n3, *p = d_scratch + (size_t)(2 * M + 2) * n3,
+           *xn = d_scratch + (size_t)(2 * M + 3) * n3;
+    double* d_G = c->partials + 150000;
+    moto_mmf_info out; memset(&out, 0, sizeof(out));
+    auto fail = [&](moto_status e) { if (info) *info = out; return e; };
+    ForceEval fe;
+    moto_status st = eval_force(c, d_state, k, tol, max_iter, warm_start, 0, d_V, F, false, &fe, &out);
+    if (st != MOTO_OK) return fail(st);
+    bool full = c->opts.method != 0;
+    moto_status ret = MOTO_OK;
+    double G[LB_NV * LB_NV], r[LB_NV];
+    for (int step = 0;; ++step) {
+        if (!full && ((fe.fn <= tau_F && fe.lam[0] < 0.0 && fe.lam[1] > 0.0) || step >= max_steps)) {
+            st = eval_force(c, d_state, k, tol, max_iter, 1, 0, d_V, F, true, &fe, &out);
+            if (st != MOTO_OK) return fail(st);
+            full = true;
+        }
+        out.steps = step; out.fnorm = fe.fn;
+        for (int a = 0; a < k; ++a) out.lambda[a] = fe.lam[a];
+        if (full && fe.fn <= tau_F && fe.lam[0] < 0.0 && fe.lam[1] > 0.0) { out.converged = 1; break; }
+        if (step >= max_steps) { ret = moto_fail(c, MOTO_ENOTCONV, "moto_mmf_run_lbfgs: max_steps reached before the saddle test held"); break; }
+        full = c->opts.method != 0;
+        // p = H F, capped at smax
+        double pn2;
+        for (;;) {
+            st = lbfgs_gram(c, h, F, G, d_G);
+            if (st != MOTO_OK) return fail(st);
+            while (lbfgs_prune_newest(h, G)) {}
+            const int nb = 2 * h.n + 1;
+            lbfgs_coeffs(G, h.n, alpha0, r);
+            double Fp = 0.0;
+            for (int b = 0; b < nb; ++b) Fp += r[b] * G[b];
+            if (h.n > 0 && !(Fp > 0.0)) { h.n = 0; continue; }
+            pn2 = 0.0;
+            for (int a = 0; a < nb; ++a) for (int b = 0; b < nb; ++b) pn2 += r[a] * r[b] * G[a * nb + b];
+            break;
+        }
+        const double pn = sqrt(pn2 > 0.0 ? pn2 : 0.0);
+        if (!(pn > 0.0)) { ret = moto_fail(c, MOTO_ESTATE, "moto_mmf_run_lbfgs: zero force"); break; }
+        const double scale = pn > smax ? smax / pn : 1.0;
+        st = lbfgs_direction(c, h, F, r, scale, p);
+        if (st != MOTO_OK) return fail(st);
+        k_relax_trial<<<grid_for(N), 256, 0, c->stream>>>(N, d_state, p, 1.0, xn, spin);
+        c->launches += 1;
+        st = eval_force(c, xn, k, tol, max_iter, 1, 1, d_V, Fn, false, &fe, &out);
+        if (st != MOTO_OK) return fail(st);
+        if (spin && h.n > 0)
+            for (int i = 0; i < h.n; ++i) { c->launches += spin_project(c, xn, h.S[h.order[i]], 1); c->launches += spin_project(c, xn, h.Y[h.order[i]], 1); }
+        int slot;
+        lbfgs_push_slot(h, &slot);
+        k_lbfgs_pair<<<grid_for(N), 256, 0, c->stream>>>(N, xn, p, 1.0, Fn, F, -1.0, spin, h.S[slot], h.Y[slot]);   // s = T(p), y = -(F_new - T(F))
+        c->launches += 1;
+        MOTO_CUDA_CHECK(c, cudaMemcpyAsync(d_state, xn, n3 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+        double* t = F; F = Fn; Fn = t;
+    }
+    MOTO_CUDA_CHECK(c, cudaGetLastError());
+    MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (info) *info = out;
+    return ret;
+}
