@@ -191,7 +191,8 @@ __global__ void __launch_bounds__(LZ_THREADS) k_lz_restart(LzBasis B, int m, int
 }
 
 // v_0 = sum of the first k slots (warm start from a block of directions; reading A25)
-__global__ void __launch_bounds__(LZ_THREADS) k_lz_sum_cols(LzBasis B, int k) {
+__global__ void __launch_bounds__(LZ_THREADS) k_lz_sum_cols(LzBasis B, int k, const int* __restrict__ done = nullptr) {
+    if (done && *done) return;
     for (long long e = blockIdx.x * (long long)LZ_THREADS + threadIdx.x; e < B.n3; e += (long long)gridDim.x * LZ_THREADS) {
         double s = 0.0;
         for (int a = 0; a < k; ++a) s += B.vec(a)[e];
@@ -202,12 +203,26 @@ __global__ void __launch_bounds__(LZ_THREADS) k_lz_sum_cols(LzBasis B, int k) {
 }  // namespace
 
 int lz_ritz(moto_ctx* c, int m, int k, double tol, int cycle);   // rayleigh_ritz.cu
+int fast_negc_max(moto_ctx*, double* partial_max, int* nmax_out);   // lobpcg_fast.cu
+int fast_acheck(moto_ctx*, int kb, int k, double tol, const double* d_T, double* partials, int store);
+int fast_cheb_coef(moto_ctx*, int k, int d, double margin, double lnorm, double hi_user, const double* partial_max, int nmax);
 
 moto_status lanczos_solve(moto_ctx* c, const double* d_state, int k, double tol, int max_iter, int warm_start,
                           moto_solve_info* info) {
     const long long n3 = 3ll * c->N;
     const long long dof = (c->kind == MOTO_KIND_TRI2D) ? 2ll * c->N : 3ll * c->N;
-    int m = (c->nblocks > 8 ? 8 : c->nblocks) * c->kmax - 1;   // the basis lives in the first eight blocks (six for atoms)
+    // Lanczos on the Chebyshev-transformed operator -p_d(A) (the transformation of the LOBPCG path, lobpcg.cu): where the TMA K1
+    // applies and k <= 2, unless precond_degree = -1.  Plain Lanczos stalls on clustered spectra at 10^6 spins (cfg 3: lambda_1..3
+    // within 4e-4 at the bottom of a spectrum 18 wide); on -p_d(A) the wanted end is stretched by ~d^2.  One start cycle on A gives
+    // Ritz values for the first interval; then phases of LZ_PHASE restart cycles on -p_d(A), each phase opened by the true
+    // A-Rayleigh quotients and A-residuals of the current Ritz vectors (the only convergence test) and a new interval from them.
+    int degree = c->opts.precond_degree;
+    const bool can_filter = c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && k <= 2;
+    if (degree == 0) degree = can_filter ? 40 : 0;
+    if (degree < 0 || !can_filter) degree = 0;
+    if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
+    // the recurrence uses T1..T4 as scratch, so the basis then lives in the six solver blocks only
+    int m = (degree > 0 ? 6 : (c->nblocks > 8 ? 8 : c->nblocks)) * c->kmax - 1;
     if (m > MOTO_LZ_MAX) m = MOTO_LZ_MAX;
     if (c->opts.ncv > 0 && c->opts.ncv < m) m = c->opts.ncv;
     if (m > dof - 1) m = (int)(dof - 1);
@@ -235,9 +250,19 @@ moto_status lanczos_solve(moto_ctx* c, const double* d_state, int k, double tol,
     k_lz_upd<2><<<grid, LZ_THREADS, 0, c->stream>>>(B, -1, c->st, c->partials);
     n += 3;
 
+    bool filtered = false, op_failed = false;   // which operator the steps apply: A, or -p_d(A) once an interval exists
+    long long hv = 0;                           // single-vector HVPs enqueued (host count; the device counts steps)
     auto step = [&](int j) {
-        if (c->kind == MOTO_KIND_TRI2D) n += spin_hvp(c, d_state, c->c, B.vec(j), 1, B.vec(j + 1), /*project_input=*/1, &c->st->done);
-        else n += cart_hvp(c, B.vec(j), 1, B.vec(j + 1), &c->st->done);
+        if (filtered) {
+            const int nk = spin_cheb_recurrence(c, d_state, c->c, B.vec(j), 1, degree, B.vec(j + 1), &c->st->cheb[0][0], &c->st->done);
+            if (nk <= 0) op_failed = true; else n += nk;
+            n += spin_project(c, d_state, B.vec(j + 1), 1);   // the recurrence does not re-project (reading A24): keep the basis tangent
+            hv += degree;
+        } else {
+            if (c->kind == MOTO_KIND_TRI2D) n += spin_hvp(c, d_state, c->c, B.vec(j), 1, B.vec(j + 1), /*project_input=*/1, &c->st->done);
+            else n += cart_hvp(c, B.vec(j), 1, B.vec(j + 1), &c->st->done);
+            hv += 1;
+        }
         k_lz_dots<<<grid, LZ_THREADS, 0, c->stream>>>(B, j, c->partials, &c->st->done);
         k_lz_fin<<<1, 32 * (MOTO_LZ_MAX + 1), 0, c->stream>>>(c->partials, grid, j, m, 1, c->st);
         k_lz_upd<1><<<grid, LZ_THREADS, 0, c->stream>>>(B, j, c->st, c->partials);
@@ -249,13 +274,36 @@ moto_status lanczos_solve(moto_ctx* c, const double* d_state, int k, double tol,
     int steps = 0, cycle = 0, k0 = 0, slot = 0, pending = 0, since = 0;
     bool finished = false;
     HostStatus last; memset(&last, 0, sizeof(last));
+    const int LZ_PHASE = 3;                     // restart cycles per interval
+    const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.01;
+    double* pmax = c->partials + (size_t)MOTO_RED_BLOCKS * 128;
+    int nmax = 0, in_phase = 0;
+    if (degree > 0) n += fast_negc_max(c, pmax, &nmax);
     while (!finished) {
         for (int j = k0; j < m; ++j) step(j);
         steps += m - k0; since += m - k0;
         ++cycle;
-        n += lz_ritz(c, m, k, tol, cycle);
+        n += lz_ritz(c, m, k, degree > 0 ? -1.0 : tol, cycle);   // filtered: the Lanczos estimates are those of -p_d(A), never the stop test
         k_lz_restart<<<grid, LZ_THREADS, 0, c->stream>>>(B, m, k, cycle, c->st); ++n;
         k0 = k;
+        if (degree > 0) {
+            // after every restart: T1 = A X of the k Ritz vectors, A-Rayleigh quotients and A-residuals -- the convergence test
+            n += spin_hvp_tma_ex(c, d_state, c->c, c->X, k, c->T1, &c->st->done, nullptr, 0, 0.0, 0.0, 0.0, nullptr, nullptr);
+            n += fast_acheck(c, k, k, tol, c->T1, pmax + 1024, /*store=*/1);
+            hv += k;
+        }
+        if (degree > 0 && (!filtered || ++in_phase >= LZ_PHASE)) {
+            // phase boundary: next interval from the A-Rayleigh quotients, and a fresh Lanczos run on the new operator from the
+            // sum of the Ritz vectors
+            n += fast_cheb_coef(c, k, degree, margin, c->lmax_L, c->opts.precond_hi, pmax, nmax);
+            if (k > 1) { k_lz_sum_cols<<<grid, LZ_THREADS, 0, c->stream>>>(B, k, &c->st->done); ++n; }
+            MOTO_CUDA_CHECK(c, cudaMemsetAsync(c->st->lz_T, 0, sizeof(c->st->lz_T), c->stream));   // no bordered rows of the old run
+            k_lz_dots<<<grid, LZ_THREADS, 0, c->stream>>>(B, -1, c->partials, &c->st->done);
+            k_lz_fin<<<1, 32 * (MOTO_LZ_MAX + 1), 0, c->stream>>>(c->partials, grid, -1, m, 0, c->st);
+            k_lz_upd<2><<<grid, LZ_THREADS, 0, c->stream>>>(B, -1, c->st, c->partials);
+            n += 3;
+            filtered = true; in_phase = 0; k0 = 0;
+        }
         const bool cap = steps >= max_iter;
         if (since >= check_every || cap) {
             since = 0;
@@ -269,8 +317,9 @@ moto_status lanczos_solve(moto_ctx* c, const double* d_state, int k, double tol,
             pending = 1;
             slot ^= 1;
         }
-        if (cap) finished = true;
+        if (cap || op_failed) finished = true;
     }
+    if (op_failed) { c->launches += n; return moto_fail(c, MOTO_ECUDA, "moto_lowest_modes (Lanczos): a launch of the Chebyshev recurrence failed"); }
     MOTO_CUDA_CHECK(c, cudaEventSynchronize(c->ev[slot ^ 1]));
     last = c->hstat[slot ^ 1];
     // true residuals of the returned pairs: AX = Hess[X], r_j = AX_j - theta_j X_j (the stop test used the Lanczos estimates)
@@ -290,7 +339,7 @@ moto_status lanczos_solve(moto_ctx* c, const double* d_state, int k, double tol,
         info->iters = last.iter;
         info->converged = conv;
         for (int a = 0; a < MOTO_KMAX; ++a) info->resid[a] = a < k ? last.resid[a] : 0.0;
-        info->hvp_count = (int64_t)last.nhvp + (last.bad ? 0 : k);
+        info->hvp_count = degree > 0 ? (int64_t)hv + (last.bad ? 0 : k) : (int64_t)last.nhvp + (last.bad ? 0 : k);
     }
     if (last.bad) return moto_fail(c, MOTO_ECUDA, "moto_lowest_modes (Lanczos): numerical breakdown (NaN or an invariant Krylov space)");
     if (!conv) return moto_fail(c, MOTO_ENOTCONV, "moto_lowest_modes (Lanczos): max_iter reached; outputs hold the best iterate");

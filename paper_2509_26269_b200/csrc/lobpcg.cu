@@ -23,7 +23,7 @@ static int project_block(moto_ctx* c, const double* d_state, double* V, int kb) 
 int fast_gram_full(moto_ctx*, int kb, int* nblk_out);
 int fast_dot_waw(moto_ctx*, int kb, const double* W, const double* AW, double* partialsK, int* nblk_out);
 int fast_negc_max(moto_ctx*, double* partial_max, int* nmax_out);
-int fast_acheck(moto_ctx*, int kb, int k, double tol, const double* d_T, double* partials);
+int fast_acheck(moto_ctx*, int kb, int k, double tol, const double* d_T, double* partials, int store = 0);
 int fast_cheb_coef(moto_ctx*, int k, int d, double margin, double lnorm, double hi_user, const double* partial_max, int nmax);
 int fast_update(moto_ctx*, const double* m_or_null, int kb, int* nblk_out);
 int rr_solve_fast(moto_ctx*, int kb, int nblkU, const double* partialsK, int nblkK, int check, int k, double tol, int hvp_inc);

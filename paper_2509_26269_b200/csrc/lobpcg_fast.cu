@@ -193,7 +193,8 @@ __global__ void __launch_bounds__(256) k_acheck_resid(long long n3, const double
     block_reduce_store<KB>(acc, partials + (size_t)blockIdx.x * KB);
 }
 
-__global__ void k_acheck_final(const double* __restrict__ partials, int nblk, int kb, int k, double tol, SolverState* st) {
+// store: also leave theta / resid in the state when the test fails (the Lanczos variant sets its next interval from them)
+__global__ void k_acheck_final(const double* __restrict__ partials, int nblk, int kb, int k, double tol, SolverState* st, int store) {
     if (st->done) return;
     __shared__ double v[MOTO_KMAX];
     const int e = threadIdx.x >> 5, lane = threadIdx.x & 31;   // one warp per column
@@ -213,10 +214,9 @@ __global__ void k_acheck_final(const double* __restrict__ partials, int nblk, in
             if (j < k) ok = ok && (rs[j] <= tol) && (r2 == r2);
         }
         st->nhvp += kb;
-        if (ok) {
+        if (ok || store)
             for (int j = 0; j < kb; ++j) { st->theta[j] = st->scal[j]; st->resid[j] = rs[j]; }
-            st->done = 1;
-        }
+        if (ok) st->done = 1;
     }
 }
 
@@ -281,7 +281,7 @@ int fast_cheb_coef_explicit(moto_ctx* c, int d, double a, double b, double aL) {
 }
 
 // T = A X must already be in d_T.  Sets done (and theta, resid) when every wanted A-residual is below tol.
-int fast_acheck(moto_ctx* c, int kb, int k, double tol, const double* d_T, double* partials) {
+int fast_acheck(moto_ctx* c, int kb, int k, double tol, const double* d_T, double* partials, int store) {
     const long long n3 = 3ll * c->N;
     const int g = fast_grid(n3);
     if (kb == 1) k_acheck_dots<1><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, partials, &c->st->done);
@@ -289,6 +289,6 @@ int fast_acheck(moto_ctx* c, int kb, int k, double tol, const double* d_T, doubl
     k_acheck_theta<<<1, 32 * 2 * kb, 0, c->stream>>>(partials, g, kb, c->st);
     if (kb == 1) k_acheck_resid<1><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, c->st, partials);
     else k_acheck_resid<2><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, c->st, partials);
-    k_acheck_final<<<1, 32 * kb, 0, c->stream>>>(partials, g, kb, k, tol, c->st);
+    k_acheck_final<<<1, 32 * kb, 0, c->stream>>>(partials, g, kb, k, tol, c->st, store);
     return 4;
 }
