@@ -91,7 +91,7 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-ORACLE_SAMPLE = dict(L=400, calls=10)   # the bounded sample BOTH arms time (cpu_baseline leg and --impl reference)
+ORACLE_SAMPLE = dict(L=400, calls=20)   # the bounded sample BOTH arms time (cpu_baseline leg and --impl reference)
 
 
 def oracle_sample(L: int = ORACLE_SAMPLE["L"], calls: int = ORACLE_SAMPLE["calls"]):
