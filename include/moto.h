@@ -296,6 +296,20 @@ moto_status moto_mmf_step_host(moto_ctx* ctx, const double* h_spins, const doubl
  * configuration is not known to be safe.  MOTO_OK for spin lattices. */
 moto_status moto_check_overflow(moto_ctx* ctx);
 
+/* moto_gram_static: moto_gram for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc).  No context and no workspace: G[i][j] = S_i . T_j (the reduced pencil of LOBPCG) for
+ *   d_S [ns][n3], d_T [nt][n3] device, fp64, rows of n3 contiguous elements (n3 = 3 N for a block vector); d_G [ns][nt]
+ *   device, row-major, written by the kernel; stream: a cudaStream_t passed as a plain pointer (NULL = the default stream).
+ * Limit: ns <= 6 and nt <= 12 (the [X W P] x [S, A S] pencil at block size 2); anything larger returns MOTO_EINVAL and
+ * launches nothing -- use moto_gram.  The per-CTA partial sums live in a file-scope __device__ array (170 752 bytes on every
+ * GPU that loads the library, held until the process exits); the call performs no cudaMalloc / cudaFree and calls no
+ * allocating library routine: one 256-byte cudaMemsetAsync (the ticket of the reduction) and one kernel, asynchronous on
+ * `stream`; the caller owns all buffers.  ALL calls on a device share that array: calls that overlap on the GPU (two streams,
+ * no dependency between them) race; order them.  Sums are formed in a fixed order (bit-identical reruns).
+ * moto_gram_static_last_error: message of this host thread's last failed moto_gram_static call ("" after a success). */
+moto_status moto_gram_static(const double* d_S, int ns, const double* d_T, int nt, int64_t n3, double* d_G, void* stream);
+const char* moto_gram_static_last_error(void);
+
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t moto_launch_count(const moto_ctx* ctx);
 const char* moto_version(void);

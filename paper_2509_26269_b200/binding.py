@@ -103,6 +103,8 @@ _SIGS = {
                                          C.c_void_p, C.POINTER(SolveInfo)]),
     "moto_mmf_step_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p, C.c_void_p]),
     "moto_launch_count": (C.c_int64, [C.c_void_p]),
+    "moto_gram_static": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int64, C.c_void_p, C.c_void_p]),
+    "moto_gram_static_last_error": (C.c_char_p, []),
 }
 EXPORTS = tuple(_SIGS)
 
@@ -426,6 +428,20 @@ def lowest_modes_batch(ctxs, spins, k, tol, max_iter=200, V0=None, allow_notconv
     out = [dict(iters=i.iters, converged=bool(i.converged), resid=list(i.resid)[:k], hvp_count=i.hvp_count, status=sts[p])
            for p, i in enumerate(infos)]
     return lams, Vs, out
+
+
+def gram_static(S, T, G, stream=None):
+    """moto_gram_static: G [ns][nt] <- S [ns][...] . T [nt][...] with no context, no workspace and no allocation (the caller
+    passes the output; ns <= 6, nt <= 12).  stream: a raw cudaStream_t handle (int) or None for the default stream."""
+    lib = load_library()
+    ns, nt = S.shape[0], T.shape[0]
+    _dev_f64(S); _dev_f64(T); _dev_f64(G, (ns, nt))
+    n3 = S[0].numel()
+    assert T[0].numel() == n3, "S and T rows differ in length"
+    st = lib.moto_gram_static(_ptr(S), ns, _ptr(T), nt, n3, _ptr(G), stream)
+    if st != OK:
+        raise MotoError(st, lib.moto_gram_static_last_error().decode())
+    return G
 
 
 def spin_context(w, kmax=None, device="cuda:0", stream=None) -> Context:
