@@ -71,7 +71,8 @@ typedef struct {
     int32_t guard;          /* extra block columns iterated but not returned            [0]  */
     int32_t check_every;    /* iterations enqueued between host looks at the status     [8]  */
     int32_t precond_degree; /* degree d of the Chebyshev spectral transformation -p_d(A) LOBPCG runs on:
-                               0 = auto (40 on spin lattices that take the TMA K1 path and kb <= 2, else off; kb > 2: opt-in),
+                               0 = auto (40 on spin lattices that take the TMA K1 path and kb <= 2, 16 inside the persistent
+                               small-lattice kernel, else off; kb > 2: opt-in),
                                -1 = off (plain LOBPCG on A, the paper's solver), 1..256 = degree          [0]  */
     int32_t hvp_path;       /* K1 kernel choice: 0 auto, 1 generic (any lattice), 2 TMA-staged (even Lx >= 8) [0] */
     double precond_lo;      /* margin: the damped interval starts at theta_k + margin           [0 -> 0.01] */
@@ -85,9 +86,11 @@ typedef struct {
                                as measured at 10^6 spins), 1 = one step per pass in one persistent cooperative launch,
                                2 = d dependent launches, 3 = two steps per pass in one cooperative launch with the intermediate
                                step kept in shared memory (spin_cheb2_tma.cu).  All give the same results to rounding.  [0]  */
-    int32_t persistent;     /* the whole solve as ONE persistent cooperative kernel (nearest-neighbour spin lattices up to 32 768
-                               sites that do not take the transformed path, k <= 2, no guard columns): 0 / 1 = where it applies,
-                               2 = never (the multi-launch solver)                                                    [0]  */
+    int32_t persistent;     /* the whole solve as ONE persistent cooperative kernel (nearest-neighbour spin lattices up to 37 888
+                               sites = 148 SMs x 256, k <= 2, no guard columns, method 0): 0 = where it applies, unless an explicit
+                               precond_degree > 0 asks for the multi-launch transformed solver; 1 = also with an explicit
+                               precond_degree <= 32; 2 = never (the multi-launch solver).  Inside the kernel precond_degree 0 = auto
+                               means degree 16 from 1024 sites on (plain LOBPCG below), -1 = plain.                  [0]  */
 } moto_solver_opts;
 
 typedef struct {

@@ -4,16 +4,22 @@
 //
 // On a 70x70 lattice a block vector is 118 KB: the multi-launch LOBPCG of lobpcg.cu spends its 46 us per iteration on launch
 // latency and on a 37 us single-CTA Rayleigh-Ritz, and a population of such solves cannot fill the GPU one launch chain at a
-// time.  Here the whole block LOBPCG (plain operator, block size kb <= 2, same algebra as lobpcg_fast.cu) of P independent
-// problems runs inside one launch:
+// time.  Here the whole block LOBPCG (block size kb <= 2, same algebra as lobpcg_fast.cu) of P independent problems runs
+// inside one launch, for every lattice up to 148 x 256 = 37 888 sites (one 256-site chunk per CTA of a full grid):
 //   grid = P x cpp CTAs, problem index = blockIdx.x / cpp; a problem's cpp CTAs own its 256-site chunks round-robin;
-//   an iteration is  [H: AW = Hess W, W^T A W partials]  barrier  [R: reduce partials, residual test, Rayleigh-Ritz]
+//   an iteration is  [H: AW = op(W), W^T (op W) partials]  barrier  [R: reduce partials, residual test, Rayleigh-Ritz]
 //                    [U: fused update of the six blocks + Gram partials]  barrier
 //   with a barrier among the cpp CTAs of ONE problem only (a counter in that problem's solver state) -- problems never wait
 //   for each other and finish at their own iteration counts;
 //   R is done redundantly by every CTA of the problem from the same partials in the same order (no broadcast step), by one
 //   warp: Cholesky whitening of the unit-diagonal Gram matrix (rank-revealing Jacobi when a pivot is small) and a
 //   round-robin parallel Jacobi on the reduced 3kb x 3kb pencil; nothing leaves the GPU until the kernel ends.
+// op is the Hessian or, from N >= 1024 sites on, the Chebyshev transformation -p_d(A) of lobpcg.cu (d = 16 three-term steps
+// per application, each one pass over the CTA's chunks + the problem barrier): the Rayleigh-Ritz (~35 us, the dominant cost
+// of a plain iteration here) is then paid once per 16 Hessian applications, and the clustered spectra that stall the plain
+// operator (cfg 3 at 100 x 100: 2155 plain iterations) converge in ~50.  8 plain iterations (cold start) fix the interval,
+// phases of 20 transformed iterations follow, each closed by a restart on A that yields the A-Ritz pairs and true
+// A-residuals (the only convergence test while transformed, together with a cheap |A x - theta x| test every 2 iterations).
 // Partial sums are formed per 256-site chunk and combined in chunk order, so the result does not depend on cpp or P: a
 // problem solved alone (moto_lowest_modes) and inside a batch (moto_lowest_modes_batch) give bit-identical results.
 #include "common.cuh"
@@ -28,6 +34,10 @@ using namespace lob;
 constexpr int PT = 256;        // threads per CTA = sites per chunk
 constexpr int PMAXP = 24;      // problems per launch (they travel as kernel parameters)
 constexpr int NM = 6;          // largest pencil (3 kb, kb <= 2)
+constexpr int PDEG = 32;       // largest degree of the Chebyshev transformation inside the kernel
+// precond_degree = 0 (auto): degree, smallest lattice that takes it, plain iterations of a cold start, phase length, iterations
+// between cheap A-residual tests -- swept on cfg 1, its 40x40 instance, random spins 64x64, cfg 3 at 100x100 and the P = 24 batch
+constexpr int PAUTO_DEGREE = 16, PAUTO_MIN_N = 1024, PAUTO_PLAIN = 8, PAUTO_PHASE = 20, PAUTO_ACHECK = 2;
 constexpr double RR_TAU = 1e-10, RR_CHOL = 1e-2;   // rank truncation / Cholesky admission, as on the fused path of rayleigh_ritz.cu
 
 struct PProb {
@@ -36,6 +46,7 @@ struct PProb {
     double* lambda;             // [k] out
     Blk6 b;                     // the six solver blocks of this problem's workspace
     double* c;                  // [N]
+    double *T1, *T2;            // [kb][N][3] each: intermediate steps of the Chebyshev recurrence
     double* part;               // chunk partials
     SolverState* st;
 };
@@ -45,6 +56,9 @@ struct PParams {
     int N, nchunk, cpp, k, max_iter, warm;
     double tol;
     unsigned long long seed;
+    // Chebyshev transformation -p_d(A) (same construction as lobpcg.cu / k_cheb_coef): degree 0 = plain operator throughout
+    int degree, plain_start, phase_len, acheck_every;
+    double margin, lnorm, hi_user;
     HostStatus* out;            // [P] device: what the host reads back (one copy for the whole batch)
 };
 
@@ -278,6 +292,9 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
     __shared__ double sscr[PT];
     __shared__ RRs rr;
     __shared__ int s_stop;
+    __shared__ double scoef[3 * PDEG];
+    __shared__ double s_hi;
+    __shared__ double sack[3 * KB];
     const int prob = blockIdx.x / q.cpp, jc = blockIdx.x - prob * q.cpp;
     const PProb& pr = batch.p[prob];
     const Lat& l = q.l;
@@ -301,95 +318,204 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
         nb[4] = nbi(l, ix, iy, -1, 1); nb[5] = nbi(l, ix, iy, 1, -1);
     };
 
-    // ---------------------------------------------------------------- phase 0: c_i = m_i . g_i, start block, zero W, P
+    // ---------------------------------------------------------------- phase 0: c_i = m_i . g_i, start block, max(-c_i)
     for (int ch = jc; ch < q.nchunk; ch += q.cpp) {
         const int i = ch * PT + tid;
-        if (i >= N) continue;
-        int nb[6];
-        neighbours6(i, nb);
-        const d3 mi = ld3(pr.m, i);
-        const d3 Lm = stencil_apply(l, ldn_cg(pr.m, nb[0]), ldn_cg(pr.m, nb[1]), ldn_cg(pr.m, nb[2]), ldn_cg(pr.m, nb[3]),
-                                    ldn_cg(pr.m, nb[4]), ldn_cg(pr.m, nb[5]), mi.z);
-        pr.c[i] = dot3(mi, Lm) - dot3(mi, muB);
-#pragma unroll
-        for (int a = 0; a < KB; ++a) {
-            d3 x;
-            if (q.warm) x = ld3(pr.V + (size_t)a * n3, i);
-            else {
-                const unsigned long long e = (unsigned long long)a * n3 + 3ull * i;
-                x.x = (double)(splitmix64(q.seed ^ splitmix64(e)) >> 11) * (1.0 / 9007199254740992.0) - 0.5;
-                x.y = (double)(splitmix64(q.seed ^ splitmix64(e + 1)) >> 11) * (1.0 / 9007199254740992.0) - 0.5;
-                x.z = (double)(splitmix64(q.seed ^ splitmix64(e + 2)) >> 11) * (1.0 / 9007199254740992.0) - 0.5;
-            }
-            st3(b.X + (size_t)a * n3, i, proj3(mi, x));
-            const d3 z = mk3(0.0, 0.0, 0.0);
-            st3(b.W + (size_t)a * n3, i, z); st3(b.AW + (size_t)a * n3, i, z);
-            st3(b.P + (size_t)a * n3, i, z); st3(b.AP + (size_t)a * n3, i, z);
-        }
-    }
-    prob_barrier(bar, q.cpp, round, &st->bad);
-    // ---------------------------------------------------------------- phase 1: AX = Hess X, Gram partials of the X block
-    for (int ch = jc; ch < q.nchunk; ch += q.cpp) {
-        const int i = ch * PT + tid;
-        double acc[NEU];
-#pragma unroll
-        for (int t = 0; t < NEU; ++t) acc[t] = 0.0;
+        double negc = -1e300;
         if (i < N) {
             int nb[6];
             neighbours6(i, nb);
             const d3 mi = ld3(pr.m, i);
-            const double ci = pr.c[i];
-            d3 x[KB], ax[KB];
+            const d3 Lm = stencil_apply(l, ldn_cg(pr.m, nb[0]), ldn_cg(pr.m, nb[1]), ldn_cg(pr.m, nb[2]), ldn_cg(pr.m, nb[3]),
+                                        ldn_cg(pr.m, nb[4]), ldn_cg(pr.m, nb[5]), mi.z);
+            const double ci = dot3(mi, Lm) - dot3(mi, muB);
+            pr.c[i] = ci;
+            negc = -ci;
 #pragma unroll
             for (int a = 0; a < KB; ++a) {
-                x[a] = ld3(b.X + (size_t)a * n3, i);
-                ax[a] = axpy3(-ci, x[a], proj3(mi, stencil_at(l, b.X + (size_t)a * n3, nb, x[a].z)));
-                st3(b.AX + (size_t)a * n3, i, ax[a]);
-            }
-#pragma unroll
-            for (int a = 0; a < KB; ++a)
-#pragma unroll
-                for (int c2 = a; c2 < KB; ++c2) {
-                    acc[T::idx(a, c2)] = x[a].x * x[c2].x + x[a].y * x[c2].y + x[a].z * x[c2].z;
-                    acc[NT + T::idx(a, c2)] = x[a].x * ax[c2].x + x[a].y * ax[c2].y + x[a].z * ax[c2].z;
+                d3 x;
+                if (q.warm) x = ld3(pr.V + (size_t)a * n3, i);
+                else {
+                    const unsigned long long e = (unsigned long long)a * n3 + 3ull * i;
+                    x.x = (double)(splitmix64(q.seed ^ splitmix64(e)) >> 11) * (1.0 / 9007199254740992.0) - 0.5;
+                    x.y = (double)(splitmix64(q.seed ^ splitmix64(e + 1)) >> 11) * (1.0 / 9007199254740992.0) - 0.5;
+                    x.z = (double)(splitmix64(q.seed ^ splitmix64(e + 2)) >> 11) * (1.0 / 9007199254740992.0) - 0.5;
                 }
+                st3(b.X + (size_t)a * n3, i, proj3(mi, x));
+            }
         }
-        block_reduce_store<NEU>(acc, partU[0] + (size_t)ch * NEU);
-        __syncthreads();
+        if (q.degree > 0) {   // chunk maximum of -c_i: the upper end of the filter interval is max_i(-c_i) + lambda_max(L)
+            sscr[tid] = negc;
+            __syncthreads();
+            for (int s = PT / 2; s > 0; s >>= 1) {
+                if (tid < s) sscr[tid] = fmax(sscr[tid], sscr[tid + s]);
+                __syncthreads();
+            }
+            if (tid == 0) partMv[ch] = sscr[0];
+            __syncthreads();
+        }
     }
     prob_barrier(bar, q.cpp, round, &st->bad);
+    if (q.degree > 0) {
+        if (tid == 0) {
+            double mx = -1e300;
+            for (int ch = 0; ch < q.nchunk; ++ch) mx = fmax(mx, __ldcg(partMv + ch));
+            s_hi = q.hi_user > 0.0 ? q.hi_user : mx + q.lnorm;
+        }
+        __syncthreads();
+    }
 
-    int parity = 0, iter = 0;
+    int parity = 0, deg = 0;
     long long nhvp = 0;
-    bool done = false, bad = false;
-    for (int it = 0;; ++it) {
+    // One step over this CTA's chunks:  dst = al (Hess[src] - c0 src) + be u   (plain: dst = Hess[src]); u, dst are touched at
+    // the thread's own site only, so dst may be u.  wd: also leave the partials of wd^T dst in partK.  Ends with the barrier.
+    auto op_step = [&](const double* src, const double* u, double* dst, bool plain, double al, double c0, double be, const double* wd) {
+        for (int ch = jc; ch < q.nchunk; ch += q.cpp) {
+            const int i = ch * PT + tid;
+            double acc[NK];
+#pragma unroll
+            for (int t = 0; t < NK; ++t) acc[t] = 0.0;
+            if (i < N) {
+                int nb[6];
+                neighbours6(i, nb);
+                const d3 mi = ld3(pr.m, i);
+                const double ci = pr.c[i];
+                d3 w[KB], y[KB];
+#pragma unroll
+                for (int a = 0; a < KB; ++a) {
+                    const d3 s = ld3(src + (size_t)a * n3, i);
+                    d3 v = axpy3(-ci, s, proj3(mi, stencil_at(l, src + (size_t)a * n3, nb, s.z)));
+                    if (!plain) {
+                        v = scale3(al, axpy3(-c0, s, v));
+                        if (u) v = axpy3(be, ld3(u + (size_t)a * n3, i), v);
+                    }
+                    st3(dst + (size_t)a * n3, i, v);
+                    y[a] = v;
+                    if (wd) w[a] = (wd == src) ? s : ld3(wd + (size_t)a * n3, i);
+                }
+                if (wd) {
+                    int t = 0;
+#pragma unroll
+                    for (int a = 0; a < KB; ++a)
+#pragma unroll
+                        for (int c2 = a; c2 < KB; ++c2) { acc[t] = dot3(w[a], y[c2]); ++t; }
+                }
+            }
+            if (wd) {
+                block_reduce_store<NK>(acc, partK + (size_t)ch * NK);
+                __syncthreads();
+            }
+        }
+        prob_barrier(bar, q.cpp, round, &st->bad);
+    };
+    // DST = op(SRC): the Hessian (deg == 0) or -p_deg(Hess) by the three-term recurrence, Y_i alternating between T1 and T2
+    auto apply_op = [&](const double* SRC, double* DST, bool dots) {
+        if (deg == 0) { op_step(SRC, nullptr, DST, true, 1.0, 0.0, 0.0, dots ? SRC : nullptr); nhvp += KB; return; }
+        double* buf[2] = {pr.T1, pr.T2};
+        const double* ym1 = SRC;       // Y_{i-1}
+        const double* ym2 = nullptr;   // Y_{i-2}
+        for (int i = 1; i <= deg; ++i) {
+            double* dst = (i == deg) ? DST : buf[i & 1];
+            op_step(ym1, ym2, dst, false, scoef[3 * i - 3], scoef[3 * i - 2], scoef[3 * i - 1], (dots && i == deg) ? SRC : nullptr);
+            ym2 = ym1; ym1 = dst;
+        }
+        nhvp += (long long)KB * deg;
+    };
+    // (re)start LOBPCG on span(X) for the current operator: AX = op(X), W = AW = P = AP = 0, Gram partials of the X block
+    auto restart = [&]() {
+        apply_op(b.X, b.AX, false);
+        parity ^= 1;
+        for (int ch = jc; ch < q.nchunk; ch += q.cpp) {
+            const int i = ch * PT + tid;
+            double acc[NEU];
+#pragma unroll
+            for (int t = 0; t < NEU; ++t) acc[t] = 0.0;
+            if (i < N) {
+                d3 x[KB], ax[KB];
+                const d3 z = mk3(0.0, 0.0, 0.0);
+#pragma unroll
+                for (int a = 0; a < KB; ++a) {
+                    x[a] = ld3(b.X + (size_t)a * n3, i); ax[a] = ld3(b.AX + (size_t)a * n3, i);
+                    st3(b.W + (size_t)a * n3, i, z); st3(b.AW + (size_t)a * n3, i, z);
+                    st3(b.P + (size_t)a * n3, i, z); st3(b.AP + (size_t)a * n3, i, z);
+                }
+#pragma unroll
+                for (int a = 0; a < KB; ++a)
+#pragma unroll
+                    for (int c2 = a; c2 < KB; ++c2) {
+                        acc[T::idx(a, c2)] = x[a].x * x[c2].x + x[a].y * x[c2].y + x[a].z * x[c2].z;
+                        acc[NT + T::idx(a, c2)] = x[a].x * ax[c2].x + x[a].y * ax[c2].y + x[a].z * ax[c2].z;
+                    }
+            }
+            block_reduce_store<NEU>(acc, partU[parity] + (size_t)ch * NEU);
+            __syncthreads();
+        }
+        prob_barrier(bar, q.cpp, round, &st->bad);
+    };
+
+    // Phases (as lobpcg.cu): plain_start iterations on A, then phases of phase_len iterations on -p_d(A) with the interval
+    // re-centred on the A-Ritz values at every boundary.  While transformed, convergence is decided on true A-residuals only:
+    // at a boundary the solver restarts on A (probing), one Rayleigh-Ritz on span(X) + update gives the A-Ritz pairs and
+    // W = A X - X Theta, and the next pass tests |W_j|.  Every decision below is taken by all CTAs of the problem from the
+    // same numbers, so they stay in step without a broadcast.
+    int iter = 0, in_phase = 0, nupd = 0;
+    bool done = false, bad = false, fresh = true, probing = false;
+    restart();
+    for (;;) {
         // ------------------------------------------------------------ R: partial sums, residual test, Rayleigh-Ritz
         reduce_chunks(partU[parity], q.nchunk, NEU, sval, sscr);
-        if (it > 0) reduce_chunks(partK, q.nchunk, NK, sval + NEU, sscr);
+        if (!fresh && !probing) reduce_chunks(partK, q.nchunk, NK, sval + NEU, sscr);
         if (tid == 0) {
             int stop = 0;
-            if (it > 0) {
+            if (!fresh) {
                 bool ok = true, nan = false;
                 for (int a = 0; a < KB; ++a) {
                     const double r = sqrt(sval[2 * NT + a]);
-                    if (lead) st->resid[a] = r;
+                    if (lead && deg == 0) st->resid[a] = r;
                     if (a < q.k) { ok = ok && (r <= q.tol); nan = nan || !(r == r); }
                 }
-                if (nan) stop = 3; else if (ok) stop = 1; else if (it > q.max_iter) stop = 2;
+                if (nan) stop = 3; else if (deg == 0 && ok) stop = 1; else if (deg == 0 && iter >= q.max_iter) stop = 2;
             }
             s_stop = stop;
         }
         __syncthreads();
         if (s_stop) { done = s_stop == 1; bad = s_stop == 3; break; }
-        if (it > 0) ++iter;
-        nhvp += KB;
+        if (!fresh && !probing) { ++iter; if (deg > 0) ++in_phase; }
+        if (q.degree > 0 && !fresh) {
+            if (deg == 0 && (probing || iter >= q.plain_start)) {
+                // interval [a, b] from the A-Ritz values of the last Rayleigh-Ritz (sC), coefficients as k_cheb_coef
+                if (tid == 0) {
+                    const double bb = s_hi, aL = sC[3 * KB * KB];
+                    double aa = sC[3 * KB * KB + q.k - 1] + q.margin;
+                    if (aa > 0.5 * (aL + bb)) aa = 0.5 * (aL + bb);
+                    const double e = 0.5 * (bb - aa), c0 = 0.5 * (bb + aa), sig1 = e / (aL - c0);
+                    double sig = sig1;
+                    for (int i = 1; i <= q.degree; ++i) {
+                        double alpha, beta;
+                        if (i == 1) { alpha = sig1 / e; beta = 0.0; }
+                        else { const double sn = 1.0 / (2.0 / sig1 - sig); alpha = 2.0 * sn / e; beta = -sig * sn; sig = sn; }
+                        if (i == q.degree) { alpha = -alpha; beta = -beta; }   // the transformed operator is -p(A)
+                        scoef[3 * i - 3] = alpha; scoef[3 * i - 2] = c0; scoef[3 * i - 1] = beta;
+                    }
+                }
+                __syncthreads();
+                deg = q.degree; in_phase = 0; nupd = 0; probing = false; fresh = true;
+                restart();
+                continue;
+            }
+            if (deg > 0 && (in_phase >= q.phase_len || iter >= q.max_iter)) {
+                deg = 0; nupd = 0; probing = true; fresh = true;
+                restart();
+                continue;
+            }
+        }
         if (warp == 0) {
             for (int t = lane; t < NS * NS; t += 32) {
                 const int i = t / NS, j = t - i * NS;
                 const int a = i < j ? i : j, c2 = i < j ? j : i;
                 const int e = T::idx(a, c2);
                 double ga = sval[NT + e];
-                if (it > 0 && a >= KB && c2 < 2 * KB) ga = sval[NEU + (a - KB) * KB - (a - KB) * (a - KB - 1) / 2 + (c2 - a)];   // (W, W) block from H
+                if (!fresh && a >= KB && c2 < 2 * KB) ga = sval[NEU + (a - KB) * KB - (a - KB) * (a - KB - 1) / 2 + (c2 - a)];   // (W, W) block from H
                 rr.B[i * NM + j] = sval[e];
                 rr.A[i * NM + j] = ga;
             }
@@ -399,7 +525,7 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
         __syncthreads();
         if (rr.bad) { bad = true; break; }
         if (lead) {
-            for (int a = 0; a < KB; ++a) st->theta[a] = sC[3 * KB * KB + a];
+            if (deg == 0) for (int a = 0; a < KB; ++a) st->theta[a] = sC[3 * KB * KB + a];
             st->nkeep = rr.na; st->iter = iter; st->nhvp = nhvp;
         }
         // ------------------------------------------------------------ U: fused update of the six blocks + Gram partials
@@ -414,34 +540,64 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
             __syncthreads();
         }
         prob_barrier(bar, q.cpp, round, &st->bad);
-        // ------------------------------------------------------------ H: AW = Hess W, W^T A W partials
-        for (int ch = jc; ch < q.nchunk; ch += q.cpp) {
-            const int i = ch * PT + tid;
-            double acc[NK];
+        fresh = false;
+        // ------------------------------------------------------------ cheap convergence test between boundaries (transformed only):
+        // T1 = A X, theta_j = x_j.t_j / x_j.x_j, |t_j - theta_j x_j| / |x_j| formed element by element (as fast_acheck, lobpcg_fast.cu)
+        ++nupd;
+        if (deg > 0 && q.acheck_every > 0 && nupd > 1 && (nupd - 1) % q.acheck_every == 0) {
+            for (int ch = jc; ch < q.nchunk; ch += q.cpp) {
+                const int i = ch * PT + tid;
+                double acc[2 * KB];
 #pragma unroll
-            for (int t = 0; t < NK; ++t) acc[t] = 0.0;
-            if (i < N) {
-                int nb[6];
-                neighbours6(i, nb);
-                const d3 mi = ld3(pr.m, i);
-                const double ci = pr.c[i];
-                d3 w[KB], aw[KB];
+                for (int t = 0; t < 2 * KB; ++t) acc[t] = 0.0;
+                if (i < N) {
+                    int nb[6];
+                    neighbours6(i, nb);
+                    const d3 mi = ld3(pr.m, i);
+                    const double ci = pr.c[i];
+#pragma unroll
+                    for (int a = 0; a < KB; ++a) {
+                        const d3 x = ld3(b.X + (size_t)a * n3, i);
+                        const d3 t = axpy3(-ci, x, proj3(mi, stencil_at(l, b.X + (size_t)a * n3, nb, x.z)));
+                        st3(pr.T1 + (size_t)a * n3, i, t);
+                        acc[2 * a] = dot3(x, x); acc[2 * a + 1] = dot3(x, t);
+                    }
+                }
+                block_reduce_store<2 * KB>(acc, partK + (size_t)ch * 2 * KB);   // 2 KB <= NK + KB: partK and partMv are free here
+                __syncthreads();
+            }
+            nhvp += KB;
+            prob_barrier(bar, q.cpp, round, &st->bad);
+            reduce_chunks(partK, q.nchunk, 2 * KB, sack, sscr);
+            for (int ch = jc; ch < q.nchunk; ch += q.cpp) {
+                const int i = ch * PT + tid;
+                double acc[KB];
 #pragma unroll
                 for (int a = 0; a < KB; ++a) {
-                    w[a] = ld3(b.W + (size_t)a * n3, i);
-                    aw[a] = axpy3(-ci, w[a], proj3(mi, stencil_at(l, b.W + (size_t)a * n3, nb, w[a].z)));
-                    st3(b.AW + (size_t)a * n3, i, aw[a]);
+                    acc[a] = 0.0;
+                    if (i < N) {
+                        const double th = sack[2 * a + 1] / sack[2 * a];
+                        const d3 x = ld3(b.X + (size_t)a * n3, i), t = ld3(pr.T1 + (size_t)a * n3, i);
+                        const d3 r = axpy3(-th, x, t);
+                        acc[a] = dot3(r, r);
+                    }
                 }
-                int t = 0;
-#pragma unroll
-                for (int a = 0; a < KB; ++a)
-#pragma unroll
-                    for (int c2 = a; c2 < KB; ++c2) { acc[t] = dot3(w[a], aw[c2]); ++t; }
+                block_reduce_store<KB>(acc, partU[parity ^ 1] + (size_t)ch * KB);   // the other parity's partials were consumed by R
+                __syncthreads();
             }
-            block_reduce_store<NK>(acc, partK + (size_t)ch * NK);
-            __syncthreads();
+            prob_barrier(bar, q.cpp, round, &st->bad);
+            reduce_chunks(partU[parity ^ 1], q.nchunk, KB, sack + 2 * KB, sscr);
+            bool ok = true;
+            for (int a = 0; a < q.k; ++a) ok = ok && (sqrt(sack[2 * KB + a] / sack[2 * a]) <= q.tol);
+            if (ok) {
+                if (lead) for (int a = 0; a < KB; ++a) { st->theta[a] = sack[2 * a + 1] / sack[2 * a]; st->resid[a] = sqrt(sack[2 * KB + a] / sack[2 * a]); }
+                ++iter;
+                done = true;
+                break;
+            }
         }
-        prob_barrier(bar, q.cpp, round, &st->bad);
+        // ------------------------------------------------------------ H: AW = op(W), W^T (op W) partials (not needed for a probe)
+        if (!(probing && q.degree > 0)) apply_op(b.W, b.AW, true);
     }
 
     // ---------------------------------------------------------------- finish: exactly tangent, sign-normalised block out
@@ -502,13 +658,15 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
 }  // namespace
 
 // May this context's solve run in the persistent kernel?  Nearest-neighbour spin lattice, block size <= 2 without guard
-// columns, plain LOBPCG (small lattices never take the transformation), small enough that a solve is launch-latency bound.
+// columns, LOBPCG, small enough that a solve is latency bound (one chunk per CTA of a full cooperative grid).
 bool persistent_applicable(const moto_ctx* c, int k, int max_iter) {
     if (c->kind != MOTO_KIND_TRI2D || c->nsh > 0 || c->opts.method != 0 || c->opts.guard > 0 || c->keep_guard) return false;
     if (k < 1 || k > 2 || k > c->kmax || max_iter < 1) return false;
-    if (c->opts.hvp_path == 2 || c->opts.precond_degree > 0 || c->opts.persistent == 2) return false;   // forced TMA / transformation / opt-out
+    if (c->opts.hvp_path == 2 || c->opts.persistent == 2) return false;                                 // forced TMA path / opt-out
+    // an explicit degree asks for the multi-launch transformation of lobpcg.cu unless the persistent kernel is asked for too
+    if (c->opts.precond_degree > 0 && (c->opts.persistent != 1 || c->opts.precond_degree > PDEG || !c->T1 || !c->T2)) return false;
     if (2ll * c->N < 3ll * k) return false;
-    return c->N <= 32768 && !(spin_tma_applicable(c) && c->opts.precond_degree == 0 && c->N >= 16384);
+    return c->N <= PT * MOTO_NUM_SMS;   // 37 888 sites: one 256-site chunk per CTA of a full cooperative grid
 }
 
 // Solve P problems (ctxs[p], d_spins[p]) in one launch chain on ctxs[0]'s stream; all contexts share lattice and parameters
@@ -535,12 +693,18 @@ moto_status persistent_solve(moto_ctx* const* ctxs, int P, const double* const* 
             PProb& pr = batch.p[p];
             pr.m = d_spins[p0 + p]; pr.V = d_V[p0 + p]; pr.lambda = d_lambda[p0 + p];
             pr.b.X = c->X; pr.b.W = c->W; pr.b.P = c->P; pr.b.AX = c->AX; pr.b.AW = c->AW; pr.b.AP = c->AP;
-            pr.c = c->c; pr.part = c->partials; pr.st = c->st;
+            pr.c = c->c; pr.T1 = c->T1; pr.T2 = c->T2; pr.part = c->partials; pr.st = c->st;
             MOTO_CUDA_CHECK(c0, cudaMemsetAsync(c->st, 0, sizeof(SolverState), c0->stream));
         }
         PParams q;
         q.l = make_lat(c0); q.N = N; q.nchunk = nchunk; q.cpp = cpp; q.k = k; q.max_iter = max_iter; q.warm = warm_start;
         q.tol = tol; q.seed = c0->opts.seed; q.out = d_out;
+        // transformation: precond_degree 0 = auto, < 0 = off; every context of the batch needs the two recurrence blocks
+        q.degree = c0->opts.precond_degree > 0 ? c0->opts.precond_degree : (c0->opts.precond_degree == 0 && N >= PAUTO_MIN_N ? PAUTO_DEGREE : 0);
+        for (int p = 0; p < Pn; ++p) if (!batch.p[p].T1 || !batch.p[p].T2) q.degree = 0;
+        if (3ll * k * 8 > 2ll * N) q.degree = 0;
+        q.plain_start = warm_start ? 0 : PAUTO_PLAIN; q.phase_len = PAUTO_PHASE; q.acheck_every = PAUTO_ACHECK;
+        q.margin = c0->opts.precond_lo > 0 ? c0->opts.precond_lo : 0.01; q.lnorm = c0->lmax_L; q.hi_user = c0->opts.precond_hi;
         void* args[2] = {(void*)&batch, (void*)&q};
         const void* fn = k == 1 ? (const void*)k_lobpcg_persistent<1> : (const void*)k_lobpcg_persistent<2>;
         MOTO_CUDA_CHECK(c0, cudaLaunchCooperativeKernel(fn, dim3(Pn * cpp), dim3(PT), args, 0, c0->stream));
