@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmoto.so")
 SOURCES = ["api.cu", "lobpcg.cu", "lobpcg_fast.cu", "lobpcg_persistent.cu", "block_algebra.cu", "rayleigh_ritz.cu", "lanczos.cu", "relax.cu", "spin_stencil.cu", "spin_stencil_tma.cu",
-           "spin_cheb2_tma.cu", "spin_shells.cu", "cart_morse.cu", "gram_static.cu"]
+           "spin_cheb2_tma.cu", "spin_shells.cu", "spin_shells_dense.cu", "cart_morse.cu", "gram_static.cu"]
 ARCH_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMPILE_FLAGS = ARCH_FLAGS + ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-O2"]
 LINK_FLAGS = ARCH_FLAGS + ["-shared", "-cudart", "static", "-lpthread"]

@@ -63,7 +63,8 @@ static WsLayout ws_layout(const moto_lattice* lat, int kmax) {
     w.cart = lat->kind == MOTO_KIND_CARTESIAN ? cart_lists_bytes(lat) : 0;
     w.nblocks = lat->kind == MOTO_KIND_TRI2D ? 10 : 6;   // spin lattices: + four rotating blocks of the Chebyshev recurrence
     w.flags = 4096;
-    w.shell = lat->kind == MOTO_KIND_TRI2D ? al256((size_t)MOTO_MAX_SHELLS * (2 * sizeof(int) + 4 * sizeof(double))) : 0;
+    w.shell = lat->kind == MOTO_KIND_TRI2D ? al256((size_t)MOTO_MAX_SHELLS * (2 * sizeof(int) + 4 * sizeof(double))) +
+                                                 al256((size_t)MOTO_SH_DENSE * 4 * sizeof(double)) + al256((size_t)MOTO_SH_SEGS * 4 * sizeof(int)) : 0;
     w.total = w.nblocks * w.block + w.c + w.g + w.stage + w.partials + w.st + w.flags + w.shell + w.cart;
     return w;
 }
@@ -120,7 +121,12 @@ moto_status moto_create(const moto_lattice* lat, const void* params, void* d_wor
     c->partials = (double*)p; p += w.partials;
     c->st = (SolverState*)p; p += w.st;
     c->flags = (unsigned long long*)p; p += w.flags;
-    if (w.shell) { c->sh_jd = (double*)p; c->sh_off = (int*)(p + (size_t)MOTO_MAX_SHELLS * 4 * sizeof(double)); p += w.shell; }
+    if (w.shell) {
+        c->sh_jd = (double*)p; c->sh_off = (int*)(p + (size_t)MOTO_MAX_SHELLS * 4 * sizeof(double));
+        char* p2 = p + al256((size_t)MOTO_MAX_SHELLS * (2 * sizeof(int) + 4 * sizeof(double)));
+        c->sh_jd2 = (double*)p2; c->sh_seg = (int*)(p2 + al256((size_t)MOTO_SH_DENSE * 4 * sizeof(double)));
+        p += w.shell;
+    }
     if (c->kind == MOTO_KIND_CARTESIAN) cart_lists_carve(c, p);
     cudaError_t e = cudaHostAlloc((void**)&c->hstat, 2 * sizeof(HostStatus), cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->flags, 0, w.flags, c->stream);

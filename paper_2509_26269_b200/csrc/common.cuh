@@ -13,6 +13,9 @@
 #define MOTO_RED_BLOCKS 296  // CTAs of every grid-reduction kernel (2 per SM): fixed => deterministic sums
 #define MOTO_MAX_NEIGH 160   // Cartesian: neighbour capacity per atom
 #define MOTO_MAX_SHELLS 512 // largest neighbour table of moto_set_shells
+#define MOTO_SH_DENSE 1024  // dense column-segment form of the table: entries (zero-filled holes included) ...
+#define MOTO_SH_SEGS 128    // ... segments of <= 12 taps of one dx column ...
+#define MOTO_SH_GROUPS 16   // ... and tap groups (warps of a CTA)
 #define MOTO_CHEB_MAX 256    // largest degree of the Chebyshev spectral transformation
 
 // Device-resident LOBPCG state: Gram matrices, Ritz coefficients, residuals, control flags.
@@ -106,6 +109,12 @@ struct moto_ctx {
     int nsh;           // > 0: general neighbour shells (moto_set_shells) replace the nearest-neighbour J, D of sp
     int* sh_off;       // [MOTO_MAX_SHELLS][2] device
     double* sh_jd;     // [MOTO_MAX_SHELLS][4] device: J, Dx, Dy, Dz
+    // the same table as dense column segments for the register-blocked kernel (spin_shells_dense.cu); sh_nseg == 0: not available
+    int sh_nseg, sh_nd;              // segments, dense entries (holes zero-filled)
+    int sh_Hx, sh_Hy;                // halo: largest |dx|, |dy| of the table
+    int sh_grp[3][MOTO_SH_GROUPS + 1];   // tap groups for S = 8, 12, 16 warps per staged field: group s owns segments [grp[s], grp[s + 1])
+    int* sh_seg;       // [MOTO_SH_SEGS][4] device: dx, dy0, n, first entry
+    double* sh_jd2;    // [MOTO_SH_DENSE][4] device
     HostStatus* hstat;  // pinned
     cudaEvent_t ev[2];
     int64_t launches;
@@ -162,6 +171,10 @@ int shell_three_term(moto_ctx*, const double* m, const double* cvec, const doubl
                      const double* U, double* out);
 int shell_mmf_pass1(moto_ctx*, const double* m, const double* v, int kr);
 moto_status shell_set(moto_ctx*, int n, const int32_t* h_off, const double* h_J, const double* h_D);
+// spin_shells_dense.cu: register-blocked direct convolution (k <= 2); 0 launches = not applicable, the caller falls back
+moto_status shell_dense_build(moto_ctx*, int n, const int32_t* h_off, const double* h_jd);
+int shell_dense_hvp(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input, const int* d_done,
+                    int cheb, double alpha, double c0, double beta, const double* U);
 // cart_morse.cu
 int cart_build_lists(moto_ctx*, const double* x);
 int cart_energy_grad(moto_ctx*, const double* x, double* d_E, double* d_g);

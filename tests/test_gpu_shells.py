@@ -157,3 +157,35 @@ def test_set_shells_errors(moto):
     cart = moto.cart_context(wl.small_cluster(5, seed=2))
     off = np.ascontiguousarray(w.offsets, np.int32)
     assert lib.moto_set_shells(cart._h, len(off), off.ctypes.data, w.Jd.ctypes.data, np.ascontiguousarray(w.Dd).ctypes.data) == moto.binding.ESTATE
+
+
+# ---------------------------------------------------------------- the register-blocked kernel (spin_shells_dense.cu)
+# Lx >= 32 and k <= 2 take k_shell_dense: fields staged in shared memory with the boundary handled there, R = 2 or 3 output
+# rows per thread (R = 3 when that leaves the fullest SM less work: 96 x 100 gives 150 CTAs at R = 2, 102 at R = 3).
+@pytest.mark.parametrize("Lx,Ly,pbc,rcut", [(70, 50, (0, 0), 5.0),      # R = 2, open: zeros beyond every edge, runs A + B in most CTAs
+                                             (33, 47, (1, 0), 4.5),      # R = 2, odd sizes: last row group has one row
+                                             (96, 100, (0, 0), 3.0),     # R = 3, open, last row group has one row (100 = 33 x 3 + 1)
+                                             (96, 100, (0, 1), 3.0),     # R = 3, open x / periodic y
+                                             (32, 40, (1, 1), 10.0)])    # halo (11) wraps a 32-wide lattice; 366 taps
+def test_dense_kernel_parity_api_and_three_term(moto, Lx, Ly, pbc, rcut):
+    w = shell_workload(Lx, Ly, pbc, rcut, seed=Lx + 3 * Ly)
+    mdl = model_of(w)
+    ctx = moto.shell_context(w, kmax=2)
+    x = dev(w.spins)
+    for k in (1, 2):
+        V = wl.random_block(w.N, k, seed=10 + k)                       # not tangent: the API projects the neighbours
+        HV = ctx.hvp(x, dev(V)).cpu().numpy()
+        assert rel_l2(HV, sh.hvp(mdl, w.spins, V)) <= 1e-11
+        assert np.max(np.abs(np.sum(HV * w.spins[None], axis=2))) <= 1e-12
+        # solver mode (tangent input, c from the context): out = alpha (Hess[V] - c0 V) + beta U
+        Vt = V - np.sum(V * w.spins[None], axis=2, keepdims=True) * w.spins[None]
+        U = wl.random_block(w.N, k, seed=20 + k)
+        alpha, c0, beta = 0.37, -0.8, 1.9
+        out = ctx.hvp_three_term(x, dev(Vt), alpha, c0, beta, dev(U)).cpu().numpy()
+        ref = alpha * (sh.hvp(mdl, w.spins, Vt) - c0 * Vt) + beta * U
+        assert rel_l2(out, ref) <= 1e-11
+        out0 = ctx.hvp_three_term(x, dev(Vt), 1.0, 0.0, 0.0, None, refresh_c=False).cpu().numpy()
+        assert rel_l2(out0, sh.hvp(mdl, w.spins, Vt)) <= 1e-11
+    # reruns are bit-identical (fixed summation order)
+    a = ctx.hvp(x, dev(V)).cpu().numpy()
+    assert np.array_equal(a, HV)
