@@ -153,6 +153,22 @@ def hvp(model: ShellModel, m: np.ndarray, V: np.ndarray) -> np.ndarray:
     return np.ascontiguousarray(out.T).reshape(k, model.N, 3)
 
 
+def transformed_operator_apply(model: ShellModel, m: np.ndarray, V: np.ndarray, d: int, a: float, b: float, a_L: float):
+    """-p_d(Hess) V for tangent-projected V ([k][N][3]): the Chebyshev spectral transformation of the solver (DESIGN.md 5,
+    Zhou-Saad filter p_d(x) = T_d(l(x)) / T_d(l(a_L)), l(x) = (2x - a - b)/(b - a)) written out by its SPECTRAL definition --
+    eigh of the explicit tangent Hessian, the polynomial applied to the eigenvalues -- as spin_oracle.transformed_operator_apply
+    does for the stencil model.  Pins: degree 1 in closed form, p_d(a_L) = 1 on an eigenvector, the nearest-neighbour table
+    against the pinned spin oracle, T_d against numpy.polynomial (tests/test_oracle_shell.py)."""
+    Ht, Bm = tangent_hessian(model, m, dense=True)
+    lam, Y = scipy.linalg.eigh(0.5 * (Ht + Ht.T))
+    ell = lambda x: (2.0 * x - a - b) / (b - a)
+    pl = so.chebyshev_T(d, ell(lam)) / so.chebyshev_T(d, np.array([ell(a_L)]))[0]
+    k = V.shape[0]
+    coeff = Y.T @ (Bm.T @ V.reshape(k, -1).T)
+    out = -(Bm @ (Y @ (pl[:, None] * coeff)))
+    return np.ascontiguousarray(out.T).reshape(k, model.N, 3)
+
+
 def mmf_step(model: ShellModel, m: np.ndarray, v: np.ndarray, dt: float) -> np.ndarray:
     """Eq. 2 + retraction (PAPER.md:64, :262, :305), as spin_oracle.mmf_step."""
     F = -projected_gradient(model, m)

@@ -98,3 +98,34 @@ def test_open_boundaries_drop_bonds_and_table_validation():
     D2 = D.copy(); D2[0, 2] += 0.1
     with pytest.raises(AssertionError):
         sh.ShellModel(5, 5, 1, 1, offs, J, D2, 0.0, (0, 0, 0))                      # D(-d) != -D(d)
+
+
+def test_transformed_operator_spectral_definition():
+    # the Chebyshev transformation -p_d(Hess) on a shell table (the operator the transformed shell solver iterates on)
+    mdl = shell_model(8, 3.0, (1, 0), Lx=9)
+    m = wl.random_spins(9, 8, 4)
+    V = wl.random_block(72, 2, 6)
+    a, b, aL = -0.4, 40.0, -1.5
+    # degree 1 in closed form: p_1(x) = (x - c0) / (a_L - c0), applied through the pinned HVP
+    PV = V - np.sum(V * m[None], axis=2, keepdims=True) * m[None]
+    c0 = 0.5 * (a + b)
+    ref1 = -(sh.hvp(mdl, m, V) - c0 * PV) / (aL - c0)
+    assert np.max(np.abs(sh.transformed_operator_apply(mdl, m, V, 1, a, b, aL) - ref1)) < 1e-12
+    # p_d(a_L) = 1: an eigenvector with eigenvalue a_L goes to minus itself; every other eigenvector is scaled by
+    # -T_d(l(lambda)) / T_d(l(a_L)) with T_d from numpy.polynomial (not the oracle's cos / cosh form)
+    lam, Vm = sh.lowest_modes(mdl, m, 3)
+    out = sh.transformed_operator_apply(mdl, m, Vm[:1], 7, lam[0] + 0.3, 40.0, lam[0])
+    assert np.max(np.abs(out + Vm[:1])) < 1e-10
+    d, a2, b2 = 6, lam[1] + 0.05, 40.0
+    ell = lambda x: (2.0 * x - a2 - b2) / (b2 - a2)
+    Td = np.polynomial.chebyshev.Chebyshev.basis(d)
+    out3 = sh.transformed_operator_apply(mdl, m, Vm, d, a2, b2, lam[0])
+    for j in range(3):
+        assert np.max(np.abs(out3[j] + Td(ell(lam[j])) / Td(ell(lam[0])) * Vm[j])) < 1e-9
+    # the nearest-neighbour table gives the pinned spin oracle's operator
+    mdl1 = shell_model(6, 1.0, (1, 1), Dz1=0.0, Lx=7)
+    ref = so.SpinModel(7, 6, 1, 1, 1.0, 0.3, 0.05, (0.01, -0.02, 0.03))
+    m1 = wl.random_spins(7, 6, 5)
+    V1 = wl.random_block(42, 2, 3)
+    assert np.max(np.abs(sh.transformed_operator_apply(mdl1, m1, V1, 5, -0.2, 15.0, -0.9)
+                         - so.transformed_operator_apply(ref, m1, V1, 5, -0.2, 15.0, -0.9))) < 1e-10
