@@ -166,7 +166,9 @@ moto_status moto_set_shells(moto_ctx* c, int n, const int32_t* h_offsets, const 
     if (!c) return MOTO_EINVAL;
     if (c->kind != MOTO_KIND_TRI2D) return moto_fail(c, MOTO_ESTATE, "moto_set_shells: spin lattices only");
     if (n < 0 || n > MOTO_MAX_SHELLS || (n > 0 && (!h_offsets || !h_J || !h_D))) return moto_fail(c, MOTO_EINVAL, "moto_set_shells: need 0 <= n <= 512 and non-null tables");
-    return shell_set(c, n, h_offsets, h_J, h_D);
+    const moto_status s = shell_set(c, n, h_offsets, h_J, h_D);
+    if (s == MOTO_OK && n == 0) c->lmax_L = stencil_lmax_bound(c->sp);
+    return s;
 }
 
 const char* moto_last_error(const moto_ctx* c) { return c ? c->err : "null context"; }
@@ -457,7 +459,7 @@ moto_status moto_cheb_apply(moto_ctx* c, const double* d_spins, const double* d_
     MOTO_CUDA_CHECK(c, cudaMemsetAsync(&c->st->done, 0, 4 * sizeof(int), c->stream));
     n += fast_cheb_coef_explicit(c, d, a, b, a_L);
     const int nk = spin_cheb_recurrence(c, d_spins, c->c, d_V, k, d, d_out, &c->st->cheb[0][0], nullptr);
-    if (nk <= 0) return moto_fail(c, MOTO_ESTATE, "moto_cheb_apply: needs the TMA K1 path (even Lx >= 8; hvp_path != 1)");
+    if (nk <= 0) return moto_fail(c, MOTO_ESTATE, "moto_cheb_apply: needs the TMA K1 path (even Lx >= 8; hvp_path != 1) or, on general shells, the dense kernel (Lx >= 32)");
     n += nk;
     c->launches += n;
     MOTO_CUDA_CHECK(c, cudaGetLastError());

@@ -174,7 +174,10 @@ moto_status shell_set(moto_ctx*, int n, const int32_t* h_off, const double* h_J,
 // spin_shells_dense.cu: register-blocked direct convolution (k <= 2); 0 launches = not applicable, the caller falls back
 moto_status shell_dense_build(moto_ctx*, int n, const int32_t* h_off, const double* h_jd);
 int shell_dense_hvp(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input, const int* d_done,
-                    int cheb, double alpha, double c0, double beta, const double* U);
+                    int cheb, double alpha, double c0, double beta, const double* U, const double* d_coef);
+bool shell_dense_applicable(const moto_ctx*, int k);
+int shell_cheb_recurrence(moto_ctx*, const double* m, const double* cvec, const double* V, int k, int d, double* OUT, const double* d_coef,
+                          const int* d_done);
 // cart_morse.cu
 int cart_build_lists(moto_ctx*, const double* x);
 int cart_energy_grad(moto_ctx*, const double* x, double* d_E, double* d_g);

@@ -9,6 +9,8 @@
 #include <stdlib.h>
 #include "common.cuh"
 
+constexpr int SHELL_AUTO_DEGREE = 16;   // precond_degree = 0 on general shells (HVP-bound: a lower degree than the stencil's 40)
+
 static int apply_operator(moto_ctx* c, const double* d_state, const double* V, int kb, double* AV) {
     if (c->kind == MOTO_KIND_TRI2D) return spin_hvp(c, d_state, c->c, V, kb, AV, /*project_input=*/0, &c->st->done);
     return cart_hvp(c, V, kb, AV, &c->st->done);
@@ -110,13 +112,16 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
 
     // spectral transformation: precond_degree 0 = auto (40 where the TMA K1 applies), < 0 = off
     int degree = c->opts.precond_degree;
-    const bool can_filter = c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && 3ll * kb * 8 <= 2ll * c->N;
-    if (degree == 0) degree = can_filter ? 40 : 0;
+    const bool shells = shell_dense_applicable(c, kb);   // general shells: the recurrence runs on k_shell_dense, one launch per step
+    const bool can_filter = c->kind == MOTO_KIND_TRI2D && (spin_tma_applicable(c) || shells) && c->T1 && 3ll * kb * 8 <= 2ll * c->N;
+    if (degree == 0) degree = can_filter ? (shells ? SHELL_AUTO_DEGREE : 40) : 0;
     if (degree < 0 || !can_filter) degree = 0;
     if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
     const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.01;
     // cold start: 20 plain iterations first so that theta_k (hence a) means something; a warm start already has it
-    const int phase_len = 20, plain_start = warm_start ? 0 : 20;   // tuned on cfg 3 (two seeds) and its 316^2 instance
+    // tuned on cfg 3 (two seeds) and its 316^2 instance; shells (degree 16, 12 plain iterations) on the 366-neighbour table at
+    // 36^2, 64^2 and 100^2
+    const int phase_len = 20, plain_start = warm_start ? 0 : (shells ? 12 : 20);
     const int acheck_every = 4;
     const double lnorm = c->lmax_L;   // b = max_i(-c_i) + lambda_max(L) >= lambda_max(Hess)
 
@@ -150,7 +155,8 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
             ++in_phase;
             if (transformed && in_phase < phase_len && in_phase % acheck_every == 0) {
                 // cheap convergence test between restarts: T1 = A X, |A x_j - (x_j.A x_j) x_j| (T1/T2 are free between applies)
-                f.n += spin_hvp_tma_ex(c, d_state, c->c, c->X, kb, c->T1, &c->st->done, nullptr, 0, 0.0, 0.0, 0.0, nullptr, nullptr);
+                if (shells) f.n += apply_operator(c, d_state, c->X, kb, c->T1);
+                else f.n += spin_hvp_tma_ex(c, d_state, c->c, c->X, kb, c->T1, &c->st->done, nullptr, 0, 0.0, 0.0, 0.0, nullptr, nullptr);
                 f.n += fast_acheck(c, kb, k, tol, c->T1, pmax + 1024);
             }
         }

@@ -502,6 +502,7 @@ int spin_cheb2_multistep(moto_ctx* c, const double* m, const double* cvec, const
 // Returns the number of launches, or -1 if the TMA K1 path does not apply / a launch failed (nothing usable in OUT).
 int spin_cheb_recurrence(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
                          const double* d_coef, const int* d_done) {
+    if (c->nsh > 0) return shell_cheb_recurrence(c, m, cvec, V, k, d, OUT, d_coef, d_done);   // general shells: one launch per step
     const int mode = c->opts.cheb_mode;
     double* T[4] = {c->T1, c->T2, c->T3, c->T4};
     if (mode == 3 && d >= 2) {

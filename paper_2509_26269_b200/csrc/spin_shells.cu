@@ -203,7 +203,7 @@ int shell_energy_grad(moto_ctx* c, const double* m, double* d_E, double* d_g, do
 }
 
 int shell_hvp(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input, const int* d_done) {
-    if (const int nd = shell_dense_hvp(c, m, cvec, V, k, HV, project_input, d_done, 0, 0.0, 0.0, 0.0, nullptr)) return nd;
+    if (const int nd = shell_dense_hvp(c, m, cvec, V, k, HV, project_input, d_done, 0, 0.0, 0.0, 0.0, nullptr, nullptr)) return nd;
     const int grid = shell_grid(c);
 #define SHELL_HVP(P, KT) k_shell_hvp<P, false, KT><<<grid, 256, 0, c->stream>>>(make_lat(c), tab_of(c), m, cvec, V, k, HV, d_done, 0.0, 0.0, 0.0, nullptr)
     if (project_input) { if (k == 1) SHELL_HVP(true, 1); else if (k == 2) SHELL_HVP(true, 2); else SHELL_HVP(true, MOTO_KMAX); }
@@ -215,7 +215,7 @@ int shell_hvp(moto_ctx* c, const double* m, const double* cvec, const double* V,
 int shell_three_term(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double alpha, double c0, double beta,
                      const double* U, double* out) {
     if (cvec)
-        if (const int nd = shell_dense_hvp(c, m, cvec, V, k, out, 0, nullptr, 1, alpha, c0, beta, U)) return nd;
+        if (const int nd = shell_dense_hvp(c, m, cvec, V, k, out, 0, nullptr, 1, alpha, c0, beta, U, nullptr)) return nd;
     if (k <= 2) k_shell_hvp<false, true, 2><<<shell_grid(c), 256, 0, c->stream>>>(make_lat(c), tab_of(c), m, cvec, V, k, out, nullptr, alpha, c0, beta, U);
     else k_shell_hvp<false, true, MOTO_KMAX><<<shell_grid(c), 256, 0, c->stream>>>(make_lat(c), tab_of(c), m, cvec, V, k, out, nullptr, alpha, c0, beta, U);
     return 1;
@@ -230,7 +230,7 @@ int shell_mmf_pass1(moto_ctx* c, const double* m, const double* v, int kr) {
 
 // host side of moto_set_shells: validate (distinct, non-zero, inversion symmetric), copy the table into the workspace
 moto_status shell_set(moto_ctx* c, int n, const int32_t* h_off, const double* h_J, const double* h_D) {
-    if (n == 0) { c->nsh = 0; c->sh_nseg = 0; return MOTO_OK; }
+    if (n == 0) { c->nsh = 0; c->sh_nseg = 0; return MOTO_OK; }   // (moto_set_shells restores the stencil's lmax_L)
     for (int t = 0; t < n; ++t) {
         const int dx = h_off[2 * t], dy = h_off[2 * t + 1];
         if (dx == 0 && dy == 0) return moto_fail(c, MOTO_EINVAL, "moto_set_shells: zero offset");
@@ -249,5 +249,9 @@ moto_status shell_set(moto_ctx* c, int n, const int32_t* h_off, const double* h_
     MOTO_CUDA_CHECK(c, cudaMemcpyAsync(c->sh_jd, jd, (size_t)n * 4 * sizeof(double), cudaMemcpyHostToDevice, c->stream));
     MOTO_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
     c->nsh = n;
+    // ||L|| <= 2 sum_delta (|J_delta| + |D_delta|) + 2 |K|: the upper end of the Chebyshev interval is max_i(-c_i) + this
+    double bound = 2.0 * fabs(c->sp.K);
+    for (int t = 0; t < n; ++t) bound += 2.0 * (fabs(h_J[t]) + sqrt(h_D[3 * t] * h_D[3 * t] + h_D[3 * t + 1] * h_D[3 * t + 1] + h_D[3 * t + 2] * h_D[3 * t + 2]));
+    c->lmax_L = bound;
     return shell_dense_build(c, n, h_off, jd);
 }

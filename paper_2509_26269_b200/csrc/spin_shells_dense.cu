@@ -63,7 +63,7 @@ template <bool PROJECT, bool NEEDC, bool CHEB, int KT, int R>
 __global__ void __launch_bounds__(768) k_shell_dense(Lat l, DenseTab tb, int Hx, int Hy, const double* __restrict__ m,
                                                                                     const double* __restrict__ cvec, const double* __restrict__ V,
                                                                                     double* __restrict__ HV, const int* __restrict__ done,
-                                                                                    double alpha, double c0, double beta, const double* U) {
+                                                                                    double alpha, double c0, double beta, const double* U, const double* __restrict__ d_coef) {
     constexpr int NF = KT + (NEEDC ? 1 : 0);     // staged / accumulated fields: the KT directions (+ m)
     constexpr int NV = NF * R * 3;               // sums per lane
     extern __shared__ double smem[];
@@ -193,6 +193,7 @@ __global__ void __launch_bounds__(768) k_shell_dense(Lat l, DenseTab tb, int Hx,
         const d3 Lv = mk3(-2.0 * sa[0], -2.0 * sa[32], -2.0 * sa[64] - 2.0 * l.K * vi.z);
         d3 h = axpy3(-c, vi, proj3(mi, Lv));
         if (CHEB) {
+            if (d_coef) { alpha = d_coef[0]; c0 = d_coef[1]; beta = d_coef[2]; }   // coefficients computed on the device (k_cheb_coef)
             h = scale3(alpha, axpy3(-c0, vi, h));
             if (U) h = axpy3(beta, ld3(U + ofs, i), h);
         }
@@ -283,7 +284,7 @@ moto_status shell_dense_build(moto_ctx* c, int n, const int32_t* h_off, const do
 
 // 1 launch, or 0 when this kernel does not apply (k > 2, no dense table): the caller falls back to k_shell_hvp
 int shell_dense_hvp(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input, const int* d_done,
-                    int cheb, double alpha, double c0, double beta, const double* U) {
+                    int cheb, double alpha, double c0, double beta, const double* U, const double* d_coef) {
     if (c->sh_nseg <= 0 || k < 1 || k > 2 || c->lat.Lx < 32) return 0;
     const int Hx = c->sh_Hx, Hy = c->sh_Hy;
     const bool needc = cvec == nullptr;
@@ -304,7 +305,7 @@ int shell_dense_hvp(moto_ctx* c, const double* m, const double* cvec, const doub
     do {                                                                                                                   \
         static std::atomic<unsigned long long> seen{0};                                                                    \
         if (smem > 48 * 1024 && !tma::ensure_smem_attr(k_shell_dense<P, NC, CH, KT, RR>, 200 * 1024, seen)) return 0;      \
-        k_shell_dense<P, NC, CH, KT, RR><<<grid, 32 * S * nf, smem, c->stream>>>(l, tb, Hx, Hy, m, cvec, V, HV, d_done, alpha, c0, beta, U); \
+        k_shell_dense<P, NC, CH, KT, RR><<<grid, 32 * S * nf, smem, c->stream>>>(l, tb, Hx, Hy, m, cvec, V, HV, d_done, alpha, c0, beta, U, d_coef); \
     } while (0)
 #define DENSE(P, NC, CH, KT) do { if (R == 3) DENSE_R(P, NC, CH, KT, 3); else DENSE_R(P, NC, CH, KT, 2); } while (0)
     if (cheb) { if (k == 1) DENSE(false, false, true, 1); else DENSE(false, false, true, 2); }
@@ -315,4 +316,24 @@ int shell_dense_hvp(moto_ctx* c, const double* m, const double* cvec, const doub
 #undef DENSE
 #undef DENSE_R
     return 1;
+}
+
+bool shell_dense_applicable(const moto_ctx* c, int k) { return c->nsh > 0 && c->sh_nseg > 0 && k >= 1 && k <= 2 && c->lat.Lx >= 32; }
+
+// OUT = Y_d of the three-term recurrence Y_i = alpha_i (Hess[Y_{i-1}] - c0 Y_{i-1}) + beta_i Y_{i-2}, Y_0 = V (tangent), with the
+// coefficients d_coef [d][4] on the device: d launches of k_shell_dense, Y_i alternating between T1 and T2 (a step writes over
+// its own three-term operand, which it touches at the thread's own site only).  -1: not applicable.
+int shell_cheb_recurrence(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
+                          const double* d_coef, const int* d_done) {
+    if (!shell_dense_applicable(c, k) || !cvec || !c->T1 || !c->T2) return -1;
+    int n = 0;
+    const double* in = V; const double* prev = nullptr;
+    for (int i = 1; i <= d; ++i) {
+        double* out = (i == d) ? OUT : ((i & 1) ? c->T1 : c->T2);
+        const int n1 = shell_dense_hvp(c, m, cvec, in, k, out, 0, d_done, 1, 0.0, 0.0, 0.0, prev, d_coef + 4 * (i - 1));
+        if (n1 <= 0) return -1;
+        n += n1;
+        prev = in; in = out;
+    }
+    return n;
 }

@@ -189,3 +189,33 @@ def test_dense_kernel_parity_api_and_three_term(moto, Lx, Ly, pbc, rcut):
     # reruns are bit-identical (fixed summation order)
     a = ctx.hvp(x, dev(V)).cpu().numpy()
     assert np.array_equal(a, HV)
+
+
+def test_cheb_apply_and_transformed_solve_on_shells(moto):
+    # the Chebyshev transformation on the shell path: d launches of k_shell_dense with device-side coefficients
+    w = shell_workload(36, 30, (1, 0), 4.5, seed=77)
+    mdl = model_of(w)
+    ctx = moto.shell_context(w, kmax=2)
+    x = dev(w.spins)
+    lam_ref, V_ref = sh.lowest_modes(mdl, w.spins, 2, extra=1)
+    a, b, aL = lam_ref[1] + 0.05, 60.0, lam_ref[0]
+    for k, d in ((1, 1), (2, 2), (2, 7), (1, 12)):
+        V = wl.random_block(w.N, k, seed=30 + d)
+        Vt = V - np.sum(V * w.spins[None], axis=2, keepdims=True) * w.spins[None]
+        out = ctx.cheb_apply(x, dev(Vt), d, a, b, aL).cpu().numpy()
+        ref = sh.transformed_operator_apply(mdl, w.spins, Vt, d, a, b, aL)
+        assert rel_l2(out, ref) <= 1e-10, (k, d)
+    # the solver on -p_16(A) (default on shells where the dense kernel applies) against the dense oracle, and against the plain solve
+    res = {}
+    for name, deg in (("auto", 0), ("plain", -1), ("d8", 8)):
+        ctx.set_solver(precond_degree=deg)
+        lam, Vm, info = ctx.lowest_modes(x, 2, tol=1e-9, max_iter=20000)
+        assert info["converged"], name
+        res[name] = info
+        lam, Vm = lam.cpu().numpy(), Vm.cpu().numpy()
+        assert np.max(np.abs(lam - lam_ref[:2]) / np.maximum(np.abs(lam_ref[:2]), 1e-3)) <= 1e-8, name
+        r = sh.hvp(mdl, w.spins, Vm) - lam[:, None, None] * Vm
+        assert np.max(np.linalg.norm(r.reshape(2, -1), axis=1)) <= 1.01e-9, name
+        if lam_ref[2] - lam_ref[1] > 1e-3:
+            assert np.max(scipy.linalg.subspace_angles(Vm.reshape(2, -1).T, V_ref[:2].reshape(2, -1).T)) <= 1e-6, name
+    assert res["auto"]["iters"] < res["plain"]["iters"] and res["auto"]["hvp_count"] > 2 * (res["auto"]["iters"] + 2)
