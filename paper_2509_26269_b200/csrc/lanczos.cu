@@ -217,8 +217,9 @@ moto_status lanczos_solve(moto_ctx* c, const double* d_state, int k, double tol,
     // Ritz values for the first interval; then phases of LZ_PHASE restart cycles on -p_d(A), each phase opened by the true
     // A-Rayleigh quotients and A-residuals of the current Ritz vectors (the only convergence test) and a new interval from them.
     int degree = c->opts.precond_degree;
-    const bool can_filter = c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && k <= 2;
-    if (degree == 0) degree = can_filter ? 40 : 0;
+    const bool shells = shell_dense_applicable(c, k <= 2 ? k : 1);   // general shells: the recurrence as d launches of k_shell_dense
+    const bool can_filter = c->kind == MOTO_KIND_TRI2D && (spin_tma_applicable(c) || shells) && c->T1 && k <= 2;
+    if (degree == 0) degree = can_filter ? (shells ? 16 : 40) : 0;
     if (degree < 0 || !can_filter) degree = 0;
     if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
     // the recurrence uses T1..T4 as scratch, so the basis then lives in the six solver blocks only
@@ -288,7 +289,8 @@ moto_status lanczos_solve(moto_ctx* c, const double* d_state, int k, double tol,
         k0 = k;
         if (degree > 0) {
             // after every restart: T1 = A X of the k Ritz vectors, A-Rayleigh quotients and A-residuals -- the convergence test
-            n += spin_hvp_tma_ex(c, d_state, c->c, c->X, k, c->T1, &c->st->done, nullptr, 0, 0.0, 0.0, 0.0, nullptr, nullptr);
+            if (shells) n += spin_hvp(c, d_state, c->c, c->X, k, c->T1, /*project_input=*/0, &c->st->done);
+            else n += spin_hvp_tma_ex(c, d_state, c->c, c->X, k, c->T1, &c->st->done, nullptr, 0, 0.0, 0.0, 0.0, nullptr, nullptr);
             n += fast_acheck(c, k, k, tol, c->T1, pmax + 1024, /*store=*/1);
             hv += k;
         }

@@ -219,3 +219,13 @@ def test_cheb_apply_and_transformed_solve_on_shells(moto):
         if lam_ref[2] - lam_ref[1] > 1e-3:
             assert np.max(scipy.linalg.subspace_angles(Vm.reshape(2, -1).T, V_ref[:2].reshape(2, -1).T)) <= 1e-6, name
     assert res["auto"]["iters"] < res["plain"]["iters"] and res["auto"]["hvp_count"] > 2 * (res["auto"]["iters"] + 2)
+    # thick-restart Lanczos on the same transformed operator (method = 1; k = 2 and k = 1)
+    for k in (2, 1):
+        ctx.set_solver(method=1, precond_degree=0)
+        lam, Vm, info = ctx.lowest_modes(x, k, tol=1e-9, max_iter=20000)
+        assert info["converged"]
+        lam, Vm = lam.cpu().numpy(), Vm.cpu().numpy()
+        assert np.max(np.abs(lam - lam_ref[:k]) / np.maximum(np.abs(lam_ref[:k]), 1e-3)) <= 1e-8
+        r = sh.hvp(mdl, w.spins, Vm) - lam[:, None, None] * Vm
+        assert np.max(np.linalg.norm(r.reshape(k, -1), axis=1)) <= 1.01e-9
+        assert info["hvp_count"] > 4 * info["iters"]                    # transformed: many HVPs per Lanczos step
