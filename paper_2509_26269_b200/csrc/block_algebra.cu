@@ -247,7 +247,7 @@ __global__ void k_check(const double* __restrict__ partials, int nblk, int kb, i
         double s = 0.0;
         for (int b = lane; b < nblk; b += 32) s += partials[b * MOTO_KMAX + j];
         s = warp_sum(s);
-        if (lane == 0) { r[j] = sqrt(s); st->resid[j] = r[j]; }
+        if (lane == 0) { r[j] = sqrt(s); if (tol >= 0.0) st->resid[j] = r[j]; }   // tol < 0: residuals of the transformed operator, never reported
     }
     __syncthreads();
     if (threadIdx.x == 0) {

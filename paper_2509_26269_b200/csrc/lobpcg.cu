@@ -235,13 +235,21 @@ static moto_status lobpcg_solve_generic_filtered(moto_ctx* c, const double* d_st
 
     int enq = 0, slot = 0, pending = 0, in_phase = 0, cur_degree = 0;
     long long hv = kb;
-    bool finished = false;
+    bool finished = false, polish = false;
     HostStatus last; memset(&last, 0, sizeof(last));
     while (!finished) {
         int batch = max_iter - enq < check_every ? max_iter - enq : check_every;
         for (int b = 0; b < batch; ++b) {
-            if ((cur_degree == 0 && enq + b >= plain_start) || (cur_degree > 0 && in_phase >= phase_len)) {
+            if (!polish && ((cur_degree == 0 && enq + b >= plain_start) || (cur_degree > 0 && in_phase >= phase_len))) {
                 if (cur_degree > 0) { n += gen_phase_start(c, d_state, kb, k, tol, 0, nblk); hv += kb; }   // A-Ritz pairs, A-residual test
+                // Close to the tolerance the restart at every boundary can cost what a phase gains (low degrees: cfg 2 at k = 6,
+                // d = 16 hovered at 1e-8 .. 1e-7 for 20 000 iterations): once the A-residuals of a boundary (the host sees them a
+                // batch late) are within 100 tol, stay on A and finish with plain iterations, which test every iteration.
+                if (cur_degree > 0) {
+                    double amax = 0.0;
+                    for (int a = 0; a < k; ++a) amax = last.resid[a] > amax ? last.resid[a] : amax;
+                    if (amax > 0.0 && amax <= 100.0 * tol) { polish = true; cur_degree = 0; in_phase = 0; continue; }
+                }
                 n += fast_cheb_coef(c, k, degree, margin, c->lmax_L, c->opts.precond_hi, pmax, nmax);
                 n += gen_phase_start(c, d_state, kb, k, tol, degree, nblk);
                 hv += (long long)kb * degree;
