@@ -119,11 +119,11 @@ const char* moto_last_error(const moto_ctx* ctx);
  * All three arrays are HOST pointers, copied (n <= 512).  The table must hold distinct non-zero offsets and be inversion
  * symmetric, J(-d) = J(d), D(-d) = -D(d) (the same bond seen from its other end, reading A2), else MOTO_EINVAL.  Ordered
  * pairs are counted as printed (reading A1).  n = 0 returns to the nearest-neighbour model.  Kind 0 only.  Every call
- * (energy_grad, hvp, lowest_modes, mmf_step, mmf_run, relax, ...) then runs on the table.  Block HVPs of k <= 2 directions on
+ * (energy_grad, hvp, lowest_modes, mmf_step, mmf_run, relax, ...) then runs on the table.  Energy / gradient and block HVPs of k <= 2 directions on
  * lattices with Lx >= 32 take the register-blocked kernel of spin_shells_dense.cu (table as dense column segments, fields staged
  * in shared memory, at most 1024 dense entries incl. zero-filled holes); there moto_cheb_apply works (d launches) and
  * moto_lowest_modes runs LOBPCG on the Chebyshev transformation -p_16(A) by default (precond_degree 0; -1 = plain).  Everything
- * else (k > 2, Lx < 32, energy / gradient) runs on the warp-per-site kernels of spin_shells.cu, without the transformation.
+ * else (k > 2, Lx < 32) runs on the warp-per-site kernels of spin_shells.cu, without the transformation.
  * The TMA path and the persistent small-lattice kernel are nearest-neighbour only. */
 moto_status moto_set_shells(moto_ctx* ctx, int n, const int32_t* h_offsets, const double* h_J, const double* h_D);
 

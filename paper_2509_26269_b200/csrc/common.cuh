@@ -176,6 +176,7 @@ moto_status shell_dense_build(moto_ctx*, int n, const int32_t* h_off, const doub
 int shell_dense_hvp(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double* HV, int project_input, const int* d_done,
                     int cheb, double alpha, double c0, double beta, const double* U, const double* d_coef);
 bool shell_dense_applicable(const moto_ctx*, int k);
+int shell_dense_energy_grad(moto_ctx*, const double* m, double* d_g, double* d_c, double* e_part, int* grid_out);
 int shell_cheb_recurrence(moto_ctx*, const double* m, const double* cvec, const double* V, int k, int d, double* OUT, const double* d_coef,
                           const int* d_done);
 // cart_morse.cu

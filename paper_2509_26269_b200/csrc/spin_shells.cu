@@ -195,6 +195,11 @@ int shell_grid(const moto_ctx* c) {
 }  // namespace
 
 int shell_energy_grad(moto_ctx* c, const double* m, double* d_E, double* d_g, double* d_c) {
+    int gd = 0;
+    if (shell_dense_energy_grad(c, m, d_g, d_c, c->partials, &gd)) {   // register-blocked kernel, m the only staged field
+        if (d_E) { k_shell_final_sum<<<1, 1024, 0, c->stream>>>(c->partials, gd, d_E); return 2; }
+        return 1;
+    }
     const int grid = shell_grid(c);
     k_shell_energy_grad<<<grid, 256, 0, c->stream>>>(make_lat(c), tab_of(c), m, d_g, d_c, c->partials);
     int n = 1;

@@ -59,11 +59,15 @@ __device__ __forceinline__ int wrap(int j, int L) {   // j mod L for any int
 // open edge, neighbours projected once per site in API mode): every load of the staging loop is independent and in flight
 // at once, and the tap loop that follows has no index arithmetic, no branch and no global load.
 // Warp (g, f) of the S x NF warps accumulates tap group g of field f (the k directions, and m when c is wanted).
-template <bool PROJECT, bool NEEDC, bool CHEB, int KT, int R>
+// GRAD (KT = 0, NEEDC): the only staged field is m; the epilogue writes the tangent-projected gradient to HV (if given), c_i to
+// c_out (if given) and the CTA's energy partial sum_i (m_i.(Lm)_i / 2 - m_i.muB) to e_part[blockIdx.x].
+template <bool PROJECT, bool NEEDC, bool CHEB, int KT, int R, bool GRAD = false>
 __global__ void __launch_bounds__(768) k_shell_dense(Lat l, DenseTab tb, int Hx, int Hy, const double* __restrict__ m,
-                                                                                    const double* __restrict__ cvec, const double* __restrict__ V,
-                                                                                    double* __restrict__ HV, const int* __restrict__ done,
-                                                                                    double alpha, double c0, double beta, const double* U, const double* __restrict__ d_coef) {
+                                                     const double* __restrict__ cvec, const double* __restrict__ V,
+                                                     double* __restrict__ HV, const int* __restrict__ done,
+                                                     double alpha, double c0, double beta, const double* U, const double* __restrict__ d_coef,
+                                                     double* __restrict__ c_out, double* __restrict__ e_part) {
+    static_assert(!GRAD || (KT == 0 && NEEDC && !PROJECT && !CHEB), "GRAD: m only");
     constexpr int NF = KT + (NEEDC ? 1 : 0);     // staged / accumulated fields: the KT directions (+ m)
     constexpr int NV = NF * R * 3;               // sums per lane
     extern __shared__ double smem[];
@@ -101,7 +105,7 @@ __global__ void __launch_bounds__(768) k_shell_dense(Lat l, DenseTab tb, int Hx,
         bool ok = true;
         if (gx < 0 || gx >= Lx) { if (l.px) gx = wrap(gx, Lx); else ok = false; }
         if (gy < 0 || gy >= Ly) { if (l.py) gy = wrap(gy, Ly); else ok = false; }
-        d3 mj = mk3(0.0, 0.0, 0.0), vj[KT];
+        d3 mj = mk3(0.0, 0.0, 0.0), vj[KT > 0 ? KT : 1];
 #pragma unroll
         for (int a = 0; a < KT; ++a) vj[a] = mk3(0.0, 0.0, 0.0);
         if (ok) {
@@ -169,6 +173,27 @@ __global__ void __launch_bounds__(768) k_shell_dense(Lat l, DenseTab tb, int Hx,
         spart[e] = s;                            // entry e of group 0 is read by this thread only
     }
     __syncthreads();
+    if (GRAD) {   // energy / gradient epilogue: warp o finishes output row o, the CTA's energy partial in warp order
+        double e = 0.0;
+        const int yg = laneB ? ygA + 1 : ygA, x = laneB ? lane - nA : xA + lane, y = R * yg + warp;
+        if (warp < R && active && y < Ly) {
+            const d3 B = mk3(l.mu * l.Bx, l.mu * l.By, l.mu * l.Bz);
+            const long long i = (long long)y * Lx + x;
+            const d3 mi = ld3(m, i);
+            const double* sm = spart + (warp * 3) * 32 + lane;
+            const d3 Lm = mk3(-2.0 * sm[0], -2.0 * sm[32], -2.0 * sm[64] - 2.0 * l.K * mi.z);
+            const d3 g = sub3(Lm, B);
+            const double c = dot3(mi, g);
+            e = 0.5 * dot3(mi, Lm) - dot3(mi, B);
+            if (HV) st3(HV, i, axpy3(-c, mi, g));
+            if (c_out) c_out[i] = c;
+        }
+        double* sred = spart + NV * 32;          // beyond the summed entries (the region holds S NV 32 >= NV 32 + R doubles)
+        if (warp < R) { e = warp_sum(e); if (lane == 0) sred[warp] = e; }
+        __syncthreads();
+        if (threadIdx.x == 0 && e_part) { double t = 0.0; for (int o = 0; o < R; ++o) t += sred[o]; e_part[blockIdx.x] = t; }
+        return;
+    }
     // epilogue: warp o finishes output row o of the 32 columns
     if (warp >= R || !active) return;
     const int yg = laneB ? ygA + 1 : ygA, x = laneB ? lane - nA : xA + lane, y = R * yg + warp;
@@ -305,7 +330,7 @@ int shell_dense_hvp(moto_ctx* c, const double* m, const double* cvec, const doub
     do {                                                                                                                   \
         static std::atomic<unsigned long long> seen{0};                                                                    \
         if (smem > 48 * 1024 && !tma::ensure_smem_attr(k_shell_dense<P, NC, CH, KT, RR>, 200 * 1024, seen)) return 0;      \
-        k_shell_dense<P, NC, CH, KT, RR><<<grid, 32 * S * nf, smem, c->stream>>>(l, tb, Hx, Hy, m, cvec, V, HV, d_done, alpha, c0, beta, U, d_coef); \
+        k_shell_dense<P, NC, CH, KT, RR><<<grid, 32 * S * nf, smem, c->stream>>>(l, tb, Hx, Hy, m, cvec, V, HV, d_done, alpha, c0, beta, U, d_coef, nullptr, nullptr); \
     } while (0)
 #define DENSE(P, NC, CH, KT) do { if (R == 3) DENSE_R(P, NC, CH, KT, 3); else DENSE_R(P, NC, CH, KT, 2); } while (0)
     if (cheb) { if (k == 1) DENSE(false, false, true, 1); else DENSE(false, false, true, 2); }
@@ -336,4 +361,33 @@ int shell_cheb_recurrence(moto_ctx* c, const double* m, const double* cvec, cons
         prev = in; in = out;
     }
     return n;
+}
+
+// energy partials (one per CTA, to e_part; *grid_out = their number), tangent-projected gradient (d_g, may be NULL) and c (d_c,
+// may be NULL) in one launch of the dense kernel with m as the only staged field.  0: not applicable, the caller falls back.
+int shell_dense_energy_grad(moto_ctx* c, const double* m, double* d_g, double* d_c, double* e_part, int* grid_out) {
+    if (c->nsh <= 0 || c->sh_nseg <= 0 || c->lat.Lx < 32) return 0;
+    const int Hx = c->sh_Hx, Hy = c->sh_Hy, S = 16, sms = MOTO_NUM_SMS;
+    auto ctas = [&](int R) { return (long long)(((long long)((c->lat.Ly + R - 1) / R) * c->lat.Lx + 31) / 32); };
+    const long long w2 = ((ctas(2) + sms - 1) / sms) * 2, w3 = ((ctas(3) + sms - 1) / sms) * 3;
+    const int R = w3 < w2 ? 3 : 2;
+    const int grid = (int)ctas(R);
+    if (grid > MOTO_RED_BLOCKS * 2 * MOTO_NS * MOTO_NS) return 0;   // e_part is the context's partials array
+    const size_t region = (size_t)(32 + 4 * Hx) * (R + 2 * Hy) * 3, part = (size_t)S * R * 3 * 32 + 8;   // doubles
+    const size_t smem = ((size_t)4 * (c->sh_nd + 2 * c->sh_nseg) + 2 * c->sh_nseg + (MOTO_SH_GROUPS + 2) / 2 + std::max(region, part)) * sizeof(double);
+    if (smem > 200 * 1024) return 0;
+    const Lat l = make_lat(c);
+    const DenseTab tb = dense_of(c, 2);
+    static std::atomic<unsigned long long> seen2{0}, seen3{0};
+    if (R == 3) {
+        if (smem > 48 * 1024 && !tma::ensure_smem_attr(k_shell_dense<false, true, false, 0, 3, true>, 200 * 1024, seen3)) return 0;
+        k_shell_dense<false, true, false, 0, 3, true><<<grid, 32 * S, smem, c->stream>>>(l, tb, Hx, Hy, m, nullptr, nullptr, d_g, nullptr, 0.0, 0.0, 0.0,
+                                                                                         nullptr, nullptr, d_c, e_part);
+    } else {
+        if (smem > 48 * 1024 && !tma::ensure_smem_attr(k_shell_dense<false, true, false, 0, 2, true>, 200 * 1024, seen2)) return 0;
+        k_shell_dense<false, true, false, 0, 2, true><<<grid, 32 * S, smem, c->stream>>>(l, tb, Hx, Hy, m, nullptr, nullptr, d_g, nullptr, 0.0, 0.0, 0.0,
+                                                                                         nullptr, nullptr, d_c, e_part);
+    }
+    *grid_out = grid;
+    return 1;
 }

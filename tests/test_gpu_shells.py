@@ -172,6 +172,13 @@ def test_dense_kernel_parity_api_and_three_term(moto, Lx, Ly, pbc, rcut):
     mdl = model_of(w)
     ctx = moto.shell_context(w, kmax=2)
     x = dev(w.spins)
+    # energy / gradient through the same kernel (m the only staged field); c reaches the three-term calls below
+    E, g = ctx.energy_grad(x)
+    E_ref = sh.energy(mdl, w.spins)
+    assert abs(E.item() - E_ref) <= 1e-12 * max(1.0, abs(E_ref))
+    assert np.max(np.abs(g.cpu().numpy() - sh.projected_gradient(mdl, w.spins))) <= 1e-12
+    E2, _ = ctx.energy_grad(x, want_grad=False)
+    assert E2.item() == E.item()
     for k in (1, 2):
         V = wl.random_block(w.N, k, seed=10 + k)                       # not tangent: the API projects the neighbours
         HV = ctx.hvp(x, dev(V)).cpu().numpy()
