@@ -164,7 +164,7 @@ def reduce_over_ranks(dist, elapsed, units, device):
 def run_report(args):
     """`--report`: the per-config table BASELINE.json north_star asks for (five configs, 1 GPU): HVPs/s, Gsite-updates/s,
     time to the lowest-k modes, MMF loop, peak incremental memory, with the oracle timed beside it (cpu_baseline leg:
-    bounded, as it stands).  Prints markdown; `profiles/r01_five_configs.md` is a committed copy of one run."""
+    bounded, as it stands).  Prints markdown; `profiles/r02_five_configs.md` is a committed copy of one run."""
     import torch
     import paper_2509_26269_b200 as moto
     from paper_2509_26269_b200 import workloads as wl
@@ -302,7 +302,7 @@ def run_report(args):
     print("| cfg | N | k | moto_hvp µs | HVP/s | Gsite-updates/s | HVP GB/s (algorithmic 24N(1+2k)) | lowest-k solve ms | iters | HVPs | max resid | peak incremental MB | MMF loop |")
     print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
     print("\n".join(rows))
-    print("\nHVP-Lanczos variant (`moto_solver_opts.method = 1`: thick-restart, full re-orthogonalisation, plain operator; PAPER.md:84):\n")
+    print("\nHVP-Lanczos variant (`moto_solver_opts.method = 1`: thick-restart, full re-orthogonalisation; on the transformed operator -p_d(A) where the TMA K1 (cfg 3, R) or the dense shell kernel (S) applies and k <= 2, on A elsewhere; PAPER.md:84):\n")
     print("| cfg | N | k | basis m | solve ms | Lanczos steps (= HVPs) | converged | max true resid | max abs(lambda - LOBPCG's) |")
     print("|---|---|---|---|---|---|---|---|---|")
     print("\n".join(lrows))
