@@ -463,9 +463,11 @@ def main():
     tt_ms, tt_launches = time_loop(lambda i: ctx.hvp_three_term(ms_sets[i], V_sets[i], 0.1, 9.0, -0.9, U=U_sets[i], out=HV_sets[i],
                                                                  refresh_c=False))
     # (iii) moto_cheb_apply: the operator application of the transformed solver = the whole degree-d recurrence in ONE
-    #       persistent cooperative launch of the same kernel (step 1 has no three-term operand: 128 B/site, then 176)
+    #       persistent cooperative launch of the same kernel.  The filter runs in product form over its Leja-ordered roots
+    #       (k_cheb_coef): every step reads m, c, Y_{s-1} and writes Y_s -- 24 + 8 + 48 k B/site = 128 at k = 2 (the three-term
+    #       recurrence of round 1 also read Y_{s-2}: 176)
     deg = 40
-    alg_bytes_ms = N * ((24 + 8 + 48 * k) + (deg - 1) * (24 + 8 + 72 * k))
+    alg_bytes_ms = N * deg * (24 + 8 + 48 * k)
     ctx.cheb_apply(ms_sets[0], V_sets[0], deg, -0.15, 18.5, -0.16, out=HV_sets[0], refresh_c=True)
     ms_reps = max(3, args.hvp_reps // 10)
     keep = args.hvp_reps
@@ -578,8 +580,8 @@ def main():
                            "algorithmic_bytes": alg_bytes_api, "achieved_gbs": achieved_api, "frac_of_measured_peak": achieved_api / peak,
                            "frac_of_8TBs_nominal": achieved_api / 8000.0},
             # `frac` is in the survey's unit: 24 (1 + 2k) N algorithmic bytes per block-HVP (read m, V; write HV),
-            # d block-HVPs per launch.  The recurrence really moves more (c and the three-term operand: 128 B/site for the first
-            # step, 176 for the others): that figure rides along as frac_recurrence_bytes.
+            # d block-HVPs per launch.  A step of the product-form recurrence also reads c (8 B/site): 128 B/site at k = 2; that
+            # figure rides along as frac_recurrence_bytes.
             "roofline": {"bound": "hbm",
                          "kernel": f"k_hvp_tma<2,0> persistent multi-step launch (moto_cheb_apply, degree {deg}): the operator application "
                                    "of the transformed solver, ~80 % of the step's GPU time",

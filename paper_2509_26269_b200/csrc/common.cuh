@@ -27,6 +27,8 @@ struct SolverState {
     double scal[8];                  // scratch scalars: F.v dots, signs ...
     double cheb[MOTO_CHEB_MAX][4];   // per-step {alpha, c0, beta, -} of the Chebyshev recurrence (k_cheb_coef)
     double cheb_ab[4];               // a, b, a_L, scale of the current transformation
+    int leja_d, leja_pad;            // degree whose Leja root order is in leja[] (0: none)
+    unsigned char leja[MOTO_CHEB_MAX];   // Leja order of the Chebyshev roots (product form of the filter, k_cheb_coef)
     // ---- thick-restart Lanczos (lanczos.cu)
     double lz_T[MOTO_LZ_MAX * MOTO_LZ_MAX];   // projected matrix V^T A V: tridiagonal, bordered-diagonal after a restart
     double lz_Y[MOTO_LZ_MAX * MOTO_KMAX];     // [m][k] Ritz coefficients of the restart

@@ -111,10 +111,59 @@ __global__ void k_negc_max(long long N, const double* __restrict__ c, double* __
     }
 }
 
+// The filter p_d(x) = T_d(l(x)) / T_d(l(a_L)), l(x) = (2x - a - b)/(b - a), is applied in PRODUCT form over its roots
+//   p_d(A) = prod_s (A - r_s) / (a_L - r_s),   r_s = c0 + e cos((2 j_s - 1) pi / (2 d)),  c0 = (a + b)/2, e = (b - a)/2
+// (same polynomial: same roots, same value 1 at a_L), i.e. as d TWO-term steps  Y_s = alpha_s (A - r_s) Y_{s-1}  with
+// alpha_s = 1 / (a_L - r_s): a step reads m, c, Y_{s-1} and writes Y_s -- 128 B/site at k = 2 -- where the three-term Chebyshev
+// recurrence also reads Y_{s-2} (176 B/site).  The product form is only stable if the roots are taken in a LEJA order (each
+// next root maximises the product of its distances to the ones already used): prefix and suffix products then stay within
+// ~3e2 of the end result, and the rounding error equals the three-term recurrence's (3e-14 relative at d = 40 and 128 on a
+// spectrum [-0.16, 18]; the natural orders lose every digit from d = 40 on).  The order depends on d only and is kept in the
+// solver state.  The coefficient rows stay {alpha, shift, beta = 0, -}: every kernel that runs the recurrence reads them
+// as a three-term step and skips the Y_{s-2} operand when beta == 0.
+//
 // explicit == 1: interval given (a = margin, b = hi_user, a_L = lnorm): the moto_cheb_apply building block
 __global__ void k_cheb_coef(SolverState* st, int k, int d, double margin, double lnorm, double hi_user,
                             const double* __restrict__ partial_max, int nmax, int explicit_ab) {
-    if (st->done || threadIdx.x != 0) return;
+    if (st->done) return;
+    const int lane = threadIdx.x;   // one warp
+    __shared__ unsigned char order[MOTO_CHEB_MAX];
+    if (st->leja_d != d) {
+        // Leja order of the d normalised roots x_j = cos((2j - 1) pi / (2d)): lane l owns candidates l, l + 32, ...; products of
+        // distances as sums of logs (fp32 is enough to rank them; ties go to the lower index, so the order is deterministic)
+        float lp[MOTO_CHEB_MAX / 32];
+        bool used[MOTO_CHEB_MAX / 32];
+#pragma unroll
+        for (int q = 0; q < MOTO_CHEB_MAX / 32; ++q) { lp[q] = 0.0f; used[q] = false; }
+        int pick = 0;                                  // x_1: the root nearest b
+        for (int s = 0; s < d; ++s) {
+            if (lane == 0) order[s] = (unsigned char)pick;
+            const double xp = cospi((2.0 * pick + 1.0) / (2.0 * d));
+            float best = -3.0e38f; int bj = 1 << 20;
+#pragma unroll
+            for (int q = 0; q < MOTO_CHEB_MAX / 32; ++q) {
+                const int j = lane + 32 * q;
+                if (j == pick) used[q] = true;
+                if (j < d && !used[q]) {
+                    lp[q] += __logf((float)fabs(cospi((2.0 * j + 1.0) / (2.0 * d)) - xp));
+                    if (lp[q] > best) { best = lp[q]; bj = j; }
+                }
+            }
+            for (int o = 16; o > 0; o >>= 1) {
+                const float ob = __shfl_xor_sync(0xffffffffu, best, o);
+                const int oj = __shfl_xor_sync(0xffffffffu, bj, o);
+                if (ob > best || (ob == best && oj < bj)) { best = ob; bj = oj; }
+            }
+            pick = bj;
+        }
+        __syncwarp();
+        for (int s = lane; s < d; s += 32) st->leja[s] = order[s];
+        __syncwarp();
+        if (lane == 0) st->leja_d = d;
+    } else {
+        for (int s = lane; s < d; s += 32) order[s] = st->leja[s];
+    }
+    __syncwarp();
     double b = hi_user;
     if (!explicit_ab && !(b > 0.0)) {
         double mx = -1e300;
@@ -124,18 +173,13 @@ __global__ void k_cheb_coef(SolverState* st, int k, int d, double margin, double
     const double aL = explicit_ab ? lnorm : st->theta[0];
     double a = explicit_ab ? margin : st->theta[k - 1] + margin;
     if (!explicit_ab && a > 0.5 * (aL + b)) a = 0.5 * (aL + b);   // crude early Ritz values: keep the interval sane
-    const double e = 0.5 * (b - a), c0 = 0.5 * (b + a), sig1 = e / (aL - c0);
-    double sig = sig1;
-    st->cheb_ab[0] = a; st->cheb_ab[1] = b; st->cheb_ab[2] = aL; st->cheb_ab[3] = (double)d;
-    for (int i = 1; i <= d; ++i) {
-        double alpha, beta;
-        if (i == 1) { alpha = sig1 / e; beta = 0.0; }
-        else {
-            const double sn = 1.0 / (2.0 / sig1 - sig);
-            alpha = 2.0 * sn / e; beta = -sig * sn; sig = sn;
-        }
-        if (i == d) { alpha = -alpha; beta = -beta; }   // the transformed operator is -p(A)
-        st->cheb[i - 1][0] = alpha; st->cheb[i - 1][1] = c0; st->cheb[i - 1][2] = beta; st->cheb[i - 1][3] = 0.0;
+    const double e = 0.5 * (b - a), c0 = 0.5 * (b + a);
+    if (lane == 0) { st->cheb_ab[0] = a; st->cheb_ab[1] = b; st->cheb_ab[2] = aL; st->cheb_ab[3] = (double)d; }
+    for (int s = lane; s < d; s += 32) {
+        const double r = c0 + e * cospi((2.0 * order[s] + 1.0) / (2.0 * d));
+        double alpha = 1.0 / (aL - r);
+        if (s == d - 1) alpha = -alpha;                            // the transformed operator is -p(A)
+        st->cheb[s][0] = alpha; st->cheb[s][1] = r; st->cheb[s][2] = 0.0; st->cheb[s][3] = 0.0;
     }
 }
 

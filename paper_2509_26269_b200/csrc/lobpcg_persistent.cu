@@ -14,8 +14,8 @@
 //   R is done redundantly by every CTA of the problem from the same partials in the same order (no broadcast step), by one
 //   warp: Cholesky whitening of the unit-diagonal Gram matrix (rank-revealing Jacobi when a pivot is small) and a
 //   round-robin parallel Jacobi on the reduced 3kb x 3kb pencil; nothing leaves the GPU until the kernel ends.
-// op is the Hessian or, from N >= 1024 sites on, the Chebyshev transformation -p_d(A) of lobpcg.cu (d = 16 three-term steps
-// per application, each one pass over the CTA's chunks + the problem barrier): the Rayleigh-Ritz (~35 us, the dominant cost
+// op is the Hessian or, from N >= 1024 sites on, the Chebyshev transformation -p_d(A) of lobpcg.cu (d = 16 steps of its product
+// form per application, each one pass over the CTA's chunks + the problem barrier): the Rayleigh-Ritz (~35 us, the dominant cost
 // of a plain iteration here) is then paid once per 16 Hessian applications, and the clustered spectra that stall the plain
 // operator (cfg 3 at 100 x 100: 2155 plain iterations) converge in ~50.  8 plain iterations (cold start) fix the interval,
 // phases of 20 transformed iterations follow, each closed by a restart on A that yields the A-Ritz pairs and true
@@ -294,6 +294,7 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
     __shared__ int s_stop;
     __shared__ double scoef[3 * PDEG];
     __shared__ double s_hi;
+    __shared__ int sord[PDEG];
     __shared__ double sack[3 * KB];
     const int prob = blockIdx.x / q.cpp, jc = blockIdx.x - prob * q.cpp;
     const PProb& pr = batch.p[prob];
@@ -362,6 +363,22 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
             for (int ch = 0; ch < q.nchunk; ++ch) mx = fmax(mx, __ldcg(partMv + ch));
             s_hi = q.hi_user > 0.0 ? q.hi_user : mx + q.lnorm;
         }
+        if (tid == 32) {   // Leja order of the normalised Chebyshev roots cos((2j + 1) pi / (2d)) (depends on d only), as k_cheb_coef
+            float lp[PDEG]; bool used[PDEG];
+            for (int j = 0; j < PDEG; ++j) { lp[j] = 0.0f; used[j] = false; }
+            int pick = 0;
+            for (int sI = 0; sI < q.degree; ++sI) {
+                sord[sI] = pick; used[pick] = true;
+                const double xp = cospi((2.0 * pick + 1.0) / (2.0 * q.degree));
+                float best = -3.0e38f; int bj = 0;
+                for (int j = 0; j < q.degree; ++j) {
+                    if (used[j]) continue;
+                    lp[j] += __logf((float)fabs(cospi((2.0 * j + 1.0) / (2.0 * q.degree)) - xp));
+                    if (lp[j] > best) { best = lp[j]; bj = j; }
+                }
+                pick = bj;
+            }
+        }
         __syncthreads();
     }
 
@@ -408,16 +425,15 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
         }
         prob_barrier(bar, q.cpp, round, &st->bad);
     };
-    // DST = op(SRC): the Hessian (deg == 0) or -p_deg(Hess) by the three-term recurrence, Y_i alternating between T1 and T2
+    // DST = op(SRC): the Hessian (deg == 0) or -p_deg(Hess) as deg product-form steps, Y_i alternating between T1 and T2
     auto apply_op = [&](const double* SRC, double* DST, bool dots) {
         if (deg == 0) { op_step(SRC, nullptr, DST, true, 1.0, 0.0, 0.0, dots ? SRC : nullptr); nhvp += KB; return; }
         double* buf[2] = {pr.T1, pr.T2};
         const double* ym1 = SRC;       // Y_{i-1}
-        const double* ym2 = nullptr;   // Y_{i-2}
         for (int i = 1; i <= deg; ++i) {
             double* dst = (i == deg) ? DST : buf[i & 1];
-            op_step(ym1, ym2, dst, false, scoef[3 * i - 3], scoef[3 * i - 2], scoef[3 * i - 1], (dots && i == deg) ? SRC : nullptr);
-            ym2 = ym1; ym1 = dst;
+            op_step(ym1, nullptr, dst, false, scoef[3 * i - 3], scoef[3 * i - 2], 0.0, (dots && i == deg) ? SRC : nullptr);
+            ym1 = dst;
         }
         nhvp += (long long)KB * deg;
     };
@@ -484,19 +500,16 @@ __global__ void __launch_bounds__(PT, 1) k_lobpcg_persistent(const __grid_consta
         if (q.degree > 0 && !fresh) {
             if (deg == 0 && (probing || iter >= q.plain_start)) {
                 // interval [a, b] from the A-Ritz values of the last Rayleigh-Ritz (sC), coefficients as k_cheb_coef
-                if (tid == 0) {
+                if (tid < q.degree) {
+                    // product form over the Leja-ordered roots (see k_cheb_coef): step s is alpha_s (A - r_s), alpha_s = 1 / (a_L - r_s)
                     const double bb = s_hi, aL = sC[3 * KB * KB];
                     double aa = sC[3 * KB * KB + q.k - 1] + q.margin;
                     if (aa > 0.5 * (aL + bb)) aa = 0.5 * (aL + bb);
-                    const double e = 0.5 * (bb - aa), c0 = 0.5 * (bb + aa), sig1 = e / (aL - c0);
-                    double sig = sig1;
-                    for (int i = 1; i <= q.degree; ++i) {
-                        double alpha, beta;
-                        if (i == 1) { alpha = sig1 / e; beta = 0.0; }
-                        else { const double sn = 1.0 / (2.0 / sig1 - sig); alpha = 2.0 * sn / e; beta = -sig * sn; sig = sn; }
-                        if (i == q.degree) { alpha = -alpha; beta = -beta; }   // the transformed operator is -p(A)
-                        scoef[3 * i - 3] = alpha; scoef[3 * i - 2] = c0; scoef[3 * i - 1] = beta;
-                    }
+                    const double e = 0.5 * (bb - aa), c0 = 0.5 * (bb + aa);
+                    const double r = c0 + e * cospi((2.0 * sord[tid] + 1.0) / (2.0 * q.degree));
+                    double alpha = 1.0 / (aL - r);
+                    if (tid == q.degree - 1) alpha = -alpha;                   // the transformed operator is -p(A)
+                    scoef[3 * tid] = alpha; scoef[3 * tid + 1] = r; scoef[3 * tid + 2] = 0.0;
                 }
                 __syncthreads();
                 deg = q.degree; in_phase = 0; nupd = 0; probing = false; fresh = true;

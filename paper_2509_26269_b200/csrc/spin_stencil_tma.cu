@@ -252,7 +252,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
         Ustep = step == 1 ? nullptr : (step == 2 ? p.V0 : ((step & 1) ? p.T1 : p.T2));     // Y_{step-2}
         outp = step == nsteps ? p.out : ((step & 1) ? p.T1 : p.T2);                          // Y_step (in place over Y_{step-2})
     }
-    const bool use_u = !API && p.cheb && Ustep;
+    const bool use_u = !API && p.cheb && Ustep && ch_beta != 0.0;   // product-form steps (beta = 0) never read Y_{step-2}
     // Even steps of a multi-step launch sweep bottom-up: the rows a CTA wrote (and read) last in step i are the first it
     // touches in step i + 1, so a good part of the 176 MB/step footprint is still in the 126 MB L2.  A reversed sweep is
     // the same code on the point-reflected lattice: row order reversed, left and right neighbours swapped, D -> -D
@@ -368,7 +368,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                     if (!API && p.cheb) {
                         oA = scale3(ch_alpha, axpy3(-ch_c0, vA[a], oA));
                         oB = scale3(ch_alpha, axpy3(-ch_c0, vB[a], oB));
-                        if (Ustep) {
+                        if (use_u) {
                             oA = axpy3(ch_beta, uA[a], oA);
                             oB = axpy3(ch_beta, uB[a], oB);
                         }
