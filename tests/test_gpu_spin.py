@@ -454,10 +454,12 @@ CHEB_CASES = [lambda: wl.config0(), lambda: custom(24, 16, 1, 0, 21), lambda: cu
 
 
 @pytest.mark.parametrize("case", range(len(CHEB_CASES)))
-@pytest.mark.parametrize("d", [1, 2, 3, 8, 40])
+@pytest.mark.parametrize("d", [1, 2, 3, 8, 40, 128, 256])
 def test_cheb_apply_parity(moto, case, d):
     # the transformed operator -p_d(Hess) of the solver (one persistent multi-step launch for d >= 2) against its
-    # definition through the oracle's dense eigen-decomposition (lattices small enough for a full dense eigh)
+    # definition through the oracle's dense eigen-decomposition (lattices small enough for a full dense eigh).  The library
+    # applies the filter in product form over its Leja-ordered roots: d = 40 .. 256 (the largest degree allowed) are the cases
+    # where any other root order loses every digit
     w = CHEB_CASES[case]()
     model = model_of(w)
     ctx = moto.spin_context(w, kmax=2)
