@@ -463,11 +463,12 @@ def main():
     tt_ms, tt_launches = time_loop(lambda i: ctx.hvp_three_term(ms_sets[i], V_sets[i], 0.1, 9.0, -0.9, U=U_sets[i], out=HV_sets[i],
                                                                  refresh_c=False))
     # (iii) moto_cheb_apply: the operator application of the transformed solver = the whole degree-d recurrence in ONE
-    #       persistent cooperative launch of the same kernel.  The filter runs in product form over its Leja-ordered roots
-    #       (k_cheb_coef): every step reads m, c, Y_{s-1} and writes Y_s -- 24 + 8 + 48 k B/site = 128 at k = 2 (the three-term
-    #       recurrence of round 1 also read Y_{s-2}: 176)
+    #       persistent cooperative launch.  The filter runs in product form over its Leja-ordered roots (k_cheb_coef) and, by
+    #       default, TWO steps per pass (k_cheb2_tma, spin_cheb2_tma.cu): a pass reads m, c, Y_{s-1}, keeps Y_s in shared memory and
+    #       writes Y_{s+1} -- 24 + 8 + 96 k B/site per two steps = 64 B/site/step at k = 2 (one step per pass: 128; the three-term
+    #       recurrence of round 1: 176).  These are the bytes the launch really has to move; `frac` stays in the survey's unit.
     deg = 40
-    alg_bytes_ms = N * deg * (24 + 8 + 48 * k)
+    alg_bytes_ms = N * (deg // 2) * (24 + 8 + 96 * k)
     ctx.cheb_apply(ms_sets[0], V_sets[0], deg, -0.15, 18.5, -0.16, out=HV_sets[0], refresh_c=True)
     ms_reps = max(3, args.hvp_reps // 10)
     keep = args.hvp_reps
@@ -481,10 +482,11 @@ def main():
     achieved_api = alg_bytes_api / (hvp_ms * 1e-3) / 1e9
     # DRAM traffic of the roofline kernel: bench.py cannot run ncu, so the number comes from the committed `ncu --set full`
     # capture of THIS kernel -- and only if the capture was taken from the kernel source that is being timed now (the CSV
-    # records the sha256 of spin_stencil_tma.cu); a stale capture gives traffic = null instead of a wrong number.
+    # records the sha256 of spin_cheb2_tma.cu, the file of the kernel the default recurrence runs); a stale capture gives
+    # traffic = null instead of a wrong number.
     traffic, traffic_source = None, None
     tp = os.path.join(ROOT, "profiles", "r02_k1_traffic.csv")
-    src = os.path.join(ROOT, "paper_2509_26269_b200", "csrc", "spin_stencil_tma.cu")
+    src = os.path.join(ROOT, "paper_2509_26269_b200", "csrc", "spin_cheb2_tma.cu")
     if os.path.exists(tp) and os.path.exists(src) and args.workload == "cfg3":
         import hashlib
         sha = hashlib.sha256(open(src, "rb").read()).hexdigest()[:16]
@@ -492,7 +494,7 @@ def main():
         hdr, rows = rows[0], rows[1:]
         for f in rows:
             r_ = dict(zip(hdr, f))
-            if r_.get("launch") == "multi-step d=40" and r_.get("kernel_src_sha16") == sha:
+            if r_.get("launch") == "two-step d=40" and r_.get("kernel_src_sha16") == sha:
                 traffic = float(r_["dram_bytes_read"]) + float(r_["dram_bytes_write"])
                 traffic_source = f"profiles/r02_k1_traffic.csv (ncu --set full capture, kernel source sha16 {sha} = the source timed here)"
         if traffic is None:
@@ -580,11 +582,11 @@ def main():
                            "algorithmic_bytes": alg_bytes_api, "achieved_gbs": achieved_api, "frac_of_measured_peak": achieved_api / peak,
                            "frac_of_8TBs_nominal": achieved_api / 8000.0},
             # `frac` is in the survey's unit: 24 (1 + 2k) N algorithmic bytes per block-HVP (read m, V; write HV),
-            # d block-HVPs per launch.  A step of the product-form recurrence also reads c (8 B/site): 128 B/site at k = 2; that
-            # figure rides along as frac_recurrence_bytes.
+            # d block-HVPs per launch.  The two-steps-per-pass launch really moves 64 B/site/step at k = 2 (see above): that figure
+            # rides along as recurrence_bytes / frac_recurrence_bytes -- the kernel is bound by its ten consumer warps, not by DRAM.
             "roofline": {"bound": "hbm",
-                         "kernel": f"k_hvp_tma<2,0> persistent multi-step launch (moto_cheb_apply, degree {deg}): the operator application "
-                                   "of the transformed solver, ~80 % of the step's GPU time",
+                         "kernel": f"k_cheb2_tma<2,1> persistent launch, two product-form steps per pass (moto_cheb_apply, degree {deg}): the "
+                                   "operator application of the transformed solver, ~75 % of the step's GPU time",
                          "achieved": deg * alg_bytes_api / (ms_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                          "frac": deg * alg_bytes_api / (ms_ms * 1e-3) / 1e9 / peak,
                          "frac_of_8TBs_nominal": deg * alg_bytes_api / (ms_ms * 1e-3) / 1e9 / 8000.0,

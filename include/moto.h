@@ -82,10 +82,11 @@ typedef struct {
                                (single start vector, guard / precond_* ignored)          [0]  */
     int32_t ncv;            /* Lanczos basis size m, k + 2 <= m <= min(24, S kmax - 1, dof - 1) with S = 8 blocks
                                (spin lattices) or 6 (Cartesian) of the workspace; 0 = the largest that fits   [0]  */
-    int32_t cheb_mode;      /* how the degree-d recurrence of -p_d(A) is launched on the TMA K1 path: 0 = auto (= 1, the fastest
-                               as measured at 10^6 spins), 1 = one step per pass in one persistent cooperative launch,
-                               2 = d dependent launches, 3 = two steps per pass in one cooperative launch with the intermediate
-                               step kept in shared memory (spin_cheb2_tma.cu).  All give the same results to rounding.  [0]  */
+    int32_t cheb_mode;      /* how the degree-d recurrence of -p_d(A) (product form: d steps alpha_s (A - r_s), k_cheb_coef) is launched
+                               on the TMA K1 path: 0 = auto (= 3, the fastest as measured at 10^6 spins), 1 = one step per pass in one
+                               persistent cooperative launch, 2 = d dependent launches, 3 = two steps per pass in one cooperative
+                               launch with the intermediate step kept in shared memory (spin_cheb2_tma.cu; odd d: + one single
+                               step).  All give bit-identical results.                                                  [0]  */
     int32_t persistent;     /* the whole solve as ONE persistent cooperative kernel (nearest-neighbour spin lattices up to 37 888
                                sites = 148 SMs x 256, k <= 2, no guard columns, method 0): 0 = where it applies, unless an explicit
                                precond_degree > 0 asks for the multi-launch transformed solver; 1 = also with an explicit

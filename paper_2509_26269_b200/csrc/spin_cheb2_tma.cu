@@ -79,7 +79,8 @@ __device__ __forceinline__ d3 ldcg3(const double* p, long long i) { return mk3(_
 // where stencil operand "box site index i" of a row lives: the main row box, or a wrap side box on the edge strips
 struct Role { int off, pitch, fstr; };   // doubles: offset of field 0 / slot 0, row-slot pitch, field stride
 
-template <int K>
+// PF: every step of the launch is a product-form step (beta = 0): the third-operand path is compiled out.
+template <int K, bool PF>
 __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant__ Maps2 maps, const KParams2 p) {
     using C = Cfg2<K>;
     constexpr int F = C::F, S = C::S, NSLOT = C::NSLOT;
@@ -221,7 +222,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
         const double* cfB = cfA + 4;
         const double alA = cfA[0], c0A = cfA[1], beA = cfA[2];
         const double alB = cfB[0], c0B = cfB[1], beB = cfB[2];
-        const double* UA = pass == 1 ? nullptr : p.B[(2 * pass - 4) & 3];        // Y_{2 pass - 3}
+        // product-form steps (beta = 0, k_cheb_coef) have no third operand: phase A then reads nothing from global memory, and
+        // Y_{2 pass - 1} -- wanted by the next pass only as ITS third operand -- never leaves shared memory: a pass moves
+        // m, c, Y_{2 pass - 2} in and Y_{2 pass} out, 128 B/site per TWO steps at k = 2
+        const double* UA = (PF || pass == 1 || beA == 0.0) ? nullptr : p.B[(2 * pass - 4) & 3];        // Y_{2 pass - 3}
+        const bool storeA = !PF && pass < p.npass && p.coef[4 * (2 * pass) + 2] != 0.0;
         double* outA = p.Bw[(2 * pass - 2) & 3];                                  // Y_{2 pass - 1}
         double* outB = pass == p.npass ? p.out : p.Bw[(2 * pass - 1) & 3];        // Y_{2 pass}
         // Even passes sweep bottom-up on the point-reflected lattice: row order reversed, left and right neighbours swapped,
@@ -304,7 +309,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
                 return lds3(scr + 3 * lane);
             };
             mbar_wait(&full[n % S], (n / S) & 1u);
-            load_u(0);
+            if (!PF && UA) load_u(0);
             for (int j = 0; j < nb; ++j) {
                 if (j + 1 < Q) mbar_wait(&full[(n + j + 1) % S], ((n + j + 1) / S) & 1u);
                 const int cur = (int)((n + j) % S), nxt = (cur + 1 == S) ? 0 : cur + 1;
@@ -345,7 +350,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
                     }
                 }
                 // The three-term operand is added last, through a round trip of the partial result in this thread's own Z slots.
-                if (UA && rA <= nrows) {   // warp-uniform: take_u synchronises the warp
+                if (!PF && UA && rA <= nrows) {   // warp-uniform: take_u synchronises the warp
                     const bool haveB = rA + 1 <= nrows;
                     bool yinA, yinB;
                     row_y(rA, yinA); row_y(rA + 1, yinB);
@@ -360,7 +365,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
                         if (inB) sts3(zpB, axpy3(beA, ub, lds3(zpB)));
                     }
                 }
-                if (actA && rA <= nrows) {   // own sites of Y_{2 pass - 1} to HBM
+                if (storeA && actA && rA <= nrows) {   // own sites of Y_{2 pass - 1} to HBM
                     bool yinA, yinB;
                     const int yA = row_y(rA, yinA), yB = row_y(rA + 1, yinB);
                     const int zA = (rA + 1) % ZS, zB = (rA + 2) % ZS;
@@ -371,7 +376,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
                         if (ownB) st3(outA + (size_t)a * 3 * N, (long long)yB * Lx + xg, lds3(sZ + ((size_t)a * ZS + zB) * ROWD + 3 * col));
                     }
                 }
-                if (j + 1 < nb) load_u(j + 1);
+                if (!PF && UA && j + 1 < nb) load_u(j + 1);
                 asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");      // Z rows of this block complete
                 // ---------------------------------------------------------------- phase B: rows rB, rB + 1 of Y_{2 pass}
                 const int rB = j * RC - 2 + 2 * rp;
@@ -402,8 +407,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
                         const double* yp = mC + (size_t)(a + 1) * NSLOT * ROWD;                 // Y_{2 pass - 2} at the centres
                         d3 oA = scale3(alB, axpy3(-c0B, u1C, axpy3(-cA, u1C, proj3(mA, LA))));
                         d3 oB = scale3(alB, axpy3(-c0B, u2C, axpy3(-cB, u2C, proj3(mB, LB))));
-                        oA = axpy3(beB, lds3(yp + sA * ROWD), oA);
-                        oB = axpy3(beB, lds3(yp + sB * ROWD), oB);
+                        if (!PF && beB != 0.0) {
+                            oA = axpy3(beB, lds3(yp + sA * ROWD), oA);
+                            oB = axpy3(beB, lds3(yp + sB * ROWD), oB);
+                        }
                         if (haveA) st3(outB + (size_t)a * 3 * N, (long long)yA * Lx + xg, oA);
                         if (haveB) st3(outB + (size_t)a * 3 * N, (long long)yB * Lx + xg, oB);
                     }
@@ -433,11 +440,11 @@ bool encode_fset(FSet* v, const double* base, int Lx, int Ly, int nvec, int ncom
            encode(&v->schunk, base, Lx, Ly, nvec, SIDED, RC, ncomp) && encode(&v->srow, base, Lx, Ly, nvec, SIDED, 1, ncomp);
 }
 
-template <int K>
+template <int K, bool PF>
 bool launch2(moto_ctx* c, const Maps2& maps, const KParams2& p, int grid) {
     using C = Cfg2<K>;
     static std::atomic<unsigned long long> attr_seen{0};
-    if (!ensure_smem_attr(k_cheb2_tma<K>, C::SMEM, attr_seen)) return false;
+    if (!ensure_smem_attr(k_cheb2_tma<K, PF>, C::SMEM, attr_seen)) return false;
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3(grid); cfg.blockDim = dim3(NTHREADS); cfg.dynamicSmemBytes = C::SMEM; cfg.stream = c->stream;
@@ -445,7 +452,7 @@ bool launch2(moto_ctx* c, const Maps2& maps, const KParams2& p, int grid) {
     attr[0].id = cudaLaunchAttributeCooperative;   // CTAs wait on each other's flags: they must all be resident
     attr[0].val.cooperative = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (cudaLaunchKernelEx(&cfg, k_cheb2_tma<K>, maps, p) == cudaSuccess) return true;
+    if (cudaLaunchKernelEx(&cfg, k_cheb2_tma<K, PF>, maps, p) == cudaSuccess) return true;
     (void)cudaGetLastError();   // the caller falls back to the one-step-per-pass path
     return false;
 }
@@ -457,8 +464,8 @@ int coop_limit2() {
     static std::atomic<unsigned long long> attr_seen{0};
     if (cudaGetDevice(&dev) != cudaSuccess) return -1;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1;
-    if (!ensure_smem_attr(k_cheb2_tma<K>, C::SMEM, attr_seen)) return -1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cheb2_tma<K>, NTHREADS, C::SMEM) != cudaSuccess) return -1;
+    if (!ensure_smem_attr(k_cheb2_tma<K, false>, C::SMEM, attr_seen)) return -1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cheb2_tma<K, false>, NTHREADS, C::SMEM) != cudaSuccess) return -1;
     return sms * per_sm;
 }
 
@@ -467,8 +474,9 @@ int coop_limit2() {
 // Two recurrence steps per pass: OUT = Y_d, d even, Y_0 = V, coefficients at d_coef + 4 (i - 1) (device memory); Y_1 .. Y_{d-1}
 // rotate through the context's four blocks T1 .. T4.  k <= 2.  Returns the number of launches, 0 if not applicable (the
 // caller then takes spin_cheb_multistep / the step-wise path).
+// product_form: every coefficient row has beta = 0 (k_cheb_coef): the kernel without the third-operand path.
 int spin_cheb2_multistep(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
-                         const double* d_coef, const int* d_done) {
+                         const double* d_coef, const int* d_done, int product_form) {
     if (!spin_tma_applicable(c) || k > 2 || d < 2 || (d & 1) || !c->T1 || !c->T3 || !cvec) return 0;
     if (((uintptr_t)m & 15) || ((uintptr_t)V & 15) || ((uintptr_t)cvec & 15)) return 0;
     const int Lx = c->lat.Lx, Ly = c->lat.Ly;
@@ -492,7 +500,8 @@ int spin_cheb2_multistep(moto_ctx* c, const double* m, const double* cvec, const
     for (int i = 0; i < 4; ++i) { p.B[i] = T[i]; p.Bw[i] = T[i]; }
     p.out = OUT; p.done = d_done;
     p.flags = c->flags; c->epoch += 1024; p.epoch = c->epoch; p.err = &c->st->bad;
-    const bool l_ok = k == 2 ? launch2<2>(c, maps, p, grid) : launch2<1>(c, maps, p, grid);
+    const bool l_ok = product_form ? (k == 2 ? launch2<2, true>(c, maps, p, grid) : launch2<1, true>(c, maps, p, grid))
+                                   : (k == 2 ? launch2<2, false>(c, maps, p, grid) : launch2<1, false>(c, maps, p, grid));
     return l_ok ? 1 : 0;
 }
 
@@ -503,12 +512,12 @@ int spin_cheb2_multistep(moto_ctx* c, const double* m, const double* cvec, const
 int spin_cheb_recurrence(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
                          const double* d_coef, const int* d_done) {
     if (c->nsh > 0) return shell_cheb_recurrence(c, m, cvec, V, k, d, OUT, d_coef, d_done);   // general shells: one launch per step
-    const int mode = c->opts.cheb_mode;
+    const int mode = c->opts.cheb_mode == 0 ? 3 : c->opts.cheb_mode;   // auto: two steps per pass (22.2 vs 24.1 us/step at 10^6 spins)
     double* T[4] = {c->T1, c->T2, c->T3, c->T4};
     if (mode == 3 && d >= 2) {
         const int de = d & ~1;
         // odd d: Y_{d-1} goes to the block it would occupy in the rotation, the last step is a single launch
-        int n = spin_cheb2_multistep(c, m, cvec, V, k, de, de == d ? OUT : T[(de - 1) & 3], d_coef, d_done);
+        int n = spin_cheb2_multistep(c, m, cvec, V, k, de, de == d ? OUT : T[(de - 1) & 3], d_coef, d_done, /*product_form=*/1);
         if (n > 0) {
             if (de == d) return n;
             const int n1 = spin_hvp_tma_ex(c, m, cvec, T[(de - 1) & 3], k, OUT, d_done, nullptr, 1, 0.0, 0.0, 0.0, T[(de - 2) & 3],
