@@ -465,10 +465,10 @@ def main():
     # (iii) moto_cheb_apply: the operator application of the transformed solver = the whole degree-d recurrence in ONE
     #       persistent cooperative launch.  The filter runs in product form over its Leja-ordered roots (k_cheb_coef) and, by
     #       default, TWO steps per pass (k_cheb2_tma, spin_cheb2_tma.cu): a pass reads m, c, Y_{s-1}, keeps Y_s in shared memory and
-    #       writes Y_{s+1} -- 24 + 8 + 96 k B/site per two steps = 64 B/site/step at k = 2 (one step per pass: 128; the three-term
+    #       writes Y_{s+1} -- 24 + 8 + 24 k + 24 k B/site per two steps = 64 B/site/step at k = 2 (one step per pass: 128; the three-term
     #       recurrence of round 1: 176).  These are the bytes the launch really has to move; `frac` stays in the survey's unit.
     deg = 40
-    alg_bytes_ms = N * (deg // 2) * (24 + 8 + 96 * k)
+    alg_bytes_ms = N * (deg // 2) * (24 + 8 + 48 * k)
     ctx.cheb_apply(ms_sets[0], V_sets[0], deg, -0.15, 18.5, -0.16, out=HV_sets[0], refresh_c=True)
     ms_reps = max(3, args.hvp_reps // 10)
     keep = args.hvp_reps

@@ -48,9 +48,10 @@ static moto_status finish(moto_ctx* c, int k, int kb, int enq, const HostStatus&
 // Fused path for kb <= 2 (lobpcg_fast.cu): per iteration  op(W) -> k_rr (check + Rayleigh-Ritz) -> k_update_fused.
 //
 // op is either the Hessian itself (one K1 launch with the W^T AW partials fused in) or, on spin lattices with the
-// TMA K1 path, the Chebyshev spectral transformation -p_d(A): d fused three-term K1 launches whose coefficients
-// live on the device (k_cheb_coef), so each outer iteration moves 176 B/site per Hessian application instead of
-// the ~700 B/site of a full LOBPCG iteration.  The transformation is fixed for a phase of `phase_len` iterations;
+// TMA K1 path (or, on general shells, the dense shell kernel), the Chebyshev spectral transformation -p_d(A): d steps of
+// its product form alpha_s (A - r_s) over the Leja-ordered roots, coefficients on the device (k_cheb_coef), two steps
+// per pass of one persistent launch -- 64 B/site per Hessian application at k = 2 instead of the ~700 B/site of a full
+// LOBPCG iteration.  The transformation is fixed for a phase of `phase_len` iterations;
 // between phases the true A-Ritz values and A-residuals are recomputed (that is also the only convergence test
 // while transformed), the interval [a, b] is re-centred on them and LOBPCG restarts from the current X.
 // The host never waits per iteration: it enqueues whole phases and looks at a pinned status copy one batch behind.

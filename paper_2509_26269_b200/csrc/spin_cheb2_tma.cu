@@ -1,18 +1,23 @@
-// spin_cheb2_tma.cu -- K1 with temporal blocking: TWO steps of the Chebyshev three-term recurrence per pass over the
-// lattice (the operator application of the transformed solver, lobpcg.cu; Eq. 4, Hv PAPER.md:156, :162).
+// spin_cheb2_tma.cu -- K1 with temporal blocking: TWO steps of the filter recurrence per pass over the lattice (the operator
+// application of the transformed solver, lobpcg.cu; Eq. 4, Hv PAPER.md:156, :162).  The default launch of the
+// recurrence (moto_solver_opts.cheb_mode 0 = 3).
 //
-//   Y_i = alpha_i (Hess[Y_{i-1}] - c0 Y_{i-1}) + beta_i Y_{i-2},   Hess[v]_i = P_i (L v)_i - c_i v_i   (solver mode, v tangent)
+//   Y_i = alpha_i (Hess[Y_{i-1}] - r_i Y_{i-1}) [+ beta_i Y_{i-2}],   Hess[v]_i = P_i (L v)_i - c_i v_i   (solver mode, v tangent)
 //
-// spin_stencil_tma.cu runs one step per pass: 176 B/site/step (m, c, Y_{i-1}, Y_{i-2} in, Y_i out) and one neighbour
-// synchronisation per step, which the round-2 probes showed to cost ~9 of ~31 us per step at 10^6 spins.  Here a pass
-// stages m, c and Y_{i-1} with a TWO-site halo (the 64-site TMA row box of a <= 60-site strip already holds it), computes
-//   phase A   Z = Y_i      on the strip plus a one-site halo ring   (written to the Z ring in shared memory, own sites to HBM)
-//   phase B   Y_{i+1}      on the strip from Z (shared memory), three-term operand Y_{i-1} = the staged centre value
-// so that m, c and Y_{i-1} cross the memory system once per two steps: (24 + 8 + 48 + 48) in + (48 + 48) out = 224 B per
-// site per TWO steps at k = 2 (112 B/site/step), and the CTAs synchronise with their halo partners once per pass.  The halo
-// ring is computed redundantly by both neighbours with the same arithmetic on the same inputs (bit-identical values), so
-// the result equals the step-by-step recurrence bit for bit.  Four rotating workspace blocks hold Y_{i-2} .. Y_{i+1}: nothing
-// is updated in place, because a CTA now reads Y_{i-2} at halo sites that belong to its neighbours.
+// The library applies the filter in product form over its Leja-ordered roots (k_cheb_coef, lobpcg_fast.cu): beta_i = 0, so a
+// step needs Y_{i-1} only.  spin_stencil_tma.cu runs one such step per pass: 128 B/site/step at k = 2 (m, c, Y_{i-1} in, Y_i out)
+// and one neighbour synchronisation per step.  Here a pass stages m, c and Y_{i-1} with a TWO-site halo (the 64-site TMA row
+// box of a <= 60-site strip already holds it), computes
+//   phase A   Z = Y_i      on the strip plus a one-site halo ring   (written to the Z ring in shared memory only)
+//   phase B   Y_{i+1}      on the strip from Z (shared memory)
+// so that m, c and Y_{i-1} cross the memory system once per two steps and Y_i never leaves the SM: (24 + 8 + 48 k) in + 48 k out
+// = 128 B/site per TWO steps at k = 2, and the CTAs synchronise with their halo partners once per pass.  The halo ring is
+// computed redundantly by both neighbours with the same arithmetic on the same inputs (bit-identical values), so the result
+// equals the step-by-step recurrence bit for bit.  The template flag PF = false keeps the general three-term step (beta != 0:
+// Y_{i-2} read from global memory as flat row segments and transposed through shared memory, Y_i also written out because the
+// next pass needs it as its third operand, four rotating blocks: 224 B/site per two steps) -- the launch the library used
+// before the product form; nothing in the library requests it any more.
+// Measured at 10^6 spins, k = 2 (B200): 22.2 us/step (one step per pass: 24.1); bound by the ten consumer warps, not by DRAM.
 //
 // Same skeleton as spin_stencil_tma.cu: persistent grid (one CTA per SM), column strips, one producer warp issuing
 // cp.async.bulk.tensor boxes into a ring of row slots guarded by full/empty mbarriers, ten consumer warps (2 column

@@ -16,8 +16,11 @@
 // Modes:  API    (moto_hvp)      HV = P (L Pv) - c Pv with c = m.(Lm - mu B) recomputed, input projected
 //         SOLVER (LOBPCG inner)  HV = P (L v) - c v, c given, v tangent; optional per-CTA partials of V^T HV and
 //                                optional three-term epilogue out = alpha (HV - c0 v) + beta u
-//         MULTI-STEP (solver)    the whole Chebyshev recurrence in one cooperative launch: per-step neighbour flags,
-//                                ping-pong blocks, alternating sweep direction (see KParams and DESIGN.md 5)
+//         MULTI-STEP (solver)    the whole filter recurrence in one cooperative launch, one step per pass: per-step
+//                                neighbour flags, ping-pong blocks, alternating sweep direction (see KParams and DESIGN.md 5).
+//                                The library's coefficient rows are product-form steps (beta = 0, k_cheb_coef): such a step
+//                                skips the third operand (128 B/site at k = 2).  cheb_mode = 1; the default launch of the
+//                                recurrence is the two-steps-per-pass kernel of spin_cheb2_tma.cu.
 #include "common.cuh"
 #include "device_utils.cuh"
 #include "stencil_math.cuh"
@@ -254,7 +257,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     }
     const bool use_u = !API && p.cheb && Ustep && ch_beta != 0.0;   // product-form steps (beta = 0) never read Y_{step-2}
     // Even steps of a multi-step launch sweep bottom-up: the rows a CTA wrote (and read) last in step i are the first it
-    // touches in step i + 1, so a good part of the 176 MB/step footprint is still in the 126 MB L2.  A reversed sweep is
+    // touches in step i + 1, so a good part of the 128 MB/step footprint is still in the 126 MB L2.  A reversed sweep is
     // the same code on the point-reflected lattice: row order reversed, left and right neighbours swapped, D -> -D
     // (the stencil is inversion symmetric up to the sign of the DMI vectors, D_{-delta} = -D_delta).
     const bool rev = nsteps > 1 && !(step & 1);
