@@ -294,10 +294,12 @@ moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, 
     if (3ll * kb > dof) kb = (int)(dof / 3 > 0 ? dof / 3 : 1);
     if (kb < k) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes: k too large for this system (need 3k <= dof)");
     if (kb <= 2 && max_iter > 0) return lobpcg_solve_fast(c, d_state, k, kb, tol, max_iter, warm_start, info);
-    // kb > 2: the transformation is opt-in (precond_degree > 0): at the sizes where such blocks are used here (cfg 2,
-    // 65 536 sites) the recurrence steps are launch-latency bound and plain LOBPCG is as fast
-    if (max_iter > 0 && c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && c->opts.precond_degree > 0) {
-        int degree = c->opts.precond_degree;
+    // kb > 2 where the TMA K1 applies: the generic block algebra on the transformed operator, degree 32 unless precond_degree says
+    // otherwise (-1: plain).  Opt-in in round 1 (with the three-term recurrence plain LOBPCG was as fast at cfg 2); with the
+    // product-form two-step launch it wins everywhere it was tried: cfg 2 k = 6 33 -> 18 ms, k = 3 130 -> 10 ms, cfg 3 at 316^2
+    // k = 4 513 -> 80 ms, cfg 3 k = 4 2185 -> 222 ms, random spins 256^2 k = 6 39 -> 22 ms (degrees 20 .. 40 all within 1.3x of 32)
+    if (max_iter > 0 && c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && c->opts.precond_degree >= 0) {
+        int degree = c->opts.precond_degree > 0 ? c->opts.precond_degree : 32;
         if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
         return lobpcg_solve_generic_filtered(c, d_state, k, kb, tol, max_iter, warm_start, degree, info);
     }
