@@ -25,6 +25,7 @@ struct SolverState {
     double GB[MOTO_NS * MOTO_NS];
     double C[MOTO_NS * MOTO_KMAX];   // [ns][kb] coefficients of the new X in the basis [X,W,P]
     double scal[8];                  // scratch scalars: F.v dots, signs ...
+    double ack[2 * MOTO_KMAX];       // A-residual check (lobpcg_fast.cu): theta_j = x_j.A x_j / x_j.x_j at [j], x_j.x_j at [KMAX + j]
     double cheb[MOTO_CHEB_MAX][4];   // per-step {alpha, c0, beta, -} of the Chebyshev recurrence (k_cheb_coef)
     double cheb_ab[4];               // a, b, a_L, scale of the current transformation
     int leja_d, leja_pad;            // degree whose Leja root order is in leja[] (0: none)

@@ -222,7 +222,7 @@ static moto_status lobpcg_solve_generic_filtered(moto_ctx* c, const double* d_st
     const size_t bs = (size_t)3 * c->N;
     const int check_every = c->opts.check_every > 0 ? c->opts.check_every : 8;
     const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.01;
-    const int phase_len = 20, plain_start = warm_start ? 0 : 20;
+    const int phase_len = 20, plain_start = warm_start ? 0 : 20, acheck_every = 4;
     double* pmax = c->g;   // [<= 296] block maxima of -c_i (the gradient scratch is free during a solve; the Gram partials fill c->partials)
     int n = 0, nmax = 0;
     n += spin_curvature(c, d_state, c->c);
@@ -263,6 +263,14 @@ static moto_status lobpcg_solve_generic_filtered(moto_ctx* c, const double* d_st
             n += block_residual(c, d_state, kb, k, cur_degree ? -1.0 : tol);
             hv += (long long)kb * (cur_degree ? cur_degree : 1);
             ++in_phase;
+            if (cur_degree > 0 && in_phase < phase_len && in_phase % acheck_every == 0) {
+                // cheap convergence test between boundaries, as on the fused path: T1 = A X, |A x_j - (x_j.A x_j) x_j|.  Without
+                // it a block that converges inside a phase is iterated past convergence until the boundary, where the residuals
+                // of the columns that were done first have drifted up again -- the solve then hovers at the tolerance
+                n += apply_operator(c, d_state, c->X, kb, c->T1);
+                n += fast_acheck(c, kb, k, tol, c->T1, c->g + 4096);
+                hv += kb;
+            }
         }
         enq += batch;
         if (n < 0) return moto_fail(c, MOTO_ECUDA, "moto_lowest_modes: a launch of the Chebyshev recurrence failed");
@@ -298,10 +306,25 @@ moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, 
     // otherwise (-1: plain).  Opt-in in round 1 (with the three-term recurrence plain LOBPCG was as fast at cfg 2); with the
     // product-form two-step launch it wins everywhere it was tried: cfg 2 k = 6 33 -> 18 ms, k = 3 130 -> 10 ms, cfg 3 at 316^2
     // k = 4 513 -> 80 ms, cfg 3 k = 4 2185 -> 222 ms, random spins 256^2 k = 6 39 -> 22 ms (degrees 20 .. 40 all within 1.3x of 32)
+    // Safety net of the automatic choice: the transformed solve gets a budget of GEN_BUDGET iterations (it needs 30 .. 150 where
+    // it works); if it has not converged by then, plain LOBPCG on A -- slower, but it has no phase structure to go wrong -- takes
+    // over from the current block.  (Short plain starts on a random-spin state made the transformed solve stall at 1e-4 in the
+    // round-2 sweeps; the shipped phase constants did not, on any workload tried.)  An explicit degree gets the whole max_iter.
+    constexpr int GEN_BUDGET = 300;
+    int it0 = 0;
+    int64_t hv0 = 0;
+    bool carried = false;
+    struct KeepGuard { moto_ctx* c; int v; ~KeepGuard() { c->keep_guard = v; } } restore_keep_guard{c, c->keep_guard};   // (the fallback sets it)
     if (max_iter > 0 && c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && c->opts.precond_degree >= 0) {
         int degree = c->opts.precond_degree > 0 ? c->opts.precond_degree : 32;
         if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
-        return lobpcg_solve_generic_filtered(c, d_state, k, kb, tol, max_iter, warm_start, degree, info);
+        const int budget = (c->opts.precond_degree > 0 || max_iter <= GEN_BUDGET) ? max_iter : GEN_BUDGET;
+        moto_solve_info i1;
+        memset(&i1, 0, sizeof(i1));
+        const moto_status s1 = lobpcg_solve_generic_filtered(c, d_state, k, kb, tol, budget, warm_start, degree, &i1);
+        if (s1 != MOTO_ENOTCONV || budget == max_iter) { if (info) *info = i1; return s1; }
+        it0 = i1.iters; hv0 = i1.hvp_count; carried = true;
+        max_iter -= budget; warm_start = 1; c->keep_guard = 1;   // continue from the whole current block, guard columns included
     }
     const size_t bs = (size_t)3 * c->N;
     const int check_every = c->opts.check_every > 0 ? c->opts.check_every : 8;
@@ -361,10 +384,10 @@ moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, 
 
     int iters = last.iter < enq ? last.iter : enq;
     if (info) {
-        info->iters = iters;
+        info->iters = iters + it0;
         info->converged = (last.done && !last.bad) ? 1 : 0;
         for (int a = 0; a < MOTO_KMAX; ++a) info->resid[a] = a < k ? last.resid[a] : 0.0;
-        info->hvp_count = (int64_t)kb * (1 + iters);
+        info->hvp_count = (int64_t)kb * (1 + iters) + hv0;
     }
     if (last.bad) return moto_fail(c, MOTO_ECUDA, "moto_lowest_modes: numerical breakdown (NaN or rank loss) in Rayleigh-Ritz");
     if (!last.done) return moto_fail(c, MOTO_ENOTCONV, "moto_lowest_modes: max_iter reached; outputs hold the best iterate");

@@ -186,7 +186,7 @@ __global__ void k_cheb_coef(SolverState* st, int k, int d, double margin, double
 // ---------------------------------------------------------------- A-residual check while LOBPCG runs on -p(A)
 // T = A X is given.  Two streaming passes, because the residual must not be formed from the expanded expression
 // tt - 2 theta xt + theta^2 xx: with tt ~ 1e-2 its rounding floor is ~ 1e-8 in |r|, so below tol ~ 1e-8 that test would
-// decide on noise.  Pass 1: partials of x_j.x_j and x_j.t_j  ->  theta_j = xt / xx (k_acheck_theta, into st->scal).
+// decide on noise.  Pass 1: partials of x_j.x_j and x_j.t_j  ->  theta_j = xt / xx (k_acheck_theta, into st->ack).
 // Pass 2: partials of |t_j - theta_j x_j|^2, formed element by element  ->  |A x_j - theta_j x_j| / |x_j|, decision.
 template <int KB>
 __global__ void __launch_bounds__(256) k_acheck_dots(long long n3, const double* __restrict__ X, const double* __restrict__ T,
@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(256) k_acheck_dots(long long n3, const double*
     block_reduce_store<2 * KB>(acc, partials + (size_t)blockIdx.x * 2 * KB);
 }
 
-// theta_j = (x_j.t_j) / (x_j.x_j) into st->scal[j], x_j.x_j into st->scal[KMAX/2 + j]   (kb <= 2 here, scal has 8 slots)
+// theta_j = (x_j.t_j) / (x_j.x_j) into st->ack[j], x_j.x_j into st->ack[KMAX + j]
 __global__ void k_acheck_theta(const double* __restrict__ partials, int nblk, int kb, SolverState* st) {
     if (st->done) return;
     __shared__ double v[2 * MOTO_KMAX];
@@ -217,7 +217,7 @@ __global__ void k_acheck_theta(const double* __restrict__ partials, int nblk, in
         if (lane == 0) v[e] = s;
     }
     __syncthreads();
-    if (threadIdx.x < kb) { st->scal[threadIdx.x] = v[2 * threadIdx.x + 1] / v[2 * threadIdx.x]; st->scal[4 + threadIdx.x] = v[2 * threadIdx.x]; }
+    if (threadIdx.x < kb) { st->ack[threadIdx.x] = v[2 * threadIdx.x + 1] / v[2 * threadIdx.x]; st->ack[MOTO_KMAX + threadIdx.x] = v[2 * threadIdx.x]; }
 }
 
 template <int KB>
@@ -226,7 +226,7 @@ __global__ void __launch_bounds__(256) k_acheck_resid(long long n3, const double
     if (st->done) return;
     double th[KB], acc[KB];
 #pragma unroll
-    for (int j = 0; j < KB; ++j) { th[j] = st->scal[j]; acc[j] = 0.0; }
+    for (int j = 0; j < KB; ++j) { th[j] = st->ack[j]; acc[j] = 0.0; }
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n3; e += (long long)gridDim.x * blockDim.x) {
 #pragma unroll
         for (int j = 0; j < KB; ++j) {
@@ -253,13 +253,13 @@ __global__ void k_acheck_final(const double* __restrict__ partials, int nblk, in
         bool ok = true;
         double rs[MOTO_KMAX];
         for (int j = 0; j < kb; ++j) {
-            const double r2 = v[j] / st->scal[4 + j];
+            const double r2 = v[j] / st->ack[MOTO_KMAX + j];
             rs[j] = sqrt(r2);
             if (j < k) ok = ok && (rs[j] <= tol) && (r2 == r2);
         }
         st->nhvp += kb;
         if (ok || store)
-            for (int j = 0; j < kb; ++j) { st->theta[j] = st->scal[j]; st->resid[j] = rs[j]; }
+            for (int j = 0; j < kb; ++j) { st->theta[j] = st->ack[j]; st->resid[j] = rs[j]; }
         if (ok) st->done = 1;
     }
 }
@@ -328,11 +328,16 @@ int fast_cheb_coef_explicit(moto_ctx* c, int d, double a, double b, double aL) {
 int fast_acheck(moto_ctx* c, int kb, int k, double tol, const double* d_T, double* partials, int store) {
     const long long n3 = 3ll * c->N;
     const int g = fast_grid(n3);
-    if (kb == 1) k_acheck_dots<1><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, partials, &c->st->done);
-    else k_acheck_dots<2><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, partials, &c->st->done);
+#define ACK_DOTS(KB) k_acheck_dots<KB><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, partials, &c->st->done)
+#define ACK_RESID(KB) k_acheck_resid<KB><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, c->st, partials)
+#define ACK_SWITCH(M) switch (kb) { case 1: M(1); break; case 2: M(2); break; case 3: M(3); break; case 4: M(4); break; \
+                                    case 5: M(5); break; case 6: M(6); break; case 7: M(7); break; default: M(8); break; }
+    ACK_SWITCH(ACK_DOTS);
     k_acheck_theta<<<1, 32 * 2 * kb, 0, c->stream>>>(partials, g, kb, c->st);
-    if (kb == 1) k_acheck_resid<1><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, c->st, partials);
-    else k_acheck_resid<2><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, c->st, partials);
+    ACK_SWITCH(ACK_RESID);
+#undef ACK_SWITCH
+#undef ACK_RESID
+#undef ACK_DOTS
     k_acheck_final<<<1, 32 * kb, 0, c->stream>>>(partials, g, kb, k, tol, c->st, store);
     return 4;
 }
