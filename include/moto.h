@@ -72,7 +72,8 @@ typedef struct {
     int32_t check_every;    /* iterations enqueued between host looks at the status     [8]  */
     int32_t precond_degree; /* degree d of the Chebyshev spectral transformation -p_d(A) LOBPCG runs on:
                                0 = auto (40 on spin lattices that take the TMA K1 path and kb <= 2, 32 there for kb > 2, 16 inside the
-                               persistent small-lattice kernel and on general shells with the dense kernel, else off),
+                               persistent small-lattice kernel and on general shells with the dense kernel, 24 for Cartesian atoms
+                               with kb <= 2 and at most 8192 atoms, else off),
                                -1 = off (plain LOBPCG on A, the paper's solver), 1..256 = degree          [0]  */
     int32_t hvp_path;       /* K1 kernel choice: 0 auto, 1 generic (any lattice), 2 TMA-staged (even Lx >= 8) [0] */
     double precond_lo;      /* margin: the damped interval starts at theta_k + margin           [0 -> 0.01] */

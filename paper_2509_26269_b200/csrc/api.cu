@@ -61,7 +61,7 @@ static WsLayout ws_layout(const moto_lattice* lat, int kmax) {
     w.partials = al256((size_t)MOTO_RED_BLOCKS * 2 * MOTO_NS * MOTO_NS * sizeof(double));
     w.st = al256(sizeof(SolverState));
     w.cart = lat->kind == MOTO_KIND_CARTESIAN ? cart_lists_bytes(lat) : 0;
-    w.nblocks = lat->kind == MOTO_KIND_TRI2D ? 10 : 6;   // spin lattices: + four rotating blocks of the Chebyshev recurrence
+    w.nblocks = lat->kind == MOTO_KIND_TRI2D ? 10 : 8;   // + blocks of the filter recurrence: four on spin lattices (T1..T4), two for atoms (T1, T2)
     w.flags = 4096;
     w.shell = lat->kind == MOTO_KIND_TRI2D ? al256((size_t)MOTO_MAX_SHELLS * (2 * sizeof(int) + 4 * sizeof(double))) +
                                                  al256((size_t)MOTO_SH_DENSE * 4 * sizeof(double)) + al256((size_t)MOTO_SH_SEGS * 4 * sizeof(int)) : 0;
@@ -111,10 +111,8 @@ moto_status moto_create(const moto_lattice* lat, const void* params, void* d_wor
     c->X = (double*)p; p += w.block;  c->AX = (double*)p; p += w.block;
     c->W = (double*)p; p += w.block;  c->AW = (double*)p; p += w.block;
     c->P = (double*)p; p += w.block;  c->AP = (double*)p; p += w.block;
-    if (w.nblocks == 10) {
-        c->T1 = (double*)p; p += w.block; c->T2 = (double*)p; p += w.block;
-        c->T3 = (double*)p; p += w.block; c->T4 = (double*)p; p += w.block;
-    }
+    if (w.nblocks >= 8) { c->T1 = (double*)p; p += w.block; c->T2 = (double*)p; p += w.block; }
+    if (w.nblocks == 10) { c->T3 = (double*)p; p += w.block; c->T4 = (double*)p; p += w.block; }
     c->c = (double*)p; p += w.c;
     c->g = (double*)p; p += w.g;
     c->stage_m = (double*)p; p += w.stage;

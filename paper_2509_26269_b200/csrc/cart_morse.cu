@@ -162,7 +162,9 @@ __global__ void __launch_bounds__(256) k_cart_energy_grad(int Na, const uint8_t*
 // warp per atom, all k columns per pass over the stored pairs
 __global__ void __launch_bounds__(256) k_cart_hvp(int Na, int k, const uint8_t* __restrict__ fixed, const int* __restrict__ nb_count,
                                                   const int* __restrict__ nb_idx, const double* __restrict__ nb_coef,
-                                                  const double* __restrict__ V, double* __restrict__ HV, const int* __restrict__ done) {
+                                                  const double* __restrict__ V, double* __restrict__ HV, const int* __restrict__ done,
+                                                  const double* __restrict__ coef) {
+    // coef != NULL: a product-form step of the filter recurrence (k_cheb_coef row {alpha, r, ...}): HV = alpha (H V - r V)
     if (done && *done) return;
     int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (i >= Na) return;
@@ -198,7 +200,11 @@ __global__ void __launch_bounds__(256) k_cart_hvp(int Na, int k, const uint8_t* 
     for (int a = 0; a < MOTO_KMAX; ++a) {
         if (a < k) {
             double x = warp_sum(acc[a][0]), y = warp_sum(acc[a][1]), z = warp_sum(acc[a][2]);
-            if (lane == 0) st3(HV + (size_t)a * 3 * Na, i, mk3(x, y, z));
+            if (lane == 0) {
+                d3 h = mk3(x, y, z);
+                if (coef) h = scale3(coef[0], axpy3(-coef[1], ld3(V + (size_t)a * 3 * Na, i), h));
+                st3(HV + (size_t)a * 3 * Na, i, h);
+            }
         }
     }
 }
@@ -313,7 +319,53 @@ int cart_energy_grad(moto_ctx* c, const double* x, double* d_E, double* d_g) {
 
 int cart_hvp(moto_ctx* c, const double* V, int k, double* HV, const int* d_done) {
     const int Na = c->N;
-    k_cart_hvp<<<(Na * 32 + 255) / 256, 256, 0, c->stream>>>(Na, k, c->lat.d_fixed, c->cl.nb_count, c->cl.nb_idx, c->cl.nb_coef, V, HV, d_done);
+    k_cart_hvp<<<(Na * 32 + 255) / 256, 256, 0, c->stream>>>(Na, k, c->lat.d_fixed, c->cl.nb_count, c->cl.nb_idx, c->cl.nb_coef, V, HV, d_done,
+                                                            nullptr);
+    return 1;
+}
+
+// OUT = Y_d of the product-form filter recurrence Y_s = alpha_s (H - r_s) Y_{s-1}, Y_0 = V (masked), rows d_coef [d][4] on the device
+// (k_cheb_coef): d launches of k_cart_hvp, Y_s alternating between T1 and T2.  The neighbour table must be current.
+int cart_cheb_recurrence(moto_ctx* c, const double* V, int k, int d, double* OUT, const double* d_coef, const int* d_done) {
+    if (!c->T1 || !c->T2) return -1;
+    const int Na = c->N;
+    const double* in = V;
+    for (int i = 1; i <= d; ++i) {
+        double* out = (i == d) ? OUT : ((i & 1) ? c->T1 : c->T2);
+        k_cart_hvp<<<(Na * 32 + 255) / 256, 256, 0, c->stream>>>(Na, k, c->lat.d_fixed, c->cl.nb_count, c->cl.nb_idx, c->cl.nb_coef, in, out, d_done,
+                                                                d_coef + 4 * (i - 1));
+        in = out;
+    }
+    return d;
+}
+
+// upper bound of the spectrum for the filter interval: block Gershgorin, max_i 2 sum_j max(|phi''_ij|, |phi'_ij / r_ij|)
+// (a pair block has eigenvalues phi'' along the bond and phi'/r across it, and sits once on the diagonal and once off it);
+// per-CTA maxima to partial_max, *nmax_out = their number
+__global__ void __launch_bounds__(256) k_cart_rowbound(int Na, const uint8_t* __restrict__ fixed, const int* __restrict__ nb_count,
+                                                       const double* __restrict__ nb_coef, double* __restrict__ partial_max) {
+    __shared__ double red[8];
+    const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double s = 0.0;
+    if (i < Na && !(fixed && fixed[i])) {
+        const double* cf = nb_coef + (size_t)i * NC * MOTO_MAX_NEIGH;
+        for (int n = lane; n < nb_count[i]; n += 32) s += fmax(fabs(cf[3 * MOTO_MAX_NEIGH + n]), fabs(cf[4 * MOTO_MAX_NEIGH + n]));
+    }
+    s = 2.0 * warp_sum(s);
+    if (lane == 0) red[warp] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double mx = 0.0;
+        for (int w = 0; w < 8; ++w) mx = fmax(mx, red[w]);
+        partial_max[blockIdx.x] = mx;
+    }
+}
+
+int cart_rowbound(moto_ctx* c, double* partial_max, int* nmax_out) {
+    const int Na = c->N, g = (Na * 32 + 255) / 256;
+    if (g > 1024) return 0;   // (the caller's array of block maxima)
+    *nmax_out = g;
+    k_cart_rowbound<<<g, 256, 0, c->stream>>>(Na, c->lat.d_fixed, c->cl.nb_count, c->cl.nb_coef, partial_max);
     return 1;
 }
 

@@ -186,6 +186,8 @@ int shell_cheb_recurrence(moto_ctx*, const double* m, const double* cvec, const 
 int cart_build_lists(moto_ctx*, const double* x);
 int cart_energy_grad(moto_ctx*, const double* x, double* d_E, double* d_g);
 int cart_hvp(moto_ctx*, const double* V, int k, double* HV, const int* d_done);
+int cart_cheb_recurrence(moto_ctx*, const double* V, int k, int d, double* OUT, const double* d_coef, const int* d_done);
+int cart_rowbound(moto_ctx*, double* partial_max, int* nmax_out);
 int cart_mmf_step(moto_ctx*, const double* x, const double* v, int kr, double dt, double* x_out, double* d_fnorm);
 int cart_mask(moto_ctx*, double* V, int k);
 size_t cart_lists_bytes(const moto_lattice* lat);

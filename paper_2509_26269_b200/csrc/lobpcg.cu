@@ -9,6 +9,7 @@
 #include <stdlib.h>
 #include "common.cuh"
 
+constexpr int ATOMS_AUTO_DEGREE = 24;   // Cartesian atoms (launch-latency bound at 10^3 atoms)
 constexpr int SHELL_AUTO_DEGREE = 16;   // precond_degree = 0 on general shells (HVP-bound: a lower degree than the stencil's 40)
 
 static int apply_operator(moto_ctx* c, const double* d_state, const double* V, int kb, double* AV) {
@@ -74,7 +75,8 @@ static void fast_apply(FastCtx& f, const double* V, double* OV) {
     }
     // the whole recurrence: two steps per pass in one persistent cooperative launch when it fits (spin_cheb2_tma.cu), else one
     // step per pass, else one launch per step (moto_solver_opts.cheb_mode)
-    const int nk = spin_cheb_recurrence(c, f.state, c->c, V, f.kb, f.degree, OV, &c->st->cheb[0][0], &c->st->done);
+    const int nk = c->kind == MOTO_KIND_TRI2D ? spin_cheb_recurrence(c, f.state, c->c, V, f.kb, f.degree, OV, &c->st->cheb[0][0], &c->st->done)
+                                              : cart_cheb_recurrence(c, V, f.kb, f.degree, OV, &c->st->cheb[0][0], &c->st->done);
     if (nk <= 0) { f.failed = true; return; }
     f.n += nk;
     f.n += fast_dot_waw(c, f.kb, V, OV, f.partialsK, &f.nblkK);
@@ -114,23 +116,29 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     // spectral transformation: precond_degree 0 = auto (40 where the TMA K1 applies), < 0 = off
     int degree = c->opts.precond_degree;
     const bool shells = shell_dense_applicable(c, kb);   // general shells: the recurrence runs on k_shell_dense, one launch per step
-    const bool can_filter = c->kind == MOTO_KIND_TRI2D && (spin_tma_applicable(c) || shells) && c->T1 && 3ll * kb * 8 <= 2ll * c->N;
-    if (degree == 0) degree = can_filter ? (shells ? SHELL_AUTO_DEGREE : 40) : 0;
+    const bool atoms = c->kind == MOTO_KIND_CARTESIAN && c->N <= 8192;   // (block maxima of the Gershgorin bound: <= 1024 CTAs)
+    const bool can_filter = (atoms || (c->kind == MOTO_KIND_TRI2D && (spin_tma_applicable(c) || shells))) && c->T1 && c->T2 &&
+                            3ll * kb * 8 <= 2ll * c->N;
+    if (degree == 0) degree = can_filter ? (shells ? SHELL_AUTO_DEGREE : (atoms ? ATOMS_AUTO_DEGREE : 40)) : 0;
     if (degree < 0 || !can_filter) degree = 0;
     if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
     const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.01;
     // cold start: 20 plain iterations first so that theta_k (hence a) means something; a warm start already has it
     // tuned on cfg 3 (two seeds) and its 316^2 instance; shells (degree 16, 12 plain iterations) on the 366-neighbour table at
     // 36^2, 64^2 and 100^2
-    const int phase_len = 20, plain_start = warm_start ? 0 : (shells ? 12 : 20);
+    const int phase_len = 20, plain_start = warm_start ? 0 : ((shells || atoms) ? 12 : 20);
     const int acheck_every = 4;
-    const double lnorm = c->lmax_L;   // b = max_i(-c_i) + lambda_max(L) >= lambda_max(Hess)
+    // b = max_i(-c_i) + lambda_max(L) >= lambda_max(Hess); atoms: the block Gershgorin bound of the stored pair coefficients
+    const double lnorm = atoms ? 0.0 : c->lmax_L;
 
     if (c->kind == MOTO_KIND_TRI2D) f.n += spin_curvature(c, d_state, c->c);
     else f.n += cart_build_lists(c, d_state);
     MOTO_CUDA_CHECK(c, cudaMemsetAsync(c->st, 0, sizeof(SolverState), c->stream));
     int nmax = 0;
-    if (degree > 0) f.n += fast_negc_max(c, pmax, &nmax);
+    if (degree > 0) {
+        if (atoms) { const int nb = cart_rowbound(c, pmax, &nmax); if (nb > 0) f.n += nb; else degree = 0; }
+        else f.n += fast_negc_max(c, pmax, &nmax);
+    }
     if (!warm_start) f.n += block_random(c, c->X, kb, c->opts.seed);
     else if (kb > k && !c->keep_guard) f.n += block_random(c, c->X + (size_t)k * bs, kb - k, c->opts.seed ^ 0x5bd1e995u);
     f.n += project_block(c, d_state, c->X, kb);
@@ -156,7 +164,7 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
             ++in_phase;
             if (transformed && in_phase < phase_len && in_phase % acheck_every == 0) {
                 // cheap convergence test between restarts: T1 = A X, |A x_j - (x_j.A x_j) x_j| (T1/T2 are free between applies)
-                if (shells) f.n += apply_operator(c, d_state, c->X, kb, c->T1);
+                if (shells || atoms) f.n += apply_operator(c, d_state, c->X, kb, c->T1);
                 else f.n += spin_hvp_tma_ex(c, d_state, c->c, c->X, kb, c->T1, &c->st->done, nullptr, 0, 0.0, 0.0, 0.0, nullptr, nullptr);
                 f.n += fast_acheck(c, kb, k, tol, c->T1, pmax + 1024);
             }

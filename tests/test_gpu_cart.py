@@ -153,3 +153,29 @@ def test_heptamer_certified_edge(moto, slab):
         assert np.all(y[w.fixed == 1] == w.positions[w.fixed == 1])
     assert abs(ends[0][0] - E_min) <= 1e-9 and np.max(np.abs(ends[0][1] - x0.cpu().numpy())) <= 1e-4   # back to the reference minimum
     assert np.max(np.abs(ends[1][1] - x0.cpu().numpy())) > 0.5                                          # a different minimum
+
+
+def test_transformed_solver_on_atoms(moto, slab):
+    # Cartesian atoms take the Chebyshev-transformed LOBPCG by default (degree 24; the upper end of the interval is the block
+    # Gershgorin bound of the stored pair coefficients): same eigenpairs as the plain solver and as the all-pairs oracle, in fewer
+    # Rayleigh-Ritz steps, on the slab (fixed bottom layers) and on a free cluster
+    wc = wl.small_cluster(38, seed=3)
+    for w, mdl in (slab, (wc, model_of(wc))):
+        pos = w.positions
+        lam_ref, V_ref = co.lowest_modes(mdl, pos, 2, extra=1)
+        res = {}
+        for name, deg in (("auto", 0), ("plain", -1), ("d8", 8), ("d40", 40)):
+            ctx = moto.cart_context(w, kmax=2)
+            ctx.set_solver(precond_degree=deg)
+            lam, V, info = ctx.lowest_modes(dev(pos), 2, tol=1e-9, max_iter=20000)
+            assert info["converged"], name
+            res[name] = info
+            lam, V = lam.cpu().numpy(), V.cpu().numpy()
+            assert np.max(np.abs(lam - lam_ref[:2]) / np.maximum(np.abs(lam_ref[:2]), 1e-3)) <= 1e-8, name
+            if lam_ref[2] - lam_ref[1] > 1e-3:
+                assert np.max(scipy.linalg.subspace_angles(V.reshape(2, -1).T, V_ref[:2].reshape(2, -1).T)) <= 1e-6, name
+            r = co.hvp(mdl, pos, V) - lam[:, None, None] * V                    # oracle-side residual
+            assert np.max(np.linalg.norm(r.reshape(2, -1), axis=1)) <= 1.01e-9, name
+            if w.fixed is not None:
+                assert np.all(V[:, w.fixed == 1, :] == 0)                        # masked rows stay zero through the recurrence
+        assert res["auto"]["iters"] < res["plain"]["iters"] and res["auto"]["hvp_count"] > 2 * (res["auto"]["iters"] + 2)
