@@ -119,7 +119,8 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     const bool atoms = c->kind == MOTO_KIND_CARTESIAN && c->N <= 8192;   // (block maxima of the Gershgorin bound: <= 1024 CTAs)
     const bool can_filter = (atoms || (c->kind == MOTO_KIND_TRI2D && (spin_tma_applicable(c) || shells))) && c->T1 && c->T2 &&
                             3ll * kb * 8 <= 2ll * c->N;
-    if (degree == 0) degree = can_filter ? (shells ? SHELL_AUTO_DEGREE : (atoms ? ATOMS_AUTO_DEGREE : 40)) : 0;
+    // (atoms, warm start: the re-solves of the MMF loop are ~35 launch-bound plain iterations = 6 ms per outer step at cfg 4, 9 ms transformed)
+    if (degree == 0) degree = can_filter ? (shells ? SHELL_AUTO_DEGREE : (atoms ? (warm_start ? 0 : ATOMS_AUTO_DEGREE) : 40)) : 0;
     if (degree < 0 || !can_filter) degree = 0;
     if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
     const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.01;
