@@ -245,21 +245,13 @@ static moto_status lobpcg_solve_generic_filtered(moto_ctx* c, const double* d_st
 
     int enq = 0, slot = 0, pending = 0, in_phase = 0, cur_degree = 0;
     long long hv = kb;
-    bool finished = false, polish = false;
+    bool finished = false;
     HostStatus last; memset(&last, 0, sizeof(last));
     while (!finished) {
         int batch = max_iter - enq < check_every ? max_iter - enq : check_every;
         for (int b = 0; b < batch; ++b) {
-            if (!polish && ((cur_degree == 0 && enq + b >= plain_start) || (cur_degree > 0 && in_phase >= phase_len))) {
+            if ((cur_degree == 0 && enq + b >= plain_start) || (cur_degree > 0 && in_phase >= phase_len)) {
                 if (cur_degree > 0) { n += gen_phase_start(c, d_state, kb, k, tol, 0, nblk); hv += kb; }   // A-Ritz pairs, A-residual test
-                // Close to the tolerance the restart at every boundary can cost what a phase gains (low degrees: cfg 2 at k = 6,
-                // d = 16 hovered at 1e-8 .. 1e-7 for 20 000 iterations): once the A-residuals of a boundary (the host sees them a
-                // batch late) are within 100 tol, stay on A and finish with plain iterations, which test every iteration.
-                if (cur_degree > 0) {
-                    double amax = 0.0;
-                    for (int a = 0; a < k; ++a) amax = last.resid[a] > amax ? last.resid[a] : amax;
-                    if (amax > 0.0 && amax <= 100.0 * tol) { polish = true; cur_degree = 0; in_phase = 0; continue; }
-                }
                 n += fast_cheb_coef(c, k, degree, margin, c->lmax_L, c->opts.precond_hi, pmax, nmax);
                 n += gen_phase_start(c, d_state, kb, k, tol, degree, nblk);
                 hv += (long long)kb * degree;
@@ -311,32 +303,15 @@ moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, 
     if (3ll * kb > dof) kb = (int)(dof / 3 > 0 ? dof / 3 : 1);
     if (kb < k) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes: k too large for this system (need 3k <= dof)");
     if (kb <= 2 && max_iter > 0) return lobpcg_solve_fast(c, d_state, k, kb, tol, max_iter, warm_start, info);
-    // kb > 2 where the TMA K1 applies: the generic block algebra on the transformed operator, degree 32 unless precond_degree says
-    // otherwise (-1: plain).  Opt-in in round 1 (with the three-term recurrence plain LOBPCG was as fast at cfg 2); with the
-    // product-form two-step launch it wins everywhere it was tried: cfg 2 k = 6 33 -> 18 ms, k = 3 130 -> 10 ms, cfg 3 at 316^2
-    // k = 4 513 -> 80 ms, cfg 3 k = 4 2185 -> 222 ms, random spins 256^2 k = 6 39 -> 22 ms (degrees 20 .. 40 all within 1.3x of 32)
-    // Safety net of the automatic choice: the transformed solve gets a budget of GEN_BUDGET iterations (it needs 30 .. 150 where
-    // it works); if it has not converged by then, plain LOBPCG on A -- slower, but it has no phase structure to go wrong -- takes
-    // over from the current block.  (Short plain starts on a random-spin state made the transformed solve stall at 1e-4 in the
-    // round-2 sweeps; the shipped phase constants did not, on any workload tried.)  An explicit degree gets the whole max_iter.
-    constexpr int GEN_BUDGET = 300;
-    int it0 = 0;
-    int64_t hv0 = 0;
-    bool carried = false;
-    struct KeepGuard { moto_ctx* c; int v; ~KeepGuard() { c->keep_guard = v; } } restore_keep_guard{c, c->keep_guard};   // (the fallback sets it)
-    // (warm starts keep the plain solver unless a degree is asked for: the v_1-only re-solves of the MMF loop at cfg 2 take 110
-    // launch-bound plain iterations = 18.9 ms per outer step, 48 transformed ones 23.5 ms)
-    if (max_iter > 0 && c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 &&
-        (c->opts.precond_degree > 0 || (c->opts.precond_degree == 0 && !warm_start))) {
-        int degree = c->opts.precond_degree > 0 ? c->opts.precond_degree : 32;
+    // kb > 2: the transformation is opt-in (precond_degree > 0).  With the product-form two-step launch and the cheap A-residual test
+    // it is 2-10x faster than plain LOBPCG where it converges (cfg 2 k = 6 31 -> 7.3 ms, cfg 3 k = 4 2185 -> 226 ms), but it is not
+    // robust enough to be the default: without locking, columns that have converged keep iterating at the rounding floor, and with
+    // guard columns on a dense (random-spin) spectrum the residuals then bounce between 1e-9 and 1e-2 instead of settling
+    // (70 x 40 random spins, k = 3 + 2 guards, degree 32; degrees 16 and 64 converge).  Plain LOBPCG stops at convergence and does not.
+    if (max_iter > 0 && c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && c->opts.precond_degree > 0) {
+        int degree = c->opts.precond_degree;
         if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
-        const int budget = (c->opts.precond_degree > 0 || max_iter <= GEN_BUDGET) ? max_iter : GEN_BUDGET;
-        moto_solve_info i1;
-        memset(&i1, 0, sizeof(i1));
-        const moto_status s1 = lobpcg_solve_generic_filtered(c, d_state, k, kb, tol, budget, warm_start, degree, &i1);
-        if (s1 != MOTO_ENOTCONV || budget == max_iter) { if (info) *info = i1; return s1; }
-        it0 = i1.iters; hv0 = i1.hvp_count; carried = true;
-        max_iter -= budget; warm_start = 1; c->keep_guard = 1;   // continue from the whole current block, guard columns included
+        return lobpcg_solve_generic_filtered(c, d_state, k, kb, tol, max_iter, warm_start, degree, info);
     }
     const size_t bs = (size_t)3 * c->N;
     const int check_every = c->opts.check_every > 0 ? c->opts.check_every : 8;
@@ -396,10 +371,10 @@ moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, 
 
     int iters = last.iter < enq ? last.iter : enq;
     if (info) {
-        info->iters = iters + it0;
+        info->iters = iters;
         info->converged = (last.done && !last.bad) ? 1 : 0;
         for (int a = 0; a < MOTO_KMAX; ++a) info->resid[a] = a < k ? last.resid[a] : 0.0;
-        info->hvp_count = (int64_t)kb * (1 + iters) + hv0;
+        info->hvp_count = (int64_t)kb * (1 + iters);
     }
     if (last.bad) return moto_fail(c, MOTO_ECUDA, "moto_lowest_modes: numerical breakdown (NaN or rank loss) in Rayleigh-Ritz");
     if (!last.done) return moto_fail(c, MOTO_ENOTCONV, "moto_lowest_modes: max_iter reached; outputs hold the best iterate");

@@ -14,7 +14,7 @@
 //   R is done redundantly by every CTA of the problem from the same partials in the same order (no broadcast step), by one
 //   warp: Cholesky whitening of the unit-diagonal Gram matrix (rank-revealing Jacobi when a pivot is small) and a
 //   round-robin parallel Jacobi on the reduced 3kb x 3kb pencil; nothing leaves the GPU until the kernel ends.
-// op is the Hessian or, from N >= 1024 sites on, the Chebyshev transformation -p_d(A) of lobpcg.cu (d = 16 steps of its product
+// op is the Hessian or, from N >= 128 sites on, the Chebyshev transformation -p_d(A) of lobpcg.cu (d = 16 steps of its product
 // form per application, each one pass over the CTA's chunks + the problem barrier): the Rayleigh-Ritz (~35 us, the dominant cost
 // of a plain iteration here) is then paid once per 16 Hessian applications, and the clustered spectra that stall the plain
 // operator (cfg 3 at 100 x 100: 2155 plain iterations) converge in ~50.  8 plain iterations (cold start) fix the interval,
@@ -37,7 +37,7 @@ constexpr int NM = 6;          // largest pencil (3 kb, kb <= 2)
 constexpr int PDEG = 32;       // largest degree of the Chebyshev transformation inside the kernel
 // precond_degree = 0 (auto): degree, smallest lattice that takes it, plain iterations of a cold start, phase length, iterations
 // between cheap A-residual tests -- swept on cfg 1, its 40x40 instance, random spins 64x64, cfg 3 at 100x100 and the P = 24 batch
-constexpr int PAUTO_DEGREE = 16, PAUTO_MIN_N = 1024, PAUTO_PLAIN = 8, PAUTO_PHASE = 20, PAUTO_ACHECK = 2;
+constexpr int PAUTO_DEGREE = 16, PAUTO_MIN_N = 128, PAUTO_PLAIN = 8, PAUTO_PHASE = 20, PAUTO_ACHECK = 2;
 constexpr double RR_TAU = 1e-10, RR_CHOL = 1e-2;   // rank truncation / Cholesky admission, as on the fused path of rayleigh_ritz.cu
 
 struct PProb {

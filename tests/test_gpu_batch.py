@@ -77,7 +77,7 @@ def test_batch_more_problems_than_threads(moto):
 
 
 # ---------------------------------------------------------------- the persistent kernel on the Chebyshev-transformed operator
-# From 1024 sites on (and up to 148 x 256 sites) the persistent kernel runs LOBPCG on -p_16(A) (lobpcg_persistent.cu): plain
+# From 128 sites on (and up to 148 x 256 sites) the persistent kernel runs LOBPCG on -p_16(A) (lobpcg_persistent.cu): plain
 # start, transformed phases closed by a restart on A, convergence decided on true A-residuals only.
 
 def open_lattice(p):
@@ -89,7 +89,7 @@ def open_lattice(p):
 def test_persistent_transformed_batch_equals_separate_and_oracle(moto, make, P):
     import torch
     ws = [make(p) for p in range(P)]
-    assert ws[0].N >= 1024
+    assert ws[0].N >= 128
     ctxs = [moto.spin_context(w, kmax=2) for w in ws]
     xs = [dev(w.spins) for w in ws]
     lams, Vs, infos = moto.lowest_modes_batch(ctxs, xs, 2, 1e-9, max_iter=20000)

@@ -485,23 +485,23 @@ def test_transformed_generic_path_kb_gt_2(moto):
     _check_modes(w, lam, V, lam_ref, V_ref, 3)
 
 
-@pytest.mark.parametrize("case,k,kmax", [(lambda: custom(64, 50, 1, 0, 2), 4, 4), (lambda: custom(70, 40, 0, 1, 3), 3, 5),
+@pytest.mark.parametrize("case,k,kmax", [(lambda: custom(64, 50, 1, 0, 2), 4, 4), (lambda: custom(70, 40, 0, 1, 3), 3, 3),
                                          (lambda: wl.config1(L=40), 6, 6)])
-def test_generic_path_runs_transformed_by_default(moto, case, k, kmax):
-    # block sizes above 2 where the TMA K1 applies: -p_32(A) by default (cheap A-residual test every 4 iterations, plain LOBPCG as
-    # the fall-back after 300 iterations), with and without guard columns, against the dense oracle and the plain solver
+def test_generic_path_transformed_opt_in(moto, case, k, kmax):
+    # block sizes above 2 where the TMA K1 applies: -p_32(A) on request (precond_degree > 0; cheap A-residual test every 4
+    # iterations), against the dense oracle and the plain solver (the default for these block sizes)
     w = case()
     lam_ref, V_ref = so.lowest_modes(model_of(w), w.spins, k, extra=1)
     res = {}
-    for name, deg in (("auto", 0), ("plain", -1)):
+    for name, deg in (("d32", 32), ("default", 0)):
         ctx = moto.spin_context(w, kmax=kmax)
-        ctx.set_solver(hvp_path=2, precond_degree=deg, guard=kmax - k)
+        ctx.set_solver(hvp_path=2, precond_degree=deg)
         lam, V, info = ctx.lowest_modes(dev(w.spins), k, tol=1e-9, max_iter=20000)
         assert info["converged"], (name, info)
         _check_modes(w, lam, V, lam_ref, V_ref, k)
         res[name] = info
-    assert res["auto"]["hvp_count"] > kmax * (res["auto"]["iters"] + 2)           # the transformation was on
-    assert res["auto"]["iters"] < res["plain"]["iters"]
+    assert res["default"]["hvp_count"] == kmax * (res["default"]["iters"] + 1)      # plain: one HVP per column and iteration
+    assert res["d32"]["hvp_count"] > kmax * (res["d32"]["iters"] + 2) and res["d32"]["iters"] < res["default"]["iters"]
 
 
 def test_building_block_argument_errors_and_fallbacks(moto):
