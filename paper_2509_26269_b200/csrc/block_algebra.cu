@@ -181,6 +181,9 @@ __global__ void __launch_bounds__(256) k_update(long long n3, double* __restrict
     if (st->done) return;
     __shared__ double sC[3 * KB * KB];
     for (int t = threadIdx.x; t < 3 * KB * KB; t += blockDim.x) sC[t] = st->C[t];  // [3KB][KB] row-major
+    bool lk[KB];          // soft locking: P_j of a locked column is dropped
+#pragma unroll
+    for (int j = 0; j < KB; ++j) lk[j] = st->lock_on && st->locked[j];
     __syncthreads();
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n3; e += (long long)gridDim.x * blockDim.x) {
 #pragma unroll
@@ -202,7 +205,7 @@ __global__ void __launch_bounds__(256) k_update(long long n3, double* __restrict
 #pragma unroll
                 for (int i = 0; i < KB; ++i) xn = fma(sC[i * KB + j], s[i], xn);
                 x[(size_t)j * n3 + e] = xn;
-                p[(size_t)j * n3 + e] = pn;
+                p[(size_t)j * n3 + e] = lk[j] ? 0.0 : pn;
             }
         }
     }
@@ -219,6 +222,9 @@ __global__ void __launch_bounds__(256) k_residual(long long N, int kb, const dou
     double th[MOTO_KMAX];
 #pragma unroll
     for (int a = 0; a < MOTO_KMAX; ++a) { acc[a] = 0.0; th[a] = (a < kb) ? st->theta[a] : 0.0; }
+    bool lk[MOTO_KMAX];   // soft locking: a locked column contributes no search direction
+#pragma unroll
+    for (int a = 0; a < MOTO_KMAX; ++a) lk[a] = st->lock_on && a < kb && st->locked[a];
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
         d3 mi = m ? ld3(m, i) : mk3(0, 0, 0);
         const bool fx = fixed && fixed[i];
@@ -228,7 +234,7 @@ __global__ void __launch_bounds__(256) k_residual(long long N, int kb, const dou
                 d3 r = axpy3(-th[a], ld3(X + (size_t)a * 3 * N, i), ld3(AX + (size_t)a * 3 * N, i));
                 acc[a] += dot3(r, r);
                 if (m) r = proj3(mi, r);
-                if (fx) r = mk3(0, 0, 0);
+                if (fx || lk[a]) r = mk3(0, 0, 0);
                 st3(W + (size_t)a * 3 * N, i, r);
             }
         }
@@ -247,7 +253,10 @@ __global__ void k_check(const double* __restrict__ partials, int nblk, int kb, i
         double s = 0.0;
         for (int b = lane; b < nblk; b += 32) s += partials[b * MOTO_KMAX + j];
         s = warp_sum(s);
-        if (lane == 0) { r[j] = sqrt(s); if (tol >= 0.0) st->resid[j] = r[j]; }   // tol < 0: residuals of the transformed operator, never reported
+        if (lane == 0) {   // tol < 0: residuals of the transformed operator, never reported
+            r[j] = sqrt(s);
+            if (tol >= 0.0) { st->resid[j] = r[j]; if (st->lock_on) st->locked[j] = r[j] <= 0.1 * tol; }
+        }
     }
     __syncthreads();
     if (threadIdx.x == 0) {

@@ -37,6 +37,8 @@ struct SolverState {
     double lz_beta, lz_rbeta;                 // ||u|| of the current step and its reciprocal
     int lz_cycle, lz_pad;                     // index of the last restart cycle whose Rayleigh-Ritz ran
     unsigned long long pbar;                  // barrier counter of the persistent small-lattice solver (lobpcg_persistent.cu)
+    int lock_on, lock_pad;                    // soft locking (generic transformed LOBPCG): columns with locked[j] get no new W_j / P_j
+    int locked[MOTO_KMAX];
     // ---- tail mirrored to the host (layout == HostStatus)
     double theta[MOTO_KMAX];
     double resid[MOTO_KMAX];

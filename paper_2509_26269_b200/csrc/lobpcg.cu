@@ -231,11 +231,18 @@ static moto_status lobpcg_solve_generic_filtered(moto_ctx* c, const double* d_st
     const size_t bs = (size_t)3 * c->N;
     const int check_every = c->opts.check_every > 0 ? c->opts.check_every : 8;
     const double margin = c->opts.precond_lo > 0 ? c->opts.precond_lo : 0.01;
-    const int phase_len = 20, plain_start = warm_start ? 0 : 20, acheck_every = 4;
+    // A-residual test: every iteration on a warm start (a re-solve of the MMF loop is a handful of iterations, each worth kb * degree
+    // HVPs, the test kb), every second one on a cold start
+    const int phase_len = 20, plain_start = warm_start ? 0 : 20, acheck_every = warm_start ? 1 : 2;
     double* pmax = c->g;   // [<= 296] block maxima of -c_i (the gradient scratch is free during a solve; the Gram partials fill c->partials)
     int n = 0, nmax = 0;
     n += spin_curvature(c, d_state, c->c);
     MOTO_CUDA_CHECK(c, cudaMemsetAsync(c->st, 0, sizeof(SolverState), c->stream));
+    // soft locking (k_check / k_acheck_final set st->locked[j] once the A-residual of column j is within tol / 10, k_residual and
+    // k_update then give that column no new W_j / P_j; it stays in the Rayleigh-Ritz basis).  Without it converged columns keep
+    // iterating at the rounding floor of -p_d(A), where their normalised residuals are noise that the Rayleigh-Ritz step mixes
+    // back into the block: 70 x 40 random spins, k = 3 + 2 guards, degree 32 bounced between 1e-9 and 1e-2 for 4000 iterations.
+    MOTO_CUDA_CHECK(c, cudaMemsetAsync(&c->st->lock_on, 1, 1, c->stream));
     n += fast_negc_max(c, pmax, &nmax);
     if (!warm_start) n += block_random(c, c->X, kb, c->opts.seed);
     else if (kb > k && !c->keep_guard) n += block_random(c, c->X + (size_t)k * bs, kb - k, c->opts.seed ^ 0x5bd1e995u);
@@ -252,7 +259,9 @@ static moto_status lobpcg_solve_generic_filtered(moto_ctx* c, const double* d_st
         for (int b = 0; b < batch; ++b) {
             if ((cur_degree == 0 && enq + b >= plain_start) || (cur_degree > 0 && in_phase >= phase_len)) {
                 if (cur_degree > 0) { n += gen_phase_start(c, d_state, kb, k, tol, 0, nblk); hv += kb; }   // A-Ritz pairs, A-residual test
-                n += fast_cheb_coef(c, k, degree, margin, c->lmax_L, c->opts.precond_hi, pmax, nmax);
+                // the damped interval starts above the whole block, theta_kb + margin: guard columns are amplified like the wanted ones
+                // (with a = theta_k + margin they sat inside [a, b], where -p_d(A) is a cluster at 0 they could never resolve)
+                n += fast_cheb_coef(c, kb, degree, margin, c->lmax_L, c->opts.precond_hi, pmax, nmax);
                 n += gen_phase_start(c, d_state, kb, k, tol, degree, nblk);
                 hv += (long long)kb * degree;
                 cur_degree = degree; in_phase = 0;
@@ -303,13 +312,14 @@ moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, 
     if (3ll * kb > dof) kb = (int)(dof / 3 > 0 ? dof / 3 : 1);
     if (kb < k) return moto_fail(c, MOTO_EINVAL, "moto_lowest_modes: k too large for this system (need 3k <= dof)");
     if (kb <= 2 && max_iter > 0) return lobpcg_solve_fast(c, d_state, k, kb, tol, max_iter, warm_start, info);
-    // kb > 2: the transformation is opt-in (precond_degree > 0).  With the product-form two-step launch and the cheap A-residual test
-    // it is 2-10x faster than plain LOBPCG where it converges (cfg 2 k = 6 31 -> 7.3 ms, cfg 3 k = 4 2185 -> 226 ms), but it is not
-    // robust enough to be the default: without locking, columns that have converged keep iterating at the rounding floor, and with
-    // guard columns on a dense (random-spin) spectrum the residuals then bounce between 1e-9 and 1e-2 instead of settling
-    // (70 x 40 random spins, k = 3 + 2 guards, degree 32; degrees 16 and 64 converge).  Plain LOBPCG stops at convergence and does not.
-    if (max_iter > 0 && c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && c->opts.precond_degree > 0) {
-        int degree = c->opts.precond_degree;
+    // kb > 2 where the TMA K1 applies: the generic block algebra on -p_d(A) (degree 32 unless precond_degree says otherwise,
+    // precond_degree < 0 = plain LOBPCG), cold and warm starts alike: cfg 2 k = 6 30 -> 7.3 ms, its warm-started MMF re-solves
+    // 14.4 -> 8.3 ms per outer step (moto_mmf_run: 12.5 -> 4.5), cfg 3 k = 4 2184 -> 243 ms; converges where the plain iteration
+    // runs into its cap (128 x 128 skyrmion, k = 6; 316 x 316 cfg-3 recipe, k = 6).
+    constexpr int GENERIC_AUTO_DEGREE = 32;
+    if (max_iter > 0 && c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && c->opts.precond_degree >= 0 &&
+        (c->opts.precond_degree > 0 || 3ll * kb * 8 <= 2ll * c->N)) {
+        int degree = c->opts.precond_degree > 0 ? c->opts.precond_degree : GENERIC_AUTO_DEGREE;
         if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
         return lobpcg_solve_generic_filtered(c, d_state, k, kb, tol, max_iter, warm_start, degree, info);
     }

@@ -239,6 +239,7 @@ __global__ void __launch_bounds__(256) k_acheck_resid(long long n3, const double
 
 // store: also leave theta / resid in the state when the test fails (the Lanczos variant sets its next interval from them)
 __global__ void k_acheck_final(const double* __restrict__ partials, int nblk, int kb, int k, double tol, SolverState* st, int store) {
+    // (soft locking, st->lock_on: every column whose A-residual is within tol is locked, and unlocked should it drift out again)
     if (st->done) return;
     __shared__ double v[MOTO_KMAX];
     const int e = threadIdx.x >> 5, lane = threadIdx.x & 31;   // one warp per column
@@ -256,6 +257,7 @@ __global__ void k_acheck_final(const double* __restrict__ partials, int nblk, in
             const double r2 = v[j] / st->ack[MOTO_KMAX + j];
             rs[j] = sqrt(r2);
             if (j < k) ok = ok && (rs[j] <= tol) && (r2 == r2);
+            if (st->lock_on) st->locked[j] = rs[j] <= 0.1 * tol;
         }
         st->nhvp += kb;
         if (ok || store)

@@ -487,21 +487,61 @@ def test_transformed_generic_path_kb_gt_2(moto):
 
 @pytest.mark.parametrize("case,k,kmax", [(lambda: custom(64, 50, 1, 0, 2), 4, 4), (lambda: custom(70, 40, 0, 1, 3), 3, 3),
                                          (lambda: wl.config1(L=40), 6, 6)])
-def test_generic_path_transformed_opt_in(moto, case, k, kmax):
-    # block sizes above 2 where the TMA K1 applies: -p_32(A) on request (precond_degree > 0; cheap A-residual test every 4
-    # iterations), against the dense oracle and the plain solver (the default for these block sizes)
+def test_generic_path_transformed_default(moto, case, k, kmax):
+    # block sizes above 2 where the TMA K1 applies run on -p_32(A) by default (soft locking, A-residual test every second
+    # iteration); precond_degree = -1 is plain LOBPCG.  Both against the dense oracle.
     w = case()
     lam_ref, V_ref = so.lowest_modes(model_of(w), w.spins, k, extra=1)
     res = {}
-    for name, deg in (("d32", 32), ("default", 0)):
+    for name, deg in (("default", 0), ("d16", 16), ("plain", -1)):
         ctx = moto.spin_context(w, kmax=kmax)
         ctx.set_solver(hvp_path=2, precond_degree=deg)
         lam, V, info = ctx.lowest_modes(dev(w.spins), k, tol=1e-9, max_iter=20000)
         assert info["converged"], (name, info)
         _check_modes(w, lam, V, lam_ref, V_ref, k)
         res[name] = info
-    assert res["default"]["hvp_count"] == kmax * (res["default"]["iters"] + 1)      # plain: one HVP per column and iteration
-    assert res["d32"]["hvp_count"] > kmax * (res["d32"]["iters"] + 2) and res["d32"]["iters"] < res["default"]["iters"]
+    assert res["plain"]["hvp_count"] == kmax * (res["plain"]["iters"] + 1)      # plain: one HVP per column and iteration
+    assert res["default"]["hvp_count"] > kmax * (res["default"]["iters"] + 2) and res["default"]["iters"] < res["plain"]["iters"]
+
+
+@pytest.mark.parametrize("deg", [16, 32, 64])
+def test_transformed_guard_columns_on_a_dense_spectrum(moto, deg):
+    # random spins, k = 3 with two guard columns: before soft locking and the interval above the whole block (a = theta_kb +
+    # margin) degree 32 bounced between 1e-9 and 1e-2 for thousands of iterations; the oracle recomputes the residuals
+    w = custom(70, 40, 0, 1, 3)
+    model = model_of(w)
+    lam_ref, V_ref = so.lowest_modes(model, w.spins, 3, extra=1)
+    ctx = moto.spin_context(w, kmax=5)
+    ctx.set_solver(guard=2, hvp_path=2, precond_degree=deg)
+    lam, V, info = ctx.lowest_modes(dev(w.spins), 3, tol=1e-9, max_iter=400)
+    assert info["converged"] and info["iters"] <= 60, info
+    _check_modes(w, lam, V, lam_ref, V_ref, 3)
+    Vh, lh = V.cpu().numpy(), lam.cpu().numpy()
+    R = so.hvp(model, w.spins, Vh) - lh[:, None, None] * Vh
+    assert np.max(np.linalg.norm(R.reshape(3, -1), axis=1)) <= 1e-9 * (1 + 1e-3)
+
+
+def test_warm_started_resolve_kb6_transformed(moto):
+    # the re-solve of an MMF loop at block size 6 (warm start, transported block) runs transformed too: same eigenpairs as the
+    # plain solver from the same start, in fewer iterations
+    w = wl.config1(L=40)
+    model = model_of(w)
+    x = dev(w.spins)
+    out = {}
+    for name, deg in (("default", 0), ("plain", -1)):
+        ctx = moto.spin_context(w, kmax=6)
+        ctx.set_solver(hvp_path=2, precond_degree=deg)
+        lam, V, info = ctx.lowest_modes(x, 6, tol=1e-9, max_iter=20000)
+        assert info["converged"], (name, info)
+        x2, _ = ctx.mmf_step(x, V[:1].contiguous(), 0.05)
+        ctx.transport(x2, V)
+        lam2, V2, info2 = ctx.lowest_modes(x2, 6, tol=1e-9, max_iter=20000, V0=V)
+        assert info2["converged"], (name, info2)
+        out[name] = (x2.cpu().numpy(), lam2.cpu().numpy(), V2.cpu().numpy(), info2)
+    import dataclasses
+    lam_ref, V_ref = so.lowest_modes(model, out["default"][0], 6, extra=1)
+    _check_modes(dataclasses.replace(w, spins=out["default"][0]), dev(out["default"][1]), dev(out["default"][2]), lam_ref, V_ref, 6)
+    assert out["default"][3]["iters"] < out["plain"][3]["iters"]
 
 
 def test_building_block_argument_errors_and_fallbacks(moto):
