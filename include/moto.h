@@ -136,7 +136,10 @@ moto_status moto_energy_grad(moto_ctx* ctx, const double* d_spins, double* d_E, 
 
 /* Block Hessian-vector product (north_star): for each column a,
  * kind 0: HV_a = P (L Pv_a) - (m.g) Pv_a   (input projected, output tangent, reading A5)
- * kind 1: HV_a = M H M v_a, M = mask of free atoms.   d_V, d_HV: [k][N][3]; must not alias. */
+ * kind 1: HV_a = M H M v_a, M = mask of free atoms.   d_V, d_HV: [k][N][3]; must not alias.
+ * The call is stateless: on Cartesian atoms moto_hvp and moto_energy_grad rebuild the cell list and the neighbour table from
+ * d_spins (= positions) on every call (three small launches, most of the ~55 us of a call at 1607 atoms); the solvers
+ * (moto_lowest_modes, moto_mmf_run*, moto_relax*) build them once per state and apply the operator on the stored table. */
 moto_status moto_hvp(moto_ctx* ctx, const double* d_spins, const double* d_V, int k, double* d_HV);
 
 /* Smallest-k eigenpairs of the (masked) tangent Hessian by device-resident block LOBPCG
