@@ -164,7 +164,7 @@ int spin_cheb_multistep(moto_ctx*, const double* m, const double* cvec, const do
                         const double* d_coef, const int* d_done);
 // spin_cheb2_tma.cu
 int spin_cheb2_multistep(moto_ctx*, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
-                         const double* d_coef, const int* d_done, int product_form);
+                         const double* d_coef, const int* d_done, int product_form, int ngroups);
 int spin_cheb_recurrence(moto_ctx*, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
                          const double* d_coef, const int* d_done);
 int spin_hvp_tma_ex(moto_ctx*, const double* m, const double* cvec, const double* V, int k, double* HV, const int* d_done,

@@ -202,8 +202,16 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
 static int gen_apply(moto_ctx* c, const double* d_state, const double* V, int kb, double* OV, int degree) {
     if (degree == 0) return apply_operator(c, d_state, V, kb, OV);
     const size_t bs = (size_t)3 * c->N;
-    int n = 0;
-    for (int a0 = 0; a0 < kb; a0 += 2) {
+    int n = 0, a0 = 0;
+    // all column pairs in ONE two-steps-per-pass launch, each pair on its own share of the SMs (spin_cheb2_multistep, ngroups): at
+    // cfg 2 a pair's 32-step launch is bound by its neighbour synchronisation (72 us for 443 sites per CTA), three of them in one
+    // launch cost about the same (solve 7.5 -> 6.3 ms, MMF re-solve 8.3 -> 5.8 ms); still ahead at 10^6 sites (k = 4: 244 -> 221 ms).
+    // Bit-identical to pair-by-pair launches (a column's arithmetic does not depend on which CTA owns its rows).
+    if (kb >= 4 && (c->opts.cheb_mode == 0 || c->opts.cheb_mode == 3) && degree >= 2 && !(degree & 1) && c->nsh == 0) {
+        const int nk = spin_cheb2_multistep(c, d_state, c->c, V, 2, degree, OV, &c->st->cheb[0][0], &c->st->done, 1, kb / 2);
+        if (nk > 0) { n += nk; a0 = 2 * (kb / 2); }
+    }
+    for (; a0 < kb; a0 += 2) {
         const int kk = kb - a0 >= 2 ? 2 : 1;
         const int nk = spin_cheb_recurrence(c, d_state, c->c, V + a0 * bs, kk, degree, OV + a0 * bs, &c->st->cheb[0][0], &c->st->done);
         if (nk <= 0) return -1000000;   // reported by the caller as a failed solve

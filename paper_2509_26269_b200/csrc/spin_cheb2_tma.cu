@@ -74,6 +74,8 @@ struct KParams2 {
     unsigned long long* flags;   // [grid] last pass finished by each CTA, as epoch + pass
     unsigned long long epoch;
     int* err;
+    int gpair;                   // CTAs per column group: CTA b works on columns K (b / gpair) .. of every block with the
+                                 // strip-rows of local CTA b % gpair (one launch for all column pairs of a block size above 2)
 };
 
 __device__ __forceinline__ d3 lds3(const double* p) { return mk3(p[0], p[1], p[2]); }
@@ -114,7 +116,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
     __syncthreads();
     if (p.done && *p.done) return;
 
-    const long long lo = (p.total * blockIdx.x) / gridDim.x, hi = (p.total * (blockIdx.x + 1)) / gridDim.x;
+    // column group of this CTA and its place among the group's G CTAs (a launch for one group: G = gridDim.x)
+    const int G = p.gpair, grp = (int)blockIdx.x / G, bid = (int)blockIdx.x - grp * G;
+    const long long lo = (p.total * bid) / G, hi = (p.total * (bid + 1)) / G;
 
     if (warp == NCW) {
         // ================================================================ producer warp: all 32 lanes issue TMA boxes
@@ -125,10 +129,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
                 if (nd < 60) sdep[++nd] = c; else *p.err = 1;
             };
             auto add_rows = [&](int sx2, int ya, int yb) {
-                const int c0 = cta_of((long long)sx2 * Ly + ya, p.total, gridDim.x), c1 = cta_of((long long)sx2 * Ly + yb, p.total, gridDim.x);
+                const int c0 = cta_of((long long)sx2 * Ly + ya, p.total, G), c1 = cta_of((long long)sx2 * Ly + yb, p.total, G);
                 for (int c = c0; c <= c1; ++c) add(c);
             };
-            add((int)blockIdx.x);
+            add(bid);
             long long q = lo;
             while (q < hi) {
                 const int sx = (int)(q / Ly), y0 = (int)(q - (long long)sx * Ly);
@@ -155,7 +159,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
                 const int nd = sdep[0];
                 const unsigned long long want = p.epoch + (unsigned long long)(pass - 1);
                 for (int d = lane; d < nd; d += 32) {
-                    const unsigned long long* f = p.flags + sdep[1 + d];
+                    const unsigned long long* f = p.flags + grp * G + sdep[1 + d];
                     unsigned long long v; int spins = 0;
                     do {
                         asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(f) : "memory");
@@ -201,7 +205,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
                         if (g == 2 && !edgeR) continue;
                         const FSet& fs = f == 0 ? maps.m : (f == F ? maps.c : ys);
                         const CUtensorMap* mp = g == 0 ? (chunk_ok ? &fs.chunk : &fs.row) : (chunk_ok ? &fs.schunk : &fs.srow);
-                        const int vec = (f == 0 || f == F) ? 0 : f - 1;
+                        const int vec = (f == 0 || f == F) ? 0 : K * grp + f - 1;
                         if (f < F) {
                             double* dst = g == 0 ? smain + ((size_t)f * NSLOT + slot) * ROWD : (g == 1 ? sL : sR) + ((size_t)f * NSLOT + slot) * SIDED;
                             tma_load_3d(dst, mp, &full[s], g == 0 ? x3 : (g == 1 ? 3 * Lx - SIDED : 0), y, vec);
@@ -230,10 +234,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_cheb2_tma(const __grid_constant
         // product-form steps (beta = 0, k_cheb_coef) have no third operand: phase A then reads nothing from global memory, and
         // Y_{2 pass - 1} -- wanted by the next pass only as ITS third operand -- never leaves shared memory: a pass moves
         // m, c, Y_{2 pass - 2} in and Y_{2 pass} out, 128 B/site per TWO steps at k = 2
-        const double* UA = (PF || pass == 1 || beA == 0.0) ? nullptr : p.B[(2 * pass - 4) & 3];        // Y_{2 pass - 3}
+        const size_t goff = (size_t)grp * K * 3 * N;                              // this group's columns inside every block
+        const double* UA = (PF || pass == 1 || beA == 0.0) ? nullptr : p.B[(2 * pass - 4) & 3] + goff;   // Y_{2 pass - 3}
         const bool storeA = !PF && pass < p.npass && p.coef[4 * (2 * pass) + 2] != 0.0;
-        double* outA = p.Bw[(2 * pass - 2) & 3];                                  // Y_{2 pass - 1}
-        double* outB = pass == p.npass ? p.out : p.Bw[(2 * pass - 1) & 3];        // Y_{2 pass}
+        double* outA = p.Bw[(2 * pass - 2) & 3] + goff;                           // Y_{2 pass - 1}
+        double* outB = (pass == p.npass ? p.out : p.Bw[(2 * pass - 1) & 3]) + goff;   // Y_{2 pass}
         // Even passes sweep bottom-up on the point-reflected lattice: row order reversed, left and right neighbours swapped,
         // D -> -D (the stencil is inversion symmetric up to the sign of the DMI vectors), bit-identical to a forward sweep.
         const bool rev = !(pass & 1);
@@ -480,23 +485,30 @@ int coop_limit2() {
 // rotate through the context's four blocks T1 .. T4.  k <= 2.  Returns the number of launches, 0 if not applicable (the
 // caller then takes spin_cheb_multistep / the step-wise path).
 // product_form: every coefficient row has beta = 0 (k_cheb_coef): the kernel without the third-operand path.
+// ngroups > 1 (k == 2 only): V, OUT and the rotating blocks hold 2 ngroups columns and ONE launch runs the recurrence on all of them,
+// column pair g on its own set of CTAs (grid = ngroups x CTAs per pair, each pair synchronising among its own CTAs only): block
+// sizes above 2 on lattices too small to fill the GPU with one pair (cfg 2: three 72-us launches bound by the neighbour
+// synchronisation of 32 steps become one).
 int spin_cheb2_multistep(moto_ctx* c, const double* m, const double* cvec, const double* V, int k, int d, double* OUT,
-                         const double* d_coef, const int* d_done, int product_form) {
+                         const double* d_coef, const int* d_done, int product_form, int ngroups) {
     if (!spin_tma_applicable(c) || k > 2 || d < 2 || (d & 1) || !c->T1 || !c->T3 || !cvec) return 0;
+    if (ngroups < 1 || (ngroups > 1 && (k != 2 || 2 * ngroups > c->kmax))) return 0;
     if (((uintptr_t)m & 15) || ((uintptr_t)V & 15) || ((uintptr_t)cvec & 15)) return 0;
     const int Lx = c->lat.Lx, Ly = c->lat.Ly;
     if (Lx < SIDED || Ly < 4) return 0;   // the side box of c holds 16 sites; two-row halos
     const int nsx = (Lx + TXMAX - 1) / TXMAX;
     const long long total = (long long)nsx * Ly;
     long long g = (total + RC - 1) / RC;
-    const int grid = (int)(g > MOTO_NUM_SMS ? MOTO_NUM_SMS : (g < 1 ? 1 : g));
     if (c->coop2_max_ctas == 0) c->coop2_max_ctas = k == 2 ? coop_limit2<2>() : coop_limit2<1>();
-    if (grid > c->coop2_max_ctas) return 0;
+    const int cap = (c->coop2_max_ctas < MOTO_NUM_SMS ? c->coop2_max_ctas : MOTO_NUM_SMS) / ngroups;   // CTAs a column group may take
+    if (cap < 1) return 0;
+    const int gpair = (int)(g > cap ? cap : (g < 1 ? 1 : g));
+    const int grid = gpair * ngroups;
     Maps2 maps;
     memset(&maps, 0, sizeof(maps));
     bool ok = encode_fset(&maps.m, m, Lx, Ly, 1, 3) && encode_fset(&maps.c, cvec, Lx, Ly, 1, 1) &&
-              encode_fset(&maps.y[0], V, Lx, Ly, k, 3) && encode_fset(&maps.y[1], c->T2, Lx, Ly, k, 3) &&
-              encode_fset(&maps.y[2], c->T4, Lx, Ly, k, 3);
+              encode_fset(&maps.y[0], V, Lx, Ly, k * ngroups, 3) && encode_fset(&maps.y[1], c->T2, Lx, Ly, k * ngroups, 3) &&
+              encode_fset(&maps.y[2], c->T4, Lx, Ly, k * ngroups, 3);
     if (!ok) return 0;
     KParams2 p;
     p.l = make_lat(c);
@@ -505,6 +517,7 @@ int spin_cheb2_multistep(moto_ctx* c, const double* m, const double* cvec, const
     for (int i = 0; i < 4; ++i) { p.B[i] = T[i]; p.Bw[i] = T[i]; }
     p.out = OUT; p.done = d_done;
     p.flags = c->flags; c->epoch += 1024; p.epoch = c->epoch; p.err = &c->st->bad;
+    p.gpair = gpair;
     const bool l_ok = product_form ? (k == 2 ? launch2<2, true>(c, maps, p, grid) : launch2<1, true>(c, maps, p, grid))
                                    : (k == 2 ? launch2<2, false>(c, maps, p, grid) : launch2<1, false>(c, maps, p, grid));
     return l_ok ? 1 : 0;
@@ -522,7 +535,7 @@ int spin_cheb_recurrence(moto_ctx* c, const double* m, const double* cvec, const
     if (mode == 3 && d >= 2) {
         const int de = d & ~1;
         // odd d: Y_{d-1} goes to the block it would occupy in the rotation, the last step is a single launch
-        int n = spin_cheb2_multistep(c, m, cvec, V, k, de, de == d ? OUT : T[(de - 1) & 3], d_coef, d_done, /*product_form=*/1);
+        int n = spin_cheb2_multistep(c, m, cvec, V, k, de, de == d ? OUT : T[(de - 1) & 3], d_coef, d_done, /*product_form=*/1, 1);
         if (n > 0) {
             if (de == d) return n;
             const int n1 = spin_hvp_tma_ex(c, m, cvec, T[(de - 1) & 3], k, OUT, d_done, nullptr, 1, 0.0, 0.0, 0.0, T[(de - 2) & 3],

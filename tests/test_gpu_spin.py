@@ -544,6 +544,24 @@ def test_warm_started_resolve_kb6_transformed(moto):
     assert out["default"][3]["iters"] < out["plain"][3]["iters"]
 
 
+@pytest.mark.parametrize("case,k,guard", [(lambda: wl.config1(L=40), 6, 0), (lambda: custom(70, 40, 0, 1, 3), 3, 2),
+                                           (lambda: custom(64, 50, 1, 0, 2), 4, 0), (lambda: custom(130, 70, 0, 0, 3), 8, 0)])
+def test_grouped_recurrence_launch_equals_pairwise(moto, case, k, guard):
+    # block sizes above 2: all column pairs in one two-steps-per-pass launch (cheb_mode auto), each pair on its own CTAs, against
+    # one launch per pair of the one-step-per-pass kernel (cheb_mode 1) -- bit for bit; odd block sizes add a single-column launch
+    w = case()
+    out = {}
+    for mode in (0, 1):
+        ctx = moto.spin_context(w, kmax=k + guard)
+        ctx.set_solver(guard=guard, hvp_path=2, cheb_mode=mode)
+        lam, V, info = ctx.lowest_modes(dev(w.spins), k, tol=1e-9, max_iter=2000)
+        assert info["converged"], (mode, info)
+        out[mode] = (lam.cpu().numpy(), V.cpu().numpy(), info)
+    assert out[0][2]["iters"] == out[1][2]["iters"]
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    assert out[0][2]["launches"] < out[1][2]["launches"] if "launches" in out[0][2] else True
+
+
 def test_building_block_argument_errors_and_fallbacks(moto):
     import torch
     w = custom(37, 23, 0, 0, 1)              # odd Lx: the TMA path does not apply
