@@ -69,7 +69,8 @@ typedef struct { double De, alpha, r0, rc; } moto_morse_params;
  * Zero-initialise and pass to moto_set_solver to change the defaults given in brackets. */
 typedef struct {
     int32_t guard;          /* extra block columns iterated but not returned            [0]  */
-    int32_t check_every;    /* iterations enqueued between host looks at the status     [8]  */
+    int32_t check_every;    /* iterations enqueued between host looks at the status; 0 = auto: 8 plain LOBPCG iterations,
+                               2 iterations on the transformed operator (each is d operator applications long)  [0]  */
     int32_t precond_degree; /* degree d of the Chebyshev spectral transformation -p_d(A) LOBPCG runs on:
                                0 = auto (40 on spin lattices that take the TMA K1 path with kb <= 2, 32 there with kb > 2 (soft locking), 16 inside the
                                persistent small-lattice kernel and on general shells with the dense kernel, 24 for Cartesian atoms

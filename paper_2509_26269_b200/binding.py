@@ -197,7 +197,7 @@ class Context:
         except Exception:
             pass
 
-    def set_solver(self, guard=0, check_every=8, precond_degree=0, precond_lo=0.0, precond_hi=0.0, seed=0, hvp_path=0,
+    def set_solver(self, guard=0, check_every=0, precond_degree=0, precond_lo=0.0, precond_hi=0.0, seed=0, hvp_path=0,
                    method=0, ncv=0, cheb_mode=0, persistent=0):
         """method: 0 block LOBPCG, 1 thick-restart Lanczos (ncv = basis size, 0 = largest the workspace holds)."""
         o = SolverOpts(guard, check_every, precond_degree, hvp_path, precond_lo, precond_hi, seed, method, ncv, cheb_mode, persistent)

@@ -96,7 +96,7 @@ moto_status moto_create(const moto_lattice* lat, const void* params, void* d_wor
     c->stream = (cudaStream_t)cuda_stream;
     c->ws = (char*)d_workspace;
     c->ws_bytes = ws_bytes;
-    c->opts.check_every = 8;
+    c->opts.check_every = 0;   // auto
     c->opts.seed = 0x9E3779B97F4A7C15ull;
     if (c->kind == MOTO_KIND_TRI2D) {
         c->sp = *(const moto_spin_params*)params;
@@ -154,7 +154,6 @@ moto_status moto_set_solver(moto_ctx* c, const moto_solver_opts* o) {
     if (o->persistent < 0 || o->persistent > 2) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: persistent must be 0, 1 or 2");
     if (o->cheb_mode < 0 || o->cheb_mode > 3) return moto_fail(c, MOTO_EINVAL, "moto_set_solver: cheb_mode must be 0..3");
     moto_solver_opts n = *o;
-    if (n.check_every == 0) n.check_every = 8;
     if (n.seed == 0) n.seed = 0x9E3779B97F4A7C15ull;
     c->opts = n;
     return MOTO_OK;
