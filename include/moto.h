@@ -88,7 +88,8 @@ typedef struct {
                                on the TMA K1 path: 0 = auto (= 3, the fastest as measured at 10^6 spins), 1 = one step per pass in one
                                persistent cooperative launch, 2 = d dependent launches, 3 = two steps per pass in one cooperative
                                launch with the intermediate step kept in shared memory (spin_cheb2_tma.cu; odd d: + one single
-                               step).  All give bit-identical results.                                                  [0]  */
+                               step; block sizes above 2: all column pairs side by side in that one launch, each pair on its
+                               own share of the SMs).  All give bit-identical results.                                  [0]  */
     int32_t persistent;     /* the whole solve as ONE persistent cooperative kernel (nearest-neighbour spin lattices up to 37 888
                                sites = 148 SMs x 256, k <= 2, no guard columns, method 0): 0 = where it applies, unless an explicit
                                precond_degree > 0 asks for the multi-launch transformed solver; 1 = also with an explicit

@@ -127,7 +127,10 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     // tuned on cfg 3 (two seeds) and its 316^2 instance; shells (degree 16, 12 plain iterations) on the 366-neighbour table at
     // 36^2, 64^2 and 100^2
     const int phase_len = 20, plain_start = warm_start ? 0 : ((shells || atoms) ? 12 : 20);
-    const int acheck_every = 4;
+    // cheap A-residual test inside transformed phases: every 4 iterations; every 2 on a warm start below 2^18 sites, where a re-solve
+    // is a handful of iterations and the test (one HVP + four streaming kernels) is short beside them (256^2, k = 2: MMF re-solve
+    // 3.6 -> 3.2 ms; at 10^6 sites the test costs what it saves: 19.5 vs 19.9 ms)
+    const int acheck_every = (warm_start && c->N <= (1 << 18)) ? 2 : 4;
     // b = max_i(-c_i) + lambda_max(L) >= lambda_max(Hess); atoms: the block Gershgorin bound of the stored pair coefficients
     const double lnorm = atoms ? 0.0 : c->lmax_L;
 
