@@ -146,6 +146,9 @@ moto_status moto_check_overflow(moto_ctx* ctx);   // api.cu (also exported, incl
 // ---- launch wrappers (each returns the number of kernels it enqueued; errors via cudaGetLastError)
 // spin_stencil.cu
 int spin_energy_grad(moto_ctx*, const double* m, double* d_E, double* d_g, double* d_c);
+int spin_energy_grad_tma(moto_ctx*, const double* m, double* d_E, double* d_g, double* d_c);   // 0: not applicable
+int spin_mmf_pass1_tma(moto_ctx*, const double* m, const double* v, double* Fbuf, double* d_alpha);   // 0: not applicable
+void launch_final_sum(moto_ctx* c, const double* partials, int nblk, int stride, int nval, double* out, int take_sqrt);
 int spin_curvature(moto_ctx*, const double* m, double* d_c);
 int spin_hvp(moto_ctx*, const double* m, const double* c_or_null, const double* V, int k, double* HV,
              int project_input, const int* d_done);

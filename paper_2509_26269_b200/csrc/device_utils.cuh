@@ -45,3 +45,24 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double* smem) {
     }
     __syncthreads();
 }
+
+// Final sum without a second launch: every CTA has written partials[blockIdx.x * stride + v] (v < nval) and then calls this with
+// all its threads; the CTA that arrives last adds the partials of all gridDim.x CTAs -- one warp per value, lanes striding over
+// the CTAs, shuffle tree: the order of k_final_sum, so the result does not depend on which CTA that is -- and leaves the arrival
+// counter at 0 for the next launch.  out == nullptr: nothing to do.
+__device__ __forceinline__ void last_cta_sum(const double* partials, int stride, int nval, double* out, int take_sqrt, unsigned* counter) {
+    if (!out) return;
+    __shared__ int s_last;
+    if (threadIdx.x == 0) { __threadfence(); s_last = atomicAdd(counter, 1u) == gridDim.x - 1 ? 1 : 0; }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+    for (int v = warp; v < nval; v += nw) {
+        double s = 0.0;
+        for (unsigned b = lane; b < gridDim.x; b += 32) s += __ldcg(partials + (size_t)b * stride + v);
+        s = warp_sum(s);
+        if (lane == 0) out[v] = take_sqrt ? sqrt(s) : s;
+    }
+    if (threadIdx.x == 0) *counter = 0u;
+}

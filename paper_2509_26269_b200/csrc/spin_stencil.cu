@@ -52,7 +52,8 @@ __device__ __forceinline__ d3 ldnp(const double* __restrict__ m, const double* _
 
 // ---------------------------------------------------------------- energy + gradient (+ c)
 __global__ void __launch_bounds__(256) k_energy_grad(Lat l, const double* __restrict__ m, double* __restrict__ g_out,
-                                                     double* __restrict__ c_out, double* __restrict__ partials) {
+                                                     double* __restrict__ c_out, double* __restrict__ partials,
+                                                     double* __restrict__ e_out, unsigned* counter) {
     __shared__ double red[32];
     const long long N = (long long)l.Lx * l.Ly;
     double e[1] = {0.0};
@@ -70,6 +71,7 @@ __global__ void __launch_bounds__(256) k_energy_grad(Lat l, const double* __rest
     }
     block_sum<1>(e, red);
     if (threadIdx.x == 0) partials[blockIdx.x] = e[0];
+    last_cta_sum(partials, 1, 1, e_out, 0, counter);   // E itself, by the CTA that finishes last
 }
 
 // ---------------------------------------------------------------- fused line-search trial of moto_relax (relax.cu)
@@ -239,7 +241,8 @@ __global__ void k_project(long long N, const double* __restrict__ m, double* __r
 // ---------------------------------------------------------------- K6 reflected-force step
 // pass 1: F = -P g  -> gbuf ; partial dots alpha_a = F . v_a
 __global__ void __launch_bounds__(256) k_mmf_pass1(Lat l, const double* __restrict__ m, const double* __restrict__ v, int kr,
-                                                   double* __restrict__ Fbuf, double* __restrict__ partials) {
+                                                   double* __restrict__ Fbuf, double* __restrict__ partials,
+                                                   double* __restrict__ alpha_out, unsigned* counter) {
     __shared__ double red[32 * MOTO_KMAX];
     const long long N = (long long)l.Lx * l.Ly;
     double acc[MOTO_KMAX];
@@ -260,6 +263,7 @@ __global__ void __launch_bounds__(256) k_mmf_pass1(Lat l, const double* __restri
     block_sum<MOTO_KMAX>(acc, red);
     if (threadIdx.x == 0)
         for (int a = 0; a < MOTO_KMAX; ++a) partials[blockIdx.x * MOTO_KMAX + a] = acc[a];
+    last_cta_sum(partials, MOTO_KMAX, MOTO_KMAX, alpha_out, 0, counter);   // alpha_a = F . v_a
 }
 
 // pass 2: F_mmf = F - 2 sum_a alpha_a v_a ; m' = normalize(m + dt F_mmf) ; partial |F_mmf|^2
@@ -267,7 +271,8 @@ __global__ void __launch_bounds__(256) k_mmf_pass1(Lat l, const double* __restri
 __global__ void __launch_bounds__(256) k_mmf_pass2(long long N, const double* m, const double* __restrict__ v, int kr,
                                                    const double* __restrict__ Fbuf, const double* __restrict__ alpha, double dt,
                                                    double* m_out, double* __restrict__ partials, int retract,
-                                                   const uint8_t* __restrict__ fixed, double* __restrict__ F_out) {
+                                                   const uint8_t* __restrict__ fixed, double* __restrict__ F_out,
+                                                   double* __restrict__ fnorm_out = nullptr, unsigned* counter = nullptr) {
     __shared__ double red[32];
     double al[MOTO_KMAX];
 #pragma unroll
@@ -287,18 +292,21 @@ __global__ void __launch_bounds__(256) k_mmf_pass2(long long N, const double* m,
     }
     block_sum<1>(f2, red);
     if (threadIdx.x == 0) partials[blockIdx.x] = f2[0];
+    last_cta_sum(partials, 1, 1, fnorm_out, 1, counter);   // |F_mmf|
 }
 
 }  // namespace
 
 // ================================================================ host wrappers
+// arrival counters of last_cta_sum: words 500.. of the flag block (512 words, zeroed at create; the K1 launches use < 148)
+static unsigned* sum_counter(moto_ctx* c, int which) { return reinterpret_cast<unsigned*>(c->flags + 500 + which); }
 int spin_energy_grad(moto_ctx* c, const double* m, double* d_E, double* d_g, double* d_c) {
     if (c->nsh > 0) return shell_energy_grad(c, m, d_E, d_g, d_c);
+    const int nt = spin_energy_grad_tma(c, m, d_E, d_g, d_c);   // spin_stencil_tma.cu: where the TMA-staged kernel applies
+    if (nt > 0) return nt;
     Lat l = make_lat(c);
-    k_energy_grad<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, d_g, d_c, c->partials);
-    int n = 1;
-    if (d_E) { k_final_sum<<<FS_GRID(1), 256, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_E, 0); ++n; }
-    return n;
+    k_energy_grad<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, d_g, d_c, c->partials, d_E, sum_counter(c, 1));
+    return 1;
 }
 
 // d_out4 = {E_t, g_t.g_t, g_t.g, g_t.d} (device); d == nullptr: plain evaluation at x (out4[2], [3] = 0)
@@ -372,14 +380,20 @@ int spin_project(moto_ctx* c, const double* m, double* V, int k) {
 int spin_mmf_step(moto_ctx* c, const double* m, const double* v, int kr, double dt, double* m_out, double* d_fnorm) {
     Lat l = make_lat(c);
     double* alpha = c->st->scal;  // [KMAX] would overflow scal[8]? KMAX == 8: exactly fits
-    int n0 = 1;
-    if (c->nsh > 0) n0 = shell_mmf_pass1(c, m, v, kr);
-    else k_mmf_pass1<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, v, kr, c->g, c->partials);
-    k_final_sum<<<FS_GRID(MOTO_KMAX), 256, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, MOTO_KMAX, MOTO_KMAX, alpha, 0);
-    k_mmf_pass2<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, m, v, kr, c->g, alpha, dt, m_out, c->partials, 1, nullptr, c->fmmf_out);
-    int n = 2 + n0;
-    if (d_fnorm) { k_final_sum<<<FS_GRID(1), 256, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, 1, 1, d_fnorm, 1); ++n; }
-    return n;
+    int n = 0;
+    if (c->nsh > 0) {
+        n += shell_mmf_pass1(c, m, v, kr);
+        k_final_sum<<<FS_GRID(MOTO_KMAX), 256, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, MOTO_KMAX, MOTO_KMAX, alpha, 0); ++n;
+    } else if (kr == 1 && spin_mmf_pass1_tma(c, m, v, c->g, alpha) > 0) {
+        ++n;   // large lattices: F = -P g and alpha_1 = F . v_1 from the TMA-staged kernel
+    } else {
+        k_mmf_pass1<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, v, kr, c->g, c->partials, alpha, sum_counter(c, 2)); ++n;
+    }
+    // |F_mmf| of the current state comes out of pass 2 itself (the CTA that finishes last takes the square root of the sum)
+    // (four CTAs per SM: 10^6 spins 51.7 -> 46.6 us per moto_mmf_step; 8 or 16 per SM are slower again)
+    k_mmf_pass2<<<2 * MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, m, v, kr, c->g, alpha, dt, m_out, c->partials, 1, nullptr, c->fmmf_out,
+                                                      d_fnorm, sum_counter(c, 3));
+    return n + 1;
 }
 
 // shared with cart_morse.cu (declared there as extern)

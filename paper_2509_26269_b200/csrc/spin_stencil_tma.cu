@@ -80,6 +80,13 @@ struct KParams {
     unsigned long long* flags;   // [grid] last step finished by each CTA, as epoch + step
     unsigned long long epoch;
     int* err;                // set when a neighbour wait times out
+    // energy / gradient mode of the <1, API> instantiation (moto_energy_grad, the c_i of a solve): only m is staged; out = the
+    // tangent-projected gradient [N][3] or NULL, c_out = c_i = m_i . g_i [N] or NULL, waw = [grid] partial energies or NULL
+    int eg = 0;
+    double* c_out = nullptr;
+    double* e_out = nullptr;          // eg: E itself [1]; the CTA that finishes last sums the partials in `waw` in fixed order
+    unsigned* counter = nullptr;      //     (its arrival counter; left at 0), so the call is one launch
+    const double* vdot = nullptr;     // eg, pass 1 of the reflected-force step: out = F = -P g, and e_out = F . vdot instead of E
 };
 
 __device__ __forceinline__ d3 lds3(const double* p) { return mk3(p[0], p[1], p[2]); }
@@ -114,6 +121,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     }
     if (warp == NCW && lane < 10) asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&maps.m_chunk + lane)) : "memory");
     const int nsteps = (!API && p.nsteps > 1) ? p.nsteps : 1;
+    const bool eg = API && K == 1 && p.eg;
     __syncthreads();
     // everything above overlapped the tail of the previous kernel; nothing it wrote has been touched yet
     asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -198,7 +206,8 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                 const bool chunk_ok = (nvalid == RC) && (!l.py || (y0 >= 0 && y0 + RC <= Ly));
                 if (lane == 0) {
                     mbar_wait(&empty[s], ph ^ 1u);
-                    mbar_expect_tx(&full[s], (unsigned)nvalid * (F * ROWD * 8 + nside * NFS * SIDED * 8 + (API ? 0 : CROWD * 8)));
+                    const int nf = eg ? 1 : F, nfs = eg ? 1 : NFS;   // energy / gradient mode stages m alone
+                    mbar_expect_tx(&full[s], (unsigned)nvalid * (nf * ROWD * 8 + nside * nfs * SIDED * 8 + (API ? 0 : CROWD * 8)));
                 }
                 __syncwarp();
                 const int nops = (chunk_ok ? 1 : nvalid) * KINDS;
@@ -209,10 +218,12 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                     const int slot = s * RC + (chunk_ok ? 0 : (rev ? RC - 1 - i : i));
                     if (kind < F) {
                         const int f = kind;
+                        if (eg && f > 0) continue;
                         const CUtensorMap* mp = f == 0 ? (chunk_ok ? &maps.m_chunk : &maps.m_row) : (chunk_ok ? &vs.chunk : &vs.row);
                         tma_load_3d(smain + ((size_t)f * NSLOT + slot) * ROWD, mp, &full[s], x3, y, f == 0 ? 0 : f - 1);
                     } else if (kind < F + 2 * NFS) {
                         const int q = kind - F, right = q >= NFS, fi = right ? q - NFS : q, f = fi + FS0;
+                        if (eg && f > 0) continue;
                         if (right ? edgeR : edgeL) {
                             const CUtensorMap* ms = f == 0 ? (chunk_ok ? &maps.m_schunk : &maps.m_srow) : (chunk_ok ? &vs.schunk : &vs.srow);
                             tma_load_3d((right ? sR : sL) + ((size_t)fi * NSLOT + slot) * SIDED, ms, &full[s], right ? 0 : 3 * Lx - SIDED, y,
@@ -331,7 +342,31 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                     const d3 LmB = stencil_apply(ls, m2R, m2L, m3C, m1C, m3L, m1R, m2C.z);
                     cA = dot3(m1C, LmA) - dot3(m1C, muB);
                     cB = dot3(m2C, LmB) - dot3(m2C, muB);
+                    if (eg && p.vdot) {   // F = -P(Lm - mu B) and its dot with v (moto_mmf_step, kr = 1)
+                        const double* vp = p.vdot + e0 + (long long)j * eBlk;
+                        const d3 FA = scale3(-1.0, axpy3(-cA, m1C, sub3(LmA, muB)));
+                        waw[0] += dot3(FA, ld3(vp, 0));
+                        st3(oA_p, 0, FA);
+                        if (haveB) {
+                            const d3 FB = scale3(-1.0, axpy3(-cB, m2C, sub3(LmB, muB)));
+                            waw[0] += dot3(FB, ld3(vp + eRow, 0));
+                            st3(oA_p + eRow, 0, FB);
+                        }
+                    } else if (eg) {   // E = sum_i (m.Lm / 2 - mu m.B), g = P(Lm - mu B), c = m.g: the m-stencil is all there is to do
+                        waw[0] += 0.5 * dot3(m1C, LmA) - dot3(m1C, muB);
+                        if (haveB) waw[0] += 0.5 * dot3(m2C, LmB) - dot3(m2C, muB);
+                        if (p.out) {
+                            st3(oA_p, 0, axpy3(-cA, m1C, sub3(LmA, muB)));
+                            if (haveB) st3(oA_p + eRow, 0, axpy3(-cB, m2C, sub3(LmB, muB)));
+                        }
+                        if (p.c_out && !p.vdot) {
+                            const long long iA = (e0 + (long long)j * eBlk) / 3;
+                            p.c_out[iA] = cA;
+                            if (haveB) p.c_out[iA + eRow / 3] = cB;
+                        }
+                    }
                 }
+                if (!eg) {
                 d3 vA[K], hA[K], vB[K], hB[K];
 #pragma unroll
                 for (int a = 0; a < K; ++a) {
@@ -379,6 +414,7 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                     st3(oA_p + (size_t)a * 3 * N, 0, oA);
                     if (haveB) st3(oA_p + (size_t)a * 3 * N + eRow, 0, oB);
                 }
+                }   // !eg
             }
             if (j + 1 < nb) load_u(j + 1);
             __syncwarp();
@@ -412,6 +448,17 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
             double s = 0.0;
             for (int wv = 0; wv < NCW; ++wv) s += sred[wv * 4 + threadIdx.x];
             p.waw[(size_t)blockIdx.x * NK + threadIdx.x] = s;
+        }
+        if (eg && p.e_out) {   // NK = 1.  Which CTA arrives last varies, the order of the sum does not.
+            if (threadIdx.x == 0) { __threadfence(); sdep[0] = atomicAdd(p.counter, 1u) == gridDim.x - 1 ? 1 : 0; }
+            asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");
+            if (sdep[0] && warp == 0) {
+                __threadfence();
+                double s = 0.0;
+                for (unsigned b = lane; b < gridDim.x; b += 32) s += __ldcg(p.waw + b);
+                s = warp_sum(s);
+                if (lane == 0) { *p.e_out = s; *p.counter = 0u; }
+            }
         }
     }
 }
@@ -500,6 +547,42 @@ int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const doub
         ++launches;
     }
     return launches;
+}
+
+// Energy, tangent-projected gradient and c_i = m_i . g_i through the TMA-staged kernel (its <1, API> instantiation with only m in the
+// ring): one pass over m, 24 B/site in and 24 (+ 8) out.  d_E, d_g, d_c may each be NULL.  Returns the number of launches, 0 if the
+// path does not apply (the caller takes k_energy_grad).  Lattices below 2^18 sites stay on k_energy_grad (65 536 sites: 17 vs 21 us).
+static int eg_launch(moto_ctx* c, const double* m, double* d_sum, double* d_out, double* d_c, const double* vdot) {
+    if (!spin_tma_applicable(c) || ((uintptr_t)m & 15)) return 0;
+    if (c->opts.hvp_path != 2 && c->N < (1 << 18)) return 0;
+    const int Lx = c->lat.Lx, Ly = c->lat.Ly;
+    Maps maps;
+    memset(&maps, 0, sizeof(maps));
+    bool ok = encode(&maps.m_chunk, m, Lx, Ly, 1, ROWD, RC) && encode(&maps.m_row, m, Lx, Ly, 1, ROWD, 1) &&
+              encode(&maps.m_schunk, m, Lx, Ly, 1, SIDED, RC) && encode(&maps.m_srow, m, Lx, Ly, 1, SIDED, 1) &&
+              encode_vset(&maps.vset[0], m, Lx, Ly, 1);   // never loaded in this mode; a valid descriptor for the prefetch
+    if (!ok) return 0;
+    KParams p;
+    p.l = make_lat(c);
+    p.nsx = (Lx + TXMAX - 1) / TXMAX;
+    p.total = (long long)p.nsx * Ly;
+    p.cvec = nullptr; p.out = d_out; p.U = nullptr;
+    p.alpha = p.c0 = p.beta = 0.0; p.cheb = 0; p.coef = nullptr;
+    p.waw = d_sum ? c->partials : nullptr; p.done = nullptr;
+    p.nsteps = 1; p.V0 = nullptr; p.T1 = p.T2 = nullptr; p.flags = nullptr; p.epoch = 0; p.err = nullptr;
+    p.eg = 1; p.c_out = d_c; p.vdot = vdot;
+    p.e_out = d_sum; p.counter = reinterpret_cast<unsigned*>(c->flags + 500);   // flags: 512 words, zeroed at create; the K1 launches use < 148
+    const int grid = spin_tma_grid(c);
+    return launch<1, true>(c, maps, p, grid) ? 1 : 0;
+}
+
+int spin_energy_grad_tma(moto_ctx* c, const double* m, double* d_E, double* d_g, double* d_c) { return eg_launch(c, m, d_E, d_g, d_c, nullptr); }
+
+// Pass 1 of the reflected-force step with one mode (moto_mmf_step, kr = 1): Fbuf = F = -P g and *d_alpha = F . v in one launch of
+// the same kernel.  Returns 1, or 0 if the path does not apply (the caller takes k_mmf_pass1).
+int spin_mmf_pass1_tma(moto_ctx* c, const double* m, const double* v, double* Fbuf, double* d_alpha) {
+    if (!v || !Fbuf || !d_alpha) return 0;
+    return eg_launch(c, m, d_alpha, Fbuf, nullptr, v);
 }
 
 template <int K>

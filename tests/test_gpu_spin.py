@@ -104,6 +104,29 @@ def test_hvp_tma_parity(moto, case, k):
     assert rel_l2(HV, HV1) <= 1e-13
 
 
+@pytest.mark.parametrize("case", range(len(TMA_CASES)))
+def test_energy_grad_tma_parity(moto, case):
+    # moto_energy_grad through the TMA-staged kernel (energy / gradient mode: only m in the ring) against the oracle, and
+    # against the generic kernel; E alone and g alone take the same path
+    w = TMA_CASES[case]()
+    model = model_of(w)
+    ctx = moto.spin_context(w)
+    ctx.set_solver(hvp_path=2)
+    n0 = ctx.launch_count
+    E, g = ctx.energy_grad(dev(w.spins))
+    assert ctx.launch_count - n0 == 1                       # one launch: the CTA that finishes last sums the energy partials
+    E_ref = so.energy(model, w.spins)
+    g_ref = so.projected_gradient(model, w.spins)
+    assert abs(E.item() - E_ref) <= 1e-12 * max(1.0, abs(E_ref))
+    assert np.max(np.abs(g.cpu().numpy() - g_ref)) <= 1e-12
+    for _ in range(3):                                      # the arrival counter is left at 0: repeated calls, bit-identical
+        E2, none = ctx.energy_grad(dev(w.spins), want_grad=False)
+        assert none is None and E2.item() == E.item()
+    ctx.set_solver(hvp_path=1)
+    E1, g1 = ctx.energy_grad(dev(w.spins))
+    assert abs(E1.item() - E.item()) <= 1e-13 * max(1.0, abs(E_ref)) and np.max(np.abs((g1 - g).cpu().numpy())) <= 1e-13
+
+
 @pytest.mark.parametrize("case", [0, 1, 2, 3, 5, 8])
 def test_lowest_modes_tma_path(moto, case):
     # solver mode of the TMA kernel (c given, fused V^T HV partials) inside the LOBPCG
@@ -281,6 +304,32 @@ def test_mmf_step_parity(moto):
         s = dev(w.spins)
         ctx.mmf_step(s, dev(V_ref[:1]), 0.05, out=s)
         assert np.max(np.abs(s.cpu().numpy() - so.mmf_step(model, w.spins, V_ref[:1], 0.05))) <= 1e-13
+
+
+@pytest.mark.parametrize("case", range(len(TMA_CASES)))
+def test_mmf_step_tma_parity(moto, case):
+    # moto_mmf_step with one mode: pass 1 (F = -P g, alpha = F . v) through the TMA-staged kernel, |F_mmf| out of pass 2 itself (two
+    # launches in all); a random tangent unit vector stands for v (the step is defined for any v); in place; repeated calls
+    w = TMA_CASES[case]()
+    model = model_of(w)
+    v = wl.random_block(w.N, 2, seed=700 + case)
+    v = v - np.sum(v * w.spins[None], axis=2, keepdims=True) * w.spins[None]
+    v /= np.linalg.norm(v.reshape(2, -1), axis=1)[:, None, None]
+    ctx = moto.spin_context(w)
+    ctx.set_solver(hvp_path=2)
+    for kr in (1, 2):
+        n0 = ctx.launch_count
+        out, fn = ctx.mmf_step(dev(w.spins), dev(v[:kr]), 0.05)
+        assert ctx.launch_count - n0 == 2
+        ref = so.mmf_step(model, w.spins, v[:kr], 0.05)
+        assert np.max(np.abs(out.cpu().numpy() - ref)) <= 1e-13
+        fref = np.linalg.norm(so.mmf_force(model, w.spins, v[:kr]))
+        assert abs(fn.item() - fref) <= 1e-12 * max(1.0, fref)
+        out2, fn2 = ctx.mmf_step(dev(w.spins), dev(v[:kr]), 0.05)          # arrival counters back at 0: bit-identical
+        assert np.array_equal(out.cpu().numpy(), out2.cpu().numpy()) and fn.item() == fn2.item()
+    s = dev(w.spins)
+    ctx.mmf_step(s, dev(v[:1]), 0.05, out=s)
+    assert np.max(np.abs(s.cpu().numpy() - so.mmf_step(model, w.spins, v[:1], 0.05))) <= 1e-13
 
 
 def test_transport(moto):
