@@ -87,6 +87,8 @@ struct KParams {
     double* e_out = nullptr;          // eg: E itself [1]; the CTA that finishes last sums the partials in `waw` in fixed order
     unsigned* counter = nullptr;      //     (its arrival counter; left at 0), so the call is one launch
     const double* vdot = nullptr;     // eg, pass 1 of the reflected-force step: out = F = -P g, and e_out = F . vdot instead of E
+    int gpair = 0;                    // single-step launches on more than K columns: CTAs per column group (CTA b works on columns
+                                      // K (b / gpair) .. with the strip-rows of local CTA b % gpair); 0 = one group, the whole grid
 };
 
 __device__ __forceinline__ d3 lds3(const double* p) { return mk3(p[0], p[1], p[2]); }
@@ -127,7 +129,8 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (p.done && *p.done) return;
 
-    const long long lo = (p.total * blockIdx.x) / gridDim.x, hi = (p.total * (blockIdx.x + 1)) / gridDim.x;
+    const int G = p.gpair > 0 ? p.gpair : (int)gridDim.x, grp = (int)blockIdx.x / G, bid = (int)blockIdx.x - grp * G;
+    const long long lo = (p.total * bid) / G, hi = (p.total * (bid + 1)) / G;
 
     if (warp == NCW) {
         // ================================================================ producer warp: all 32 lanes issue TMA boxes
@@ -220,14 +223,14 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
                         const int f = kind;
                         if (eg && f > 0) continue;
                         const CUtensorMap* mp = f == 0 ? (chunk_ok ? &maps.m_chunk : &maps.m_row) : (chunk_ok ? &vs.chunk : &vs.row);
-                        tma_load_3d(smain + ((size_t)f * NSLOT + slot) * ROWD, mp, &full[s], x3, y, f == 0 ? 0 : f - 1);
+                        tma_load_3d(smain + ((size_t)f * NSLOT + slot) * ROWD, mp, &full[s], x3, y, f == 0 ? 0 : K * grp + f - 1);
                     } else if (kind < F + 2 * NFS) {
                         const int q = kind - F, right = q >= NFS, fi = right ? q - NFS : q, f = fi + FS0;
                         if (eg && f > 0) continue;
                         if (right ? edgeR : edgeL) {
                             const CUtensorMap* ms = f == 0 ? (chunk_ok ? &maps.m_schunk : &maps.m_srow) : (chunk_ok ? &vs.schunk : &vs.srow);
                             tma_load_3d((right ? sR : sL) + ((size_t)fi * NSLOT + slot) * SIDED, ms, &full[s], right ? 0 : 3 * Lx - SIDED, y,
-                                        f == 0 ? 0 : f - 1);
+                                        f == 0 ? 0 : K * grp + f - 1);
                         }
                     } else {
                         tma_load_3d(sc + (size_t)slot * CROWD, chunk_ok ? &maps.c_chunk : &maps.c_row, &full[s], xb - 2, y, 0);
@@ -260,8 +263,9 @@ k_hvp_tma(const __grid_constant__ Maps maps, const KParams p) {
     // per-step operands: coefficients, three-term operand Y_{step-2} (same-site, same-thread data), destination
     const double* cf = use_coef ? p.coef + 4 * (step - 1) : nullptr;
     const double ch_alpha = cf ? cf[0] : p.alpha, ch_c0 = cf ? cf[1] : p.c0, ch_beta = cf ? cf[2] : p.beta;
-    const double* Ustep = p.U;
-    double* outp = p.out;
+    const size_t goff = (size_t)grp * K * 3 * N;          // this column group's slice of the blocks (single-step launches)
+    const double* Ustep = p.U ? p.U + goff : nullptr;
+    double* outp = p.out ? p.out + goff : nullptr;
     if (nsteps > 1) {
         Ustep = step == 1 ? nullptr : (step == 2 ? p.V0 : ((step & 1) ? p.T1 : p.T2));     // Y_{step-2}
         outp = step == nsteps ? p.out : ((step & 1) ? p.T1 : p.T2);                          // Y_step (in place over Y_{step-2})
@@ -520,8 +524,31 @@ int spin_hvp_tma_ex(moto_ctx* c, const double* m, const double* cvec, const doub
     if (waw_partials && k > 2) return 0;
     const int Lx = c->lat.Lx, Ly = c->lat.Ly;
     const size_t bs = (size_t)3 * c->N;
-    int launches = 0;
-    for (int a0 = 0; a0 < k; a0 += 2) {
+    int launches = 0, a_first = 0;
+    if (k >= 4 && !waw_partials) {
+        // all column pairs in ONE launch, pair g on its own share of the SMs (KParams::gpair): below ~10^5 sites a launch is its
+        // ramp and tail, and k / 2 of them in a row cost k / 2 times that (moto_hvp at cfg 2, k = 6: 19.3 us in three launches)
+        const int ng = k / 2, cap = MOTO_NUM_SMS / ng, g1 = spin_tma_grid(c), gp = g1 < cap ? g1 : cap;
+        Maps maps;
+        memset(&maps, 0, sizeof(maps));
+        bool ok = gp >= 1 && encode(&maps.m_chunk, m, Lx, Ly, 1, ROWD, RC) && encode(&maps.m_row, m, Lx, Ly, 1, ROWD, 1) &&
+                  encode(&maps.m_schunk, m, Lx, Ly, 1, SIDED, RC) && encode(&maps.m_srow, m, Lx, Ly, 1, SIDED, 1) &&
+                  encode_vset(&maps.vset[0], V, Lx, Ly, 2 * ng);
+        if (ok && cvec) ok = encode(&maps.c_chunk, cvec, Lx, Ly, 1, CROWD, RC, 1) && encode(&maps.c_row, cvec, Lx, Ly, 1, CROWD, 1, 1);
+        if (ok) {
+            KParams p;
+            p.l = make_lat(c);
+            p.nsx = (Lx + TXMAX - 1) / TXMAX;
+            p.total = (long long)p.nsx * Ly;
+            p.cvec = cvec; p.out = HV; p.U = U;
+            p.alpha = alpha; p.c0 = c0; p.beta = beta; p.cheb = cheb; p.coef = d_coef;
+            p.waw = nullptr; p.done = d_done;
+            p.nsteps = 1; p.V0 = nullptr; p.T1 = p.T2 = nullptr; p.flags = nullptr; p.epoch = 0; p.err = nullptr;
+            p.gpair = gp;
+            if (cvec ? launch<2, false>(c, maps, p, gp * ng) : launch<2, true>(c, maps, p, gp * ng)) { ++launches; a_first = 2 * ng; }
+        }
+    }
+    for (int a0 = a_first; a0 < k; a0 += 2) {
         const int kk = (k - a0) >= 2 ? 2 : 1;
         Maps maps;
         memset(&maps, 0, sizeof(maps));

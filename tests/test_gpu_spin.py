@@ -87,7 +87,7 @@ TMA_CASES = [
 
 
 @pytest.mark.parametrize("case", range(len(TMA_CASES)))
-@pytest.mark.parametrize("k", [1, 2, 3, 6])
+@pytest.mark.parametrize("k", [1, 2, 3, 5, 6])      # k >= 4: all column pairs in one launch (+ a single-column launch for odd k)
 def test_hvp_tma_parity(moto, case, k):
     w = TMA_CASES[case]()
     model = model_of(w)
@@ -436,7 +436,7 @@ def test_hvp_three_term_parity(moto, case, path):
     ctx = moto.spin_context(w, kmax=8)
     ctx.set_solver(hvp_path=path)
     rng = np.random.default_rng(case)
-    for k in (1, 2, 3):
+    for k in (1, 2, 3, 5):                    # 5 on the TMA path: two pairs in one grouped launch + a single-column launch
         V = wl.random_block(w.N, k, seed=300 + case)
         V = V - np.sum(V * w.spins[None], axis=2, keepdims=True) * w.spins[None]     # tangent input
         U = wl.random_block(w.N, k, seed=400 + case)
