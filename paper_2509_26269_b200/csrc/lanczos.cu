@@ -307,7 +307,8 @@ moto_status lanczos_solve(moto_ctx* c, const double* d_state, int k, double tol,
             filtered = true; in_phase = 0; k0 = 0;
         }
         const bool cap = steps >= max_iter;
-        if (since >= check_every || cap) {
+        // host look: every 8 steps on A, every 2 on the transformed operator (a step is then d applications long; as in lobpcg.cu)
+        if (since >= (c->opts.check_every > 0 ? check_every : (filtered ? 2 : 8)) || cap) {
             since = 0;
             MOTO_CUDA_CHECK(c, cudaMemcpyAsync(&c->hstat[slot], &c->st->theta, sizeof(HostStatus), cudaMemcpyDeviceToHost, c->stream));
             MOTO_CUDA_CHECK(c, cudaEventRecord(c->ev[slot], c->stream));

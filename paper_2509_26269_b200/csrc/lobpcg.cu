@@ -138,6 +138,11 @@ static moto_status lobpcg_solve_fast(moto_ctx* c, const double* d_state, int k, 
     else f.n += cart_build_lists(c, d_state);
     MOTO_CUDA_CHECK(c, cudaMemsetAsync(c->st, 0, sizeof(SolverState), c->stream));
     int nmax = 0;
+    // soft locking, as in the generic transformed solver: a column whose A-residual is within tol / 10 (k_rr where the residuals are
+    // A's, k_acheck_final inside transformed phases) gets no new W_j / P_j from k_update_fused.  Without it a column that is done
+    // keeps iterating at the rounding floor of -p_d(A) and its noise decides when the other one converges: 10^6 random spins took 32
+    // or 36 iterations depending on the last bits of c_i (1090 vs 1412 HVPs).
+    if (degree > 0) MOTO_CUDA_CHECK(c, cudaMemsetAsync(&c->st->lock_on, 1, 1, c->stream));
     if (degree > 0) {
         if (atoms) { const int nb = cart_rowbound(c, pmax, &nmax); if (nb > 0) f.n += nb; else degree = 0; }
         else f.n += fast_negc_max(c, pmax, &nmax);

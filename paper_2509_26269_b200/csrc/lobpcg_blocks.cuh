@@ -59,9 +59,11 @@ __device__ __forceinline__ void block_reduce_store(double (&acc)[NV], double* __
 // writes X' = S C, P' = [W,P] C_wp, AX', AP' by the same coefficients and W' = P_m (AX' - X' Theta), and accumulates
 // |r_j|^2 and every Gram entry of the next Rayleigh-Ritz except W'^T A W' into acc.
 // sC: [3 KB][KB] coefficients followed by theta[KB].  e0 = 3 * site, n3 = 3 N.
+// lk[j]: column j is soft-locked -- it gets no new search directions (W'_j = P'_j = AP'_j = 0, in the blocks and in the Gram
+// entries alike) but is updated like the others and keeps its residual norm; the Rayleigh-Ritz step drops the null directions.
 template <int KB, bool PROJECT>
 __device__ __forceinline__ void update_site(const Blk6& b, const double* __restrict__ m, const double* sC, long long e0, long long n3,
-                                            double (&acc)[Tri<KB>::NEU]) {
+                                            double (&acc)[Tri<KB>::NEU], const bool (&lk)[KB]) {
     using T = Tri<KB>;
     double in_s[3][T::NS], in_a[3][T::NS], mm[3];
 #pragma unroll
@@ -87,12 +89,14 @@ __device__ __forceinline__ void update_site(const Blk6& b, const double* __restr
             double x = p, ax = ap;
 #pragma unroll
             for (int i = 0; i < KB; ++i) { x = fma(sC[i * KB + j], in_s[q][i], x); ax = fma(sC[i * KB + j], in_a[q][i], ax); }
-            const double rr = fma(-sC[3 * KB * KB + j], x, ax);
+            const double rt = fma(-sC[3 * KB * KB + j], x, ax);
+            acc[2 * T::NT + j] = fma(rt, rt, acc[2 * T::NT + j]);
+            const double rr = lk[j] ? 0.0 : rt;
+            if (lk[j]) { p = 0.0; ap = 0.0; }
             s[j] = x; s[KB + j] = rr; s[2 * KB + j] = p;
             a[j] = ax; a[KB + j] = 0.0; a[2 * KB + j] = ap;
             r[q][j] = rr;
             dm[j] = fma(mm[q], rr, dm[j]);
-            acc[2 * T::NT + j] = fma(rr, rr, acc[2 * T::NT + j]);
             b.X[j * n3 + e0 + q] = x; b.P[j * n3 + e0 + q] = p;
             b.AX[j * n3 + e0 + q] = ax; b.AP[j * n3 + e0 + q] = ap;
         }
@@ -106,6 +110,15 @@ __device__ __forceinline__ void update_site(const Blk6& b, const double* __restr
     for (int q = 0; q < 3; ++q)
 #pragma unroll
         for (int j = 0; j < KB; ++j) b.W[j * n3 + e0 + q] = fma(-dm[j], mm[q], r[q][j]);
+}
+
+template <int KB, bool PROJECT>
+__device__ __forceinline__ void update_site(const Blk6& b, const double* __restrict__ m, const double* sC, long long e0, long long n3,
+                                            double (&acc)[Tri<KB>::NEU]) {
+    bool lk[KB];
+#pragma unroll
+    for (int j = 0; j < KB; ++j) lk[j] = false;
+    update_site<KB, PROJECT>(b, m, sC, e0, n3, acc, lk);
 }
 
 }  // namespace lob

@@ -81,13 +81,16 @@ __global__ void __launch_bounds__(256) k_update_fused(long long N, Blk6 b, const
     using T = Tri<KB>;
     __shared__ double sC[3 * KB * KB + KB];
     for (int t = threadIdx.x; t < 3 * KB * KB + KB; t += blockDim.x) sC[t] = t < 3 * KB * KB ? st->C[t] : st->theta[t - 3 * KB * KB];
+    bool lk[KB];   // soft locking (transformed solves): see lobpcg_solve_fast
+#pragma unroll
+    for (int j = 0; j < KB; ++j) lk[j] = st->lock_on && st->locked[j];
     __syncthreads();
     double acc[T::NEU];
 #pragma unroll
     for (int i = 0; i < T::NEU; ++i) acc[i] = 0.0;
     const long long n3 = 3 * N;
     for (long long site = blockIdx.x * (long long)blockDim.x + threadIdx.x; site < N; site += (long long)gridDim.x * blockDim.x)
-        update_site<KB, PROJECT>(b, m, sC, 3 * site, n3, acc);
+        update_site<KB, PROJECT>(b, m, sC, 3 * site, n3, acc, lk);
     block_reduce_store<T::NEU>(acc, partials + (size_t)blockIdx.x * T::NEU);
 }
 

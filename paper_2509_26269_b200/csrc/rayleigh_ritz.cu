@@ -243,6 +243,7 @@ __global__ void __launch_bounds__(RR_THREADS_MAX) k_rr(const double* __restrict_
             for (int a = 0; a < kb; ++a) {
                 double r = sqrt(vals[2 * nT + a]);
                 st->resid[a] = r;
+                if (st->lock_on) st->locked[a] = r <= 0.1 * fz.tol;   // soft locking: true A-residuals here (plain phase / phase boundary)
                 if (a < fz.k) { ok = ok && (r <= fz.tol); bad = bad || !(r == r); }
             }
             if (bad) { st->bad = 1; st->done = 1; stop_s = 1; }

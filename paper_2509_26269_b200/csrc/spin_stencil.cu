@@ -302,7 +302,7 @@ __global__ void __launch_bounds__(256) k_mmf_pass2(long long N, const double* m,
 static unsigned* sum_counter(moto_ctx* c, int which) { return reinterpret_cast<unsigned*>(c->flags + 500 + which); }
 int spin_energy_grad(moto_ctx* c, const double* m, double* d_E, double* d_g, double* d_c) {
     if (c->nsh > 0) return shell_energy_grad(c, m, d_E, d_g, d_c);
-    const int nt = spin_energy_grad_tma(c, m, d_E, d_g, d_c);   // spin_stencil_tma.cu: where the TMA-staged kernel applies
+    const int nt = spin_energy_grad_tma(c, m, d_E, d_g, d_c);   // spin_stencil_tma.cu: where the TMA-staged kernel applies   // spin_stencil_tma.cu: where the TMA-staged kernel applies
     if (nt > 0) return nt;
     Lat l = make_lat(c);
     k_energy_grad<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>(l, m, d_g, d_c, c->partials, d_E, sum_counter(c, 1));
