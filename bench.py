@@ -459,6 +459,24 @@ def main():
         return e0.elapsed_time(e1) / args.hvp_reps, (ctx.launch_count - l0) / args.hvp_reps
 
     hvp_ms, hvp_launches = time_loop(lambda i: ctx.hvp(ms_sets[i], V_sets[i], out=HV_sets[i]))
+    # the same call at k = 6 (configs[2]'s block size): the three column pairs go in ONE launch, pair g on its own third of the SMs
+    k6 = 6
+    ctx6 = moto.spin_context(w, kmax=k6, device=f"cuda:{local}")
+    V6 = [torch.randn(k6, N, 3, dtype=torch.float64, device=dev) for _ in range(2)]
+    HV6 = [torch.empty(k6, N, 3, dtype=torch.float64, device=dev) for _ in range(2)]
+    for i in range(4):
+        ctx6.hvp(ms_sets[i % nsets], V6[i % 2], out=HV6[i % 2])
+    torch.cuda.synchronize()
+    l6 = ctx6.launch_count
+    e0.record()
+    for i in range(args.hvp_reps):
+        ctx6.hvp(ms_sets[i % nsets], V6[i % 2], out=HV6[i % 2])
+    e1.record()
+    torch.cuda.synchronize()
+    hvp6_ms, hvp6_launches = e0.elapsed_time(e1) / args.hvp_reps, (ctx6.launch_count - l6) / args.hvp_reps
+    alg_bytes_api6 = 24 * N * (1 + 2 * k6)
+    del ctx6, V6, HV6
+    torch.cuda.empty_cache()
     ctx.hvp_three_term(ms_sets[0], V_sets[0], 0.1, 9.0, -0.9, U=U_sets[0], out=HV_sets[0], refresh_c=True)   # c cached (all sets share m)
     tt_ms, tt_launches = time_loop(lambda i: ctx.hvp_three_term(ms_sets[i], V_sets[i], 0.1, 9.0, -0.9, U=U_sets[i], out=HV_sets[i],
                                                                  refresh_c=False))
@@ -600,6 +618,13 @@ def main():
                          "kernel_hvp": {"call": "moto_hvp, k_hvp_tma<2,1> (the kernel north_star names: input projected, c recomputed)",
                                         "ms": hvp_ms, "algorithmic_bytes": alg_bytes_api, "achieved": achieved_api,
                                         "frac": achieved_api / peak, "frac_of_8TBs_nominal": achieved_api / 8000.0},
+                         "kernel_hvp_k6": {"call": "moto_hvp at k = 6, k_hvp_tma<2,1> with three column pairs in one launch (each pair on a third of "
+                                                   "the SMs; successive calls alternate between two 144 MB input blocks, so nothing of V or HV is "
+                                                   "left in L2; m is read by the three groups side by side)",
+                                           "ms": hvp6_ms, "launches_per_call": hvp6_launches, "algorithmic_bytes": alg_bytes_api6,
+                                           "achieved": alg_bytes_api6 / (hvp6_ms * 1e-3) / 1e9,
+                                           "frac": alg_bytes_api6 / (hvp6_ms * 1e-3) / 1e9 / peak,
+                                           "frac_of_8TBs_nominal": alg_bytes_api6 / (hvp6_ms * 1e-3) / 1e9 / 8000.0},
                          "single_step": {"call": "moto_hvp_three_term (one recurrence step per launch, programmatic dependent launch)",
                                          "ms": tt_ms, "algorithmic_bytes": alg_bytes_api, "achieved": alg_bytes_api / (tt_ms * 1e-3) / 1e9,
                                          "frac": alg_bytes_api / (tt_ms * 1e-3) / 1e9 / peak,
