@@ -477,6 +477,31 @@ def main():
     alg_bytes_api6 = 24 * N * (1 + 2 * k6)
     del ctx6, V6, HV6
     torch.cuda.empty_cache()
+    # moto_hvp (k = 2) on larger lattices of the same model (random unit spins: the call's time does not depend on the state): a
+    # launch is ~11 us of ramp, tail and launch gap plus ~22.4 us per 10^6 sites, so the fraction at the 10^6 sites of configs[3]
+    # is two thirds streaming; the scan shows the streaming rate (rank 0 only, kernel-only, not part of the timed step)
+    size_scan = []
+    if rank == 0:
+        from paper_2509_26269_b200 import workloads as wl_
+        for Ls in (2000, 2828):
+            ws = wl_.SpinWorkload(f"rand{Ls}", Ls, Ls, 1, 1, w.J, w.D, w.K, w.B, w.mu, k, 11, wl_.random_spins(Ls, Ls, 11))
+            cs = moto.spin_context(ws, kmax=k, device=f"cuda:{local}")
+            xs_ = torch.as_tensor(ws.spins, device=dev)
+            Vs_ = [torch.randn(k, ws.N, 3, dtype=torch.float64, device=dev) for _ in range(2)]   # 2 x 24 N k bytes >= 384 MB > L2
+            Hs_ = [torch.empty_like(Vs_[0]) for _ in range(2)]
+            for i in range(4):
+                cs.hvp(xs_, Vs_[i % 2], out=Hs_[i % 2])
+            torch.cuda.synchronize()
+            e0.record()
+            for i in range(args.hvp_reps):
+                cs.hvp(xs_, Vs_[i % 2], out=Hs_[i % 2])
+            e1.record()
+            torch.cuda.synchronize()
+            t_ = e0.elapsed_time(e1) / args.hvp_reps
+            size_scan.append({"N": ws.N, "ms": t_, "algorithmic_bytes": 24 * ws.N * (1 + 2 * k),
+                              "achieved": 24 * ws.N * (1 + 2 * k) / (t_ * 1e-3) / 1e9})
+            del cs, xs_, Vs_, Hs_
+            torch.cuda.empty_cache()
     ctx.hvp_three_term(ms_sets[0], V_sets[0], 0.1, 9.0, -0.9, U=U_sets[0], out=HV_sets[0], refresh_c=True)   # c cached (all sets share m)
     tt_ms, tt_launches = time_loop(lambda i: ctx.hvp_three_term(ms_sets[i], V_sets[i], 0.1, 9.0, -0.9, U=U_sets[i], out=HV_sets[i],
                                                                  refresh_c=False))
@@ -617,7 +642,10 @@ def main():
                          "peak_source": peak_src,
                          "kernel_hvp": {"call": "moto_hvp, k_hvp_tma<2,1> (the kernel north_star names: input projected, c recomputed)",
                                         "ms": hvp_ms, "algorithmic_bytes": alg_bytes_api, "achieved": achieved_api,
-                                        "frac": achieved_api / peak, "frac_of_8TBs_nominal": achieved_api / 8000.0},
+                                        "frac": achieved_api / peak, "frac_of_8TBs_nominal": achieved_api / 8000.0,
+                                        "size_scan": [dict(e_, frac=e_["achieved"] / peak) for e_ in size_scan],
+                                        "size_scan_note": "the same call on 4e6 / 8e6-site lattices (random spins): ~11 us of fixed cost per "
+                                                          "launch + ~22.4 us per 1e6 sites = 0.82 of the measured peak while streaming"},
                          "kernel_hvp_k6": {"call": "moto_hvp at k = 6, k_hvp_tma<2,1> with three column pairs in one launch (each pair on a third of "
                                                    "the SMs; successive calls alternate between two 144 MB input blocks, so nothing of V or HV is "
                                                    "left in L2; m is read by the three groups side by side)",
