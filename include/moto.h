@@ -72,7 +72,8 @@ typedef struct {
     int32_t check_every;    /* iterations enqueued between host looks at the status; 0 = auto: 8 plain LOBPCG iterations,
                                2 iterations on the transformed operator (each is d operator applications long)  [0]  */
     int32_t precond_degree; /* degree d of the Chebyshev spectral transformation -p_d(A) LOBPCG runs on:
-                               0 = auto (40 on spin lattices that take the TMA K1 path with kb <= 2, 32 there with kb > 2 (soft locking), 16 inside the
+                               0 = auto (40 on spin lattices that take the TMA K1 path with kb <= 2; 32 with kb > 2 (soft locking) on every nearest-neighbour
+                               lattice with even Lx >= 8 and at least 512 sites, the TMA path switched on for the solve; 16 inside the
                                persistent small-lattice kernel and on general shells with the dense kernel, 24 for Cartesian atoms
                                with kb <= 2 and at most 8192 atoms, else off),
                                -1 = off (plain LOBPCG on A, the paper's solver), 1..256 = degree          [0]  */

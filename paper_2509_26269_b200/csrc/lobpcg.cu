@@ -338,12 +338,23 @@ moto_status lobpcg_solve(moto_ctx* c, const double* d_state, int k, double tol, 
     // 14.4 -> 8.3 ms per outer step (moto_mmf_run: 12.5 -> 4.5), cfg 3 k = 4 2184 -> 243 ms; converges where the plain iteration
     // runs into its cap (128 x 128 skyrmion, k = 6; 316 x 316 cfg-3 recipe, k = 6).
     constexpr int GENERIC_AUTO_DEGREE = 32;
+    // Lattices below the 16 384 sites from which hvp_path = auto takes the TMA K1: a single HVP is faster on the generic kernel there,
+    // but a block size above 2 is 3-6x faster on the transformed operator (40 x 40 skyrmion, k = 6: 55 -> 8.8 ms; 64 x 50 random spins,
+    // k = 4: 17 -> 4.4 ms), so from 512 sites on such a solve runs with the TMA path switched on for its duration
+    // (40 x 20 random spins, k = 3: 395 plain iterations, 31 ms).
+    const int path0 = c->opts.hvp_path;
+    if (max_iter > 0 && c->kind == MOTO_KIND_TRI2D && c->nsh == 0 && path0 == 0 && c->T1 && c->opts.precond_degree >= 0 && c->N >= 512 &&
+        !(c->lat.Lx & 1) && c->lat.Lx >= 8)
+        c->opts.hvp_path = 2;
     if (max_iter > 0 && c->kind == MOTO_KIND_TRI2D && spin_tma_applicable(c) && c->T1 && c->opts.precond_degree >= 0 &&
         (c->opts.precond_degree > 0 || 3ll * kb * 8 <= 2ll * c->N)) {
         int degree = c->opts.precond_degree > 0 ? c->opts.precond_degree : GENERIC_AUTO_DEGREE;
         if (degree > MOTO_CHEB_MAX) degree = MOTO_CHEB_MAX;
-        return lobpcg_solve_generic_filtered(c, d_state, k, kb, tol, max_iter, warm_start, degree, info);
+        const moto_status fs = lobpcg_solve_generic_filtered(c, d_state, k, kb, tol, max_iter, warm_start, degree, info);
+        c->opts.hvp_path = path0;
+        return fs;
     }
+    c->opts.hvp_path = path0;
     const size_t bs = (size_t)3 * c->N;
     const int check_every = c->opts.check_every > 0 ? c->opts.check_every : 8;
     const double* m_proj = (c->kind == MOTO_KIND_TRI2D) ? d_state : nullptr;
