@@ -24,6 +24,7 @@
 // no rate advantage over DFMA on this part).  Falls back to spin_shells.cu for k > 2, Lx < 32 or tables that do not fit.
 #include <algorithm>
 #include <vector>
+#include <string.h>
 #include "common.cuh"
 #include "device_utils.cuh"
 #include "stencil_math.cuh"
@@ -71,7 +72,10 @@ __global__ void __launch_bounds__(768) k_shell_dense(Lat l, DenseTab tb, int Hx,
     constexpr int NF = KT + (NEEDC ? 1 : 0);     // staged / accumulated fields: the KT directions (+ m)
     constexpr int NV = NF * R * 3;               // sums per lane
     extern __shared__ double smem[];
-    if (done && *done) return;
+    // programmatic dependent launch: the next launch of the recurrence may start on free SMs right away and stage its copy of the
+    // coupling table (constant since moto_set_shells) while this one still runs; it reads nothing this launch writes -- the done flag,
+    // the fields, the coefficients -- before its own griddepcontrol.wait below
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, S = (blockDim.x >> 5) / NF;
     const int grp = warp / NF, fld = warp - grp * NF;
     const int nent = tb.nd + 2 * tb.nseg;                            // the host puts two zero entries after every segment
@@ -82,6 +86,8 @@ __global__ void __launch_bounds__(768) k_shell_dense(Lat l, DenseTab tb, int Hx,
     for (int t = threadIdx.x; t < 4 * nent; t += blockDim.x) sjd[t] = tb.jd[t];
     for (int t = threadIdx.x; t < 4 * tb.nseg; t += blockDim.x) sseg[t] = tb.seg[t];
     if (threadIdx.x <= MOTO_SH_GROUPS) sgrp[threadIdx.x] = tb.grp[threadIdx.x];   // (the table of this launch's S)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (done && *done) return;
 
     const int Lx = l.Lx, Ly = l.Ly;
     const long long N = (long long)Lx * Ly;
@@ -330,7 +336,18 @@ int shell_dense_hvp(moto_ctx* c, const double* m, const double* cvec, const doub
     do {                                                                                                                   \
         static std::atomic<unsigned long long> seen{0};                                                                    \
         if (smem > 48 * 1024 && !tma::ensure_smem_attr(k_shell_dense<P, NC, CH, KT, RR>, 200 * 1024, seen)) return 0;      \
-        k_shell_dense<P, NC, CH, KT, RR><<<grid, 32 * S * nf, smem, c->stream>>>(l, tb, Hx, Hy, m, cvec, V, HV, d_done, alpha, c0, beta, U, d_coef, nullptr, nullptr); \
+        cudaLaunchConfig_t cfg;                                                                                            \
+        memset(&cfg, 0, sizeof(cfg));                                                                                      \
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(32 * S * nf); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;   \
+        cudaLaunchAttribute attr[1];                                                                                       \
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                                                   \
+        attr[0].val.programmaticStreamSerializationAllowed = 1;                                                            \
+        cfg.attrs = attr; cfg.numAttrs = 1;                                                                                \
+        double* const np_ = nullptr;                                                                                       \
+        if (cudaLaunchKernelEx(&cfg, k_shell_dense<P, NC, CH, KT, RR>, l, tb, Hx, Hy, m, cvec, V, HV, d_done, alpha, c0, beta, U, d_coef, np_, np_) != cudaSuccess) { \
+            (void)cudaGetLastError();                                                                                      \
+            k_shell_dense<P, NC, CH, KT, RR><<<grid, 32 * S * nf, smem, c->stream>>>(l, tb, Hx, Hy, m, cvec, V, HV, d_done, alpha, c0, beta, U, d_coef, nullptr, nullptr); \
+        }                                                                                                                  \
     } while (0)
 #define DENSE(P, NC, CH, KT) do { if (R == 3) DENSE_R(P, NC, CH, KT, 3); else DENSE_R(P, NC, CH, KT, 2); } while (0)
     if (cheb) { if (k == 1) DENSE(false, false, true, 1); else DENSE(false, false, true, 2); }
