@@ -10,6 +10,7 @@
 // neighbour table with the pair coefficients (n, phi'', phi'/r, phi', phi - phi(rc)) stored once per
 // configuration, so every HVP of an eigen-solve is a gather over ~57 stored pairs per atom.
 // Deterministic: cells are sorted by atom id, neighbour order is fixed, reductions are fixed-order.
+#include <string.h>
 #include "common.cuh"
 #include "device_utils.cuh"
 
@@ -165,6 +166,10 @@ __global__ void __launch_bounds__(256) k_cart_hvp(int Na, int k, const uint8_t* 
                                                   const double* __restrict__ V, double* __restrict__ HV, const int* __restrict__ done,
                                                   const double* __restrict__ coef) {
     // coef != NULL: a product-form step of the filter recurrence (k_cheb_coef row {alpha, r, ...}): HV = alpha (H V - r V)
+    // programmatic dependent launch: the next step's CTAs become resident while this one runs and wait here, so a step of the
+    // recurrence does not pay the launch latency (the kernel itself is ~4 us at 1607 atoms)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (done && *done) return;
     int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (i >= Na) return;
@@ -317,10 +322,25 @@ int cart_energy_grad(moto_ctx* c, const double* x, double* d_E, double* d_g) {
     return n;
 }
 
-int cart_hvp(moto_ctx* c, const double* V, int k, double* HV, const int* d_done) {
+static void launch_cart_hvp(moto_ctx* c, const double* V, int k, double* HV, const int* d_done, const double* coef) {
     const int Na = c->N;
-    k_cart_hvp<<<(Na * 32 + 255) / 256, 256, 0, c->stream>>>(Na, k, c->lat.d_fixed, c->cl.nb_count, c->cl.nb_idx, c->cl.nb_coef, V, HV, d_done,
-                                                            nullptr);
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((Na * 32 + 255) / 256); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    const uint8_t* fixed = c->lat.d_fixed;
+    const int* nbc = c->cl.nb_count; const int* nbi = c->cl.nb_idx; const double* nbf = c->cl.nb_coef;
+    if (cudaLaunchKernelEx(&cfg, k_cart_hvp, Na, k, fixed, nbc, nbi, nbf, V, HV, d_done, coef) != cudaSuccess) {
+        (void)cudaGetLastError();
+        k_cart_hvp<<<(Na * 32 + 255) / 256, 256, 0, c->stream>>>(Na, k, fixed, nbc, nbi, nbf, V, HV, d_done, coef);
+    }
+}
+
+int cart_hvp(moto_ctx* c, const double* V, int k, double* HV, const int* d_done) {
+    launch_cart_hvp(c, V, k, HV, d_done, nullptr);
     return 1;
 }
 
@@ -328,12 +348,10 @@ int cart_hvp(moto_ctx* c, const double* V, int k, double* HV, const int* d_done)
 // (k_cheb_coef): d launches of k_cart_hvp, Y_s alternating between T1 and T2.  The neighbour table must be current.
 int cart_cheb_recurrence(moto_ctx* c, const double* V, int k, int d, double* OUT, const double* d_coef, const int* d_done) {
     if (!c->T1 || !c->T2) return -1;
-    const int Na = c->N;
     const double* in = V;
     for (int i = 1; i <= d; ++i) {
         double* out = (i == d) ? OUT : ((i & 1) ? c->T1 : c->T2);
-        k_cart_hvp<<<(Na * 32 + 255) / 256, 256, 0, c->stream>>>(Na, k, c->lat.d_fixed, c->cl.nb_count, c->cl.nb_idx, c->cl.nb_coef, in, out, d_done,
-                                                                d_coef + 4 * (i - 1));
+        launch_cart_hvp(c, in, k, out, d_done, d_coef + 4 * (i - 1));
         in = out;
     }
     return d;
