@@ -81,6 +81,7 @@ constexpr int GS_LMAX = 10;       // staged values per thread per chunk: 2 n Q /
 
 __global__ void __launch_bounds__(GS_THREADS) k_gram_sym(GramPtrs P, int n, int nslice, long long n3,
                                                          double* __restrict__ partials, const int* __restrict__ done) {
+    MOTO_PDL_PROLOGUE();
     if (done && *done) return;
     extern __shared__ double sm[];
     const int nb = n / 3, ntile = nb * (nb + 1) / 2, NR = 2 * n + 1, Q = nslice * GS_QPER;
@@ -162,6 +163,7 @@ __global__ void __launch_bounds__(GS_THREADS) k_gram_sym(GramPtrs P, int n, int 
 // out[e] = sum_b partials[b][e]: one warp per entry, lanes stride over the CTAs, fixed shuffle tree
 __global__ void __launch_bounds__(256) k_reduce_partials(const double* __restrict__ partials, int nblk, int ne, double* __restrict__ out,
                                                          const int* __restrict__ done) {
+    MOTO_PDL_PROLOGUE();
     if (done && *done) return;
     const int e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (e >= ne) return;
@@ -178,6 +180,7 @@ template <int KB>
 __global__ void __launch_bounds__(256) k_update(long long n3, double* __restrict__ X, double* __restrict__ W,
                                                 double* __restrict__ P, double* __restrict__ AX, double* __restrict__ AW,
                                                 double* __restrict__ AP, const SolverState* __restrict__ st) {
+    MOTO_PDL_PROLOGUE();
     if (st->done) return;
     __shared__ double sC[3 * KB * KB];
     for (int t = threadIdx.x; t < 3 * KB * KB; t += blockDim.x) sC[t] = st->C[t];  // [3KB][KB] row-major
@@ -216,6 +219,7 @@ __global__ void __launch_bounds__(256) k_residual(long long N, int kb, const dou
                                                   const uint8_t* __restrict__ fixed, const double* __restrict__ X,
                                                   const double* __restrict__ AX, double* __restrict__ W,
                                                   const SolverState* __restrict__ st, double* __restrict__ partials) {
+    MOTO_PDL_PROLOGUE();
     if (st->done) return;
     __shared__ double red[32 * MOTO_KMAX];
     double acc[MOTO_KMAX];
@@ -246,6 +250,7 @@ __global__ void __launch_bounds__(256) k_residual(long long N, int kb, const dou
 
 // single thread block: finish the residual norms, convergence decision, iteration counter
 __global__ void k_check(const double* __restrict__ partials, int nblk, int kb, int k, double tol, SolverState* st) {
+    MOTO_PDL_PROLOGUE();
     if (st->done) return;
     __shared__ double r[MOTO_KMAX];
     const int j = threadIdx.x >> 5, lane = threadIdx.x & 31;   // one warp per column, lanes over CTAs, fixed order
@@ -399,8 +404,8 @@ int block_gram_lobpcg(moto_ctx* c, int kb) {
     const int blocks = (int)(nchunk < MOTO_RED_BLOCKS ? nchunk : MOTO_RED_BLOCKS);
     size_t smem = (size_t)Q * (2 * n + 1) * sizeof(double), smem_red = (size_t)GS_THREADS * 18 * sizeof(double);
     if (smem < smem_red) smem = smem_red;
-    k_gram_sym<<<blocks, GS_THREADS, smem, c->stream>>>(P, n, nslice, n3, c->partials, &c->st->done);
-    k_reduce_partials<<<(2 * nT * 32 + 255) / 256, 256, 0, c->stream>>>(c->partials, blocks, 2 * nT, gram_reduced(c), &c->st->done);
+    launch_pdl(k_gram_sym, dim3(blocks), dim3(GS_THREADS), smem, c->stream, P, n, nslice, n3, c->partials, &c->st->done);
+    launch_pdl(k_reduce_partials, dim3((2 * nT * 32 + 255) / 256), dim3(256), 0, c->stream, c->partials, blocks, 2 * nT, gram_reduced(c), &c->st->done);
     return 2;
 }
 
@@ -413,16 +418,16 @@ int gram_blocks(const moto_ctx* c) {
 int block_update(moto_ctx* c, int kb) {
     const long long n3 = 3ll * c->N;
     int g = grid_for(n3, 256);
-#define UPD(KB) case KB: k_update<KB><<<g, 256, 0, c->stream>>>(n3, c->X, c->W, c->P, c->AX, c->AW, c->AP, c->st); break;
+#define UPD(KB) case KB: launch_pdl(k_update<KB>, dim3(g), dim3(256), 0, c->stream, n3, c->X, c->W, c->P, c->AX, c->AW, c->AP, c->st); break;
     switch (kb) { UPD(1) UPD(2) UPD(3) UPD(4) UPD(5) UPD(6) UPD(7) UPD(8) }
 #undef UPD
     return 1;
 }
 
 int block_residual(moto_ctx* c, const double* m_or_null, int kb, int k, double tol) {
-    k_residual<<<MOTO_RED_BLOCKS, 256, 0, c->stream>>>((long long)c->N, kb, m_or_null, c->kind == MOTO_KIND_CARTESIAN ? c->lat.d_fixed : nullptr,
+    launch_pdl(k_residual, dim3(MOTO_RED_BLOCKS), dim3(256), 0, c->stream, (long long)c->N, kb, m_or_null, c->kind == MOTO_KIND_CARTESIAN ? c->lat.d_fixed : nullptr,
                                                        c->X, c->AX, c->W, c->st, c->partials);
-    k_check<<<1, 32 * kb, 0, c->stream>>>(c->partials, MOTO_RED_BLOCKS, kb, k, tol, c->st);
+    launch_pdl(k_check, dim3(1), dim3(32 * kb), 0, c->stream, c->partials, MOTO_RED_BLOCKS, kb, k, tol, c->st);
     return 2;
 }
 

@@ -236,3 +236,28 @@ moto_status persistent_solve(moto_ctx* const* ctxs, int P, const double* const* 
 // lobpcg.cu
 moto_status lobpcg_solve(moto_ctx*, const double* d_state, int k, double tol, int max_iter, int warm_start,
                          moto_solve_info* info);
+
+// ---- programmatic dependent launch for the small kernels of a solver iteration: a kernel that starts with MOTO_PDL_PROLOGUE() and is
+// launched through launch_pdl becomes resident while its predecessor in the stream still runs and waits at griddepcontrol.wait until that
+// one has completed and flushed -- stream order as before, minus the launch latency (~2 us per launch of a launch-bound iteration).
+#ifdef __CUDACC__
+#define MOTO_PDL_PROLOGUE()                                                 \
+    do {                                                                    \
+        asm volatile("griddepcontrol.launch_dependents;" ::: "memory");    \
+        asm volatile("griddepcontrol.wait;" ::: "memory");                 \
+    } while (0)
+template <typename... KArgs, typename... Args>
+static inline void launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...) != cudaSuccess) {
+        (void)cudaGetLastError();
+        kern<<<grid, block, smem, st>>>(static_cast<KArgs>(args)...);
+    }
+}
+#endif

@@ -45,6 +45,7 @@ __global__ void __launch_bounds__(256) k_gram_tri(long long n3, Blk6 b, double* 
 template <int KB>
 __global__ void __launch_bounds__(256) k_dot_waw(long long n3, const double* __restrict__ W, const double* __restrict__ AW,
                                                  double* __restrict__ partials, const int* __restrict__ done) {
+    MOTO_PDL_PROLOGUE();
     if (*done) return;
     constexpr int NK = Tri<KB>::NK;
     double acc[NK];
@@ -77,6 +78,7 @@ __global__ void __launch_bounds__(256) k_dot_waw(long long n3, const double* __r
 template <int KB, bool PROJECT>
 __global__ void __launch_bounds__(256) k_update_fused(long long N, Blk6 b, const double* __restrict__ m,
                                                       const SolverState* __restrict__ st, double* __restrict__ partials) {
+    MOTO_PDL_PROLOGUE();
     if (st->done) return;
     using T = Tri<KB>;
     __shared__ double sC[3 * KB * KB + KB];
@@ -194,6 +196,7 @@ __global__ void k_cheb_coef(SolverState* st, int k, int d, double margin, double
 template <int KB>
 __global__ void __launch_bounds__(256) k_acheck_dots(long long n3, const double* __restrict__ X, const double* __restrict__ T,
                                                      double* __restrict__ partials, const int* __restrict__ done) {
+    MOTO_PDL_PROLOGUE();
     if (*done) return;
     double acc[2 * KB];
 #pragma unroll
@@ -210,6 +213,7 @@ __global__ void __launch_bounds__(256) k_acheck_dots(long long n3, const double*
 
 // theta_j = (x_j.t_j) / (x_j.x_j) into st->ack[j], x_j.x_j into st->ack[KMAX + j]
 __global__ void k_acheck_theta(const double* __restrict__ partials, int nblk, int kb, SolverState* st) {
+    MOTO_PDL_PROLOGUE();
     if (st->done) return;
     __shared__ double v[2 * MOTO_KMAX];
     const int e = threadIdx.x >> 5, lane = threadIdx.x & 31;   // one warp per entry
@@ -226,6 +230,7 @@ __global__ void k_acheck_theta(const double* __restrict__ partials, int nblk, in
 template <int KB>
 __global__ void __launch_bounds__(256) k_acheck_resid(long long n3, const double* __restrict__ X, const double* __restrict__ T,
                                                       const SolverState* __restrict__ st, double* __restrict__ partials) {
+    MOTO_PDL_PROLOGUE();
     if (st->done) return;
     double th[KB], acc[KB];
 #pragma unroll
@@ -242,6 +247,7 @@ __global__ void __launch_bounds__(256) k_acheck_resid(long long n3, const double
 
 // store: also leave theta / resid in the state when the test fails (the Lanczos variant sets its next interval from them)
 __global__ void k_acheck_final(const double* __restrict__ partials, int nblk, int kb, int k, double tol, SolverState* st, int store) {
+    MOTO_PDL_PROLOGUE();
     // (soft locking, st->lock_on: every column whose A-residual is within tol is locked, and unlocked should it drift out again)
     if (st->done) return;
     __shared__ double v[MOTO_KMAX];
@@ -292,8 +298,8 @@ int fast_dot_waw(moto_ctx* c, int kb, const double* W, const double* AW, double*
     const long long n3 = 3ll * c->N;
     const int g = fast_grid(n3);
     *nblk_out = g;
-    if (kb == 1) k_dot_waw<1><<<g, 256, 0, c->stream>>>(n3, W, AW, partialsK, &c->st->done);
-    else k_dot_waw<2><<<g, 256, 0, c->stream>>>(n3, W, AW, partialsK, &c->st->done);
+    if (kb == 1) launch_pdl(k_dot_waw<1>, dim3(g), dim3(256), 0, c->stream, n3, W, AW, partialsK, &c->st->done);
+    else launch_pdl(k_dot_waw<2>, dim3(g), dim3(256), 0, c->stream, n3, W, AW, partialsK, &c->st->done);
     return 1;
 }
 
@@ -303,11 +309,11 @@ int fast_update(moto_ctx* c, const double* m_or_null, int kb, int* nblk_out) {
     *nblk_out = g;
     Blk6 b = blocks_of(c);
     if (kb == 1) {
-        if (m_or_null) k_update_fused<1, true><<<g, 256, 0, c->stream>>>(N, b, m_or_null, c->st, c->partials);
-        else k_update_fused<1, false><<<g, 256, 0, c->stream>>>(N, b, m_or_null, c->st, c->partials);
+        if (m_or_null) launch_pdl(k_update_fused<1, true>, dim3(g), dim3(256), 0, c->stream, N, b, m_or_null, c->st, c->partials);
+        else launch_pdl(k_update_fused<1, false>, dim3(g), dim3(256), 0, c->stream, N, b, m_or_null, c->st, c->partials);
     } else {
-        if (m_or_null) k_update_fused<2, true><<<g, 256, 0, c->stream>>>(N, b, m_or_null, c->st, c->partials);
-        else k_update_fused<2, false><<<g, 256, 0, c->stream>>>(N, b, m_or_null, c->st, c->partials);
+        if (m_or_null) launch_pdl(k_update_fused<2, true>, dim3(g), dim3(256), 0, c->stream, N, b, m_or_null, c->st, c->partials);
+        else launch_pdl(k_update_fused<2, false>, dim3(g), dim3(256), 0, c->stream, N, b, m_or_null, c->st, c->partials);
     }
     return 1;
 }
@@ -333,16 +339,16 @@ int fast_cheb_coef_explicit(moto_ctx* c, int d, double a, double b, double aL) {
 int fast_acheck(moto_ctx* c, int kb, int k, double tol, const double* d_T, double* partials, int store) {
     const long long n3 = 3ll * c->N;
     const int g = fast_grid(n3);
-#define ACK_DOTS(KB) k_acheck_dots<KB><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, partials, &c->st->done)
-#define ACK_RESID(KB) k_acheck_resid<KB><<<g, 256, 0, c->stream>>>(n3, c->X, d_T, c->st, partials)
+#define ACK_DOTS(KB) launch_pdl(k_acheck_dots<KB>, dim3(g), dim3(256), 0, c->stream, n3, c->X, d_T, partials, &c->st->done)
+#define ACK_RESID(KB) launch_pdl(k_acheck_resid<KB>, dim3(g), dim3(256), 0, c->stream, n3, c->X, d_T, c->st, partials)
 #define ACK_SWITCH(M) switch (kb) { case 1: M(1); break; case 2: M(2); break; case 3: M(3); break; case 4: M(4); break; \
                                     case 5: M(5); break; case 6: M(6); break; case 7: M(7); break; default: M(8); break; }
     ACK_SWITCH(ACK_DOTS);
-    k_acheck_theta<<<1, 32 * 2 * kb, 0, c->stream>>>(partials, g, kb, c->st);
+    launch_pdl(k_acheck_theta, dim3(1), dim3(32 * 2 * kb), 0, c->stream, partials, g, kb, c->st);
     ACK_SWITCH(ACK_RESID);
 #undef ACK_SWITCH
 #undef ACK_RESID
 #undef ACK_DOTS
-    k_acheck_final<<<1, 32 * kb, 0, c->stream>>>(partials, g, kb, k, tol, c->st, store);
+    launch_pdl(k_acheck_final, dim3(1), dim3(32 * kb), 0, c->stream, partials, g, kb, k, tol, c->st, store);
     return 4;
 }

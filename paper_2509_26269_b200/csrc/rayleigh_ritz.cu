@@ -220,6 +220,7 @@ struct RRFast {            // inputs of the fused kb <= 2 path (lobpcg_fast.cu);
 __global__ void __launch_bounds__(RR_THREADS_MAX) k_rr(const double* __restrict__ partials, int nblk, const double* __restrict__ GA_in,
                                                    const double* __restrict__ GB_in, int n, int nev, double* __restrict__ theta_out,
                                                    double* __restrict__ C_out, int mode, SolverState* st, double tau, double chol_thr, RRFast fz) {
+    MOTO_PDL_PROLOGUE();
     if (st && st->done) return;
     __shared__ double A[NMAX * LD], B[NMAX * LD], U[NMAX * LD], M[NMAX * LD], T[NMAX * LD], Z[NMAX * LD];
     __shared__ double vals[NMAX * 2 * NMAX];
@@ -476,7 +477,7 @@ int rr_solve(moto_ctx* c, const double* d_GA, const double* d_GB, int n, int nev
 int rr_solve_lobpcg(moto_ctx* c, int kb, int /*nblk*/) {
     const double tau = 1e-10;
     RRFast fz = {nullptr, 0, 0, 0, 0, 0, 0.0};
-    k_rr<<<1, rr_threads(3 * kb), 0, c->stream>>>(gram_reduced(c), -1, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, CHOL_THR, fz);
+    launch_pdl(k_rr, dim3(1), dim3(rr_threads(3 * kb)), 0, c->stream, gram_reduced(c), -1, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, CHOL_THR, fz);
     return 1;
 }
 
@@ -484,7 +485,7 @@ int rr_solve_lobpcg(moto_ctx* c, int kb, int /*nblk*/) {
 int rr_solve_fast(moto_ctx* c, int kb, int nblkU, const double* partialsK, int nblkK, int check, int k, double tol, int hvp_inc) {
     const double tau = 1e-10;
     RRFast fz = {partialsK, nblkK, kb, check, hvp_inc, k, tol};
-    k_rr<<<1, RR_THREADS, 0, c->stream>>>(c->partials, nblkU, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, CHOL_THR_FAST, fz);
+    launch_pdl(k_rr, dim3(1), dim3(RR_THREADS), 0, c->stream, c->partials, nblkU, nullptr, nullptr, 3 * kb, kb, c->st->theta, c->st->C, 0, c->st, tau, CHOL_THR_FAST, fz);
     return 1;
 }
 
